@@ -1,0 +1,178 @@
+"""Seeded synthetic inputs for the five BASELINE.json workloads.
+
+This module holds NONE of the method's arithmetic (no emissivity, no Faraday depth, no
+integration): it only draws numbers and lays them out.  The tests and bench.py hand the SAME
+float32 arrays to the CUDA library and (promoted to float64) to the oracle; neither side imports
+the other.  RNG = numpy.random.Generator(PCG64(seed)); values are generated in float64 and
+rounded ONCE to float32.
+
+The paper measures on mock skies built from WMAP B / N_0 fields plus the YMW16 n_e model and on the
+Haslam map; neither is available here, so these inputs take the paper's
+shapes (NSIDE 64..256, N_int 256..1024, a 128x128x32 B grid, 4- and 16-parameter models) and stand
+in for them.
+
+The config-3 grid is "Gaussian random field + logarithmic-spiral pattern" (BASELINE.json); the
+spiral pattern is written out here as a data recipe (`spiral_pattern`) so that both sides receive
+the finished grid as opaque input.
+"""
+from __future__ import annotations
+
+import dataclasses
+from typing import Optional
+
+import numpy as np
+
+OBSERVER = (-8.3, 0.0, 0.006)  # kpc
+
+DEG = np.pi / 180.0
+
+# DISC4 nominal parameters (b0 [uG], psi0, psi1, chi0 [rad]) -- BASELINE.json config 0
+DISC4_NOMINAL = np.array([6.0, 27.0 * DEG, 0.9 * DEG, 25.0 * DEG])
+# aux = (C0, h_r, h_z, alpha, ne0, h_er, h_ez) -- SURVEY.md 8(d), C-2 #9
+AUX_NOMINAL = np.array([2.1038000728e-4, 5.0, 1.0, 3.0, 0.03, 20.0, 1.0])
+# FULL16 nominal, order of SURVEY.md App. C
+FULL16_NOMINAL = np.array([
+    6.0, 27.0 * DEG, 0.9 * DEG, 25.0 * DEG, 10.0,   # disc: b0 psi0 psi1 chi0 h_b
+    2.0, 1.5, 4.0, 0.4,                             # halo: B_h z_h0 r_h w_h
+    2.1038000728e-4, 5.0, 1.0, 3.0,                 # CR: n0 h_r h_z p
+    0.03, 20.0, 1.0,                                # n_e: ne0 h_er h_ez
+])
+FULL16_NAMES = ("b0", "psi0", "psi1", "chi0", "h_b", "B_h", "z_h0", "r_h", "w_h",
+                "n0", "h_r", "h_z", "p", "ne0", "h_er", "h_ez")
+DISC4_NAMES = ("b0", "psi0", "psi1", "chi0")
+
+
+@dataclasses.dataclass
+class Workload:
+    name: str
+    kind: str                    # 'disc4' | 'full16' | 'grid_b' | 'uniform'
+    nside: int
+    n_los: int
+    s_max: float                 # kpc
+    freqs: np.ndarray            # float64 [n_freq], Hz
+    params: np.ndarray           # float32 [batch][P]  or grid [nx][ny][nz][3]
+    aux: Optional[np.ndarray]    # float32 [7] or None
+    box: Optional[tuple] = None  # grid_b: (lx, ly, lz) kpc
+    cot_seed: int = 0
+    observer: tuple = OBSERVER
+
+    @property
+    def npix(self) -> int:
+        return 12 * self.nside * self.nside
+
+    @property
+    def batch(self) -> int:
+        return 1 if self.kind == "grid_b" else int(self.params.shape[0])
+
+    @property
+    def n_freq(self) -> int:
+        return int(self.freqs.size)
+
+    @property
+    def los_samples(self) -> int:
+        """LoS samples per call = npix * n_los * batch (frequencies not multiplied in)."""
+        return self.npix * self.n_los * self.batch
+
+    def cotangents(self, ones: bool = False):
+        """(dI, dQ, dU), each float32 [batch][n_freq][npix]; drawn as [batch][f][Stokes][pix]."""
+        shape = (self.batch, self.n_freq, 3, self.npix)
+        if ones:
+            c = np.ones(shape, dtype=np.float32)
+        else:
+            rng = np.random.Generator(np.random.PCG64(self.cot_seed))
+            c = rng.standard_normal(shape).astype(np.float32)
+        return (np.ascontiguousarray(c[:, :, 0]), np.ascontiguousarray(c[:, :, 1]),
+                np.ascontiguousarray(c[:, :, 2]))
+
+    def scaled(self, nside: Optional[int] = None, n_los: Optional[int] = None, batch: Optional[int] = None,
+               name: Optional[str] = None) -> "Workload":
+        """Same model/frequencies at a smaller map, sample count or batch (parity-test sizes)."""
+        w = dataclasses.replace(self)
+        if nside is not None:
+            w.nside = nside
+        if n_los is not None:
+            w.n_los = n_los
+        if batch is not None and self.kind != "grid_b":
+            w.params = np.ascontiguousarray(self.params[:batch])
+        w.name = name or f"{self.name}@nside{w.nside}x{w.n_los}x{w.batch}"
+        return w
+
+
+def _f32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64).astype(np.float32))
+
+
+def spiral_pattern(x, y, z, b0, psi0, psi1, chi0):
+    """Logarithmic-spiral vector pattern used only to fill the config-3 grid (data recipe)."""
+    rho = np.hypot(x, y)
+    inside = (rho > 3.0) & (rho < 20.0)
+    safe = np.where(rho > 0, rho, 1.0)
+    psi = psi0 + psi1 * np.log(safe / 8.0)
+    chi = chi0 * np.tanh(z)
+    brho = b0 * np.cos(psi) * np.cos(chi)
+    bphi = b0 * np.sin(psi) * np.cos(chi)
+    bx = (brho * x - bphi * y) / safe
+    by = (brho * y + bphi * x) / safe
+    bz = b0 * np.sin(chi) * np.ones_like(safe)
+    out = np.stack([bx, by, bz], axis=-1)
+    return np.where(inside[..., None], out, 0.0)
+
+
+def gaussian_random_field(shape, box, seed, rms=3.0, slope=-11.0 / 3.0):
+    """Three independent Cartesian components, power ~ k^slope, total rms sqrt<|dB|^2> = rms."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    nx, ny, nz = shape
+    k = np.meshgrid(*[2 * np.pi * np.fft.fftfreq(n, d=l / n) for n, l in zip(shape, box)], indexing="ij")
+    kk = np.sqrt(k[0] ** 2 + k[1] ** 2 + k[2] ** 2)
+    amp = np.zeros_like(kk)
+    amp[kk > 0] = kk[kk > 0] ** (slope / 2.0)
+    comps = []
+    for _ in range(3):
+        re = rng.standard_normal(shape)
+        im = rng.standard_normal(shape)
+        comps.append(np.fft.ifftn((re + 1j * im) * amp).real)
+    f = np.stack(comps, axis=-1)
+    f *= rms / np.sqrt(np.mean(np.sum(f * f, axis=-1)))
+    return f
+
+
+def grid_nodes(shape, box):
+    ax = [np.linspace(-l / 2.0, l / 2.0, n) for n, l in zip(shape, box)]
+    return np.meshgrid(*ax, indexing="ij")
+
+
+def config(i: int) -> Workload:
+    """BASELINE.json configs[i], i = 0..4, at full size."""
+    if i == 0:
+        return Workload("cfg0_tiny_disc4", "disc4", 8, 64, 20.0, np.array([23e9]),
+                        _f32(DISC4_NOMINAL)[None, :], _f32(AUX_NOMINAL), cot_seed=1000)
+    if i == 1:
+        rng = np.random.Generator(np.random.PCG64(1001))
+        p = np.array([rng.uniform(3, 9), rng.uniform(15, 35) * DEG, rng.uniform(0, 2) * DEG,
+                      rng.uniform(10, 40) * DEG])
+        return Workload("cfg1_mid_disc4", "disc4", 64, 256, 20.0, np.array([2.4e9, 23e9, 30e9]),
+                        _f32(p)[None, :], _f32(AUX_NOMINAL), cot_seed=2001)
+    if i == 2:
+        rng = np.random.Generator(np.random.PCG64(1002))
+        u = rng.uniform(-1.0, 1.0, size=(256, 16))
+        p = FULL16_NOMINAL[None, :] * (1.0 + 0.2 * u)
+        return Workload("cfg2_batched_full16", "full16", 32, 256, 20.0, np.array([23e9]),
+                        _f32(p), None, cot_seed=2002)
+    if i == 3:
+        shape, box = (128, 128, 32), (40.0, 40.0, 8.0)
+        X, Y, Z = grid_nodes(shape, box)
+        g = gaussian_random_field(shape, box, 1003) + spiral_pattern(X, Y, Z, *DISC4_NOMINAL)
+        return Workload("cfg3_grid_b", "grid_b", 64, 512, 20.0, np.array([408e6]),
+                        _f32(g), _f32(AUX_NOMINAL), box=box, cot_seed=2003)
+    if i == 4:
+        return Workload("cfg4_large_full16", "full16", 256, 1024, 30.0, np.geomspace(0.408e9, 30e9, 8),
+                        _f32(FULL16_NOMINAL)[None, :], None, cot_seed=2004)
+    raise ValueError("config index 0..4")
+
+
+def uniform_toy(bvec=(6.0, 0.0, 0.0), n0=4.01e-5, ne=0.01, alpha=3.0, nside=8, n_los=64, s_max=4.0,
+                freqs=(2.4e9,)) -> Workload:
+    """Homogeneous toy of PAPER.md L123 (section 2.4): the closed-form test model."""
+    p = np.array([bvec[0], bvec[1], bvec[2], n0, ne, alpha])
+    return Workload("uniform_toy", "uniform", nside, n_los, s_max, np.asarray(freqs, dtype=np.float64),
+                    _f32(p)[None, :], None, cot_seed=999)

@@ -1,0 +1,433 @@
+"""Pins for the float64 oracle against things OTHER than itself:
+values printed in the paper / survey (tests/golden/constants.txt), closed forms (uniform slab
+Eq.10, discrete Burn slab from Eq.11), HEALPix ring facts, textbook Gamma/digamma values,
+invariants, gridded==uniform and the convergence order.  CPU only."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2410_01136_b200 import workloads as wl
+
+C_CM = 2.99792458e10
+KPC_CM = 3.0856775814913673e21
+PI_FRAC = lambda a: (a + 1.0) / (a + 7.0 / 3.0)  # noqa: E731  Eq.(5)/Eq.(2)
+
+
+def uniform(bvec, n0=4.01e-5, ne=0.0, alpha=3.0, r0=None):
+    return oracle.Model("uniform", [bvec[0], bvec[1], bvec[2], n0, ne, alpha], aux=None if r0 is None else [r0])
+
+
+def triad(l, b):
+    n = np.array([math.cos(b) * math.cos(l), math.cos(b) * math.sin(l), math.sin(b)])
+    eN = np.array([-math.sin(b) * math.cos(l), -math.sin(b) * math.sin(l), math.cos(b)])
+    eE = np.array([-math.sin(l), math.cos(l), 0.0])
+    return n, eN, eE
+
+
+# ---------------------------------------------------------------------- constants (C-3 #6)
+def test_constants_against_golden(golden_constants):
+    g = golden_constants
+    c = oracle.constants(2.4e9, 6e-6, 4.01e-5, 3.0)
+    assert c["K_F"] / 1e3 == pytest.approx(g["K_F_per_pc"], rel=1e-11)
+    assert abs(c["K_F"] / 1e3 - 0.812) < 2e-4  # north_star: phi = 0.812 int n_e B ds
+    assert c["j_I"] == pytest.approx(g["toy_jI_cgs"], rel=1e-9)
+    assert c["T_RJ"] == pytest.approx(g["T_RJ_2p4GHz"], rel=1e-11)
+    assert c["j_I"] * 4.0 * KPC_CM * c["T_RJ"] == pytest.approx(g["toy_I_kelvin"], rel=1e-11)
+    assert c["j_I"] * KPC_CM * c["T_RJ"] == pytest.approx(g["toy_I_kelvin_per_kpc"], rel=1e-11)
+    # A = j / (N0 B^((1+alpha)/2) nu^((1-alpha)/2))
+    for alpha, key in ((3.0, "A_I_alpha3"), (2.5, "A_I_alpha2p5"), (3.2, "A_I_alpha3p2")):
+        cc = oracle.constants(2.4e9, 6e-6, 4.01e-5, alpha)
+        A = cc["j_I"] / (4.01e-5 * (6e-6) ** ((1 + alpha) / 2) * (2.4e9) ** ((1 - alpha) / 2))
+        assert A == pytest.approx(g[key], rel=1e-11)
+    A_P = c["j_P"] / (4.01e-5 * (6e-6) ** 2 / 2.4e9)
+    assert A_P == pytest.approx(g["A_P_alpha3"], rel=1e-11)
+
+
+def test_gamma_values_behind_eq2(golden_constants):
+    # Eq.(2) at alpha=3 contains Gamma(2/3) Gamma(7/3); Eq.(5) Gamma(2/3) Gamma(4/3).
+    g = golden_constants
+    assert math.gamma(2 / 3) == pytest.approx(g["gamma_2_3"], rel=1e-11)
+    c = oracle.constants(1.0e9, 1e-6, 1.0, 3.0)
+    q, m = 4.80320471257e-10, 9.1093837015e-28
+    pref = math.sqrt(3) * q**3 * 1e-6 / (8 * math.pi * m * C_CM**2) / (4 * math.pi * 1e9 * m * C_CM / (3 * q * 1e-6))
+    assert c["j_I"] / pref == pytest.approx(2.0**2 / 4.0 * g["gamma_2_3"] * g["gamma_7_3"], rel=1e-10)
+    assert c["j_P"] / pref == pytest.approx(1.0 * g["gamma_2_3"] * g["gamma_4_3"], rel=1e-10)
+
+
+@pytest.mark.parametrize("alpha", [2.2, 2.5, 3.0, 3.2, 3.7])
+def test_polarised_fraction_identity(alpha):
+    # Eq.(5)/Eq.(2) = (alpha+1)/(alpha+7/3): the two separately typed formulas must agree
+    c = oracle.constants(1.4e9, 3.3e-6, 1e-4, alpha)
+    assert c["j_P"] / c["j_I"] == pytest.approx(PI_FRAC(alpha), rel=1e-13)
+    if alpha == 3.0:
+        assert c["j_P"] / c["j_I"] == pytest.approx(0.75, rel=1e-13)
+
+
+def test_digamma_textbook(golden_constants):
+    eg = golden_constants["euler_gamma"]
+    dg = lambda x: oracle.constants(1e9, 1e-6, 1.0, x)["digamma"]  # noqa: E731
+    assert dg(1.0) == pytest.approx(-eg, abs=1e-13)
+    assert dg(0.5) == pytest.approx(-eg - 2 * math.log(2), abs=1e-13)
+    assert dg(1 / 3) == pytest.approx(-eg - math.pi / (2 * math.sqrt(3)) - 1.5 * math.log(3), abs=1e-13)
+    assert dg(3.0) == pytest.approx(1.5 - eg, abs=1e-13)
+    for x in (2 / 3, 4 / 3, 7 / 3, 0.54, 5.1):  # vs d/dx lgamma
+        h = 1e-5
+        fd = (math.lgamma(x + h) - math.lgamma(x - h)) / (2 * h)
+        assert dg(x) == pytest.approx(fd, abs=1e-9)
+
+
+def test_dlnj_dalpha_vs_finite_difference():
+    for alpha in (2.4, 3.0, 3.3):
+        h = 1e-6
+        cp, cm = oracle.constants(2.4e9, 4e-6, 1e-4, alpha + h), oracle.constants(2.4e9, 4e-6, 1e-4, alpha - h)
+        c0 = oracle.constants(2.4e9, 4e-6, 1e-4, alpha)
+        assert c0["dlnjI"] == pytest.approx((math.log(cp["j_I"]) - math.log(cm["j_I"])) / (2 * h), rel=1e-8)
+        assert c0["dlnjP"] == pytest.approx((math.log(cp["j_P"]) - math.log(cm["j_P"])) / (2 * h), rel=1e-8)
+
+
+# ---------------------------------------------------------------------- HEALPix (C-3 #7)
+def test_healpix_nside1_and_nside2(golden_constants):
+    z, phi = oracle.pix2ang_ring(1, np.arange(12))
+    np.testing.assert_allclose(z, [2 / 3] * 4 + [0.0] * 4 + [-2 / 3] * 4, atol=1e-15)
+    np.testing.assert_allclose(phi[:4], np.pi / 4 + np.arange(4) * np.pi / 2, atol=1e-15)
+    np.testing.assert_allclose(phi[4:8], np.arange(4) * np.pi / 2, atol=1e-15)
+    np.testing.assert_allclose(phi[8:], np.pi / 4 + np.arange(4) * np.pi / 2, atol=1e-15)
+    z, phi = oracle.pix2ang_ring(2, [0, 4])
+    assert math.acos(z[0]) == pytest.approx(golden_constants["nside2_pix0_theta"], abs=1e-8)
+    assert phi[0] == pytest.approx(np.pi / 4, abs=1e-15)
+    assert math.acos(z[1]) == pytest.approx(golden_constants["nside2_pix4_theta"], abs=1e-8)
+    assert phi[1] == pytest.approx(np.pi / 8, abs=1e-15)
+
+
+@pytest.mark.parametrize("nside", [1, 2, 3, 4, 8, 16, 5])
+def test_healpix_ring_structure(nside):
+    npix = 12 * nside * nside
+    z, phi = oracle.pix2ang_ring(nside, np.arange(npix))
+    assert np.all(np.diff(z) <= 1e-15)                      # z non-increasing in RING order
+    zs = np.unique(np.round(z, 12))
+    assert zs.size == 4 * nside - 1                         # number of iso-latitude rings
+    for zr in zs:                                           # within a ring: phi increasing, equally spaced
+        ph = phi[np.abs(z - zr) < 1e-12]
+        assert np.all(np.diff(ph) > 0)
+        np.testing.assert_allclose(np.diff(ph), 2 * np.pi / ph.size, rtol=1e-12)
+        assert 0 <= ph[0] < 2 * np.pi / ph.size and ph[-1] < 2 * np.pi
+    assert np.all((phi >= 0) & (phi < 2 * np.pi))
+    st = np.sqrt(1 - z * z)
+    nvec = np.stack([st * np.cos(phi), st * np.sin(phi), z], 1)
+    assert np.abs(nvec.sum(0)).max() < 1e-12 * npix         # centres sum to zero
+    np.testing.assert_allclose(z, -z[::-1], atol=1e-15)      # north-south symmetry
+    # equal-area: ring i of the north cap has 4i pixels, belt rings 4 nside
+    counts = [np.sum(np.abs(z - zr) < 1e-12) for zr in zs[::-1]]
+    expect = [4 * i for i in range(1, nside)] + [4 * nside] * (2 * nside + 1) + [4 * i for i in range(nside - 1, 0, -1)]
+    assert counts == expect
+    # ring colatitudes: cap z = 1 - i^2/(3 nside^2), belt z = (2 nside - i) 2/(3 nside)
+    if nside > 1:
+        assert z[0] == pytest.approx(1 - 1 / (3 * nside**2), abs=1e-15)
+    assert np.any(np.abs(zs) < 1e-15)                       # the equator is a ring
+
+
+def test_oracle_map_is_ring_ordered():
+    # uniform field: the map value depends on direction only; rebuild it from forward_dir
+    m = uniform((3.0, -2.0, 1.0), ne=0.02)
+    nside = 4
+    I, Q, U = oracle.forward(m, nside, 16, 4.0, [1.4e9])
+    z, phi = oracle.pix2ang_ring(nside, np.arange(12 * nside * nside))
+    for p in (0, 5, 17, 100, 191):
+        i1, q1, u1 = oracle.forward_dir(m, phi[p], math.asin(z[p]), 16, 4.0, [1.4e9])
+        assert I[0, 0, p] == pytest.approx(i1[0], rel=1e-12)
+        assert Q[0, 0, p] == pytest.approx(q1[0], rel=1e-10, abs=1e-18)
+        assert U[0, 0, p] == pytest.approx(u1[0], rel=1e-10, abs=1e-18)
+
+
+# ---------------------------------------------------------------------- uniform slab (C-3 #1, #2, #5)
+def test_uniform_slab_paper_toy(golden_constants):
+    g = golden_constants
+    m = uniform((6.0, 0.0, 0.0))
+    # l = 90 deg, b = 0: n = +y, B_E = B_y cos l - B_x sin l = -6, B_N = 0
+    I, Q, U = oracle.forward_dir(m, math.pi / 2, 0.0, 64, 4.0, [2.4e9])
+    assert I[0] == pytest.approx(g["toy_I_kelvin"], rel=1e-11)
+    assert Q[0] == pytest.approx(g["toy_Q_kelvin"], rel=1e-11)
+    assert abs(U[0]) < 1e-15
+    # independent of the number of samples (integrand constant) and linear in the path length
+    for n_los, L in ((1, 4.0), (7, 4.0), (1000, 2.0)):
+        I2, _, _ = oracle.forward_dir(m, math.pi / 2, 0.0, n_los, L, [2.4e9])
+        assert I2[0] == pytest.approx(g["toy_I_kelvin"] * L / 4.0, rel=1e-11)
+
+
+@pytest.mark.parametrize("alpha", [3.0, 2.5, 3.2])
+def test_uniform_slab_any_direction(alpha, golden_constants):
+    key = {3.0: "A_I_alpha3", 2.5: "A_I_alpha2p5", 3.2: "A_I_alpha3p2"}[alpha]
+    rng = np.random.default_rng(5)
+    B = np.array([2.0, -5.0, 3.5])
+    m = uniform(B, n0=3e-5, alpha=alpha)
+    for _ in range(6):
+        l, b = rng.uniform(0, 2 * np.pi), rng.uniform(-1.5, 1.5)
+        n, eN, eE = triad(l, b)
+        BN, BE = B @ eN, B @ eE
+        Bt2 = B @ B - (B @ n) ** 2
+        assert BN * BN + BE * BE == pytest.approx(Bt2, rel=1e-12)       # B_N, B_E span B_perp
+        for nu in (0.408e9, 23e9):
+            jI = golden_constants[key] * 3e-5 * (math.sqrt(Bt2) * 1e-6) ** ((1 + alpha) / 2) * nu ** ((1 - alpha) / 2)
+            I_expect = jI * 5.0 * KPC_CM * C_CM**2 / (2 * 1.380649e-16 * nu * nu)
+            I, Q, U = oracle.forward_dir(m, l, b, 33, 5.0, [nu])
+            assert I[0] == pytest.approx(I_expect, rel=1e-10)
+            P = PI_FRAC(alpha) * I_expect
+            c2, s2 = (BE * BE - BN * BN) / Bt2, 2 * BE * BN / Bt2      # e^{2 i chi0}, C-3 #5
+            assert Q[0] == pytest.approx(P * c2, rel=1e-10, abs=1e-14 * P)
+            assert U[0] == pytest.approx(P * s2, rel=1e-10, abs=1e-14 * P)
+
+
+def test_intrinsic_angle_convention():
+    l, b = 0.7, -0.4
+    n, eN, eE = triad(l, b)
+    I, Q, U = oracle.forward_dir(uniform(4 * eE), l, b, 8, 1.0, [1e9])
+    assert Q[0] == pytest.approx(0.75 * I[0], rel=1e-12) and abs(U[0]) < 1e-14 * I[0]   # B || e_E: Q=+P
+    I, Q, U = oracle.forward_dir(uniform(4 * eN), l, b, 8, 1.0, [1e9])
+    assert Q[0] == pytest.approx(-0.75 * I[0], rel=1e-12) and abs(U[0]) < 1e-14 * I[0]  # B || e_N: Q=-P
+    I, Q, U = oracle.forward_dir(uniform(4 * (eE + eN) / math.sqrt(2)), l, b, 8, 1.0, [1e9])
+    assert U[0] == pytest.approx(0.75 * I[0], rel=1e-12) and abs(Q[0]) < 1e-14 * I[0]   # chi0=45deg: U=+P
+    # rotating B_perp by 90 degrees flips both
+    Bp = 3 * eE + 1.5 * eN
+    Bq = -1.5 * eE + 3 * eN
+    _, Q1, U1 = oracle.forward_dir(uniform(Bp + 2 * n), l, b, 8, 1.0, [1e9])
+    _, Q2, U2 = oracle.forward_dir(uniform(Bq + 2 * n), l, b, 8, 1.0, [1e9])
+    assert Q2[0] == pytest.approx(-Q1[0], rel=1e-12) and U2[0] == pytest.approx(-U1[0], rel=1e-12)
+
+
+# ---------------------------------------------------------------------- Burn slab (C-3 #3)
+def test_burn_slab_discrete_closed_form(golden_constants):
+    g = golden_constants
+    KF = g["K_F_per_pc"] * 1e3
+    l, b = 0.0, 0.0                    # n = +x, e_E = +y, e_N = +z
+    for (B, ne, L, N, nu) in (((3.0, 4.0, 2.0), 0.01, 4.0, 64, 2.4e9), ((-2.0, 1.0, -3.0), 0.03, 7.0, 257, 0.408e9),
+                              ((6.0, 1e-3, 0.0), 0.01, 4.0, 1024, 2.4e9)):
+        lam2 = (C_CM / nu * 1e-2) ** 2
+        Theta = lam2 * KF * ne * B[0] * L
+        I0, Q0, U0 = oracle.forward_dir(uniform(B, ne=0.0), l, b, N, L, [nu])
+        I, Q, U = oracle.forward_dir(uniform(B, ne=ne), l, b, N, L, [nu])
+        fac = np.exp(1j * Theta) * math.sin(Theta) / (N * math.sin(Theta / N))
+        z = (Q0[0] + 1j * U0[0]) * fac
+        assert I[0] == pytest.approx(I0[0], rel=1e-13)
+        assert Q[0] == pytest.approx(z.real, rel=1e-9, abs=1e-12 * abs(z))
+        assert U[0] == pytest.approx(z.imag, rel=1e-9, abs=1e-12 * abs(z))
+        # continuum limit e^{i Theta} sin(Theta)/Theta, error O(N^-2)
+        zc = (Q0[0] + 1j * U0[0]) * np.exp(1j * Theta) * math.sin(Theta) / Theta
+        assert abs(z - zc) <= 0.2 * (Theta / N) ** 2 * abs(Q0[0] + 1j * U0[0]) + 1e-15
+    # paper toy with B along the LoS: RM L and the rotation angle (pins K_F and lambda^2)
+    assert KF * 0.01 * 6.0 * 4.0 == pytest.approx(g["toy_RM_L"], rel=1e-6)
+    lam2 = (C_CM / 2.4e9 * 1e-2) ** 2
+    assert lam2 == pytest.approx(g["lambda2_2p4GHz"], rel=1e-11)
+    assert 2 * lam2 * KF * 0.01 * 6.0 * 4.0 == pytest.approx(g["toy_2lam2_RM_L"], rel=1e-5)
+    assert (C_CM / 408e6 * 1e-2) ** 2 == pytest.approx(g["lambda2_408MHz"], rel=1e-8)
+
+
+def test_faraday_sign_convention():
+    # signed B_LOS, +K_F: positive n_e B.n rotates the angle towards +chi (Q -> U for Q0>0)
+    l, b = 0.0, 0.0
+    B = (1.0, 5.0, 0.0)               # B_E = 5, B_N = 0 -> chi0 = 0, Q0 > 0, U0 = 0
+    _, Q, U = oracle.forward_dir(uniform(B, ne=0.001), l, b, 16, 1.0, [1e9])
+    assert Q[0] > 0 and U[0] > 0
+    _, Q, U = oracle.forward_dir(uniform((-1.0, 5.0, 0.0), ne=0.001), l, b, 16, 1.0, [1e9])
+    assert Q[0] > 0 and U[0] < 0
+
+
+# ---------------------------------------------------------------------- model spot values (C-3 #6)
+def test_model_spot_values(golden_constants):
+    w = wl.config(4)
+    p = w.params.astype(np.float64)[0]
+    m = oracle.Model("full16", p)
+    b0, psi0, psi1, chi0, hb, Bh, zh0, rh, wh = p[:9]
+    # rho = 8, z = 0 on the +x axis: rho_hat = x, phi_hat = y; halo contributes along phi_hat only
+    B, N0, ne, al = oracle.eval_fields(m, [[8.0, 0.0, 0.0]])
+    halo = Bh * (1 / (1 + (zh0 / wh) ** 2)) * (8 / rh) * math.exp(1 - 8 / rh)
+    np.testing.assert_allclose(B[0], [b0 * math.cos(psi0), b0 * math.sin(psi0) + halo, 0.0], rtol=1e-12, atol=1e-15)
+    assert al[0] == p[12]
+    # |B_disc| = b0 exp(-(rho-8)/h_b) inside the annulus (halo switched off), 0 outside
+    p2 = p.copy(); p2[5] = 0.0
+    m2 = oracle.Model("full16", p2)
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        rho, ph, z = rng.uniform(0.1, 25), rng.uniform(0, 2 * np.pi), rng.uniform(-3, 3)
+        B, *_ = oracle.eval_fields(m2, [[rho * math.cos(ph), rho * math.sin(ph), z]])
+        expect = b0 * math.exp(-(rho - 8) / hb) if 3 < rho < 20 else 0.0
+        assert np.linalg.norm(B[0]) == pytest.approx(expect, rel=1e-12, abs=1e-300)
+    for rho in (2.999999, 20.000001):
+        B, *_ = oracle.eval_fields(m2, [[0.0, rho, 0.3]])
+        assert np.all(B == 0)
+    # pitch: B_phi/B_rho = tan(psi0 + psi1 ln(rho/8)); tilt: B_z/|B| = sin(chi0 tanh z)
+    B, *_ = oracle.eval_fields(m2, [[0.0, 12.0, 0.7]])      # rho_hat = +y, phi_hat = -x
+    assert math.atan2(-B[0, 0], B[0, 1]) == pytest.approx(psi0 + psi1 * math.log(12 / 8), rel=1e-12)
+    assert B[0, 2] / np.linalg.norm(B[0]) == pytest.approx(math.sin(chi0 * math.tanh(0.7)), rel=1e-12)
+    # halo alone: B_h phi_hat at rho = r_h, |z| = z_h0
+    p3 = p.copy(); p3[0] = 0.0
+    m3 = oracle.Model("full16", p3)
+    for zz in (zh0, -zh0):
+        B, *_ = oracle.eval_fields(m3, [[rh, 0.0, zz]])
+        np.testing.assert_allclose(B[0], [0.0, Bh, 0.0], atol=1e-15)
+    # N_0(r_obs) = 4.0e-5 with the C_0 of the golden file; n_e(0,0,0) = ne0
+    assert float(p[9]) == pytest.approx(golden_constants["C0_cr"], rel=1e-7)
+    m4 = oracle.Model("full16", np.concatenate([p[:9], [golden_constants["C0_cr"]], p[10:]]))
+    _, N0, ne, _ = oracle.eval_fields(m4, [list(wl.OBSERVER), [0.0, 0.0, 0.0]])
+    assert N0[0] == pytest.approx(golden_constants["N0_earth"], rel=1e-9)
+    assert ne[1] == pytest.approx(p[13], rel=1e-15)
+    # exponential disc law: N0(rho+5, z) / N0(rho, z) = e^-1 for h_r = 5; sech^2 in z
+    _, N0, _, _ = oracle.eval_fields(m4, [[4.0, 0.0, 0.0], [9.0, 0.0, 0.0], [4.0, 0.0, 1.0]])
+    assert N0[1] / N0[0] == pytest.approx(math.exp(-1.0), rel=1e-12)
+    assert N0[2] / N0[0] == pytest.approx(1 / math.cosh(1.0) ** 2, rel=1e-12)
+
+
+def test_disc4_equals_full16_limit():
+    w = wl.config(0)
+    p = w.params.astype(np.float64)[0]
+    aux = w.aux.astype(np.float64)
+    m4 = oracle.Model("disc4", p, aux=aux)
+    p16 = np.array([p[0], p[1], p[2], p[3], 1e300, 0.0, 1.5, 4.0, 0.4, aux[0], aux[1], aux[2], aux[3], aux[4], aux[5], aux[6]])
+    m16 = oracle.Model("full16", p16)
+    a = oracle.forward(m4, 4, 32, 20.0, [2.4e9])
+    c = oracle.forward(m16, 4, 32, 20.0, [2.4e9])
+    for x, y in zip(a, c):
+        np.testing.assert_allclose(x, y, rtol=1e-12, atol=1e-20)
+
+
+# ---------------------------------------------------------------------- invariants (C-3 #4)
+@pytest.fixture(scope="module")
+def small_full16():
+    w = wl.config(4).scaled(nside=4, n_los=96)
+    return w, oracle.Model("full16", w.params.astype(np.float64))
+
+
+def test_polarisation_bound_and_npix(small_full16):
+    w, m = small_full16
+    I, Q, U = oracle.forward(m, w.nside, w.n_los, w.s_max, w.freqs)
+    assert I.shape == (1, 8, 12 * 4 * 4)
+    P = np.sqrt(Q * Q + U * U)
+    assert np.all(P <= PI_FRAC(3.0) * I * (1 + 1e-12))
+    assert np.all(I > 0)
+    # depolarisation grows towards low frequency: P/I smaller at 408 MHz than at 30 GHz on average
+    assert (P[0, 0] / I[0, 0]).mean() < (P[0, -1] / I[0, -1]).mean()
+    # I_f is a pure power law in frequency: nu^((1-alpha)/2 - 2) = nu^-3 at alpha = 3
+    np.testing.assert_allclose(I[0, 0] / I[0, -1], (w.freqs[-1] / w.freqs[0]) ** 3, rtol=1e-11)
+
+
+def test_sign_invariants(small_full16):
+    w, m = small_full16
+    p = w.params.astype(np.float64)[0]
+    args = (w.nside, w.n_los, w.s_max, w.freqs[:2])
+    I, Q, U = oracle.forward(m, *args)
+    flipB = p.copy(); flipB[0] *= -1; flipB[5] *= -1            # B -> -B
+    I2, Q2, U2 = oracle.forward(oracle.Model("full16", flipB), *args)
+    np.testing.assert_allclose(I2, I, rtol=1e-12)                # (i) I invariant
+    assert np.abs(Q2 - Q).max() > 1e-3 * np.abs(Q).max()         # signed B_LOS: Q,U do change
+    both = flipB.copy(); both[13] *= -1                          # (iii) joint flip (B, n_e) -> (-B, -n_e)
+    I3, Q3, U3 = oracle.forward(oracle.Model("full16", both), *args)
+    np.testing.assert_allclose(Q3, Q, rtol=1e-10, atol=1e-16 * np.abs(Q).max())
+    np.testing.assert_allclose(U3, U, rtol=1e-10, atol=1e-16 * np.abs(U).max())
+    none = p.copy(); none[13] = 0.0                              # (ii) n_e = 0: B -> -B leaves Q,U
+    nflip = flipB.copy(); nflip[13] = 0.0
+    a = oracle.forward(oracle.Model("full16", none), *args)
+    c = oracle.forward(oracle.Model("full16", nflip), *args)
+    for x, y in zip(a, c):
+        np.testing.assert_allclose(x, y, rtol=1e-10, atol=1e-16 * np.abs(x).max())
+    # n_e = 0: no rotation, Q_f/I_f and U_f/I_f independent of frequency
+    np.testing.assert_allclose(a[1][0, 0] / a[0][0, 0], a[1][0, 1] / a[0][0, 1], rtol=1e-10, atol=1e-14)
+    np.testing.assert_allclose(a[2][0, 0] / a[0][0, 0], a[2][0, 1] / a[0][0, 1], rtol=1e-10, atol=1e-14)
+
+
+def test_scalings(small_full16):
+    w, m = small_full16
+    p = w.params.astype(np.float64)[0]
+    args = (w.nside, w.n_los, w.s_max, [1.4e9])
+    I, Q, U = oracle.forward(m, *args)
+    p2 = p.copy(); p2[9] *= 2.5                                  # e linear in N_0
+    I2, Q2, U2 = oracle.forward(oracle.Model("full16", p2), *args)
+    np.testing.assert_allclose(I2, 2.5 * I, rtol=1e-12)
+    np.testing.assert_allclose(Q2, 2.5 * Q, rtol=1e-10, atol=1e-18)
+    # DISC4: I ~ b0^((alpha+1)/2)
+    w0 = wl.config(0)
+    q = w0.params.astype(np.float64)[0]
+    aux = w0.aux.astype(np.float64); aux[3] = 2.6
+    Ia, _, _ = oracle.forward(oracle.Model("disc4", q, aux=aux), 4, 64, 20.0, [23e9])
+    q2 = q.copy(); q2[0] *= 1.7
+    Ib, _, _ = oracle.forward(oracle.Model("disc4", q2, aux=aux), 4, 64, 20.0, [23e9])
+    np.testing.assert_allclose(Ib, Ia * 1.7 ** ((2.6 + 1) / 2), rtol=1e-12)
+
+
+# ---------------------------------------------------------------------- grid (C-3 #8)
+def test_grid_trilinear_reproduces_linear_function():
+    rng = np.random.default_rng(11)
+    shape, box = (5, 7, 4), (10.0, 14.0, 6.0)
+    X, Y, Z = wl.grid_nodes(shape, box)
+    a = rng.normal(size=3); M = rng.normal(size=(3, 3))
+    G = a + np.stack([X, Y, Z], -1) @ M.T
+    m = oracle.Model("grid_b", G, aux=wl.AUX_NOMINAL, box=box)
+    pts = rng.uniform(-1, 1, size=(50, 3)) * np.array(box) / 2
+    B, *_ = oracle.eval_fields(m, pts)
+    np.testing.assert_allclose(B, a + pts @ M.T, rtol=1e-12, atol=1e-12)
+    # nodes are on the faces: the node value itself is returned at a node, zero just outside
+    B, *_ = oracle.eval_fields(m, [[-5.0, -7.0, -3.0], [5.0, 7.0, 3.0], [5.0000001, 0, 0], [0, 0, -3.0000001]])
+    np.testing.assert_allclose(B[0], G[0, 0, 0], rtol=1e-13)
+    np.testing.assert_allclose(B[1], G[-1, -1, -1], rtol=1e-13)
+    assert np.all(B[2:] == 0)
+    # layout [ix][iy][iz][c]: a single nonzero node value is seen only near that node
+    G2 = np.zeros(shape + (3,)); G2[3, 2, 1, 2] = 7.0
+    m2 = oracle.Model("grid_b", G2, aux=wl.AUX_NOMINAL, box=box)
+    B, *_ = oracle.eval_fields(m2, [[X[3, 2, 1], Y[3, 2, 1], Z[3, 2, 1]], [X[2, 2, 1], Y[2, 2, 1], Z[2, 2, 1]]])
+    np.testing.assert_allclose(B, [[0, 0, 7.0], [0, 0, 0]], atol=1e-13)
+
+
+def test_constant_grid_equals_uniform():
+    Bv = np.array([2.0, -1.0, 0.5])
+    G = np.broadcast_to(Bv, (6, 6, 5, 3)).copy()
+    aux = [3e-5, 1e30, 1e30, 2.8, 0.02, 1e30, 1e30]
+    mg = oracle.Model("grid_b", G, aux=aux, box=(40.0, 40.0, 8.0))
+    mu = oracle.Model("uniform", [*Bv, 3e-5, 0.02, 2.8])
+    a = oracle.forward(mg, 4, 40, 3.9, [0.408e9, 2.4e9])
+    c = oracle.forward(mu, 4, 40, 3.9, [0.408e9, 2.4e9])
+    for x, y in zip(a, c):
+        np.testing.assert_allclose(x, y, rtol=1e-11, atol=1e-16 * np.abs(y).max())
+
+
+def test_grid_sampled_from_disc_converges_to_analytic():
+    # Fig. 6 lower: the gridded-B map approaches the analytic-B map as N_x grows
+    w0 = wl.config(0)
+    p = w0.params.astype(np.float64)[0]; aux = w0.aux.astype(np.float64)
+    ana = oracle.forward(oracle.Model("disc4", p, aux=aux), 4, 128, 20.0, [2.4e9])
+    errs = []
+    for nx in (32, 64, 128):
+        shape, box = (nx, nx, nx // 4), (44.0, 44.0, 10.0)
+        X, Y, Z = wl.grid_nodes(shape, box)
+        G = wl.spiral_pattern(X, Y, Z, *p)
+        grd = oracle.forward(oracle.Model("grid_b", G, aux=aux, box=box), 4, 128, 20.0, [2.4e9])
+        errs.append(max(np.std(g - a) / np.std(a) for g, a in zip(grd, ana)))
+    assert errs[0] > errs[1] > errs[2]
+    assert errs[2] < 0.08
+
+
+# ---------------------------------------------------------------------- convergence (C-3 #9)
+def test_convergence_order_smooth_and_clipped(golden_constants):
+    # smooth fields (exponential discs + halo, no spiral cut-off): midpoint rule is second order
+    p = wl.FULL16_NOMINAL.copy(); p[0] = 0.0
+    m = oracle.Model("full16", p)
+    ref = np.array(oracle.forward_dir(m, 0.3, 0.05, 4096, 30.0, [1.4e9])).ravel()
+    e = [np.abs(np.array(oracle.forward_dir(m, 0.3, 0.05, n, 30.0, [1.4e9])).ravel() - ref).max() for n in (128, 256, 512)]
+    assert 3.3 < e[0] / e[1] < 4.7 and 3.3 < e[1] / e[2] < 4.9
+    # paper toy: homogeneous sphere R0 = 4 kpc clipped inside [0, s_max]: first order,
+    # "for every doubling of the integration points, the error is halved"; residuals below 1 mK
+    toy = uniform((6.0, 0.0, 0.0), ne=0.01, r0=4.0)
+    exact_I = golden_constants["toy_I_kelvin"]
+    # the paper's paths end on the box faces, so every sightline has its own Delta r_i; with the fixed
+    # s_max of this build the same spread of Delta is obtained by varying s_max (15..25 kpc here).
+    s_maxes = np.linspace(15.0, 25.0, 64)
+    stds = []
+    for n in (512, 1024, 2048, 4096):
+        resid = np.array([oracle.forward_dir(toy, math.pi / 2, 0.0, n, s, [2.4e9])[0][0] - exact_I for s in s_maxes])
+        stds.append(np.std(resid))
+        bound = 0.5 * (s_maxes.max() / n) * golden_constants["toy_I_kelvin_per_kpc"]
+        assert np.abs(resid).max() <= bound * (1 + 1e-9)          # at most half a cell of emission is mis-assigned
+        if n == 1024:
+            assert np.abs(resid).max() < golden_constants["toy_residual_max_kelvin"]
+            assert 0.3 * golden_constants["toy_residual_std_I"] < stds[-1] < 3 * golden_constants["toy_residual_std_I"]
+    ratios = np.array(stds[:-1]) / np.array(stds[1:])
+    assert np.all((ratios > 1.5) & (ratios < 2.6)), ratios
