@@ -1,0 +1,123 @@
+/* synax.h -- C ABI of libsynax: line-of-sight integration of Galactic synchrotron Stokes I/Q/U with
+ * Faraday rotation on HEALPix sightlines, and its adjoint (VJP) w.r.t. the field-model parameters.
+ * Hand-written CUDA for NVIDIA B200 (sm_100a).  No CPU fallback: every call needs a CUDA device.
+ *
+ * The operation is the hot path of arXiv:2410.01136 ("synax"); citations P:L<n> are line numbers of
+ * the paper text (reference PAPER.md), S:<tag> the readings listed in DESIGN.md section 3.
+ *
+ *   direction of RING pixel i -> (l_i, b_i)                         P:L108 (healpy; Gorski+05 P:L352)
+ *   N_int equal segments on [0, s_max], midpoints r_{i,n}            P:L108, observer P:L49
+ *   fields B, N_0, n_e, alpha at r_{i,n} (analytic or gridded)       P:L99-110, Eq.12-13
+ *   j_I Eq.(2), j_P Eq.(5), chi_0 Eq.(8)
+ *   Faraday depth Eq.(7) P:L79 (half-cell midpoint form), chi = RM lambda^2 + chi_0 Eq.(6)
+ *   I,Q,U = sum_n j {1, cos 2chi, sin 2chi} Delta_r  Eq.(9), in Kelvin (Rayleigh-Jeans)
+ *   reverse-mode gradient of all of the above (the paper uses JAX AD)
+ *
+ * Units: micro-gauss, kpc, cm^-3, rad, Hz, Kelvin.  HEALPix RING pixel order.  The line of sight n
+ * points away from the observer; B_LOS = B.n is signed; +Q is along increasing Galactic longitude
+ * (B along e_E gives Q = +P).
+ *
+ * Pointers: "DEVICE" = device memory of the plan's CUDA device, "HOST" = ordinary host memory.  All
+ * buffers are caller-owned; the library never frees or keeps them.  Device calls are asynchronous on
+ * `cuda_stream` (a cudaStream_t; NULL = default stream) and the buffers must stay alive until the
+ * stream reaches the call; *_host calls return after their results are in the host buffers.
+ * Every failure returns a non-zero status and sets synax_last_error(); nothing aborts or throws.
+ * Invalid arguments launch no kernel.  Parameter VALUES are not range-checked (NaN in, NaN out).
+ */
+#ifndef SYNAX_H
+#define SYNAX_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct synax_plan synax_plan; /* opaque, library-owned */
+
+typedef enum {
+  SYNAX_OK = 0,
+  SYNAX_ERR_INVALID_ARG = 1,
+  SYNAX_ERR_UNSUPPORTED = 2,
+  SYNAX_ERR_CUDA = 3,
+  SYNAX_ERR_ALLOC = 4
+} synax_status;
+
+typedef enum {
+  /* WMAP logarithmic spiral, Eq.(13): params (b0 [uG], psi0, psi1, chi0 [rad]);
+   * B = 0 outside 3 < rho < 20 kpc (S:C-2#7).  CR density Eq.(12), alpha and n_e come from `aux`. */
+  SYNAX_MODEL_DISC4 = 0,
+  /* 16 parameters (BASELINE.json configs 2/4; S:App.C):
+   * b0 psi0 psi1 chi0 h_b | B_h z_h0 r_h w_h | n0 h_r h_z alpha | ne0 h_er h_ez
+   * disc = DISC4 * exp(-(rho-8)/h_b); halo = B_h /(1+((|z|-z_h0)/w_h)^2) (rho/r_h) exp(1-rho/r_h) phi_hat;
+   * N_0 = n0 exp(-rho/h_r) sech^2(z/h_z) Eq.(12); n_e likewise. */
+  SYNAX_MODEL_FULL16 = 1,
+  /* B on a regular grid [nx][ny][nz][3] (fp32, c fastest), nodes on the faces of a box of lengths
+   * (lx,ly,lz) centred on the Galactic centre, trilinear interpolation, zero outside (
+   * S:C-2#12).  params IS the grid; CR/alpha/n_e from `aux`.  batch must be 1. */
+  SYNAX_MODEL_GRID_B = 2,
+  /* homogeneous fields everywhere (toy of P:L123): params (Bx,By,Bz [uG], N0, n_e, alpha). */
+  SYNAX_MODEL_UNIFORM = 3
+} synax_model_kind;
+
+typedef struct {
+  int32_t kind;     /* synax_model_kind */
+  int32_t n_params; /* 4, 16, nx*ny*nz*3 (<2^31), 6 -- must match kind */
+  const float* aux; /* HOST. DISC4 / GRID_B: {C0, h_r, h_z, alpha, ne0, h_er, h_ez}; else NULL */
+  int32_t nx, ny, nz; /* GRID_B only, each >= 2 */
+  float lx, ly, lz;   /* GRID_B only, kpc, > 0 */
+} synax_model;
+
+/* Plan = geometry shared by all calls: HEALPix nside (1..8192), samples per sightline n_los
+ * (1..65536), path length s_max > 0 (every sightline is integrated over [0, s_max], S:C-2#6),
+ * frequencies (HOST, 1..32 values, Hz, > 0) and the observer position (HOST, kpc; P:L49 uses
+ * (-8.3, 0, 0.006)).  Created on the current CUDA device; computes and caches the pixel directions
+ * there (step A1) and returns after that kernel finished. */
+synax_status synax_plan_create(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
+                               int32_t n_freq, const double observer_kpc[3], synax_plan** out);
+synax_status synax_plan_destroy(synax_plan* plan); /* NULL is allowed */
+int64_t synax_plan_npix(const synax_plan* plan);  /* 12 nside^2, or -1 for NULL */
+
+/* Options (tests / experiments).  key "precision": 0 = auto (default: fp32 pass, sightlines whose
+ * Faraday rotation angle exceeds "escalate_rad" are redone with a float64 Faraday chain),
+ * 1 = fp32 only, 2 = float64 Faraday chain for every sightline.  key "escalate_rad": threshold in
+ * radians.  key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32). */
+synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value);
+
+/* Pixel directions as cached by the plan: out[4*p..] = (cos l, sin l, cos b, sin b), DEVICE float64
+ * [npix][4].  For tests of step A1. */
+synax_status synax_plan_directions(const synax_plan* plan, double* out_device, void* cuda_stream);
+
+/* Forward.  params: DEVICE fp32 [batch][n_params] (GRID_B: the grid, batch == 1).
+ * I, Q, U: DEVICE fp32 [batch][n_freq][npix], overwritten, Kelvin. */
+synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
+                           int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
+
+/* VJP.  dI, dQ, dU: DEVICE fp32 [batch][n_freq][npix] cotangents (any may be NULL = zeros).
+ * grad: DEVICE fp32 [batch][n_params] (GRID_B: [nx][ny][nz][3]); overwritten:
+ * grad[b][j] = sum_{f,p} dI dI/dtheta_j + dQ dQ/dtheta_j + dU dU/dtheta_j.
+ * DISC4 / GRID_B: `aux` values are constants (not differentiated). */
+synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,
+                       int32_t batch, const float* dI, const float* dQ, const float* dU, float* grad,
+                       void* cuda_stream);
+
+/* Same operations with HOST buffers of the same shapes: the call copies the inputs to the device,
+ * runs, copies the results back and synchronises the stream before returning. */
+synax_status synax_forward_host(const synax_plan* plan, const synax_model* model, const float* params,
+                                int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
+synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, const float* params,
+                            int32_t batch, const float* dI, const float* dQ, const float* dU,
+                            float* grad, void* cuda_stream);
+
+/* Counters since plan creation (for bench.py's gpu_launches): out[0] = kernels launched,
+ * out[1] = sightlines redone with the float64 Faraday chain in the last forward (read back lazily:
+ * valid after the stream has been synchronised). */
+synax_status synax_plan_stats(const synax_plan* plan, int64_t out[2]);
+
+const char* synax_last_error(void); /* thread-local, library-owned, never NULL */
+const char* synax_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SYNAX_H */

@@ -1,0 +1,218 @@
+"""ctypes binding of libsynax.so -- same names and argument order as include/synax.h.
+
+PyTorch is used for device memory and streams only.  Nothing is computed here.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libsynax.so"
+
+STATUS = {0: "SYNAX_OK", 1: "SYNAX_ERR_INVALID_ARG", 2: "SYNAX_ERR_UNSUPPORTED", 3: "SYNAX_ERR_CUDA",
+          4: "SYNAX_ERR_ALLOC"}
+KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
+
+# every symbol include/synax.h declares
+exported_symbols = ("synax_plan_create", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_option",
+                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host",
+                    "synax_plan_stats", "synax_last_error", "synax_version")
+
+
+class SynaxError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class _CModel(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("n_params", ctypes.c_int32), ("aux", ctypes.POINTER(ctypes.c_float)),
+                ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
+                ("lx", ctypes.c_float), ("ly", ctypes.c_float), ("lz", ctypes.c_float)]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Load the in-tree CUDA library; raise loudly when it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2410_01136_b200.build` "
+                          "(nvcc, sm_100a).  There is no CPU fallback.")
+    L = ctypes.CDLL(str(_LIB_PATH))
+    vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+    L.synax_plan_create.argtypes = [i32, i32, dbl, ctypes.POINTER(dbl), i32, ctypes.POINTER(dbl), ctypes.POINTER(vp)]
+    L.synax_plan_create.restype = ctypes.c_int
+    L.synax_plan_destroy.argtypes = [vp]
+    L.synax_plan_destroy.restype = ctypes.c_int
+    L.synax_plan_npix.argtypes = [vp]
+    L.synax_plan_npix.restype = i64
+    L.synax_plan_set_option.argtypes = [vp, ctypes.c_char_p, dbl]
+    L.synax_plan_set_option.restype = ctypes.c_int
+    L.synax_plan_directions.argtypes = [vp, vp, vp]
+    L.synax_plan_directions.restype = ctypes.c_int
+    L.synax_plan_stats.argtypes = [vp, ctypes.POINTER(i64)]
+    L.synax_plan_stats.restype = ctypes.c_int
+    fwd = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, vp]
+    bwd = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, vp, vp]
+    for name, at in (("synax_forward", fwd), ("synax_forward_host", fwd), ("synax_vjp", bwd), ("synax_vjp_host", bwd)):
+        getattr(L, name).argtypes = at
+        getattr(L, name).restype = ctypes.c_int
+    L.synax_last_error.restype = ctypes.c_char_p
+    L.synax_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise SynaxError(rc, load_library().synax_last_error().decode())
+
+
+class Model:
+    """Mirror of `synax_model`.  kind: 'disc4' | 'full16' | 'grid_b' | 'uniform'."""
+
+    def __init__(self, kind: str, aux: Optional[Sequence[float]] = None, grid_shape=None, box=None):
+        self.kind = kind
+        self._aux = None if aux is None else np.ascontiguousarray(np.asarray(aux, dtype=np.float32))
+        c = _CModel()
+        c.kind = KINDS[kind]
+        if kind == "grid_b":
+            c.nx, c.ny, c.nz = (int(v) for v in grid_shape)
+            c.lx, c.ly, c.lz = (float(v) for v in box)
+            c.n_params = c.nx * c.ny * c.nz * 3
+        else:
+            c.n_params = {"disc4": 4, "full16": 16, "uniform": 6}[kind]
+        c.aux = None if self._aux is None else self._aux.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+        self.c = c
+
+    @property
+    def n_params(self) -> int:
+        return int(self.c.n_params)
+
+
+class Plan:
+    """synax_plan_create / synax_plan_destroy."""
+
+    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006)):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("synax needs a CUDA device (B200); there is no CPU fallback")
+        L = load_library()
+        torch.cuda.current_stream()  # make sure the CUDA context of the current device exists
+        torch.zeros(1, device="cuda")
+        f = np.ascontiguousarray(np.asarray(freqs, dtype=np.float64).ravel())
+        o = np.ascontiguousarray(np.asarray(observer, dtype=np.float64).ravel())
+        h = ctypes.c_void_p()
+        _check(L.synax_plan_create(int(nside), int(n_los), float(s_max), f.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                   int(f.size), o.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), ctypes.byref(h)))
+        self.h = h
+        self.nside, self.n_los, self.s_max, self.freqs = int(nside), int(n_los), float(s_max), f
+        self.n_freq = int(f.size)
+        self.npix = int(L.synax_plan_npix(h))
+
+    def set_option(self, key: str, value: float):
+        _check(load_library().synax_plan_set_option(self.h, key.encode(), float(value)))
+
+    def directions(self):
+        import torch
+        out = torch.empty((self.npix, 4), dtype=torch.float64, device="cuda")
+        _check(load_library().synax_plan_directions(self.h, out.data_ptr(), _stream()))
+        return out
+
+    def stats(self):
+        out = (ctypes.c_int64 * 2)()
+        _check(load_library().synax_plan_stats(self.h, out))
+        return {"launches": int(out[0]), "escalated": int(out[1])}
+
+    def close(self):
+        if getattr(self, "h", None):
+            load_library().synax_plan_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev_f32(t, what):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{what} must be a contiguous float32 CUDA tensor")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _batch_of(model: Model, params) -> int:
+    if model.kind == "grid_b":
+        if params.numel() != model.n_params:
+            raise ValueError("grid tensor does not match the model's grid shape")
+        return 1
+    if params.shape[-1] != model.n_params:
+        raise ValueError(f"params last dim {params.shape[-1]} != n_params {model.n_params}")
+    return int(params.numel() // model.n_params)
+
+
+def forward(plan: Plan, model: Model, params, out=None):
+    """synax_forward: params CUDA fp32 [batch][P] (or the grid) -> (I, Q, U) CUDA fp32 [batch][n_freq][npix]."""
+    import torch
+    batch = _batch_of(model, params)
+    if out is None:
+        out = tuple(torch.empty((batch, plan.n_freq, plan.npix), dtype=torch.float32, device=params.device) for _ in range(3))
+    I, Q, U = out
+    _check(load_library().synax_forward(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
+                                        _dev_f32(I, "I"), _dev_f32(Q, "Q"), _dev_f32(U, "U"), _stream()))
+    return I, Q, U
+
+
+def vjp(plan: Plan, model: Model, params, dI, dQ, dU, out=None):
+    """synax_vjp: cotangent maps CUDA fp32 [batch][n_freq][npix] (None = zeros) -> grad CUDA fp32 like params."""
+    import torch
+    batch = _batch_of(model, params)
+    if out is None:
+        out = torch.empty_like(params)
+    ptr = lambda t, n: ctypes.c_void_p(None) if t is None else _dev_f32(t, n)  # noqa: E731
+    _check(load_library().synax_vjp(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
+                                    ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _dev_f32(out, "grad"), _stream()))
+    return out
+
+
+def _host_f32(a, what):
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous):
+        raise TypeError(f"{what} must be a C-contiguous float32 numpy array")
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+def forward_host(plan: Plan, model: Model, params: np.ndarray, out=None):
+    """synax_forward_host: numpy float32 in, numpy float32 (I, Q, U) out; copies inside the call."""
+    batch = 1 if model.kind == "grid_b" else int(params.size // model.n_params)
+    if out is None:
+        out = tuple(np.empty((batch, plan.n_freq, plan.npix), dtype=np.float32) for _ in range(3))
+    I, Q, U = out
+    _check(load_library().synax_forward_host(plan.h, ctypes.byref(model.c), _host_f32(params, "params"), batch,
+                                             _host_f32(I, "I"), _host_f32(Q, "Q"), _host_f32(U, "U"), _stream()))
+    return I, Q, U
+
+
+def vjp_host(plan: Plan, model: Model, params: np.ndarray, dI, dQ, dU, out=None):
+    """synax_vjp_host: numpy float32 in/out; copies inside the call."""
+    batch = 1 if model.kind == "grid_b" else int(params.size // model.n_params)
+    if out is None:
+        out = np.empty_like(params)
+    ptr = lambda a, n: ctypes.c_void_p(None) if a is None else _host_f32(a, n)  # noqa: E731
+    _check(load_library().synax_vjp_host(plan.h, ctypes.byref(model.c), _host_f32(params, "params"), batch,
+                                         ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _host_f32(out, "grad"), _stream()))
+    return out

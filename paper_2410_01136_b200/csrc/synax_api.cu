@@ -1,0 +1,413 @@
+// synax_api.cu -- the C ABI of libsynax (include/synax.h): plan object, argument validation, kernel
+// dispatch.  Host-side only orchestration; every step of the hot path runs in the kernels of
+// synax_forward.cuh / synax_vjp.cuh / synax_grid.cuh.
+#include "../../include/synax.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "synax_forward.cuh"
+#include "synax_vjp.cuh"
+#include "synax_grid.cuh"
+
+using namespace synax;
+
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+static synax_status fail(synax_status st, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return st;
+}
+#define CUDA_TRY(expr)                                                                        \
+  do {                                                                                        \
+    cudaError_t e_ = (expr);                                                                  \
+    if (e_ != cudaSuccess)                                                                    \
+      return fail(e_ == cudaErrorMemoryAllocation ? SYNAX_ERR_ALLOC : SYNAX_ERR_CUDA,         \
+                  "%s failed: %s", #expr, cudaGetErrorString(e_));                            \
+  } while (0)
+
+struct synax_plan {
+  int nside, n_los, n_freq, device;
+  int64_t npix;
+  double s_max, delta;
+  double obs[3];
+  double* dirs;       // device [npix][4]
+  FreqTab ft;
+  int precision;      // 0 auto, 1 fp32 only, 2 float64 chain everywhere
+  double escalate_rad;
+  int lanes;          // 0 heuristic
+  int* d_flag_count;  // device
+  int* h_flag_count;  // pinned host mirror (last forward)
+  mutable int64_t launches;
+};
+
+static double faraday_K_per_kpc() {
+  const double K = SYNAX_QE * SYNAX_QE * SYNAX_QE / (2.0 * SYNAX_PI * SYNAX_ME * SYNAX_ME * SYNAX_C * SYNAX_C * SYNAX_C * SYNAX_C);
+  return K * 1.0e4 * 1.0e-6 * SYNAX_KPC;  // rad m^-2 per (cm^-3 uG kpc), Eq.(7)
+}
+
+extern "C" const char* synax_last_error(void) { return g_err; }
+extern "C" const char* synax_version(void) { return "synax-b200 0.1 (sm_100a)"; }
+
+extern "C" synax_status synax_plan_create(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
+                                          int32_t n_freq, const double observer_kpc[3], synax_plan** out) {
+  if (!out) return fail(SYNAX_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (nside < 1 || nside > 8192) return fail(SYNAX_ERR_INVALID_ARG, "nside %d not in 1..8192", nside);
+  if (n_los < 1 || n_los > 65536) return fail(SYNAX_ERR_INVALID_ARG, "n_los %d not in 1..65536", n_los);
+  if (!(s_max_kpc > 0.0) || !std::isfinite(s_max_kpc)) return fail(SYNAX_ERR_INVALID_ARG, "s_max must be > 0");
+  if (!freqs_hz || n_freq < 1 || n_freq > kMaxFreq) return fail(SYNAX_ERR_INVALID_ARG, "n_freq %d not in 1..32 or freqs NULL", n_freq);
+  if (!observer_kpc) return fail(SYNAX_ERR_INVALID_ARG, "observer is NULL");
+  for (int i = 0; i < 3; ++i)
+    if (!std::isfinite(observer_kpc[i])) return fail(SYNAX_ERR_INVALID_ARG, "observer not finite");
+  for (int f = 0; f < n_freq; ++f)
+    if (!(freqs_hz[f] > 0.0) || !std::isfinite(freqs_hz[f])) return fail(SYNAX_ERR_INVALID_ARG, "freqs[%d] must be > 0", f);
+
+  synax_plan* p = new (std::nothrow) synax_plan();
+  if (!p) return fail(SYNAX_ERR_ALLOC, "host allocation failed");
+  std::memset(p, 0, sizeof(*p));
+  p->nside = nside; p->n_los = n_los; p->n_freq = n_freq;
+  p->npix = 12LL * nside * nside;
+  p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los;
+  for (int i = 0; i < 3; ++i) p->obs[i] = observer_kpc[i];
+  p->precision = 0; p->escalate_rad = 100.0; p->lanes = 0;
+  const double KF = faraday_K_per_kpc();
+  p->ft.n_freq = n_freq;
+  for (int f = 0; f < kMaxFreq; ++f) {
+    if (f < n_freq) {
+      const double lam = SYNAX_C / freqs_hz[f] * 1.0e-2;  // m
+      const double k = 2.0 * lam * lam * KF * p->delta;   // rad per unit sum(n_e B_LOS)
+      p->ft.k_rad[f] = (float)k; p->ft.k_turn[f] = k / (2.0 * SYNAX_PI); p->ft.freq[f] = freqs_hz[f];
+    } else {
+      p->ft.k_rad[f] = 0.f; p->ft.k_turn[f] = 0.0; p->ft.freq[f] = 1.0;
+    }
+  }
+  cudaError_t e = cudaGetDevice(&p->device);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->dirs, (size_t)p->npix * 4 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, sizeof(int));
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_flag_count, sizeof(int));
+  if (e == cudaSuccess) {
+    *p->h_flag_count = 0;
+    e = cudaMemset(p->d_flag_count, 0, sizeof(int));
+  }
+  if (e == cudaSuccess) {
+    const int64_t blocks = (p->npix + 255) / 256;
+    pix2ang_kernel<<<(unsigned)blocks, 256>>>((int64_t)nside, p->npix, p->dirs);
+    p->launches++;
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  }
+  if (e != cudaSuccess) {
+    synax_status st = fail(e == cudaErrorMemoryAllocation ? SYNAX_ERR_ALLOC : SYNAX_ERR_CUDA, "plan_create: %s", cudaGetErrorString(e));
+    if (p->dirs) cudaFree(p->dirs);
+    if (p->d_flag_count) cudaFree(p->d_flag_count);
+    if (p->h_flag_count) cudaFreeHost(p->h_flag_count);
+    delete p;
+    return st;
+  }
+  *out = p;
+  return SYNAX_OK;
+}
+
+extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
+  if (!plan) return SYNAX_OK;
+  cudaFree(plan->dirs);
+  cudaFree(plan->d_flag_count);
+  cudaFreeHost(plan->h_flag_count);
+  delete plan;
+  return SYNAX_OK;
+}
+
+extern "C" int64_t synax_plan_npix(const synax_plan* plan) { return plan ? plan->npix : -1; }
+
+extern "C" synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value) {
+  if (!plan || !key) return fail(SYNAX_ERR_INVALID_ARG, "plan or key is NULL");
+  if (!std::strcmp(key, "precision")) {
+    if (value != 0 && value != 1 && value != 2) return fail(SYNAX_ERR_INVALID_ARG, "precision must be 0, 1 or 2");
+    plan->precision = (int)value;
+  } else if (!std::strcmp(key, "escalate_rad")) {
+    if (!(value > 0)) return fail(SYNAX_ERR_INVALID_ARG, "escalate_rad must be > 0");
+    plan->escalate_rad = value;
+  } else if (!std::strcmp(key, "lanes")) {
+    if (value != 0 && value != 1 && value != 8 && value != 32) return fail(SYNAX_ERR_INVALID_ARG, "lanes must be 0, 1, 8 or 32");
+    plan->lanes = (int)value;
+  } else {
+    return fail(SYNAX_ERR_INVALID_ARG, "unknown option '%s'", key);
+  }
+  return SYNAX_OK;
+}
+
+extern "C" synax_status synax_plan_directions(const synax_plan* plan, double* out_device, void* cuda_stream) {
+  if (!plan || !out_device) return fail(SYNAX_ERR_INVALID_ARG, "plan or out is NULL");
+  CUDA_TRY(cudaMemcpyAsync(out_device, plan->dirs, (size_t)plan->npix * 4 * sizeof(double), cudaMemcpyDeviceToDevice,
+                           (cudaStream_t)cuda_stream));
+  return SYNAX_OK;
+}
+
+extern "C" synax_status synax_plan_stats(const synax_plan* plan, int64_t out[2]) {
+  if (!plan || !out) return fail(SYNAX_ERR_INVALID_ARG, "plan or out is NULL");
+  out[0] = plan->launches;
+  out[1] = *plan->h_flag_count;
+  return SYNAX_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+static synax_status check_model(const synax_plan* plan, const synax_model* m, const void* params, int32_t batch,
+                                int* code) {
+  if (!plan) return fail(SYNAX_ERR_INVALID_ARG, "plan is NULL");
+  if (!m) return fail(SYNAX_ERR_INVALID_ARG, "model is NULL");
+  if (!params) return fail(SYNAX_ERR_INVALID_ARG, "params is NULL");
+  if (batch < 1) return fail(SYNAX_ERR_INVALID_ARG, "batch %d < 1", batch);
+  switch (m->kind) {
+    case SYNAX_MODEL_DISC4:
+      if (m->n_params != 4) return fail(SYNAX_ERR_INVALID_ARG, "DISC4 needs n_params == 4");
+      if (!m->aux) return fail(SYNAX_ERR_INVALID_ARG, "DISC4 needs aux");
+      *code = kAnalyticDisc; break;
+    case SYNAX_MODEL_FULL16:
+      if (m->n_params != 16) return fail(SYNAX_ERR_INVALID_ARG, "FULL16 needs n_params == 16");
+      *code = kAnalyticFull; break;
+    case SYNAX_MODEL_UNIFORM:
+      if (m->n_params != 6) return fail(SYNAX_ERR_INVALID_ARG, "UNIFORM needs n_params == 6");
+      *code = kUniform; break;
+    case SYNAX_MODEL_GRID_B: {
+      if (!m->aux) return fail(SYNAX_ERR_INVALID_ARG, "GRID_B needs aux");
+      if (batch != 1) return fail(SYNAX_ERR_INVALID_ARG, "GRID_B needs batch == 1");
+      if (m->nx < 2 || m->ny < 2 || m->nz < 2) return fail(SYNAX_ERR_INVALID_ARG, "grid dims must be >= 2");
+      if (!(m->lx > 0) || !(m->ly > 0) || !(m->lz > 0)) return fail(SYNAX_ERR_INVALID_ARG, "grid box lengths must be > 0");
+      const int64_t n = (int64_t)m->nx * m->ny * m->nz * 3;
+      if (n >= (1LL << 31) || m->n_params != (int32_t)n) return fail(SYNAX_ERR_INVALID_ARG, "GRID_B needs n_params == nx*ny*nz*3 < 2^31");
+      *code = kGridB; break;
+    }
+    default: return fail(SYNAX_ERR_INVALID_ARG, "unknown model kind %d", m->kind);
+  }
+  if ((int64_t)batch * plan->npix >= (1LL << 31)) return fail(SYNAX_ERR_INVALID_ARG, "batch * npix must be < 2^31");
+  return SYNAX_OK;
+}
+
+static int pick_lanes(const synax_plan* plan, int64_t n_sl) {
+  if (plan->lanes) return plan->lanes;
+  const int64_t want = 300000;  // threads needed to fill 148 SMs a few times over
+  if (n_sl >= want) return 1;
+  if (n_sl * 8 >= want) return 8;
+  return 32;
+}
+
+static int next_freq_block(int remaining) {
+  if (remaining >= 8) return 8;
+  if (remaining >= 4) return 4;
+  return remaining;  // 1, 2, 3
+}
+
+template <int CODE, int G>
+static void launch_forward_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+  switch (nf) {
+    case 1: forward_kernel<CODE, G, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 2: forward_kernel<CODE, G, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 3: forward_kernel<CODE, G, 3><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 4: forward_kernel<CODE, G, 4><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    default: forward_kernel<CODE, G, 8><<<blocks, kBlock, 0, st>>>(a, ft); break;
+  }
+}
+template <int CODE>
+static void launch_forward(int G, int nf, int64_t n_sl, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+  const unsigned blocks = (unsigned)((n_sl * G + kBlock - 1) / kBlock);
+  if (G == 1) launch_forward_nf<CODE, 1>(nf, blocks, st, a, ft);
+  else if (G == 8) launch_forward_nf<CODE, 8>(nf, blocks, st, a, ft);
+  else launch_forward_nf<CODE, 32>(nf, blocks, st, a, ft);
+}
+template <int CODE>
+static void launch_precise(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+  switch (nf) {
+    case 1: forward_precise_kernel<CODE, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 2: forward_precise_kernel<CODE, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 3: forward_precise_kernel<CODE, 3><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 4: forward_precise_kernel<CODE, 4><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    default: forward_precise_kernel<CODE, 8><<<blocks, kBlock, 0, st>>>(a, ft); break;
+  }
+}
+
+static AuxHost make_aux(const synax_model* m) {
+  AuxHost a;
+  for (int i = 0; i < 7; ++i) a.v[i] = m->aux ? m->aux[i] : 0.0f;
+  return a;
+}
+
+static Geometry make_geo(const synax_plan* plan) {
+  Geometry g;
+  g.npix = plan->npix; g.n_los = plan->n_los; g.delta = plan->delta;
+  for (int i = 0; i < 3; ++i) g.obs[i] = plan->obs[i];
+  g.dirs = plan->dirs;
+  return g;
+}
+
+static int sm_count(int device) {
+  static int cached[64];
+  if (device < 0 || device >= 64) return 148;
+  if (!cached[device]) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || n <= 0) n = 148;
+    cached[device] = n;
+  }
+  return cached[device];
+}
+
+extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
+                                      int32_t batch, float* I, float* Q, float* U, void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int64_t n_sl = plan->npix * batch;
+
+  BatchConsts* bc = nullptr;
+  CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
+  prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
+                                                      make_aux(model), plan->ft, plan->delta, bc);
+  plan->launches++;
+
+  ForwardArgs a;
+  a.geo = make_geo(plan); a.bc = bc; a.batch = batch; a.I = I; a.Q = Q; a.U = U;
+  a.n_freq_total = plan->n_freq;
+  a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
+
+  if (code == kGridB) {
+    synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, st, &plan->launches);
+    cudaFreeAsync(bc, st);
+    if (gs != SYNAX_OK) return fail(gs, "grid forward failed: %s", cudaGetErrorString(cudaGetLastError()));
+    return SYNAX_OK;
+  }
+
+  float k_max = 0.f;
+  for (int f = 0; f < plan->n_freq; ++f) k_max = fmaxf(k_max, plan->ft.k_rad[f]);
+  const bool fast = plan->precision != 2;
+  const bool escalate = plan->precision == 0;
+  if (escalate) {
+    CUDA_TRY(cudaMallocAsync((void**)&a.flag_list, sizeof(int) * (size_t)n_sl, st));
+    CUDA_TRY(cudaMemsetAsync(plan->d_flag_count, 0, sizeof(int), st));
+    a.flag_S = (float)(plan->escalate_rad / (double)k_max);
+  }
+  const int G = pick_lanes(plan, n_sl);
+  const unsigned pblocks = (unsigned)(sm_count(plan->device) * 8);
+  for (int f0 = 0; f0 < plan->n_freq;) {
+    const int nf = next_freq_block(plan->n_freq - f0);
+    a.f0 = f0;
+    if (fast) {
+      if (code == kAnalyticDisc) launch_forward<kAnalyticDisc>(G, nf, n_sl, st, a, plan->ft);
+      else if (code == kAnalyticFull) launch_forward<kAnalyticFull>(G, nf, n_sl, st, a, plan->ft);
+      else launch_forward<kUniform>(G, nf, n_sl, st, a, plan->ft);
+      plan->launches++;
+    }
+    f0 += nf;
+  }
+  if (!fast || escalate) {
+    ForwardArgs pa = a;
+    if (!fast) pa.flag_list = nullptr;  // every sightline
+    for (int f0 = 0; f0 < plan->n_freq;) {
+      const int nf = next_freq_block(plan->n_freq - f0);
+      pa.f0 = f0;
+      if (code == kAnalyticDisc) launch_precise<kAnalyticDisc>(nf, pblocks, st, pa, plan->ft);
+      else if (code == kAnalyticFull) launch_precise<kAnalyticFull>(nf, pblocks, st, pa, plan->ft);
+      else launch_precise<kUniform>(nf, pblocks, st, pa, plan->ft);
+      plan->launches++;
+      f0 += nf;
+    }
+  }
+  cudaError_t e = cudaGetLastError();
+  if (escalate) {
+    cudaMemcpyAsync(plan->h_flag_count, plan->d_flag_count, sizeof(int), cudaMemcpyDeviceToHost, st);
+    cudaFreeAsync(a.flag_list, st);
+  }
+  cudaFreeAsync(bc, st);
+  if (e != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward launch failed: %s", cudaGetErrorString(e));
+  return SYNAX_OK;
+}
+
+extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,
+                                  int32_t batch, const float* dI, const float* dQ, const float* dU, float* grad,
+                                  void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  BatchConsts* bc = nullptr;
+  CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
+  prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
+                                                      make_aux(model), plan->ft, plan->delta, bc);
+  plan->launches++;
+  synax_status rs;
+  if (code == kGridB)
+    rs = grid_vjp(plan->ft, make_geo(plan), bc, model, params, dI, dQ, dU, grad, st, &plan->launches);
+  else
+    rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
+                      dI, dQ, dU, grad, st, &plan->launches);
+  cudaFreeAsync(bc, st);
+  if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));
+  return SYNAX_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// HOST-buffer variants: copies inside the call, stream synchronised on return.
+// ------------------------------------------------------------------------------------------------
+extern "C" synax_status synax_forward_host(const synax_plan* plan, const synax_model* model, const float* params,
+                                           int32_t batch, float* I, float* Q, float* U, void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t pbytes = sizeof(float) * (size_t)model->n_params * (size_t)batch;
+  const size_t mbytes = sizeof(float) * (size_t)batch * plan->n_freq * (size_t)plan->npix;
+  float *dp = nullptr, *dm = nullptr;
+  CUDA_TRY(cudaMallocAsync((void**)&dp, pbytes, st));
+  CUDA_TRY(cudaMallocAsync((void**)&dm, 3 * mbytes, st));
+  CUDA_TRY(cudaMemcpyAsync(dp, params, pbytes, cudaMemcpyHostToDevice, st));
+  float* dI = dm; float* dQ = dm + mbytes / sizeof(float); float* dU = dm + 2 * (mbytes / sizeof(float));
+  synax_status rs = synax_forward(plan, model, dp, batch, dI, dQ, dU, cuda_stream);
+  if (rs == SYNAX_OK) {
+    CUDA_TRY(cudaMemcpyAsync(I, dI, mbytes, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(Q, dQ, mbytes, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(U, dU, mbytes, cudaMemcpyDeviceToHost, st));
+  }
+  cudaFreeAsync(dp, st);
+  cudaFreeAsync(dm, st);
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return rs;
+}
+
+extern "C" synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, const float* params,
+                                       int32_t batch, const float* dI, const float* dQ, const float* dU, float* grad,
+                                       void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t pbytes = sizeof(float) * (size_t)model->n_params * (size_t)batch;
+  const size_t mcount = (size_t)batch * plan->n_freq * (size_t)plan->npix;
+  float *dp = nullptr, *dg = nullptr, *dc = nullptr;
+  CUDA_TRY(cudaMallocAsync((void**)&dp, pbytes, st));
+  CUDA_TRY(cudaMallocAsync((void**)&dg, pbytes, st));
+  CUDA_TRY(cudaMallocAsync((void**)&dc, 3 * mcount * sizeof(float), st));
+  CUDA_TRY(cudaMemcpyAsync(dp, params, pbytes, cudaMemcpyHostToDevice, st));
+  const float* src[3] = {dI, dQ, dU};
+  const float* dev[3] = {nullptr, nullptr, nullptr};
+  for (int k = 0; k < 3; ++k)
+    if (src[k]) {
+      CUDA_TRY(cudaMemcpyAsync(dc + k * mcount, src[k], mcount * sizeof(float), cudaMemcpyHostToDevice, st));
+      dev[k] = dc + k * mcount;
+    }
+  synax_status rs = synax_vjp(plan, model, dp, batch, dev[0], dev[1], dev[2], dg, cuda_stream);
+  if (rs == SYNAX_OK) CUDA_TRY(cudaMemcpyAsync(grad, dg, pbytes, cudaMemcpyDeviceToHost, st));
+  cudaFreeAsync(dp, st); cudaFreeAsync(dg, st); cudaFreeAsync(dc, st);
+  CUDA_TRY(cudaStreamSynchronize(st));
+  return rs;
+}

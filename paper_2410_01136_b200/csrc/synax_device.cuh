@@ -1,0 +1,231 @@
+// synax_device.cuh -- device-side building blocks of libsynax (sm_100a): math helpers, per-batch
+// constants, analytic field evaluators (fp32 fast chain, fp64 precise chain).
+// Shares nothing with oracle/ (see DESIGN.md).  Citations: P:L<n> = paper text line, S:<tag> =
+// DESIGN.md section 3 reading.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace synax {
+
+constexpr int kMaxFreq = 32;
+constexpr int kMaxAnalyticParams = 16;
+
+// ---- physical constants, Gaussian CGS (CODATA 2018) -- used on the host and in the fp64 prologue
+#define SYNAX_QE 4.80320471257e-10
+#define SYNAX_ME 9.1093837015e-28
+#define SYNAX_C 2.99792458e10
+#define SYNAX_KB 1.380649e-16
+#define SYNAX_KPC 3.0856775814913673e21
+#define SYNAX_PI 3.14159265358979323846
+
+// ------------------------------------------------------------------------------------------------
+// fp32 hardware approximations (XU / MUFU pipe), flush-to-zero.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rsqrt(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_sin(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_cos(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// sin and cos on the FMA pipe, ~1 ulp for |x| < ~200 (Cody-Waite reduction by pi/2 + minimax
+// polynomials on [-pi/4, pi/4]).  Used where the MUFU's 5e-7 absolute error would be systematic
+// along a sightline (the pitch / tilt angles of the disc field), see DESIGN.md section 5.
+__device__ __forceinline__ void sincos_fma(float x, float& s, float& c) {
+  const float t = fmaf(x, 0.636619772367581343f, 12582912.0f);  // 1.5 * 2^23: round to nearest int
+  const int q = __float_as_int(t);
+  const float k = t - 12582912.0f;
+  float r = fmaf(k, -1.57079625129699707031f, x);
+  r = fmaf(k, -7.54978941586159635335e-08f, r);
+  const float r2 = r * r;
+  float ps = fmaf(r2, -1.9515295891e-4f, 8.3321608736e-3f);
+  ps = fmaf(ps, r2, -1.6666654611e-1f);
+  ps = fmaf(ps * r2, r, r);                                     // sin(r)
+  float pc = fmaf(r2, 2.443315711809948e-5f, -1.388731625493765e-3f);
+  pc = fmaf(pc, r2, 4.166664568298827e-2f);
+  pc = fmaf(pc * r2, r2, fmaf(r2, -0.5f, 1.0f));                // cos(r)
+  const float ss = (q & 1) ? pc : ps;
+  const float cs = (q & 1) ? ps : pc;
+  s = (q & 2) ? -ss : ss;
+  c = ((q + 1) & 2) ? -cs : cs;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-batch-element constants, written by prologue_kernel (fp64 math, rounded once).
+// Canonical 16-parameter analytic model; DISC4 maps onto it with h_b = inf, B_h = 0.
+// ------------------------------------------------------------------------------------------------
+struct BatchConsts {
+  // raw parameters, canonical FULL16 order (S:App.C), as float and double
+  float p[kMaxAnalyticParams];
+  // derived fp32
+  float k_hb;        // -log2(e)/h_b      (0 for DISC4)
+  float inv_wh, inv_rh;
+  float k_hr, k_hz;  // -log2(e)/h_r, -2 log2(e)/h_z
+  float k_her, k_hez;
+  float q_exp;       // (alpha-3)/4 : (B_perp^2)^q_exp
+  float pi_frac;     // (alpha+1)/(alpha+7/3)   Eq.(5)/Eq.(2)
+  int alpha_is_3;
+  float coefI[kMaxFreq];  // c_f(alpha) * Delta  [K per (cm^-3 uG^((alpha+1)/2))]
+  float coefP[kMaxFreq];  // pi_frac * coefI
+  // VJP only
+  float dlnc_dalpha[kMaxFreq];  // d ln c_f / d alpha
+  float dpi_dalpha_over_pi;     // d ln Pi / d alpha
+  // uniform model
+  float uB[3], uN0, une;
+};
+
+struct FreqTab {
+  int n_freq;
+  float k_rad[kMaxFreq];    // 2 lambda_f^2 K_F Delta : Faraday angle (rad) per unit sum(n_e B_LOS)
+  double k_turn[kMaxFreq];  // the same / (2 pi), float64, for exact turn reduction of large offsets
+  double freq[kMaxFreq];
+};
+
+struct Geometry {
+  int64_t npix;
+  int n_los;
+  double delta;   // s_max / n_los  (kpc)
+  double obs[3];
+  const double* dirs;  // [npix][4] = cos l, sin l, cos b, sin b
+};
+
+// per-sightline direction triad
+struct Triad {
+  double nxd, nyd, nzd;    // line of sight, float64 (positions, mask)
+  float nx, ny, nz;
+  float eNx, eNy, eNz;     // towards Galactic north
+  float eEx, eEy;          // towards increasing l (z component is 0)
+};
+
+__device__ __forceinline__ Triad load_triad(const double* __restrict__ dirs, int64_t pix) {
+  const double4 d = *reinterpret_cast<const double4*>(dirs + 4 * pix);  // cl, sl, cb, sb
+  Triad t;
+  t.nxd = d.z * d.x; t.nyd = d.z * d.y; t.nzd = d.w;
+  t.nx = (float)t.nxd; t.ny = (float)t.nyd; t.nz = (float)t.nzd;
+  t.eNx = (float)(-d.w * d.x); t.eNy = (float)(-d.w * d.y); t.eNz = (float)d.z;
+  t.eEx = (float)(-d.y); t.eEy = (float)d.x;
+  return t;
+}
+
+// What one sample hands to the integrator (fp32): B projections, densities.
+struct SampleF {
+  float Bpar, BN, BE;  // uG
+  float N0, ne;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Analytic model, fp32 fast chain.  x,y,z,rho2 are the float64 sample coordinates rounded to fp32;
+// `inside` is the annulus test 3 < rho < 20 kpc taken in float64 (S:C-2#7).
+// Everything needed by the adjoint is kept in AnalyticAux.
+// ------------------------------------------------------------------------------------------------
+struct AnalyticAux {
+  float ir, rho, xr, yr;   // 1/rho, rho, x/rho, y/rho
+  float lr;                // ln(rho/8)
+  float sp, cp, sc, cc;    // sin/cos psi, sin/cos chi
+  float t;                 // tanh(z / 1 kpc)
+  float A;                 // b0 exp(-(rho-8)/h_b) inside the annulus, else 0
+  float u, L, R;           // halo: u, 1/(1+u^2), (rho/r_h) exp(1-rho/r_h)
+  float thz, thez;         // tanh(z/h_z), tanh(z/h_ez)
+};
+
+template <bool kHalo>
+__device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Triad& T, float x, float y,
+                                                  float z, float rho2, bool inside, SampleF& S,
+                                                  AnalyticAux& a) {
+  const float kLog2e = 1.4426950408889634f;
+  a.ir = mufu_rsqrt(rho2);
+  a.rho = rho2 * a.ir;
+  a.xr = x * a.ir; a.yr = y * a.ir;
+  const float az = fabsf(z);
+  // --- disc: B = A [cos psi cos chi rho_hat + sin psi cos chi phi_hat + sin chi z_hat]   Eq.(13)
+  a.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;        // ln(rho/8) = ln2/2 (lg2 rho^2 - 6)
+  const float psi = fmaf(P.p[2], a.lr, P.p[1]);
+  sincos_fma(psi, a.sp, a.cp);
+  const float e1 = mufu_ex2(-2.0f * kLog2e * az);               // tanh(|z|) = (1-e)/(1+e)
+  a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
+  const float chi = P.p[3] * a.t;
+  sincos_fma(chi, a.sc, a.cc);
+  const float rad = (P.k_hb != 0.0f) ? mufu_ex2(P.k_hb * (a.rho - 8.0f)) : 1.0f;
+  a.A = inside ? P.p[0] * rad : 0.0f;
+  const float Brho = a.A * a.cp * a.cc;
+  float Bphi = a.A * a.sp * a.cc;
+  const float Bz = a.A * a.sc;
+  if (kHalo) {  // toroidal halo, S:App.C
+    a.u = (az - P.p[6]) * P.inv_wh;
+    a.L = mufu_rcp(fmaf(a.u, a.u, 1.0f));
+    const float q = a.rho * P.inv_rh;
+    a.R = q * mufu_ex2(kLog2e * (1.0f - q));
+    Bphi = fmaf(P.p[5] * a.L, a.R, Bphi);
+  }
+  const float Bx = Brho * a.xr - Bphi * a.yr;
+  const float By = fmaf(Brho, a.yr, Bphi * a.xr);
+  S.Bpar = fmaf(Bx, T.nx, fmaf(By, T.ny, Bz * T.nz));           // B.n, signed (S:C-2#3)
+  S.BN = fmaf(Bx, T.eNx, fmaf(By, T.eNy, Bz * T.eNz));          // Eq.(8) numerator
+  S.BE = fmaf(Bx, T.eEx, By * T.eEy);                           // Eq.(8) denominator (S:C-2#4)
+  // --- N_0 = n0 exp(-rho/h_r) sech^2(z/h_z)  Eq.(12);  sech^2 w = 4e/(1+e)^2, e = exp(-2|w|)
+  const float ez = mufu_ex2(P.k_hz * az);
+  const float dz = 1.0f + ez;
+  const float iz = mufu_rcp(dz * dz);
+  S.N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * a.rho) * ez * iz;
+  a.thz = copysignf((1.0f - ez) * dz * iz, z);                  // tanh = (1-e)/(1+e)
+  const float ee = mufu_ex2(P.k_hez * az);
+  const float de = 1.0f + ee;
+  const float ie = mufu_rcp(de * de);
+  S.ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * a.rho) * ee * ie;
+  a.thez = copysignf((1.0f - ee) * de * ie, z);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Analytic model, float64 chain for the Faraday integrand (and, reused, for the emission inputs).
+// Used only for sightlines whose Faraday rotation is so large that fp32 round-off in n_e B_LOS
+// would exceed the parity tolerance.
+// ------------------------------------------------------------------------------------------------
+struct SampleD { double Bpar, BN, BE, N0, ne; };
+
+template <bool kHalo>
+__device__ __forceinline__ void eval_analytic_f64(const BatchConsts& P, const double4 dir, double x, double y,
+                                                  double z, SampleD& S) {
+  const double rho2 = x * x + y * y;
+  const double rho = sqrt(rho2);
+  const bool inside = (rho2 > 9.0) && (rho2 < 400.0);
+  double Brho = 0.0, Bphi = 0.0, Bz = 0.0;
+  const double az = fabs(z);
+  if (inside) {
+    const double psi = (double)P.p[1] + (double)P.p[2] * log(rho * 0.125);
+    const double chi = (double)P.p[3] * tanh(z);
+    double sp, cp, sc, cc;
+    sincos(psi, &sp, &cp);
+    sincos(chi, &sc, &cc);
+    double A = (double)P.p[0];
+    if (P.k_hb != 0.0f) A *= exp(-(rho - 8.0) / (double)P.p[4]);
+    Brho = A * cp * cc; Bphi = A * sp * cc; Bz = A * sc;
+  }
+  if (kHalo) {
+    const double u = (az - (double)P.p[6]) / (double)P.p[8];
+    const double q = rho / (double)P.p[7];
+    Bphi += (double)P.p[5] / (1.0 + u * u) * q * exp(1.0 - q);
+  }
+  const double ir = (rho > 0.0) ? 1.0 / rho : 0.0;
+  const double xr = x * ir, yr = y * ir;
+  const double Bx = Brho * xr - Bphi * yr, By = Brho * yr + Bphi * xr;
+  const double cl = dir.x, sl = dir.y, cb = dir.z, sb = dir.w;
+  S.Bpar = Bx * (cb * cl) + By * (cb * sl) + Bz * sb;
+  S.BN = Bz * cb - sb * (Bx * cl + By * sl);
+  S.BE = By * cl - Bx * sl;
+  const double chz = cosh(z / (double)P.p[11]);
+  S.N0 = (double)P.p[9] * exp(-rho / (double)P.p[10]) / (chz * chz);
+  const double che = cosh(z / (double)P.p[15]);
+  S.ne = (double)P.p[13] * exp(-rho / (double)P.p[14]) / (che * che);
+}
+
+// digamma for x > 0 (prologue only)
+__device__ inline double digamma_d(double x) {
+  double r = 0.0;
+  while (x < 10.0) { r -= 1.0 / x; x += 1.0; }
+  const double f = 1.0 / (x * x);
+  const double ser = f * (1.0 / 12.0 - f * (1.0 / 120.0 - f * (1.0 / 252.0 - f * (1.0 / 240.0 - f * (1.0 / 132.0)))));
+  return r + log(x) - 0.5 / x - ser;
+}
+
+}  // namespace synax

@@ -1,0 +1,392 @@
+// synax_forward.cuh -- plan geometry kernel (A1), per-batch prologue, forward kernels (A2-A8, A12).
+#pragma once
+#include "synax_device.cuh"
+
+namespace synax {
+
+constexpr int kBlock = 128;   // threads per CTA for the sightline kernels
+constexpr int kTile = 32;     // samples between re-basing of the local Faraday sum
+
+enum ModelCode { kAnalyticDisc = 0, kAnalyticFull = 1, kGridB = 2, kUniform = 3 };
+
+// ------------------------------------------------------------------------------------------------
+// A1: HEALPix RING pixel -> (cos l, sin l, cos b, sin b) in float64 (Gorski et al. 2005).
+// Integer ring arithmetic as in DESIGN.md section 4; once per plan.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int64_t isqrt_i64(int64_t v) {
+  int64_t r = (int64_t)sqrt((double)v);
+  while (r * r > v) --r;
+  while ((r + 1) * (r + 1) <= v) ++r;
+  return r;
+}
+
+__global__ void pix2ang_kernel(int64_t nside, int64_t npix, double* __restrict__ dirs) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= npix) return;
+  const int64_t ncap = 2 * nside * (nside - 1);
+  double z, phi, omz;  // omz = 1 - |z| kept separately for accurate cos b near the poles
+  if (p < ncap) {
+    const int64_t i = (1 + isqrt_i64(1 + 2 * p)) / 2;
+    const int64_t j = p + 1 - 2 * i * (i - 1);
+    omz = (double)(i * i) / (3.0 * (double)(nside * nside));
+    z = 1.0 - omz;
+    phi = ((double)j - 0.5) * SYNAX_PI / (2.0 * (double)i);
+  } else if (p < npix - ncap) {
+    const int64_t pp = p - ncap;
+    const int64_t i = pp / (4 * nside) + nside;
+    const int64_t j = pp % (4 * nside) + 1;
+    const double s = ((i + nside) & 1) ? 1.0 : 0.5;
+    z = (double)(2 * nside - i) * 2.0 / (3.0 * (double)nside);
+    omz = 1.0 - fabs(z);
+    phi = ((double)j - s) * SYNAX_PI / (2.0 * (double)nside);
+  } else {
+    const int64_t pp = npix - p;
+    const int64_t i = (1 + isqrt_i64(2 * pp - 1)) / 2;
+    const int64_t j = 4 * i + 1 - (pp - 2 * i * (i - 1));
+    omz = (double)(i * i) / (3.0 * (double)(nside * nside));
+    z = -1.0 + omz;
+    phi = ((double)j - 0.5) * SYNAX_PI / (2.0 * (double)i);
+  }
+  double sl, cl;
+  sincos(phi, &sl, &cl);
+  const double cb = sqrt(omz * (1.0 + fabs(z)));  // sin(theta) = sqrt((1-|z|)(1+|z|))
+  dirs[4 * p + 0] = cl; dirs[4 * p + 1] = sl; dirs[4 * p + 2] = cb; dirs[4 * p + 3] = z;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Prologue: raw parameters -> BatchConsts (float64 math, once per batch element per call).
+// Folds Eq.(2)'s constants, the Rayleigh-Jeans conversion (S:C-2#1) and the units into
+// c_f(alpha) so that I_f = c_f Delta sum_n N_0 (B_perp^2)^((alpha+1)/4)  with B in uG.
+// ------------------------------------------------------------------------------------------------
+struct AuxHost { float v[7]; };  // C0, h_r, h_z, alpha, ne0, h_er, h_ez
+
+__global__ void prologue_kernel(int code, const float* __restrict__ params, int n_params, int batch,
+                                AuxHost aux, FreqTab ft, double delta, BatchConsts* __restrict__ out) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= batch) return;
+  BatchConsts c;
+  double p[16];
+  for (int j = 0; j < 16; ++j) p[j] = 0.0;
+  double alpha;
+  if (code == kAnalyticFull) {
+    for (int j = 0; j < 16; ++j) p[j] = (double)params[(size_t)b * n_params + j];
+  } else if (code == kUniform) {
+    const float* q = params + (size_t)b * n_params;
+    c.uB[0] = q[0]; c.uB[1] = q[1]; c.uB[2] = q[2]; c.uN0 = q[3]; c.une = q[4];
+    p[12] = (double)q[5];
+    p[4] = p[7] = p[8] = p[10] = p[11] = p[14] = p[15] = 1.0;
+  } else {  // DISC4 or GRID_B: densities and alpha from aux
+    if (code == kAnalyticDisc)
+      for (int j = 0; j < 4; ++j) p[j] = (double)params[(size_t)b * n_params + j];
+    p[4] = 1.0;  // unused: k_hb = 0
+    p[6] = 0.0; p[7] = 1.0; p[8] = 1.0;
+    p[9] = aux.v[0]; p[10] = aux.v[1]; p[11] = aux.v[2]; p[12] = aux.v[3];
+    p[13] = aux.v[4]; p[14] = aux.v[5]; p[15] = aux.v[6];
+  }
+  alpha = p[12];
+  for (int j = 0; j < 16; ++j) c.p[j] = (float)p[j];
+  const double log2e = 1.4426950408889634;
+  c.k_hb = (code == kAnalyticFull) ? (float)(-log2e / p[4]) : 0.0f;
+  c.inv_wh = (float)(1.0 / p[8]);
+  c.inv_rh = (float)(1.0 / p[7]);
+  c.k_hr = (float)(-log2e / p[10]);
+  c.k_hz = (float)(-2.0 * log2e / fabs(p[11]));
+  c.k_her = (float)(-log2e / p[14]);
+  c.k_hez = (float)(-2.0 * log2e / fabs(p[15]));
+  c.q_exp = (float)((alpha - 3.0) * 0.25);
+  c.pi_frac = (float)((alpha + 1.0) / (alpha + 7.0 / 3.0));
+  c.alpha_is_3 = (c.p[12] == 3.0f) ? 1 : 0;
+  c.dpi_dalpha_over_pi = (float)(1.0 / (alpha + 1.0) - 1.0 / (alpha + 7.0 / 3.0));
+  // Eq.(2) prefactor with B^((1+alpha)/2) nu^((1-alpha)/2) factored out
+  const double g1 = tgamma(alpha * 0.25 - 1.0 / 12.0), g2 = tgamma(alpha * 0.25 + 19.0 / 12.0);
+  const double w = 4.0 * SYNAX_PI * SYNAX_ME * SYNAX_C / (3.0 * SYNAX_QE);
+  const double A_I = sqrt(3.0) * SYNAX_QE * SYNAX_QE * SYNAX_QE / (8.0 * SYNAX_PI * SYNAX_ME * SYNAX_C * SYNAX_C) *
+                     pow(w, (1.0 - alpha) * 0.5) * pow(2.0, (alpha + 1.0) * 0.5) / (alpha + 1.0) * g1 * g2;
+  const double dlnA = -0.5 * log(w) + 0.5 * log(2.0) - 1.0 / (alpha + 1.0) +
+                      0.25 * digamma_d(alpha * 0.25 - 1.0 / 12.0) + 0.25 * digamma_d(alpha * 0.25 + 19.0 / 12.0) +
+                      0.5 * log(1.0e-6);
+  for (int f = 0; f < kMaxFreq; ++f) {
+    if (f < ft.n_freq) {
+      const double nu = ft.freq[f];
+      const double TRJ = SYNAX_C * SYNAX_C / (2.0 * SYNAX_KB * nu * nu);
+      const double cf = TRJ * A_I * pow(nu, (1.0 - alpha) * 0.5) * pow(1.0e-6, (alpha + 1.0) * 0.5) * SYNAX_KPC * delta;
+      c.coefI[f] = (float)cf;
+      c.coefP[f] = (float)(cf * (alpha + 1.0) / (alpha + 7.0 / 3.0));
+      c.dlnc_dalpha[f] = (float)(dlnA - 0.5 * log(nu));
+    } else {
+      c.coefI[f] = c.coefP[f] = c.dlnc_dalpha[f] = 0.0f;
+    }
+  }
+  out[b] = c;
+}
+
+// ------------------------------------------------------------------------------------------------
+// small warp helpers over groups of G lanes (G = 1, 2, 4, ..., 32; groups are aligned)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double shfl_up_d(double v, int d, int width) {
+  int lo = __double2loint(v), hi = __double2hiint(v);
+  lo = __shfl_up_sync(0xffffffffu, lo, d, width);
+  hi = __shfl_up_sync(0xffffffffu, hi, d, width);
+  return __hiloint2double(hi, lo);
+}
+
+// exclusive prefix sum over the G lanes of a group
+template <int G>
+__device__ __forceinline__ double group_exclusive_scan(double v, int g) {
+  double incl = v;
+#pragma unroll
+  for (int d = 1; d < G; d <<= 1) {
+    const double o = shfl_up_d(incl, d, G);
+    if (g >= d) incl += o;
+  }
+  return incl - v;
+}
+
+template <int G>
+__device__ __forceinline__ float group_sum(float v) {
+#pragma unroll
+  for (int d = G / 2; d >= 1; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d, G);
+  return v;
+}
+template <int G>
+__device__ __forceinline__ float group_max(float v) {
+#pragma unroll
+  for (int d = G / 2; d >= 1; d >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, d, G));
+  return v;
+}
+
+// rotate (q,u) by the Faraday angle of a float64 offset: turns reduced in float64 (never form a
+// large angle in fp32), sin/cos of the reduced angle on the MUFU.
+__device__ __forceinline__ void rotate_by_offset(double k_turn, double S, float& q, float& u) {
+  double t = k_turn * S;
+  t -= rint(t);
+  const float a = (float)t * 6.283185307179586f;
+  const float c = mufu_cos(a), s = mufu_sin(a);
+  const float q2 = q * c - u * s;
+  u = fmaf(q, s, u * c);
+  q = q2;
+}
+
+// emission terms of one sample (A5): e~ = N0 (B_perp^2)^((alpha+1)/4), and e~ e^{2 i chi0}
+// = N0 (B_perp^2)^((alpha-3)/4) (B_E + i B_N)^2  -- no atan2, no division (S:C-2#19 for B_perp = 0).
+__device__ __forceinline__ void emission(const BatchConsts& P, float BN, float BE, float N0, float& eI,
+                                         float& a, float& b) {
+  const float bn2 = BN * BN, be2 = BE * BE;
+  const float Bt2 = bn2 + be2;
+  float w = N0;
+  if (!P.alpha_is_3) w = (Bt2 > 0.0f) ? N0 * mufu_ex2(P.q_exp * mufu_lg2(Bt2)) : 0.0f;
+  eI = w * Bt2;
+  a = w * (be2 - bn2);
+  b = w * (2.0f * BE * BN);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Forward, fp32 fast chain.  G lanes per sightline, each lane owns a contiguous chunk of samples
+// (no per-sample scan: each lane integrates with a chunk-local Faraday depth and its partial Q+iU
+// is rotated once by the float64 offset of the preceding lanes).  NF frequencies per pass.
+// ------------------------------------------------------------------------------------------------
+struct ForwardArgs {
+  Geometry geo;
+  const BatchConsts* bc;
+  int batch;
+  int f0;                 // first frequency of this pass
+  float* I; float* Q; float* U;
+  int n_freq_total;
+  float flag_S;           // flag a sightline when max |sum n_e B_LOS| exceeds this (<=0: never)
+  int* flag_count;        // device counter
+  int* flag_list;         // device list of flagged sightline ids (b * npix + p)
+};
+
+template <int CODE, int G, int NF>
+__global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__ ForwardArgs A,
+                                                         const __grid_constant__ FreqTab ft) {
+  const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const int g = (int)(tid % G);
+  int64_t sl = tid / G;
+  const int64_t n_sl = A.geo.npix * A.batch;
+  const bool valid = sl < n_sl;
+  if (!valid) sl = n_sl - 1;  // keep the lane alive for the shuffles
+  const int b = (int)(sl / A.geo.npix);
+  const int64_t pix = sl - (int64_t)b * A.geo.npix;
+  const BatchConsts& P = A.bc[b];
+  const Triad T = load_triad(A.geo.dirs, pix);
+
+  const int C = (A.geo.n_los + G - 1) / G;
+  const int n0 = g * C;
+  const int n1 = min(n0 + C, A.geo.n_los);
+  const double delta = A.geo.delta;
+  double s_d = ((double)n0 + 0.5) * delta;
+
+  float k_rad[NF];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[A.f0 + f];
+
+  float accI = 0.0f, accQ[NF], accU[NF];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
+  double carry = 0.0;            // chunk-local sum of n_e B_LOS over finished tiles
+  float cmax = 0.0f, cmin = 0.0f;
+
+  for (int ts = n0; ts < n1; ts += kTile) {
+    const int te = min(ts + kTile, n1);
+    float hi = 0.0f, lo = 0.0f;  // tile-local two-float sum of n_e B_LOS
+    float tq[NF], tu[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { tq[f] = 0.0f; tu[f] = 0.0f; }
+    for (int n = ts; n < te; ++n) {
+      // A2: midpoint position in float64 (mask decisions), rounded once to fp32 for the fields
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      s_d += delta;
+      SampleF S;
+      if (CODE == kUniform) {
+        S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz));
+        S.BN = fmaf(P.uB[0], T.eNx, fmaf(P.uB[1], T.eNy, P.uB[2] * T.eNz));
+        S.BE = fmaf(P.uB[0], T.eEx, P.uB[1] * T.eEy);
+        S.N0 = P.uN0; S.ne = P.une;
+      } else {
+        const double rho2d = fma(xd, xd, yd * yd);
+        const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+        AnalyticAux aux;
+        eval_analytic_f32<CODE == kAnalyticFull>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+      }
+      float eI, a, bq;
+      emission(P, S.BN, S.BE, S.N0, eI, a, bq);
+      accI += eI;
+      // A6: half-cell Faraday sum (S:C-2#5), tile-local, compensated
+      const float gn = S.ne * S.Bpar;
+      const float ph = fmaf(0.5f, gn, hi);
+      const float sum = hi + gn;
+      lo += gn - (sum - hi);
+      hi = sum;
+      // A7: rotate and accumulate per frequency
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const float th = k_rad[f] * ph;
+        const float c = mufu_cos(th), s = mufu_sin(th);
+        tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
+        tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+      }
+    }
+    if (ts == n0) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) { accQ[f] = tq[f]; accU[f] = tu[f]; }
+    } else {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        rotate_by_offset(ft.k_turn[A.f0 + f], carry, tq[f], tu[f]);
+        accQ[f] += tq[f]; accU[f] += tu[f];
+      }
+    }
+    carry += (double)hi + (double)lo;
+    cmax = fmaxf(cmax, (float)carry); cmin = fminf(cmin, (float)carry);
+  }
+
+  // combine the G lanes of the sightline
+  float absS;
+  if (G > 1) {
+    const double off = group_exclusive_scan<G>(carry, g);
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      if (g > 0) rotate_by_offset(ft.k_turn[A.f0 + f], off, accQ[f], accU[f]);
+      accQ[f] = group_sum<G>(accQ[f]);
+      accU[f] = group_sum<G>(accU[f]);
+    }
+    accI = group_sum<G>(accI);
+    absS = group_max<G>(fmaxf(fabsf((float)off + cmax), fabsf((float)off + cmin)));
+  } else {
+    absS = fmaxf(cmax, -cmin);
+  }
+  if (valid && g == 0) {
+    const int64_t npix = A.geo.npix;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * npix + pix;
+      A.I[o] = P.coefI[A.f0 + f] * accI;
+      A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
+      A.U[o] = P.coefP[A.f0 + f] * accU[f];
+    }
+    if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
+      const int k = atomicAdd(A.flag_count, 1);
+      A.flag_list[k] = (int)sl;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Forward, float64 Faraday chain, one warp per flagged sightline (list written by forward_kernel or
+// "all sightlines" when list == nullptr).  Persistent grid: warps stride over the list.
+// ------------------------------------------------------------------------------------------------
+template <int CODE, int NF>
+__global__ void __launch_bounds__(kBlock) forward_precise_kernel(const __grid_constant__ ForwardArgs A,
+                                                                 const __grid_constant__ FreqTab ft) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
+  const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
+  const int64_t n_sl = A.geo.npix * A.batch;
+  const int64_t count = A.flag_list ? (int64_t)(*A.flag_count) : n_sl;
+  const double delta = A.geo.delta;
+  const int C = (A.geo.n_los + 31) / 32;
+  for (int64_t it = warp; it < count; it += n_warps) {
+    const int64_t sl = A.flag_list ? (int64_t)A.flag_list[it] : it;
+    const int b = (int)(sl / A.geo.npix);
+    const int64_t pix = sl - (int64_t)b * A.geo.npix;
+    const BatchConsts& P = A.bc[b];
+    const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
+    const double nxd = dir.z * dir.x, nyd = dir.z * dir.y, nzd = dir.w;
+    const int n0 = lane * C, n1 = min(n0 + C, A.geo.n_los);
+    float accI = 0.0f, accQ[NF], accU[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
+    double S_loc = 0.0;
+    for (int n = n0; n < n1; ++n) {
+      const double s_d = ((double)n + 0.5) * delta;
+      const double xd = fma(s_d, nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, nzd, A.geo.obs[2]);
+      SampleD S;
+      if (CODE == kUniform) {
+        const double Bx = P.uB[0], By = P.uB[1], Bz = P.uB[2];
+        S.Bpar = Bx * nxd + By * nyd + Bz * nzd;
+        S.BN = Bz * dir.z - dir.w * (Bx * dir.x + By * dir.y);
+        S.BE = By * dir.x - Bx * dir.y;
+        S.N0 = P.uN0; S.ne = P.une;
+      } else {
+        eval_analytic_f64<CODE == kAnalyticFull>(P, dir, xd, yd, zd, S);
+      }
+      float eI, a, bq;
+      emission(P, (float)S.BN, (float)S.BE, (float)S.N0, eI, a, bq);
+      accI += eI;
+      const double gn = S.ne * S.Bpar;
+      const double ph = S_loc + 0.5 * gn;
+      S_loc += gn;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        float q = a, u = bq;
+        rotate_by_offset(ft.k_turn[A.f0 + f], ph, q, u);
+        accQ[f] += q; accU[f] += u;
+      }
+    }
+    const double off = group_exclusive_scan<32>(S_loc, lane);
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      rotate_by_offset(ft.k_turn[A.f0 + f], off, accQ[f], accU[f]);
+      accQ[f] = group_sum<32>(accQ[f]);
+      accU[f] = group_sum<32>(accU[f]);
+    }
+    accI = group_sum<32>(accI);
+    if (lane == 0) {
+      const int64_t npix = A.geo.npix;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * npix + pix;
+        A.I[o] = P.coefI[A.f0 + f] * accI;
+        A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
+        A.U[o] = P.coefP[A.f0 + f] * accU[f];
+      }
+    }
+  }
+}
+
+}  // namespace synax

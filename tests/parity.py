@@ -1,0 +1,79 @@
+"""Shared helpers for the GPU parity tests: run the CUDA library and the oracle on the same seeded
+inputs (paper_2410_01136_b200.workloads) and compare per map.  Imported only by tests/ and bench.py."""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle
+from paper_2410_01136_b200 import workloads as wl
+
+MAP_TOL = 1.0e-4    # max |delta| <= MAP_TOL * RMS(oracle map), per (batch, frequency, Stokes) -- BASELINE.json north_star
+GRAD_TOL = 1.0e-3   # relative error per gradient component -- BASELINE.json north_star
+
+
+def oracle_model(w: wl.Workload) -> oracle.Model:
+    p = w.params.astype(np.float64)
+    aux = None if w.aux is None else w.aux.astype(np.float64)
+    return oracle.Model(w.kind, p, aux=aux, box=w.box)
+
+
+def oracle_forward(w: wl.Workload, pix=None):
+    return oracle.forward(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix=pix)
+
+
+def oracle_vjp(w: wl.Workload, cots, pix=None):
+    return oracle.vjp(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, *cots, observer=w.observer, pix=pix)
+
+
+def gpu_objects(w: wl.Workload, **options):
+    import torch
+    import paper_2410_01136_b200 as sx
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer)
+    for k, v in options.items():
+        plan.set_option(k, v)
+    if w.kind == "grid_b":
+        model = sx.Model("grid_b", aux=w.aux, grid_shape=w.params.shape[:3], box=w.box)
+    else:
+        model = sx.Model(w.kind, aux=w.aux)
+    params = torch.from_numpy(w.params).cuda().contiguous()
+    return plan, model, params
+
+
+def gpu_forward(w: wl.Workload, **options):
+    import torch
+    import paper_2410_01136_b200 as sx
+    plan, model, params = gpu_objects(w, **options)
+    I, Q, U = sx.forward(plan, model, params)
+    torch.cuda.synchronize()
+    out = tuple(t.cpu().numpy().astype(np.float64) for t in (I, Q, U))
+    stats = plan.stats()
+    plan.close()
+    return out, stats
+
+
+def gpu_vjp(w: wl.Workload, cots, **options):
+    import torch
+    import paper_2410_01136_b200 as sx
+    plan, model, params = gpu_objects(w, **options)
+    d = [None if c is None else torch.from_numpy(np.ascontiguousarray(c, dtype=np.float32)).cuda() for c in cots]
+    g = sx.vjp(plan, model, params, *d)
+    torch.cuda.synchronize()
+    out = g.cpu().numpy().astype(np.float64)
+    plan.close()
+    return out
+
+
+def map_errors(gpu_maps, ref_maps):
+    """max |delta| / RMS(ref) per (Stokes, batch, freq) -> array [3][batch][n_freq]."""
+    errs = []
+    for g, r in zip(gpu_maps, ref_maps):
+        rms = np.sqrt(np.mean(r * r, axis=-1))
+        errs.append(np.abs(g - r).max(axis=-1) / rms)
+    return np.array(errs)
+
+
+def assert_maps_close(gpu_maps, ref_maps, tol=MAP_TOL, what=""):
+    e = map_errors(gpu_maps, ref_maps)
+    assert np.all(np.isfinite(e)), f"{what}: non-finite map"
+    assert e.max() <= tol, f"{what}: max|d|/RMS = {e.max():.3e} > {tol:g} (I,Q,U worst: {e.reshape(3, -1).max(1)})"
+    return e
