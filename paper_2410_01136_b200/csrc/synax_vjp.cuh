@@ -1,14 +1,402 @@
-// synax_vjp.cuh -- adjoint kernels for the analytic models (A9-A11).
+// synax_vjp.cuh -- adjoint (VJP) kernels for the analytic models: A9 cotangent fan-out, A10 reverse
+// half-cell scan (single forward-order sweep using sum_{n>m} = T - P_m),
+// A11 field partials and reductions.  Nothing of the forward is stored: everything is recomputed.
 #pragma once
-#include "synax_forward.cuh"
+#include <type_traits>
+
 #include "../../include/synax.h"
+#include "synax_forward.cuh"
 
 namespace synax {
+
+// ------------------------------------------------------------------------------------------------
+// Per-lane gradient accumulators.  Every parameter gradient is  acc1_j + Tw * acc2_j  where acc2
+// collects the unweighted Faraday terms h_mj = d(n_e B_LOS)_m / d theta_j  and acc1 the direct terms
+// minus (P_m - 1/2 Sbar_m) h_mj; Tw = T - P_off is known only after the sweep.
+// ------------------------------------------------------------------------------------------------
+template <int CODE>
+struct GradAcc;
+
+// rho/phi/z components of a Cartesian vector at a point with unit vectors rho_hat = (xr, yr, 0)
+__device__ __forceinline__ void to_cyl(float vx, float vy, float xr, float yr, float& vr, float& vp) {
+  vr = fmaf(vx, xr, vy * yr);
+  vp = fmaf(vy, xr, -vx * yr);
+}
+
+template <bool kFull>
+struct AnalyticGrad {
+  static constexpr int NB = kFull ? 9 : 4;
+  float b1[NB], b2[NB];      // B parameters: functional applied to V1 / V2
+  float n1[3];               // CR density parameters (direct only)
+  float e1[3], e2[3];        // n_e parameters
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int j = 0; j < NB; ++j) { b1[j] = 0.f; b2[j] = 0.f; }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { n1[j] = 0.f; e1[j] = 0.f; e2[j] = 0.f; }
+  }
+  // V1 = BbarN e_N + BbarE e_E - wgt ne n ; V2 = ne n ; MK = N0bar * N0 ; h-terms for n_e
+  __device__ __forceinline__ void add(const BatchConsts& P, const Triad& T, const AnalyticAux& a, const SampleF& S,
+                                      float z, float BNb, float BEb, float wgt, float MK) {
+    const float wn = wgt * S.ne;
+    const float v1x = fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, -wn * T.nx));
+    const float v1y = fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, -wn * T.ny));
+    const float v1z = fmaf(BNb, T.eNz, -wn * T.nz);
+    float v1r, v1p, nr, np;
+    to_cyl(v1x, v1y, a.xr, a.yr, v1r, v1p);
+    to_cyl(T.nx, T.ny, a.xr, a.yr, nr, np);
+    const float v2r = S.ne * nr, v2p = S.ne * np, v2z = S.ne * T.nz;
+    // disc: B = A [cp cc rho_hat + sp cc phi_hat + sc z_hat]
+    const float Acc = a.A * a.cc;
+    {
+      const float d1 = fmaf(Acc, fmaf(a.cp, v1r, a.sp * v1p), a.A * a.sc * v1z);  // B_disc . V1
+      const float d2 = fmaf(Acc, fmaf(a.cp, v2r, a.sp * v2p), a.A * a.sc * v2z);
+      b1[0] += d1; b2[0] += d2;                                                    // * 1/b0 at the end
+      const float p1 = Acc * fmaf(a.cp, v1p, -a.sp * v1r);                        // dB/dpsi0 . V
+      const float p2 = Acc * fmaf(a.cp, v2p, -a.sp * v2r);
+      b1[1] += p1; b2[1] += p2;
+      b1[2] = fmaf(a.lr, p1, b1[2]); b2[2] = fmaf(a.lr, p2, b2[2]);
+      const float tA = a.t * a.A;
+      b1[3] = fmaf(tA, fmaf(a.cc, v1z, -a.sc * fmaf(a.cp, v1r, a.sp * v1p)), b1[3]);
+      b2[3] = fmaf(tA, fmaf(a.cc, v2z, -a.sc * fmaf(a.cp, v2r, a.sp * v2p)), b2[3]);
+      if (kFull) {
+        const float dr = a.rho - 8.0f;
+        b1[4] = fmaf(dr, d1, b1[4]); b2[4] = fmaf(dr, d2, b2[4]);                 // * 1/h_b^2
+      }
+    }
+    if (kFull) {  // halo: B_h L R phi_hat
+      const float LR = a.L * a.R;
+      b1[5] = fmaf(LR, v1p, b1[5]); b2[5] = fmaf(LR, v2p, b2[5]);
+      const float RuL2 = a.R * a.u * a.L * a.L;
+      b1[6] = fmaf(RuL2, v1p, b1[6]); b2[6] = fmaf(RuL2, v2p, b2[6]);             // * 2 B_h / w_h
+      const float q = LR * fmaf(a.rho, P.inv_rh, -1.0f);
+      b1[7] = fmaf(q, v1p, b1[7]); b2[7] = fmaf(q, v2p, b2[7]);                   // * B_h / r_h
+      const float Ru2L2 = RuL2 * a.u;
+      b1[8] = fmaf(Ru2L2, v1p, b1[8]); b2[8] = fmaf(Ru2L2, v2p, b2[8]);           // * 2 B_h / w_h
+    }
+    if (kFull) {
+      // N_0 = n0 exp(-rho/h_r) sech^2(z/h_z):  dN0/dn0 = N0/n0, /dh_r = N0 rho/h_r^2, /dh_z = N0 2 tanh(z/h_z) z/h_z^2
+      n1[0] += MK; n1[1] = fmaf(MK, a.rho, n1[1]); n1[2] = fmaf(MK * a.thz, z, n1[2]);
+      const float h = S.ne * S.Bpar;  // d(ne Bpar)/d ln ne
+      const float hw = -wgt * h;
+      e1[0] += hw; e1[1] = fmaf(hw, a.rho, e1[1]); e1[2] = fmaf(hw * a.thez, z, e1[2]);
+      e2[0] += h; e2[1] = fmaf(h, a.rho, e2[1]); e2[2] = fmaf(h * a.thez, z, e2[2]);
+    }
+  }
+  // out[0..15] in canonical order (alpha handled by the caller)
+  __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
+    float g[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) g[j] = fmaf(Tw, b2[j], b1[j]);
+    out[0] = g[0] / P.p[0];
+    out[1] = g[1]; out[2] = g[2]; out[3] = g[3];
+    if (kFull) {
+      out[4] = g[4] / (P.p[4] * P.p[4]);
+      out[5] = g[5];
+      out[6] = g[6] * 2.0f * P.p[5] * P.inv_wh;
+      out[7] = g[7] * P.p[5] * P.inv_rh;
+      out[8] = g[8] * 2.0f * P.p[5] * P.inv_wh;
+      out[9] = n1[0] / P.p[9];
+      out[10] = n1[1] / (P.p[10] * P.p[10]);
+      out[11] = n1[2] * 2.0f / (P.p[11] * P.p[11]);
+      const float e0 = fmaf(Tw, e2[0], e1[0]), e1v = fmaf(Tw, e2[1], e1[1]), e2v = fmaf(Tw, e2[2], e1[2]);
+      out[13] = e0 / P.p[13];
+      out[14] = e1v / (P.p[14] * P.p[14]);
+      out[15] = e2v * 2.0f / (P.p[15] * P.p[15]);
+    }
+  }
+};
+
+struct UniformGrad {
+  float b1[3], b2[3], n1, e1, e2;
+  __device__ __forceinline__ void zero() {
+    for (int j = 0; j < 3; ++j) { b1[j] = 0.f; b2[j] = 0.f; }
+    n1 = e1 = e2 = 0.f;
+  }
+  __device__ __forceinline__ void add(const Triad& T, const SampleF& S, float BNb, float BEb, float wgt, float MK) {
+    const float wn = wgt * S.ne;
+    b1[0] += fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, -wn * T.nx));
+    b1[1] += fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, -wn * T.ny));
+    b1[2] += fmaf(BNb, T.eNz, -wn * T.nz);
+    b2[0] += S.ne * T.nx; b2[1] += S.ne * T.ny; b2[2] += S.ne * T.nz;
+    n1 += MK;                         // * 1/N0
+    e1 -= wgt * S.Bpar; e2 += S.Bpar;  // d(ne Bpar)/d ne = Bpar
+  }
+  __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
+    for (int j = 0; j < 3; ++j) out[j] = fmaf(Tw, b2[j], b1[j]);
+    out[3] = n1 / P.uN0;
+    out[4] = fmaf(Tw, e2, e1);
+  }
+};
+
+struct VjpArgs {
+  Geometry geo;
+  const BatchConsts* bc;
+  int batch, f0, n_freq_total;
+  const float* dI; const float* dQ; const float* dU;   // may be null
+  float* partial;   // [batch][n_blocks][16]
+  int n_blocks;     // blocks per batch element (gridDim.x)
+  int accumulate;   // 0: overwrite partials (first frequency block), 1: add
+};
+
+// grid = (n_blocks, batch); block = kBlock threads; G lanes per sightline.
+template <int CODE, int G, int NF>
+__global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
+  constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
+  const int b = blockIdx.y;
+  const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const int g = (int)(tid % G);
+  int64_t pix = tid / G;
+  const bool valid = pix < A.geo.npix;
+  if (!valid) pix = A.geo.npix - 1;
+  const BatchConsts& P = A.bc[b];
+  const Triad T = load_triad(A.geo.dirs, pix);
+  const int C = (A.geo.n_los + G - 1) / G;
+  const int n0 = g * C, n1 = min(n0 + C, A.geo.n_los);
+  const double delta = A.geo.delta;
+
+  // cotangents of this sightline, coefficients folded in (zero for padded lanes)
+  float cI = 0.f, cQ[NF], cU[NF], kr[NF];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+    const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * A.geo.npix + pix;
+    const float vI = (valid && A.dI) ? A.dI[o] : 0.f;
+    cQ[f] = (valid && A.dQ) ? A.dQ[o] * P.coefP[A.f0 + f] : 0.f;
+    cU[f] = (valid && A.dU) ? A.dU[o] * P.coefP[A.f0 + f] : 0.f;
+    cI = fmaf(vI, P.coefI[A.f0 + f], cI);
+    kr[f] = ft.k_rad[A.f0 + f];
+  }
+
+  // ---- pre-pass (G > 1): Faraday sum of each lane's chunk -> float64 offset of the preceding lanes
+  double off = 0.0;
+  if (G > 1) {
+    double s_d = ((double)n0 + 0.5) * delta;
+    double Sl = 0.0;
+    float hi = 0.f, lo = 0.f;
+    for (int n = n0; n < n1; ++n) {
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      s_d += delta;
+      SampleF S;
+      if (CODE == kUniform) {
+        S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz)); S.ne = P.une;
+      } else {
+        const double rho2d = fma(xd, xd, yd * yd);
+        AnalyticAux aux;
+        eval_analytic_f32<CODE == kAnalyticFull>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
+                                                 (rho2d > 9.0) && (rho2d < 400.0), S, aux);
+      }
+      const float gn = S.ne * S.Bpar;
+      const float sum = hi + gn;
+      lo += gn - (sum - hi);
+      hi = sum;
+      if (((n - n0) & (kTile - 1)) == kTile - 1) { Sl += (double)hi + (double)lo; hi = 0.f; lo = 0.f; }
+    }
+    Sl += (double)hi + (double)lo;
+    off = group_exclusive_scan<G>(Sl, g);
+  }
+
+  // ---- main sweep
+  typename std::conditional<CODE == kUniform, UniformGrad, AnalyticGrad<CODE == kAnalyticFull>>::type acc;
+  acc.zero();
+  float gAlpha = 0.f;          // sum_n 1/4 ln(B_perp^2) M K
+  float sumE = 0.f;            // sum_n e~_n
+  float pq[NF];                // sum_n (a u_f + b v_f) = Qbar_f Q_f + Ubar_f U_f (coefficients folded)
+#pragma unroll
+  for (int f = 0; f < NF; ++f) pq[f] = 0.f;
+  float Pl = 0.f;              // lane-local inclusive prefix of Sbar
+  double carry = 0.0;
+  double s_d = ((double)n0 + 0.5) * delta;
+  for (int ts = n0; ts < n1; ts += kTile) {
+    const int te = min(ts + kTile, n1);
+    // cotangents rotated by the Faraday angle of everything before this tile
+    float rq[NF], ru[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      // Qb cos(tb + tl) + Ub sin(tb + tl) = Qb' cos tl + Ub' sin tl,  Qb' = Qb cb + Ub sb, Ub' = -Qb sb + Ub cb
+      float q = cQ[f], u = cU[f];
+      rotate_by_offset(-ft.k_turn[A.f0 + f], off + carry, q, u);
+      rq[f] = q; ru[f] = u;
+    }
+    float hi = 0.f, lo = 0.f;
+    for (int n = ts; n < te; ++n) {
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      s_d += delta;
+      SampleF S;
+      AnalyticAux aux;
+      const float zf = (float)zd;
+      if (CODE == kUniform) {
+        S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz));
+        S.BN = fmaf(P.uB[0], T.eNx, fmaf(P.uB[1], T.eNy, P.uB[2] * T.eNz));
+        S.BE = fmaf(P.uB[0], T.eEx, P.uB[1] * T.eEy);
+        S.N0 = P.uN0; S.ne = P.une;
+      } else {
+        const double rho2d = fma(xd, xd, yd * yd);
+        eval_analytic_f32<CODE == kAnalyticFull>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
+                                                 (rho2d > 9.0) && (rho2d < 400.0), S, aux);
+      }
+      // emission terms
+      const float bn2 = S.BN * S.BN, be2 = S.BE * S.BE;
+      const float Bt2 = bn2 + be2;
+      float w = 1.0f, lgB = 0.f;
+      if (kAlpha || !P.alpha_is_3) {
+        lgB = (Bt2 > 0.f) ? mufu_lg2(Bt2) : 0.f;
+        if (!P.alpha_is_3) w = (Bt2 > 0.f) ? mufu_ex2(P.q_exp * lgB) : 0.f;
+      }
+      const float M = w * S.N0;
+      const float d2 = be2 - bn2, p2 = 2.0f * S.BE * S.BN;
+      const float a = M * d2, bq = M * p2;
+      // Faraday phase of this sample, tile-local
+      const float gn = S.ne * S.Bpar;
+      const float ph = fmaf(0.5f, gn, hi);
+      const float sum = hi + gn;
+      lo += gn - (sum - hi);
+      hi = sum;
+      // A9: fan-out over frequencies
+      float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const float th = kr[f] * ph;
+        const float c = mufu_cos(th), s = mufu_sin(th);
+        const float u = fmaf(rq[f], c, ru[f] * s);
+        const float v = fmaf(ru[f], c, -rq[f] * s);
+        Xc += u; Xs += v;
+        Yc = fmaf(kr[f], u, Yc); Ys = fmaf(kr[f], v, Ys);
+        if (kAlpha) pq[f] = fmaf(a, u, fmaf(bq, v, pq[f]));
+      }
+      // L_n = M K,  K = cI Bt2 + Xc d2 + Xs p2
+      const float K = fmaf(cI, Bt2, fmaf(Xc, d2, Xs * p2));
+      const float MK = M * K;
+      sumE = fmaf(M, Bt2, sumE);
+      if (kAlpha) gAlpha = fmaf(lgB, MK, gAlpha);
+      // cotangent of the phase variable S at this sample, and the D.4 weight
+      const float Sbar = fmaf(a, Ys, -bq * Yc);
+      Pl += Sbar;
+      const float wgt = fmaf(-0.5f, Sbar, Pl);
+      // B_N, B_E cotangents (direct): from M, d2, p2, Bt2 and the (B_perp^2)^q factor
+      const float tq_ = (Bt2 > 0.f) ? P.q_exp * MK / Bt2 : 0.f;  // d/dBt2 through w
+      const float BEb = 2.0f * fmaf(M, fmaf(S.BE, cI + Xc, S.BN * Xs), S.BE * tq_);
+      const float BNb = 2.0f * fmaf(M, fmaf(S.BN, cI - Xc, S.BE * Xs), S.BN * tq_);
+      if constexpr (CODE == kUniform) acc.add(T, S, BNb, BEb, wgt, MK);
+      else acc.add(P, T, aux, S, zf, BNb, BEb, wgt, MK);
+    }
+    carry += (double)hi + (double)lo;
+  }
+
+  // ---- combine: Tw = T - P_off for this lane
+  float Tw;
+  if (G > 1) {
+    const double Poff = group_exclusive_scan<G>((double)Pl, g);
+    float Tt = Pl;
+    Tt = group_sum<G>(Tt);
+    Tw = Tt - (float)Poff;
+  } else {
+    Tw = Pl;
+  }
+  float out[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) out[j] = 0.f;
+  acc.finish(P, Tw, out);
+  if (kAlpha) {
+    // alpha: 1/4 ln(B_perp^2) term + d ln c_f / d alpha * (Ibar I + Qbar Q + Ubar U) + dPi/Pi * (Qbar Q + Ubar U)
+    float ga = 0.25f * 0.6931471805599453f * gAlpha;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * A.geo.npix + pix;
+      const float vI = (valid && A.dI) ? A.dI[o] * P.coefI[A.f0 + f] : 0.f;
+      ga = fmaf(P.dlnc_dalpha[A.f0 + f], fmaf(vI, sumE, pq[f]), ga);
+      ga = fmaf(P.dpi_dalpha_over_pi, pq[f], ga);
+    }
+    out[CODE == kUniform ? 5 : 12] = ga;
+  }
+
+  // ---- block reduction -> partial[b][block][16]
+  constexpr int NP = (CODE == kUniform) ? 6 : (CODE == kAnalyticFull ? 16 : 4);
+  __shared__ float red[kBlock / 32][16];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int j = 0; j < NP; ++j) {
+    float v = out[j];
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    if (lane == 0) red[wid][j] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < NP) {
+    float v = 0.f;
+#pragma unroll
+    for (int k = 0; k < kBlock / 32; ++k) v += red[k][threadIdx.x];
+    float* dst = A.partial + ((size_t)b * A.n_blocks + blockIdx.x) * 16 + threadIdx.x;
+    *dst = A.accumulate ? (*dst + v) : v;
+  }
+}
+
+// partial[b][n_blocks][16] -> grad[b][n_params], float64 accumulation, deterministic order
+__global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_blocks, int n_params, float* __restrict__ grad) {
+  const int b = blockIdx.x;
+  const int j = threadIdx.x & 15;
+  const int part = threadIdx.x >> 4;        // 16 partial sums per parameter
+  __shared__ double sh[16][17];
+  double s = 0.0;
+  if (j < n_params)
+    for (int k = part; k < n_blocks; k += 16) s += (double)partial[((size_t)b * n_blocks + k) * 16 + j];
+  sh[part][j] = s;
+  __syncthreads();
+  if (threadIdx.x < n_params) {
+    double t = 0.0;
+    for (int k = 0; k < 16; ++k) t += sh[k][threadIdx.x];
+    grad[(size_t)b * n_params + threadIdx.x] = (float)t;
+  }
+}
+
+template <int CODE, int G>
+static void launch_vjp_nf(int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
+  switch (nf) {
+    case 1: vjp_kernel<CODE, G, 1><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 2: vjp_kernel<CODE, G, 2><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 3: vjp_kernel<CODE, G, 3><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 4: vjp_kernel<CODE, G, 4><<<grid, kBlock, 0, st>>>(a, ft); break;
+    default: vjp_kernel<CODE, G, 8><<<grid, kBlock, 0, st>>>(a, ft); break;
+  }
+}
+template <int CODE>
+static void launch_vjp(int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
+  if (G == 1) launch_vjp_nf<CODE, 1>(nf, grid, st, a, ft);
+  else if (G == 8) launch_vjp_nf<CODE, 8>(nf, grid, st, a, ft);
+  else launch_vjp_nf<CODE, 32>(nf, grid, st, a, ft);
+}
 
 static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, int batch,
                                  int n_params, int G, const float* dI, const float* dQ, const float* dU, float* grad,
                                  cudaStream_t st, int64_t* launches) {
-  return SYNAX_ERR_UNSUPPORTED;
+  VjpArgs a;
+  a.geo = geo; a.bc = bc; a.batch = batch; a.n_freq_total = ft.n_freq;
+  a.dI = dI; a.dQ = dQ; a.dU = dU;
+  a.n_blocks = (int)((geo.npix * G + kBlock - 1) / kBlock);
+  if (batch > 65535) return SYNAX_ERR_UNSUPPORTED;
+  float* partial = nullptr;
+  if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
+    return SYNAX_ERR_ALLOC;
+  a.partial = partial;
+  const dim3 grid((unsigned)a.n_blocks, (unsigned)batch);
+  for (int f0 = 0; f0 < ft.n_freq;) {
+    const int rem = ft.n_freq - f0;
+    const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
+    a.f0 = f0; a.accumulate = f0 > 0;
+    if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc>(G, nf, grid, st, a, ft);
+    else if (code == kAnalyticFull) launch_vjp<kAnalyticFull>(G, nf, grid, st, a, ft);
+    else launch_vjp<kUniform>(G, nf, grid, st, a, ft);
+    ++*launches;
+    f0 += nf;
+  }
+  vjp_reduce_kernel<<<batch, 256, 0, st>>>(partial, a.n_blocks, n_params, grad);
+  ++*launches;
+  const cudaError_t e = cudaGetLastError();
+  cudaFreeAsync(partial, st);
+  return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 
 }  // namespace synax
