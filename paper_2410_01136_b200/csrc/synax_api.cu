@@ -279,7 +279,8 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
 
   if (code == kGridB) {
-    synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, st, &plan->launches);
+    synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, sm_count(plan->device),
+                                   plan->d_flag_count, plan->h_flag_count, st, &plan->launches);
     cudaFreeAsync(bc, st);
     if (gs != SYNAX_OK) return fail(gs, "grid forward failed: %s", cudaGetErrorString(cudaGetLastError()));
     return SYNAX_OK;
@@ -345,7 +346,8 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   plan->launches++;
   synax_status rs;
   if (code == kGridB)
-    rs = grid_vjp(plan->ft, make_geo(plan), bc, model, params, dI, dQ, dU, grad, st, &plan->launches);
+    rs = grid_vjp(plan->ft, make_geo(plan), bc, model, params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
+                  sm_count(plan->device), st, &plan->launches);
   else
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       dI, dQ, dU, grad, st, &plan->launches);

@@ -1,18 +1,521 @@
-// synax_grid.cuh -- gridded-B forward (A3') and adjoint with scatter-add (A11').
+// synax_grid.cuh -- gridded-B model (cfg 3): forward with trilinear gathers (A3') and the adjoint with
+// scatter-add into the grid gradient (A11').  One warp per sightline.
+//   forward / adjoint sweep 1: lanes take CONSECUTIVE samples (neighbouring lanes read neighbouring
+//     cells -> gathers coalesce), Faraday depth by a warp inclusive scan per 32-sample tile plus a
+//     float64 carry;
+//   adjoint sweep 2: lanes take CONTIGUOUS chunks, so a lane stays in one cell for several samples and
+//     accumulates its 8x3 corner contributions in registers, flushing with red.global.add only when
+//     the cell changes.  Per-sample cotangents travel from sweep 1 to sweep 2 through shared memory.
 #pragma once
-#include "synax_forward.cuh"
 #include "../../include/synax.h"
+#include "synax_forward.cuh"
 
 namespace synax {
 
-static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a, const synax_model* m, const float* grid,
-                                 int precision, double escalate_rad, cudaStream_t st, int64_t* launches) {
-  return SYNAX_ERR_UNSUPPORTED;
+struct GridDesc {
+  const float* g;       // [nx][ny][nz][3]
+  int nx, ny, nz;
+  double sx, sy, sz;    // (n-1)/l
+  double bx, by, bz;    // (n-1)/2
+};
+
+struct Cell {
+  int base;             // float index of corner (i,j,k), component 0
+  float tx, ty, tz;
+  bool inbox;
+};
+
+__device__ __forceinline__ Cell locate(const GridDesc& G, double x, double y, double z) {
+  const double ux = fma(x, G.sx, G.bx), uy = fma(y, G.sy, G.by), uz = fma(z, G.sz, G.bz);
+  Cell c;
+  c.inbox = (ux >= 0.0) && (ux <= (double)(G.nx - 1)) && (uy >= 0.0) && (uy <= (double)(G.ny - 1)) &&
+            (uz >= 0.0) && (uz <= (double)(G.nz - 1));
+  int i = __double2int_rd(ux), j = __double2int_rd(uy), k = __double2int_rd(uz);
+  i = max(0, min(i, G.nx - 2)); j = max(0, min(j, G.ny - 2)); k = max(0, min(k, G.nz - 2));
+  c.tx = (float)(ux - (double)i); c.ty = (float)(uy - (double)j); c.tz = (float)(uz - (double)k);
+  c.base = ((i * G.ny + j) * G.nz + k) * 3;
+  return c;
 }
+
+// trilinear weights in the order (a,b,d) = (0,0,0),(0,0,1),(0,1,0),(0,1,1),(1,0,0),...
+__device__ __forceinline__ void weights(const Cell& c, float w[8]) {
+  const float x0 = 1.0f - c.tx, y0 = 1.0f - c.ty, z0 = 1.0f - c.tz;
+  const float a00 = x0 * y0, a01 = x0 * c.ty, a10 = c.tx * y0, a11 = c.tx * c.ty;
+  w[0] = a00 * z0; w[1] = a00 * c.tz; w[2] = a01 * z0; w[3] = a01 * c.tz;
+  w[4] = a10 * z0; w[5] = a10 * c.tz; w[6] = a11 * z0; w[7] = a11 * c.tz;
+}
+
+__device__ __forceinline__ int corner_offset(const GridDesc& G, int q) {  // q = a*4 + b*2 + d
+  return (((q >> 2) * G.ny + ((q >> 1) & 1)) * G.nz + (q & 1)) * 3;
+}
+
+__device__ __forceinline__ void gather_B(const GridDesc& G, const Cell& c, float B[3]) {
+  float w[8];
+  weights(c, w);
+  B[0] = B[1] = B[2] = 0.f;
+  if (!c.inbox) return;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const float* p = G.g + c.base + corner_offset(G, q);
+    B[0] = fmaf(w[q], __ldg(p), B[0]);
+    B[1] = fmaf(w[q], __ldg(p + 1), B[1]);
+    B[2] = fmaf(w[q], __ldg(p + 2), B[2]);
+  }
+}
+
+// CR and thermal-electron exponential discs from aux (fp32 chain), Eq.(12)
+__device__ __forceinline__ void densities_f32(const BatchConsts& P, float rho2, float z, float& N0, float& ne) {
+  const float rho = rho2 * mufu_rsqrt(fmaxf(rho2, 1e-30f));
+  const float az = fabsf(z);
+  const float ez = mufu_ex2(P.k_hz * az), dz = 1.0f + ez;
+  N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
+  const float ee = mufu_ex2(P.k_hez * az), de = 1.0f + ee;
+  ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * rho) * ee * mufu_rcp(de * de);
+}
+
+__device__ __forceinline__ float warp_inclusive_scan(float v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const float o = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += o;
+  }
+  return v;
+}
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_xor_sync(0xffffffffu, lo, d); hi = __shfl_xor_sync(0xffffffffu, hi, d);
+    v += __hiloint2double(hi, lo);
+  }
+  return v;
+}
+
+// sin/cos of the Faraday angle k_turn * S for a float64 S (turn reduction in float64)
+__device__ __forceinline__ void faraday_sincos(double k_turn, double S, float& c, float& s) {
+  double t = k_turn * S;
+  t -= rint(t);
+  const float a = (float)t * 6.283185307179586f;
+  c = mufu_cos(a); s = mufu_sin(a);
+}
+
+// float64 chain for one sample: coordinates, trilinear weights, interpolation, densities, projections
+__device__ __forceinline__ void fields_f64(const GridDesc& G, const BatchConsts& P, const double4 dir, double xd,
+                                           double yd, double zd, double& Bpar, double& BN, double& BE, double& N0,
+                                           double& ne) {
+  const double ux = fma(xd, G.sx, G.bx), uy = fma(yd, G.sy, G.by), uz = fma(zd, G.sz, G.bz);
+  const bool inbox = (ux >= 0.0) && (ux <= (double)(G.nx - 1)) && (uy >= 0.0) && (uy <= (double)(G.ny - 1)) &&
+                     (uz >= 0.0) && (uz <= (double)(G.nz - 1));
+  int i = __double2int_rd(ux), j = __double2int_rd(uy), k = __double2int_rd(uz);
+  i = max(0, min(i, G.nx - 2)); j = max(0, min(j, G.ny - 2)); k = max(0, min(k, G.nz - 2));
+  const double tx = ux - (double)i, ty = uy - (double)j, tz = uz - (double)k;
+  double B[3] = {0.0, 0.0, 0.0};
+  if (inbox) {
+    const int base = ((i * G.ny + j) * G.nz + k) * 3;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const double w = ((q & 4) ? tx : 1.0 - tx) * ((q & 2) ? ty : 1.0 - ty) * ((q & 1) ? tz : 1.0 - tz);
+      const float* p = G.g + base + corner_offset(G, q);
+      B[0] += w * (double)__ldg(p); B[1] += w * (double)__ldg(p + 1); B[2] += w * (double)__ldg(p + 2);
+    }
+  }
+  const double rho = sqrt(fma(xd, xd, yd * yd));
+  const double chz = cosh(zd / (double)P.p[11]), che = cosh(zd / (double)P.p[15]);
+  N0 = (double)P.p[9] * exp(-rho / (double)P.p[10]) / (chz * chz);
+  ne = (double)P.p[13] * exp(-rho / (double)P.p[14]) / (che * che);
+  Bpar = B[0] * (dir.z * dir.x) + B[1] * (dir.z * dir.y) + B[2] * dir.w;
+  BN = B[2] * dir.z - dir.w * (B[0] * dir.x + B[1] * dir.y);
+  BE = B[1] * dir.x - B[0] * dir.y;
+}
+
+__device__ __forceinline__ double warp_inclusive_scan_d(double v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const double o = shfl_up_d(v, d, 32);
+    if (lane >= d) v += o;
+  }
+  return v;
+}
+__device__ __forceinline__ double warp_bcast_d(double v, int src) {
+  int lo = __double2loint(v), hi = __double2hiint(v);
+  lo = __shfl_sync(0xffffffffu, lo, src); hi = __shfl_sync(0xffffffffu, hi, src);
+  return __hiloint2double(hi, lo);
+}
+
+struct GridFwdArgs {
+  ForwardArgs f;
+  GridDesc grid;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Forward.  PRECISE = float64 trilinear weights / densities / scan for flagged sightlines.
+// Persistent warps striding over sightlines (or over the flag list).
+// ------------------------------------------------------------------------------------------------
+template <int NF, bool PRECISE>
+__global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_constant__ GridFwdArgs GA,
+                                                              const __grid_constant__ FreqTab ft) {
+  const ForwardArgs& A = GA.f;
+  const GridDesc& G = GA.grid;
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
+  const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
+  const int64_t count = (PRECISE && A.flag_list) ? (int64_t)(*A.flag_count) : A.geo.npix;
+  const BatchConsts& P = A.bc[0];
+  const double delta = A.geo.delta;
+  for (int64_t it = warp; it < count; it += n_warps) {
+    const int64_t pix = (PRECISE && A.flag_list) ? (int64_t)A.flag_list[it] : it;
+    const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
+    const Triad T = load_triad(A.geo.dirs, pix);
+    float accI = 0.f, accQ[NF], accU[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { accQ[f] = 0.f; accU[f] = 0.f; }
+    double carry = 0.0;
+    float absS = 0.f;
+    for (int nt = 0; nt < A.geo.n_los; nt += 32) {
+      const int n = nt + lane;
+      const bool active = n < A.geo.n_los;
+      const double s_d = ((double)n + 0.5) * delta;
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      float eI = 0.f, a = 0.f, bq = 0.f;
+      double S_here;  // sum_{m<n} g_m + g_n/2 relative to the start of the sightline
+      if (!PRECISE) {
+        const Cell c = locate(G, xd, yd, zd);
+        float B[3];
+        gather_B(G, c, B);
+        float N0, ne;
+        densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+        const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
+        const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
+        const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
+        if (active) emission(P, BN, BE, N0, eI, a, bq);
+        const float gn = active ? ne * Bpar : 0.f;
+        const float incl = warp_inclusive_scan(gn, lane);
+        S_here = carry + (double)(incl - 0.5f * gn);
+        carry += warp_sum_d((double)gn);
+      } else {
+        double Bpar, BN, BE, N0, ne;
+        fields_f64(G, P, dir, xd, yd, zd, Bpar, BN, BE, N0, ne);
+        if (active) emission(P, (float)BN, (float)BE, (float)N0, eI, a, bq);
+        const double gn = active ? ne * Bpar : 0.0;
+        const double incl = warp_inclusive_scan_d(gn, lane);
+        S_here = carry + incl - 0.5 * gn;
+        carry += warp_bcast_d(incl, 31);
+      }
+      absS = fmaxf(absS, fabsf((float)carry));
+      accI += eI;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        float c, s;
+        faraday_sincos(ft.k_turn[A.f0 + f], S_here, c, s);
+        accQ[f] = fmaf(a, c, fmaf(-bq, s, accQ[f]));
+        accU[f] = fmaf(a, s, fmaf(bq, c, accU[f]));
+      }
+    }
+    accI = group_sum<32>(accI);
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { accQ[f] = group_sum<32>(accQ[f]); accU[f] = group_sum<32>(accU[f]); }
+    if (lane == 0) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const int64_t o = (int64_t)(A.f0 + f) * A.geo.npix + pix;
+        A.I[o] = P.coefI[A.f0 + f] * accI;
+        A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
+        A.U[o] = P.coefP[A.f0 + f] * accU[f];
+      }
+      if (!PRECISE && A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
+        const int k = atomicAdd(A.flag_count, 1);
+        A.flag_list[k] = (int)pix;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Adjoint.  grad_grid must be zero on entry (the host wrapper clears it).
+// Dynamic shared memory: 4 float arrays of 32*(C+1) per warp, C = chunk length (power of two).
+// ------------------------------------------------------------------------------------------------
+struct GridVjpArgs {
+  Geometry geo;
+  const BatchConsts* bc;
+  GridDesc grid;
+  int f0, n_freq_total;
+  const float* dI; const float* dQ; const float* dU;
+  float* grad;          // [nx][ny][nz][3]
+  int chunk_log2;       // C = 1 << chunk_log2, 32*C >= n_los
+  int mode;             // 0 auto, 1 fp32 chain, 2 float64 Faraday chain
+  float flag_S;         // auto: redo a sightline in float64 when max |sum n_e B_LOS| exceeds this
+};
+
+// Sweep 1 of the gridded adjoint for one sightline (whole warp): per-sample forward quantities, cotangent
+// fan-out (A9) and the per-sample hand-over to sweep 2 through shared memory.  Returns max |sum n_e B_LOS|.
+template <int NF, bool PRECISE>
+__device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const FreqTab& ft, const GridDesc& G,
+                                                 const BatchConsts& P, const Triad& T, const double4 dir, int lane,
+                                                 float cI, const float (&cQ)[NF], const float (&cU)[NF],
+                                                 const float (&kr)[NF], float* st_w, float* st_n, float* st_e,
+                                                 float* st_d) {
+  const int C = 1 << A.chunk_log2, Cp = C + 1;
+  const double delta = A.geo.delta;
+  double carry = 0.0;
+  float absS = 0.f;
+  for (int nt = 0; nt < A.geo.n_los; nt += 32) {
+    const int n = nt + lane;
+    const bool active = n < A.geo.n_los;
+    const double s_d = ((double)n + 0.5) * delta;
+    const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+    const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+    const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+    float BN, BE, N0, ne;
+    double S_here;
+    if (!PRECISE) {
+      const Cell c = locate(G, xd, yd, zd);
+      float B[3];
+      gather_B(G, c, B);
+      densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
+      BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
+      BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
+      const float gn = active ? ne * Bpar : 0.f;
+      const float incl = warp_inclusive_scan(gn, lane);
+      S_here = carry + (double)(incl - 0.5f * gn);
+      carry += warp_sum_d((double)gn);
+    } else {
+      double Bpar, BNd, BEd, N0d, ned;
+      fields_f64(G, P, dir, xd, yd, zd, Bpar, BNd, BEd, N0d, ned);
+      BN = (float)BNd; BE = (float)BEd; N0 = (float)N0d; ne = (float)ned;
+      const double gn = active ? ned * Bpar : 0.0;
+      const double incl = warp_inclusive_scan_d(gn, lane);
+      S_here = carry + incl - 0.5 * gn;
+      carry += warp_bcast_d(incl, 31);
+    }
+    absS = fmaxf(absS, fabsf((float)carry));
+    const float bn2 = BN * BN, be2 = BE * BE, Bt2 = bn2 + be2;
+    float w = 1.0f;
+    if (!P.alpha_is_3) w = (Bt2 > 0.f) ? mufu_ex2(P.q_exp * mufu_lg2(Bt2)) : 0.f;
+    const float M = active ? w * N0 : 0.f;
+    const float d2 = be2 - bn2, p2 = 2.0f * BE * BN;
+    float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      float cc, ss;
+      faraday_sincos(ft.k_turn[A.f0 + f], S_here, cc, ss);
+      const float u = fmaf(cQ[f], cc, cU[f] * ss);
+      const float v = fmaf(cU[f], cc, -cQ[f] * ss);
+      Xc += u; Xs += v;
+      Yc = fmaf(kr[f], u, Yc); Ys = fmaf(kr[f], v, Ys);
+    }
+    const float K = fmaf(cI, Bt2, fmaf(Xc, d2, Xs * p2));
+    const float MK = M * K;
+    const float Sbar = M * fmaf(d2, Ys, -p2 * Yc);   // cotangent of this sample's Faraday sum
+    const float tq_ = (Bt2 > 0.f) ? P.q_exp * MK / Bt2 : 0.f;
+    const float BEb = 2.0f * fmaf(M, fmaf(BE, cI + Xc, BN * Xs), BE * tq_);
+    const float BNb = 2.0f * fmaf(M, fmaf(BN, cI - Xc, BE * Xs), BN * tq_);
+    if (active) {
+      const int idx = (n >> A.chunk_log2) * Cp + (n & (C - 1));
+      st_w[idx] = Sbar; st_n[idx] = BNb; st_e[idx] = BEb; st_d[idx] = ne;
+    }
+  }
+  return absS;
+}
+
+template <int NF>
+__global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant__ GridVjpArgs A,
+                                                          const __grid_constant__ FreqTab ft) {
+  extern __shared__ float smem[];
+  const GridDesc& G = A.grid;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int C = 1 << A.chunk_log2, Cp = C + 1;
+  float* st_w = smem + (size_t)wid * 4 * 32 * Cp;   // Sbar_m: cotangent of the Faraday sum at sample m
+  float* st_n = st_w + 32 * Cp;                     // BbarN (direct)
+  float* st_e = st_n + 32 * Cp;                     // BbarE (direct)
+  float* st_d = st_e + 32 * Cp;                     // n_e
+  const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
+  const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
+  const BatchConsts& P = A.bc[0];
+  const double delta = A.geo.delta;
+  for (int64_t pix = warp; pix < A.geo.npix; pix += n_warps) {
+    const Triad T = load_triad(A.geo.dirs, pix);
+    const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
+    float cI = 0.f, cQ[NF], cU[NF], kr[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int64_t o = (int64_t)(A.f0 + f) * A.geo.npix + pix;
+      cI = fmaf(A.dI ? __ldg(A.dI + o) : 0.f, P.coefI[A.f0 + f], cI);
+      cQ[f] = (A.dQ ? __ldg(A.dQ + o) : 0.f) * P.coefP[A.f0 + f];
+      cU[f] = (A.dU ? __ldg(A.dU + o) : 0.f) * P.coefP[A.f0 + f];
+      kr[f] = ft.k_rad[A.f0 + f];
+    }
+    // ---- sweep 1: consecutive samples per lane; fp32 chain first, redone with the float64 Faraday chain
+    // when the rotation angle of this sightline is large (warp-uniform decision)
+    float absS = 0.f;
+    if (A.mode != 2) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
+    if (A.mode == 2 || (A.mode == 0 && absS > A.flag_S)) {
+      __syncwarp();
+      grid_vjp_sweep1<NF, true>(A, ft, G, P, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
+    }
+    __syncwarp();
+    // ---- sweep 2: contiguous chunk per lane walked BACKWARDS, so that the suffix sum of Sbar that the
+    // transposed half-cell scan needs (gbar_m = sum_{n>m} Sbar_n + Sbar_m / 2) is a running sum with no
+    // cancellation; register accumulation per cell, red.global.add only when the cell changes.
+    const int m0 = lane << A.chunk_log2;
+    const int m1 = min(m0 + C, A.geo.n_los);
+    float tot = 0.f;
+    for (int m = m0; m < m1; ++m) tot += st_w[lane * Cp + (m - m0)];
+    float incl = tot;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const float o = __shfl_down_sync(0xffffffffu, incl, d);
+      if (lane + d < 32) incl += o;
+    }
+    float suf = incl - tot;      // sum of Sbar over all later lanes
+    float acc[24];
+#pragma unroll
+    for (int q = 0; q < 24; ++q) acc[q] = 0.f;
+    int cur = -1;
+    for (int m = m1 - 1; m >= m0 - 1; --m) {
+      Cell c; c.base = -1; c.inbox = false; c.tx = c.ty = c.tz = 0.f;
+      if (m >= m0) {
+        const double s_d = ((double)m + 0.5) * delta;
+        c = locate(G, fma(s_d, T.nxd, A.geo.obs[0]), fma(s_d, T.nyd, A.geo.obs[1]), fma(s_d, T.nzd, A.geo.obs[2]));
+      }
+      const int cell = (m >= m0 && c.inbox) ? c.base : -1;
+      if (cell != cur) {
+        if (cur >= 0) {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            float* p = A.grad + cur + corner_offset(G, q);
+            atomicAdd(p, acc[3 * q]); atomicAdd(p + 1, acc[3 * q + 1]); atomicAdd(p + 2, acc[3 * q + 2]);
+            acc[3 * q] = 0.f; acc[3 * q + 1] = 0.f; acc[3 * q + 2] = 0.f;
+          }
+        }
+        cur = cell;
+      }
+      if (m >= m0) {
+        const int idx = lane * Cp + (m - m0);
+        const float Sb = st_w[idx];
+        const float gbar = fmaf(0.5f, Sb, suf);
+        suf += Sb;
+        if (cell >= 0) {
+          const float BNb = st_n[idx], BEb = st_e[idx], gn = gbar * st_d[idx];
+          const float bx = fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, gn * T.nx));
+          const float by = fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, gn * T.ny));
+          const float bz = fmaf(BNb, T.eNz, gn * T.nz);
+          float w[8];
+          weights(c, w);
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            acc[3 * q] = fmaf(w[q], bx, acc[3 * q]);
+            acc[3 * q + 1] = fmaf(w[q], by, acc[3 * q + 1]);
+            acc[3 * q + 2] = fmaf(w[q], bz, acc[3 * q + 2]);
+          }
+        }
+      }
+    }
+    __syncwarp();
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-side dispatch
+// ------------------------------------------------------------------------------------------------
+static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
+  GridDesc g;
+  g.g = grid; g.nx = m->nx; g.ny = m->ny; g.nz = m->nz;
+  g.sx = (double)(m->nx - 1) / (double)m->lx; g.sy = (double)(m->ny - 1) / (double)m->ly; g.sz = (double)(m->nz - 1) / (double)m->lz;
+  g.bx = 0.5 * (double)(m->nx - 1); g.by = 0.5 * (double)(m->ny - 1); g.bz = 0.5 * (double)(m->nz - 1);
+  return g;
+}
+
+template <bool PRECISE>
+static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft) {
+  switch (nf) {
+    case 1: grid_forward_kernel<1, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 2: grid_forward_kernel<2, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 3: grid_forward_kernel<3, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 4: grid_forward_kernel<4, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    default: grid_forward_kernel<8, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
+  }
+}
+
+static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_model* m, const float* grid,
+                                 int precision, double escalate_rad, int sms, int* d_flag_count, int* h_flag_count,
+                                 cudaStream_t st, int64_t* launches) {
+  GridFwdArgs ga;
+  ga.f = a0; ga.grid = make_grid_desc(m, grid);
+  float k_max = 0.f;
+  for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
+  const bool fast = precision != 2, escalate = precision == 0;
+  ga.f.flag_list = nullptr; ga.f.flag_S = 0.f; ga.f.flag_count = d_flag_count;
+  if (escalate) {
+    if (cudaMallocAsync((void**)&ga.f.flag_list, sizeof(int) * (size_t)a0.geo.npix, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
+    cudaMemsetAsync(d_flag_count, 0, sizeof(int), st);
+    ga.f.flag_S = (float)(escalate_rad / (double)k_max);
+  }
+  const int64_t warps_needed = a0.geo.npix;
+  const unsigned max_blocks = (unsigned)(sms * 16);
+  const unsigned blocks = (unsigned)min((int64_t)max_blocks, (warps_needed * 32 + kBlock - 1) / kBlock);
+  for (int f0 = 0; f0 < ft.n_freq;) {
+    const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
+    ga.f.f0 = f0;
+    if (fast) { launch_grid_forward<false>(nf, blocks, st, ga, ft); ++*launches; }
+    f0 += nf;
+  }
+  if (!fast || escalate) {
+    GridFwdArgs pa = ga;
+    if (!fast) pa.f.flag_list = nullptr;
+    for (int f0 = 0; f0 < ft.n_freq;) {
+      const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
+      pa.f.f0 = f0;
+      launch_grid_forward<true>(nf, blocks, st, pa, ft); ++*launches;
+      f0 += nf;
+    }
+  }
+  const cudaError_t e = cudaGetLastError();
+  if (escalate) {
+    cudaMemcpyAsync(h_flag_count, d_flag_count, sizeof(int), cudaMemcpyDeviceToHost, st);
+    cudaFreeAsync(ga.f.flag_list, st);
+  }
+  return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
+}
+
 static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const synax_model* m,
                              const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
-                             cudaStream_t st, int64_t* launches) {
-  return SYNAX_ERR_UNSUPPORTED;
+                             int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches) {
+  GridVjpArgs a;
+  a.geo = geo; a.bc = bc; a.grid = make_grid_desc(m, grid);
+  a.n_freq_total = ft.n_freq; a.dI = dI; a.dQ = dQ; a.dU = dU; a.grad = grad;
+  int cl = 0;
+  while ((32 << cl) < geo.n_los) ++cl;
+  a.chunk_log2 = cl;
+  float k_max = 0.f;
+  for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
+  a.mode = precision; a.flag_S = (float)(escalate_rad / (double)k_max);
+  const size_t smem = (size_t)(kBlock / 32) * 4 * 32 * ((1u << cl) + 1) * sizeof(float);
+  if (smem > 200 * 1024) return SYNAX_ERR_UNSUPPORTED;  // n_los too large for the shared-memory hand-over
+  if (cudaMemsetAsync(grad, 0, sizeof(float) * (size_t)m->n_params, st) != cudaSuccess) return SYNAX_ERR_CUDA;
+  const unsigned blocks = (unsigned)min((int64_t)sms * 8, (geo.npix * 32 + kBlock - 1) / kBlock);
+  for (int f0 = 0; f0 < ft.n_freq;) {
+    const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
+    a.f0 = f0;
+#define SYNAX_GV(NFV)                                                                                      \
+  do {                                                                                                     \
+    cudaFuncSetAttribute(grid_vjp_kernel<NFV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
+    grid_vjp_kernel<NFV><<<blocks, kBlock, smem, st>>>(a, ft);                                             \
+  } while (0)
+    switch (nf) {
+      case 1: SYNAX_GV(1); break;
+      case 2: SYNAX_GV(2); break;
+      case 3: SYNAX_GV(3); break;
+      case 4: SYNAX_GV(4); break;
+      default: SYNAX_GV(8); break;
+    }
+#undef SYNAX_GV
+    ++*launches;
+    f0 += nf;
+  }
+  return cudaGetLastError() == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 
 }  // namespace synax
