@@ -1,0 +1,366 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the synax hot path (forward + VJP) on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: synax_forward followed by
+synax_vjp on the same stream (BASELINE.json metric "LoS samples/s (fwd,
+fwd+VJP) at nside=256 x 1024 pts").  Default workload = BASELINE.json configs[4] (nside=256, 1024 samples,
+8 frequencies, 16-parameter model).  LoS samples = npix * n_los * batch per call (frequencies not
+multiplied in).  `value` = samples / (forward + VJP time), inputs resident in HBM.  `e2e` = the same
+through synax_forward_host / synax_vjp_host with pinned HOST buffers (copies inside the timed region).
+
+N > 1 (torchrun, one rank per GPU): weak scaling -- every rank integrates the full sky for its own
+parameter vector (independent HMC chains); no data-path collective.
+
+--impl reference: the float64 CPU oracle (oracle/), as it stands, on the host cores, on a bounded pixel
+subset of the same workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "LoS samples/s (fwd+VJP)"
+UNIT = "samples/s"
+
+# Algorithmic FP32 lane-instructions per LoS sample (DESIGN.md section 7 / SURVEY.md 8(d) table), fixed
+# before tuning: shared part + per-frequency part, forward and VJP (VJP = recompute + adjoint).
+ALG_FP = {
+    "disc4":  dict(fwd=(70, 12), vjp=(70 + 90, 12 + 14)),
+    "full16": dict(fwd=(85, 12), vjp=(85 + 125, 12 + 14)),
+    "grid_b": dict(fwd=(120, 12), vjp=(120 + 60, 12 + 14)),
+    "uniform": dict(fwd=(30, 12), vjp=(60, 26)),
+}
+ALG_MUFU = {"disc4": (14, 2), "full16": (19, 2), "grid_b": (10, 2), "uniform": (0, 2)}
+SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16
+
+
+def alg_fp(kind, n_freq, which):
+    s, f = ALG_FP[kind][which]
+    return s + f * n_freq
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return float(d.get("sm_max_mhz", 1965.0)), "MEASURED_PEAKS.json sm_max_mhz"
+    return 1965.0, "fallback 1965 MHz (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi -lms sampling of SM clock and throttle reasons during the timed region."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, reasons, mx, pw = [], set(), None, []
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        try:
+            for line in Path(self.path).read_text().splitlines():
+                c = [x.strip() for x in line.split(",")]
+                if len(c) < 7:
+                    continue
+                try:
+                    sm.append(float(c[0])); mx = float(c[1]); pw.append(float(c[2]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, c[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=mx, reasons=sorted(reasons), samples=len(sm),
+                       sm_mhz_min=float(min(sm)), power_w_max=float(max(pw)) if pw else None)
+        return out
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def rank_workload(cfg, rank):
+    """Weak scaling: rank r > 0 takes the config's model with its own parameter vector(s) (an independent
+    chain): each analytic parameter scaled by (1 + 0.05 u), u ~ U[-1,1] from seed 7000 + r.  Rank 0 is the
+    config as BASELINE.json states it."""
+    from paper_2410_01136_b200 import workloads as wl
+    w = wl.config(cfg)
+    if rank > 0 and w.kind != "grid_b":
+        rng = np.random.Generator(np.random.PCG64(7000 + rank))
+        w.params = np.ascontiguousarray((w.params.astype(np.float64) * (1.0 + 0.05 * rng.uniform(-1, 1, w.params.shape))).astype(np.float32))
+    elif rank > 0:
+        rng = np.random.Generator(np.random.PCG64(7000 + rank))
+        w.params = np.ascontiguousarray((w.params.astype(np.float64) * (1.0 + 0.05 * rng.uniform(-1, 1))).astype(np.float32))
+    return w
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline of the default run, and --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_pixels(w, target_samples):
+    """Bounded sample of the workload: pixels p = 0 (mod stride), stride chosen so that the sample holds about
+    `target_samples` LoS samples (all batch elements, all frequencies, all n_los points of those pixels)."""
+    per_pix = w.n_los * w.batch
+    want = max(1, int(target_samples // per_pix))
+    stride = max(1, w.npix // want)
+    return np.arange(0, w.npix, stride, dtype=np.int64), stride
+
+
+def oracle_step(w, pix, cots_sub):
+    """One forward + VJP of the oracle over the pixel subset; returns seconds."""
+    sys.path.insert(0, str(ROOT / "tests"))
+    import parity
+    t = time.perf_counter()
+    parity.oracle_forward(w, pix=pix)
+    t1 = time.perf_counter()
+    parity.oracle_vjp(w, cots_sub, pix=pix)
+    t2 = time.perf_counter()
+    return t1 - t, t2 - t1
+
+
+def oracle_baseline(w, seconds_budget=15.0, steps=1, warmup=0):
+    import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    # ~7 us per sample per core for FULL16 at 8 frequencies forward+VJP (measured on the build box): size the
+    # sample so one step is about `seconds_budget` of wall time on this host
+    per_sample_core = 1.2e-6 * (1.0 + 0.6 * w.n_freq)
+    target = seconds_budget * cores / per_sample_core
+    pix, stride = oracle_sample_pixels(w, min(target, w.los_samples))
+    cots = w.cotangents()
+    cots_sub = tuple(np.ascontiguousarray(c[..., pix]) for c in cots)
+    n_samples = pix.size * w.n_los * w.batch
+    for _ in range(warmup):
+        oracle_step(w, pix, cots_sub)
+    tf = tv = 0.0
+    for _ in range(steps):
+        a, b = oracle_step(w, pix, cots_sub)
+        tf += a; tv += b
+    tf /= steps; tv /= steps
+    return dict(value=n_samples / (tf + tv), unit=UNIT, cores=cores, kind="oracle",
+                sample=f"pixels p = 0 (mod {stride}) of {w.name}: {pix.size} sightlines x {w.n_los} samples x batch {w.batch} "
+                       f"= {n_samples} LoS samples per step, forward + VJP, float64, OpenMP over sightlines",
+                forward_samples_per_s=n_samples / tf, ms_per_step=1e3 * (tf + tv), samples_per_step=int(n_samples))
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    from paper_2410_01136_b200 import workloads as wl
+    w = wl.config(args.config)
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    # keep the whole run within a few minutes: total oracle time ~ 120 s split over steps + warm-ups
+    budget = min(15.0, 120.0 / (steps + warmup))
+    cb = oracle_baseline(w, seconds_budget=budget, steps=steps, warmup=warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": warmup, "ms_per_step": cb["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, workloads.py)",
+            "config": {"workload": w.name, "nside": w.nside, "n_los": w.n_los, "n_freq": w.n_freq, "batch": w.batch,
+                       "model": w.kind, "sample": cb["sample"]},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "forward_samples_per_s": cb["forward_samples_per_s"]}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True):
+    """Device-resident timing of forward and VJP with CUDA events on the launching stream, L2 flushed between
+    timed calls; then (optionally) the host-buffer entry points."""
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer)
+    if w.kind == "grid_b":
+        model = sx.Model("grid_b", aux=w.aux, grid_shape=w.params.shape[:3], box=w.box)
+    else:
+        model = sx.Model(w.kind, aux=w.aux)
+    params = torch.from_numpy(w.params).cuda().contiguous()
+    cots_h = w.cotangents()
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    out = tuple(torch.empty((w.batch, w.n_freq, w.npix), dtype=torch.float32, device="cuda") for _ in range(3))
+    grad = torch.empty_like(params)
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        if ev: ev[0].record(stream)
+        sx.forward(plan, model, params, out=out)
+        if ev: ev[1].record(stream)
+        sx.vjp(plan, model, params, *cots, out=grad)
+        if ev: ev[2].record(stream)
+
+    for _ in range(warmup):
+        step()
+        flush_buf.add_(1.0)
+    torch.cuda.synchronize()
+    l0 = plan.stats()["launches"]
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    for k in range(steps):
+        step(evs[k])
+        flush_buf.add_(1.0)          # > L2 (126 MB): every timed step starts with a cold L2
+    torch.cuda.synchronize()
+    l1 = plan.stats()["launches"]
+    tf = np.array([e[0].elapsed_time(e[1]) for e in evs]) * 1e-3
+    tv = np.array([e[1].elapsed_time(e[2]) for e in evs]) * 1e-3
+    res = dict(t_fwd=float(tf.mean()), t_vjp=float(tv.mean()), t_fwd_min=float(tf.min()), t_vjp_min=float(tv.min()),
+               launches=int(l1 - l0), escalated=plan.stats()["escalated"])
+    if want_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
+        hp = pin(w.params); hc = [pin(c) for c in cots_h]
+        ho = tuple(torch.empty((w.batch, w.n_freq, w.npix), dtype=torch.float32).pin_memory() for _ in range(3))
+        hg = torch.empty(w.params.shape, dtype=torch.float32).pin_memory()
+        npv = lambda t: t.numpy()  # noqa: E731
+
+        def host_step():
+            sx.forward_host(plan, model, npv(hp), out=tuple(npv(t) for t in ho))
+            sx.vjp_host(plan, model, npv(hp), *[npv(c) for c in hc], out=npv(hg))
+
+        n_e2e = max(3, min(steps, 10))
+        for _ in range(2):
+            host_step()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            host_step()            # each *_host call synchronises its stream before returning
+        torch.cuda.synchronize()
+        res["t_e2e"] = (time.perf_counter() - t0) / n_e2e
+        res["h2d"] = int(2 * hp.numel() * 4 + sum(c.numel() for c in hc) * 4)
+        res["d2h"] = int(sum(t.numel() for t in ho) * 4 + hg.numel() * 4)
+    plan.close()
+    return res
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the synax hot path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", torch.cuda.current_device()))
+    import paper_2410_01136_b200 as sx
+    sx.load_library()                       # fails loudly when libsynax.so is missing
+    w = rank_workload(args.config, rank)
+    flush_buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # untimed first touch (context, module load)
+    time_config(sx, torch, w, 1, 1, flush_buf, want_e2e=False)
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device())
+    if rank == 0:
+        sampler.start()
+    barrier()
+    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    e = time_config(sx, torch, w, min(args.steps, 5), 1, flush_buf, want_e2e=True)
+    t_step = r["t_fwd"] + r["t_vjp"]
+    vals = torch.tensor([t_step, r["t_fwd"], r["t_vjp"], e["t_e2e"]], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+    t_step, t_fwd, t_vjp, t_e2e = (float(v) for v in vals.cpu())
+    samples = w.los_samples
+    line = None
+    if rank == 0:
+        sm_max, peak_src = peaks()
+        peak = SM_COUNT * FP32_LANES * sm_max * 1e6 / 1e12       # T lane-instr/s
+        fp_vjp = alg_fp(w.kind, w.n_freq, "vjp")
+        fp_fwd = alg_fp(w.kind, w.n_freq, "fwd")
+        achieved = fp_vjp * samples / r["t_vjp"] / 1e12
+        line = {
+            "metric": METRIC, "value": world * samples / t_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, workloads.py)",
+            "config": {"workload": w.name, "nside": w.nside, "n_los": w.n_los, "n_freq": w.n_freq, "batch": w.batch,
+                       "model": w.kind, "samples_per_step": samples, "l2": "flushed between timed steps (256 MB write)",
+                       "parallelism": f"independent parameter vectors x{world}" if world > 1 else "single GPU"},
+            "forward_samples_per_s": world * samples / t_fwd, "vjp_samples_per_s": world * samples / t_vjp,
+            "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,
+            "sample_freq_per_s": world * samples * w.n_freq / t_step,
+            "e2e": {"value": world * samples / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
+                    "ms_per_step": 1e3 * t_e2e},
+            "gpu_launches": r["launches"], "escalated_sightlines": r["escalated"],
+            "clocks": clocks,
+            "roofline": {"bound": "alu", "kernel": "vjp_kernel (analytic adjoint)" if w.kind != "grid_b" else "grid_vjp_kernel",
+                         "achieved": achieved, "peak": peak, "unit": "T fp32 lane-instr/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": f"148 SM x 128 FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
+                         "alg_fp32_per_sample": fp_vjp, "forward": {"alg_fp32_per_sample": fp_fwd,
+                                                                    "achieved": fp_fwd * samples / r["t_fwd"] / 1e12,
+                                                                    "frac": fp_fwd * samples / r["t_fwd"] / 1e12 / peak}},
+        }
+        if clocks and clocks.get("sm_mhz"):
+            line["roofline"]["frac_at_sustained_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
+        if world == 1 and not args.no_cpu_baseline:
+            from paper_2410_01136_b200 import workloads as wl
+            line["cpu_baseline"] = {k: v for k, v in oracle_baseline(wl.config(args.config), seconds_budget=args.cpu_seconds).items()
+                                    if k in ("value", "unit", "cores", "kind", "sample", "forward_samples_per_s")}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: the metric's workload)")
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline oracle sample")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,314 @@
+"""GPU parity: the CUDA library (through the C ABI, via the ctypes binding) against the float64 oracle,
+element by element on the same seeded inputs (BASELINE.json configs 0-4).
+
+Tolerances (BASELINE.json north_star): max |delta| <= 1e-4 x RMS(oracle map) per (batch, frequency,
+Stokes) map; <= 1e-3 relative error per gradient component (grid gradient: + 1e-4 x RMS(grad) floor,
+DESIGN.md section 3 reading C-2#14).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import parity
+from paper_2410_01136_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def _check_grad(g, ref, what):
+    rel = np.abs(g - ref) / np.abs(ref)
+    assert np.all(np.isfinite(g)), what
+    assert rel.max() <= parity.GRAD_TOL, f"{what}: max rel err {rel.max():.3e} at {np.unravel_index(rel.argmax(), rel.shape)}"
+    return rel.max()
+
+
+def _check_grid_grad(g, ref, what):
+    rms = np.sqrt(np.mean(ref * ref))
+    bound = parity.GRAD_TOL * np.abs(ref) + 1.0e-4 * rms
+    bad = np.abs(g - ref) > bound
+    assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} grid components out of tolerance; worst {np.abs(g - ref).max() / rms:.3e} RMS"
+    # cells no sightline touches: exactly zero on both sides
+    assert np.array_equal(ref == 0.0, g == 0.0), f"{what}: untouched cells differ"
+
+
+# ------------------------------------------------------------------------------------------------
+# step A1: pixel directions
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nside", [1, 2, 3, 8, 64])
+def test_directions_match_oracle_pix2ang(nside):
+    import paper_2410_01136_b200 as sx
+    plan = sx.Plan(nside, 4, 1.0, [1e9])
+    d = plan.directions().cpu().numpy()
+    z, phi = oracle.pix2ang_ring(nside, np.arange(12 * nside * nside))
+    assert np.abs(d[:, 0] - np.cos(phi)).max() < 1e-15
+    assert np.abs(d[:, 1] - np.sin(phi)).max() < 1e-15
+    assert np.abs(d[:, 3] - z).max() < 1e-15
+    assert np.abs(d[:, 2] - np.sqrt(1 - z * z)).max() < 1e-15
+    plan.close()
+
+
+def test_directions_large_nside_sampled():
+    import paper_2410_01136_b200 as sx
+    nside = 256
+    plan = sx.Plan(nside, 4, 1.0, [1e9])
+    d = plan.directions().cpu().numpy()
+    pix = np.unique(np.concatenate([np.arange(0, 12 * nside * nside, 997), [12 * nside * nside - 1]]))
+    z, phi = oracle.pix2ang_ring(nside, pix)
+    assert np.abs(d[pix, 3] - z).max() < 1e-15 and np.abs(d[pix, 0] - np.cos(phi)).max() < 1e-15
+    n = np.stack([d[:, 2] * d[:, 0], d[:, 2] * d[:, 1], d[:, 3]], 1)
+    assert np.abs(n.sum(0)).max() < 1e-9 * len(n)     # C-3 #7
+    plan.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# configs at full size where the oracle finishes in seconds: 0, 1, 3
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lanes", [0, 1, 8, 32])
+def test_cfg0_forward_and_vjp(lanes):
+    w = wl.config(0)
+    maps, _ = parity.gpu_forward(w, lanes=lanes)
+    ref = parity.oracle_forward(w)
+    parity.assert_maps_close(maps, ref, what="cfg0 forward")
+    for ones in (True, False):
+        cots = w.cotangents(ones=ones)
+        g = parity.gpu_vjp(w, cots, lanes=lanes)
+        _check_grad(g, parity.oracle_vjp(w, cots), f"cfg0 vjp ones={ones} lanes={lanes}")
+
+
+def test_cfg1_forward_and_vjp_full_size():
+    w = wl.config(1)
+    maps, _ = parity.gpu_forward(w)
+    ref = parity.oracle_forward(w)
+    parity.assert_maps_close(maps, ref, what="cfg1 forward")
+    cots = w.cotangents()
+    _check_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), "cfg1 vjp")
+
+
+def test_cfg3_grid_forward_full_size():
+    w = wl.config(3)
+    maps, stats = parity.gpu_forward(w)
+    ref = parity.oracle_forward(w)
+    parity.assert_maps_close(maps, ref, what="cfg3 forward")
+    assert 0 < stats["escalated"] < w.npix      # 408 MHz: some sightlines need the float64 Faraday chain
+
+
+def test_cfg3_grid_vjp_full_size():
+    w = wl.config(3)
+    cots = w.cotangents()
+    _check_grid_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), "cfg3 vjp")
+
+
+# ------------------------------------------------------------------------------------------------
+# configs 2 and 4: scaled element-by-element, then full size on sampled outputs
+# ------------------------------------------------------------------------------------------------
+def test_cfg2_scaled_forward_and_vjp():
+    w = wl.config(2).scaled(nside=8, n_los=256, batch=16)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what="cfg2 scaled forward")
+    cots = w.cotangents()
+    _check_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), "cfg2 scaled vjp")
+
+
+def test_cfg2_full_size_sampled_batch_elements():
+    """Full launch configuration (256 x 12288 sightlines); the oracle recomputes 3 whole batch elements."""
+    w = wl.config(2)
+    maps, _ = parity.gpu_forward(w)
+    cots = w.cotangents()
+    g = parity.gpu_vjp(w, cots)
+    assert np.all(np.isfinite(g))
+    for b in (0, 101, 255):
+        wb = wl.Workload(w.name, w.kind, w.nside, w.n_los, w.s_max, w.freqs, w.params[b:b + 1], None, cot_seed=0)
+        ref = parity.oracle_forward(wb)
+        parity.assert_maps_close(tuple(m[b:b + 1] for m in maps), ref, what=f"cfg2 forward b={b}")
+        gb = parity.oracle_vjp(wb, tuple(c[b:b + 1] for c in cots))
+        _check_grad(g[b:b + 1], gb, f"cfg2 vjp b={b}")
+
+
+def test_cfg4_scaled_forward_and_vjp():
+    w = wl.config(4).scaled(nside=16, n_los=1024)
+    maps, stats = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what="cfg4 scaled forward")
+    cots = w.cotangents()
+    _check_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), "cfg4 scaled vjp")
+
+
+def _cfg4_sample_pixels(w):
+    """Every 64th pixel plus a band of in-plane pixels towards the inner Galaxy (the ill-conditioned ones)."""
+    z, phi = oracle.pix2ang_ring(w.nside, np.arange(0, w.npix, 7))
+    inner = np.arange(0, w.npix, 7)[(np.abs(z) < np.sin(np.radians(5.0))) & ((phi < 0.9) | (phi > 2 * np.pi - 0.9))]
+    return np.unique(np.concatenate([np.arange(0, w.npix, 64), inner[::8]]))
+
+
+def test_cfg4_full_size_forward_sampled_pixels():
+    w = wl.config(4)
+    maps, stats = parity.gpu_forward(w)
+    pix = _cfg4_sample_pixels(w)
+    ref = parity.oracle_forward(w, pix=pix)
+    sub = tuple(m[..., pix] for m in maps)
+    # RMS of the sampled oracle pixels stands in for the map RMS (uniform 1/64 subsample dominates)
+    parity.assert_maps_close(sub, ref, what="cfg4 full-size forward (sampled pixels)")
+    assert all(np.all(np.isfinite(m)) for m in maps)
+
+
+def test_cfg4_full_size_vjp_sparse_cotangent():
+    """The VJP is linear in the cotangent: a cotangent that is non-zero on every 48th pixel only makes the
+    full-size launch (all 786,432 sightlines) comparable with an oracle run over those pixels."""
+    w = wl.config(4)
+    pix = np.arange(5, w.npix, 48)
+    full = w.cotangents()
+    cots = tuple(np.zeros_like(c) for c in full)
+    for c, f in zip(cots, full):
+        c[..., pix] = f[..., pix]
+    g = parity.gpu_vjp(w, cots)
+    ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots), pix=pix)
+    _check_grad(g, ref, "cfg4 full-size vjp (sparse cotangent)")
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_los", [1, 2, 31, 33, 100, 257])
+@pytest.mark.parametrize("lanes", [1, 8, 32])
+def test_ragged_sample_counts(n_los, lanes):
+    w = wl.config(1).scaled(nside=4, n_los=n_los)
+    maps, _ = parity.gpu_forward(w, lanes=lanes)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=f"n_los={n_los} lanes={lanes}")
+    cots = w.cotangents()
+    _check_grad(parity.gpu_vjp(w, cots, lanes=lanes), parity.oracle_vjp(w, cots), f"vjp n_los={n_los} lanes={lanes}")
+
+
+@pytest.mark.parametrize("n_los", [1, 31, 100, 513])
+def test_ragged_sample_counts_grid(n_los):
+    w = wl.config(3).scaled(nside=4, n_los=n_los)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=f"grid n_los={n_los}")
+    cots = w.cotangents()
+    _check_grid_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), f"grid vjp n_los={n_los}")
+
+
+@pytest.mark.parametrize("n_freq", [2, 5, 13, 32])
+def test_frequency_block_splits(n_freq):
+    base = wl.config(4)
+    w = wl.Workload("nf", "full16", 4, 128, 30.0, np.geomspace(1.0e9, 40e9, n_freq), base.params, None, cot_seed=7)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=f"n_freq={n_freq}")
+    cots = w.cotangents()
+    _check_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), f"vjp n_freq={n_freq}")
+
+
+def test_nside_one_and_non_power_of_two():
+    for nside in (1, 3, 5):
+        w = wl.config(0).scaled(nside=nside, n_los=64)
+        maps, _ = parity.gpu_forward(w)
+        parity.assert_maps_close(maps, parity.oracle_forward(w), what=f"nside={nside}")
+
+
+def test_alpha_not_three_full16():
+    w = wl.config(4).scaled(nside=8, n_los=256)
+    w.params = w.params.copy()
+    w.params[0, 12] = 2.6
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what="alpha=2.6 forward")
+    cots = w.cotangents()
+    _check_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), "alpha=2.6 vjp")
+
+
+def test_null_cotangents_are_zero_maps():
+    w = wl.config(1).scaled(nside=8, n_los=128)
+    dI, dQ, dU = w.cotangents()
+    for cots in ((dI, None, None), (None, dQ, None), (None, None, dU), (dI, None, dU)):
+        _check_grad(parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots), "vjp with NULL cotangents")
+    g0 = parity.gpu_vjp(w, (None, None, None))
+    assert np.all(g0 == 0.0)
+
+
+def test_uniform_toy_closed_form_and_oracle():
+    """The paper's homogeneous toy: GPU against the oracle AND the slab closed form I = j L."""
+    w = wl.uniform_toy(nside=8, n_los=256)
+    maps, _ = parity.gpu_forward(w)
+    ref = parity.oracle_forward(w)
+    parity.assert_maps_close(maps, ref, what="uniform toy")
+    from conftest import load_golden
+    gold = load_golden("constants.txt")
+    # pixel with the largest B_perp: I = 0.264914 K (SURVEY C-3 #1) -- reached when n is perpendicular to B
+    assert abs(maps[0].max() / gold["toy_I_kelvin"] - 1) < 2e-3
+    cots = w.cotangents()
+    g = parity.gpu_vjp(w, cots)
+    gr = parity.oracle_vjp(w, cots)
+    nz = np.abs(gr) > 0
+    assert np.all(np.abs(g - gr)[nz] <= parity.GRAD_TOL * np.abs(gr)[nz])
+
+
+@pytest.mark.parametrize("precision", [1, 2])
+def test_precision_modes_high_frequency(precision):
+    """At 23-30 GHz the fp32 chain alone (1) and the float64 chain everywhere (2) both meet the tolerance."""
+    w = wl.Workload("hf", "disc4", 8, 256, 20.0, np.array([23e9, 30e9]), wl.config(0).params, wl.config(0).aux, cot_seed=5)
+    maps, _ = parity.gpu_forward(w, precision=precision)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=f"precision={precision}")
+
+
+def test_escalation_counts_and_strong_faraday_parity():
+    w = wl.config(4).scaled(nside=32, n_los=1024)
+    maps, stats = parity.gpu_forward(w)
+    ref = parity.oracle_forward(w)
+    e = parity.assert_maps_close(maps, ref, what="cfg4@nside32 forward")
+    assert 0 < stats["escalated"] < 0.5 * w.npix
+    maps2, stats2 = parity.gpu_forward(w, precision=2)
+    parity.assert_maps_close(maps2, ref, what="cfg4@nside32 forward, float64 chain everywhere")
+
+
+# ------------------------------------------------------------------------------------------------
+# host-buffer entry points and properties of the GPU path alone (T4)
+# ------------------------------------------------------------------------------------------------
+def test_host_entry_points_match_device_entry_points():
+    import paper_2410_01136_b200 as sx
+    w = wl.config(1).scaled(nside=8, n_los=128)
+    plan, model, params = parity.gpu_objects(w)
+    I, Q, U = sx.forward(plan, model, params)
+    Ih, Qh, Uh = sx.forward_host(plan, model, w.params)
+    assert np.array_equal(I.cpu().numpy(), Ih) and np.array_equal(Q.cpu().numpy(), Qh) and np.array_equal(U.cpu().numpy(), Uh)
+    cots = w.cotangents()
+    gh = sx.vjp_host(plan, model, w.params, *cots)
+    _check_grad(gh.astype(np.float64), parity.oracle_vjp(w, cots), "vjp_host")
+    plan.close()
+
+
+def test_gpu_invariants():
+    """SURVEY C-3 #4 on the GPU path: P <= Pi I; I ~ N0 (linear); joint sign flip (B, n_e) -> (-B, -n_e)."""
+    w = wl.config(4).scaled(nside=8, n_los=256)
+    (I, Q, U), _ = parity.gpu_forward(w)
+    assert np.all(np.hypot(Q, U) <= 0.75 * I * (1 + 1e-5) + 1e-30)
+    w2 = wl.config(4).scaled(nside=8, n_los=256)
+    w2.params = w.params.copy()
+    w2.params[0, 9] *= 2.0
+    (I2, Q2, U2), _ = parity.gpu_forward(w2)
+    assert np.allclose(I2, 2 * I, rtol=1e-6) and np.allclose(Q2, 2 * Q, rtol=1e-5, atol=1e-9 * np.abs(Q).max())
+    w3 = wl.config(4).scaled(nside=8, n_los=256)
+    w3.params = w.params.copy()
+    w3.params[0, [0, 5, 13]] *= -1.0
+    (I3, Q3, U3), _ = parity.gpu_forward(w3)
+    assert np.allclose(I3, I, rtol=1e-6) and np.allclose(Q3, Q, rtol=1e-5, atol=1e-7 * np.abs(Q).max())
+    assert np.allclose(U3, U, rtol=1e-5, atol=1e-7 * np.abs(U).max())
+
+
+def test_gpu_vjp_matches_gpu_finite_difference_direction():
+    """Directional derivative of the GPU forward (central difference) against <grad, direction>."""
+    w = wl.config(2).scaled(nside=8, n_los=128, batch=1)
+    cots = w.cotangents()
+    g = parity.gpu_vjp(w, cots)[0]
+    rng = np.random.Generator(np.random.PCG64(11))
+    v = rng.standard_normal(16) * np.abs(w.params[0].astype(np.float64))
+    h = 2e-3
+
+    def loss(p):
+        ww = wl.config(2).scaled(nside=8, n_los=128, batch=1)
+        ww.params = p.astype(np.float32)[None, :]
+        (I, Q, U), _ = parity.gpu_forward(ww)
+        used = ww.params[0].astype(np.float64)
+        return float((I * cots[0]).sum() + (Q * cots[1]).sum() + (U * cots[2]).sum()), used
+
+    lp, pp = loss(w.params[0].astype(np.float64) + h * v)
+    lm, pm = loss(w.params[0].astype(np.float64) - h * v)
+    fd = lp - lm
+    an = float(g @ (pp - pm))
+    assert abs(fd - an) <= 2e-2 * abs(an) + 1e-12
