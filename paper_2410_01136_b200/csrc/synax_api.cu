@@ -3,6 +3,7 @@
 // synax_forward.cuh / synax_vjp.cuh / synax_grid.cuh.
 #include "../../include/synax.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -43,9 +44,10 @@ struct synax_plan {
   int precision;      // 0 auto, 1 fp32 only, 2 float64 chain everywhere
   double escalate_rad;
   int lanes;          // 0 heuristic
-  int* d_flag_count;  // device
+  int* d_flag_count;  // device control block, kCtrlWords ints: [flag count, pilot flagged, mode, -]
   int* h_flag_count;  // pinned host mirror (last forward)
   mutable int64_t launches;
+  mutable int64_t last_n_sl;  // sightlines of the last forward (for stats when every one took the float64 chain)
 };
 
 static double faraday_K_per_kpc() {
@@ -77,7 +79,7 @@ extern "C" synax_status synax_plan_create(int32_t nside, int32_t n_los, double s
   p->npix = 12LL * nside * nside;
   p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los;
   for (int i = 0; i < 3; ++i) p->obs[i] = observer_kpc[i];
-  p->precision = 0; p->escalate_rad = 100.0; p->lanes = 0;
+  p->precision = 0; p->escalate_rad = 50.0; p->lanes = 0;
   const double KF = faraday_K_per_kpc();
   p->ft.n_freq = n_freq;
   for (int f = 0; f < kMaxFreq; ++f) {
@@ -91,11 +93,11 @@ extern "C" synax_status synax_plan_create(int32_t nside, int32_t n_los, double s
   }
   cudaError_t e = cudaGetDevice(&p->device);
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->dirs, (size_t)p->npix * 4 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, sizeof(int));
-  if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_flag_count, sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, kCtrlWords * sizeof(int));
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_flag_count, kCtrlWords * sizeof(int));
   if (e == cudaSuccess) {
-    *p->h_flag_count = 0;
-    e = cudaMemset(p->d_flag_count, 0, sizeof(int));
+    for (int i = 0; i < kCtrlWords; ++i) p->h_flag_count[i] = 0;
+    e = cudaMemset(p->d_flag_count, 0, kCtrlWords * sizeof(int));
   }
   if (e == cudaSuccess) {
     const int64_t blocks = (p->npix + 255) / 256;
@@ -154,7 +156,7 @@ extern "C" synax_status synax_plan_directions(const synax_plan* plan, double* ou
 extern "C" synax_status synax_plan_stats(const synax_plan* plan, int64_t out[2]) {
   if (!plan || !out) return fail(SYNAX_ERR_INVALID_ARG, "plan or out is NULL");
   out[0] = plan->launches;
-  out[1] = *plan->h_flag_count;
+  out[1] = plan->h_flag_count[kCtrlMode] == kModeAllF64 ? plan->last_n_sl : plan->h_flag_count[kCtrlFlagCount];
   return SYNAX_OK;
 }
 
@@ -222,15 +224,21 @@ static void launch_forward(int G, int nf, int64_t n_sl, cudaStream_t st, const F
   else if (G == 8) launch_forward_nf<CODE, 8>(nf, blocks, st, a, ft);
   else launch_forward_nf<CODE, 32>(nf, blocks, st, a, ft);
 }
-template <int CODE>
-static void launch_precise(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+template <int CODE, int G>
+static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
   switch (nf) {
-    case 1: forward_precise_kernel<CODE, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 2: forward_precise_kernel<CODE, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 3: forward_precise_kernel<CODE, 3><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 4: forward_precise_kernel<CODE, 4><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    default: forward_precise_kernel<CODE, 8><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 1: forward_f64_kernel<CODE, G, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 2: forward_f64_kernel<CODE, G, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 3: forward_f64_kernel<CODE, G, 3><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 4: forward_f64_kernel<CODE, G, 4><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    default: forward_f64_kernel<CODE, G, 8><<<blocks, kBlock, 0, st>>>(a, ft); break;
   }
+}
+template <int CODE>
+static void launch_f64(int G, int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+  if (G == 1) launch_f64_nf<CODE, 1>(nf, blocks, st, a, ft);
+  else if (G == 8) launch_f64_nf<CODE, 8>(nf, blocks, st, a, ft);
+  else launch_f64_nf<CODE, 32>(nf, blocks, st, a, ft);
 }
 
 static AuxHost make_aux(const synax_model* m) {
@@ -268,13 +276,15 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   const int64_t n_sl = plan->npix * batch;
 
   BatchConsts* bc = nullptr;
+  BatchConstsD* bd = nullptr;
   CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
+  CUDA_TRY(cudaMallocAsync((void**)&bd, sizeof(BatchConstsD) * (size_t)batch, st));
   prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
-                                                      make_aux(model), plan->ft, plan->delta, bc);
+                                                      make_aux(model), plan->ft, plan->delta, bc, bd);
   plan->launches++;
 
   ForwardArgs a;
-  a.geo = make_geo(plan); a.bc = bc; a.batch = batch; a.I = I; a.Q = Q; a.U = U;
+  a.geo = make_geo(plan); a.bc = bc; a.bd = bd; a.batch = batch; a.I = I; a.Q = Q; a.U = U;
   a.n_freq_total = plan->n_freq;
   a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
 
@@ -282,6 +292,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, sm_count(plan->device),
                                    plan->d_flag_count, plan->h_flag_count, st, &plan->launches);
     cudaFreeAsync(bc, st);
+    cudaFreeAsync(bd, st);
     if (gs != SYNAX_OK) return fail(gs, "grid forward failed: %s", cudaGetErrorString(cudaGetLastError()));
     return SYNAX_OK;
   }
@@ -290,43 +301,70 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   for (int f = 0; f < plan->n_freq; ++f) k_max = fmaxf(k_max, plan->ft.k_rad[f]);
   const bool fast = plan->precision != 2;
   const bool escalate = plan->precision == 0;
+  int* ctrl = plan->d_flag_count;
+  plan->last_n_sl = n_sl;
+  CUDA_TRY(cudaMemsetAsync(ctrl, 0, kCtrlWords * sizeof(int), st));   // mode = fp32 pass then flagged list
+  a.mode = nullptr; a.run_when = 0;
+  const int sms = sm_count(plan->device);
+  // precision 0: a pilot over ~8k sightlines decides ON THE DEVICE between "fp32 pass + float64 redo of the flagged
+  // sightlines" and "float64 Faraday chain for every sightline" (cheaper once more than a quarter is flagged).
+  bool piloted = false;
   if (escalate) {
     CUDA_TRY(cudaMallocAsync((void**)&a.flag_list, sizeof(int) * (size_t)n_sl, st));
-    CUDA_TRY(cudaMemsetAsync(plan->d_flag_count, 0, sizeof(int), st));
     a.flag_S = (float)(plan->escalate_rad / (double)k_max);
+    if (n_sl > 16384) {
+      const int64_t stride = (n_sl / 8192) | 1;
+      const int64_t n_pilot = (n_sl + stride - 1) / stride;
+      const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
+      if (code == kAnalyticDisc) pilot_kernel<kAnalyticDisc><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
+      else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
+      else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
+      decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot);
+      plan->launches += 2;
+      a.mode = ctrl + kCtrlMode;
+      piloted = true;
+    }
   }
   const int G = pick_lanes(plan, n_sl);
-  const unsigned pblocks = (unsigned)(sm_count(plan->device) * 8);
-  for (int f0 = 0; f0 < plan->n_freq;) {
-    const int nf = next_freq_block(plan->n_freq - f0);
-    a.f0 = f0;
-    if (fast) {
+  auto blocks_for = [&](int lanes) {
+    return (unsigned)std::min<int64_t>((n_sl * lanes + kBlock - 1) / kBlock, (int64_t)sms * 16);
+  };
+  auto run_f64 = [&](int lanes, int run_when, bool use_list) {
+    ForwardArgs pa = a;
+    pa.run_when = run_when;
+    if (!use_list) pa.flag_list = nullptr;
+    for (int f0 = 0; f0 < plan->n_freq;) {
+      const int nf = next_freq_block(plan->n_freq - f0);
+      pa.f0 = f0;
+      if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
+      else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
+      else launch_f64<kUniform>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
+      plan->launches++;
+      f0 += nf;
+    }
+  };
+  if (fast) {
+    for (int f0 = 0; f0 < plan->n_freq;) {
+      const int nf = next_freq_block(plan->n_freq - f0);
+      a.f0 = f0;
       if (code == kAnalyticDisc) launch_forward<kAnalyticDisc>(G, nf, n_sl, st, a, plan->ft);
       else if (code == kAnalyticFull) launch_forward<kAnalyticFull>(G, nf, n_sl, st, a, plan->ft);
       else launch_forward<kUniform>(G, nf, n_sl, st, a, plan->ft);
       plan->launches++;
-    }
-    f0 += nf;
-  }
-  if (!fast || escalate) {
-    ForwardArgs pa = a;
-    if (!fast) pa.flag_list = nullptr;  // every sightline
-    for (int f0 = 0; f0 < plan->n_freq;) {
-      const int nf = next_freq_block(plan->n_freq - f0);
-      pa.f0 = f0;
-      if (code == kAnalyticDisc) launch_precise<kAnalyticDisc>(nf, pblocks, st, pa, plan->ft);
-      else if (code == kAnalyticFull) launch_precise<kAnalyticFull>(nf, pblocks, st, pa, plan->ft);
-      else launch_precise<kUniform>(nf, pblocks, st, pa, plan->ft);
-      plan->launches++;
       f0 += nf;
     }
+    if (escalate) {
+      run_f64(8, piloted ? 1 : 0, true);          // the flagged list, 8 lanes per sightline
+      if (piloted) run_f64(G, 2, false);          // or everything (exits at once unless the pilot chose it)
+    }
+  } else {
+    run_f64(G, 0, false);
   }
   cudaError_t e = cudaGetLastError();
-  if (escalate) {
-    cudaMemcpyAsync(plan->h_flag_count, plan->d_flag_count, sizeof(int), cudaMemcpyDeviceToHost, st);
-    cudaFreeAsync(a.flag_list, st);
-  }
+  cudaMemcpyAsync(plan->h_flag_count, ctrl, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (escalate) cudaFreeAsync(a.flag_list, st);
   cudaFreeAsync(bc, st);
+  cudaFreeAsync(bd, st);
   if (e != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward launch failed: %s", cudaGetErrorString(e));
   return SYNAX_OK;
 }
@@ -342,7 +380,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   BatchConsts* bc = nullptr;
   CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
   prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
-                                                      make_aux(model), plan->ft, plan->delta, bc);
+                                                      make_aux(model), plan->ft, plan->delta, bc, nullptr);
   plan->launches++;
   synax_status rs;
   if (code == kGridB)

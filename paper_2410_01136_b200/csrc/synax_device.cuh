@@ -51,6 +51,37 @@ __device__ __forceinline__ void sincos_fma(float x, float& s, float& c) {
   c = ((q + 1) & 2) ? -cs : cs;
 }
 
+// 2^x on the FMA pipe: round-to-nearest split x = k + f, |f| <= 1/2, degree-6 near-minimax polynomial
+// (approximation error 2.6e-9, so what is left is fp32 rounding: ~3e-8 rms, mean 1e-9, i.e. it
+// averages out along a sightline, unlike the table-based MUFU.EX2 whose ~1e-7 error is systematic
+// over many consecutive samples).  Used for every exponential the Faraday integrand n_e B_LOS sees
+// (DESIGN.md section 5).  x is clamped at -125 (result stays a normal number).
+__device__ __forceinline__ float exp2_fma(float x) {
+  x = fmaxf(x, -125.0f);
+  const float t = x + 12582912.0f;                 // 1.5 * 2^23: the integer part lands in the low mantissa bits
+  const float f = x - (t - 12582912.0f);           // exact
+  float p = fmaf(1.5469732170458883e-4f, f, 1.3400432653725147e-3f);
+  p = fmaf(p, f, 9.61802527308464e-3f);
+  p = fmaf(p, f, 5.550327152013779e-2f);
+  p = fmaf(p, f, 2.4022650718688965e-1f);
+  p = fmaf(p, f, 6.931471824645996e-1f);
+  p = fmaf(p, f, 1.0f);
+  return __int_as_float(__float_as_int(p) + (__float_as_int(t) << 23));
+}
+// 1/x: MUFU seed + one Newton step (removes the seed's systematic ~1 ulp error)
+__device__ __forceinline__ float rcp_nr(float x) {
+  const float y = mufu_rcp(x);
+  return fmaf(y, fmaf(-x, y, 1.0f), y);
+}
+// 1/sqrt(x) and sqrt(x): MUFU seed + one Newton step each
+__device__ __forceinline__ void rsqrt_sqrt_nr(float x, float& ir, float& r) {
+  float y = mufu_rsqrt(x);
+  y = fmaf(0.5f * y, fmaf(-x * y, y, 1.0f), y);
+  float s = x * y;
+  s = fmaf(0.5f * y, fmaf(-s, s, x), s);
+  ir = y; r = s;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Per-batch-element constants, written by prologue_kernel (fp64 math, rounded once).
 // Canonical 16-parameter analytic model; DISC4 maps onto it with h_b = inf, B_h = 0.
@@ -60,12 +91,14 @@ struct BatchConsts {
   float p[kMaxAnalyticParams];
   // derived fp32
   float k_hb;        // -log2(e)/h_b      (0 for DISC4)
+  float k_hb_lo, k_her_lo;  // float64 value minus its fp32 rounding (the constants multiply rho ~ 10 kpc)
   float inv_wh, inv_rh;
   float k_hr, k_hz;  // -log2(e)/h_r, -2 log2(e)/h_z
   float k_her, k_hez;
   float q_exp;       // (alpha-3)/4 : (B_perp^2)^q_exp
   float pi_frac;     // (alpha+1)/(alpha+7/3)   Eq.(5)/Eq.(2)
   int alpha_is_3;
+  int tile_d;        // samples per tile of the float64-chain kernel (prologue_kernel)
   float coefI[kMaxFreq];  // c_f(alpha) * Delta  [K per (cm^-3 uG^((alpha+1)/2))]
   float coefP[kMaxFreq];  // pi_frac * coefI
   // VJP only
@@ -94,6 +127,7 @@ struct Geometry {
 struct Triad {
   double nxd, nyd, nzd;    // line of sight, float64 (positions, mask)
   float nx, ny, nz;
+  float nxl, nyl, nzl;     // n - (float)n: low parts, so that B.n does not carry a per-sightline 3e-8 bias
   float eNx, eNy, eNz;     // towards Galactic north
   float eEx, eEy;          // towards increasing l (z component is 0)
 };
@@ -103,6 +137,7 @@ __device__ __forceinline__ Triad load_triad(const double* __restrict__ dirs, int
   Triad t;
   t.nxd = d.z * d.x; t.nyd = d.z * d.y; t.nzd = d.w;
   t.nx = (float)t.nxd; t.ny = (float)t.nyd; t.nz = (float)t.nzd;
+  t.nxl = (float)(t.nxd - (double)t.nx); t.nyl = (float)(t.nyd - (double)t.ny); t.nzl = (float)(t.nzd - (double)t.nz);
   t.eNx = (float)(-d.w * d.x); t.eNy = (float)(-d.w * d.y); t.eNz = (float)d.z;
   t.eEx = (float)(-d.y); t.eEy = (float)d.x;
   return t;
@@ -129,38 +164,61 @@ struct AnalyticAux {
   float thz, thez;         // tanh(z/h_z), tanh(z/h_ez)
 };
 
-template <bool kHalo>
+template <bool kHalo, bool kAcc = false>
 __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Triad& T, float x, float y,
                                                   float z, float rho2, bool inside, SampleF& S,
                                                   AnalyticAux& a) {
+  // kAcc: everything the Faraday integrand n_e B_LOS depends on is evaluated so that no error is
+  // systematic along the sightline above ~1e-8 (Newton-corrected reciprocals/roots, FMA-pipe
+  // exponentials, hi+lo constants); N_0 (emission only) stays on the MUFU.
   const float kLog2e = 1.4426950408889634f;
-  a.ir = mufu_rsqrt(rho2);
-  a.rho = rho2 * a.ir;
+  rho2 = fmaxf(rho2, 1.0e-30f);
+  if (kAcc) {
+    rsqrt_sqrt_nr(rho2, a.ir, a.rho);
+  } else {
+    a.ir = mufu_rsqrt(rho2);
+    a.rho = rho2 * a.ir;
+  }
   a.xr = x * a.ir; a.yr = y * a.ir;
   const float az = fabsf(z);
   // --- disc: B = A [cos psi cos chi rho_hat + sin psi cos chi phi_hat + sin chi z_hat]   Eq.(13)
   a.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;        // ln(rho/8) = ln2/2 (lg2 rho^2 - 6)
   const float psi = fmaf(P.p[2], a.lr, P.p[1]);
   sincos_fma(psi, a.sp, a.cp);
-  const float e1 = mufu_ex2(-2.0f * kLog2e * az);               // tanh(|z|) = (1-e)/(1+e)
-  a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
+  if (kAcc) {
+    const float e1 = exp2_fma(-2.0f * kLog2e * az);             // tanh(|z|) = (1-e)/(1+e)
+    a.t = copysignf((1.0f - e1) * rcp_nr(1.0f + e1), z);
+  } else {
+    const float e1 = mufu_ex2(-2.0f * kLog2e * az);
+    a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
+  }
   const float chi = P.p[3] * a.t;
   sincos_fma(chi, a.sc, a.cc);
-  const float rad = (P.k_hb != 0.0f) ? mufu_ex2(P.k_hb * (a.rho - 8.0f)) : 1.0f;
+  float rad = 1.0f;
+  if (P.k_hb != 0.0f) {
+    const float dr = a.rho - 8.0f;
+    rad = kAcc ? exp2_fma(fmaf(P.k_hb, dr, P.k_hb_lo * dr)) : mufu_ex2(P.k_hb * dr);
+  }
   a.A = inside ? P.p[0] * rad : 0.0f;
   const float Brho = a.A * a.cp * a.cc;
   float Bphi = a.A * a.sp * a.cc;
   const float Bz = a.A * a.sc;
   if (kHalo) {  // toroidal halo, S:App.C
     a.u = (az - P.p[6]) * P.inv_wh;
-    a.L = mufu_rcp(fmaf(a.u, a.u, 1.0f));
     const float q = a.rho * P.inv_rh;
-    a.R = q * mufu_ex2(kLog2e * (1.0f - q));
+    if (kAcc) {
+      a.L = rcp_nr(fmaf(a.u, a.u, 1.0f));
+      a.R = q * exp2_fma(kLog2e * (1.0f - q));
+    } else {
+      a.L = mufu_rcp(fmaf(a.u, a.u, 1.0f));
+      a.R = q * mufu_ex2(kLog2e * (1.0f - q));
+    }
     Bphi = fmaf(P.p[5] * a.L, a.R, Bphi);
   }
   const float Bx = Brho * a.xr - Bphi * a.yr;
   const float By = fmaf(Brho, a.yr, Bphi * a.xr);
   S.Bpar = fmaf(Bx, T.nx, fmaf(By, T.ny, Bz * T.nz));           // B.n, signed (S:C-2#3)
+  if (kAcc) S.Bpar += fmaf(Bx, T.nxl, fmaf(By, T.nyl, Bz * T.nzl));
   S.BN = fmaf(Bx, T.eNx, fmaf(By, T.eNy, Bz * T.eNz));          // Eq.(8) numerator
   S.BE = fmaf(Bx, T.eEx, By * T.eEy);                           // Eq.(8) denominator (S:C-2#4)
   // --- N_0 = n0 exp(-rho/h_r) sech^2(z/h_z)  Eq.(12);  sech^2 w = 4e/(1+e)^2, e = exp(-2|w|)
@@ -169,11 +227,19 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
   const float iz = mufu_rcp(dz * dz);
   S.N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * a.rho) * ez * iz;
   a.thz = copysignf((1.0f - ez) * dz * iz, z);                  // tanh = (1-e)/(1+e)
-  const float ee = mufu_ex2(P.k_hez * az);
-  const float de = 1.0f + ee;
-  const float ie = mufu_rcp(de * de);
-  S.ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * a.rho) * ee * ie;
-  a.thez = copysignf((1.0f - ee) * de * ie, z);
+  if (kAcc) {
+    const float ee = exp2_fma(P.k_hez * az);
+    const float de = 1.0f + ee;
+    const float ie = rcp_nr(de * de);
+    S.ne = 4.0f * P.p[13] * exp2_fma(fmaf(P.k_her, a.rho, P.k_her_lo * a.rho)) * ee * ie;
+    a.thez = copysignf((1.0f - ee) * de * ie, z);
+  } else {
+    const float ee = mufu_ex2(P.k_hez * az);
+    const float de = 1.0f + ee;
+    const float ie = mufu_rcp(de * de);
+    S.ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * a.rho) * ee * ie;
+    a.thez = copysignf((1.0f - ee) * de * ie, z);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------

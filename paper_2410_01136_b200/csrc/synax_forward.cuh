@@ -1,11 +1,14 @@
 // synax_forward.cuh -- plan geometry kernel (A1), per-batch prologue, forward kernels (A2-A8, A12).
 #pragma once
 #include "synax_device.cuh"
+#include "synax_f64.cuh"
 
 namespace synax {
 
 constexpr int kBlock = 128;   // threads per CTA for the sightline kernels
 constexpr int kTile = 32;     // samples between re-basing of the local Faraday sum
+constexpr int kTileDMax = 16;  // float64-chain kernel: at most this many samples per tile (BatchConsts::tile_d)
+constexpr float kTilePhase = 48.0f;  // ... and at most about this much Faraday angle (rad) inside a tile
 
 enum ModelCode { kAnalyticDisc = 0, kAnalyticFull = 1, kGridB = 2, kUniform = 3 };
 
@@ -61,7 +64,8 @@ __global__ void pix2ang_kernel(int64_t nside, int64_t npix, double* __restrict__
 struct AuxHost { float v[7]; };  // C0, h_r, h_z, alpha, ne0, h_er, h_ez
 
 __global__ void prologue_kernel(int code, const float* __restrict__ params, int n_params, int batch,
-                                AuxHost aux, FreqTab ft, double delta, BatchConsts* __restrict__ out) {
+                                AuxHost aux, FreqTab ft, double delta, BatchConsts* __restrict__ out,
+                                BatchConstsD* __restrict__ outd) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= batch) return;
   BatchConsts c;
@@ -87,11 +91,13 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
   for (int j = 0; j < 16; ++j) c.p[j] = (float)p[j];
   const double log2e = 1.4426950408889634;
   c.k_hb = (code == kAnalyticFull) ? (float)(-log2e / p[4]) : 0.0f;
+  c.k_hb_lo = (code == kAnalyticFull) ? (float)(-log2e / p[4] - (double)c.k_hb) : 0.0f;
   c.inv_wh = (float)(1.0 / p[8]);
   c.inv_rh = (float)(1.0 / p[7]);
   c.k_hr = (float)(-log2e / p[10]);
   c.k_hz = (float)(-2.0 * log2e / fabs(p[11]));
   c.k_her = (float)(-log2e / p[14]);
+  c.k_her_lo = (float)(-log2e / p[14] - (double)c.k_her);
   c.k_hez = (float)(-2.0 * log2e / fabs(p[15]));
   c.q_exp = (float)((alpha - 3.0) * 0.25);
   c.pi_frac = (float)((alpha + 1.0) / (alpha + 7.0 / 3.0));
@@ -117,7 +123,34 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
       c.coefI[f] = c.coefP[f] = c.dlnc_dalpha[f] = 0.0f;
     }
   }
+  // Tile length of the float64-chain kernel: the fp32 angle k_f * (tile-local Faraday sum) must stay small
+  // enough for its 6e-8 relative round-off not to matter.  Bound on |n_e B_LOS| per sample:
+  {
+    double gmax;
+    if (code == kUniform) {
+      gmax = fabs((double)c.une) * (fabs((double)c.uB[0]) + fabs((double)c.uB[1]) + fabs((double)c.uB[2]));
+    } else {
+      double bmax = fabs(p[0]);
+      if (code == kAnalyticFull) bmax = bmax * fmax(exp(5.0 / p[4]), exp(-12.0 / p[4])) + fabs(p[5]);
+      gmax = fabs(p[13]) * bmax;
+    }
+    double kmax = 0.0;
+    for (int f = 0; f < ft.n_freq; ++f) kmax = fmax(kmax, (double)ft.k_rad[f]);
+    const double per_step = kmax * gmax;
+    int t = kTileDMax;
+    if (per_step * t > (double)kTilePhase) t = (int)((double)kTilePhase / per_step);
+    c.tile_d = t < 1 ? 1 : t;
+  }
   out[b] = c;
+  if (outd) {
+    BatchConstsD d;
+    d.b0 = p[0]; d.psi0 = p[1]; d.psi1 = p[2]; d.chi0 = p[3];
+    d.k_hb = (code == kAnalyticFull) ? -log2e / p[4] : 0.0;
+    d.Bh = p[5]; d.zh0 = p[6]; d.inv_rh = 1.0 / p[7]; d.inv_wh = 1.0 / p[8];
+    d.ne0x4 = 4.0 * p[13]; d.k_her = -log2e / p[14]; d.k_hez = -2.0 * log2e / fabs(p[15]);
+    d.psi1_small = fabs(p[2]) <= 0.05 ? 1 : 0;
+    outd[b] = d;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -188,6 +221,7 @@ __device__ __forceinline__ void emission(const BatchConsts& P, float BN, float B
 struct ForwardArgs {
   Geometry geo;
   const BatchConsts* bc;
+  const BatchConstsD* bd; // float64 constants (float64 Faraday chain only)
   int batch;
   int f0;                 // first frequency of this pass
   float* I; float* Q; float* U;
@@ -195,11 +229,17 @@ struct ForwardArgs {
   float flag_S;           // flag a sightline when max |sum n_e B_LOS| exceeds this (<=0: never)
   int* flag_count;        // device counter
   int* flag_list;         // device list of flagged sightline ids (b * npix + p)
+  const int* mode;        // device: kModeFastThenList / kModeAllF64 (written by decide_kernel), or null
+  int run_when;           // forward_f64_kernel: 0 always, 1 only in list mode, 2 only in all-float64 mode
 };
+
+enum { kModeFastThenList = 0, kModeAllF64 = 1 };
+enum { kCtrlFlagCount = 0, kCtrlPilotFlagged = 1, kCtrlMode = 2, kCtrlWords = 4 };
 
 template <int CODE, int G, int NF>
 __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__ ForwardArgs A,
                                                          const __grid_constant__ FreqTab ft) {
+  if (A.mode && *A.mode == kModeAllF64) return;   // the pilot found mostly strong Faraday rotation
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
   int64_t sl = tid / G;
@@ -225,7 +265,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 #pragma unroll
   for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
   double carry = 0.0;            // chunk-local sum of n_e B_LOS over finished tiles
-  float cmax = 0.0f, cmin = 0.0f;
+  float gabs = 0.0f;             // sum n_e (|B_LOS| + |B_N| + |B_E|): scale of the fp32 round-off in the Faraday sum
 
   for (int ts = n0; ts < n1; ts += kTile) {
     const int te = min(ts + kTile, n1);
@@ -249,13 +289,14 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         const double rho2d = fma(xd, xd, yd * yd);
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
       float eI, a, bq;
       emission(P, S.BN, S.BE, S.N0, eI, a, bq);
       accI += eI;
       // A6: half-cell Faraday sum (S:C-2#5), tile-local, compensated
       const float gn = S.ne * S.Bpar;
+      gabs = fmaf(fabsf(S.ne), fabsf(S.Bpar) + fabsf(S.BN) + fabsf(S.BE), gabs);
       const float ph = fmaf(0.5f, gn, hi);
       const float sum = hi + gn;
       lo += gn - (sum - hi);
@@ -280,7 +321,6 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       }
     }
     carry += (double)hi + (double)lo;
-    cmax = fmaxf(cmax, (float)carry); cmin = fminf(cmin, (float)carry);
   }
 
   // combine the G lanes of the sightline
@@ -294,9 +334,9 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       accU[f] = group_sum<G>(accU[f]);
     }
     accI = group_sum<G>(accI);
-    absS = group_max<G>(fmaxf(fabsf((float)off + cmax), fabsf((float)off + cmin)));
+    absS = group_sum<G>(gabs);
   } else {
-    absS = fmaxf(cmax, -cmin);
+    absS = gabs;
   }
   if (valid && g == 0) {
     const int64_t npix = A.geo.npix;
@@ -315,68 +355,107 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 }
 
 // ------------------------------------------------------------------------------------------------
-// Forward, float64 Faraday chain, one warp per flagged sightline (list written by forward_kernel or
-// "all sightlines" when list == nullptr).  Persistent grid: warps stride over the list.
+// Forward, float64 Faraday chain (synax_f64.cuh): B and n_e in float64 from short polynomials, the
+// Faraday sum in float64; emission, N_0 and the per-frequency rotation in fp32 as in the fast kernel
+// (the rotation angle is taken relative to the start of a 32-sample tile, whose own float64 angle is
+// reduced to turns exactly).  G lanes per sightline; groups stride over the flag list written by
+// forward_kernel, or over all sightlines when the list is null.
 // ------------------------------------------------------------------------------------------------
-template <int CODE, int NF>
-__global__ void __launch_bounds__(kBlock) forward_precise_kernel(const __grid_constant__ ForwardArgs A,
-                                                                 const __grid_constant__ FreqTab ft) {
-  const int lane = threadIdx.x & 31;
-  const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
-  const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
+template <int CODE, int G, int NF>
+__global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_constant__ ForwardArgs A,
+                                                             const __grid_constant__ FreqTab ft) {
+  const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const int g = (int)(tid % G);
+  const int64_t n_groups = ((int64_t)gridDim.x * kBlock) / G;
   const int64_t n_sl = A.geo.npix * A.batch;
-  const int64_t count = A.flag_list ? (int64_t)(*A.flag_count) : n_sl;
+  if (A.run_when == 1 && *A.mode == kModeAllF64) return;
+  if (A.run_when == 2 && *A.mode != kModeAllF64) return;
+  const bool use_list = A.flag_list && A.run_when != 2;
+  const int64_t count = use_list ? (int64_t)(*A.flag_count) : n_sl;
+  const int C = (A.geo.n_los + G - 1) / G;
+  const int n0 = g * C;
+  const int n1 = min(n0 + C, A.geo.n_los);
   const double delta = A.geo.delta;
-  const int C = (A.geo.n_los + 31) / 32;
-  for (int64_t it = warp; it < count; it += n_warps) {
-    const int64_t sl = A.flag_list ? (int64_t)A.flag_list[it] : it;
+  float k_rad[NF];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[A.f0 + f];
+
+  for (int64_t it = tid / G;; it += n_groups) {
+    if (it - ((threadIdx.x & 31) / G) >= count) break;   // first group of this warp: warp-uniform exit
+    const bool valid = it < count;
+    const int64_t item = valid ? it : count - 1;
+    const int64_t sl = use_list ? (int64_t)A.flag_list[item] : item;
     const int b = (int)(sl / A.geo.npix);
     const int64_t pix = sl - (int64_t)b * A.geo.npix;
     const BatchConsts& P = A.bc[b];
-    const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
-    const double nxd = dir.z * dir.x, nyd = dir.z * dir.y, nzd = dir.w;
-    const int n0 = lane * C, n1 = min(n0 + C, A.geo.n_los);
+    const BatchConstsD& D = A.bd[b];
+    const Triad T = load_triad(A.geo.dirs, pix);
+    double s_d = ((double)n0 + 0.5) * delta;
     float accI = 0.0f, accQ[NF], accU[NF];
 #pragma unroll
     for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
-    double S_loc = 0.0;
-    for (int n = n0; n < n1; ++n) {
-      const double s_d = ((double)n + 0.5) * delta;
-      const double xd = fma(s_d, nxd, A.geo.obs[0]);
-      const double yd = fma(s_d, nyd, A.geo.obs[1]);
-      const double zd = fma(s_d, nzd, A.geo.obs[2]);
-      SampleD S;
-      if (CODE == kUniform) {
-        const double Bx = P.uB[0], By = P.uB[1], Bz = P.uB[2];
-        S.Bpar = Bx * nxd + By * nyd + Bz * nzd;
-        S.BN = Bz * dir.z - dir.w * (Bx * dir.x + By * dir.y);
-        S.BE = By * dir.x - Bx * dir.y;
-        S.N0 = P.uN0; S.ne = P.une;
-      } else {
-        eval_analytic_f64<CODE == kAnalyticFull>(P, dir, xd, yd, zd, S);
+    double S_loc = 0.0;      // sum of n_e B_LOS over this lane's finished samples
+    const int tile = P.tile_d;
+    for (int ts = n0; ts < n1; ts += tile) {
+      const int te = min(ts + tile, n1);
+      const double S_tile = S_loc;
+      float tq[NF], tu[NF];
+#pragma unroll
+      for (int f = 0; f < NF; ++f) { tq[f] = 0.0f; tu[f] = 0.0f; }
+      for (int n = ts; n < te; ++n) {
+        const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+        const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+        const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+        s_d += delta;
+        double Bx, By, Bz, ne;
+        float N0;
+        if (CODE == kUniform) {
+          Bx = (double)P.uB[0]; By = (double)P.uB[1]; Bz = (double)P.uB[2]; ne = (double)P.une; N0 = P.uN0;
+        } else {
+          const double rho2d = fma(xd, xd, yd * yd);
+          const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+          eval_analytic_d<CODE == kAnalyticFull>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
+          // N_0 (emission only): fp32 MUFU chain, Eq.(12)
+          const float rho2f = fmaxf((float)rho2d, 1.0e-30f);
+          const float rho = rho2f * mufu_rsqrt(rho2f);
+          const float ez = mufu_ex2(P.k_hz * fabsf((float)zd));
+          const float dz = 1.0f + ez;
+          N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
+        }
+        const double gn = ne * fma(Bx, T.nxd, fma(By, T.nyd, Bz * T.nzd));   // n_e B.n, signed (S:C-2#3)
+        const float ph = (float)fma(0.5, gn, S_loc - S_tile);                  // half-cell (S:C-2#5), tile-local
+        S_loc += gn;
+        const float bx = (float)Bx, by = (float)By, bz = (float)Bz;
+        const float BN = fmaf(bx, T.eNx, fmaf(by, T.eNy, bz * T.eNz));
+        const float BE = fmaf(bx, T.eEx, by * T.eEy);
+        float eI, a, bq;
+        emission(P, BN, BE, N0, eI, a, bq);
+        accI += eI;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          const float th = k_rad[f] * ph;
+          const float c = mufu_cos(th), s = mufu_sin(th);
+          tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
+          tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+        }
       }
-      float eI, a, bq;
-      emission(P, (float)S.BN, (float)S.BE, (float)S.N0, eI, a, bq);
-      accI += eI;
-      const double gn = S.ne * S.Bpar;
-      const double ph = S_loc + 0.5 * gn;
-      S_loc += gn;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        float q = a, u = bq;
-        rotate_by_offset(ft.k_turn[A.f0 + f], ph, q, u);
-        accQ[f] += q; accU[f] += u;
+        rotate_by_offset(ft.k_turn[A.f0 + f], S_tile, tq[f], tu[f]);
+        accQ[f] += tq[f]; accU[f] += tu[f];
       }
     }
-    const double off = group_exclusive_scan<32>(S_loc, lane);
+    if (G > 1) {
+      const double off = group_exclusive_scan<G>(S_loc, g);
 #pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      rotate_by_offset(ft.k_turn[A.f0 + f], off, accQ[f], accU[f]);
-      accQ[f] = group_sum<32>(accQ[f]);
-      accU[f] = group_sum<32>(accU[f]);
+      for (int f = 0; f < NF; ++f) {
+        rotate_by_offset(ft.k_turn[A.f0 + f], off, accQ[f], accU[f]);
+        accQ[f] = group_sum<G>(accQ[f]);
+        accU[f] = group_sum<G>(accU[f]);
+      }
+      accI = group_sum<G>(accI);
     }
-    accI = group_sum<32>(accI);
-    if (lane == 0) {
+    if (valid && g == 0) {
       const int64_t npix = A.geo.npix;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
@@ -387,6 +466,52 @@ __global__ void __launch_bounds__(kBlock) forward_precise_kernel(const __grid_co
       }
     }
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Pilot: Faraday sums only (MUFU-grade fp32 chain), one warp per sampled sightline (every `stride`-th),
+// counting those whose rotation angle exceeds the escalation threshold.  decide_kernel then picks the
+// forward strategy on the device -- no host synchronisation: fp32 pass + float64 redo of the flagged
+// list when they are few, or the float64-chain kernel for every sightline when they are many.
+// ------------------------------------------------------------------------------------------------
+template <int CODE>
+__global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ ForwardArgs A, int64_t stride,
+                                                       int64_t n_pilot, int* __restrict__ ctrl) {
+  const int lane = threadIdx.x & 31;
+  const int64_t j = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
+  if (j >= n_pilot) return;
+  const int64_t sl = j * stride;
+  const int b = (int)(sl / A.geo.npix);
+  const int64_t pix = sl - (int64_t)b * A.geo.npix;
+  const BatchConsts& P = A.bc[b];
+  const Triad T = load_triad(A.geo.dirs, pix);
+  const int C = (A.geo.n_los + 31) / 32;
+  const int n0 = lane * C, n1 = min(n0 + C, A.geo.n_los);
+  float gabs = 0.0f;
+  for (int n = n0; n < n1; ++n) {
+    const double s_d = ((double)n + 0.5) * A.geo.delta;
+    float gn;
+    if (CODE == kUniform) {
+      gn = fabsf(P.une) * (fabsf(P.uB[0]) + fabsf(P.uB[1]) + fabsf(P.uB[2]));
+    } else {
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      const double rho2d = fma(xd, xd, yd * yd);
+      SampleF Sm; AnalyticAux aux;
+      eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
+                                                      (rho2d > 9.0) && (rho2d < 400.0), Sm, aux);
+      gn = fabsf(Sm.ne) * (fabsf(Sm.Bpar) + fabsf(Sm.BN) + fabsf(Sm.BE));
+    }
+    gabs += gn;
+  }
+  const float absS = group_sum<32>(gabs);
+  if (lane == 0 && absS > A.flag_S) atomicAdd(ctrl + kCtrlPilotFlagged, 1);
+}
+
+__global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot) {
+  // more than a quarter flagged: redoing them after an fp32 pass costs more than one float64-chain pass
+  ctrl[kCtrlMode] = (4 * (int64_t)ctrl[kCtrlPilotFlagged] > n_pilot) ? kModeAllF64 : kModeFastThenList;
 }
 
 }  // namespace synax

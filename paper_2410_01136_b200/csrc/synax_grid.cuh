@@ -191,6 +191,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
         const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
         if (active) emission(P, BN, BE, N0, eI, a, bq);
         const float gn = active ? ne * Bpar : 0.f;
+        if (active) absS = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), absS);
         const float incl = warp_inclusive_scan(gn, lane);
         S_here = carry + (double)(incl - 0.5f * gn);
         carry += warp_sum_d((double)gn);
@@ -203,7 +204,6 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
         S_here = carry + incl - 0.5 * gn;
         carry += warp_bcast_d(incl, 31);
       }
-      absS = fmaxf(absS, fabsf((float)carry));
       accI += eI;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
@@ -214,6 +214,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
       }
     }
     accI = group_sum<32>(accI);
+    absS = group_sum<32>(absS);   // sum n_e (|B_LOS| + |B_N| + |B_E|): scale of the fp32 round-off in the Faraday sum
 #pragma unroll
     for (int f = 0; f < NF; ++f) { accQ[f] = group_sum<32>(accQ[f]); accU[f] = group_sum<32>(accU[f]); }
     if (lane == 0) {
@@ -249,7 +250,7 @@ struct GridVjpArgs {
 };
 
 // Sweep 1 of the gridded adjoint for one sightline (whole warp): per-sample forward quantities, cotangent
-// fan-out (A9) and the per-sample hand-over to sweep 2 through shared memory.  Returns max |sum n_e B_LOS|.
+// fan-out (A9) and the per-sample hand-over to sweep 2 through shared memory.  Returns sum n_e (|B_LOS| + |B_N| + |B_E|).
 template <int NF, bool PRECISE>
 __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const FreqTab& ft, const GridDesc& G,
                                                  const BatchConsts& P, const Triad& T, const double4 dir, int lane,
@@ -278,6 +279,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
       BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
       const float gn = active ? ne * Bpar : 0.f;
+      if (active) absS = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), absS);
       const float incl = warp_inclusive_scan(gn, lane);
       S_here = carry + (double)(incl - 0.5f * gn);
       carry += warp_sum_d((double)gn);
@@ -290,7 +292,6 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       S_here = carry + incl - 0.5 * gn;
       carry += warp_bcast_d(incl, 31);
     }
-    absS = fmaxf(absS, fabsf((float)carry));
     const float bn2 = BN * BN, be2 = BE * BE, Bt2 = bn2 + be2;
     float w = 1.0f;
     if (!P.alpha_is_3) w = (Bt2 > 0.f) ? mufu_ex2(P.q_exp * mufu_lg2(Bt2)) : 0.f;
@@ -317,7 +318,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       st_w[idx] = Sbar; st_n[idx] = BNb; st_e[idx] = BEb; st_d[idx] = ne;
     }
   }
-  return absS;
+  return group_sum<32>(absS);
 }
 
 template <int NF>
@@ -450,7 +451,7 @@ static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const
   ga.f.flag_list = nullptr; ga.f.flag_S = 0.f; ga.f.flag_count = d_flag_count;
   if (escalate) {
     if (cudaMallocAsync((void**)&ga.f.flag_list, sizeof(int) * (size_t)a0.geo.npix, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
-    cudaMemsetAsync(d_flag_count, 0, sizeof(int), st);
+    cudaMemsetAsync(d_flag_count, 0, kCtrlWords * sizeof(int), st);
     ga.f.flag_S = (float)(escalate_rad / (double)k_max);
   }
   const int64_t warps_needed = a0.geo.npix;
@@ -474,7 +475,7 @@ static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const
   }
   const cudaError_t e = cudaGetLastError();
   if (escalate) {
-    cudaMemcpyAsync(h_flag_count, d_flag_count, sizeof(int), cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(h_flag_count, d_flag_count, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
     cudaFreeAsync(ga.f.flag_list, st);
   }
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
