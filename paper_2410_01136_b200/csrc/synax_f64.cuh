@@ -14,24 +14,32 @@
 
 namespace synax {
 
-// 2^x, x <= ~60; relative error < 1e-11 (Taylor in f ln2, |f| <= 1/2, degree 9).  Returns 0 below 2^-1000.
+// Polynomial coefficients live in constant memory so that DFMA takes them as c[bank][offset] operands
+// (a 64-bit literal costs two UMOV issue slots each time it is used).
+__constant__ double kExp2C[9] = {   // ln2^k / k!, k = 9 .. 1
+    1.0178086009239699e-7, 1.3215486790144307e-6, 1.5252733804059841e-5, 1.5403530393381609e-4,
+    1.3333558146428443e-3, 9.6181291076284772e-3, 5.5504108664821580e-2, 2.4022650695910071e-1,
+    6.9314718055994531e-1};
+__constant__ double kSinC[5] = {-2.5052108385441718775e-8, 2.7557319223985890653e-6, -1.9841269841269841270e-4,
+                                8.3333333333333333333e-3, -1.6666666666666666667e-1};
+__constant__ double kCosC[6] = {2.0876756987868098979e-9, -2.7557319223985890653e-7, 2.4801587301587301587e-5,
+                                -1.3888888888888888889e-3, 4.1666666666666666667e-2, -0.5};
+__constant__ double kMiscC[4] = {6755399441055744.0,          // 1.5 * 2^52
+                                 0.63661977236758134308,      // 2/pi
+                                 -1.5707963267948966192,      // -pi/2 hi
+                                 -6.1232339957367658860e-17}; // -pi/2 lo
+
+// 2^x, x <= ~60; relative error < 1e-11 (Taylor in f ln2, |f| <= 1/2, degree 9).  Below 2^-1000 the result is
+// pinned at ~2^-1000 (1e-301), which is zero for every use here.
 __device__ __forceinline__ double exp2_d(double x) {
-  const double kMagic = 6755399441055744.0;  // 1.5 * 2^52
-  const double t = x + kMagic;
-  const int k = __double2loint(t);
-  const double f = x - (t - kMagic);         // exact, |f| <= 1/2
-  double p = 1.0178086009239699e-7;          // ln2^9 / 9!
-  p = fma(p, f, 1.3215486790144307e-6);
-  p = fma(p, f, 1.5252733804059841e-5);
-  p = fma(p, f, 1.5403530393381609e-4);
-  p = fma(p, f, 1.3333558146428443e-3);
-  p = fma(p, f, 9.6181291076284772e-3);
-  p = fma(p, f, 5.5504108664821580e-2);
-  p = fma(p, f, 2.4022650695910071e-1);
-  p = fma(p, f, 6.9314718055994531e-1);
+  const double t = x + kMiscC[0];
+  const int k = max(__double2loint(t), -1000);
+  const double f = x - (t - kMiscC[0]);         // exact, |f| <= 1/2 (garbage but finite when k was clamped)
+  double p = kExp2C[0];
+#pragma unroll
+  for (int i = 1; i < 9; ++i) p = fma(p, f, kExp2C[i]);
   p = fma(p, f, 1.0);
-  const int hi = __double2hiint(p) + (k << 20);
-  return (x < -1000.0) ? 0.0 : __hiloint2double(hi, __double2loint(p));
+  return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
 // 1/x for finite x with |x| in fp32 range: MUFU.RCP seed (1e-7) + one Newton step (-> 1e-14)
@@ -40,34 +48,28 @@ __device__ __forceinline__ double rcp_d(double x) {
   return fma(y, fma(-x, y, 1.0), y);
 }
 
-// 1/sqrt(x) for x > 0 in fp32 range: MUFU.RSQ seed + one Newton step (-> ~4e-15)
+// 1/sqrt(x) for x >= 0 in fp32 range: MUFU.RSQ seed + one Newton step (-> ~4e-15); finite (huge) for x -> 0
 __device__ __forceinline__ double rsqrt_d(double x) {
-  const double y = (double)mufu_rsqrt((float)x);
+  const double y = (double)mufu_rsqrt(fmaxf((float)x, 1.0e-30f));
   const double e = fma(-x * y, y, 1.0);
   return fma(0.5 * y, e, y);
 }
 
 // sin and cos, |x| < ~1e6; absolute error < 1e-11 (reduction by pi/2, odd degree 11 / even degree 12)
 __device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
-  const double kMagic = 6755399441055744.0;
-  const double t = fma(x, 0.63661977236758134308, kMagic);
+  const double t = fma(x, kMiscC[1], kMiscC[0]);
   const int q = __double2loint(t);
-  const double k = t - kMagic;
-  double r = fma(k, -1.5707963267948966192, x);
-  r = fma(k, -6.1232339957367658860e-17, r);
+  const double k = t - kMiscC[0];
+  double r = fma(k, kMiscC[2], x);
+  r = fma(k, kMiscC[3], r);
   const double r2 = r * r;
-  double ps = -2.5052108385441718775e-8;      // -1/11!
-  ps = fma(ps, r2, 2.7557319223985890653e-6);
-  ps = fma(ps, r2, -1.9841269841269841270e-4);
-  ps = fma(ps, r2, 8.3333333333333333333e-3);
-  ps = fma(ps, r2, -1.6666666666666666667e-1);
+  double ps = kSinC[0];
+#pragma unroll
+  for (int i = 1; i < 5; ++i) ps = fma(ps, r2, kSinC[i]);
   ps = fma(ps * r2, r, r);
-  double pc = 2.0876756987868098979e-9;       // 1/12!
-  pc = fma(pc, r2, -2.7557319223985890653e-7);
-  pc = fma(pc, r2, 2.4801587301587301587e-5);
-  pc = fma(pc, r2, -1.3888888888888888889e-3);
-  pc = fma(pc, r2, 4.1666666666666666667e-2);
-  pc = fma(pc, r2, -0.5);
+  double pc = kCosC[0];
+#pragma unroll
+  for (int i = 1; i < 6; ++i) pc = fma(pc, r2, kCosC[i]);
   pc = fma(pc, r2, 1.0);
   const double ss = (q & 1) ? pc : ps;
   const double cs = (q & 1) ? ps : pc;
@@ -95,6 +97,32 @@ __device__ __forceinline__ double log_d(double v) {
   return fma((double)e, 0.69314718055994530942, 2.0 * p);
 }
 
+// N independent 2^x evaluated in lockstep: the compiler emits each Horner chain serially when they sit in
+// different basic blocks (a DFMA depends on the previous one, ~8 cycles apart), so the exponentials of one
+// sample are gathered here and advanced together -- N chains in flight instead of one.
+template <int N>
+__device__ __forceinline__ void exp2_d_n(const double (&x)[N], double (&out)[N]) {
+  double f[N], p[N];
+  int k[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double t = x[j] + kMiscC[0];
+    k[j] = max(__double2loint(t), -1000);
+    f[j] = x[j] - (t - kMiscC[0]);
+    p[j] = kExp2C[0];
+  }
+#pragma unroll
+  for (int i = 1; i < 9; ++i) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) p[j] = fma(p[j], f[j], kExp2C[i]);
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    p[j] = fma(p[j], f[j], 1.0);
+    out[j] = __hiloint2double(__double2hiint(p[j]) + (k[j] << 20), __double2loint(p[j]));
+  }
+}
+
 // Per-batch-element float64 constants of the analytic model (prologue_kernel writes them).
 struct BatchConstsD {
   double b0, psi0, psi1, chi0;
@@ -104,43 +132,128 @@ struct BatchConstsD {
   int psi1_small;         // |psi1| <= 0.05: the MUFU lg2 (abs err 2e-7) is accurate enough for ln(rho/8)
 };
 
-// B (Cartesian, uG) and n_e (cm^-3) at a point, float64 with the short polynomials above.
-// Eq.(12)-(13) P:L173-180 and the halo of DESIGN.md section 3 (S:App.C); `inside` as in the fp32 chain.
-template <bool kHalo>
-__device__ __forceinline__ void eval_analytic_d(const BatchConstsD& D, double x, double y, double z, double rho2,
-                                                bool inside, double& Bx, double& By, double& Bz, double& ne) {
+// M independent sincos in lockstep (same polynomials as sincos_d)
+template <int M>
+__device__ __forceinline__ void sincos_d_n(const double (&x)[M], double (&s)[M], double (&c)[M]) {
+  double r[M], r2[M], ps[M], pc[M];
+  int q[M];
+#pragma unroll
+  for (int j = 0; j < M; ++j) {
+    const double t = fma(x[j], kMiscC[1], kMiscC[0]);
+    q[j] = __double2loint(t);
+    const double k = t - kMiscC[0];
+    r[j] = fma(k, kMiscC[3], fma(k, kMiscC[2], x[j]));
+    r2[j] = r[j] * r[j];
+    ps[j] = kSinC[0]; pc[j] = kCosC[0];
+  }
+#pragma unroll
+  for (int i = 1; i < 6; ++i) {
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      if (i < 5) ps[j] = fma(ps[j], r2[j], kSinC[i]);
+      pc[j] = fma(pc[j], r2[j], kCosC[i]);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < M; ++j) {
+    ps[j] = fma(ps[j] * r2[j], r[j], r[j]);
+    pc[j] = fma(pc[j], r2[j], 1.0);
+    const double ss = (q[j] & 1) ? pc[j] : ps[j];
+    const double cs = (q[j] & 1) ? ps[j] : pc[j];
+    s[j] = (q[j] & 2) ? -ss : ss;
+    c[j] = ((q[j] + 1) & 2) ? -cs : cs;
+  }
+}
+
+// B (Cartesian, uG) and n_e (cm^-3) at M consecutive samples of one sightline, float64 with the short
+// polynomials above.  Eq.(12)-(13) P:L173-180 and the halo of DESIGN.md section 3 (S:App.C); `inside` as in
+// the fp32 chain.  Everything is advanced in lockstep over the M samples and over the independent functions
+// of one sample (the kernel is bound by dependent-issue latency, not by a pipe: ncu "wait" stalls), with two
+// straight-line variants: some sample inside the disc annulus (the others masked) / all outside.
+template <bool kHalo, int M>
+__device__ __forceinline__ void eval_analytic_dm(const BatchConstsD& D, const double (&x)[M], const double (&y)[M],
+                                                 const double (&z)[M], const double (&rho2)[M], const bool (&inside)[M],
+                                                 double (&Bx)[M], double (&By)[M], double (&Bz)[M], double (&ne)[M]) {
   const double kLog2e = 1.4426950408889634074;
-  rho2 = fmax(rho2, 1.0e-30);
-  const double ir = rsqrt_d(rho2);
-  const double rho = rho2 * ir;
-  const double xr = x * ir, yr = y * ir;
-  const double az = fabs(z);
-  double Brho = 0.0, Bphi = 0.0;
-  Bz = 0.0;
-  if (inside) {   // warp-divergent only at the annulus edges
-    const double lr = D.psi1_small ? (double)((mufu_lg2((float)rho2) - 6.0f) * 0.34657359027997264f)
-                                   : 0.5 * log_d(rho2 * 0.015625);
-    double sp, cp, sc, cc;
-    sincos_d(fma(D.psi1, lr, D.psi0), sp, cp);
-    const double e1 = exp2_d(-2.0 * kLog2e * az);               // tanh|z| = (1 - e)/(1 + e)
-    const double th = (1.0 - e1) * rcp_d(1.0 + e1);
-    sincos_d(D.chi0 * copysign(th, z), sc, cc);
-    double A = D.b0;
-    if (D.k_hb != 0.0) A *= exp2_d(D.k_hb * (rho - 8.0));
-    const double Acc = A * cc;
-    Brho = Acc * cp; Bphi = Acc * sp; Bz = A * sc;
+  double ir[M], rho[M], az[M], q[M], u[M];
+  bool any = false;
+#pragma unroll
+  for (int j = 0; j < M; ++j) {
+    ir[j] = rsqrt_d(rho2[j]);
+    rho[j] = rho2[j] * ir[j];
+    az[j] = fabs(z[j]);
+    q[j] = rho[j] * D.inv_rh;
+    u[j] = (az[j] - D.zh0) * D.inv_wh;
+    any = any || inside[j];
   }
-  if (kHalo) {
-    const double u = (az - D.zh0) * D.inv_wh;
-    const double L = rcp_d(fma(u, u, 1.0));
-    const double q = rho * D.inv_rh;
-    Bphi = fma(D.Bh * L, q * exp2_d(kLog2e * (1.0 - q)), Bphi);
+  double Brho[M], Bphi[M], ee[M], er[M], eh[M];
+  if (any) {
+    constexpr int NE = kHalo ? 5 : 3;
+    double xs[NE * M], o[NE * M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      xs[j] = D.k_hez * az[j];
+      xs[M + j] = D.k_her * rho[j];
+      xs[2 * M + j] = -2.0 * kLog2e * az[j];
+      if (kHalo) {
+        xs[3 * M + j] = kLog2e * (1.0 - q[j]);
+        xs[4 * M + j] = D.k_hb * (rho[j] - 8.0);
+      }
+    }
+    exp2_d_n<NE * M>(xs, o);
+    double ang[2 * M], sn[2 * M], cs[2 * M], A[M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      ee[j] = o[j]; er[j] = o[M + j];
+      const double e1 = o[2 * M + j];
+      eh[j] = kHalo ? o[3 * M + j] : 0.0;
+      A[j] = inside[j] ? (kHalo ? D.b0 * o[4 * M + j] : D.b0) : 0.0;
+      const double lr = D.psi1_small ? (double)((mufu_lg2((float)rho2[j]) - 6.0f) * 0.34657359027997264f)
+                                     : 0.5 * log_d(rho2[j] * 0.015625);
+      const double th = (1.0 - e1) * rcp_d(1.0 + e1);           // tanh|z| = (1 - e)/(1 + e)
+      ang[j] = fma(D.psi1, lr, D.psi0);
+      ang[M + j] = D.chi0 * copysign(th, z[j]);
+    }
+    sincos_d_n<2 * M>(ang, sn, cs);
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      const double Acc = A[j] * cs[M + j];
+      Brho[j] = Acc * cs[j]; Bphi[j] = Acc * sn[j]; Bz[j] = A[j] * sn[M + j];
+    }
+  } else {
+    constexpr int NE = kHalo ? 3 : 2;
+    double xs[NE * M], o[NE * M];
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      xs[j] = D.k_hez * az[j];
+      xs[M + j] = D.k_her * rho[j];
+      if (kHalo) xs[2 * M + j] = kLog2e * (1.0 - q[j]);
+    }
+    exp2_d_n<NE * M>(xs, o);
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      ee[j] = o[j]; er[j] = o[M + j];
+      eh[j] = kHalo ? o[2 * M + j] : 0.0;
+      Brho[j] = 0.0; Bphi[j] = 0.0; Bz[j] = 0.0;
+    }
   }
-  Bx = Brho * xr - Bphi * yr;
-  By = fma(Brho, yr, Bphi * xr);
-  const double ee = exp2_d(D.k_hez * az);                       // sech^2 w = 4 e / (1 + e)^2
-  const double de = 1.0 + ee;
-  ne = D.ne0x4 * exp2_d(D.k_her * rho) * ee * rcp_d(de * de);
+#pragma unroll
+  for (int j = 0; j < M; ++j) {
+    const double de = 1.0 + ee[j];                              // sech^2 w = 4 e / (1 + e)^2
+    double ide2;                                                // 1 / (1 + e)^2
+    if (kHalo) {   // one reciprocal serves the halo's Lorentzian and sech^2
+      const double lu = fma(u[j], u[j], 1.0), de2 = de * de;
+      const double inv = rcp_d(lu * de2);
+      ide2 = inv * lu;
+      Bphi[j] = fma(D.Bh * (inv * de2), q[j] * eh[j], Bphi[j]);
+    } else {
+      ide2 = rcp_d(de * de);
+    }
+    const double xr = x[j] * ir[j], yr = y[j] * ir[j];
+    Bx[j] = Brho[j] * xr - Bphi[j] * yr;
+    By[j] = fma(Brho[j], yr, Bphi[j] * xr);
+    ne[j] = D.ne0x4 * er[j] * ee[j] * ide2;
+  }
 }
 
 }  // namespace synax

@@ -8,7 +8,11 @@ namespace synax {
 constexpr int kBlock = 128;   // threads per CTA for the sightline kernels
 constexpr int kTile = 32;     // samples between re-basing of the local Faraday sum
 constexpr int kTileDMax = 16;  // float64-chain kernel: at most this many samples per tile (BatchConsts::tile_d)
-constexpr float kTilePhase = 48.0f;  // ... and at most about this much Faraday angle (rad) inside a tile
+#ifndef SYNAX_UNROLL_D
+#define SYNAX_UNROLL_D 1
+#endif
+constexpr int kUnrollD = SYNAX_UNROLL_D;  // ... samples advanced in lockstep per iteration
+constexpr float kTilePhase = 96.0f;  // ... and at most about this much Faraday angle (rad) inside a tile
 
 enum ModelCode { kAnalyticDisc = 0, kAnalyticFull = 1, kGridB = 2, kUniform = 3 };
 
@@ -139,6 +143,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     const double per_step = kmax * gmax;
     int t = kTileDMax;
     if (per_step * t > (double)kTilePhase) t = (int)((double)kTilePhase / per_step);
+    if (t > kUnrollD) t -= t % kUnrollD;
     c.tile_d = t < 1 ? 1 : t;
   }
   out[b] = c;
@@ -388,7 +393,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
     const int b = (int)(sl / A.geo.npix);
     const int64_t pix = sl - (int64_t)b * A.geo.npix;
     const BatchConsts& P = A.bc[b];
-    const BatchConstsD& D = A.bd[b];
+    const BatchConstsD D = A.bd[b];   // by value: kept in registers across the sample loop
     const Triad T = load_triad(A.geo.dirs, pix);
     double s_d = ((double)n0 + 0.5) * delta;
     float accI = 0.0f, accQ[NF], accU[NF];
@@ -402,41 +407,59 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
       float tq[NF], tu[NF];
 #pragma unroll
       for (int f = 0; f < NF; ++f) { tq[f] = 0.0f; tu[f] = 0.0f; }
-      for (int n = ts; n < te; ++n) {
-        const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
-        const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
-        const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
-        s_d += delta;
-        double Bx, By, Bz, ne;
-        float N0;
-        if (CODE == kUniform) {
-          Bx = (double)P.uB[0]; By = (double)P.uB[1]; Bz = (double)P.uB[2]; ne = (double)P.une; N0 = P.uN0;
-        } else {
-          const double rho2d = fma(xd, xd, yd * yd);
-          const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
-          eval_analytic_d<CODE == kAnalyticFull>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
-          // N_0 (emission only): fp32 MUFU chain, Eq.(12)
-          const float rho2f = fmaxf((float)rho2d, 1.0e-30f);
-          const float rho = rho2f * mufu_rsqrt(rho2f);
-          const float ez = mufu_ex2(P.k_hz * fabsf((float)zd));
-          const float dz = 1.0f + ez;
-          N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
-        }
-        const double gn = ne * fma(Bx, T.nxd, fma(By, T.nyd, Bz * T.nzd));   // n_e B.n, signed (S:C-2#3)
-        const float ph = (float)fma(0.5, gn, S_loc - S_tile);                  // half-cell (S:C-2#5), tile-local
-        S_loc += gn;
-        const float bx = (float)Bx, by = (float)By, bz = (float)Bz;
-        const float BN = fmaf(bx, T.eNx, fmaf(by, T.eNy, bz * T.eNz));
-        const float BE = fmaf(bx, T.eEx, by * T.eEy);
-        float eI, a, bq;
-        emission(P, BN, BE, N0, eI, a, bq);
-        accI += eI;
+      for (int n = ts; n < te; n += kUnrollD) {
+        // kUnrollD consecutive samples advanced together (latency hiding); those past the tile end are computed
+        // at harmless positions and masked out
+        double xd[kUnrollD], yd[kUnrollD], zd[kUnrollD], rho2d[kUnrollD], Bx[kUnrollD], By[kUnrollD], Bz[kUnrollD],
+            ne[kUnrollD];
+        bool inside[kUnrollD], live[kUnrollD];
+        float N0[kUnrollD];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) {
-          const float th = k_rad[f] * ph;
-          const float c = mufu_cos(th), s = mufu_sin(th);
-          tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
-          tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+        for (int j = 0; j < kUnrollD; ++j) {
+          live[j] = n + j < te;
+          xd[j] = fma(s_d, T.nxd, A.geo.obs[0]);
+          yd[j] = fma(s_d, T.nyd, A.geo.obs[1]);
+          zd[j] = fma(s_d, T.nzd, A.geo.obs[2]);
+          if (live[j]) s_d += delta;
+          rho2d[j] = fma(xd[j], xd[j], yd[j] * yd[j]);
+          inside[j] = (rho2d[j] > 9.0) && (rho2d[j] < 400.0);
+        }
+        if (CODE == kUniform) {
+#pragma unroll
+          for (int j = 0; j < kUnrollD; ++j) {
+            Bx[j] = (double)P.uB[0]; By[j] = (double)P.uB[1]; Bz[j] = (double)P.uB[2]; ne[j] = (double)P.une; N0[j] = P.uN0;
+          }
+        } else {
+          eval_analytic_dm<CODE == kAnalyticFull, kUnrollD>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
+#pragma unroll
+          for (int j = 0; j < kUnrollD; ++j) {
+            // N_0 (emission only): fp32 MUFU chain, Eq.(12)
+            const float rho2f = fmaxf((float)rho2d[j], 1.0e-30f);
+            const float rho = rho2f * mufu_rsqrt(rho2f);
+            const float ez = mufu_ex2(P.k_hz * fabsf((float)zd[j]));
+            const float dz = 1.0f + ez;
+            N0[j] = 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < kUnrollD; ++j) {
+          double gn = ne[j] * fma(Bx[j], T.nxd, fma(By[j], T.nyd, Bz[j] * T.nzd));   // n_e B.n, signed (S:C-2#3)
+          if (!live[j]) gn = 0.0;
+          const float ph = (float)fma(0.5, gn, S_loc - S_tile);                  // half-cell (S:C-2#5), tile-local
+          S_loc += gn;
+          const float bx = (float)Bx[j], by = (float)By[j], bz = (float)Bz[j];
+          const float BN = fmaf(bx, T.eNx, fmaf(by, T.eNy, bz * T.eNz));
+          const float BE = fmaf(bx, T.eEx, by * T.eEy);
+          float eI, a, bq;
+          emission(P, BN, BE, live[j] ? N0[j] : 0.0f, eI, a, bq);
+          accI += eI;
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            const float th = k_rad[f] * ph;
+            const float c = mufu_cos(th), s = mufu_sin(th);
+            tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
+            tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+          }
         }
       }
 #pragma unroll
