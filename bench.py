@@ -205,18 +205,22 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True):
+def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False):
     """Device-resident timing of forward and VJP with CUDA events on the launching stream, L2 flushed between
-    timed calls; then (optionally) the host-buffer entry points."""
-    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer)
+    timed calls; then (optionally) the host-buffer entry points.  pix_range: this rank's pixel shard (strong
+    scaling), with the one gradient all-reduce of the method inside the timed VJP when reduce_grad is set."""
+    from paper_2410_01136_b200 import sharding
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
+    npix = plan.npix
+    p0 = 0 if pix_range is None else pix_range[0]
     if w.kind == "grid_b":
         model = sx.Model("grid_b", aux=w.aux, grid_shape=w.params.shape[:3], box=w.box)
     else:
         model = sx.Model(w.kind, aux=w.aux)
     params = torch.from_numpy(w.params).cuda().contiguous()
-    cots_h = w.cotangents()
+    cots_h = tuple(np.ascontiguousarray(c[..., p0:p0 + npix]) for c in w.cotangents())
     cots = [torch.from_numpy(c).cuda() for c in cots_h]
-    out = tuple(torch.empty((w.batch, w.n_freq, w.npix), dtype=torch.float32, device="cuda") for _ in range(3))
+    out = tuple(torch.empty((w.batch, w.n_freq, npix), dtype=torch.float32, device="cuda") for _ in range(3))
     grad = torch.empty_like(params)
     stream = torch.cuda.current_stream()
 
@@ -225,6 +229,7 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True):
         sx.forward(plan, model, params, out=out)
         if ev: ev[1].record(stream)
         sx.vjp(plan, model, params, *cots, out=grad)
+        if reduce_grad: sharding.reduce_gradient(grad)
         if ev: ev[2].record(stream)
 
     for _ in range(warmup):
@@ -245,13 +250,17 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True):
     if want_e2e:
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
         hp = pin(w.params); hc = [pin(c) for c in cots_h]
-        ho = tuple(torch.empty((w.batch, w.n_freq, w.npix), dtype=torch.float32).pin_memory() for _ in range(3))
+        ho = tuple(torch.empty((w.batch, w.n_freq, npix), dtype=torch.float32).pin_memory() for _ in range(3))
         hg = torch.empty(w.params.shape, dtype=torch.float32).pin_memory()
         npv = lambda t: t.numpy()  # noqa: E731
 
         def host_step():
             sx.forward_host(plan, model, npv(hp), out=tuple(npv(t) for t in ho))
             sx.vjp_host(plan, model, npv(hp), *[npv(c) for c in hc], out=npv(hg))
+            if reduce_grad:
+                gd = hg.cuda(non_blocking=True)
+                sharding.reduce_gradient(gd)
+                hg.copy_(gd)
 
         n_e2e = max(3, min(steps, 10))
         for _ in range(2):
@@ -279,7 +288,15 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", torch.cuda.current_device()))
     import paper_2410_01136_b200 as sx
     sx.load_library()                       # fails loudly when libsynax.so is missing
-    w = rank_workload(args.config, rank)
+    strong = args.scaling == "strong" and world > 1
+    pix_range = None
+    if strong:      # one map, pixel shards, one gradient all-reduce per step
+        from paper_2410_01136_b200 import sharding, workloads as wl
+        w = wl.config(args.config)
+        pix_range = sharding.shard_of(w.npix, rank, world)
+    else:           # independent chains: every rank integrates the whole sky for its own parameter vector
+        w = rank_workload(args.config, rank)
+    kw = dict(pix_range=pix_range, reduce_grad=strong)
     flush_buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
 
     def barrier():
@@ -288,49 +305,59 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # untimed first touch (context, module load)
-    time_config(sx, torch, w, 1, 1, flush_buf, want_e2e=False)
+    time_config(sx, torch, w, 1, 1, flush_buf, want_e2e=False, **kw)
     barrier()
     sampler = ClockSampler(torch.cuda.current_device())
     if rank == 0:
         sampler.start()
     barrier()
-    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False)
+    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False, **kw)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
-    e = time_config(sx, torch, w, min(args.steps, 5), 1, flush_buf, want_e2e=True)
+    e = time_config(sx, torch, w, min(args.steps, 5), 1, flush_buf, want_e2e=True, **kw)
     t_step = r["t_fwd"] + r["t_vjp"]
     vals = torch.tensor([t_step, r["t_fwd"], r["t_vjp"], e["t_e2e"]], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(vals, op=dist.ReduceOp.MAX)
     t_step, t_fwd, t_vjp, t_e2e = (float(v) for v in vals.cpu())
-    samples = w.los_samples
+    samples = w.los_samples                 # per rank (weak) or of the whole map (strong)
+    local_samples = samples if not strong else pix_range[1] * w.n_los * w.batch
+    total = samples if strong else world * samples
     line = None
     if rank == 0:
         sm_max, peak_src = peaks()
         peak = SM_COUNT * FP32_LANES * sm_max * 1e6 / 1e12       # T lane-instr/s
         fp_vjp = alg_fp(w.kind, w.n_freq, "vjp")
         fp_fwd = alg_fp(w.kind, w.n_freq, "fwd")
-        achieved = fp_vjp * samples / r["t_vjp"] / 1e12
+        achieved = fp_vjp * local_samples / r["t_vjp"] / 1e12
+        traffic = None
+        tcsv = ROOT / "profiles" / "r01_dram_traffic.csv"
+        if tcsv.exists() and w.name.startswith("cfg4") and not strong:
+            for row in tcsv.read_text().splitlines()[1:]:
+                c = row.split(",")
+                if c[0] == "vjp_kernel":
+                    traffic = int(c[1]) + int(c[2])
         line = {
-            "metric": METRIC, "value": world * samples / t_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
+            "metric": METRIC, "value": total / t_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "strong" if strong else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, workloads.py)",
             "config": {"workload": w.name, "nside": w.nside, "n_los": w.n_los, "n_freq": w.n_freq, "batch": w.batch,
                        "model": w.kind, "samples_per_step": samples, "l2": "flushed between timed steps (256 MB write)",
-                       "parallelism": f"independent parameter vectors x{world}" if world > 1 else "single GPU"},
-            "forward_samples_per_s": world * samples / t_fwd, "vjp_samples_per_s": world * samples / t_vjp,
+                       "parallelism": ("single GPU" if world == 1 else f"pixel shards x{world} + gradient all-reduce" if strong
+                                       else f"independent parameter vectors x{world}")},
+            "forward_samples_per_s": total / t_fwd, "vjp_samples_per_s": total / t_vjp,
             "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,
-            "sample_freq_per_s": world * samples * w.n_freq / t_step,
-            "e2e": {"value": world * samples / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
+            "sample_freq_per_s": total * w.n_freq / t_step,
+            "e2e": {"value": total / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
                     "ms_per_step": 1e3 * t_e2e},
             "gpu_launches": r["launches"], "escalated_sightlines": r["escalated"],
             "clocks": clocks,
             "roofline": {"bound": "alu", "kernel": "vjp_kernel (analytic adjoint)" if w.kind != "grid_b" else "grid_vjp_kernel",
                          "achieved": achieved, "peak": peak, "unit": "T fp32 lane-instr/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": f"148 SM x 128 FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
+                         "traffic": traffic, "peak_source": f"148 SM x 128 FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
                          "alg_fp32_per_sample": fp_vjp, "forward": {"alg_fp32_per_sample": fp_fwd,
-                                                                    "achieved": fp_fwd * samples / r["t_fwd"] / 1e12,
-                                                                    "frac": fp_fwd * samples / r["t_fwd"] / 1e12 / peak}},
+                                                                    "achieved": fp_fwd * local_samples / r["t_fwd"] / 1e12,
+                                                                    "frac": fp_fwd * local_samples / r["t_fwd"] / 1e12 / peak}},
         }
         if clocks and clocks.get("sm_mhz"):
             line["roofline"]["frac_at_sustained_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
@@ -353,6 +380,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: the metric's workload)")
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--scaling", choices=("weak", "strong"), default="weak",
+                    help="N > 1: weak = one parameter vector (chain) per rank, no collective; strong = pixel shards of one map "
+                         "+ one gradient all-reduce per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline oracle sample")
     args = ap.parse_args()

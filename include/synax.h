@@ -75,8 +75,15 @@ typedef struct {
  * there (step A1) and returns after that kernel finished. */
 synax_status synax_plan_create(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
                                int32_t n_freq, const double observer_kpc[3], synax_plan** out);
+/* The same for a shard of the sky: RING pixels pix_begin .. pix_begin + pix_count - 1 only (sightlines are
+ * independent).  Every map / cotangent buffer of this plan then has pix_count pixels
+ * per (batch, frequency), and synax_vjp returns the shard's partial gradient (sum over its pixels): summing
+ * the partial gradients of disjoint shards that cover the map gives the gradient of the whole map. */
+synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
+                                     int32_t n_freq, const double observer_kpc[3], int64_t pix_begin,
+                                     int64_t pix_count, synax_plan** out);
 synax_status synax_plan_destroy(synax_plan* plan); /* NULL is allowed */
-int64_t synax_plan_npix(const synax_plan* plan);  /* 12 nside^2, or -1 for NULL */
+int64_t synax_plan_npix(const synax_plan* plan);  /* pixels of this plan (12 nside^2 unless a shard), -1 for NULL */
 
 /* Options (tests / experiments).  key "precision": 0 = auto (default: fp32 pass, sightlines whose
  * Faraday rotation angle exceeds "escalate_rad" are redone with a float64 Faraday chain),

@@ -18,7 +18,7 @@ STATUS = {0: "SYNAX_OK", 1: "SYNAX_ERR_INVALID_ARG", 2: "SYNAX_ERR_UNSUPPORTED",
 KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
 
 # every symbol include/synax.h declares
-exported_symbols = ("synax_plan_create", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_option",
+exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_option",
                     "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
@@ -50,6 +50,9 @@ def load_library() -> ctypes.CDLL:
     vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
     L.synax_plan_create.argtypes = [i32, i32, dbl, ctypes.POINTER(dbl), i32, ctypes.POINTER(dbl), ctypes.POINTER(vp)]
     L.synax_plan_create.restype = ctypes.c_int
+    L.synax_plan_create_shard.argtypes = [i32, i32, dbl, ctypes.POINTER(dbl), i32, ctypes.POINTER(dbl), i64, i64,
+                                          ctypes.POINTER(vp)]
+    L.synax_plan_create_shard.restype = ctypes.c_int
     L.synax_plan_destroy.argtypes = [vp]
     L.synax_plan_destroy.restype = ctypes.c_int
     L.synax_plan_npix.argtypes = [vp]
@@ -99,9 +102,9 @@ class Model:
 
 
 class Plan:
-    """synax_plan_create / synax_plan_destroy."""
+    """synax_plan_create / synax_plan_create_shard (pix_range=(begin, count)) / synax_plan_destroy."""
 
-    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006)):
+    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006), pix_range=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("synax needs a CUDA device (B200); there is no CPU fallback")
@@ -111,8 +114,13 @@ class Plan:
         f = np.ascontiguousarray(np.asarray(freqs, dtype=np.float64).ravel())
         o = np.ascontiguousarray(np.asarray(observer, dtype=np.float64).ravel())
         h = ctypes.c_void_p()
-        _check(L.synax_plan_create(int(nside), int(n_los), float(s_max), f.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
-                                   int(f.size), o.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), ctypes.byref(h)))
+        fp, op = f.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), o.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        if pix_range is None:
+            _check(L.synax_plan_create(int(nside), int(n_los), float(s_max), fp, int(f.size), op, ctypes.byref(h)))
+        else:
+            _check(L.synax_plan_create_shard(int(nside), int(n_los), float(s_max), fp, int(f.size), op,
+                                             int(pix_range[0]), int(pix_range[1]), ctypes.byref(h)))
+        self.pix_range = None if pix_range is None else (int(pix_range[0]), int(pix_range[1]))
         self.h = h
         self.nside, self.n_los, self.s_max, self.freqs = int(nside), int(n_los), float(s_max), f
         self.n_freq = int(f.size)

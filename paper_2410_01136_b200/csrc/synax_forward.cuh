@@ -27,9 +27,12 @@ __device__ __forceinline__ int64_t isqrt_i64(int64_t v) {
   return r;
 }
 
-__global__ void pix2ang_kernel(int64_t nside, int64_t npix, double* __restrict__ dirs) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= npix) return;
+// Writes dirs[i] for the `count` pixels p = pix0 + i of the nside map (a plan may hold a shard of the sky).
+__global__ void pix2ang_kernel(int64_t nside, int64_t pix0, int64_t count, double* __restrict__ dirs) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= count) return;
+  const int64_t p = pix0 + idx;
+  const int64_t npix = 12 * nside * nside;
   const int64_t ncap = 2 * nside * (nside - 1);
   double z, phi, omz;  // omz = 1 - |z| kept separately for accurate cos b near the poles
   if (p < ncap) {
@@ -57,7 +60,7 @@ __global__ void pix2ang_kernel(int64_t nside, int64_t npix, double* __restrict__
   double sl, cl;
   sincos(phi, &sl, &cl);
   const double cb = sqrt(omz * (1.0 + fabs(z)));  // sin(theta) = sqrt((1-|z|)(1+|z|))
-  dirs[4 * p + 0] = cl; dirs[4 * p + 1] = sl; dirs[4 * p + 2] = cb; dirs[4 * p + 3] = z;
+  dirs[4 * idx + 0] = cl; dirs[4 * idx + 1] = sl; dirs[4 * idx + 2] = cb; dirs[4 * idx + 3] = z;
 }
 
 // ------------------------------------------------------------------------------------------------

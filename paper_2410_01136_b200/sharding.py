@@ -1,0 +1,64 @@
+"""Multi-GPU sharding of the line-of-sight path.
+
+Sightlines are independent, so a map shards by contiguous RING pixel ranges with no
+exchange in the forward pass; the VJP of a shard is the partial gradient over its pixels, and the only
+data-path collective of the whole method is ONE sum all-reduce of `grad` (batch x P floats, or the
+6.3 MB grid gradient).  This module holds the host-side logic only -- the partition and the
+collective call (torch.distributed: NCCL over NVLink on GPUs, gloo in the CPU tests).  No method
+arithmetic lives here.
+"""
+from __future__ import annotations
+
+from typing import List, Tuple
+
+
+def pixel_shards(npix: int, world_size: int) -> List[Tuple[int, int]]:
+    """Contiguous, balanced (begin, count) ranges covering 0..npix-1; the first npix % world ranks get one more.
+    Ranks beyond npix (world_size > npix) get an empty range (count 0) and must skip the call."""
+    if npix < 1 or world_size < 1:
+        raise ValueError("npix and world_size must be >= 1")
+    base, extra = divmod(npix, world_size)
+    out, begin = [], 0
+    for r in range(world_size):
+        count = base + (1 if r < extra else 0)
+        out.append((begin, count))
+        begin += count
+    return out
+
+
+def shard_of(npix: int, rank: int, world_size: int) -> Tuple[int, int]:
+    if not 0 <= rank < world_size:
+        raise ValueError("rank out of range")
+    return pixel_shards(npix, world_size)[rank]
+
+
+def batch_shards(batch: int, world_size: int) -> List[Tuple[int, int]]:
+    """The same partition over batch elements (independent parameter vectors / HMC chains): no collective at all."""
+    return pixel_shards(batch, world_size) if batch >= world_size else \
+        [(r, 1) if r < batch else (batch, 0) for r in range(world_size)]
+
+
+def reduce_gradient(grad, group=None):
+    """Sum the partial gradients of the pixel shards in place on every rank (one all-reduce).  `grad` is a torch
+    tensor on the device the process group communicates on (CUDA for NCCL, CPU for gloo)."""
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(grad, op=dist.ReduceOp.SUM, group=group)
+    return grad
+
+
+def gather_maps(local_map, npix: int, group=None):
+    """Optional: assemble the full [batch][n_freq][npix] map on every rank from the shards' [batch][n_freq][count]
+    slices (all_gather of equal-size padded slices; 75 MB at cfg 4).  Not needed by the VJP."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
+        return local_map
+    world = dist.get_world_size(group)
+    shards = pixel_shards(npix, world)
+    width = max(c for _, c in shards)
+    pad = torch.zeros(local_map.shape[:-1] + (width,), dtype=local_map.dtype, device=local_map.device)
+    pad[..., :local_map.shape[-1]] = local_map
+    parts = [torch.empty_like(pad) for _ in range(world)]
+    dist.all_gather(parts, pad, group=group)
+    return torch.cat([p[..., :c] for p, (_, c) in zip(parts, shards)], dim=-1)

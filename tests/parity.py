@@ -25,10 +25,10 @@ def oracle_vjp(w: wl.Workload, cots, pix=None):
     return oracle.vjp(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, *cots, observer=w.observer, pix=pix)
 
 
-def gpu_objects(w: wl.Workload, **options):
+def gpu_objects(w: wl.Workload, pix_range=None, **options):
     import torch
     import paper_2410_01136_b200 as sx
-    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer)
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
     for k, v in options.items():
         plan.set_option(k, v)
     if w.kind == "grid_b":
