@@ -93,7 +93,7 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   p->npix = pix_count; p->pix0 = pix_begin;
   p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los;
   for (int i = 0; i < 3; ++i) p->obs[i] = observer_kpc[i];
-  p->precision = 0; p->escalate_rad = 50.0; p->lanes = 0;
+  p->precision = 0; p->escalate_rad = 100.0; p->lanes = 0;
   const double KF = faraday_K_per_kpc();
   p->ft.n_freq = n_freq;
   for (int f = 0; f < kMaxFreq; ++f) {
@@ -222,7 +222,8 @@ static int next_freq_block(int remaining) {
 }
 
 template <int CODE, int G>
-static void launch_forward_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+static void launch_forward_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
+  const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
     case 1: forward_kernel<CODE, G, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
     case 2: forward_kernel<CODE, G, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
@@ -239,7 +240,8 @@ static void launch_forward(int G, int nf, int64_t n_sl, cudaStream_t st, const F
   else launch_forward_nf<CODE, 32>(nf, blocks, st, a, ft);
 }
 template <int CODE, int G>
-static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
+static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
+  const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
     case 1: forward_f64_kernel<CODE, G, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
     case 2: forward_f64_kernel<CODE, G, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;

@@ -115,6 +115,17 @@ struct FreqTab {
   double freq[kMaxFreq];
 };
 
+// the table of one frequency pass: entries f0 .. f0 + n - 1 moved to the front, so that the kernels index it with
+// compile-time constants (k_rad[f], k_turn[f] become constant-bank operands instead of registers)
+static inline FreqTab shift_freqs(const FreqTab& ft, int f0) {
+  FreqTab o = ft;
+  for (int f = 0; f < kMaxFreq; ++f) {
+    const int g = f0 + f < kMaxFreq ? f0 + f : kMaxFreq - 1;
+    o.k_rad[f] = ft.k_rad[g]; o.k_turn[f] = ft.k_turn[g]; o.freq[f] = ft.freq[g];
+  }
+  return o;
+}
+
 struct Geometry {
   int64_t npix;
   int n_los;
@@ -164,7 +175,8 @@ struct AnalyticAux {
   float thz, thez;         // tanh(z/h_z), tanh(z/h_ez)
 };
 
-template <bool kHalo, bool kAcc = false>
+// kFastTrig: sin/cos of the pitch and tilt angles on the MUFU (abs err 5e-7: enough for the 1e-3 gradient bound)
+template <bool kHalo, bool kAcc = false, bool kFastTrig = false>
 __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Triad& T, float x, float y,
                                                   float z, float rho2, bool inside, SampleF& S,
                                                   AnalyticAux& a) {
@@ -184,7 +196,7 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
   // --- disc: B = A [cos psi cos chi rho_hat + sin psi cos chi phi_hat + sin chi z_hat]   Eq.(13)
   a.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;        // ln(rho/8) = ln2/2 (lg2 rho^2 - 6)
   const float psi = fmaf(P.p[2], a.lr, P.p[1]);
-  sincos_fma(psi, a.sp, a.cp);
+  if (kFastTrig) { a.sp = mufu_sin(psi); a.cp = mufu_cos(psi); } else sincos_fma(psi, a.sp, a.cp);
   if (kAcc) {
     const float e1 = exp2_fma(-2.0f * kLog2e * az);             // tanh(|z|) = (1-e)/(1+e)
     a.t = copysignf((1.0f - e1) * rcp_nr(1.0f + e1), z);
@@ -193,7 +205,7 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
     a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
   }
   const float chi = P.p[3] * a.t;
-  sincos_fma(chi, a.sc, a.cc);
+  if (kFastTrig) { a.sc = mufu_sin(chi); a.cc = mufu_cos(chi); } else sincos_fma(chi, a.sc, a.cc);
   float rad = 1.0f;
   if (P.k_hb != 0.0f) {
     const float dr = a.rho - 8.0f;

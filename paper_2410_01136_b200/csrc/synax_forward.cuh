@@ -5,6 +5,9 @@
 
 namespace synax {
 
+#ifndef SYNAX_FAST_ACC
+#define SYNAX_FAST_ACC false
+#endif
 constexpr int kBlock = 128;   // threads per CTA for the sightline kernels
 constexpr int kTile = 32;     // samples between re-basing of the local Faraday sum
 constexpr int kTileDMax = 16;  // float64-chain kernel: at most this many samples per tile (BatchConsts::tile_d)
@@ -267,7 +270,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 
   float k_rad[NF];
 #pragma unroll
-  for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[A.f0 + f];
+  for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[f];
 
   float accI = 0.0f, accQ[NF], accU[NF];
 #pragma unroll
@@ -297,7 +300,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         const double rho2d = fma(xd, xd, yd * yd);
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
       float eI, a, bq;
       emission(P, S.BN, S.BE, S.N0, eI, a, bq);
@@ -324,7 +327,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
     } else {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        rotate_by_offset(ft.k_turn[A.f0 + f], carry, tq[f], tu[f]);
+        rotate_by_offset(ft.k_turn[f], carry, tq[f], tu[f]);
         accQ[f] += tq[f]; accU[f] += tu[f];
       }
     }
@@ -337,7 +340,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
     const double off = group_exclusive_scan<G>(carry, g);
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
-      if (g > 0) rotate_by_offset(ft.k_turn[A.f0 + f], off, accQ[f], accU[f]);
+      if (g > 0) rotate_by_offset(ft.k_turn[f], off, accQ[f], accU[f]);
       accQ[f] = group_sum<G>(accQ[f]);
       accU[f] = group_sum<G>(accU[f]);
     }
@@ -386,7 +389,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
   const double delta = A.geo.delta;
   float k_rad[NF];
 #pragma unroll
-  for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[A.f0 + f];
+  for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[f];
 
   for (int64_t it = tid / G;; it += n_groups) {
     if (it - ((threadIdx.x & 31) / G) >= count) break;   // first group of this warp: warp-uniform exit
@@ -467,7 +470,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
       }
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        rotate_by_offset(ft.k_turn[A.f0 + f], S_tile, tq[f], tu[f]);
+        rotate_by_offset(ft.k_turn[f], S_tile, tq[f], tu[f]);
         accQ[f] += tq[f]; accU[f] += tu[f];
       }
     }
@@ -475,7 +478,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
       const double off = group_exclusive_scan<G>(S_loc, g);
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        rotate_by_offset(ft.k_turn[A.f0 + f], off, accQ[f], accU[f]);
+        rotate_by_offset(ft.k_turn[f], off, accQ[f], accU[f]);
         accQ[f] = group_sum<G>(accQ[f]);
         accU[f] = group_sum<G>(accU[f]);
       }

@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         float c, s;
-        faraday_sincos(ft.k_turn[A.f0 + f], S_here, c, s);
+        faraday_sincos(ft.k_turn[f], S_here, c, s);
         accQ[f] = fmaf(a, c, fmaf(-bq, s, accQ[f]));
         accU[f] = fmaf(a, s, fmaf(bq, c, accU[f]));
       }
@@ -301,7 +301,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       float cc, ss;
-      faraday_sincos(ft.k_turn[A.f0 + f], S_here, cc, ss);
+      faraday_sincos(ft.k_turn[f], S_here, cc, ss);
       const float u = fmaf(cQ[f], cc, cU[f] * ss);
       const float v = fmaf(cU[f], cc, -cQ[f] * ss);
       Xc += u; Xs += v;
@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
       cI = fmaf(A.dI ? __ldg(A.dI + o) : 0.f, P.coefI[A.f0 + f], cI);
       cQ[f] = (A.dQ ? __ldg(A.dQ + o) : 0.f) * P.coefP[A.f0 + f];
       cU[f] = (A.dU ? __ldg(A.dU + o) : 0.f) * P.coefP[A.f0 + f];
-      kr[f] = ft.k_rad[A.f0 + f];
+      kr[f] = ft.k_rad[f];
     }
     // ---- sweep 1: consecutive samples per lane; fp32 chain first, redone with the float64 Faraday chain
     // when the rotation angle of this sightline is large (warp-uniform decision)
@@ -430,7 +430,8 @@ static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
 }
 
 template <bool PRECISE>
-static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft) {
+static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft0) {
+  const FreqTab ft = shift_freqs(ft0, a.f.f0);
   switch (nf) {
     case 1: grid_forward_kernel<1, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
     case 2: grid_forward_kernel<2, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
@@ -503,7 +504,7 @@ static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const Batch
 #define SYNAX_GV(NFV)                                                                                      \
   do {                                                                                                     \
     cudaFuncSetAttribute(grid_vjp_kernel<NFV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
-    grid_vjp_kernel<NFV><<<blocks, kBlock, smem, st>>>(a, ft);                                             \
+    grid_vjp_kernel<NFV><<<blocks, kBlock, smem, st>>>(a, shift_freqs(ft, a.f0));                                          \
   } while (0)
     switch (nf) {
       case 1: SYNAX_GV(1); break;

@@ -156,15 +156,13 @@ __global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ Vjp
   const double delta = A.geo.delta;
 
   // cotangents of this sightline, coefficients folded in (zero for padded lanes)
-  float cI = 0.f, cQ[NF], cU[NF], kr[NF];
+  // (dQ, dU are re-read at every tile start -- L1 hits -- instead of being held in 2 NF registers)
+  float cI = 0.f;
+  const int64_t o0 = ((int64_t)b * A.n_freq_total + A.f0) * A.geo.npix + pix;
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
-    const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * A.geo.npix + pix;
-    const float vI = (valid && A.dI) ? A.dI[o] : 0.f;
-    cQ[f] = (valid && A.dQ) ? A.dQ[o] * P.coefP[A.f0 + f] : 0.f;
-    cU[f] = (valid && A.dU) ? A.dU[o] * P.coefP[A.f0 + f] : 0.f;
+    const float vI = (valid && A.dI) ? A.dI[o0 + f * A.geo.npix] : 0.f;
     cI = fmaf(vI, P.coefI[A.f0 + f], cI);
-    kr[f] = ft.k_rad[A.f0 + f];
   }
 
   // ---- pre-pass (G > 1): Faraday sum of each lane's chunk -> float64 offset of the preceding lanes
@@ -184,7 +182,7 @@ __global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ Vjp
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
+        eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
       }
       const float gn = S.ne * S.Bpar;
@@ -215,8 +213,9 @@ __global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ Vjp
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       // Qb cos(tb + tl) + Ub sin(tb + tl) = Qb' cos tl + Ub' sin tl,  Qb' = Qb cb + Ub sb, Ub' = -Qb sb + Ub cb
-      float q = cQ[f], u = cU[f];
-      rotate_by_offset(-ft.k_turn[A.f0 + f], off + carry, q, u);
+      float q = (valid && A.dQ) ? __ldg(A.dQ + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] : 0.f;
+      float u = (valid && A.dU) ? __ldg(A.dU + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] : 0.f;
+      rotate_by_offset(-ft.k_turn[f], off + carry, q, u);
       rq[f] = q; ru[f] = u;
     }
     float hi = 0.f, lo = 0.f;
@@ -235,7 +234,7 @@ __global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ Vjp
         S.N0 = P.uN0; S.ne = P.une;
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
-        eval_analytic_f32<CODE == kAnalyticFull>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
+        eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
       }
       // emission terms
@@ -259,12 +258,12 @@ __global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ Vjp
       float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        const float th = kr[f] * ph;
+        const float th = ft.k_rad[f] * ph;
         const float c = mufu_cos(th), s = mufu_sin(th);
         const float u = fmaf(rq[f], c, ru[f] * s);
         const float v = fmaf(ru[f], c, -rq[f] * s);
         Xc += u; Xs += v;
-        Yc = fmaf(kr[f], u, Yc); Ys = fmaf(kr[f], v, Ys);
+        Yc = fmaf(ft.k_rad[f], u, Yc); Ys = fmaf(ft.k_rad[f], v, Ys);
         if (kAlpha) pq[f] = fmaf(a, u, fmaf(bq, v, pq[f]));
       }
       // L_n = M K,  K = cI Bt2 + Xc d2 + Xs p2
@@ -277,7 +276,8 @@ __global__ void __launch_bounds__(kBlock) vjp_kernel(const __grid_constant__ Vjp
       Pl += Sbar;
       const float wgt = fmaf(-0.5f, Sbar, Pl);
       // B_N, B_E cotangents (direct): from M, d2, p2, Bt2 and the (B_perp^2)^q factor
-      const float tq_ = (Bt2 > 0.f) ? P.q_exp * MK / Bt2 : 0.f;  // d/dBt2 through w
+      float tq_ = 0.f;                                             // d/dBt2 through w (alpha != 3 only)
+      if (!P.alpha_is_3 && Bt2 > 0.f) tq_ = P.q_exp * MK * mufu_rcp(Bt2);
       const float BEb = 2.0f * fmaf(M, fmaf(S.BE, cI + Xc, S.BN * Xs), S.BE * tq_);
       const float BNb = 2.0f * fmaf(M, fmaf(S.BN, cI - Xc, S.BE * Xs), S.BN * tq_);
       if constexpr (CODE == kUniform) acc.add(T, S, BNb, BEb, wgt, MK);
@@ -353,7 +353,8 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_block
 }
 
 template <int CODE, int G>
-static void launch_vjp_nf(int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
+static void launch_vjp_nf(int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft0) {
+  const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
     case 1: vjp_kernel<CODE, G, 1><<<grid, kBlock, 0, st>>>(a, ft); break;
     case 2: vjp_kernel<CODE, G, 2><<<grid, kBlock, 0, st>>>(a, ft); break;
