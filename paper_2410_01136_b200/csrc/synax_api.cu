@@ -394,18 +394,21 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   BatchConsts* bc = nullptr;
+  BatchConstsD* bd = nullptr;
   CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
+  if (code == kGridB) CUDA_TRY(cudaMallocAsync((void**)&bd, sizeof(BatchConstsD) * (size_t)batch, st));
   prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
-                                                      make_aux(model), plan->ft, plan->delta, bc, nullptr);
+                                                      make_aux(model), plan->ft, plan->delta, bc, bd);
   plan->launches++;
   synax_status rs;
   if (code == kGridB)
-    rs = grid_vjp(plan->ft, make_geo(plan), bc, model, params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
+    rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
                   sm_count(plan->device), st, &plan->launches);
   else
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       dI, dQ, dU, grad, st, &plan->launches);
   cudaFreeAsync(bc, st);
+  if (bd) cudaFreeAsync(bd, st);
   if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));
   return SYNAX_OK;
 }

@@ -99,10 +99,18 @@ __device__ __forceinline__ void faraday_sincos(double k_turn, double S, float& c
   c = mufu_cos(a); s = mufu_sin(a);
 }
 
-// float64 chain for one sample: coordinates, trilinear weights, interpolation, densities, projections
-__device__ __forceinline__ void fields_f64(const GridDesc& G, const BatchConsts& P, const double4 dir, double xd,
-                                           double yd, double zd, double& Bpar, double& BN, double& BE, double& N0,
-                                           double& ne) {
+// CR density only (fp32 MUFU chain), Eq.(12) P:L173 -- the emission needs no more than that
+__device__ __forceinline__ float n0_f32(const BatchConsts& P, float rho2, float z) {
+  const float rho = rho2 * mufu_rsqrt(fmaxf(rho2, 1e-30f));
+  const float ez = mufu_ex2(P.k_hz * fabsf(z)), dz = 1.0f + ez;
+  return 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
+}
+
+// float64 chain for one sample: coordinates, trilinear weights and interpolation in float64, n_e in float64 from
+// the short polynomials of synax_f64.cuh; N_0 stays fp32.
+__device__ __forceinline__ void fields_f64(const GridDesc& G, const BatchConsts& P, const BatchConstsD& D,
+                                           const double4 dir, double xd, double yd, double zd, double& Bpar,
+                                           double& BN, double& BE, float& N0, double& ne) {
   const double ux = fma(xd, G.sx, G.bx), uy = fma(yd, G.sy, G.by), uz = fma(zd, G.sz, G.bz);
   const bool inbox = (ux >= 0.0) && (ux <= (double)(G.nx - 1)) && (uy >= 0.0) && (uy <= (double)(G.ny - 1)) &&
                      (uz >= 0.0) && (uz <= (double)(G.nz - 1));
@@ -112,17 +120,23 @@ __device__ __forceinline__ void fields_f64(const GridDesc& G, const BatchConsts&
   double B[3] = {0.0, 0.0, 0.0};
   if (inbox) {
     const int base = ((i * G.ny + j) * G.nz + k) * 3;
+    const double x0 = 1.0 - tx, y0 = 1.0 - ty, z0 = 1.0 - tz;
+    const double wxy[4] = {x0 * y0, x0 * ty, tx * y0, tx * ty};
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-      const double w = ((q & 4) ? tx : 1.0 - tx) * ((q & 2) ? ty : 1.0 - ty) * ((q & 1) ? tz : 1.0 - tz);
+      const double w = wxy[q >> 1] * ((q & 1) ? tz : z0);
       const float* p = G.g + base + corner_offset(G, q);
-      B[0] += w * (double)__ldg(p); B[1] += w * (double)__ldg(p + 1); B[2] += w * (double)__ldg(p + 2);
+      B[0] = fma(w, (double)__ldg(p), B[0]); B[1] = fma(w, (double)__ldg(p + 1), B[1]); B[2] = fma(w, (double)__ldg(p + 2), B[2]);
     }
   }
-  const double rho = sqrt(fma(xd, xd, yd * yd));
-  const double chz = cosh(zd / (double)P.p[11]), che = cosh(zd / (double)P.p[15]);
-  N0 = (double)P.p[9] * exp(-rho / (double)P.p[10]) / (chz * chz);
-  ne = (double)P.p[13] * exp(-rho / (double)P.p[14]) / (che * che);
+  const double rho2 = fma(xd, xd, yd * yd);
+  const double rho = rho2 * rsqrt_d(rho2);
+  const double xs[2] = {D.k_hez * fabs(zd), D.k_her * rho};
+  double o[2];
+  exp2_d_n<2>(xs, o);
+  const double de = 1.0 + o[0];
+  ne = D.ne0x4 * o[1] * o[0] * rcp_d(de * de);
+  N0 = n0_f32(P, (float)rho2, (float)zd);
   Bpar = B[0] * (dir.z * dir.x) + B[1] * (dir.z * dir.y) + B[2] * dir.w;
   BN = B[2] * dir.z - dir.w * (B[0] * dir.x + B[1] * dir.y);
   BE = B[1] * dir.x - B[0] * dir.y;
@@ -145,13 +159,97 @@ __device__ __forceinline__ double warp_bcast_d(double v, int src) {
 struct GridFwdArgs {
   ForwardArgs f;
   GridDesc grid;
+  int mode;            // 0 auto, 1 fp32 chain only, 2 float64 Faraday chain for every sightline
 };
 
-// ------------------------------------------------------------------------------------------------
-// Forward.  PRECISE = float64 trilinear weights / densities / scan for flagged sightlines.
-// Persistent warps striding over sightlines (or over the flag list).
-// ------------------------------------------------------------------------------------------------
+// Round-off scale of a sightline's Faraday sum, k-independent part: sum_n |n_e| (|B_LOS| + |B_N| + |B_E|),
+// estimated from every 8th sample with the fp32 chain (whole warp; returns the same value in every lane).
+__device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const BatchConsts& P, const Triad& T,
+                                                        const Geometry& geo, int lane) {
+  float acc = 0.f;
+  for (int n = 4 + 8 * lane; n < geo.n_los; n += 256) {
+    const double s_d = ((double)n + 0.5) * geo.delta;
+    const double xd = fma(s_d, T.nxd, geo.obs[0]), yd = fma(s_d, T.nyd, geo.obs[1]), zd = fma(s_d, T.nzd, geo.obs[2]);
+    const Cell c = locate(G, xd, yd, zd);
+    float B[3], N0, ne;
+    gather_B(G, c, B);
+    densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+    const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
+    const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
+    const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
+    acc = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), acc);
+  }
+  return 8.0f * group_sum<32>(acc);
+}
+
+// One sightline, whole warp, lanes on CONSECUTIVE samples (neighbouring lanes gather neighbouring cells).
+// PRECISE = float64 trilinear weights / n_e / scan.  Returns the (exact, not estimated) round-off scale.
 template <int NF, bool PRECISE>
+__device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const GridDesc& G, const FreqTab& ft,
+                                                    const BatchConsts& P, const BatchConstsD& D, const Triad& T,
+                                                    const double4 dir, int lane, float& accI, float (&accQ)[NF],
+                                                    float (&accU)[NF]) {
+  accI = 0.f;
+#pragma unroll
+  for (int f = 0; f < NF; ++f) { accQ[f] = 0.f; accU[f] = 0.f; }
+  double carry = 0.0;
+  float absS = 0.f;
+  const double delta = A.geo.delta;
+  for (int nt = 0; nt < A.geo.n_los; nt += 32) {
+    const int n = nt + lane;
+    const bool active = n < A.geo.n_los;
+    const double s_d = ((double)n + 0.5) * delta;
+    const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+    const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+    const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+    float eI = 0.f, a = 0.f, bq = 0.f;
+    double S_here;  // sum_{m<n} g_m + g_n/2 relative to the start of the sightline
+    if (!PRECISE) {
+      const Cell c = locate(G, xd, yd, zd);
+      float B[3];
+      gather_B(G, c, B);
+      float N0, ne;
+      densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
+      const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
+      const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
+      if (active) emission(P, BN, BE, N0, eI, a, bq);
+      const float gn = active ? ne * Bpar : 0.f;
+      if (active) absS = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), absS);
+      const float incl = warp_inclusive_scan(gn, lane);
+      S_here = carry + (double)(incl - 0.5f * gn);
+      carry += warp_sum_d((double)gn);
+    } else {
+      double Bpar, BN, BE, ne;
+      float N0;
+      fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BN, BE, N0, ne);
+      if (active) emission(P, (float)BN, (float)BE, N0, eI, a, bq);
+      const double gn = active ? ne * Bpar : 0.0;
+      const double incl = warp_inclusive_scan_d(gn, lane);
+      S_here = carry + incl - 0.5 * gn;
+      carry += warp_bcast_d(incl, 31);
+    }
+    accI += eI;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      float c, s;
+      faraday_sincos(ft.k_turn[f], S_here, c, s);
+      accQ[f] = fmaf(a, c, fmaf(-bq, s, accQ[f]));
+      accU[f] = fmaf(a, s, fmaf(bq, c, accU[f]));
+    }
+  }
+  accI = group_sum<32>(accI);
+#pragma unroll
+  for (int f = 0; f < NF; ++f) { accQ[f] = group_sum<32>(accQ[f]); accU[f] = group_sum<32>(accU[f]); }
+  return group_sum<32>(absS);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Forward: persistent warps striding over sightlines.  Per sightline (warp-uniform): a cheap estimate of the
+// round-off scale from every 8th sample sends it straight to the float64 chain when the Faraday rotation is
+// strong; otherwise the fp32 sweep runs and is redone in float64 only if its exact criterion fires.
+// ------------------------------------------------------------------------------------------------
+template <int NF>
 __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_constant__ GridFwdArgs GA,
                                                               const __grid_constant__ FreqTab ft) {
   const ForwardArgs& A = GA.f;
@@ -159,64 +257,19 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
   const int lane = threadIdx.x & 31;
   const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
   const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
-  const int64_t count = (PRECISE && A.flag_list) ? (int64_t)(*A.flag_count) : A.geo.npix;
   const BatchConsts& P = A.bc[0];
-  const double delta = A.geo.delta;
-  for (int64_t it = warp; it < count; it += n_warps) {
-    const int64_t pix = (PRECISE && A.flag_list) ? (int64_t)A.flag_list[it] : it;
+  const BatchConstsD D = A.bd[0];
+  for (int64_t pix = warp; pix < A.geo.npix; pix += n_warps) {
     const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
     const Triad T = load_triad(A.geo.dirs, pix);
-    float accI = 0.f, accQ[NF], accU[NF];
-#pragma unroll
-    for (int f = 0; f < NF; ++f) { accQ[f] = 0.f; accU[f] = 0.f; }
-    double carry = 0.0;
-    float absS = 0.f;
-    for (int nt = 0; nt < A.geo.n_los; nt += 32) {
-      const int n = nt + lane;
-      const bool active = n < A.geo.n_los;
-      const double s_d = ((double)n + 0.5) * delta;
-      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
-      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
-      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
-      float eI = 0.f, a = 0.f, bq = 0.f;
-      double S_here;  // sum_{m<n} g_m + g_n/2 relative to the start of the sightline
-      if (!PRECISE) {
-        const Cell c = locate(G, xd, yd, zd);
-        float B[3];
-        gather_B(G, c, B);
-        float N0, ne;
-        densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
-        const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
-        const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
-        const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
-        if (active) emission(P, BN, BE, N0, eI, a, bq);
-        const float gn = active ? ne * Bpar : 0.f;
-        if (active) absS = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), absS);
-        const float incl = warp_inclusive_scan(gn, lane);
-        S_here = carry + (double)(incl - 0.5f * gn);
-        carry += warp_sum_d((double)gn);
-      } else {
-        double Bpar, BN, BE, N0, ne;
-        fields_f64(G, P, dir, xd, yd, zd, Bpar, BN, BE, N0, ne);
-        if (active) emission(P, (float)BN, (float)BE, (float)N0, eI, a, bq);
-        const double gn = active ? ne * Bpar : 0.0;
-        const double incl = warp_inclusive_scan_d(gn, lane);
-        S_here = carry + incl - 0.5 * gn;
-        carry += warp_bcast_d(incl, 31);
-      }
-      accI += eI;
-#pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        float c, s;
-        faraday_sincos(ft.k_turn[f], S_here, c, s);
-        accQ[f] = fmaf(a, c, fmaf(-bq, s, accQ[f]));
-        accU[f] = fmaf(a, s, fmaf(bq, c, accU[f]));
-      }
+    float accI, accQ[NF], accU[NF];
+    bool precise = GA.mode == 2;
+    if (GA.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, lane) > A.flag_S;
+    if (!precise) {
+      const float scale = grid_forward_sweep<NF, false>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
+      precise = GA.mode == 0 && scale > A.flag_S;
     }
-    accI = group_sum<32>(accI);
-    absS = group_sum<32>(absS);   // sum n_e (|B_LOS| + |B_N| + |B_E|): scale of the fp32 round-off in the Faraday sum
-#pragma unroll
-    for (int f = 0; f < NF; ++f) { accQ[f] = group_sum<32>(accQ[f]); accU[f] = group_sum<32>(accU[f]); }
+    if (precise) grid_forward_sweep<NF, true>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
     if (lane == 0) {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
@@ -225,10 +278,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
         A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
         A.U[o] = P.coefP[A.f0 + f] * accU[f];
       }
-      if (!PRECISE && A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
-        const int k = atomicAdd(A.flag_count, 1);
-        A.flag_list[k] = (int)pix;
-      }
+      if (precise && GA.mode == 0 && A.f0 == 0) atomicAdd(A.flag_count, 1);
     }
   }
 }
@@ -240,6 +290,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
 struct GridVjpArgs {
   Geometry geo;
   const BatchConsts* bc;
+  const BatchConstsD* bd;
   GridDesc grid;
   int f0, n_freq_total;
   const float* dI; const float* dQ; const float* dU;
@@ -253,7 +304,8 @@ struct GridVjpArgs {
 // fan-out (A9) and the per-sample hand-over to sweep 2 through shared memory.  Returns sum n_e (|B_LOS| + |B_N| + |B_E|).
 template <int NF, bool PRECISE>
 __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const FreqTab& ft, const GridDesc& G,
-                                                 const BatchConsts& P, const Triad& T, const double4 dir, int lane,
+                                                 const BatchConsts& P, const BatchConstsD& D, const Triad& T,
+                                                 const double4 dir, int lane,
                                                  float cI, const float (&cQ)[NF], const float (&cU)[NF],
                                                  const float (&kr)[NF], float* st_w, float* st_n, float* st_e,
                                                  float* st_d) {
@@ -284,9 +336,9 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       S_here = carry + (double)(incl - 0.5f * gn);
       carry += warp_sum_d((double)gn);
     } else {
-      double Bpar, BNd, BEd, N0d, ned;
-      fields_f64(G, P, dir, xd, yd, zd, Bpar, BNd, BEd, N0d, ned);
-      BN = (float)BNd; BE = (float)BEd; N0 = (float)N0d; ne = (float)ned;
+      double Bpar, BNd, BEd, ned;
+      fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BNd, BEd, N0, ned);
+      BN = (float)BNd; BE = (float)BEd; ne = (float)ned;
       const double gn = active ? ned * Bpar : 0.0;
       const double incl = warp_inclusive_scan_d(gn, lane);
       S_here = carry + incl - 0.5 * gn;
@@ -335,6 +387,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
   const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
   const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
   const BatchConsts& P = A.bc[0];
+  const BatchConstsD D = A.bd[0];
   const double delta = A.geo.delta;
   for (int64_t pix = warp; pix < A.geo.npix; pix += n_warps) {
     const Triad T = load_triad(A.geo.dirs, pix);
@@ -351,10 +404,12 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     // ---- sweep 1: consecutive samples per lane; fp32 chain first, redone with the float64 Faraday chain
     // when the rotation angle of this sightline is large (warp-uniform decision)
     float absS = 0.f;
-    if (A.mode != 2) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
-    if (A.mode == 2 || (A.mode == 0 && absS > A.flag_S)) {
+    bool precise = A.mode == 2;
+    if (A.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, lane) > A.flag_S;
+    if (!precise) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
+    if (precise || (A.mode == 0 && absS > A.flag_S)) {
       __syncwarp();
-      grid_vjp_sweep1<NF, true>(A, ft, G, P, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
+      grid_vjp_sweep1<NF, true>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
     }
     __syncwarp();
     // ---- sweep 2: contiguous chunk per lane walked BACKWARDS, so that the suffix sum of Sbar that the
@@ -429,15 +484,14 @@ static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
   return g;
 }
 
-template <bool PRECISE>
 static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f.f0);
   switch (nf) {
-    case 1: grid_forward_kernel<1, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 2: grid_forward_kernel<2, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 3: grid_forward_kernel<3, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 4: grid_forward_kernel<4, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    default: grid_forward_kernel<8, PRECISE><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 1: grid_forward_kernel<1><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 2: grid_forward_kernel<2><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 3: grid_forward_kernel<3><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 4: grid_forward_kernel<4><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    default: grid_forward_kernel<8><<<blocks, kBlock, 0, st>>>(a, ft); break;
   }
 }
 
@@ -445,48 +499,30 @@ static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const
                                  int precision, double escalate_rad, int sms, int* d_flag_count, int* h_flag_count,
                                  cudaStream_t st, int64_t* launches) {
   GridFwdArgs ga;
-  ga.f = a0; ga.grid = make_grid_desc(m, grid);
+  ga.f = a0; ga.grid = make_grid_desc(m, grid); ga.mode = precision;
   float k_max = 0.f;
   for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
-  const bool fast = precision != 2, escalate = precision == 0;
-  ga.f.flag_list = nullptr; ga.f.flag_S = 0.f; ga.f.flag_count = d_flag_count;
-  if (escalate) {
-    if (cudaMallocAsync((void**)&ga.f.flag_list, sizeof(int) * (size_t)a0.geo.npix, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
-    cudaMemsetAsync(d_flag_count, 0, kCtrlWords * sizeof(int), st);
-    ga.f.flag_S = (float)(escalate_rad / (double)k_max);
-  }
-  const int64_t warps_needed = a0.geo.npix;
-  const unsigned max_blocks = (unsigned)(sms * 16);
-  const unsigned blocks = (unsigned)min((int64_t)max_blocks, (warps_needed * 32 + kBlock - 1) / kBlock);
+  ga.f.flag_list = nullptr; ga.f.flag_count = d_flag_count;
+  ga.f.flag_S = (float)(escalate_rad / (double)k_max);
+  cudaMemsetAsync(d_flag_count, 0, kCtrlWords * sizeof(int), st);
+  const unsigned blocks = (unsigned)min((int64_t)sms * 16, (a0.geo.npix * 32 + kBlock - 1) / kBlock);
   for (int f0 = 0; f0 < ft.n_freq;) {
     const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
     ga.f.f0 = f0;
-    if (fast) { launch_grid_forward<false>(nf, blocks, st, ga, ft); ++*launches; }
+    launch_grid_forward(nf, blocks, st, ga, ft); ++*launches;
     f0 += nf;
   }
-  if (!fast || escalate) {
-    GridFwdArgs pa = ga;
-    if (!fast) pa.f.flag_list = nullptr;
-    for (int f0 = 0; f0 < ft.n_freq;) {
-      const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
-      pa.f.f0 = f0;
-      launch_grid_forward<true>(nf, blocks, st, pa, ft); ++*launches;
-      f0 += nf;
-    }
-  }
   const cudaError_t e = cudaGetLastError();
-  if (escalate) {
-    cudaMemcpyAsync(h_flag_count, d_flag_count, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
-    cudaFreeAsync(ga.f.flag_list, st);
-  }
+  cudaMemcpyAsync(h_flag_count, d_flag_count, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 
-static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const synax_model* m,
+static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const BatchConstsD* bd,
+                             const synax_model* m,
                              const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
                              int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches) {
   GridVjpArgs a;
-  a.geo = geo; a.bc = bc; a.grid = make_grid_desc(m, grid);
+  a.geo = geo; a.bc = bc; a.bd = bd; a.grid = make_grid_desc(m, grid);
   a.n_freq_total = ft.n_freq; a.dI = dI; a.dQ = dQ; a.dU = dU; a.grad = grad;
   int cl = 0;
   while ((32 << cl) < geo.n_los) ++cl;
