@@ -1,0 +1,28 @@
+"""Microbenchmarks behind the roofline denominators: python -m paper_2410_01136_b200.ubench
+
+  pipes.cu         FFMA / DFMA / MUFU / F2F throughput and dependent-issue latency (the "alu" peak, the FP64 and XU
+                   pipe rates the float64 Faraday chain is measured against)
+  grid_streams.cu  gather and red.global.add ceilings on config 3's actual index stream (gridded path)
+
+Each is compiled with nvcc for sm_100a into a temporary binary and run on the current GPU."""
+import subprocess
+import sys
+import tempfile
+from pathlib import Path
+
+HERE = Path(__file__).resolve().parent
+
+
+def main():
+    which = sys.argv[1:] or ["pipes", "grid_streams"]
+    for name in which:
+        with tempfile.TemporaryDirectory() as d:
+            exe = Path(d) / name
+            subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+                            "-o", str(exe), str(HERE / f"{name}.cu")], check=True)
+            print(f"== {name}", flush=True)
+            subprocess.run([str(exe)], check=True)
+
+
+if __name__ == "__main__":
+    main()
