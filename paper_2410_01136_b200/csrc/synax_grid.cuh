@@ -298,7 +298,7 @@ __global__ void grid_grad_compact_kernel(const float4* __restrict__ g4, int64_t 
 
 // ------------------------------------------------------------------------------------------------
 // Adjoint.  grad_grid must be zero on entry (the host wrapper clears it).
-// Dynamic shared memory: 4 float arrays of 32*(C+1) per warp, C = chunk length (power of two).
+// Dynamic shared memory: 3 float arrays of 32*(C+1) per warp, C = chunk length (power of two).
 // ------------------------------------------------------------------------------------------------
 struct GridVjpArgs {
   Geometry geo;
@@ -320,8 +320,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
                                                  const BatchConsts& P, const BatchConstsD& D, const Triad& T,
                                                  const double4 dir, int lane,
                                                  float cI, const float (&cQ)[NF], const float (&cU)[NF],
-                                                 const float (&kr)[NF], float* st_w, float* st_n, float* st_e,
-                                                 float* st_d) {
+                                                 const float (&kr)[NF], float* st_w, float* st_n, float* st_e) {
   const int C = 1 << A.chunk_log2, Cp = C + 1;
   const double delta = A.geo.delta;
   double carry = 0.0;
@@ -380,7 +379,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
     const float BNb = 2.0f * fmaf(M, fmaf(BN, cI - Xc, BE * Xs), BN * tq_);
     if (active) {
       const int idx = (n >> A.chunk_log2) * Cp + (n & (C - 1));
-      st_w[idx] = Sbar; st_n[idx] = BNb; st_e[idx] = BEb; st_d[idx] = ne;
+      st_w[idx] = Sbar; st_n[idx] = BNb; st_e[idx] = BEb;
     }
   }
   return group_sum<32>(absS);
@@ -393,10 +392,9 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
   const GridDesc& G = A.grid;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int C = 1 << A.chunk_log2, Cp = C + 1;
-  float* st_w = smem + (size_t)wid * 4 * 32 * Cp;   // Sbar_m: cotangent of the Faraday sum at sample m
+  float* st_w = smem + (size_t)wid * 3 * 32 * Cp;   // Sbar_m: cotangent of the Faraday sum at sample m
   float* st_n = st_w + 32 * Cp;                     // BbarN (direct)
   float* st_e = st_n + 32 * Cp;                     // BbarE (direct)
-  float* st_d = st_e + 32 * Cp;                     // n_e
   const int64_t warp = ((int64_t)blockIdx.x * kBlock + threadIdx.x) >> 5;
   const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
   const BatchConsts& P = A.bc[0];
@@ -419,10 +417,10 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     float absS = 0.f;
     bool precise = A.mode == 2;
     if (A.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, lane) > A.flag_S;
-    if (!precise) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
+    if (!precise) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
     if (precise || (A.mode == 0 && absS > A.flag_S)) {
       __syncwarp();
-      grid_vjp_sweep1<NF, true>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e, st_d);
+      grid_vjp_sweep1<NF, true>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
     }
     __syncwarp();
     // ---- sweep 2: contiguous chunk per lane walked BACKWARDS, so that the suffix sum of Sbar that the
@@ -445,9 +443,13 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     int cur = -1;
     for (int m = m1 - 1; m >= m0 - 1; --m) {
       Cell c; c.base = -1; c.inbox = false; c.tx = c.ty = c.tz = 0.f;
+      float ne_m = 0.f;   // recomputed (fp32, 4 MUFU) rather than handed over: 25 % less shared memory per warp
       if (m >= m0) {
         const double s_d = ((double)m + 0.5) * delta;
-        c = locate(G, fma(s_d, T.nxd, A.geo.obs[0]), fma(s_d, T.nyd, A.geo.obs[1]), fma(s_d, T.nzd, A.geo.obs[2]));
+        const double xd = fma(s_d, T.nxd, A.geo.obs[0]), yd = fma(s_d, T.nyd, A.geo.obs[1]), zd = fma(s_d, T.nzd, A.geo.obs[2]);
+        c = locate(G, xd, yd, zd);
+        float N0_unused;
+        densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0_unused, ne_m);
       }
       const int cell = (m >= m0 && c.inbox) ? c.base : -1;
       if (cell != cur) {
@@ -467,7 +469,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
         const float gbar = fmaf(0.5f, Sb, suf);
         suf += Sb;
         if (cell >= 0) {
-          const float BNb = st_n[idx], BEb = st_e[idx], gn = gbar * st_d[idx];
+          const float BNb = st_n[idx], BEb = st_e[idx], gn = gbar * ne_m;
           const float bx = fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, gn * T.nx));
           const float by = fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, gn * T.ny));
           const float bz = fmaf(BNb, T.eNz, gn * T.nz);
@@ -546,7 +548,7 @@ static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const Batch
   float k_max = 0.f;
   for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
   a.mode = precision; a.flag_S = (float)(escalate_rad / (double)k_max);
-  const size_t smem = (size_t)(kBlock / 32) * 4 * 32 * ((1u << cl) + 1) * sizeof(float);
+  const size_t smem = (size_t)(kBlock / 32) * 3 * 32 * ((1u << cl) + 1) * sizeof(float);
   if (smem > 200 * 1024) return SYNAX_ERR_UNSUPPORTED;  // n_los too large for the shared-memory hand-over
   const unsigned blocks = (unsigned)min((int64_t)sms * 8, (geo.npix * 32 + kBlock - 1) / kBlock);
   for (int f0 = 0; f0 < ft.n_freq;) {
