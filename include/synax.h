@@ -116,6 +116,18 @@ synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, co
                             int32_t batch, const float* dI, const float* dQ, const float* dU,
                             float* grad, void* cuda_stream);
 
+/* Gaussian pixel log-likelihood of Eq.(15) P:L193-197 and its gradient in ONE call (the inner loop of the
+ * paper's HMC / ADAM runs): forward, residuals, VJP, with no map leaving the device:
+ *   logL[b] = -1/2 sum_{f,p} [ w[0] (I - I_obs)^2 + w[1] (Q - Q_obs)^2 + w[2] (U - U_obs)^2 ]
+ *   grad[b][j] = d logL[b] / d theta_j
+ * I_obs, Q_obs, U_obs: DEVICE fp32 [n_freq][npix], ONE observation shared by all batch elements; a NULL map takes
+ * that Stokes parameter out of the likelihood (the paper uses Q and U only, sigma = 1 mK: w = 1/sigma^2 in K^-2).
+ * inv_var: HOST, 3 weights >= 0.  logL: DEVICE float64 [batch], overwritten.  grad: DEVICE fp32 as in synax_vjp.
+ * Scratch for the three maps ([batch][n_freq][npix] fp32 each) is taken from the stream-ordered pool. */
+synax_status synax_loglike_vjp(const synax_plan* plan, const synax_model* model, const float* params,
+                               int32_t batch, const float* I_obs, const float* Q_obs, const float* U_obs,
+                               const double inv_var[3], double* logL, float* grad, void* cuda_stream);
+
 /* Counters since plan creation (for bench.py's gpu_launches): out[0] = kernels launched,
  * out[1] = sightlines redone with the float64 Faraday chain in the last forward (read back lazily:
  * valid after the stream has been synchronised). */

@@ -181,3 +181,23 @@ def vjp(model: Model, nside, n_los, s_max, freqs, dI, dQ, dU, observer=(-8.3, 0.
     if model.kind == "grid_b":
         return grad.reshape(tuple(model.gdim) + (3,))
     return grad
+
+
+def loglike_vjp(model: Model, nside, n_los, s_max, freqs, I_obs, Q_obs, U_obs, inv_var, observer=(-8.3, 0.0, 0.006)):
+    """Gaussian pixel log-likelihood of Eq.(15) and its gradient, written out as the
+    composition it is: maps = forward(theta); logL[b] = -1/2 sum_k w_k sum_{f,p} (X_k - X_k_obs)^2 over the Stokes
+    maps k with an observation (None = not in the likelihood; the paper uses Q and U with w = 1/sigma^2,
+    sigma = 1 mK); d logL / d theta = VJP with cotangent -w_k (X_k - X_k_obs).  Observations [n_freq][npix] are
+    shared by all batch elements.  Returns (logL float64 [batch], grad like vjp())."""
+    maps = forward(model, nside, n_los, s_max, freqs, observer=observer)
+    logL = np.zeros(model.batch)
+    cots = []
+    for X, obs, w in zip(maps, (I_obs, Q_obs, U_obs), inv_var):
+        if obs is None or w == 0.0:
+            cots.append(None)
+            continue
+        r = X - _f64(obs).reshape((1,) + X.shape[1:])
+        logL += -0.5 * float(w) * np.sum(r * r, axis=(1, 2))
+        cots.append(-float(w) * r)
+    grad = vjp(model, nside, n_los, s_max, freqs, cots[0], cots[1], cots[2], observer=observer)
+    return logL, grad

@@ -19,7 +19,7 @@ KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
 
 # every symbol include/synax.h declares
 exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_option",
-                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host",
+                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
 
@@ -68,6 +68,8 @@ def load_library() -> ctypes.CDLL:
     for name, at in (("synax_forward", fwd), ("synax_forward_host", fwd), ("synax_vjp", bwd), ("synax_vjp_host", bwd)):
         getattr(L, name).argtypes = at
         getattr(L, name).restype = ctypes.c_int
+    L.synax_loglike_vjp.argtypes = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, ctypes.POINTER(dbl), vp, vp, vp]
+    L.synax_loglike_vjp.restype = ctypes.c_int
     L.synax_last_error.restype = ctypes.c_char_p
     L.synax_version.restype = ctypes.c_char_p
     _lib = L
@@ -196,6 +198,27 @@ def vjp(plan: Plan, model: Model, params, dI, dQ, dU, out=None):
     _check(load_library().synax_vjp(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
                                     ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _dev_f32(out, "grad"), _stream()))
     return out
+
+
+def loglike_vjp(plan: Plan, model: Model, params, I_obs, Q_obs, U_obs, inv_var, out=None):
+    """synax_loglike_vjp: observed maps CUDA fp32 [n_freq][npix] (None = not in the likelihood), inv_var = 3 weights
+    1/sigma^2 -> (logL CUDA float64 [batch], grad CUDA fp32 like params)."""
+    import torch
+    batch = _batch_of(model, params)
+    if out is None:
+        out = (torch.empty((batch,), dtype=torch.float64, device=params.device), torch.empty_like(params))
+    logL, grad = out
+    if not (logL.is_cuda and logL.dtype == torch.float64 and logL.is_contiguous() and logL.numel() == batch):
+        raise TypeError("logL must be a contiguous float64 CUDA tensor [batch]")
+    w = (ctypes.c_double * 3)(*[float(v) for v in inv_var])
+    ptr = lambda t, n: ctypes.c_void_p(None) if t is None else _dev_f32(t, n)  # noqa: E731
+    for t in (I_obs, Q_obs, U_obs):
+        if t is not None and t.numel() != plan.n_freq * plan.npix:
+            raise ValueError("observed maps must have n_freq * npix elements")
+    _check(load_library().synax_loglike_vjp(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
+                                            ptr(I_obs, "I_obs"), ptr(Q_obs, "Q_obs"), ptr(U_obs, "U_obs"), w,
+                                            ctypes.c_void_p(logL.data_ptr()), _dev_f32(grad, "grad"), _stream()))
+    return logL, grad
 
 
 def _host_f32(a, what):

@@ -414,6 +414,71 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
 }
 
 // ------------------------------------------------------------------------------------------------
+// Fused Gaussian likelihood (Eq.(15)): forward -> residual cotangents + logL -> VJP.
+// ------------------------------------------------------------------------------------------------
+// In place: map <- -w (map - obs) (the cotangent of logL), and logL[b] -= w/2 sum (map - obs)^2.
+__global__ void __launch_bounds__(256) loglike_residual_kernel(float* __restrict__ map, const float* __restrict__ obs,
+                                                               int64_t per_batch, float w, double* __restrict__ logL) {
+  const int b = blockIdx.y;
+  float* m = map + (int64_t)b * per_batch;
+  double acc = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < per_batch; i += (int64_t)gridDim.x * blockDim.x) {
+    const float r = m[i] - __ldg(obs + i);
+    m[i] = -w * r;
+    acc += (double)r * (double)r;
+  }
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) {
+    int lo = __double2loint(acc), hi = __double2hiint(acc);
+    lo = __shfl_xor_sync(0xffffffffu, lo, d); hi = __shfl_xor_sync(0xffffffffu, hi, d);
+    acc += __hiloint2double(hi, lo);
+  }
+  __shared__ double part[8];
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int k = 0; k < 8; ++k) t += part[k];
+    atomicAdd(logL + b, -0.5 * (double)w * t);
+  }
+}
+
+extern "C" synax_status synax_loglike_vjp(const synax_plan* plan, const synax_model* model, const float* params,
+                                          int32_t batch, const float* I_obs, const float* Q_obs, const float* U_obs,
+                                          const double inv_var[3], double* logL, float* grad, void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!inv_var || !logL || !grad) return fail(SYNAX_ERR_INVALID_ARG, "inv_var, logL or grad is NULL");
+  for (int k = 0; k < 3; ++k)
+    if (!(inv_var[k] >= 0.0) || !std::isfinite(inv_var[k])) return fail(SYNAX_ERR_INVALID_ARG, "inv_var[%d] must be finite and >= 0", k);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int64_t per_batch = (int64_t)plan->n_freq * plan->npix;
+  const size_t count = (size_t)batch * (size_t)per_batch;
+  float* maps = nullptr;
+  CUDA_TRY(cudaMallocAsync((void**)&maps, 3 * count * sizeof(float), st));
+  float* m[3] = {maps, maps + count, maps + 2 * count};
+  synax_status rs = synax_forward(plan, model, params, batch, m[0], m[1], m[2], cuda_stream);
+  if (rs == SYNAX_OK) {
+    CUDA_TRY(cudaMemsetAsync(logL, 0, sizeof(double) * (size_t)batch, st));
+    const float* obs[3] = {I_obs, Q_obs, U_obs};
+    const float* cot[3] = {nullptr, nullptr, nullptr};
+    const unsigned bx = (unsigned)std::min<int64_t>((per_batch + 255) / 256, (int64_t)sm_count(plan->device) * 8);
+    for (int k = 0; k < 3; ++k) {
+      if (!obs[k] || inv_var[k] == 0.0) continue;
+      loglike_residual_kernel<<<dim3(bx, (unsigned)batch), 256, 0, st>>>(m[k], obs[k], per_batch, (float)inv_var[k], logL);
+      plan->launches++;
+      cot[k] = m[k];
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) rs = fail(SYNAX_ERR_CUDA, "loglike residual launch failed: %s", cudaGetErrorString(e));
+    else rs = synax_vjp(plan, model, params, batch, cot[0], cot[1], cot[2], grad, cuda_stream);
+  }
+  cudaFreeAsync(maps, st);
+  return rs;
+}
+
+// ------------------------------------------------------------------------------------------------
 // HOST-buffer variants: copies inside the call, stream synchronised on return.
 // ------------------------------------------------------------------------------------------------
 extern "C" synax_status synax_forward_host(const synax_plan* plan, const synax_model* model, const float* params,

@@ -1,0 +1,92 @@
+"""Fused Gaussian likelihood (Eq. 15): oracle pins on CPU, GPU parity through synax_loglike_vjp."""
+import numpy as np
+import pytest
+
+import oracle
+import parity
+from paper_2410_01136_b200 import workloads as wl
+
+SIGMA = 1.0e-3     # K: "sigma = 1 mK" per pixel on Q and U
+
+
+def _mock(w, seed=31, scale=1.0):
+    """Mock observation as in the paper's section 3.1: maps at 'true' parameters + N(0, sigma) per pixel."""
+    truth = wl.Workload(w.name, w.kind, w.nside, w.n_los, w.s_max, w.freqs, w.params[:1] if w.kind != "grid_b" else w.params,
+                        w.aux, box=w.box)
+    I, Q, U = parity.oracle_forward(truth)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    noise = rng.standard_normal((3,) + I.shape[1:]) * SIGMA * scale
+    return [np.ascontiguousarray((m[0] + n).astype(np.float32)) for m, n in zip((I, Q, U), noise)]
+
+
+def _oracle_ll(w, obs, inv_var):
+    return oracle.loglike_vjp(parity.oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, *obs, inv_var, observer=w.observer)
+
+
+def test_oracle_loglike_closed_forms():
+    w = wl.config(0).scaled(nside=4, n_los=32)
+    I, Q, U = parity.oracle_forward(w)
+    exact = [I[0], Q[0], U[0]]
+    ll, g = _oracle_ll(w, exact, (1.0, 1.0, 1.0))
+    assert ll[0] == 0.0 and np.all(g == 0.0)                      # observation = model: maximum of logL
+    shifted = [I[0], Q[0] + 2.0e-3, None]
+    ll, _ = _oracle_ll(w, shifted, (0.0, 1.0 / SIGMA ** 2, 1.0 / SIGMA ** 2))
+    assert abs(ll[0] - (-0.5 * 4.0 * Q[0].size)) < 1e-9 * Q[0].size    # every pixel 2 sigma off in Q only
+    ll2, _ = _oracle_ll(w, shifted, (0.0, 3.0 / SIGMA ** 2, 0.0))
+    assert abs(ll2[0] / ll[0] - 3.0) < 1e-12                      # linear in the weight
+
+
+def test_oracle_loglike_gradient_matches_finite_differences():
+    w = wl.config(2).scaled(nside=2, n_los=48, batch=2)
+    p0 = w.params.astype(np.float64).copy()
+    p0[:, :] *= 1.03                                               # away from the truth used for the mock
+    w.params = p0.astype(np.float32)
+    obs = _mock(wl.config(2).scaled(nside=2, n_los=48, batch=2))
+    inv_var = (0.0, 1.0 / SIGMA ** 2, 1.0 / SIGMA ** 2)
+    ll, g = _oracle_ll(w, [None, obs[1], obs[2]], inv_var)
+    base = w.params.astype(np.float64)
+    for j in (0, 1, 3, 5, 9, 12, 13, 15):
+        h = 1e-6 * abs(base[1, j])
+        vals = []
+        for sgn in (+1, -1):
+            q = base.copy(); q[1, j] += sgn * h
+            m = oracle.Model("full16", q)
+            vals.append(oracle.loglike_vjp(m, w.nside, w.n_los, w.s_max, w.freqs, None, obs[1], obs[2], inv_var)[0][1])
+        fd = (vals[0] - vals[1]) / (2 * h)
+        assert abs(fd - g[1, j]) <= 2e-5 * abs(g[1, j]) + 1e-12, (j, fd, g[1, j])
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", ["cfg1", "cfg2", "cfg3"])
+def test_gpu_loglike_vjp_matches_oracle(case):
+    import torch
+    import paper_2410_01136_b200 as sx
+    if case == "cfg1":
+        w = wl.config(1).scaled(nside=16, n_los=128)
+    elif case == "cfg2":
+        w = wl.config(2).scaled(nside=8, n_los=128, batch=5)
+    else:
+        w = wl.config(3).scaled(nside=8, n_los=256)
+    obs = _mock(w)
+    if w.kind != "grid_b":
+        w.params = (w.params.astype(np.float64) * 1.02).astype(np.float32)   # evaluate away from the truth
+    else:
+        w.params = (w.params.astype(np.float64) * 1.02).astype(np.float32)
+    inv_var = (0.0, 1.0 / SIGMA ** 2, 1.0 / SIGMA ** 2)
+    ll_ref, g_ref = _oracle_ll(w, [None, obs[1], obs[2]], inv_var)
+    plan, model, params = parity.gpu_objects(w)
+    d = [None, torch.from_numpy(obs[1]).cuda(), torch.from_numpy(obs[2]).cuda()]
+    ll, g = sx.loglike_vjp(plan, model, params, *d, inv_var)
+    torch.cuda.synchronize()
+    ll, g = ll.cpu().numpy(), g.cpu().numpy().astype(np.float64)
+    plan.close()
+    # logL is a sum of squares of (map - obs) / sigma: the map tolerance 1e-4 RMS moves it by at most ~2 |r| 1e-4 RMS / sigma^2
+    assert np.all(np.abs(ll - ll_ref) <= 2e-3 * np.abs(ll_ref))
+    if w.kind == "grid_b":
+        rms = np.sqrt(np.mean(g_ref[g_ref != 0] ** 2))
+        assert np.all(np.abs(g.reshape(g_ref.shape) - g_ref) <= 2e-3 * np.abs(g_ref) + 2e-4 * rms)
+    else:
+        assert np.all(np.abs(g - g_ref) <= 2e-3 * np.abs(g_ref))
+    # NULL observation = Stokes parameter out of the likelihood; zero weight likewise
+    with pytest.raises(sx.SynaxError):
+        sx.loglike_vjp(*parity.gpu_objects(w), None, None, None, (-1.0, 0.0, 0.0))
