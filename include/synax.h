@@ -128,6 +128,13 @@ synax_status synax_loglike_vjp(const synax_plan* plan, const synax_model* model,
                                int32_t batch, const float* I_obs, const float* Q_obs, const float* U_obs,
                                const double inv_var[3], double* logL, float* grad, void* cuda_stream);
 
+/* One ADAM update (the optimiser of the paper's field-level fits: Optax ADAM on the 128x128x32 B grid),
+ * elementwise on DEVICE buffers of n floats: with g = -grad when `maximize` != 0 (grad of a log-likelihood) else grad,
+ *   m <- b1 m + (1-b1) g;  v <- b2 v + (1-b2) g^2;  theta <- theta - lr (m / (1-b1^t)) / (sqrt(v / (1-b2^t)) + eps)
+ * (Kingma & Ba 2015, Algorithm 1; t = 1, 2, ... is the step number).  m and v must be zero before the first step. */
+synax_status synax_adam_step(float* theta, const float* grad, float* m, float* v, int64_t n, double lr, double beta1,
+                             double beta2, double eps, int32_t t, int32_t maximize, void* cuda_stream);
+
 /* Counters since plan creation (for bench.py's gpu_launches): out[0] = kernels launched,
  * out[1] = sightlines redone with the float64 Faraday chain in the last forward (read back lazily:
  * valid after the stream has been synchronised). */

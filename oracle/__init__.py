@@ -201,3 +201,14 @@ def loglike_vjp(model: Model, nside, n_los, s_max, freqs, I_obs, Q_obs, U_obs, i
         cots.append(-float(w) * r)
     grad = vjp(model, nside, n_los, s_max, freqs, cots[0], cots[1], cots[2], observer=observer)
     return logL, grad
+
+
+def adam_step(theta, grad, m, v, t, lr=1e-3, beta1=0.9, beta2=0.999, eps=1e-8, maximize=False):
+    """ADAM update of Kingma & Ba (2015), Algorithm 1, as used for the paper's field-level fits:
+    returns (theta, m, v) after step t (float64; inputs untouched)."""
+    g = -_f64(grad) if maximize else _f64(grad)
+    m = beta1 * _f64(m) + (1.0 - beta1) * g
+    v = beta2 * _f64(v) + (1.0 - beta2) * g * g
+    mhat = m / (1.0 - beta1 ** t)
+    vhat = v / (1.0 - beta2 ** t)
+    return _f64(theta) - lr * mhat / (np.sqrt(vhat) + eps), m, v

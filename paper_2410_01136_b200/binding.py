@@ -19,7 +19,7 @@ KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
 
 # every symbol include/synax.h declares
 exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_option",
-                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp",
+                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
 
@@ -70,6 +70,8 @@ def load_library() -> ctypes.CDLL:
         getattr(L, name).restype = ctypes.c_int
     L.synax_loglike_vjp.argtypes = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, ctypes.POINTER(dbl), vp, vp, vp]
     L.synax_loglike_vjp.restype = ctypes.c_int
+    L.synax_adam_step.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, i32, i32, vp]
+    L.synax_adam_step.restype = ctypes.c_int
     L.synax_last_error.restype = ctypes.c_char_p
     L.synax_version.restype = ctypes.c_char_p
     _lib = L
@@ -219,6 +221,18 @@ def loglike_vjp(plan: Plan, model: Model, params, I_obs, Q_obs, U_obs, inv_var, 
                                             ptr(I_obs, "I_obs"), ptr(Q_obs, "Q_obs"), ptr(U_obs, "U_obs"), w,
                                             ctypes.c_void_p(logL.data_ptr()), _dev_f32(grad, "grad"), _stream()))
     return logL, grad
+
+
+def adam_step(theta, grad, m, v, t: int, lr=1e-3, beta1=0.9, beta2=0.999, eps=1e-8, maximize=False):
+    """synax_adam_step: in-place ADAM update of the CUDA fp32 tensor `theta` (m, v: moment buffers, zero at t = 1)."""
+    n = theta.numel()
+    for x, name in ((grad, "grad"), (m, "m"), (v, "v")):
+        if x.numel() != n:
+            raise ValueError(f"{name} must have as many elements as theta")
+    _check(load_library().synax_adam_step(_dev_f32(theta, "theta"), _dev_f32(grad, "grad"), _dev_f32(m, "m"), _dev_f32(v, "v"),
+                                          n, float(lr), float(beta1), float(beta2), float(eps), int(t), int(bool(maximize)),
+                                          _stream()))
+    return theta
 
 
 def _host_f32(a, what):

@@ -478,6 +478,34 @@ extern "C" synax_status synax_loglike_vjp(const synax_plan* plan, const synax_mo
   return rs;
 }
 
+// ADAM (Kingma & Ba 2015, Algorithm 1) -- the paper's field-level optimiser
+__global__ void adam_kernel(float* __restrict__ theta, const float* __restrict__ grad, float* __restrict__ m,
+                            float* __restrict__ v, int64_t n, float lr, float b1, float b2, float eps, float c1, float c2,
+                            float sign) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float g = sign * grad[i];
+  const float mi = fmaf(b1, m[i], (1.0f - b1) * g);
+  const float vi = fmaf(b2, v[i], (1.0f - b2) * g * g);
+  m[i] = mi; v[i] = vi;
+  theta[i] -= lr * (mi * c1) / (sqrtf(vi * c2) + eps);
+}
+
+extern "C" synax_status synax_adam_step(float* theta, const float* grad, float* m, float* v, int64_t n, double lr,
+                                        double beta1, double beta2, double eps, int32_t t, int32_t maximize,
+                                        void* cuda_stream) {
+  if (!theta || !grad || !m || !v) return fail(SYNAX_ERR_INVALID_ARG, "theta, grad, m or v is NULL");
+  if (n < 1 || t < 1) return fail(SYNAX_ERR_INVALID_ARG, "n and t must be >= 1");
+  if (!(beta1 >= 0 && beta1 < 1 && beta2 >= 0 && beta2 < 1) || !(eps >= 0) || !std::isfinite(lr))
+    return fail(SYNAX_ERR_INVALID_ARG, "need 0 <= beta < 1, eps >= 0, finite lr");
+  const double c1 = 1.0 / (1.0 - std::pow(beta1, (double)t)), c2 = 1.0 / (1.0 - std::pow(beta2, (double)t));
+  adam_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+      theta, grad, m, v, n, (float)lr, (float)beta1, (float)beta2, (float)eps, (float)c1, (float)c2, maximize ? -1.0f : 1.0f);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(SYNAX_ERR_CUDA, "adam launch failed: %s", cudaGetErrorString(e));
+  return SYNAX_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // HOST-buffer variants: copies inside the call, stream synchronised on return.
 // ------------------------------------------------------------------------------------------------
