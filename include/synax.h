@@ -85,6 +85,13 @@ synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, double s_max_
 synax_status synax_plan_destroy(synax_plan* plan); /* NULL is allowed */
 int64_t synax_plan_npix(const synax_plan* plan);  /* pixels of this plan (12 nside^2 unless a shard), -1 for NULL */
 
+/* Integration extent of the paper (Fig. 1): from the observer to where the sightline leaves a box of
+ * side lengths box_kpc[3] centred on the Galactic centre, cut into n_los equal segments -- every sightline then has
+ * its own segment length Delta r_i = L_i / n_los.  The observer must be strictly inside the box (else
+ * SYNAX_ERR_INVALID_ARG).  Replaces the fixed [0, s_max] for all later calls with this plan; NULL restores it.
+ * HOST pointer; synchronises the device. */
+synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
+
 /* Options (tests / experiments).  key "precision": 0 = auto (default: fp32 pass, sightlines whose
  * Faraday rotation angle exceeds "escalate_rad" are redone with a float64 Faraday chain),
  * 1 = fp32 only, 2 = float64 Faraday chain for every sightline.  key "escalate_rad": threshold in

@@ -125,10 +125,36 @@ def eval_fields(model: Model, r, observer=(-8.3, 0.0, 0.006), b=0):
     return B, N0, ne, al
 
 
-def forward_dir(model: Model, l, b, n_los, s_max, freqs, observer=(-8.3, 0.0, 0.006), batch_index=0):
+class _clip:
+    """Context manager: integrate from the observer to the faces of `box` (lx, ly, lz kpc, centred on the Galactic
+    centre) instead of over the fixed [0, s_max]."""
+
+    def __init__(self, box, observer):
+        self.box = None if box is None else _f64(box)
+        self.obs = _f64(observer)
+
+    def __enter__(self):
+        if self.box is not None and lib().oracle_set_clip_box(_p(self.box), _p(self.obs)):
+            raise ValueError("observer must be strictly inside the clip box")
+
+    def __exit__(self, *a):
+        lib().oracle_set_clip_box(None, None)
+
+
+def exit_distance(observer, l, b, box):
+    lib().oracle_exit_distance.restype = ctypes.c_double
+    return float(lib().oracle_exit_distance(_p(_f64(observer)), ctypes.c_double(l), ctypes.c_double(b), _p(_f64(box))))
+
+
+def forward_dir(model: Model, l, b, n_los, s_max, freqs, observer=(-8.3, 0.0, 0.006), batch_index=0, clip_box=None):
     """I,Q,U [n_freq] (K) of one sightline towards Galactic (l,b) [rad]."""
     freqs = _f64(freqs).ravel()
     obs = _f64(observer)
+    with _clip(clip_box, observer):
+        return _forward_dir(model, l, b, n_los, s_max, freqs, obs, batch_index)
+
+
+def _forward_dir(model, l, b, n_los, s_max, freqs, obs, batch_index):
     I = np.zeros(freqs.size); Q = np.zeros(freqs.size); U = np.zeros(freqs.size)
     lib().oracle_forward_dir(ctypes.c_int(model.k), _p(model.params[batch_index]), _p(model.aux), _p(model.gdim),
                              _p(model.gbox), ctypes.c_double(l), ctypes.c_double(b), ctypes.c_int64(n_los),
@@ -136,8 +162,13 @@ def forward_dir(model: Model, l, b, n_los, s_max, freqs, observer=(-8.3, 0.0, 0.
     return I, Q, U
 
 
-def forward(model: Model, nside, n_los, s_max, freqs, observer=(-8.3, 0.0, 0.006), pix=None):
+def forward(model: Model, nside, n_los, s_max, freqs, observer=(-8.3, 0.0, 0.006), pix=None, clip_box=None):
     """I,Q,U maps float64 [batch][n_freq][n_out] in Kelvin; pix=None -> all 12 nside^2 pixels."""
+    with _clip(clip_box, observer):
+        return _forward(model, nside, n_los, s_max, freqs, observer, pix)
+
+
+def _forward(model, nside, n_los, s_max, freqs, observer, pix):
     freqs = _f64(freqs).ravel()
     obs = _f64(observer)
     if pix is not None:
@@ -154,8 +185,13 @@ def forward(model: Model, nside, n_los, s_max, freqs, observer=(-8.3, 0.0, 0.006
     return I, Q, U
 
 
-def vjp(model: Model, nside, n_los, s_max, freqs, dI, dQ, dU, observer=(-8.3, 0.0, 0.006), pix=None):
+def vjp(model: Model, nside, n_los, s_max, freqs, dI, dQ, dU, observer=(-8.3, 0.0, 0.006), pix=None, clip_box=None):
     """grad float64 [batch][P] (grid_b: [nx][ny][nz][3]) for cotangent maps [batch][n_freq][n_out]."""
+    with _clip(clip_box, observer):
+        return _vjp(model, nside, n_los, s_max, freqs, dI, dQ, dU, observer, pix)
+
+
+def _vjp(model, nside, n_los, s_max, freqs, dI, dQ, dU, observer, pix):
     freqs = _f64(freqs).ravel()
     obs = _f64(observer)
     if pix is not None:

@@ -397,6 +397,26 @@ struct Sightline {
   int64_t n_los; double s_max; const double* obs; const double* freqs; int n_freq;
 };
 
+// Integration extent of the paper (Fig. 1): from the observer to where the sightline leaves the
+// simulation box (centred on the Galactic centre, side lengths box[3]), cut into n_los equal segments, so each
+// sightline has its own Delta r_i.  Returns the exit distance, or a negative number if the observer is not
+// strictly inside the box.  When a clip box is set (oracle_set_clip_box) it REPLACES the fixed s_max.
+bool g_clip = false;
+double g_clip_box[3] = {0.0, 0.0, 0.0};
+double exit_distance(const double* obs, const double* n, const double* box) {
+  double L = std::numeric_limits<double>::infinity();
+  for (int k = 0; k < 3; ++k) {
+    const double half = 0.5 * box[k];
+    if (!(std::fabs(obs[k]) < half)) return -1.0;
+    if (n[k] > 0.0) L = std::fmin(L, (half - obs[k]) / n[k]);
+    else if (n[k] < 0.0) L = std::fmin(L, (-half - obs[k]) / n[k]);
+  }
+  return L;
+}
+double path_length(const double* obs, const Triad& T, double s_max) {
+  return g_clip ? exit_distance(obs, T.n, g_clip_box) : s_max;
+}
+
 void sightline_forward(const Model& m, const Sightline& S, const Triad& T,
                        double* I, double* Q, double* U /* [n_freq] */) {
   const int64_t N = S.n_los;
@@ -563,7 +583,8 @@ int oracle_forward_dir(int kind, const double* params, const double* aux, const 
                        double* I, double* Q, double* U) {
   const Model m = make_model(kind, params, aux, gdim, gbox, observer);
   Triad T; make_triad(l, b, T);
-  Sightline S{n_los, s_max, observer, freqs, n_freq};
+  Sightline S{n_los, path_length(observer, T, s_max), observer, freqs, n_freq};
+  if (!(S.s_max > 0.0)) return 1;
   sightline_forward(m, S, T, I, Q, U);
   return 0;
 }
@@ -579,12 +600,12 @@ int oracle_forward(int kind, const double* params, int64_t n_params, const doubl
   const int64_t n_out = pix ? n_pix : 12 * nside * nside;
   for (int64_t bi = 0; bi < batch; ++bi) {
     const Model m = make_model(kind, params + bi * n_params, aux, gdim, gbox, observer);
-    Sightline S{n_los, s_max, observer, freqs, n_freq};
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t k = 0; k < n_out; ++k) {
       const int64_t p = pix ? pix[k] : k;
       double z, phi; pix2ang_ring(nside, p, &z, &phi);
       Triad T; make_triad(phi, 0.5 * PI - std::acos(z), T);  // l = phi, b = pi/2 - theta
+      Sightline S{n_los, path_length(observer, T, s_max), observer, freqs, n_freq};
       double Iv[64], Qv[64], Uv[64];
       sightline_forward(m, S, T, Iv, Qv, Uv);
       for (int f = 0; f < n_freq; ++f) {
@@ -607,7 +628,6 @@ int oracle_vjp(int kind, const double* params, int64_t n_params, const double* a
   const int64_t n_out = pix ? n_pix : 12 * nside * nside;
   for (int64_t bi = 0; bi < batch; ++bi) {
     const Model m = make_model(kind, params + bi * n_params, aux, gdim, gbox, observer);
-    Sightline S{n_los, s_max, observer, freqs, n_freq};
     double* g_out = grad + bi * n_params;
     for (int64_t j = 0; j < n_params; ++j) g_out[j] = 0.0;
 #pragma omp parallel
@@ -618,6 +638,7 @@ int oracle_vjp(int kind, const double* params, int64_t n_params, const double* a
         const int64_t p = pix ? pix[k] : k;
         double z, phi; pix2ang_ring(nside, p, &z, &phi);
         Triad T; make_triad(phi, 0.5 * PI - std::acos(z), T);
+        Sightline S{n_los, path_length(observer, T, s_max), observer, freqs, n_freq};
         double a[64], b[64], c[64];
         for (int f = 0; f < n_freq; ++f) {
           const int64_t o = (bi * n_freq + f) * n_out + k;
@@ -630,6 +651,23 @@ int oracle_vjp(int kind, const double* params, int64_t n_params, const double* a
     }
   }
   return 0;
+}
+
+// box == NULL: integrate every sightline over [0, s_max] (BASELINE.json configs); else clip at the box faces.
+// Returns 1 if the observer is not strictly inside the box.
+int oracle_set_clip_box(const double* box, const double* observer) {
+  if (!box) { g_clip = false; return 0; }
+  for (int k = 0; k < 3; ++k) {
+    if (!(box[k] > 0.0) || (observer && !(std::fabs(observer[k]) < 0.5 * box[k]))) return 1;
+    g_clip_box[k] = box[k];
+  }
+  g_clip = true;
+  return 0;
+}
+// exit distance of one direction (for the pins)
+double oracle_exit_distance(const double* observer, double l, double b, const double* box) {
+  Triad T; make_triad(l, b, T);
+  return exit_distance(observer, T.n, box);
 }
 
 int oracle_num_threads(void) {

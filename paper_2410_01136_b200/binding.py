@@ -18,7 +18,7 @@ STATUS = {0: "SYNAX_OK", 1: "SYNAX_ERR_INVALID_ARG", 2: "SYNAX_ERR_UNSUPPORTED",
 KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
 
 # every symbol include/synax.h declares
-exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_option",
+exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_box", "synax_plan_set_option",
                     "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
@@ -57,6 +57,8 @@ def load_library() -> ctypes.CDLL:
     L.synax_plan_destroy.restype = ctypes.c_int
     L.synax_plan_npix.argtypes = [vp]
     L.synax_plan_npix.restype = i64
+    L.synax_plan_set_box.argtypes = [vp, ctypes.POINTER(dbl)]
+    L.synax_plan_set_box.restype = ctypes.c_int
     L.synax_plan_set_option.argtypes = [vp, ctypes.c_char_p, dbl]
     L.synax_plan_set_option.restype = ctypes.c_int
     L.synax_plan_directions.argtypes = [vp, vp, vp]
@@ -129,6 +131,14 @@ class Plan:
         self.nside, self.n_los, self.s_max, self.freqs = int(nside), int(n_los), float(s_max), f
         self.n_freq = int(f.size)
         self.npix = int(L.synax_plan_npix(h))
+
+    def set_box(self, box):
+        """synax_plan_set_box: integrate from the observer to the faces of a box (lx, ly, lz kpc); None = fixed s_max."""
+        if box is None:
+            _check(load_library().synax_plan_set_box(self.h, None))
+        else:
+            b = (ctypes.c_double * 3)(*[float(v) for v in box])
+            _check(load_library().synax_plan_set_box(self.h, b))
 
     def set_option(self, key: str, value: float):
         _check(load_library().synax_plan_set_option(self.h, key.encode(), float(value)))

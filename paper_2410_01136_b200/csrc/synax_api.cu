@@ -41,6 +41,9 @@ struct synax_plan {
   double s_max, delta;
   double obs[3];
   double* dirs;       // device [npix][4]
+  double* path;       // device [npix] path length / s_max, or null (every sightline integrates [0, s_max])
+  double s_max_fixed; // s_max given at creation (restored when the box is removed)
+  double freqs[kMaxFreq];
   FreqTab ft;
   int precision;      // 0 auto, 1 fp32 only, 2 float64 chain everywhere
   double escalate_rad;
@@ -54,6 +57,21 @@ struct synax_plan {
 static double faraday_K_per_kpc() {
   const double K = SYNAX_QE * SYNAX_QE * SYNAX_QE / (2.0 * SYNAX_PI * SYNAX_ME * SYNAX_ME * SYNAX_C * SYNAX_C * SYNAX_C * SYNAX_C);
   return K * 1.0e4 * 1.0e-6 * SYNAX_KPC;  // rad m^-2 per (cm^-3 uG kpc), Eq.(7)
+}
+
+// k_f = 2 lambda_f^2 K_F delta: Faraday angle per unit sum(n_e B_LOS) for the plan's segment length (Eq.(6)-(7))
+static void fill_freq_table(synax_plan* p) {
+  const double KF = faraday_K_per_kpc();
+  p->ft.n_freq = p->n_freq;
+  for (int f = 0; f < kMaxFreq; ++f) {
+    if (f < p->n_freq) {
+      const double lam = SYNAX_C / p->freqs[f] * 1.0e-2;  // m
+      const double k = 2.0 * lam * lam * KF * p->delta;   // rad per unit sum(n_e B_LOS)
+      p->ft.k_rad[f] = (float)k; p->ft.k_turn[f] = k / (2.0 * SYNAX_PI); p->ft.freq[f] = p->freqs[f];
+    } else {
+      p->ft.k_rad[f] = 0.f; p->ft.k_turn[f] = 0.0; p->ft.freq[f] = 1.0;
+    }
+  }
 }
 
 extern "C" const char* synax_last_error(void) { return g_err; }
@@ -91,20 +109,11 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   std::memset(p, 0, sizeof(*p));
   p->nside = nside; p->n_los = n_los; p->n_freq = n_freq;
   p->npix = pix_count; p->pix0 = pix_begin;
-  p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los;
+  p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los; p->s_max_fixed = s_max_kpc; p->path = nullptr;
+  for (int f = 0; f < n_freq; ++f) p->freqs[f] = freqs_hz[f];
   for (int i = 0; i < 3; ++i) p->obs[i] = observer_kpc[i];
   p->precision = 0; p->escalate_rad = 100.0; p->lanes = 0;
-  const double KF = faraday_K_per_kpc();
-  p->ft.n_freq = n_freq;
-  for (int f = 0; f < kMaxFreq; ++f) {
-    if (f < n_freq) {
-      const double lam = SYNAX_C / freqs_hz[f] * 1.0e-2;  // m
-      const double k = 2.0 * lam * lam * KF * p->delta;   // rad per unit sum(n_e B_LOS)
-      p->ft.k_rad[f] = (float)k; p->ft.k_turn[f] = k / (2.0 * SYNAX_PI); p->ft.freq[f] = freqs_hz[f];
-    } else {
-      p->ft.k_rad[f] = 0.f; p->ft.k_turn[f] = 0.0; p->ft.freq[f] = 1.0;
-    }
-  }
+  fill_freq_table(p);
   cudaError_t e = cudaGetDevice(&p->device);
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->dirs, (size_t)p->npix * 4 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, kCtrlWords * sizeof(int));
@@ -135,6 +144,7 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
 extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
   if (!plan) return SYNAX_OK;
   cudaFree(plan->dirs);
+  if (plan->path) cudaFree(plan->path);
   cudaFree(plan->d_flag_count);
   cudaFreeHost(plan->h_flag_count);
   delete plan;
@@ -142,6 +152,34 @@ extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
 }
 
 extern "C" int64_t synax_plan_npix(const synax_plan* plan) { return plan ? plan->npix : -1; }
+
+extern "C" synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]) {
+  if (!plan) return fail(SYNAX_ERR_INVALID_ARG, "plan is NULL");
+  if (!box_kpc) {   // back to the fixed [0, s_max]
+    if (plan->path) { cudaFree(plan->path); plan->path = nullptr; }
+    plan->s_max = plan->s_max_fixed; plan->delta = plan->s_max / (double)plan->n_los;
+    fill_freq_table(plan);
+    return SYNAX_OK;
+  }
+  double far2 = 0.0;
+  for (int k = 0; k < 3; ++k) {
+    if (!(box_kpc[k] > 0.0) || !std::isfinite(box_kpc[k])) return fail(SYNAX_ERR_INVALID_ARG, "box lengths must be > 0");
+    if (!(std::fabs(plan->obs[k]) < 0.5 * box_kpc[k])) return fail(SYNAX_ERR_INVALID_ARG, "the observer must be strictly inside the box");
+    const double d = 0.5 * box_kpc[k] + std::fabs(plan->obs[k]);
+    far2 += d * d;
+  }
+  if (!plan->path) CUDA_TRY(cudaMalloc((void**)&plan->path, (size_t)plan->npix * sizeof(double)));
+  // reference length = distance to the farthest corner, so that every path[i] <= 1 (tile-length bounds stay valid)
+  plan->s_max = std::sqrt(far2); plan->delta = plan->s_max / (double)plan->n_los;
+  fill_freq_table(plan);
+  box_path_kernel<<<(unsigned)((plan->npix + 255) / 256), 256>>>(plan->dirs, plan->npix, plan->obs[0], plan->obs[1], plan->obs[2],
+                                                               0.5 * box_kpc[0], 0.5 * box_kpc[1], 0.5 * box_kpc[2],
+                                                               1.0 / plan->s_max, plan->path);
+  plan->launches++;
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaDeviceSynchronize());
+  return SYNAX_OK;
+}
 
 extern "C" synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value) {
   if (!plan || !key) return fail(SYNAX_ERR_INVALID_ARG, "plan or key is NULL");
@@ -267,7 +305,7 @@ static Geometry make_geo(const synax_plan* plan) {
   Geometry g;
   g.npix = plan->npix; g.n_los = plan->n_los; g.delta = plan->delta;
   for (int i = 0; i < 3; ++i) g.obs[i] = plan->obs[i];
-  g.dirs = plan->dirs;
+  g.dirs = plan->dirs; g.path = plan->path;
   return g;
 }
 

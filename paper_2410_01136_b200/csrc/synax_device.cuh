@@ -132,6 +132,8 @@ struct Geometry {
   double delta;   // s_max / n_los  (kpc)
   double obs[3];
   const double* dirs;  // [npix][4] = cos l, sin l, cos b, sin b
+  const double* path;  // [npix] path length of the sightline in units of s_max = n_los * delta, or null (= 1):
+                       // set by synax_plan_set_box (integration from the observer to the box face)
 };
 
 // per-sightline direction triad
@@ -141,6 +143,8 @@ struct Triad {
   float nxl, nyl, nzl;     // n - (float)n: low parts, so that B.n does not carry a per-sightline 3e-8 bias
   float eNx, eNy, eNz;     // towards Galactic north
   float eEx, eEy;          // towards increasing l (z component is 0)
+  double scale;            // Delta_i / delta: this sightline's segment length relative to the plan's (1 without a box)
+  float scalef;
 };
 
 __device__ __forceinline__ Triad load_triad(const double* __restrict__ dirs, int64_t pix) {
@@ -151,6 +155,15 @@ __device__ __forceinline__ Triad load_triad(const double* __restrict__ dirs, int
   t.nxl = (float)(t.nxd - (double)t.nx); t.nyl = (float)(t.nyd - (double)t.ny); t.nzl = (float)(t.nzd - (double)t.nz);
   t.eNx = (float)(-d.w * d.x); t.eNy = (float)(-d.w * d.y); t.eNz = (float)d.z;
   t.eEx = (float)(-d.y); t.eEy = (float)d.x;
+  t.scale = 1.0; t.scalef = 1.0f;
+  return t;
+}
+// With the per-sightline segment length: positions step by delta * scale, and because the Faraday constants k_f and
+// the intensity coefficients c_f are folded with the plan's delta, n_e (which enters only through the Faraday
+// integrand n_e B_LOS Delta) and the final sums (cotangents in the adjoint) are multiplied by scale.
+__device__ __forceinline__ Triad load_triad(const Geometry& geo, int64_t pix) {
+  Triad t = load_triad(geo.dirs, pix);
+  if (geo.path) { t.scale = geo.path[pix]; t.scalef = (float)t.scale; }
   return t;
 }
 

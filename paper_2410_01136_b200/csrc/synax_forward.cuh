@@ -66,6 +66,24 @@ __global__ void pix2ang_kernel(int64_t nside, int64_t pix0, int64_t count, doubl
   dirs[4 * idx + 0] = cl; dirs[4 * idx + 1] = sl; dirs[4 * idx + 2] = cb; dirs[4 * idx + 3] = z;
 }
 
+// Path length of every sightline of the plan from the observer (strictly inside the box) to the face of a box of
+// side lengths `box` centred on the Galactic centre, in units of s_ref (Fig. 1): path[i] = L_i / s_ref.
+__global__ void box_path_kernel(const double* __restrict__ dirs, int64_t count, double ox, double oy, double oz,
+                                double hx, double hy, double hz, double inv_s_ref, double* __restrict__ path) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  const double4 d = *reinterpret_cast<const double4*>(dirs + 4 * i);   // cos l, sin l, cos b, sin b
+  const double n[3] = {d.z * d.x, d.z * d.y, d.w};
+  const double o[3] = {ox, oy, oz}, h[3] = {hx, hy, hz};
+  double L = 1.0e300;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    if (n[k] > 0.0) L = fmin(L, (h[k] - o[k]) / n[k]);
+    else if (n[k] < 0.0) L = fmin(L, (-h[k] - o[k]) / n[k]);
+  }
+  path[i] = L * inv_s_ref;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Prologue: raw parameters -> BatchConsts (float64 math, once per batch element per call).
 // Folds Eq.(2)'s constants, the Rayleigh-Jeans conversion (S:C-2#1) and the units into
@@ -260,12 +278,12 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
   const int b = (int)(sl / A.geo.npix);
   const int64_t pix = sl - (int64_t)b * A.geo.npix;
   const BatchConsts& P = A.bc[b];
-  const Triad T = load_triad(A.geo.dirs, pix);
+  const Triad T = load_triad(A.geo, pix);
 
   const int C = (A.geo.n_los + G - 1) / G;
   const int n0 = g * C;
   const int n1 = min(n0 + C, A.geo.n_los);
-  const double delta = A.geo.delta;
+  const double delta = A.geo.delta * T.scale;
   double s_d = ((double)n0 + 0.5) * delta;
 
   float k_rad[NF];
@@ -302,6 +320,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         AnalyticAux aux;
         eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
+      S.ne *= T.scalef;
       float eI, a, bq;
       emission(P, S.BN, S.BE, S.N0, eI, a, bq);
       accI += eI;
@@ -354,9 +373,9 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * npix + pix;
-      A.I[o] = P.coefI[A.f0 + f] * accI;
-      A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
-      A.U[o] = P.coefP[A.f0 + f] * accU[f];
+      A.I[o] = P.coefI[A.f0 + f] * T.scalef * accI;
+      A.Q[o] = P.coefP[A.f0 + f] * T.scalef * accQ[f];
+      A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
     }
     if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
       const int k = atomicAdd(A.flag_count, 1);
@@ -386,7 +405,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
   const int C = (A.geo.n_los + G - 1) / G;
   const int n0 = g * C;
   const int n1 = min(n0 + C, A.geo.n_los);
-  const double delta = A.geo.delta;
+  const double delta0 = A.geo.delta;
   float k_rad[NF];
 #pragma unroll
   for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[f];
@@ -400,7 +419,8 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
     const int64_t pix = sl - (int64_t)b * A.geo.npix;
     const BatchConsts& P = A.bc[b];
     const BatchConstsD D = A.bd[b];   // by value: kept in registers across the sample loop
-    const Triad T = load_triad(A.geo.dirs, pix);
+    const Triad T = load_triad(A.geo, pix);
+    const double delta = delta0 * T.scale;
     double s_d = ((double)n0 + 0.5) * delta;
     float accI = 0.0f, accQ[NF], accU[NF];
 #pragma unroll
@@ -433,10 +453,12 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
         if (CODE == kUniform) {
 #pragma unroll
           for (int j = 0; j < kUnrollD; ++j) {
-            Bx[j] = (double)P.uB[0]; By[j] = (double)P.uB[1]; Bz[j] = (double)P.uB[2]; ne[j] = (double)P.une; N0[j] = P.uN0;
+            Bx[j] = (double)P.uB[0]; By[j] = (double)P.uB[1]; Bz[j] = (double)P.uB[2]; ne[j] = (double)P.une * T.scale; N0[j] = P.uN0;
           }
         } else {
           eval_analytic_dm<CODE == kAnalyticFull, kUnrollD>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
+#pragma unroll
+          for (int j = 0; j < kUnrollD; ++j) ne[j] *= T.scale;
 #pragma unroll
           for (int j = 0; j < kUnrollD; ++j) {
             // N_0 (emission only): fp32 MUFU chain, Eq.(12)
@@ -489,9 +511,9 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * npix + pix;
-        A.I[o] = P.coefI[A.f0 + f] * accI;
-        A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
-        A.U[o] = P.coefP[A.f0 + f] * accU[f];
+        A.I[o] = P.coefI[A.f0 + f] * T.scalef * accI;
+        A.Q[o] = P.coefP[A.f0 + f] * T.scalef * accQ[f];
+        A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
       }
     }
   }
@@ -513,12 +535,12 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
   const int b = (int)(sl / A.geo.npix);
   const int64_t pix = sl - (int64_t)b * A.geo.npix;
   const BatchConsts& P = A.bc[b];
-  const Triad T = load_triad(A.geo.dirs, pix);
+  const Triad T = load_triad(A.geo, pix);
   const int C = (A.geo.n_los + 31) / 32;
   const int n0 = lane * C, n1 = min(n0 + C, A.geo.n_los);
   float gabs = 0.0f;
   for (int n = n0; n < n1; ++n) {
-    const double s_d = ((double)n + 0.5) * A.geo.delta;
+    const double s_d = ((double)n + 0.5) * A.geo.delta * T.scale;
     float gn;
     if (CODE == kUniform) {
       gn = fabsf(P.une) * (fabsf(P.uB[0]) + fabsf(P.uB[1]) + fabsf(P.uB[2]));
@@ -534,7 +556,7 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
     }
     gabs += gn;
   }
-  const float absS = group_sum<32>(gabs);
+  const float absS = T.scalef * group_sum<32>(gabs);
   if (lane == 0 && absS > A.flag_S) atomicAdd(ctrl + kCtrlPilotFlagged, 1);
 }
 

@@ -168,7 +168,7 @@ __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const
                                                         const Geometry& geo, int lane) {
   float acc = 0.f;
   for (int n = 4 + 8 * lane; n < geo.n_los; n += 256) {
-    const double s_d = ((double)n + 0.5) * geo.delta;
+    const double s_d = ((double)n + 0.5) * geo.delta * T.scale;
     const double xd = fma(s_d, T.nxd, geo.obs[0]), yd = fma(s_d, T.nyd, geo.obs[1]), zd = fma(s_d, T.nzd, geo.obs[2]);
     const Cell c = locate(G, xd, yd, zd);
     float B[3], N0, ne;
@@ -179,7 +179,7 @@ __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const
     const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
     acc = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), acc);
   }
-  return 8.0f * group_sum<32>(acc);
+  return 8.0f * T.scalef * group_sum<32>(acc);
 }
 
 // One sightline, whole warp, lanes on CONSECUTIVE samples (neighbouring lanes gather neighbouring cells).
@@ -194,7 +194,7 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
   for (int f = 0; f < NF; ++f) { accQ[f] = 0.f; accU[f] = 0.f; }
   double carry = 0.0;
   float absS = 0.f;
-  const double delta = A.geo.delta;
+  const double delta = A.geo.delta * T.scale;
   for (int nt = 0; nt < A.geo.n_los; nt += 32) {
     const int n = nt + lane;
     const bool active = n < A.geo.n_los;
@@ -210,6 +210,7 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       gather_B(G, c, B);
       float N0, ne;
       densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      ne *= T.scalef;
       const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
       const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
       const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
@@ -223,6 +224,7 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       double Bpar, BN, BE, ne;
       float N0;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BN, BE, N0, ne);
+      ne *= T.scale;
       if (active) emission(P, (float)BN, (float)BE, N0, eI, a, bq);
       const double gn = active ? ne * Bpar : 0.0;
       const double incl = warp_inclusive_scan_d(gn, lane);
@@ -261,7 +263,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
   const BatchConstsD D = A.bd[0];
   for (int64_t pix = warp; pix < A.geo.npix; pix += n_warps) {
     const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
-    const Triad T = load_triad(A.geo.dirs, pix);
+    const Triad T = load_triad(A.geo, pix);
     float accI, accQ[NF], accU[NF];
     bool precise = GA.mode == 2;
     if (GA.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, lane) > A.flag_S;
@@ -274,9 +276,9 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         const int64_t o = (int64_t)(A.f0 + f) * A.geo.npix + pix;
-        A.I[o] = P.coefI[A.f0 + f] * accI;
-        A.Q[o] = P.coefP[A.f0 + f] * accQ[f];
-        A.U[o] = P.coefP[A.f0 + f] * accU[f];
+        A.I[o] = P.coefI[A.f0 + f] * T.scalef * accI;
+        A.Q[o] = P.coefP[A.f0 + f] * T.scalef * accQ[f];
+        A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
       }
       if (precise && GA.mode == 0 && A.f0 == 0) atomicAdd(A.flag_count, 1);
     }
@@ -322,7 +324,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
                                                  float cI, const float (&cQ)[NF], const float (&cU)[NF],
                                                  const float (&kr)[NF], float* st_w, float* st_n, float* st_e) {
   const int C = 1 << A.chunk_log2, Cp = C + 1;
-  const double delta = A.geo.delta;
+  const double delta = A.geo.delta * T.scale;
   double carry = 0.0;
   float absS = 0.f;
   for (int nt = 0; nt < A.geo.n_los; nt += 32) {
@@ -339,6 +341,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       float B[3];
       gather_B(G, c, B);
       densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      ne *= T.scalef;
       const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
       BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
       BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
@@ -350,6 +353,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
     } else {
       double Bpar, BNd, BEd, ned;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BNd, BEd, N0, ned);
+      ned *= T.scale;
       BN = (float)BNd; BE = (float)BEd; ne = (float)ned;
       const double gn = active ? ned * Bpar : 0.0;
       const double incl = warp_inclusive_scan_d(gn, lane);
@@ -399,17 +403,17 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
   const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
   const BatchConsts& P = A.bc[0];
   const BatchConstsD D = A.bd[0];
-  const double delta = A.geo.delta;
   for (int64_t pix = warp; pix < A.geo.npix; pix += n_warps) {
-    const Triad T = load_triad(A.geo.dirs, pix);
+    const Triad T = load_triad(A.geo, pix);
+    const double delta = A.geo.delta * T.scale;
     const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
     float cI = 0.f, cQ[NF], cU[NF], kr[NF];
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       const int64_t o = (int64_t)(A.f0 + f) * A.geo.npix + pix;
-      cI = fmaf(A.dI ? __ldg(A.dI + o) : 0.f, P.coefI[A.f0 + f], cI);
-      cQ[f] = (A.dQ ? __ldg(A.dQ + o) : 0.f) * P.coefP[A.f0 + f];
-      cU[f] = (A.dU ? __ldg(A.dU + o) : 0.f) * P.coefP[A.f0 + f];
+      cI = fmaf(A.dI ? __ldg(A.dI + o) : 0.f, P.coefI[A.f0 + f] * T.scalef, cI);
+      cQ[f] = (A.dQ ? __ldg(A.dQ + o) : 0.f) * P.coefP[A.f0 + f] * T.scalef;
+      cU[f] = (A.dU ? __ldg(A.dU + o) : 0.f) * P.coefP[A.f0 + f] * T.scalef;
       kr[f] = ft.k_rad[f];
     }
     // ---- sweep 1: consecutive samples per lane; fp32 chain first, redone with the float64 Faraday chain
@@ -450,6 +454,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
         c = locate(G, xd, yd, zd);
         float N0_unused;
         densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0_unused, ne_m);
+        ne_m *= T.scalef;
       }
       const int cell = (m >= m0 && c.inbox) ? c.base : -1;
       if (cell != cur) {

@@ -120,7 +120,7 @@ struct UniformGrad {
     b1[2] += fmaf(BNb, T.eNz, -wn * T.nz);
     b2[0] += S.ne * T.nx; b2[1] += S.ne * T.ny; b2[2] += S.ne * T.nz;
     n1 += MK;                         // * 1/N0
-    e1 -= wgt * S.Bpar; e2 += S.Bpar;  // d(ne Bpar)/d ne = Bpar
+    e1 -= wgt * T.scalef * S.Bpar; e2 += T.scalef * S.Bpar;  // d(scale ne Bpar)/d ne = scale Bpar (S.ne carries scale)
   }
   __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
     for (int j = 0; j < 3; ++j) out[j] = fmaf(Tw, b2[j], b1[j]);
@@ -153,10 +153,10 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   const bool valid = pix < A.geo.npix;
   if (!valid) pix = A.geo.npix - 1;
   const BatchConsts& P = A.bc[b];
-  const Triad T = load_triad(A.geo.dirs, pix);
+  const Triad T = load_triad(A.geo, pix);
   const int C = (A.geo.n_los + G - 1) / G;
   const int n0 = g * C, n1 = min(n0 + C, A.geo.n_los);
-  const double delta = A.geo.delta;
+  const double delta = A.geo.delta * T.scale;
 
   // cotangents of this sightline, coefficients folded in (zero for padded lanes)
   // (dQ, dU are re-read at every tile start -- L1 hits -- instead of being held in 2 NF registers)
@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
     const float vI = (valid && A.dI) ? A.dI[o0 + f * A.geo.npix] : 0.f;
     cI = fmaf(vI, P.coefI[A.f0 + f], cI);
   }
+  cI *= T.scalef;   // the maps are scale * coef * sums (per-sightline segment length, synax_plan_set_box)
 
   // ---- pre-pass (G > 1): Faraday sum of each lane's chunk -> float64 offset of the preceding lanes
   double off = 0.0;
@@ -188,7 +189,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
       }
-      const float gn = S.ne * S.Bpar;
+      const float gn = T.scalef * S.ne * S.Bpar;
       const float sum = hi + gn;
       lo += gn - (sum - hi);
       hi = sum;
@@ -216,8 +217,8 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       // Qb cos(tb + tl) + Ub sin(tb + tl) = Qb' cos tl + Ub' sin tl,  Qb' = Qb cb + Ub sb, Ub' = -Qb sb + Ub cb
-      float q = (valid && A.dQ) ? __ldg(A.dQ + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] : 0.f;
-      float u = (valid && A.dU) ? __ldg(A.dU + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] : 0.f;
+      float q = (valid && A.dQ) ? __ldg(A.dQ + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] * T.scalef : 0.f;
+      float u = (valid && A.dU) ? __ldg(A.dU + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] * T.scalef : 0.f;
       rotate_by_offset(-ft.k_turn[f], off + carry, q, u);
       rq[f] = q; ru[f] = u;
     }
@@ -240,6 +241,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
       }
+      S.ne *= T.scalef;   // n_e enters only through the Faraday integrand n_e B_LOS Delta_i
       // emission terms
       const float bn2 = S.BN * S.BN, be2 = S.BE * S.BE;
       const float Bt2 = bn2 + be2;
@@ -309,7 +311,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * A.geo.npix + pix;
-      const float vI = (valid && A.dI) ? A.dI[o] * P.coefI[A.f0 + f] : 0.f;
+      const float vI = (valid && A.dI) ? A.dI[o] * P.coefI[A.f0 + f] * T.scalef : 0.f;
       ga = fmaf(P.dlnc_dalpha[A.f0 + f], fmaf(vI, sumE, pq[f]), ga);
       ga = fmaf(P.dpi_dalpha_over_pi, pq[f], ga);
     }

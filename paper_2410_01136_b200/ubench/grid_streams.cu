@@ -117,7 +117,7 @@ int main() {
   CK(cudaMemset(grid, 0, ngrid * 4)); CK(cudaMemset(grad, 0, ngrid * 4));
   pix2ang_kernel<<<(unsigned)((npix + 255) / 256), 256>>>(nside, 0, npix, dirs);
   Geometry geo; geo.npix = npix; geo.n_los = n_los; geo.delta = s_max / n_los;
-  geo.obs[0] = -8.3; geo.obs[1] = 0.0; geo.obs[2] = 0.006; geo.dirs = dirs;
+  geo.obs[0] = -8.3; geo.obs[1] = 0.0; geo.obs[2] = 0.006; geo.dirs = dirs; geo.path = nullptr;
   GridDesc G; G.g = grid; G.nx = nx; G.ny = ny; G.nz = nz;
   G.sx = (nx - 1) / 40.0; G.sy = (ny - 1) / 40.0; G.sz = (nz - 1) / 8.0;
   G.bx = 0.5 * (nx - 1); G.by = 0.5 * (ny - 1); G.bz = 0.5 * (nz - 1);

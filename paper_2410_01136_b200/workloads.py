@@ -55,6 +55,7 @@ class Workload:
     box: Optional[tuple] = None  # grid_b: (lx, ly, lz) kpc
     cot_seed: int = 0
     observer: tuple = OBSERVER
+    clip_box: Optional[tuple] = None  # (lx, ly, lz) kpc: integrate observer -> box face instead of [0, s_max]
 
     @property
     def npix(self) -> int:

@@ -18,17 +18,21 @@ def oracle_model(w: wl.Workload) -> oracle.Model:
 
 
 def oracle_forward(w: wl.Workload, pix=None):
-    return oracle.forward(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix=pix)
+    return oracle.forward(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix=pix,
+                          clip_box=w.clip_box)
 
 
 def oracle_vjp(w: wl.Workload, cots, pix=None):
-    return oracle.vjp(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, *cots, observer=w.observer, pix=pix)
+    return oracle.vjp(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, *cots, observer=w.observer, pix=pix,
+                      clip_box=w.clip_box)
 
 
 def gpu_objects(w: wl.Workload, pix_range=None, **options):
     import torch
     import paper_2410_01136_b200 as sx
     plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
+    if w.clip_box is not None:
+        plan.set_box(w.clip_box)
     for k, v in options.items():
         plan.set_option(k, v)
     if w.kind == "grid_b":
