@@ -130,6 +130,9 @@ struct BatchConstsD {
   double Bh, zh0, inv_rh, inv_wh;
   double ne0x4, k_her, k_hez;   // 4 ne0, -log2(e)/h_er, -2 log2(e)/|h_ez|
   int psi1_small;         // |psi1| <= 0.05: the MUFU lg2 (abs err 2e-7) is accurate enough for ln(rho/8)
+  int angles_small;       // |psi0| + |psi1| <= pi/4 and |chi0| <= pi/4: psi (|ln(rho/8)| < 1 inside the annulus) and
+                          // chi = chi0 tanh z never leave [-pi/4, pi/4], so sincos needs no range reduction
+  int hez_is_one;         // h_ez == 1 kpc exactly: exp(-2|z|/h_ez) is the tanh(z / 1 kpc) exponential, evaluated once
 };
 
 // M independent sincos in lockstep (same polynomials as sincos_d)
@@ -165,6 +168,27 @@ __device__ __forceinline__ void sincos_d_n(const double (&x)[M], double (&s)[M],
   }
 }
 
+// the same polynomials without range reduction, for arguments known to lie in [-pi/4, pi/4]
+template <int M>
+__device__ __forceinline__ void sincos_d_small_n(const double (&x)[M], double (&s)[M], double (&c)[M]) {
+  double r2[M], ps[M], pc[M];
+#pragma unroll
+  for (int j = 0; j < M; ++j) { r2[j] = x[j] * x[j]; ps[j] = kSinC[0]; pc[j] = kCosC[0]; }
+#pragma unroll
+  for (int i = 1; i < 6; ++i) {
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      if (i < 5) ps[j] = fma(ps[j], r2[j], kSinC[i]);
+      pc[j] = fma(pc[j], r2[j], kCosC[i]);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < M; ++j) {
+    s[j] = fma(ps[j] * r2[j], x[j], x[j]);
+    c[j] = fma(pc[j], r2[j], 1.0);
+  }
+}
+
 // B (Cartesian, uG) and n_e (cm^-3) at M consecutive samples of one sightline, float64 with the short
 // polynomials above.  Eq.(12)-(13) P:L173-180 and the halo of DESIGN.md section 3 (S:App.C); `inside` as in
 // the fp32 chain.  Everything is advanced in lockstep over the M samples and over the independent functions
@@ -188,33 +212,48 @@ __device__ __forceinline__ void eval_analytic_dm(const BatchConstsD& D, const do
   }
   double Brho[M], Bphi[M], ee[M], er[M], eh[M];
   if (any) {
+    // exponentials of this sample in lockstep: n_e's two, tanh's (skipped when it IS n_e's z-exponential), halo's two
     constexpr int NE = kHalo ? 5 : 3;
     double xs[NE * M], o[NE * M];
 #pragma unroll
     for (int j = 0; j < M; ++j) {
       xs[j] = D.k_hez * az[j];
       xs[M + j] = D.k_her * rho[j];
-      xs[2 * M + j] = -2.0 * kLog2e * az[j];
       if (kHalo) {
-        xs[3 * M + j] = kLog2e * (1.0 - q[j]);
-        xs[4 * M + j] = D.k_hb * (rho[j] - 8.0);
+        xs[2 * M + j] = kLog2e * (1.0 - q[j]);
+        xs[3 * M + j] = D.k_hb * (rho[j] - 8.0);
+        xs[4 * M + j] = -2.0 * kLog2e * az[j];
+      } else {
+        xs[2 * M + j] = -2.0 * kLog2e * az[j];
       }
     }
-    exp2_d_n<NE * M>(xs, o);
+    if (D.hez_is_one) {
+      double xr[(NE - 1) * M], orr[(NE - 1) * M];
+#pragma unroll
+      for (int j = 0; j < (NE - 1) * M; ++j) xr[j] = xs[j];
+      exp2_d_n<(NE - 1) * M>(xr, orr);
+#pragma unroll
+      for (int j = 0; j < (NE - 1) * M; ++j) o[j] = orr[j];
+#pragma unroll
+      for (int j = 0; j < M; ++j) o[(NE - 1) * M + j] = orr[j];
+    } else {
+      exp2_d_n<NE * M>(xs, o);
+    }
     double ang[2 * M], sn[2 * M], cs[2 * M], A[M];
 #pragma unroll
     for (int j = 0; j < M; ++j) {
       ee[j] = o[j]; er[j] = o[M + j];
-      const double e1 = o[2 * M + j];
-      eh[j] = kHalo ? o[3 * M + j] : 0.0;
-      A[j] = inside[j] ? (kHalo ? D.b0 * o[4 * M + j] : D.b0) : 0.0;
+      const double e1 = o[(NE - 1) * M + j];
+      eh[j] = kHalo ? o[2 * M + j] : 0.0;
+      A[j] = inside[j] ? (kHalo ? D.b0 * o[3 * M + j] : D.b0) : 0.0;
       const double lr = D.psi1_small ? (double)((mufu_lg2((float)rho2[j]) - 6.0f) * 0.34657359027997264f)
                                      : 0.5 * log_d(rho2[j] * 0.015625);
       const double th = (1.0 - e1) * rcp_d(1.0 + e1);           // tanh|z| = (1 - e)/(1 + e)
       ang[j] = fma(D.psi1, lr, D.psi0);
       ang[M + j] = D.chi0 * copysign(th, z[j]);
     }
-    sincos_d_n<2 * M>(ang, sn, cs);
+    if (D.angles_small) sincos_d_small_n<2 * M>(ang, sn, cs);
+    else sincos_d_n<2 * M>(ang, sn, cs);
 #pragma unroll
     for (int j = 0; j < M; ++j) {
       const double Acc = A[j] * cs[M + j];

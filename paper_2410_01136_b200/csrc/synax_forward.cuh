@@ -178,6 +178,8 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     d.Bh = p[5]; d.zh0 = p[6]; d.inv_rh = 1.0 / p[7]; d.inv_wh = 1.0 / p[8];
     d.ne0x4 = 4.0 * p[13]; d.k_her = -log2e / p[14]; d.k_hez = -2.0 * log2e / fabs(p[15]);
     d.psi1_small = fabs(p[2]) <= 0.05 ? 1 : 0;
+    d.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4
+    d.hez_is_one = (p[15] == 1.0 || p[15] == -1.0) ? 1 : 0;
     outd[b] = d;
   }
 }
