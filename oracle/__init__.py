@@ -125,6 +125,29 @@ def eval_fields(model: Model, r, observer=(-8.3, 0.0, 0.006), b=0):
     return B, N0, ne, al
 
 
+class scalar_grids:
+    """Context manager: n_e and / or N_0 of the DISC4 and GRID_B models come from regular grids [nx][ny][nz] over
+    boxes (lx, ly, lz) centred on the Galactic centre, trilinear, zero outside."""
+
+    def __init__(self, ne=None, ne_box=None, n0=None, n0_box=None):
+        self.items = []
+        for which, g, b in ((0, ne, ne_box), (1, n0, n0_box)):
+            if g is not None:
+                g = _f64(g)
+                assert g.ndim == 3
+                self.items.append((which, g, np.asarray(g.shape, dtype=np.int64), _f64(b)))
+
+    def __enter__(self):
+        for which, g, dim, box in self.items:
+            if lib().oracle_set_scalar_grid(ctypes.c_int(which), _p(g), _p(dim), _p(box)):
+                raise ValueError("bad scalar grid")
+        return self
+
+    def __exit__(self, *a):
+        for which, *_ in self.items:
+            lib().oracle_set_scalar_grid(ctypes.c_int(which), None, None, None)
+
+
 class _clip:
     """Context manager: integrate from the observer to the faces of `box` (lx, ly, lz kpc, centred on the Galactic
     centre) instead of over the fixed [0, s_max]."""

@@ -167,6 +167,31 @@ void grid_field(const Model& m, double x, double y, double z, double B[3]) {
       }
 }
 
+// Gridded scalar fields (the paper's n_e is the YMW16 model sampled on a (256,256,64) grid;
+// N_0 may be gridded the same way): regular grid [nx][ny][nz], nodes on the faces of a box centred on the
+// Galactic centre, trilinear interpolation, zero outside.  Set process-wide by oracle_set_scalar_grids; they
+// REPLACE the analytic exponential discs of the DISC4 and GRID_B models (whose n_e / N_0 are not differentiated).
+struct ScalarGrid { const double* g = nullptr; int64_t n[3] = {0, 0, 0}; double len[3] = {0, 0, 0}; };
+ScalarGrid g_ne_grid, g_n0_grid;
+double scalar_grid_value(const ScalarGrid& S, double x, double y, double z) {
+  const double p[3] = {x, y, z};
+  int64_t i[3]; double t[3];
+  for (int a = 0; a < 3; ++a) {
+    const double u = (p[a] + 0.5 * S.len[a]) * (double)(S.n[a] - 1) / S.len[a];
+    if (!(u >= 0.0 && u <= (double)(S.n[a] - 1))) return 0.0;
+    int64_t k = (int64_t)std::floor(u);
+    if (k > S.n[a] - 2) k = S.n[a] - 2;
+    i[a] = k; t[a] = u - (double)k;
+  }
+  double v = 0.0;
+  for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b)
+      for (int d = 0; d < 2; ++d)
+        v += (a ? t[0] : 1.0 - t[0]) * (b ? t[1] : 1.0 - t[1]) * (d ? t[2] : 1.0 - t[2]) *
+             S.g[((i[0] + a) * S.n[1] + (i[1] + b)) * S.n[2] + (i[2] + d)];
+  return v;
+}
+
 // step 3: all fields at one point.
 void eval_fields(const Model& m, const double r[3], Fields& F) {
   const double x = r[0], y = r[1], z = r[2];
@@ -209,6 +234,10 @@ void eval_fields(const Model& m, const double r[3], Fields& F) {
       F.ne = inside ? p[4] : 0.0;
       F.alpha = p[5];
     } break;
+  }
+  if (m.kind == KIND_DISC4 || m.kind == KIND_GRID_B) {
+    if (g_ne_grid.g) F.ne = scalar_grid_value(g_ne_grid, x, y, z);
+    if (g_n0_grid.g) F.N0 = scalar_grid_value(g_n0_grid, x, y, z);
   }
 }
 
@@ -668,6 +697,18 @@ int oracle_set_clip_box(const double* box, const double* observer) {
 double oracle_exit_distance(const double* observer, double l, double b, const double* box) {
   Triad T; make_triad(l, b, T);
   return exit_distance(observer, T.n, box);
+}
+
+// which: 0 = n_e, 1 = N_0.  grid == NULL removes it.  The array must stay alive while set.
+int oracle_set_scalar_grid(int which, const double* grid, const int64_t* dim, const double* box) {
+  ScalarGrid& S = which == 0 ? g_ne_grid : g_n0_grid;
+  if (!grid) { S.g = nullptr; return 0; }
+  for (int a = 0; a < 3; ++a) {
+    if (dim[a] < 2 || !(box[a] > 0.0)) return 1;
+    S.n[a] = dim[a]; S.len[a] = box[a];
+  }
+  S.g = grid;
+  return 0;
 }
 
 int oracle_num_threads(void) {

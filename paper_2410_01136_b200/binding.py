@@ -32,7 +32,9 @@ class SynaxError(RuntimeError):
 class _CModel(ctypes.Structure):
     _fields_ = [("kind", ctypes.c_int32), ("n_params", ctypes.c_int32), ("aux", ctypes.POINTER(ctypes.c_float)),
                 ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
-                ("lx", ctypes.c_float), ("ly", ctypes.c_float), ("lz", ctypes.c_float)]
+                ("lx", ctypes.c_float), ("ly", ctypes.c_float), ("lz", ctypes.c_float),
+                ("ne_grid", ctypes.c_void_p), ("ne_n", ctypes.c_int32 * 3), ("ne_l", ctypes.c_float * 3),
+                ("n0_grid", ctypes.c_void_p), ("n0_n", ctypes.c_int32 * 3), ("n0_l", ctypes.c_float * 3)]
 
 
 _lib = None
@@ -88,8 +90,12 @@ def _check(rc: int):
 class Model:
     """Mirror of `synax_model`.  kind: 'disc4' | 'full16' | 'grid_b' | 'uniform'."""
 
-    def __init__(self, kind: str, aux: Optional[Sequence[float]] = None, grid_shape=None, box=None):
+    def __init__(self, kind: str, aux: Optional[Sequence[float]] = None, grid_shape=None, box=None,
+                 ne_grid=None, ne_box=None, n0_grid=None, n0_box=None):
+        """ne_grid / n0_grid: contiguous float32 CUDA tensors [nx][ny][nz] over boxes ne_box / n0_box (kpc), replacing the
+        analytic n_e / N_0 discs of a 'disc4' or 'grid_b' model (kept alive by this object)."""
         self.kind = kind
+        self._grids = (ne_grid, n0_grid)
         self._aux = None if aux is None else np.ascontiguousarray(np.asarray(aux, dtype=np.float32))
         c = _CModel()
         c.kind = KINDS[kind]
@@ -100,6 +106,15 @@ class Model:
         else:
             c.n_params = {"disc4": 4, "full16": 16, "uniform": 6}[kind]
         c.aux = None if self._aux is None else self._aux.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
+        for name, g, b in (("ne", ne_grid, ne_box), ("n0", n0_grid, n0_box)):
+            if g is None:
+                continue
+            if not (g.is_cuda and g.is_contiguous() and g.dim() == 3 and str(g.dtype) == "torch.float32"):
+                raise TypeError(f"{name}_grid must be a contiguous float32 CUDA tensor [nx][ny][nz]")
+            setattr(c, f"{name}_grid", g.data_ptr())
+            for a in range(3):
+                getattr(c, f"{name}_n")[a] = int(g.shape[a])
+                getattr(c, f"{name}_l")[a] = float(b[a])
         self.c = c
 
     @property

@@ -242,7 +242,26 @@ static synax_status check_model(const synax_plan* plan, const synax_model* m, co
     default: return fail(SYNAX_ERR_INVALID_ARG, "unknown model kind %d", m->kind);
   }
   if ((int64_t)batch * plan->npix >= (1LL << 31)) return fail(SYNAX_ERR_INVALID_ARG, "batch * npix must be < 2^31");
+  const float* sg[2] = {m->ne_grid, m->n0_grid};
+  const int32_t* sn[2] = {m->ne_n, m->n0_n};
+  const float* sl[2] = {m->ne_l, m->n0_l};
+  for (int k = 0; k < 2; ++k) {
+    if (!sg[k]) continue;
+    if (m->kind != SYNAX_MODEL_DISC4 && m->kind != SYNAX_MODEL_GRID_B)
+      return fail(SYNAX_ERR_INVALID_ARG, "gridded n_e / N_0 need a DISC4 or GRID_B model");
+    for (int a = 0; a < 3; ++a)
+      if (sn[k][a] < 2 || !(sl[k][a] > 0.0f)) return fail(SYNAX_ERR_INVALID_ARG, "scalar grid dims must be >= 2 and box lengths > 0");
+  }
   return SYNAX_OK;
+}
+
+static ScalarGridDesc make_scalar_desc(const float* g, const int32_t n[3], const float l[3]) {
+  ScalarGridDesc d;
+  d.g = g; d.nx = g ? n[0] : 2; d.ny = g ? n[1] : 2; d.nz = g ? n[2] : 2;
+  d.sx = g ? (double)(n[0] - 1) / (double)l[0] : 0.0; d.sy = g ? (double)(n[1] - 1) / (double)l[1] : 0.0;
+  d.sz = g ? (double)(n[2] - 1) / (double)l[2] : 0.0;
+  d.bx = 0.5 * (double)(d.nx - 1); d.by = 0.5 * (double)(d.ny - 1); d.bz = 0.5 * (double)(d.nz - 1);
+  return d;
 }
 
 static int pick_lanes(const synax_plan* plan, int64_t n_sl) {
@@ -340,6 +359,8 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   ForwardArgs a;
   a.geo = make_geo(plan); a.bc = bc; a.bd = bd; a.batch = batch; a.I = I; a.Q = Q; a.U = U;
   a.n_freq_total = plan->n_freq;
+  a.sg_ne = make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l);
+  a.sg_n0 = make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l);
   a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
 
   if (code == kGridB) {
@@ -440,10 +461,13 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   plan->launches++;
   synax_status rs;
   if (code == kGridB)
-    rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
+    rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
+                  make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
                   sm_count(plan->device), st, &plan->launches);
   else
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
+                      make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
+                      make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l),
                       dI, dQ, dU, grad, st, &plan->launches);
   cudaFreeAsync(bc, st);
   if (bd) cudaFreeAsync(bd, st);

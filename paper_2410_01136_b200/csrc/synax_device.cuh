@@ -136,6 +136,35 @@ struct Geometry {
                        // set by synax_plan_set_box (integration from the observer to the box face)
 };
 
+// Gridded scalar field (n_e or N_0): regular grid [nx][ny][nz] fp32, nodes on the faces of a box
+// centred on the Galactic centre, trilinear interpolation, zero outside.  g == nullptr: not used (analytic disc).
+struct ScalarGridDesc {
+  const float* g;
+  int nx, ny, nz;
+  double sx, sy, sz;    // (n-1)/l
+  double bx, by, bz;    // (n-1)/2
+};
+
+// coordinates, box test and cell in float64 (as for the B grid); weights and sum in fp32 or float64
+template <typename R>
+__device__ __forceinline__ R scalar_grid_at(const ScalarGridDesc& G, double x, double y, double z) {
+  const double ux = fma(x, G.sx, G.bx), uy = fma(y, G.sy, G.by), uz = fma(z, G.sz, G.bz);
+  const bool inbox = (ux >= 0.0) && (ux <= (double)(G.nx - 1)) && (uy >= 0.0) && (uy <= (double)(G.ny - 1)) &&
+                     (uz >= 0.0) && (uz <= (double)(G.nz - 1));
+  if (!inbox) return (R)0;
+  int i = __double2int_rd(ux), j = __double2int_rd(uy), k = __double2int_rd(uz);
+  i = min(i, G.nx - 2); j = min(j, G.ny - 2); k = min(k, G.nz - 2);
+  const R tx = (R)(ux - (double)i), ty = (R)(uy - (double)j), tz = (R)(uz - (double)k);
+  const R x0 = (R)1 - tx, y0 = (R)1 - ty, z0 = (R)1 - tz;
+  const float* p = G.g + ((size_t)i * G.ny + j) * G.nz + k;
+  const size_t dy = (size_t)G.nz, dx = (size_t)G.ny * G.nz;
+  const R c00 = z0 * (R)__ldg(p) + tz * (R)__ldg(p + 1);
+  const R c01 = z0 * (R)__ldg(p + dy) + tz * (R)__ldg(p + dy + 1);
+  const R c10 = z0 * (R)__ldg(p + dx) + tz * (R)__ldg(p + dx + 1);
+  const R c11 = z0 * (R)__ldg(p + dx + dy) + tz * (R)__ldg(p + dx + dy + 1);
+  return x0 * (y0 * c00 + ty * c01) + tx * (y0 * c10 + ty * c11);
+}
+
 // per-sightline direction triad
 struct Triad {
   double nxd, nyd, nzd;    // line of sight, float64 (positions, mask)

@@ -260,6 +260,7 @@ struct ForwardArgs {
   float flag_S;           // flag a sightline when max |sum n_e B_LOS| exceeds this (<=0: never)
   int* flag_count;        // device counter
   int* flag_list;         // device list of flagged sightline ids (b * npix + p)
+  ScalarGridDesc sg_ne, sg_n0;  // gridded n_e / N_0 replacing the analytic discs (DISC4, GRID_B), g == nullptr: unused
   const int* mode;        // device: kModeFastThenList / kModeAllF64 (written by decide_kernel), or null
   int run_when;           // forward_f64_kernel: 0 always, 1 only in list mode, 2 only in all-float64 mode
 };
@@ -321,6 +322,10 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
         eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+      }
+      if (CODE == kAnalyticDisc) {
+        if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+        if (A.sg_n0.g) S.N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       }
       S.ne *= T.scalef;
       float eI, a, bq;
@@ -460,7 +465,10 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
         } else {
           eval_analytic_dm<CODE == kAnalyticFull, kUnrollD>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
 #pragma unroll
-          for (int j = 0; j < kUnrollD; ++j) ne[j] *= T.scale;
+          for (int j = 0; j < kUnrollD; ++j) {
+            if (CODE == kAnalyticDisc && A.sg_ne.g) ne[j] = scalar_grid_at<double>(A.sg_ne, xd[j], yd[j], zd[j]);
+            ne[j] *= T.scale;
+          }
 #pragma unroll
           for (int j = 0; j < kUnrollD; ++j) {
             // N_0 (emission only): fp32 MUFU chain, Eq.(12)
@@ -469,6 +477,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
             const float ez = mufu_ex2(P.k_hz * fabsf((float)zd[j]));
             const float dz = 1.0f + ez;
             N0[j] = 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
+            if (CODE == kAnalyticDisc && A.sg_n0.g) N0[j] = scalar_grid_at<float>(A.sg_n0, xd[j], yd[j], zd[j]);
           }
         }
 #pragma unroll
@@ -554,6 +563,7 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
       SampleF Sm; AnalyticAux aux;
       eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
                                                       (rho2d > 9.0) && (rho2d < 400.0), Sm, aux);
+      if (CODE == kAnalyticDisc && A.sg_ne.g) Sm.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
       gn = fabsf(Sm.ne) * (fabsf(Sm.Bpar) + fabsf(Sm.BN) + fabsf(Sm.BE));
     }
     gabs += gn;

@@ -165,7 +165,7 @@ struct GridFwdArgs {
 // Round-off scale of a sightline's Faraday sum, k-independent part: sum_n |n_e| (|B_LOS| + |B_N| + |B_E|),
 // estimated from every 8th sample with the fp32 chain (whole warp; returns the same value in every lane).
 __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const BatchConsts& P, const Triad& T,
-                                                        const Geometry& geo, int lane) {
+                                                        const Geometry& geo, const ScalarGridDesc& sg_ne, int lane) {
   float acc = 0.f;
   for (int n = 4 + 8 * lane; n < geo.n_los; n += 256) {
     const double s_d = ((double)n + 0.5) * geo.delta * T.scale;
@@ -174,6 +174,7 @@ __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const
     float B[3], N0, ne;
     gather_B(G, c, B);
     densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+    if (sg_ne.g) ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
     const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
     const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
     const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
@@ -210,6 +211,8 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       gather_B(G, c, B);
       float N0, ne;
       densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      if (A.sg_ne.g) ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ne *= T.scalef;
       const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
       const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
@@ -224,6 +227,8 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       double Bpar, BN, BE, ne;
       float N0;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BN, BE, N0, ne);
+      if (A.sg_ne.g) ne = scalar_grid_at<double>(A.sg_ne, xd, yd, zd);
+      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ne *= T.scale;
       if (active) emission(P, (float)BN, (float)BE, N0, eI, a, bq);
       const double gn = active ? ne * Bpar : 0.0;
@@ -266,7 +271,7 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
     const Triad T = load_triad(A.geo, pix);
     float accI, accQ[NF], accU[NF];
     bool precise = GA.mode == 2;
-    if (GA.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, lane) > A.flag_S;
+    if (GA.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
     if (!precise) {
       const float scale = grid_forward_sweep<NF, false>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
       precise = GA.mode == 0 && scale > A.flag_S;
@@ -304,6 +309,7 @@ __global__ void grid_grad_compact_kernel(const float4* __restrict__ g4, int64_t 
 // ------------------------------------------------------------------------------------------------
 struct GridVjpArgs {
   Geometry geo;
+  ScalarGridDesc sg_ne, sg_n0;
   const BatchConsts* bc;
   const BatchConstsD* bd;
   GridDesc grid;
@@ -341,6 +347,8 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       float B[3];
       gather_B(G, c, B);
       densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      if (A.sg_ne.g) ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ne *= T.scalef;
       const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
       BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
@@ -353,6 +361,8 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
     } else {
       double Bpar, BNd, BEd, ned;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BNd, BEd, N0, ned);
+      if (A.sg_ne.g) ned = scalar_grid_at<double>(A.sg_ne, xd, yd, zd);
+      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ned *= T.scale;
       BN = (float)BNd; BE = (float)BEd; ne = (float)ned;
       const double gn = active ? ned * Bpar : 0.0;
@@ -420,7 +430,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     // when the rotation angle of this sightline is large (warp-uniform decision)
     float absS = 0.f;
     bool precise = A.mode == 2;
-    if (A.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, lane) > A.flag_S;
+    if (A.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
     if (!precise) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
     if (precise || (A.mode == 0 && absS > A.flag_S)) {
       __syncwarp();
@@ -454,6 +464,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
         c = locate(G, xd, yd, zd);
         float N0_unused;
         densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0_unused, ne_m);
+        if (A.sg_ne.g) ne_m = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
         ne_m *= T.scalef;
       }
       const int cell = (m >= m0 && c.inbox) ? c.base : -1;
@@ -538,11 +549,11 @@ static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const
 }
 
 static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const BatchConstsD* bd,
-                             const synax_model* m,
+                             const synax_model* m, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0,
                              const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
                              int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches) {
   GridVjpArgs a;
-  a.geo = geo; a.bc = bc; a.bd = bd; a.grid = make_grid_desc(m, grid);
+  a.geo = geo; a.bc = bc; a.bd = bd; a.grid = make_grid_desc(m, grid); a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_freq_total = ft.n_freq; a.dI = dI; a.dQ = dQ; a.dU = dU;
   const int64_t n_nodes = (int64_t)m->nx * m->ny * m->nz;
   if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;

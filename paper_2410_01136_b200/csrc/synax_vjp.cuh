@@ -134,6 +134,7 @@ struct VjpArgs {
   const BatchConsts* bc;
   int batch, f0, n_freq_total;
   const float* dI; const float* dQ; const float* dU;   // may be null
+  ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
   float* partial;   // [batch][n_blocks][16]
   int n_blocks;     // blocks per batch element (gridDim.x)
   int accumulate;   // 0: overwrite partials (first frequency block), 1: add
@@ -188,6 +189,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         AnalyticAux aux;
         eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
+        if (CODE == kAnalyticDisc && A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
       }
       const float gn = T.scalef * S.ne * S.Bpar;
       const float sum = hi + gn;
@@ -240,6 +242,10 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         const double rho2d = fma(xd, xd, yd * yd);
         eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
+        if (CODE == kAnalyticDisc) {
+          if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+          if (A.sg_n0.g) S.N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
+        }
       }
       S.ne *= T.scalef;   // n_e enters only through the Faraday integrand n_e B_LOS Delta_i
       // emission terms
@@ -376,11 +382,11 @@ static void launch_vjp(int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs&
 }
 
 static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, int batch,
-                                 int n_params, int G, const float* dI, const float* dQ, const float* dU, float* grad,
+                                 int n_params, int G, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0, const float* dI, const float* dQ, const float* dU, float* grad,
                                  cudaStream_t st, int64_t* launches) {
   VjpArgs a;
   a.geo = geo; a.bc = bc; a.batch = batch; a.n_freq_total = ft.n_freq;
-  a.dI = dI; a.dQ = dQ; a.dU = dU;
+  a.dI = dI; a.dQ = dQ; a.dU = dU; a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_blocks = (int)((geo.npix * G + kBlock - 1) / kBlock);
   if (batch > 65535) return SYNAX_ERR_UNSUPPORTED;
   float* partial = nullptr;

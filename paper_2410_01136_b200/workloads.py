@@ -56,6 +56,10 @@ class Workload:
     cot_seed: int = 0
     observer: tuple = OBSERVER
     clip_box: Optional[tuple] = None  # (lx, ly, lz) kpc: integrate observer -> box face instead of [0, s_max]
+    ne_grid: Optional[np.ndarray] = None   # float32 [nx][ny][nz]: gridded n_e replacing the analytic disc (disc4 / grid_b)
+    ne_box: Optional[tuple] = None
+    n0_grid: Optional[np.ndarray] = None   # the same for the CR density N_0
+    n0_box: Optional[tuple] = None
 
     @property
     def npix(self) -> int:
@@ -140,6 +144,16 @@ def gaussian_random_field(shape, box, seed, rms=3.0, slope=-11.0 / 3.0):
 def grid_nodes(shape, box):
     ax = [np.linspace(-l / 2.0, l / 2.0, n) for n, l in zip(shape, box)]
     return np.meshgrid(*ax, indexing="ij")
+
+
+def clumpy_disc_grid(shape, box, amp, h_r, h_z, seed, contrast=0.3):
+    """Data recipe for a gridded scalar field standing in for the paper's YMW16 n_e grid (not in the
+    container): an exponential disc amp * exp(-rho/h_r) / cosh^2(z/h_z) at the nodes, modulated by exp(contrast * g)
+    with g a unit-variance Gaussian random field (k^-11/3), rounded once to float32."""
+    X, Y, Z = grid_nodes(shape, box)
+    g = gaussian_random_field(shape, box, seed, rms=np.sqrt(3.0))[..., 0]
+    v = amp * np.exp(-np.hypot(X, Y) / h_r) / np.cosh(Z / h_z) ** 2 * np.exp(contrast * g)
+    return _f32(v)
 
 
 def config(i: int) -> Workload:

@@ -17,12 +17,26 @@ def oracle_model(w: wl.Workload) -> oracle.Model:
     return oracle.Model(w.kind, p, aux=aux, box=w.box)
 
 
+def _grids(w):
+    return oracle.scalar_grids(ne=w.ne_grid, ne_box=w.ne_box, n0=w.n0_grid, n0_box=w.n0_box)
+
+
 def oracle_forward(w: wl.Workload, pix=None):
+    with _grids(w):
+        return _oracle_forward(w, pix)
+
+
+def oracle_vjp(w: wl.Workload, cots, pix=None):
+    with _grids(w):
+        return _oracle_vjp(w, cots, pix)
+
+
+def _oracle_forward(w: wl.Workload, pix=None):
     return oracle.forward(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix=pix,
                           clip_box=w.clip_box)
 
 
-def oracle_vjp(w: wl.Workload, cots, pix=None):
+def _oracle_vjp(w: wl.Workload, cots, pix=None):
     return oracle.vjp(oracle_model(w), w.nside, w.n_los, w.s_max, w.freqs, *cots, observer=w.observer, pix=pix,
                       clip_box=w.clip_box)
 
@@ -35,10 +49,15 @@ def gpu_objects(w: wl.Workload, pix_range=None, **options):
         plan.set_box(w.clip_box)
     for k, v in options.items():
         plan.set_option(k, v)
+    sg = {}
+    if w.ne_grid is not None:
+        sg.update(ne_grid=torch.from_numpy(w.ne_grid).cuda().contiguous(), ne_box=w.ne_box)
+    if w.n0_grid is not None:
+        sg.update(n0_grid=torch.from_numpy(w.n0_grid).cuda().contiguous(), n0_box=w.n0_box)
     if w.kind == "grid_b":
-        model = sx.Model("grid_b", aux=w.aux, grid_shape=w.params.shape[:3], box=w.box)
+        model = sx.Model("grid_b", aux=w.aux, grid_shape=w.params.shape[:3], box=w.box, **sg)
     else:
-        model = sx.Model(w.kind, aux=w.aux)
+        model = sx.Model(w.kind, aux=w.aux, **sg)
     params = torch.from_numpy(w.params).cuda().contiguous()
     return plan, model, params
 
