@@ -131,6 +131,17 @@ def rank_workload(cfg, rank):
     return w
 
 
+def apply_overrides(w, args):
+    """--nside / --n-los / --freq-hz: the config's model at another map size, sample count or at one frequency
+    (the Fig. 7-style runtime sweep of PAPER.md L260, L277); the workload name says so."""
+    if args.nside or args.n_los:
+        w = w.scaled(nside=args.nside or None, n_los=args.n_los or None)
+    if args.freq_hz:
+        w.freqs = np.array([float(args.freq_hz)])
+        w.name += f"@{args.freq_hz:g}Hz"
+    return w
+
+
 # ------------------------------------------------------------------------------------------------
 # the oracle leg (cpu_baseline of the default run, and --impl reference)
 # ------------------------------------------------------------------------------------------------
@@ -185,7 +196,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     from paper_2410_01136_b200 import workloads as wl
-    w = wl.config(args.config)
+    w = apply_overrides(wl.config(args.config), args)
     steps, warmup = max(1, args.steps), max(0, args.warmup)
     # keep the whole run within a few minutes: total oracle time ~ 120 s split over steps + warm-ups
     budget = min(15.0, 120.0 / (steps + warmup))
@@ -292,10 +303,10 @@ def run_ours(args):
     pix_range = None
     if strong:      # one map, pixel shards, one gradient all-reduce per step
         from paper_2410_01136_b200 import sharding, workloads as wl
-        w = wl.config(args.config)
+        w = apply_overrides(wl.config(args.config), args)
         pix_range = sharding.shard_of(w.npix, rank, world)
     else:           # independent chains: every rank integrates the whole sky for its own parameter vector
-        w = rank_workload(args.config, rank)
+        w = apply_overrides(rank_workload(args.config, rank), args)
     kw = dict(pix_range=pix_range, reduce_grad=strong)
     flush_buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
 
@@ -363,7 +374,8 @@ def run_ours(args):
             line["roofline"]["frac_at_sustained_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
         if world == 1 and not args.no_cpu_baseline:
             from paper_2410_01136_b200 import workloads as wl
-            line["cpu_baseline"] = {k: v for k, v in oracle_baseline(wl.config(args.config), seconds_budget=args.cpu_seconds).items()
+            line["cpu_baseline"] = {k: v for k, v in oracle_baseline(apply_overrides(wl.config(args.config), args),
+                                                                     seconds_budget=args.cpu_seconds).items()
                                     if k in ("value", "unit", "cores", "kind", "sample", "forward_samples_per_s")}
     if world > 1:
         dist.barrier()
@@ -383,6 +395,9 @@ def main():
     ap.add_argument("--scaling", choices=("weak", "strong"), default="weak",
                     help="N > 1: weak = one parameter vector (chain) per rank, no collective; strong = pixel shards of one map "
                          "+ one gradient all-reduce per step")
+    ap.add_argument("--nside", type=int, default=0, help="override the config's nside (runtime sweeps)")
+    ap.add_argument("--n-los", type=int, default=0, help="override the config's samples per sightline")
+    ap.add_argument("--freq-hz", type=float, default=0.0, help="run at this single frequency instead of the config's")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline oracle sample")
     args = ap.parse_args()
