@@ -57,13 +57,18 @@ typedef enum {
    * S:C-2#12).  params IS the grid; CR/alpha/n_e from `aux`.  batch must be 1. */
   SYNAX_MODEL_GRID_B = 2,
   /* homogeneous fields everywhere (toy of P:L123): params (Bx,By,Bz [uG], N0, n_e, alpha). */
-  SYNAX_MODEL_UNIFORM = 3
+  SYNAX_MODEL_UNIFORM = 3,
+  /* the paper's own 16-parameter model, Eq.(16) P:L283-289 with Table 3: params (b0 [uG], psi0, psi1,
+   * chi0 [rad]) x 4 WMAP spirals B_1..B_4, stacked as
+   *   B_x = .6 B1x + .3 B2x + .1 B3z + .3 B4y;  B_y = .6 B1y + .3 B2z + .1 B3y + .3 B4x;  B_z = .6 B1z + .3 B2y + .1 B3x + .3 B4z
+   * CR density, alpha and n_e from `aux` (or the optional grids) as for DISC4. */
+  SYNAX_MODEL_STACK16 = 4
 } synax_model_kind;
 
 typedef struct {
   int32_t kind;     /* synax_model_kind */
-  int32_t n_params; /* 4, 16, nx*ny*nz*3 (<2^31), 6 -- must match kind */
-  const float* aux; /* HOST. DISC4 / GRID_B: {C0, h_r, h_z, alpha, ne0, h_er, h_ez}; else NULL */
+  int32_t n_params; /* 4, 16, nx*ny*nz*3 (<2^31), 6, 16 -- must match kind */
+  const float* aux; /* HOST. DISC4 / GRID_B / STACK16: {C0, h_r, h_z, alpha, ne0, h_er, h_ez}; else NULL */
   int32_t nx, ny, nz; /* GRID_B only, each >= 2 */
   float lx, ly, lz;   /* GRID_B only, kpc, > 0 */
   /* Optional gridded scalar fields (the paper's n_e is the YMW16 model on a (256,256,64) grid):

@@ -20,8 +20,8 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "synax_oracle.cpp"
 _LIB = _HERE / "liboracle.so"
 
-KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
-N_PARAMS = {"disc4": 4, "full16": 16, "uniform": 6}
+KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3, "stack16": 4}
+N_PARAMS = {"disc4": 4, "full16": 16, "uniform": 6, "stack16": 16}
 
 
 def build(force: bool = False) -> Path:
@@ -80,7 +80,7 @@ class Model:
             self.batch, self.n_params = self.params.shape
             assert self.n_params == N_PARAMS[kind]
         self.aux = None if aux is None else _f64(aux)
-        if kind in ("disc4", "grid_b"):
+        if kind in ("disc4", "grid_b", "stack16"):
             assert self.aux is not None and self.aux.size == 7
 
 

@@ -57,7 +57,7 @@ const double KPC_CM = 1.0e3 * PC_CM;
 const double PI = 3.14159265358979323846264338327950288;
 
 // model kinds (the oracle's own numbering; the python wrapper maps names to these)
-enum { KIND_DISC4 = 0, KIND_FULL16 = 1, KIND_GRID_B = 2, KIND_UNIFORM = 3 };
+enum { KIND_DISC4 = 0, KIND_FULL16 = 1, KIND_GRID_B = 2, KIND_UNIFORM = 3, KIND_STACK16 = 4 };
 
 struct Model {
   int kind;
@@ -73,6 +73,7 @@ int n_params_of(const Model& m) {
     case KIND_DISC4: return 4;
     case KIND_FULL16: return 16;
     case KIND_UNIFORM: return 6;
+    case KIND_STACK16: return 16;
     case KIND_GRID_B: return (int)(m.nx * m.ny * m.nz * 3);
   }
   return -1;
@@ -192,6 +193,17 @@ double scalar_grid_value(const ScalarGrid& S, double x, double y, double z) {
   return v;
 }
 
+// The paper's 16-parameter model, Eq.(16): four WMAP spirals B_k (parameters (b0, psi0, psi1, chi0)_k,
+// k = 1..4, Table 3) stacked with the printed weights and component permutations:
+//   B_x = 0.6 B1x + 0.3 B2x + 0.1 B3z + 0.3 B4y
+//   B_y = 0.6 B1y + 0.3 B2z + 0.1 B3y + 0.3 B4x
+//   B_z = 0.6 B1z + 0.3 B2y + 0.1 B3x + 0.3 B4z
+// kStackSrc[k][c] = which component of B_k feeds component c of the total.  (The text also says B_2..4 "are
+// rotated before stacking" without giving the rotation; the permutations printed in Eq.(16) are taken as
+// that rotation -- DESIGN.md section 3.)
+const double kStackW[4] = {0.6, 0.3, 0.1, 0.3};
+const int kStackSrc[4][3] = {{0, 1, 2}, {0, 2, 1}, {2, 1, 0}, {1, 0, 2}};
+
 // step 3: all fields at one point.
 void eval_fields(const Model& m, const double r[3], Fields& F) {
   const double x = r[0], y = r[1], z = r[2];
@@ -221,6 +233,18 @@ void eval_fields(const Model& m, const double r[3], Fields& F) {
       F.alpha = a[3];
       F.ne = exp_disc(a[4], a[5], a[6], rho, z);
     } break;
+    case KIND_STACK16: {
+      F.B[0] = F.B[1] = F.B[2] = 0.0;
+      for (int k = 0; k < 4; ++k) {
+        double Bk[3];
+        disc_field(p[4 * k], p[4 * k + 1], p[4 * k + 2], p[4 * k + 3], 0.0, x, y, z, Bk);
+        for (int c = 0; c < 3; ++c) F.B[c] += kStackW[k] * Bk[kStackSrc[k][c]];
+      }
+      const double* a = m.aux;
+      F.N0 = exp_disc(a[0], a[1], a[2], rho, z);
+      F.alpha = a[3];
+      F.ne = exp_disc(a[4], a[5], a[6], rho, z);
+    } break;
     case KIND_UNIFORM: {
       // homogeneous toy fields; aux[0] = R0 > 0 confines them to a sphere of radius
       // R0 around the observer ("zero outside").
@@ -235,7 +259,7 @@ void eval_fields(const Model& m, const double r[3], Fields& F) {
       F.alpha = p[5];
     } break;
   }
-  if (m.kind == KIND_DISC4 || m.kind == KIND_GRID_B) {
+  if (m.kind == KIND_DISC4 || m.kind == KIND_GRID_B || m.kind == KIND_STACK16) {
     if (g_ne_grid.g) F.ne = scalar_grid_value(g_ne_grid, x, y, z);
     if (g_n0_grid.g) F.N0 = scalar_grid_value(g_n0_grid, x, y, z);
   }
@@ -303,6 +327,14 @@ void fields_vjp(const Model& m, const double r[3], const double Bb[3], double N0
       disc_field_vjp(p[0], p[1], p[2], p[3], 0.0, false, x, y, z, Bb, &grad[0], &grad[1], &grad[2],
                      &grad[3], &dummy);
       // CR / n_e / alpha come from aux and are not differentiated (S:App.C)
+    } break;
+    case KIND_STACK16: {
+      for (int k = 0; k < 4; ++k) {   // transpose of the stacking: cotangent of B_k's component kStackSrc[k][c] += w_k Bb[c]
+        double Bbk[3] = {0.0, 0.0, 0.0}, dummy = 0.0;
+        for (int c = 0; c < 3; ++c) Bbk[kStackSrc[k][c]] += kStackW[k] * Bb[c];
+        disc_field_vjp(p[4 * k], p[4 * k + 1], p[4 * k + 2], p[4 * k + 3], 0.0, false, x, y, z, Bbk, &grad[4 * k],
+                       &grad[4 * k + 1], &grad[4 * k + 2], &grad[4 * k + 3], &dummy);
+      }
     } break;
     case KIND_FULL16: {
       disc_field_vjp(p[0], p[1], p[2], p[3], p[4], true, x, y, z, Bb, &grad[0], &grad[1], &grad[2],

@@ -15,7 +15,7 @@ _LIB_PATH = _PKG / "libsynax.so"
 
 STATUS = {0: "SYNAX_OK", 1: "SYNAX_ERR_INVALID_ARG", 2: "SYNAX_ERR_UNSUPPORTED", 3: "SYNAX_ERR_CUDA",
           4: "SYNAX_ERR_ALLOC"}
-KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3}
+KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3, "stack16": 4}
 
 # every symbol include/synax.h declares
 exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_box", "synax_plan_set_option",
@@ -104,7 +104,7 @@ class Model:
             c.lx, c.ly, c.lz = (float(v) for v in box)
             c.n_params = c.nx * c.ny * c.nz * 3
         else:
-            c.n_params = {"disc4": 4, "full16": 16, "uniform": 6}[kind]
+            c.n_params = {"disc4": 4, "full16": 16, "uniform": 6, "stack16": 16}[kind]
         c.aux = None if self._aux is None else self._aux.ctypes.data_as(ctypes.POINTER(ctypes.c_float))
         for name, g, b in (("ne", ne_grid, ne_box), ("n0", n0_grid, n0_box)):
             if g is None:

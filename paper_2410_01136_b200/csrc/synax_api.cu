@@ -227,6 +227,10 @@ static synax_status check_model(const synax_plan* plan, const synax_model* m, co
     case SYNAX_MODEL_FULL16:
       if (m->n_params != 16) return fail(SYNAX_ERR_INVALID_ARG, "FULL16 needs n_params == 16");
       *code = kAnalyticFull; break;
+    case SYNAX_MODEL_STACK16:
+      if (m->n_params != 16) return fail(SYNAX_ERR_INVALID_ARG, "STACK16 needs n_params == 16");
+      if (!m->aux) return fail(SYNAX_ERR_INVALID_ARG, "STACK16 needs aux");
+      *code = kStack16; break;
     case SYNAX_MODEL_UNIFORM:
       if (m->n_params != 6) return fail(SYNAX_ERR_INVALID_ARG, "UNIFORM needs n_params == 6");
       *code = kUniform; break;
@@ -247,8 +251,8 @@ static synax_status check_model(const synax_plan* plan, const synax_model* m, co
   const float* sl[2] = {m->ne_l, m->n0_l};
   for (int k = 0; k < 2; ++k) {
     if (!sg[k]) continue;
-    if (m->kind != SYNAX_MODEL_DISC4 && m->kind != SYNAX_MODEL_GRID_B)
-      return fail(SYNAX_ERR_INVALID_ARG, "gridded n_e / N_0 need a DISC4 or GRID_B model");
+    if (m->kind != SYNAX_MODEL_DISC4 && m->kind != SYNAX_MODEL_GRID_B && m->kind != SYNAX_MODEL_STACK16)
+      return fail(SYNAX_ERR_INVALID_ARG, "gridded n_e / N_0 need a DISC4, STACK16 or GRID_B model");
     for (int a = 0; a < 3; ++a)
       if (sn[k][a] < 2 || !(sl[k][a] > 0.0f)) return fail(SYNAX_ERR_INVALID_ARG, "scalar grid dims must be >= 2 and box lengths > 0");
   }
@@ -392,6 +396,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       const int64_t n_pilot = (n_sl + stride - 1) / stride;
       const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
       if (code == kAnalyticDisc) pilot_kernel<kAnalyticDisc><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
+      else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot);
@@ -412,6 +417,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       const int nf = next_freq_block(plan->n_freq - f0);
       pa.f0 = f0;
       if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
+      else if (code == kStack16) launch_f64<kStack16>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
       else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
       else launch_f64<kUniform>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
       plan->launches++;
@@ -423,6 +429,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       const int nf = next_freq_block(plan->n_freq - f0);
       a.f0 = f0;
       if (code == kAnalyticDisc) launch_forward<kAnalyticDisc>(G, nf, n_sl, st, a, plan->ft);
+      else if (code == kStack16) launch_forward<kStack16>(G, nf, n_sl, st, a, plan->ft);
       else if (code == kAnalyticFull) launch_forward<kAnalyticFull>(G, nf, n_sl, st, a, plan->ft);
       else launch_forward<kUniform>(G, nf, n_sl, st, a, plan->ft);
       plan->launches++;

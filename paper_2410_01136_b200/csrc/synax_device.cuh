@@ -89,6 +89,7 @@ __device__ __forceinline__ void rsqrt_sqrt_nr(float x, float& ir, float& r) {
 struct BatchConsts {
   // raw parameters, canonical FULL16 order (S:App.C), as float and double
   float p[kMaxAnalyticParams];
+  float sp[16];      // STACK16 only: (b0, psi0, psi1, chi0) of the four stacked spirals (p[] then holds the aux densities)
   // derived fp32
   float k_hb;        // -log2(e)/h_b      (0 for DISC4)
   float k_hb_lo, k_her_lo;  // float64 value minus its fp32 rounding (the constants multiply rho ~ 10 kpc)
@@ -294,6 +295,59 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
     S.ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * a.rho) * ee * ie;
     a.thez = copysignf((1.0f - ee) * de * ie, z);
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// The paper's own 16-parameter model, Eq.(16) P:L283-289 (Table 3): four WMAP spirals B_k stacked with
+// the printed weights and component permutations,
+//   B_x = .6 B1x + .3 B2x + .1 B3z + .3 B4y,  B_y = .6 B1y + .3 B2z + .1 B3y + .3 B4x,  B_z = .6 B1z + .3 B2y + .1 B3x + .3 B4z
+// (DESIGN.md section 3 on the "rotation before stacking").  CR / n_e / alpha from aux as for DISC4.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float stack_w(int k) { return k == 0 ? 0.6f : (k == 2 ? 0.1f : 0.3f); }
+// component of B_k that feeds component c of the total
+__device__ __forceinline__ constexpr int stack_src(int k, int c) {
+  return k == 0 ? c : (k == 1 ? (c == 0 ? 0 : (c == 1 ? 2 : 1)) : (k == 2 ? (c == 0 ? 2 : (c == 1 ? 1 : 0)) : (c == 0 ? 1 : (c == 1 ? 0 : 2))));
+}
+
+struct StackAux {
+  float ir, rho, xr, yr, lr, t;
+  float sp[4], cp[4], sc[4], cc[4];
+  float mask;              // 1 inside the annulus 3 < rho < 20 kpc, else 0
+};
+
+template <bool kFastTrig>
+__device__ __forceinline__ void eval_stack16_f32(const BatchConsts& P, const Triad& T, float x, float y, float z,
+                                                 float rho2, bool inside, SampleF& S, StackAux& a) {
+  const float kLog2e = 1.4426950408889634f;
+  rho2 = fmaxf(rho2, 1.0e-30f);
+  a.ir = mufu_rsqrt(rho2);
+  a.rho = rho2 * a.ir;
+  a.xr = x * a.ir; a.yr = y * a.ir;
+  const float az = fabsf(z);
+  a.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;
+  const float e1 = mufu_ex2(-2.0f * kLog2e * az);
+  a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
+  a.mask = inside ? 1.0f : 0.0f;
+  float B[3] = {0.0f, 0.0f, 0.0f};
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const float psi = fmaf(P.sp[4 * k + 2], a.lr, P.sp[4 * k + 1]);
+    const float chi = P.sp[4 * k + 3] * a.t;
+    if (kFastTrig) { a.sp[k] = mufu_sin(psi); a.cp[k] = mufu_cos(psi); a.sc[k] = mufu_sin(chi); a.cc[k] = mufu_cos(chi); }
+    else { sincos_fma(psi, a.sp[k], a.cp[k]); sincos_fma(chi, a.sc[k], a.cc[k]); }
+    const float A = a.mask * stack_w(k) * P.sp[4 * k];
+    const float Brho = A * a.cp[k] * a.cc[k], Bphi = A * a.sp[k] * a.cc[k];
+    const float comp[3] = {Brho * a.xr - Bphi * a.yr, fmaf(Brho, a.yr, Bphi * a.xr), A * a.sc[k]};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) B[c] += comp[stack_src(k, c)];
+  }
+  S.Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
+  S.BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
+  S.BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
+  const float ez = mufu_ex2(P.k_hz * az), dz = 1.0f + ez;
+  S.N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * a.rho) * ez * mufu_rcp(dz * dz);
+  const float ee = mufu_ex2(P.k_hez * az), de = 1.0f + ee;
+  S.ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * a.rho) * ee * mufu_rcp(de * de);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -133,6 +133,7 @@ struct BatchConstsD {
   int angles_small;       // |psi0| + |psi1| <= pi/4 and |chi0| <= pi/4: psi (|ln(rho/8)| < 1 inside the annulus) and
                           // chi = chi0 tanh z never leave [-pi/4, pi/4], so sincos needs no range reduction
   int hez_is_one;         // h_ez == 1 kpc exactly: exp(-2|z|/h_ez) is the tanh(z / 1 kpc) exponential, evaluated once
+  double sb0[4], spsi0[4], spsi1[4], schi0[4];   // STACK16 only: the four stacked spirals (b0 already times its weight)
 };
 
 // M independent sincos in lockstep (same polynomials as sincos_d)
@@ -293,6 +294,46 @@ __device__ __forceinline__ void eval_analytic_dm(const BatchConstsD& D, const do
     By[j] = fma(Brho[j], yr, Bphi[j] * xr);
     ne[j] = D.ne0x4 * er[j] * ee[j] * ide2;
   }
+}
+
+// STACK16 (Eq.(16)), float64: shared geometry, n_e's exponentials and tanh, then eight sincos in lockstep.
+__device__ __forceinline__ void eval_stack16_d(const BatchConstsD& D, double x, double y, double z, double rho2,
+                                               bool inside, double& Bx, double& By, double& Bz, double& ne) {
+  const double kLog2e = 1.4426950408889634074;
+  const double ir = rsqrt_d(rho2);
+  const double rho = rho2 * ir;
+  const double xr = x * ir, yr = y * ir;
+  const double az = fabs(z);
+  double B[3] = {0.0, 0.0, 0.0};
+  double ee, er;
+  if (inside) {
+    const double xs[3] = {D.k_hez * az, D.k_her * rho, -2.0 * kLog2e * az};
+    double o[3];
+    exp2_d_n<3>(xs, o);
+    ee = o[0]; er = o[1];
+    const double th = copysign((1.0 - o[2]) * rcp_d(1.0 + o[2]), z);
+    const double lr = 0.5 * log_d(rho2 * 0.015625);      // Table 3's psi1 are O(1): the MUFU lg2 is not enough
+    double ang[8], sn[8], cs[8];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { ang[k] = fma(D.spsi1[k], lr, D.spsi0[k]); ang[4 + k] = D.schi0[k] * th; }
+    sincos_d_n<8>(ang, sn, cs);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const double A = D.sb0[k];
+      const double Brho = A * cs[k] * cs[4 + k], Bphi = A * sn[k] * cs[4 + k];
+      const double comp[3] = {Brho * xr - Bphi * yr, fma(Brho, yr, Bphi * xr), A * sn[4 + k]};
+#pragma unroll
+      for (int c = 0; c < 3; ++c) B[c] += comp[stack_src(k, c)];
+    }
+  } else {
+    const double xs[2] = {D.k_hez * az, D.k_her * rho};
+    double o[2];
+    exp2_d_n<2>(xs, o);
+    ee = o[0]; er = o[1];
+  }
+  Bx = B[0]; By = B[1]; Bz = B[2];
+  const double de = 1.0 + ee;
+  ne = D.ne0x4 * er * ee * rcp_d(de * de);
 }
 
 }  // namespace synax

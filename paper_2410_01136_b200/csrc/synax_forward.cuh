@@ -17,7 +17,7 @@ constexpr int kTileDMax = 16;  // float64-chain kernel: at most this many sample
 constexpr int kUnrollD = SYNAX_UNROLL_D;  // ... samples advanced in lockstep per iteration
 constexpr float kTilePhase = 96.0f;  // ... and at most about this much Faraday angle (rad) inside a tile
 
-enum ModelCode { kAnalyticDisc = 0, kAnalyticFull = 1, kGridB = 2, kUniform = 3 };
+enum ModelCode { kAnalyticDisc = 0, kAnalyticFull = 1, kGridB = 2, kUniform = 3, kStack16 = 4 };
 
 // ------------------------------------------------------------------------------------------------
 // A1: HEALPix RING pixel -> (cos l, sin l, cos b, sin b) in float64 (Gorski et al. 2005).
@@ -97,6 +97,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= batch) return;
   BatchConsts c;
+  for (int j = 0; j < 16; ++j) c.sp[j] = 0.0f;
   double p[16];
   for (int j = 0; j < 16; ++j) p[j] = 0.0;
   double alpha;
@@ -107,7 +108,9 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     c.uB[0] = q[0]; c.uB[1] = q[1]; c.uB[2] = q[2]; c.uN0 = q[3]; c.une = q[4];
     p[12] = (double)q[5];
     p[4] = p[7] = p[8] = p[10] = p[11] = p[14] = p[15] = 1.0;
-  } else {  // DISC4 or GRID_B: densities and alpha from aux
+  } else {  // DISC4, STACK16 or GRID_B: densities and alpha from aux
+    if (code == kStack16)
+      for (int j = 0; j < 16; ++j) c.sp[j] = params[(size_t)b * n_params + j];
     if (code == kAnalyticDisc)
       for (int j = 0; j < 4; ++j) p[j] = (double)params[(size_t)b * n_params + j];
     p[4] = 1.0;  // unused: k_hb = 0
@@ -159,6 +162,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
       gmax = fabs((double)c.une) * (fabs((double)c.uB[0]) + fabs((double)c.uB[1]) + fabs((double)c.uB[2]));
     } else {
       double bmax = fabs(p[0]);
+      if (code == kStack16) bmax = 0.6 * fabs((double)c.sp[0]) + 0.3 * fabs((double)c.sp[4]) + 0.1 * fabs((double)c.sp[8]) + 0.3 * fabs((double)c.sp[12]);
       if (code == kAnalyticFull) bmax = bmax * fmax(exp(5.0 / p[4]), exp(-12.0 / p[4])) + fabs(p[5]);
       gmax = fabs(p[13]) * bmax;
     }
@@ -180,6 +184,12 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     d.psi1_small = fabs(p[2]) <= 0.05 ? 1 : 0;
     d.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4
     d.hez_is_one = (p[15] == 1.0 || p[15] == -1.0) ? 1 : 0;
+    for (int k = 0; k < 4; ++k) {
+      const bool st = code == kStack16;
+      const double w = k == 0 ? 0.6 : (k == 2 ? 0.1 : 0.3);
+      d.sb0[k] = st ? w * (double)c.sp[4 * k] : 0.0; d.spsi0[k] = st ? (double)c.sp[4 * k + 1] : 0.0;
+      d.spsi1[k] = st ? (double)c.sp[4 * k + 2] : 0.0; d.schi0[k] = st ? (double)c.sp[4 * k + 3] : 0.0;
+    }
     outd[b] = d;
   }
 }
@@ -317,13 +327,17 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         S.BN = fmaf(P.uB[0], T.eNx, fmaf(P.uB[1], T.eNy, P.uB[2] * T.eNz));
         S.BE = fmaf(P.uB[0], T.eEx, P.uB[1] * T.eEy);
         S.N0 = P.uN0; S.ne = P.une;
+      } else if (CODE == kStack16) {
+        const double rho2d = fma(xd, xd, yd * yd);
+        StackAux sa;
+        eval_stack16_f32<false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
         eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
-      if (CODE == kAnalyticDisc) {
+      if (CODE == kAnalyticDisc || CODE == kStack16) {
         if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
         if (A.sg_n0.g) S.N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       }
@@ -463,10 +477,15 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
             Bx[j] = (double)P.uB[0]; By[j] = (double)P.uB[1]; Bz[j] = (double)P.uB[2]; ne[j] = (double)P.une * T.scale; N0[j] = P.uN0;
           }
         } else {
-          eval_analytic_dm<CODE == kAnalyticFull, kUnrollD>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
+          if (CODE == kStack16) {
+#pragma unroll
+            for (int j = 0; j < kUnrollD; ++j) eval_stack16_d(D, xd[j], yd[j], zd[j], rho2d[j], inside[j], Bx[j], By[j], Bz[j], ne[j]);
+          } else {
+            eval_analytic_dm<CODE == kAnalyticFull, kUnrollD>(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
+          }
 #pragma unroll
           for (int j = 0; j < kUnrollD; ++j) {
-            if (CODE == kAnalyticDisc && A.sg_ne.g) ne[j] = scalar_grid_at<double>(A.sg_ne, xd[j], yd[j], zd[j]);
+            if ((CODE == kAnalyticDisc || CODE == kStack16) && A.sg_ne.g) ne[j] = scalar_grid_at<double>(A.sg_ne, xd[j], yd[j], zd[j]);
             ne[j] *= T.scale;
           }
 #pragma unroll
@@ -477,7 +496,7 @@ __global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_consta
             const float ez = mufu_ex2(P.k_hz * fabsf((float)zd[j]));
             const float dz = 1.0f + ez;
             N0[j] = 4.0f * P.p[9] * mufu_ex2(P.k_hr * rho) * ez * mufu_rcp(dz * dz);
-            if (CODE == kAnalyticDisc && A.sg_n0.g) N0[j] = scalar_grid_at<float>(A.sg_n0, xd[j], yd[j], zd[j]);
+            if ((CODE == kAnalyticDisc || CODE == kStack16) && A.sg_n0.g) N0[j] = scalar_grid_at<float>(A.sg_n0, xd[j], yd[j], zd[j]);
           }
         }
 #pragma unroll
@@ -560,10 +579,16 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
       const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       const double rho2d = fma(xd, xd, yd * yd);
-      SampleF Sm; AnalyticAux aux;
-      eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
-                                                      (rho2d > 9.0) && (rho2d < 400.0), Sm, aux);
-      if (CODE == kAnalyticDisc && A.sg_ne.g) Sm.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+      SampleF Sm;
+      if (CODE == kStack16) {
+        StackAux sa;
+        eval_stack16_f32<true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, (rho2d > 9.0) && (rho2d < 400.0), Sm, sa);
+      } else {
+        AnalyticAux aux;
+        eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
+                                                        (rho2d > 9.0) && (rho2d < 400.0), Sm, aux);
+      }
+      if ((CODE == kAnalyticDisc || CODE == kStack16) && A.sg_ne.g) Sm.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
       gn = fabsf(Sm.ne) * (fabsf(Sm.Bpar) + fabsf(Sm.BN) + fabsf(Sm.BE));
     }
     gabs += gn;

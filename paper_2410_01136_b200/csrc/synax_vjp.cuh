@@ -129,6 +129,53 @@ struct UniformGrad {
   }
 };
 
+// STACK16 (Eq.(16)): (b0, psi0, psi1, chi0) of the four stacked spirals.  The cotangent of B_k is the
+// un-permuted total cotangent (the weight w_k is folded into the amplitude A, as in eval_stack16_f32).
+struct StackGrad {
+  float b1[16], b2[16];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int j = 0; j < 16; ++j) { b1[j] = 0.f; b2[j] = 0.f; }
+  }
+  __device__ __forceinline__ void add(const BatchConsts& P, const Triad& T, const StackAux& a, const SampleF& S,
+                                      float BNb, float BEb, float wgt) {
+    const float wn = wgt * S.ne;
+    const float v1[3] = {fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, -wn * T.nx)), fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, -wn * T.ny)),
+                         fmaf(BNb, T.eNz, -wn * T.nz)};
+    const float v2[3] = {S.ne * T.nx, S.ne * T.ny, S.ne * T.nz};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float u1[3], u2[3];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { u1[stack_src(k, c)] = v1[c]; u2[stack_src(k, c)] = v2[c]; }
+      float u1r, u1p, u2r, u2p;
+      to_cyl(u1[0], u1[1], a.xr, a.yr, u1r, u1p);
+      to_cyl(u2[0], u2[1], a.xr, a.yr, u2r, u2p);
+      const float A = a.mask * stack_w(k) * P.sp[4 * k];
+      const float Acc = A * a.cc[k], Asc = A * a.sc[k];
+      const float h1 = fmaf(a.cp[k], u1r, a.sp[k] * u1p), h2 = fmaf(a.cp[k], u2r, a.sp[k] * u2p);
+      b1[4 * k] += fmaf(Acc, h1, Asc * u1[2]);                       // B_k . V  (* 1/b0 at the end)
+      b2[4 * k] += fmaf(Acc, h2, Asc * u2[2]);
+      const float p1 = Acc * fmaf(a.cp[k], u1p, -a.sp[k] * u1r), p2 = Acc * fmaf(a.cp[k], u2p, -a.sp[k] * u2r);
+      b1[4 * k + 1] += p1; b2[4 * k + 1] += p2;
+      b1[4 * k + 2] = fmaf(a.lr, p1, b1[4 * k + 2]); b2[4 * k + 2] = fmaf(a.lr, p2, b2[4 * k + 2]);
+      const float tA = a.t * A;
+      b1[4 * k + 3] = fmaf(tA, fmaf(a.cc[k], u1[2], -a.sc[k] * h1), b1[4 * k + 3]);
+      b2[4 * k + 3] = fmaf(tA, fmaf(a.cc[k], u2[2], -a.sc[k] * h2), b2[4 * k + 3]);
+    }
+  }
+  __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
+#pragma unroll
+    for (int j = 0; j < 16; ++j) out[j] = fmaf(Tw, b2[j], b1[j]);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) out[4 * k] /= P.sp[4 * k];
+  }
+};
+
+template <int CODE> struct GradOf { using type = AnalyticGrad<CODE == kAnalyticFull>; };
+template <> struct GradOf<kUniform> { using type = UniformGrad; };
+template <> struct GradOf<kStack16> { using type = StackGrad; };
+
 struct VjpArgs {
   Geometry geo;
   const BatchConsts* bc;
@@ -184,6 +231,11 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       SampleF S;
       if (CODE == kUniform) {
         S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz)); S.ne = P.une;
+      } else if (CODE == kStack16) {
+        const double rho2d = fma(xd, xd, yd * yd);
+        StackAux sa;
+        eval_stack16_f32<true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
+        if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
         AnalyticAux aux;
@@ -202,7 +254,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   }
 
   // ---- main sweep
-  typename std::conditional<CODE == kUniform, UniformGrad, AnalyticGrad<CODE == kAnalyticFull>>::type acc;
+  typename GradOf<CODE>::type acc;
   acc.zero();
   float gAlpha = 0.f;          // sum_n 1/4 ln(B_perp^2) M K
   float sumE = 0.f;            // sum_n e~_n
@@ -232,8 +284,14 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       s_d += delta;
       SampleF S;
       AnalyticAux aux;
+      StackAux sa;
       const float zf = (float)zd;
-      if (CODE == kUniform) {
+      if (CODE == kStack16) {
+        const double rho2d = fma(xd, xd, yd * yd);
+        eval_stack16_f32<true>(P, T, (float)xd, (float)yd, zf, (float)rho2d, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
+        if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+        if (A.sg_n0.g) S.N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
+      } else if (CODE == kUniform) {
         S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz));
         S.BN = fmaf(P.uB[0], T.eNx, fmaf(P.uB[1], T.eNy, P.uB[2] * T.eNz));
         S.BE = fmaf(P.uB[0], T.eEx, P.uB[1] * T.eEy);
@@ -292,6 +350,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const float BEb = 2.0f * fmaf(M, fmaf(S.BE, cI + Xc, S.BN * Xs), S.BE * tq_);
       const float BNb = 2.0f * fmaf(M, fmaf(S.BN, cI - Xc, S.BE * Xs), S.BN * tq_);
       if constexpr (CODE == kUniform) acc.add(T, S, BNb, BEb, wgt, MK);
+      else if constexpr (CODE == kStack16) acc.add(P, T, sa, S, BNb, BEb, wgt);
       else acc.add(P, T, aux, S, zf, BNb, BEb, wgt, MK);
     }
     carry += (double)hi + (double)lo;
@@ -325,7 +384,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   }
 
   // ---- block reduction -> partial[b][block][16]
-  constexpr int NP = (CODE == kUniform) ? 6 : (CODE == kAnalyticFull ? 16 : 4);
+  constexpr int NP = (CODE == kUniform) ? 6 : ((CODE == kAnalyticFull || CODE == kStack16) ? 16 : 4);
   __shared__ float red[kBlock / 32][16];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
@@ -399,6 +458,7 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
     const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
     a.f0 = f0; a.accumulate = f0 > 0;
     if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc>(G, nf, grid, st, a, ft);
+    else if (code == kStack16) launch_vjp<kStack16>(G, nf, grid, st, a, ft);
     else if (code == kAnalyticFull) launch_vjp<kAnalyticFull>(G, nf, grid, st, a, ft);
     else launch_vjp<kUniform>(G, nf, grid, st, a, ft);
     ++*launches;

@@ -40,6 +40,12 @@ FULL16_NOMINAL = np.array([
 FULL16_NAMES = ("b0", "psi0", "psi1", "chi0", "h_b", "B_h", "z_h0", "r_h", "w_h",
                 "n0", "h_r", "h_z", "p", "ne0", "h_er", "h_ez")
 DISC4_NAMES = ("b0", "psi0", "psi1", "chi0")
+# The paper's own 16-parameter model: Table 3, (b0 [uG], psi0, psi1, chi0 [rad]) x 4 spirals,
+# stacked by Eq. (16)
+STACK16_TABLE3 = np.array([1.20, 0.4712, 0.0157, 0.4363,
+                           3.50, 0.6457, 0.5393, 0.6108,
+                           7.70, 1.1693, 1.0629, 1.1344,
+                           5.70, 1.6930, 1.5865, 1.6580])
 
 
 @dataclasses.dataclass
@@ -183,6 +189,16 @@ def config(i: int) -> Workload:
         return Workload("cfg4_large_full16", "full16", 256, 1024, 30.0, np.geomspace(0.408e9, 30e9, 8),
                         _f32(FULL16_NOMINAL)[None, :], None, cot_seed=2004)
     raise ValueError("config index 0..4")
+
+
+def stack16(nside=32, n_los=256, s_max=20.0, freqs=(2.4e9,), batch=1, seed=1016) -> Workload:
+    """The paper's section 4.3 model (Eq. 16, Table 3): batch > 1 draws each vector within +-10 % of Table 3."""
+    p = np.tile(STACK16_TABLE3, (batch, 1))
+    if batch > 1:
+        rng = np.random.Generator(np.random.PCG64(seed))
+        p[1:] *= 1.0 + 0.1 * rng.uniform(-1.0, 1.0, size=(batch - 1, 16))
+    return Workload("stack16_table3", "stack16", nside, n_los, s_max, np.asarray(freqs, dtype=np.float64), _f32(p),
+                    _f32(AUX_NOMINAL), cot_seed=3016)
 
 
 def uniform_toy(bvec=(6.0, 0.0, 0.0), n0=4.01e-5, ne=0.01, alpha=3.0, nside=8, n_los=64, s_max=4.0,
