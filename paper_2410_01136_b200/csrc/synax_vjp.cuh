@@ -189,7 +189,7 @@ struct VjpArgs {
 
 // grid = (n_blocks, batch); block = kBlock threads; G lanes per sightline.
 #ifndef SYNAX_VJP_MINB
-#define SYNAX_VJP_MINB 3
+#define SYNAX_VJP_MINB 1
 #endif
 template <int CODE, int G, int NF>
 __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
