@@ -412,8 +412,11 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 // reduced to turns exactly).  G lanes per sightline; groups stride over the flag list written by
 // forward_kernel, or over all sightlines when the list is null.
 // ------------------------------------------------------------------------------------------------
+#ifndef SYNAX_F64_MINB
+#define SYNAX_F64_MINB 4
+#endif
 template <int CODE, int G, int NF>
-__global__ void __launch_bounds__(kBlock) forward_f64_kernel(const __grid_constant__ ForwardArgs A,
+__global__ void __launch_bounds__(kBlock, SYNAX_F64_MINB) forward_f64_kernel(const __grid_constant__ ForwardArgs A,
                                                              const __grid_constant__ FreqTab ft) {
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
