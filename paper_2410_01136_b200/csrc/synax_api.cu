@@ -535,8 +535,11 @@ extern "C" synax_status synax_loglike_vjp(const synax_plan* plan, const synax_mo
     const unsigned bx = (unsigned)std::min<int64_t>((per_batch + 255) / 256, (int64_t)sm_count(plan->device) * 8);
     for (int k = 0; k < 3; ++k) {
       if (!obs[k] || inv_var[k] == 0.0) continue;
-      loglike_residual_kernel<<<dim3(bx, (unsigned)batch), 256, 0, st>>>(m[k], obs[k], per_batch, (float)inv_var[k], logL);
-      plan->launches++;
+      for (int b0 = 0; b0 < batch; b0 += 65535) {   // gridDim.y limit
+        loglike_residual_kernel<<<dim3(bx, (unsigned)std::min(65535, batch - b0)), 256, 0, st>>>(
+            m[k] + (size_t)b0 * per_batch, obs[k], per_batch, (float)inv_var[k], logL + b0);
+        plan->launches++;
+      }
       cot[k] = m[k];
     }
     cudaError_t e = cudaGetLastError();

@@ -2,6 +2,7 @@
 // half-cell scan (single forward-order sweep using sum_{n>m} = T - P_m),
 // A11 field partials and reductions.  Nothing of the forward is stored: everything is recomputed.
 #pragma once
+#include <algorithm>
 #include <type_traits>
 
 #include "../../include/synax.h"
@@ -180,6 +181,7 @@ struct VjpArgs {
   Geometry geo;
   const BatchConsts* bc;
   int batch, f0, n_freq_total;
+  int b0;           // first batch element of this launch (gridDim.y <= 65535 per launch)
   const float* dI; const float* dQ; const float* dU;   // may be null
   ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
   float* partial;   // [batch][n_blocks][16]
@@ -194,7 +196,7 @@ struct VjpArgs {
 template <int CODE, int G, int NF>
 __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
   constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
-  const int b = blockIdx.y;
+  const int b = A.b0 + blockIdx.y;
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
   int64_t pix = tid / G;
@@ -447,22 +449,24 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   a.geo = geo; a.bc = bc; a.batch = batch; a.n_freq_total = ft.n_freq;
   a.dI = dI; a.dQ = dQ; a.dU = dU; a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_blocks = (int)((geo.npix * G + kBlock - 1) / kBlock);
-  if (batch > 65535) return SYNAX_ERR_UNSUPPORTED;
   float* partial = nullptr;
   if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
     return SYNAX_ERR_ALLOC;
   a.partial = partial;
-  const dim3 grid((unsigned)a.n_blocks, (unsigned)batch);
-  for (int f0 = 0; f0 < ft.n_freq;) {
-    const int rem = ft.n_freq - f0;
-    const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
-    a.f0 = f0; a.accumulate = f0 > 0;
-    if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc>(G, nf, grid, st, a, ft);
-    else if (code == kStack16) launch_vjp<kStack16>(G, nf, grid, st, a, ft);
-    else if (code == kAnalyticFull) launch_vjp<kAnalyticFull>(G, nf, grid, st, a, ft);
-    else launch_vjp<kUniform>(G, nf, grid, st, a, ft);
-    ++*launches;
-    f0 += nf;
+  for (int b0 = 0; b0 < batch; b0 += 65535) {   // gridDim.y limit
+    const dim3 grid((unsigned)a.n_blocks, (unsigned)std::min(65535, batch - b0));
+    a.b0 = b0;
+    for (int f0 = 0; f0 < ft.n_freq;) {
+      const int rem = ft.n_freq - f0;
+      const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
+      a.f0 = f0; a.accumulate = f0 > 0;
+      if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc>(G, nf, grid, st, a, ft);
+      else if (code == kStack16) launch_vjp<kStack16>(G, nf, grid, st, a, ft);
+      else if (code == kAnalyticFull) launch_vjp<kAnalyticFull>(G, nf, grid, st, a, ft);
+      else launch_vjp<kUniform>(G, nf, grid, st, a, ft);
+      ++*launches;
+      f0 += nf;
+    }
   }
   vjp_reduce_kernel<<<batch, 256, 0, st>>>(partial, a.n_blocks, n_params, grad);
   ++*launches;

@@ -1,0 +1,101 @@
+"""Maximum sizes and robustness of the CUDA path (all through the C ABI): n_los = 65536, a large nside on sampled
+pixels, batches beyond the 65535 grid.y limit, two plans on two streams, NaN parameters."""
+import numpy as np
+import pytest
+
+import oracle
+import parity
+from paper_2410_01136_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def test_max_samples_per_sightline():
+    w = wl.config(1).scaled(nside=1, n_los=65536)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what="n_los = 65536")
+    cots = w.cotangents()
+    g, ref = parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref))
+
+
+def test_large_nside_on_sampled_pixels():
+    """nside = 2048 (50,331,648 sightlines, full launch); the oracle recomputes every 100,003rd pixel."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(0).scaled(nside=2048, n_los=4)
+    plan, model, params = parity.gpu_objects(w)
+    assert plan.npix == 12 * 2048 * 2048
+    I, Q, U = sx.forward(plan, model, params)
+    torch.cuda.synchronize()
+    pix = np.arange(7, plan.npix, 100003)
+    idx = torch.from_numpy(pix).cuda()
+    sub = tuple(t[..., idx].cpu().numpy().astype(np.float64) for t in (I, Q, U))
+    assert all(bool(torch.isfinite(t).all()) for t in (I, Q, U))
+    plan.close()
+    ref = parity.oracle_forward(w, pix=pix)
+    parity.assert_maps_close(sub, ref, what="nside = 2048 (sampled pixels)")
+
+
+def test_batch_beyond_grid_y_limit():
+    """70,000 parameter vectors: the VJP launches in chunks of 65,535 batch elements."""
+    base = wl.config(2).scaled(nside=1, n_los=16, batch=1)
+    rng = np.random.Generator(np.random.PCG64(70))
+    p = base.params.astype(np.float64) * (1.0 + 0.1 * rng.uniform(-1, 1, (70000, 16)))
+    w = wl.Workload("big_batch", "full16", 1, 16, 20.0, base.freqs, p.astype(np.float32), None, cot_seed=71)
+    maps, _ = parity.gpu_forward(w)
+    cots = w.cotangents()
+    g = parity.gpu_vjp(w, cots)
+    assert np.all(np.isfinite(g))
+    for b in (0, 65534, 65535, 69999):
+        wb = wl.Workload("b", "full16", 1, 16, 20.0, base.freqs, w.params[b:b + 1], None)
+        parity.assert_maps_close(tuple(m[b:b + 1] for m in maps), parity.oracle_forward(wb), what=f"batch element {b}")
+        gb = parity.oracle_vjp(wb, tuple(c[b:b + 1] for c in cots))
+        assert np.all(np.abs(g[b:b + 1] - gb) <= parity.GRAD_TOL * np.abs(gb)), b
+
+
+def test_batch_times_npix_limit_is_an_error():
+    import torch
+    import paper_2410_01136_b200 as sx
+    plan = sx.Plan(256, 4, 20.0, [23e9])                      # npix = 786,432: batch 4096 -> 3.2e9 sightlines >= 2^31
+    params = torch.zeros((4096, 16), device="cuda")
+    I = torch.zeros(8, device="cuda")
+    with pytest.raises(sx.SynaxError, match="INVALID_ARG"):
+        sx.forward(plan, sx.Model("full16"), params, out=(I, I, I))
+    plan.close()
+
+
+def test_two_plans_on_two_streams_match_serial_results():
+    import torch
+    import paper_2410_01136_b200 as sx
+    wa, wb = wl.config(1).scaled(nside=32, n_los=128), wl.config(4).scaled(nside=16, n_los=256)
+    pa, ma, xa = parity.gpu_objects(wa)
+    pb, mb, xb = parity.gpu_objects(wb)
+    ra = [t.clone() for t in sx.forward(pa, ma, xa)]
+    rb = [t.clone() for t in sx.forward(pb, mb, xb)]
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(3):
+        with torch.cuda.stream(s1):
+            oa = sx.forward(pa, ma, xa)
+        with torch.cuda.stream(s2):
+            ob = sx.forward(pb, mb, xb)
+    s1.synchronize(); s2.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(ra, oa)) and all(torch.equal(a, b) for a, b in zip(rb, ob))
+    pa.close(); pb.close()
+
+
+def test_nan_parameters_give_nan_maps_not_a_fault():
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(0)
+    plan, model, params = parity.gpu_objects(w)
+    params[0, 0] = float("nan")
+    I, Q, U = sx.forward(plan, model, params)
+    g = sx.vjp(plan, model, params, *[torch.from_numpy(c).cuda() for c in w.cotangents()])
+    torch.cuda.synchronize()
+    assert bool(torch.isnan(I).any()) and bool(torch.isnan(g).any())
+    params[0, 0] = 6.0                                          # the plan and the library are still usable
+    I2, _, _ = sx.forward(plan, model, params)
+    assert bool(torch.isfinite(I2).all())
+    plan.close()
