@@ -216,7 +216,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False):
+def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False, graph=False):
     """Device-resident timing of forward and VJP with CUDA events on the launching stream, L2 flushed between
     timed calls; then (optionally) the host-buffer entry points.  pix_range: this rank's pixel shard (strong
     scaling), with the one gradient all-reduce of the method inside the timed VJP when reduce_grad is set."""
@@ -258,6 +258,23 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     tv = np.array([e[1].elapsed_time(e[2]) for e in evs]) * 1e-3
     res = dict(t_fwd=float(tf.mean()), t_vjp=float(tv.mean()), t_fwd_min=float(tf.min()), t_vjp_min=float(tv.min()),
                launches=int(l1 - l0), escalated=plan.stats()["escalated"])
+    if graph and not reduce_grad:
+        # the whole step captured once in a CUDA graph and replayed (pays off when a step is launch-bound: cfg 0, 1)
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            step()
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            g.replay()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        res["t_graph"] = e0.elapsed_time(e1) * 1e-3 / steps
     if want_e2e:
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
         hp = pin(w.params); hc = [pin(c) for c in cots_h]
@@ -322,7 +339,7 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     barrier()
-    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False, **kw)
+    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False, graph=args.graph, **kw)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     e = time_config(sx, torch, w, min(args.steps, 5), 1, flush_buf, want_e2e=True, **kw)
@@ -370,6 +387,9 @@ def run_ours(args):
                                                                     "achieved": fp_fwd * local_samples / r["t_fwd"] / 1e12,
                                                                     "frac": fp_fwd * local_samples / r["t_fwd"] / 1e12 / peak}},
         }
+        if "t_graph" in r:
+            line["cuda_graph"] = {"ms_per_step": 1e3 * r["t_graph"], "value": samples / r["t_graph"], "unit": UNIT,
+                                  "note": "forward + VJP captured once, replayed back to back (no L2 flush between replays)"}
         if clocks and clocks.get("sm_mhz"):
             line["roofline"]["frac_at_sustained_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
         if world == 1 and not args.no_cpu_baseline:
@@ -398,6 +418,7 @@ def main():
     ap.add_argument("--nside", type=int, default=0, help="override the config's nside (runtime sweeps)")
     ap.add_argument("--n-los", type=int, default=0, help="override the config's samples per sightline")
     ap.add_argument("--freq-hz", type=float, default=0.0, help="run at this single frequency instead of the config's")
+    ap.add_argument("--graph", action="store_true", help="also time the step captured in a CUDA graph (launch-bound configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline oracle sample")
     args = ap.parse_args()

@@ -99,3 +99,39 @@ def test_nan_parameters_give_nan_maps_not_a_fault():
     I2, _, _ = sx.forward(plan, model, params)
     assert bool(torch.isfinite(I2).all())
     plan.close()
+
+
+def test_forward_and_vjp_are_cuda_graph_capturable():
+    """No call synchronises or allocates outside the stream-ordered pool: a whole step can be captured once and
+    replayed (the launch-bound regime of config 0: 9 launches per step)."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(0)
+    plan, model, params = parity.gpu_objects(w)
+    cots = [torch.from_numpy(c).cuda() for c in w.cotangents()]
+    out = sx.forward(plan, model, params)
+    g = sx.vjp(plan, model, params, *cots)
+    torch.cuda.synchronize()
+    ref_out, ref_g = [t.clone() for t in out], g.clone()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):                                   # warm-up on the capture stream
+        sx.forward(plan, model, params, out=out)
+        sx.vjp(plan, model, params, *cots, out=g)
+    s.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        sx.forward(plan, model, params, out=out)
+        sx.vjp(plan, model, params, *cots, out=g)
+    for t in out:
+        t.zero_()
+    g.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(out, ref_out)) and torch.equal(g, ref_g)
+    params.mul_(1.1)                                             # same graph, new parameter values
+    graph.replay()
+    torch.cuda.synchronize()
+    eager = sx.forward(plan, model, params)
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(out, eager))
+    plan.close()
