@@ -164,6 +164,7 @@ struct GridFwdArgs {
 
 // Round-off scale of a sightline's Faraday sum, k-independent part: sum_n |n_e| (|B_LOS| + |B_N| + |B_E|),
 // estimated from every 8th sample with the fp32 chain (whole warp; returns the same value in every lane).
+template <bool SG>
 __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const BatchConsts& P, const Triad& T,
                                                         const Geometry& geo, const ScalarGridDesc& sg_ne, int lane) {
   float acc = 0.f;
@@ -174,7 +175,7 @@ __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const
     float B[3], N0, ne;
     gather_B(G, c, B);
     densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
-    if (sg_ne.g) ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
+    if (SG && sg_ne.g) ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
     const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
     const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
     const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
@@ -185,7 +186,7 @@ __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const
 
 // One sightline, whole warp, lanes on CONSECUTIVE samples (neighbouring lanes gather neighbouring cells).
 // PRECISE = float64 trilinear weights / n_e / scan.  Returns the (exact, not estimated) round-off scale.
-template <int NF, bool PRECISE>
+template <int NF, bool PRECISE, bool SG>
 __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const GridDesc& G, const FreqTab& ft,
                                                     const BatchConsts& P, const BatchConstsD& D, const Triad& T,
                                                     const double4 dir, int lane, float& accI, float (&accQ)[NF],
@@ -211,8 +212,8 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       gather_B(G, c, B);
       float N0, ne;
       densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
-      if (A.sg_ne.g) ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
-      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
+      if (SG && A.sg_ne.g) ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+      if (SG && A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ne *= T.scalef;
       const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
       const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
@@ -227,8 +228,8 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       double Bpar, BN, BE, ne;
       float N0;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BN, BE, N0, ne);
-      if (A.sg_ne.g) ne = scalar_grid_at<double>(A.sg_ne, xd, yd, zd);
-      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
+      if (SG && A.sg_ne.g) ne = scalar_grid_at<double>(A.sg_ne, xd, yd, zd);
+      if (SG && A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ne *= T.scale;
       if (active) emission(P, (float)BN, (float)BE, N0, eI, a, bq);
       const double gn = active ? ne * Bpar : 0.0;
@@ -256,7 +257,7 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
 // round-off scale from every 8th sample sends it straight to the float64 chain when the Faraday rotation is
 // strong; otherwise the fp32 sweep runs and is redone in float64 only if its exact criterion fires.
 // ------------------------------------------------------------------------------------------------
-template <int NF>
+template <int NF, bool SG>
 __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_constant__ GridFwdArgs GA,
                                                               const __grid_constant__ FreqTab ft) {
   const ForwardArgs& A = GA.f;
@@ -271,12 +272,12 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
     const Triad T = load_triad(A.geo, pix);
     float accI, accQ[NF], accU[NF];
     bool precise = GA.mode == 2;
-    if (GA.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
+    if (GA.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
     if (!precise) {
-      const float scale = grid_forward_sweep<NF, false>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
+      const float scale = grid_forward_sweep<NF, false, SG>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
       precise = GA.mode == 0 && scale > A.flag_S;
     }
-    if (precise) grid_forward_sweep<NF, true>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
+    if (precise) grid_forward_sweep<NF, true, SG>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
     if (lane == 0) {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
@@ -323,7 +324,7 @@ struct GridVjpArgs {
 
 // Sweep 1 of the gridded adjoint for one sightline (whole warp): per-sample forward quantities, cotangent
 // fan-out (A9) and the per-sample hand-over to sweep 2 through shared memory.  Returns sum n_e (|B_LOS| + |B_N| + |B_E|).
-template <int NF, bool PRECISE>
+template <int NF, bool PRECISE, bool SG>
 __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const FreqTab& ft, const GridDesc& G,
                                                  const BatchConsts& P, const BatchConstsD& D, const Triad& T,
                                                  const double4 dir, int lane,
@@ -347,8 +348,8 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       float B[3];
       gather_B(G, c, B);
       densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
-      if (A.sg_ne.g) ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
-      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
+      if (SG && A.sg_ne.g) ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+      if (SG && A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ne *= T.scalef;
       const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
       BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
@@ -361,8 +362,8 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
     } else {
       double Bpar, BNd, BEd, ned;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BNd, BEd, N0, ned);
-      if (A.sg_ne.g) ned = scalar_grid_at<double>(A.sg_ne, xd, yd, zd);
-      if (A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
+      if (SG && A.sg_ne.g) ned = scalar_grid_at<double>(A.sg_ne, xd, yd, zd);
+      if (SG && A.sg_n0.g) N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       ned *= T.scale;
       BN = (float)BNd; BE = (float)BEd; ne = (float)ned;
       const double gn = active ? ned * Bpar : 0.0;
@@ -399,7 +400,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
   return group_sum<32>(absS);
 }
 
-template <int NF>
+template <int NF, bool SG>
 __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant__ GridVjpArgs A,
                                                           const __grid_constant__ FreqTab ft) {
   extern __shared__ float smem[];
@@ -430,11 +431,11 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     // when the rotation angle of this sightline is large (warp-uniform decision)
     float absS = 0.f;
     bool precise = A.mode == 2;
-    if (A.mode == 0) precise = grid_roundoff_estimate(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
-    if (!precise) absS = grid_vjp_sweep1<NF, false>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
+    if (A.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
+    if (!precise) absS = grid_vjp_sweep1<NF, false, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
     if (precise || (A.mode == 0 && absS > A.flag_S)) {
       __syncwarp();
-      grid_vjp_sweep1<NF, true>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
+      grid_vjp_sweep1<NF, true, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
     }
     __syncwarp();
     // ---- sweep 2: contiguous chunk per lane walked BACKWARDS, so that the suffix sum of Sbar that the
@@ -464,7 +465,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
         c = locate(G, xd, yd, zd);
         float N0_unused;
         densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0_unused, ne_m);
-        if (A.sg_ne.g) ne_m = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+        if (SG && A.sg_ne.g) ne_m = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
         ne_m *= T.scalef;
       }
       const int cell = (m >= m0 && c.inbox) ? c.base : -1;
@@ -517,13 +518,20 @@ static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
 
 static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f.f0);
+  const bool sg = a.f.sg_ne.g || a.f.sg_n0.g;   // gridded n_e / N_0: separate instantiation keeps the common path lean
+#define SYNAX_GF(NFV)                                                                  \
+  do {                                                                                 \
+    if (sg) grid_forward_kernel<NFV, true><<<blocks, kBlock, 0, st>>>(a, ft);          \
+    else grid_forward_kernel<NFV, false><<<blocks, kBlock, 0, st>>>(a, ft);            \
+  } while (0)
   switch (nf) {
-    case 1: grid_forward_kernel<1><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 2: grid_forward_kernel<2><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 3: grid_forward_kernel<3><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 4: grid_forward_kernel<4><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    default: grid_forward_kernel<8><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 1: SYNAX_GF(1); break;
+    case 2: SYNAX_GF(2); break;
+    case 3: SYNAX_GF(3); break;
+    case 4: SYNAX_GF(4); break;
+    default: SYNAX_GF(8); break;
   }
+#undef SYNAX_GF
 }
 
 static synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_model* m, const float* grid,
@@ -570,10 +578,16 @@ static synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const Batch
   for (int f0 = 0; f0 < ft.n_freq;) {
     const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
     a.f0 = f0;
-#define SYNAX_GV(NFV)                                                                                      \
-  do {                                                                                                     \
-    cudaFuncSetAttribute(grid_vjp_kernel<NFV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
-    grid_vjp_kernel<NFV><<<blocks, kBlock, smem, st>>>(a, shift_freqs(ft, a.f0));                                          \
+    const bool sg = a.sg_ne.g || a.sg_n0.g;
+#define SYNAX_GV(NFV)                                                                                              \
+  do {                                                                                                             \
+    if (sg) {                                                                                                      \
+      cudaFuncSetAttribute(grid_vjp_kernel<NFV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
+      grid_vjp_kernel<NFV, true><<<blocks, kBlock, smem, st>>>(a, shift_freqs(ft, a.f0));                          \
+    } else {                                                                                                       \
+      cudaFuncSetAttribute(grid_vjp_kernel<NFV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   \
+      grid_vjp_kernel<NFV, false><<<blocks, kBlock, smem, st>>>(a, shift_freqs(ft, a.f0));                         \
+    }                                                                                                              \
   } while (0)
     switch (nf) {
       case 1: SYNAX_GV(1); break;
