@@ -406,8 +406,12 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     }
   }
   const int G = pick_lanes(plan, n_sl);
-  auto blocks_for = [&](int lanes) {
-    return (unsigned)std::min<int64_t>((n_sl * lanes + kBlock - 1) / kBlock, (int64_t)sms * 16);
+  // Every sightline (count known on the host): one group per sightline and the hardware block scheduler balances the
+  // CTAs (a persistent grid of 16 CTAs/SM left a 14 % tail at cfg 4: 2.6 sightlines per thread).  Flag list (length
+  // known only on the device): persistent grid, groups stride over the list.
+  auto blocks_for = [&](int lanes, bool use_list) {
+    const int64_t full = (n_sl * lanes + kBlock - 1) / kBlock;
+    return (unsigned)(use_list ? std::min<int64_t>(full, (int64_t)sms * 16) : full);
   };
   auto run_f64 = [&](int lanes, int run_when, bool use_list) {
     ForwardArgs pa = a;
@@ -416,10 +420,10 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       pa.f0 = f0;
-      if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
-      else if (code == kStack16) launch_f64<kStack16>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
-      else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
-      else launch_f64<kUniform>(lanes, nf, blocks_for(lanes), st, pa, plan->ft);
+      if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
+      else if (code == kStack16) launch_f64<kStack16>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
+      else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
+      else launch_f64<kUniform>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
       plan->launches++;
       f0 += nf;
     }

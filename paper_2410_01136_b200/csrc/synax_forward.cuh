@@ -5,6 +5,9 @@
 
 namespace synax {
 
+#ifndef SYNAX_FWD_FASTTRIG
+#define SYNAX_FWD_FASTTRIG false
+#endif
 #ifndef SYNAX_FAST_ACC
 #define SYNAX_FAST_ACC false
 #endif
@@ -335,7 +338,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         const double rho2d = fma(xd, xd, yd * yd);
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC, SYNAX_FWD_FASTTRIG>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
       if (CODE == kAnalyticDisc || CODE == kStack16) {
         if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
