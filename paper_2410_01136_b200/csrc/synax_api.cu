@@ -48,6 +48,7 @@ struct synax_plan {
   int precision;      // 0 auto, 1 fp32 only, 2 float64 chain everywhere
   double escalate_rad;
   int lanes;          // 0 heuristic
+  int* d_vjp_ctrl;    // device control block of the adjoint's pilot (kCtrlWords ints)
   int* d_flag_count;  // device control block, kCtrlWords ints: [flag count, pilot flagged, mode, -]
   int* h_flag_count;  // pinned host mirror (last forward)
   mutable int64_t launches;
@@ -117,6 +118,7 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   cudaError_t e = cudaGetDevice(&p->device);
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->dirs, (size_t)p->npix * 4 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, kCtrlWords * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_vjp_ctrl, kCtrlWords * sizeof(int));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_flag_count, kCtrlWords * sizeof(int));
   if (e == cudaSuccess) {
     for (int i = 0; i < kCtrlWords; ++i) p->h_flag_count[i] = 0;
@@ -133,6 +135,7 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
     synax_status st = fail(e == cudaErrorMemoryAllocation ? SYNAX_ERR_ALLOC : SYNAX_ERR_CUDA, "plan_create: %s", cudaGetErrorString(e));
     if (p->dirs) cudaFree(p->dirs);
     if (p->d_flag_count) cudaFree(p->d_flag_count);
+    if (p->d_vjp_ctrl) cudaFree(p->d_vjp_ctrl);
     if (p->h_flag_count) cudaFreeHost(p->h_flag_count);
     delete p;
     return st;
@@ -146,6 +149,7 @@ extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
   cudaFree(plan->dirs);
   if (plan->path) cudaFree(plan->path);
   cudaFree(plan->d_flag_count);
+  cudaFree(plan->d_vjp_ctrl);
   cudaFreeHost(plan->h_flag_count);
   delete plan;
   return SYNAX_OK;
@@ -399,7 +403,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
-      decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot);
+      decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 1, 4);
       plan->launches += 2;
       a.mode = ctrl + kCtrlMode;
       piloted = true;
@@ -466,7 +470,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   BatchConsts* bc = nullptr;
   BatchConstsD* bd = nullptr;
   CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
-  if (code == kGridB) CUDA_TRY(cudaMallocAsync((void**)&bd, sizeof(BatchConstsD) * (size_t)batch, st));
+  CUDA_TRY(cudaMallocAsync((void**)&bd, sizeof(BatchConstsD) * (size_t)batch, st));
   prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
                                                       make_aux(model), plan->ft, plan->delta, bc, bd);
   plan->launches++;
@@ -476,9 +480,10 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
                   make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
                   sm_count(plan->device), st, &plan->launches);
   else
-    rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
+    rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
-                      make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l),
+                      make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
+                      plan->d_vjp_ctrl,
                       dI, dQ, dU, grad, st, &plan->launches);
   cudaFreeAsync(bc, st);
   if (bd) cudaFreeAsync(bd, st);

@@ -603,9 +603,10 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
   if (lane == 0 && absS > A.flag_S) atomicAdd(ctrl + kCtrlPilotFlagged, 1);
 }
 
-__global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot) {
-  // more than a quarter flagged: redoing them after an fp32 pass costs more than one float64-chain pass
-  ctrl[kCtrlMode] = (4 * (int64_t)ctrl[kCtrlPilotFlagged] > n_pilot) ? kModeAllF64 : kModeFastThenList;
+__global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot, int num, int den) {
+  // forward (1/4): more than a quarter flagged -> redoing them after an fp32 pass costs more than one float64-chain
+  // pass.  adjoint (3/20): see analytic_vjp.
+  ctrl[kCtrlMode] = ((int64_t)den * ctrl[kCtrlPilotFlagged] > (int64_t)num * n_pilot) ? kModeAllF64 : kModeFastThenList;
 }
 
 }  // namespace synax

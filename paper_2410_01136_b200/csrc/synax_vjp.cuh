@@ -182,6 +182,8 @@ struct VjpArgs {
   const BatchConsts* bc;
   int batch, f0, n_freq_total;
   int b0;           // first batch element of this launch (gridDim.y <= 65535 per launch)
+  const BatchConstsD* bd;   // float64 constants (float64 Faraday chain variant)
+  const int* mode;  // device mode word written by decide_kernel, or null: the kernel whose variant is not chosen exits
   const float* dI; const float* dQ; const float* dU;   // may be null
   ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
   float* partial;   // [batch][n_blocks][16]
@@ -189,13 +191,41 @@ struct VjpArgs {
   int accumulate;   // 0: overwrite partials (first frequency block), 1: add
 };
 
+// n_e B_LOS Delta_i / Delta of one sample from the float64 chain (synax_f64.cuh) -- the adjoint's Faraday ANGLE needs
+// the same accuracy as the forward's when the rotation is strong (measured: fp32 angle, n_e doubled at 408 MHz ->
+// gradient errors 2.4e-3); the adjoint algebra itself stays fp32.
+template <int CODE>
+__device__ __forceinline__ double faraday_term_d(const BatchConsts& P, const BatchConstsD& D, const Triad& T,
+                                                 const ScalarGridDesc& sg_ne, double xd, double yd, double zd) {
+  double Bx, By, Bz, ne;
+  if (CODE == kUniform) {
+    Bx = (double)P.uB[0]; By = (double)P.uB[1]; Bz = (double)P.uB[2]; ne = (double)P.une;
+  } else {
+    const double rho2d = fma(xd, xd, yd * yd);
+    const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+    if (CODE == kStack16) {
+      eval_stack16_d(D, xd, yd, zd, rho2d, inside, Bx, By, Bz, ne);
+    } else {
+      const double x1[1] = {xd}, y1[1] = {yd}, z1[1] = {zd}, r1[1] = {rho2d};
+      const bool in1[1] = {inside};
+      double bx[1], by[1], bz[1], n1[1];
+      eval_analytic_dm<CODE == kAnalyticFull, 1>(D, x1, y1, z1, r1, in1, bx, by, bz, n1);
+      Bx = bx[0]; By = by[0]; Bz = bz[0]; ne = n1[0];
+    }
+    if ((CODE == kAnalyticDisc || CODE == kStack16) && sg_ne.g) ne = scalar_grid_at<double>(sg_ne, xd, yd, zd);
+  }
+  return T.scale * ne * fma(Bx, T.nxd, fma(By, T.nyd, Bz * T.nzd));
+}
+
 // grid = (n_blocks, batch); block = kBlock threads; G lanes per sightline.
+// PREC: Faraday sums and angles from the float64 chain (tile length P.tile_d as in forward_f64_kernel).
 #ifndef SYNAX_VJP_MINB
 #define SYNAX_VJP_MINB 1
 #endif
-template <int CODE, int G, int NF>
+template <int CODE, int G, int NF, bool PREC>
 __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
   constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
+  if (A.mode && ((*A.mode == kModeAllF64) != PREC)) return;   // the pilot chose the other variant
   const int b = A.b0 + blockIdx.y;
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
@@ -203,6 +233,8 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   const bool valid = pix < A.geo.npix;
   if (!valid) pix = A.geo.npix - 1;
   const BatchConsts& P = A.bc[b];
+  BatchConstsD D;
+  if (PREC) D = A.bd[b];
   const Triad T = load_triad(A.geo, pix);
   const int C = (A.geo.n_los + G - 1) / G;
   const int n0 = g * C, n1 = min(n0 + C, A.geo.n_los);
@@ -230,6 +262,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
       const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       s_d += delta;
+      if (PREC) { Sl += faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd); continue; }
       SampleF S;
       if (CODE == kUniform) {
         S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz)); S.ne = P.une;
@@ -266,8 +299,9 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   float Pl = 0.f;              // lane-local inclusive prefix of Sbar
   double carry = 0.0;
   double s_d = ((double)n0 + 0.5) * delta;
-  for (int ts = n0; ts < n1; ts += kTile) {
-    const int te = min(ts + kTile, n1);
+  const int tile = PREC ? P.tile_d : kTile;
+  for (int ts = n0; ts < n1; ts += tile) {
+    const int te = min(ts + tile, n1);
     // cotangents rotated by the Faraday angle of everything before this tile
     float rq[NF], ru[NF];
 #pragma unroll
@@ -279,6 +313,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       rq[f] = q; ru[f] = u;
     }
     float hi = 0.f, lo = 0.f;
+    double dl = 0.0;             // PREC: tile-local Faraday sum in float64
     for (int n = ts; n < te; ++n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
@@ -320,11 +355,18 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const float d2 = be2 - bn2, p2 = 2.0f * S.BE * S.BN;
       const float a = M * d2, bq = M * p2;
       // Faraday phase of this sample, tile-local
-      const float gn = S.ne * S.Bpar;
-      const float ph = fmaf(0.5f, gn, hi);
-      const float sum = hi + gn;
-      lo += gn - (sum - hi);
-      hi = sum;
+      float ph;
+      if (PREC) {
+        const double gd = faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd);
+        ph = (float)fma(0.5, gd, dl);
+        dl += gd;
+      } else {
+        const float gn = S.ne * S.Bpar;
+        ph = fmaf(0.5f, gn, hi);
+        const float sum = hi + gn;
+        lo += gn - (sum - hi);
+        hi = sum;
+      }
       // A9: fan-out over frequencies
       float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f;
 #pragma unroll
@@ -355,7 +397,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       else if constexpr (CODE == kStack16) acc.add(P, T, sa, S, BNb, BEb, wgt);
       else acc.add(P, T, aux, S, zf, BNb, BEb, wgt, MK);
     }
-    carry += (double)hi + (double)lo;
+    carry += PREC ? dl : (double)hi + (double)lo;
   }
 
   // ---- combine: Tw = T - P_off for this lane
@@ -424,31 +466,66 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_block
   }
 }
 
-template <int CODE, int G>
+template <int CODE, int G, bool PREC>
 static void launch_vjp_nf(int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
-    case 1: vjp_kernel<CODE, G, 1><<<grid, kBlock, 0, st>>>(a, ft); break;
-    case 2: vjp_kernel<CODE, G, 2><<<grid, kBlock, 0, st>>>(a, ft); break;
-    case 3: vjp_kernel<CODE, G, 3><<<grid, kBlock, 0, st>>>(a, ft); break;
-    case 4: vjp_kernel<CODE, G, 4><<<grid, kBlock, 0, st>>>(a, ft); break;
-    default: vjp_kernel<CODE, G, 8><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 1: vjp_kernel<CODE, G, 1, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 2: vjp_kernel<CODE, G, 2, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 3: vjp_kernel<CODE, G, 3, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 4: vjp_kernel<CODE, G, 4, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
+    default: vjp_kernel<CODE, G, 8, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
   }
 }
-template <int CODE>
+template <int CODE, bool PREC>
 static void launch_vjp(int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
-  if (G == 1) launch_vjp_nf<CODE, 1>(nf, grid, st, a, ft);
-  else if (G == 8) launch_vjp_nf<CODE, 8>(nf, grid, st, a, ft);
-  else launch_vjp_nf<CODE, 32>(nf, grid, st, a, ft);
+  if (G == 1) launch_vjp_nf<CODE, 1, PREC>(nf, grid, st, a, ft);
+  else if (G == 8) launch_vjp_nf<CODE, 8, PREC>(nf, grid, st, a, ft);
+  else launch_vjp_nf<CODE, 32, PREC>(nf, grid, st, a, ft);
+}
+template <bool PREC>
+static void launch_vjp_code(int code, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
+  if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc, PREC>(G, nf, grid, st, a, ft);
+  else if (code == kStack16) launch_vjp<kStack16, PREC>(G, nf, grid, st, a, ft);
+  else if (code == kAnalyticFull) launch_vjp<kAnalyticFull, PREC>(G, nf, grid, st, a, ft);
+  else launch_vjp<kUniform, PREC>(G, nf, grid, st, a, ft);
 }
 
-static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, int batch,
-                                 int n_params, int G, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0, const float* dI, const float* dQ, const float* dU, float* grad,
-                                 cudaStream_t st, int64_t* launches) {
+// The adjoint tolerates ~10x the Faraday round-off scale the forward does (gradients are sums over all pixels,
+// bound 1e-3 instead of 1e-4): measured at cfg 4, nominal n_e (10 % of the sightlines above 10 x escalate_rad) the
+// fp32 angles give <= 4e-4, n_e doubled gives 2.4e-3.  precision 0: a pilot over ~8k sightlines counts those above
+// 10 x escalate_rad; above 15 % the whole call uses float64 angles (no per-sightline mixing: the outputs are sums).
+constexpr double kVjpEscalateFactor = 10.0;
+
+static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
+                                 const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
+                                 const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int* ctrl,
+                                 const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
+                                 int64_t* launches) {
   VjpArgs a;
-  a.geo = geo; a.bc = bc; a.batch = batch; a.n_freq_total = ft.n_freq;
+  a.geo = geo; a.bc = bc; a.bd = bd; a.batch = batch; a.n_freq_total = ft.n_freq;
   a.dI = dI; a.dQ = dQ; a.dU = dU; a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_blocks = (int)((geo.npix * G + kBlock - 1) / kBlock);
+  a.mode = nullptr;
+  if (precision == 0) {
+    float k_max = 0.f;
+    for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
+    ForwardArgs pa;
+    pa.geo = geo; pa.bc = bc; pa.bd = bd; pa.batch = batch; pa.sg_ne = sg_ne; pa.sg_n0 = sg_n0;
+    pa.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
+    const int64_t n_sl = geo.npix * batch;
+    const int64_t stride = (n_sl / 8192) | 1;
+    const int64_t n_pilot = (n_sl + stride - 1) / stride;
+    const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
+    if (cudaMemsetAsync(ctrl, 0, kCtrlWords * sizeof(int), st) != cudaSuccess) return SYNAX_ERR_CUDA;
+    if (code == kAnalyticDisc) pilot_kernel<kAnalyticDisc><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
+    else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
+    else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
+    else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
+    decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 3, 20);
+    *launches += 2;
+    a.mode = ctrl + kCtrlMode;
+  }
   float* partial = nullptr;
   if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
     return SYNAX_ERR_ALLOC;
@@ -460,11 +537,8 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       const int rem = ft.n_freq - f0;
       const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
       a.f0 = f0; a.accumulate = f0 > 0;
-      if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc>(G, nf, grid, st, a, ft);
-      else if (code == kStack16) launch_vjp<kStack16>(G, nf, grid, st, a, ft);
-      else if (code == kAnalyticFull) launch_vjp<kAnalyticFull>(G, nf, grid, st, a, ft);
-      else launch_vjp<kUniform>(G, nf, grid, st, a, ft);
-      ++*launches;
+      if (precision != 2) { launch_vjp_code<false>(code, G, nf, grid, st, a, ft); ++*launches; }
+      if (precision != 1) { launch_vjp_code<true>(code, G, nf, grid, st, a, ft); ++*launches; }
       f0 += nf;
     }
   }

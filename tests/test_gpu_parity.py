@@ -348,3 +348,16 @@ def test_gpu_vjp_matches_gpu_finite_difference_direction():
     fd = lp - lm
     an = float(g @ (pp - pm))
     assert abs(fd - an) <= 2e-2 * abs(an) + 1e-12
+
+
+@pytest.mark.parametrize("ne_scale", [2.0, 4.0])
+def test_vjp_strong_rotation_uses_float64_angles(ne_scale):
+    """n_e doubled / quadrupled at 408 MHz: with fp32 Faraday angles the gradient misses the 1e-3 bound (2.4e-3 /
+    9e-3 measured); the adjoint's pilot must switch the call to float64 angles."""
+    w = wl.config(4).scaled(nside=16, n_los=1024)
+    w.params = w.params.copy()
+    w.params[0, 13] *= ne_scale
+    cots = w.cotangents()
+    ref = parity.oracle_vjp(w, cots)
+    _check_grad(parity.gpu_vjp(w, cots), ref, f"vjp n_e x{ne_scale} (auto)")
+    _check_grad(parity.gpu_vjp(w, cots, precision=2), ref, f"vjp n_e x{ne_scale} (float64 angles)")
