@@ -82,6 +82,17 @@ __device__ __forceinline__ void rsqrt_sqrt_nr(float x, float& ir, float& r) {
   ir = y; r = s;
 }
 
+// the same polynomials without the reduction, for |x| <= pi/4 (BatchConsts::angles_small)
+__device__ __forceinline__ void sincos_fma_small(float r, float& s, float& c) {
+  const float r2 = r * r;
+  float ps = fmaf(r2, -1.9515295891e-4f, 8.3321608736e-3f);
+  ps = fmaf(ps, r2, -1.6666654611e-1f);
+  s = fmaf(ps * r2, r, r);
+  float pc = fmaf(r2, 2.443315711809948e-5f, -1.388731625493765e-3f);
+  pc = fmaf(pc, r2, 4.166664568298827e-2f);
+  c = fmaf(pc * r2, r2, fmaf(r2, -0.5f, 1.0f));
+}
+
 // ------------------------------------------------------------------------------------------------
 // Per-batch-element constants, written by prologue_kernel (fp64 math, rounded once).
 // Canonical 16-parameter analytic model; DISC4 maps onto it with h_b = inf, B_h = 0.
@@ -99,6 +110,7 @@ struct BatchConsts {
   float q_exp;       // (alpha-3)/4 : (B_perp^2)^q_exp
   float pi_frac;     // (alpha+1)/(alpha+7/3)   Eq.(5)/Eq.(2)
   int alpha_is_3;
+  int angles_small;  // |psi0| + |psi1| <= pi/4 and |chi0| <= pi/4: psi and chi never leave [-pi/4, pi/4] (no range reduction)
   int tile_d;        // samples per tile of the float64-chain kernel (prologue_kernel)
   float coefI[kMaxFreq];  // c_f(alpha) * Delta  [K per (cm^-3 uG^((alpha+1)/2))]
   float coefP[kMaxFreq];  // pi_frac * coefI
@@ -239,7 +251,9 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
   // --- disc: B = A [cos psi cos chi rho_hat + sin psi cos chi phi_hat + sin chi z_hat]   Eq.(13)
   a.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;        // ln(rho/8) = ln2/2 (lg2 rho^2 - 6)
   const float psi = fmaf(P.p[2], a.lr, P.p[1]);
-  if (kFastTrig) { a.sp = mufu_sin(psi); a.cp = mufu_cos(psi); } else sincos_fma(psi, a.sp, a.cp);
+  if (kFastTrig) { a.sp = mufu_sin(psi); a.cp = mufu_cos(psi); }
+  else if (P.angles_small) sincos_fma_small(psi, a.sp, a.cp);
+  else sincos_fma(psi, a.sp, a.cp);
   if (kAcc) {
     const float e1 = exp2_fma(-2.0f * kLog2e * az);             // tanh(|z|) = (1-e)/(1+e)
     a.t = copysignf((1.0f - e1) * rcp_nr(1.0f + e1), z);
@@ -248,7 +262,9 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
     a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
   }
   const float chi = P.p[3] * a.t;
-  if (kFastTrig) { a.sc = mufu_sin(chi); a.cc = mufu_cos(chi); } else sincos_fma(chi, a.sc, a.cc);
+  if (kFastTrig) { a.sc = mufu_sin(chi); a.cc = mufu_cos(chi); }
+  else if (P.angles_small) sincos_fma_small(chi, a.sc, a.cc);
+  else sincos_fma(chi, a.sc, a.cc);
   float rad = 1.0f;
   if (P.k_hb != 0.0f) {
     const float dr = a.rho - 8.0f;

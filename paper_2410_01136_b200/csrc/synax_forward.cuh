@@ -136,6 +136,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
   c.q_exp = (float)((alpha - 3.0) * 0.25);
   c.pi_frac = (float)((alpha + 1.0) / (alpha + 7.0 / 3.0));
   c.alpha_is_3 = (c.p[12] == 3.0f) ? 1 : 0;
+  c.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4; |ln(rho/8)| < 1 in the annulus
   c.dpi_dalpha_over_pi = (float)(1.0 / (alpha + 1.0) - 1.0 / (alpha + 7.0 / 3.0));
   // Eq.(2) prefactor with B^((1+alpha)/2) nu^((1-alpha)/2) factored out
   const double g1 = tgamma(alpha * 0.25 - 1.0 / 12.0), g2 = tgamma(alpha * 0.25 + 19.0 / 12.0);
