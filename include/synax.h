@@ -106,8 +106,8 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
 /* Options.  key "precision": 0 = auto (default), 1 = fp32 only, 2 = float64 Faraday chain for every sightline.
  * Auto, forward: sightlines whose Faraday round-off scale k_max sum_n |n_e| (|B_LOS|+|B_N|+|B_E|) exceeds
  * "escalate_rad" (default 100 rad) take the float64 Faraday chain -- as a redo of a flagged list after the fp32
- * pass, or for every sightline when a device-side pilot finds more than a quarter flagged.  Auto, VJP: the whole
- * call uses float64 Faraday angles when the pilot finds more than 15 % of the sightlines above 10 x escalate_rad.
+ * pass, or for every sightline when a device-side pilot finds more than a quarter flagged.  Auto, VJP: decided per
+ * sightline inside the kernel -- those above 10 x escalate_rad take their Faraday angles from the float64 chain.
  * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0).
  * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32). */
 synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value);

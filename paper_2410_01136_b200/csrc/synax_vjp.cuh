@@ -183,7 +183,9 @@ struct VjpArgs {
   int batch, f0, n_freq_total;
   int b0;           // first batch element of this launch (gridDim.y <= 65535 per launch)
   const BatchConstsD* bd;   // float64 constants (float64 Faraday chain variant)
-  const int* mode;  // device mode word written by decide_kernel, or null: the kernel whose variant is not chosen exits
+  float flag_S;     // PMODE 2: sightlines whose round-off scale exceeds this take the float64 chain
+  const int* mode;  // auto: device word from decide_kernel -- kModeAllF64 = "some sightline is near the threshold: run the
+                    // per-sightline variant (PMODE 2)", else the lean fp32 variant (PMODE 0) runs; the other exits; or null
   const float* dI; const float* dQ; const float* dU;   // may be null
   ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
   float* partial;   // [batch][n_blocks][16]
@@ -218,14 +220,17 @@ __device__ __forceinline__ double faraday_term_d(const BatchConsts& P, const Bat
 }
 
 // grid = (n_blocks, batch); block = kBlock threads; G lanes per sightline.
-// PREC: Faraday sums and angles from the float64 chain (tile length P.tile_d as in forward_f64_kernel).
+// PMODE 0: fp32 Faraday angles; 1: Faraday sums and angles from the float64 chain for every sightline; 2: decided per
+// sightline -- its round-off scale k_max sum |n_e|(|B_LOS|+|B_N|+|B_E|), estimated from every 16th sample, against
+// A.flag_S (= 10 x escalate_rad / k_max): sightlines below it carry an angle error <= ~3e-7 x 1000 rad = 3e-4 rad,
+// inside the 1e-3 gradient bound; the others take the float64 chain.  The tile length is warp-uniform.
 #ifndef SYNAX_VJP_MINB
 #define SYNAX_VJP_MINB 1
 #endif
-template <int CODE, int G, int NF, bool PREC>
+template <int CODE, int G, int NF, int PMODE>
 __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
   constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
-  if (A.mode && ((*A.mode == kModeAllF64) != PREC)) return;   // the pilot chose the other variant
+  if (A.mode && ((*A.mode == kModeAllF64) != (PMODE == 2))) return;
   const int b = A.b0 + blockIdx.y;
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
@@ -234,11 +239,40 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   if (!valid) pix = A.geo.npix - 1;
   const BatchConsts& P = A.bc[b];
   BatchConstsD D;
-  if (PREC) D = A.bd[b];
+  if (PMODE != 0) D = A.bd[b];
   const Triad T = load_triad(A.geo, pix);
   const int C = (A.geo.n_los + G - 1) / G;
   const int n0 = g * C, n1 = min(n0 + C, A.geo.n_los);
   const double delta = A.geo.delta * T.scale;
+
+  bool prec = PMODE == 1;
+  if (PMODE == 2) {
+    const int step = (n1 - n0 >= 32) ? 16 : 1;
+    float est = 0.f;
+    for (int n = n0 + step / 2; n < n1; n += step) {
+      const double s_e = ((double)n + 0.5) * delta;
+      const double xd = fma(s_e, T.nxd, A.geo.obs[0]), yd = fma(s_e, T.nyd, A.geo.obs[1]), zd = fma(s_e, T.nzd, A.geo.obs[2]);
+      SampleF S;
+      if (CODE == kUniform) {
+        S.Bpar = fabsf(P.uB[0]) + fabsf(P.uB[1]) + fabsf(P.uB[2]); S.BN = 0.f; S.BE = 0.f; S.ne = P.une;
+      } else {
+        const double rho2d = fma(xd, xd, yd * yd);
+        const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+        if (CODE == kStack16) {
+          StackAux sa;
+          eval_stack16_f32<true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, sa);
+        } else {
+          AnalyticAux aux;
+          eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        }
+        if ((CODE == kAnalyticDisc || CODE == kStack16) && A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
+      }
+      est = fmaf(fabsf(S.ne), fabsf(S.Bpar) + fabsf(S.BN) + fabsf(S.BE), est);
+    }
+    est = group_sum<G>(est) * (float)step * T.scalef;
+    prec = est > A.flag_S;
+  }
+  const bool warp_prec = PMODE == 1 || (PMODE == 2 && __any_sync(0xffffffffu, prec));
 
   // cotangents of this sightline, coefficients folded in (zero for padded lanes)
   // (dQ, dU are re-read at every tile start -- L1 hits -- instead of being held in 2 NF registers)
@@ -262,7 +296,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
       const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       s_d += delta;
-      if (PREC) { Sl += faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd); continue; }
+      if (PMODE != 0 && prec) { Sl += faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd); continue; }
       SampleF S;
       if (CODE == kUniform) {
         S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz)); S.ne = P.une;
@@ -299,7 +333,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   float Pl = 0.f;              // lane-local inclusive prefix of Sbar
   double carry = 0.0;
   double s_d = ((double)n0 + 0.5) * delta;
-  const int tile = PREC ? P.tile_d : kTile;
+  const int tile = warp_prec ? P.tile_d : kTile;
   for (int ts = n0; ts < n1; ts += tile) {
     const int te = min(ts + tile, n1);
     // cotangents rotated by the Faraday angle of everything before this tile
@@ -313,7 +347,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       rq[f] = q; ru[f] = u;
     }
     float hi = 0.f, lo = 0.f;
-    double dl = 0.0;             // PREC: tile-local Faraday sum in float64
+    double dl = 0.0;             // float64-chain sightlines: tile-local Faraday sum in float64
     for (int n = ts; n < te; ++n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
@@ -356,7 +390,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const float a = M * d2, bq = M * p2;
       // Faraday phase of this sample, tile-local
       float ph;
-      if (PREC) {
+      if (PMODE != 0 && prec) {
         const double gd = faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd);
         ph = (float)fma(0.5, gd, dl);
         dl += gd;
@@ -397,7 +431,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       else if constexpr (CODE == kStack16) acc.add(P, T, sa, S, BNb, BEb, wgt);
       else acc.add(P, T, aux, S, zf, BNb, BEb, wgt, MK);
     }
-    carry += PREC ? dl : (double)hi + (double)lo;
+    carry += (PMODE != 0 && prec) ? dl : (double)hi + (double)lo;
   }
 
   // ---- combine: Tw = T - P_off for this lane
@@ -466,35 +500,35 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_block
   }
 }
 
-template <int CODE, int G, bool PREC>
+template <int CODE, int G, int PMODE>
 static void launch_vjp_nf(int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
-    case 1: vjp_kernel<CODE, G, 1, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
-    case 2: vjp_kernel<CODE, G, 2, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
-    case 3: vjp_kernel<CODE, G, 3, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
-    case 4: vjp_kernel<CODE, G, 4, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
-    default: vjp_kernel<CODE, G, 8, PREC><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 1: vjp_kernel<CODE, G, 1, PMODE><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 2: vjp_kernel<CODE, G, 2, PMODE><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 3: vjp_kernel<CODE, G, 3, PMODE><<<grid, kBlock, 0, st>>>(a, ft); break;
+    case 4: vjp_kernel<CODE, G, 4, PMODE><<<grid, kBlock, 0, st>>>(a, ft); break;
+    default: vjp_kernel<CODE, G, 8, PMODE><<<grid, kBlock, 0, st>>>(a, ft); break;
   }
 }
-template <int CODE, bool PREC>
+template <int CODE, int PMODE>
 static void launch_vjp(int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
-  if (G == 1) launch_vjp_nf<CODE, 1, PREC>(nf, grid, st, a, ft);
-  else if (G == 8) launch_vjp_nf<CODE, 8, PREC>(nf, grid, st, a, ft);
-  else launch_vjp_nf<CODE, 32, PREC>(nf, grid, st, a, ft);
+  if (G == 1) launch_vjp_nf<CODE, 1, PMODE>(nf, grid, st, a, ft);
+  else if (G == 8) launch_vjp_nf<CODE, 8, PMODE>(nf, grid, st, a, ft);
+  else launch_vjp_nf<CODE, 32, PMODE>(nf, grid, st, a, ft);
 }
-template <bool PREC>
+template <int PMODE>
 static void launch_vjp_code(int code, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
-  if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc, PREC>(G, nf, grid, st, a, ft);
-  else if (code == kStack16) launch_vjp<kStack16, PREC>(G, nf, grid, st, a, ft);
-  else if (code == kAnalyticFull) launch_vjp<kAnalyticFull, PREC>(G, nf, grid, st, a, ft);
-  else launch_vjp<kUniform, PREC>(G, nf, grid, st, a, ft);
+  if (code == kAnalyticDisc) launch_vjp<kAnalyticDisc, PMODE>(G, nf, grid, st, a, ft);
+  else if (code == kStack16) launch_vjp<kStack16, PMODE>(G, nf, grid, st, a, ft);
+  else if (code == kAnalyticFull) launch_vjp<kAnalyticFull, PMODE>(G, nf, grid, st, a, ft);
+  else launch_vjp<kUniform, PMODE>(G, nf, grid, st, a, ft);
 }
 
 // The adjoint tolerates ~10x the Faraday round-off scale the forward does (gradients are sums over all pixels,
-// bound 1e-3 instead of 1e-4): measured at cfg 4, nominal n_e (10 % of the sightlines above 10 x escalate_rad) the
-// fp32 angles give <= 4e-4, n_e doubled gives 2.4e-3.  precision 0: a pilot over ~8k sightlines counts those above
-// 10 x escalate_rad; above 15 % the whole call uses float64 angles (no per-sightline mixing: the outputs are sums).
+// bound 1e-3 instead of 1e-4).  precision 0: per sightline (PMODE 2), threshold 10 x escalate_rad -- unless a pilot
+// over ~8k sightlines finds none above HALF that threshold, in which case the lean fp32 variant (PMODE 0: fewer
+// registers, no estimate) runs (cfg 2 at 23 GHz: 8.2 instead of 9.5 ms).  Decided on the device, no host sync.
 constexpr double kVjpEscalateFactor = 10.0;
 
 static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
@@ -506,13 +540,14 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   a.geo = geo; a.bc = bc; a.bd = bd; a.batch = batch; a.n_freq_total = ft.n_freq;
   a.dI = dI; a.dQ = dQ; a.dU = dU; a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_blocks = (int)((geo.npix * G + kBlock - 1) / kBlock);
+  float k_max = 0.f;
+  for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
+  a.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
   a.mode = nullptr;
   if (precision == 0) {
-    float k_max = 0.f;
-    for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
     ForwardArgs pa;
     pa.geo = geo; pa.bc = bc; pa.bd = bd; pa.batch = batch; pa.sg_ne = sg_ne; pa.sg_n0 = sg_n0;
-    pa.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
+    pa.flag_S = 0.5f * a.flag_S;
     const int64_t n_sl = geo.npix * batch;
     const int64_t stride = (n_sl / 8192) | 1;
     const int64_t n_pilot = (n_sl + stride - 1) / stride;
@@ -522,7 +557,7 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
     else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
     else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
     else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
-    decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 3, 20);
+    decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 0, 1);   // any sampled sightline above half the threshold
     *launches += 2;
     a.mode = ctrl + kCtrlMode;
   }
@@ -537,8 +572,14 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       const int rem = ft.n_freq - f0;
       const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
       a.f0 = f0; a.accumulate = f0 > 0;
-      if (precision != 2) { launch_vjp_code<false>(code, G, nf, grid, st, a, ft); ++*launches; }
-      if (precision != 1) { launch_vjp_code<true>(code, G, nf, grid, st, a, ft); ++*launches; }
+      if (precision == 1) launch_vjp_code<0>(code, G, nf, grid, st, a, ft);
+      else if (precision == 2) launch_vjp_code<1>(code, G, nf, grid, st, a, ft);
+      else {
+        launch_vjp_code<0>(code, G, nf, grid, st, a, ft);
+        launch_vjp_code<2>(code, G, nf, grid, st, a, ft);
+        ++*launches;
+      }
+      ++*launches;
       f0 += nf;
     }
   }

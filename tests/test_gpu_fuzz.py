@@ -1,0 +1,32 @@
+"""Seeded random-parameter sweep of the analytic path: parity must hold away from the nominal parameter values too
+(frequencies 0.3-40 GHz, parameters within a factor 1.5 of nominal, alpha in [2.4, 3.4], both precision regimes)."""
+import numpy as np
+import pytest
+
+import parity
+from paper_2410_01136_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def _draw(seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    p = wl.FULL16_NOMINAL * np.exp(rng.uniform(-np.log(1.5), np.log(1.5), 16))
+    p[12] = rng.uniform(2.4, 3.4)
+    p[[0, 5]] *= rng.choice([-1.0, 1.0], 2)                       # field reversals are legal
+    freqs = np.sort(np.exp(rng.uniform(np.log(0.3e9), np.log(40e9), int(rng.integers(1, 7)))))
+    return wl.Workload(f"fuzz{seed}", "full16", 8, int(rng.integers(100, 700)), float(rng.uniform(15.0, 35.0)), freqs,
+                       p[None, :].astype(np.float32), None, cot_seed=seed)
+
+
+@pytest.mark.parametrize("seed", range(4000, 4012))
+def test_random_full16_forward_and_vjp(seed):
+    w = _draw(seed)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=w.name)
+    cots = w.cotangents()
+    g, ref = parity.gpu_vjp(w, cots)[0], parity.oracle_vjp(w, cots)[0]
+    # gradient in log-parameter space; a component that is a cancelling sum gets the floor of DESIGN.md C-2#14's kind
+    th = w.params[0].astype(np.float64)
+    lg, lref = g * th, ref * th
+    assert np.all(np.abs(lg - lref) <= 1e-3 * np.abs(lref) + 1e-5 * np.abs(lref).max()), (seed, np.abs(lg - lref) / np.abs(lref))
