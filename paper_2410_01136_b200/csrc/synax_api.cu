@@ -286,23 +286,23 @@ static int next_freq_block(int remaining) {
   return remaining;  // 1, 2, 3
 }
 
-template <int CODE, int G>
+template <int CODE, int G, bool LIST>
 static void launch_forward_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
-    case 1: forward_kernel<CODE, G, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 2: forward_kernel<CODE, G, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 3: forward_kernel<CODE, G, 3><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 4: forward_kernel<CODE, G, 4><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    default: forward_kernel<CODE, G, 8><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 1: forward_kernel<CODE, G, 1, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 2: forward_kernel<CODE, G, 2, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 3: forward_kernel<CODE, G, 3, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 4: forward_kernel<CODE, G, 4, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    default: forward_kernel<CODE, G, 8, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
   }
 }
-template <int CODE>
+template <int CODE, bool LIST>
 static void launch_forward(int G, int nf, int64_t n_sl, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
   const unsigned blocks = (unsigned)((n_sl * G + kBlock - 1) / kBlock);
-  if (G == 1) launch_forward_nf<CODE, 1>(nf, blocks, st, a, ft);
-  else if (G == 8) launch_forward_nf<CODE, 8>(nf, blocks, st, a, ft);
-  else launch_forward_nf<CODE, 32>(nf, blocks, st, a, ft);
+  if (G == 1) launch_forward_nf<CODE, 1, LIST>(nf, blocks, st, a, ft);
+  else if (G == 8) launch_forward_nf<CODE, 8, LIST>(nf, blocks, st, a, ft);
+  else launch_forward_nf<CODE, 32, LIST>(nf, blocks, st, a, ft);
 }
 template <int CODE, int G>
 static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
@@ -387,11 +387,12 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   int* ctrl = plan->d_flag_count;
   plan->last_n_sl = n_sl;
   CUDA_TRY(cudaMemsetAsync(ctrl, 0, kCtrlWords * sizeof(int), st));   // mode = fp32 pass then flagged list
-  a.mode = nullptr; a.run_when = 0;
+  a.mode = nullptr; a.run_when = 0; a.list_u = nullptr; a.count_u = nullptr;
   const int sms = sm_count(plan->device);
   // precision 0: a pilot over ~8k sightlines decides ON THE DEVICE between "fp32 pass + float64 redo of the flagged
-  // sightlines" and "float64 Faraday chain for every sightline" (cheaper once more than a quarter is flagged).
-  bool piloted = false;
+  // sightlines" (hardly any flagged), "float64 Faraday chain for every sightline" (nearly all flagged) and "split":
+  // classify_kernel sorts the sightlines into one list per chain (decide_forward_kernel).
+  bool piloted = false, split_ok = false;
   if (escalate) {
     CUDA_TRY(cudaMallocAsync((void**)&a.flag_list, sizeof(int) * (size_t)n_sl, st));
     a.flag_S = (float)(plan->escalate_rad / (double)k_max);
@@ -403,8 +404,22 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
       else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
-      decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 1, 4);
-      plan->launches += 2;
+      // the split mode costs four more launches: only for calls long enough not to notice (cfg 1: 0.19 ms in all)
+      split_ok = n_sl >= 262144;
+      if (split_ok) {
+        decide_forward_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot);
+        CUDA_TRY(cudaMallocAsync((void**)&a.list_u, sizeof(int) * (size_t)n_sl, st));
+        a.count_u = ctrl + kCtrlCountU;
+        const unsigned cb = (unsigned)std::min<int64_t>((n_sl + kBlock - 1) / kBlock, (int64_t)sm_count(plan->device) * 16);
+        if (code == kAnalyticDisc) classify_kernel<kAnalyticDisc><<<cb, kBlock, 0, st>>>(a, ctrl);
+        else if (code == kStack16) classify_kernel<kStack16><<<cb, kBlock, 0, st>>>(a, ctrl);
+        else if (code == kAnalyticFull) classify_kernel<kAnalyticFull><<<cb, kBlock, 0, st>>>(a, ctrl);
+        else classify_kernel<kUniform><<<cb, kBlock, 0, st>>>(a, ctrl);
+        plan->launches += 3;
+      } else {
+        decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 1, 4);   // more than a quarter flagged: all-float64
+        plan->launches += 2;
+      }
       a.mode = ctrl + kCtrlMode;
       piloted = true;
     }
@@ -413,9 +428,11 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   // Every sightline (count known on the host): one group per sightline and the hardware block scheduler balances the
   // CTAs (a persistent grid of 16 CTAs/SM left a 14 % tail at cfg 4: 2.6 sightlines per thread).  Flag list (length
   // known only on the device): persistent grid, groups stride over the list.
-  auto blocks_for = [&](int lanes, bool use_list) {
+  // Split mode: the list is long (2-85 % of the sightlines), so it takes the lane count of the full pass and a grid
+  // sized for all sightlines (CTAs past the list's end exit at once).
+  auto blocks_for = [&](int lanes, bool use_list, int run_when) {
     const int64_t full = (n_sl * lanes + kBlock - 1) / kBlock;
-    return (unsigned)(use_list ? std::min<int64_t>(full, (int64_t)sms * 16) : full);
+    return (unsigned)(use_list && run_when != 3 ? std::min<int64_t>(full, (int64_t)sms * 16) : full);
   };
   auto run_f64 = [&](int lanes, int run_when, bool use_list) {
     ForwardArgs pa = a;
@@ -424,10 +441,10 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       pa.f0 = f0;
-      if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
-      else if (code == kStack16) launch_f64<kStack16>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
-      else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
-      else launch_f64<kUniform>(lanes, nf, blocks_for(lanes, use_list), st, pa, plan->ft);
+      if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
+      else if (code == kStack16) launch_f64<kStack16>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
+      else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
+      else launch_f64<kUniform>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
       plan->launches++;
       f0 += nf;
     }
@@ -436,16 +453,23 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       a.f0 = f0;
-      if (code == kAnalyticDisc) launch_forward<kAnalyticDisc>(G, nf, n_sl, st, a, plan->ft);
-      else if (code == kStack16) launch_forward<kStack16>(G, nf, n_sl, st, a, plan->ft);
-      else if (code == kAnalyticFull) launch_forward<kAnalyticFull>(G, nf, n_sl, st, a, plan->ft);
-      else launch_forward<kUniform>(G, nf, n_sl, st, a, plan->ft);
+      if (code == kAnalyticDisc) launch_forward<kAnalyticDisc, false>(G, nf, n_sl, st, a, plan->ft);
+      else if (code == kStack16) launch_forward<kStack16, false>(G, nf, n_sl, st, a, plan->ft);
+      else if (code == kAnalyticFull) launch_forward<kAnalyticFull, false>(G, nf, n_sl, st, a, plan->ft);
+      else launch_forward<kUniform, false>(G, nf, n_sl, st, a, plan->ft);
       plan->launches++;
+      if (split_ok) {   // the same pass over list_u (exits at once unless the pilot chose the split mode)
+        if (code == kAnalyticDisc) launch_forward<kAnalyticDisc, true>(G, nf, n_sl, st, a, plan->ft);
+        else if (code == kStack16) launch_forward<kStack16, true>(G, nf, n_sl, st, a, plan->ft);
+        else if (code == kAnalyticFull) launch_forward<kAnalyticFull, true>(G, nf, n_sl, st, a, plan->ft);
+        else launch_forward<kUniform, true>(G, nf, n_sl, st, a, plan->ft);
+        plan->launches++;
+      }
       f0 += nf;
     }
     if (escalate) {
       run_f64(8, piloted ? 1 : 0, true);          // the flagged list, 8 lanes per sightline
-      if (piloted) run_f64(G, 2, false);          // or everything (exits at once unless the pilot chose it)
+      if (piloted) run_f64(G, 3, true);           // or the long list of the split mode / every sightline (all-float64)
     }
   } else {
     run_f64(G, 0, false);
@@ -453,6 +477,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   cudaError_t e = cudaGetLastError();
   cudaMemcpyAsync(plan->h_flag_count, ctrl, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
   if (escalate) cudaFreeAsync(a.flag_list, st);
+  if (a.list_u) cudaFreeAsync(a.list_u, st);
   cudaFreeAsync(bc, st);
   cudaFreeAsync(bd, st);
   if (e != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward launch failed: %s", cudaGetErrorString(e));

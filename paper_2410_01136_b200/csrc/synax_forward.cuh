@@ -275,23 +275,65 @@ struct ForwardArgs {
   int* flag_count;        // device counter
   int* flag_list;         // device list of flagged sightline ids (b * npix + p)
   ScalarGridDesc sg_ne, sg_n0;  // gridded n_e / N_0 replacing the analytic discs (DISC4, GRID_B), g == nullptr: unused
-  const int* mode;        // device: kModeFastThenList / kModeAllF64 (written by decide_kernel), or null
-  int run_when;           // forward_f64_kernel: 0 always, 1 only in list mode, 2 only in all-float64 mode
+  const int* mode;        // device: kModeFastThenList / kModeAllF64 / kModeSplit (written by decide_kernel), or null
+  int run_when;           // forward_f64_kernel: 0 always, 1 only in mode fast-then-list (flag list), 2 only in mode
+                          // all-float64 (every sightline), 3 in both all-float64 (every sightline) and split (flag list)
+  int* list_u;            // kModeSplit: sightlines classify_kernel left to the fp32 kernel (count in ctrl[kCtrlCountU])
+  const int* count_u;
 };
 
-enum { kModeFastThenList = 0, kModeAllF64 = 1 };
-enum { kCtrlFlagCount = 0, kCtrlPilotFlagged = 1, kCtrlMode = 2, kCtrlWords = 4 };
+// kModeSplit: classify_kernel sorts the sightlines by an estimate of the round-off scale into the flag list (float64
+// chain) and list_u (fp32 kernel, whose exact criterion still appends what the estimate missed to the flag list).
+enum { kModeFastThenList = 0, kModeAllF64 = 1, kModeSplit = 2 };
+enum { kCtrlFlagCount = 0, kCtrlPilotFlagged = 1, kCtrlMode = 2, kCtrlCountU = 3, kCtrlWords = 4 };
 
-template <int CODE, int G, int NF>
+// Estimate of one lane's share of the round-off scale  sum_n |n_e| (|B_LOS| + |B_N| + |B_E|)  over samples [n0, n1):
+// every 16th sample (all of them for short chunks), MUFU-grade fp32 chain; the caller sums the lanes of the
+// sightline and multiplies by Triad::scalef.
+template <int CODE>
+__device__ __forceinline__ float roundoff_scale_estimate(const Geometry& geo, const BatchConsts& P, const Triad& T,
+                                                         const ScalarGridDesc& sg_ne, int n0, int n1) {
+  const int step = (n1 - n0 >= 32) ? 16 : 1;
+  const double delta = geo.delta * T.scale;
+  float est = 0.f;
+  for (int n = n0 + step / 2; n < n1; n += step) {
+    const double s_e = ((double)n + 0.5) * delta;
+    const double xd = fma(s_e, T.nxd, geo.obs[0]), yd = fma(s_e, T.nyd, geo.obs[1]), zd = fma(s_e, T.nzd, geo.obs[2]);
+    SampleF S;
+    if (CODE == kUniform) {
+      S.Bpar = fabsf(P.uB[0]) + fabsf(P.uB[1]) + fabsf(P.uB[2]); S.BN = 0.f; S.BE = 0.f; S.ne = P.une;
+    } else {
+      const double rho2d = fma(xd, xd, yd * yd);
+      const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+      if (CODE == kStack16) {
+        StackAux sa;
+        eval_stack16_f32<true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, sa);
+      } else {
+        AnalyticAux aux;
+        eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+      }
+      if ((CODE == kAnalyticDisc || CODE == kStack16) && sg_ne.g) S.ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
+    }
+    est = fmaf(fabsf(S.ne), fabsf(S.Bpar) + fabsf(S.BN) + fabsf(S.BE), est);
+  }
+  return est * (float)step;
+}
+
+// LIST = false: every sightline, runs in kModeFastThenList (or without a pilot); LIST = true: the sightlines of
+// list_u, runs in kModeSplit.  (Two instantiations rather than a run-time switch: the switch put two more
+// F2F conversions per sample into the loop of the NF = 1 kernel, +4 % at cfg 2.)
+template <int CODE, int G, int NF, bool LIST>
 __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__ ForwardArgs A,
                                                          const __grid_constant__ FreqTab ft) {
-  if (A.mode && *A.mode == kModeAllF64) return;   // the pilot found mostly strong Faraday rotation
+  if (LIST ? (*A.mode != kModeSplit) : (A.mode && *A.mode != kModeFastThenList)) return;
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
   int64_t sl = tid / G;
-  const int64_t n_sl = A.geo.npix * A.batch;
+  const int64_t n_sl = LIST ? (int64_t)(*A.count_u) : A.geo.npix * A.batch;
+  if (LIST && sl - ((threadIdx.x & 31) / G) >= n_sl) return;   // the whole warp is past the end of the list
   const bool valid = sl < n_sl;
   if (!valid) sl = n_sl - 1;  // keep the lane alive for the shuffles
+  if (LIST) sl = (int64_t)A.list_u[sl];
   const int b = (int)(sl / A.geo.npix);
   const int64_t pix = sl - (int64_t)b * A.geo.npix;
   const BatchConsts& P = A.bc[b];
@@ -426,9 +468,10 @@ __global__ void __launch_bounds__(kBlock, SYNAX_F64_MINB) forward_f64_kernel(con
   const int g = (int)(tid % G);
   const int64_t n_groups = ((int64_t)gridDim.x * kBlock) / G;
   const int64_t n_sl = A.geo.npix * A.batch;
-  if (A.run_when == 1 && *A.mode == kModeAllF64) return;
+  if (A.run_when == 1 && *A.mode != kModeFastThenList) return;
   if (A.run_when == 2 && *A.mode != kModeAllF64) return;
-  const bool use_list = A.flag_list && A.run_when != 2;
+  if (A.run_when == 3 && *A.mode == kModeFastThenList) return;
+  const bool use_list = A.flag_list && (A.run_when == 3 ? *A.mode == kModeSplit : A.run_when != 2);
   const int64_t count = use_list ? (int64_t)(*A.flag_count) : n_sl;
   const int C = (A.geo.n_los + G - 1) / G;
   const int n0 = g * C;
@@ -604,9 +647,58 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
   if (lane == 0 && absS > A.flag_S) atomicAdd(ctrl + kCtrlPilotFlagged, 1);
 }
 
+// kModeSplit: one thread per sightline; sightlines whose estimated round-off scale exceeds flag_S go to the head of
+// the flag list (float64 chain), the others to list_u (fp32 kernel).  Block-ordered compaction: within a CTA the
+// sightlines keep their order (neighbouring pixels stay neighbours in the lists); the CTAs' segments land in the
+// order their atomics arrive -- the maps do not depend on it.
+template <int CODE>
+__global__ void __launch_bounds__(kBlock) classify_kernel(const __grid_constant__ ForwardArgs A, int* __restrict__ ctrl) {
+  if (ctrl[kCtrlMode] != kModeSplit) return;
+  __shared__ int w_cnt[2][kBlock / 32];
+  __shared__ int w_base[2][kBlock / 32];
+  const int64_t n_sl = A.geo.npix * A.batch;
+  for (int64_t chunk = blockIdx.x; chunk * kBlock < n_sl; chunk += gridDim.x) {   // block-uniform trip count
+  const int64_t sl = chunk * kBlock + threadIdx.x;
+  const bool valid = sl < n_sl;
+  bool flagged = false;
+  if (valid) {
+    const int b = (int)(sl / A.geo.npix);
+    const int64_t pix = sl - (int64_t)b * A.geo.npix;
+    const BatchConsts& P = A.bc[b];
+    const Triad T = load_triad(A.geo, pix);
+    flagged = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, 0, A.geo.n_los) * T.scalef > A.flag_S;
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned mf = __ballot_sync(0xffffffffu, valid && flagged), mu = __ballot_sync(0xffffffffu, valid && !flagged);
+  if (lane == 0) { w_cnt[0][warp] = __popc(mf); w_cnt[1][warp] = __popc(mu); }
+  __syncthreads();
+  if (threadIdx.x < 2) {
+    int tot = 0;
+    for (int w = 0; w < kBlock / 32; ++w) { w_base[threadIdx.x][w] = tot; tot += w_cnt[threadIdx.x][w]; }
+    const int base = tot ? atomicAdd(ctrl + (threadIdx.x == 0 ? kCtrlFlagCount : kCtrlCountU), tot) : 0;
+    for (int w = 0; w < kBlock / 32; ++w) w_base[threadIdx.x][w] += base;
+  }
+  __syncthreads();
+  if (valid) {
+    const unsigned below = (1u << lane) - 1u;
+    if (flagged) A.flag_list[w_base[0][warp] + __popc(mf & below)] = (int)sl;
+    else A.list_u[w_base[1][warp] + __popc(mu & below)] = (int)sl;
+  }
+  __syncthreads();
+  }
+}
+
+// Forward: the pilot's flagged share picks the mode -- below 1/50: fp32 pass + float64 redo of its flag list; above
+// 3/4: float64 chain for every sightline; in between: split by classify_kernel.  (cfg 4 @ 408 MHz, fp32 pass 7.2 ms,
+// float64 pass 11.1 ms: measured split 11.9 / 10.4 / 9.1 ms at 78 / 50 / 28 % flagged.)
+__global__ void decide_forward_kernel(int* __restrict__ ctrl, int64_t n_pilot) {
+  const int64_t f = ctrl[kCtrlPilotFlagged];
+  ctrl[kCtrlMode] = (50 * f <= n_pilot) ? kModeFastThenList : (4 * f > 3 * n_pilot) ? kModeAllF64 : kModeSplit;
+}
+
 __global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot, int num, int den) {
-  // forward (1/4): more than a quarter flagged -> redoing them after an fp32 pass costs more than one float64-chain
-  // pass.  adjoint (3/20): see analytic_vjp.
+  // short forward calls (1/4): more than a quarter flagged -> one float64-chain pass costs less than fp32 + redo.
+  // adjoint (0/1): any sampled sightline above half the threshold, see analytic_vjp.
   ctrl[kCtrlMode] = ((int64_t)den * ctrl[kCtrlPilotFlagged] > (int64_t)num * n_pilot) ? kModeAllF64 : kModeFastThenList;
 }
 

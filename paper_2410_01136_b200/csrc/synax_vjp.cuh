@@ -247,29 +247,8 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
 
   bool prec = PMODE == 1;
   if (PMODE == 2) {
-    const int step = (n1 - n0 >= 32) ? 16 : 1;
-    float est = 0.f;
-    for (int n = n0 + step / 2; n < n1; n += step) {
-      const double s_e = ((double)n + 0.5) * delta;
-      const double xd = fma(s_e, T.nxd, A.geo.obs[0]), yd = fma(s_e, T.nyd, A.geo.obs[1]), zd = fma(s_e, T.nzd, A.geo.obs[2]);
-      SampleF S;
-      if (CODE == kUniform) {
-        S.Bpar = fabsf(P.uB[0]) + fabsf(P.uB[1]) + fabsf(P.uB[2]); S.BN = 0.f; S.BE = 0.f; S.ne = P.une;
-      } else {
-        const double rho2d = fma(xd, xd, yd * yd);
-        const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
-        if (CODE == kStack16) {
-          StackAux sa;
-          eval_stack16_f32<true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, sa);
-        } else {
-          AnalyticAux aux;
-          eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
-        }
-        if ((CODE == kAnalyticDisc || CODE == kStack16) && A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
-      }
-      est = fmaf(fabsf(S.ne), fabsf(S.Bpar) + fabsf(S.BN) + fabsf(S.BE), est);
-    }
-    est = group_sum<G>(est) * (float)step * T.scalef;
+    float est = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, n0, n1);
+    est = group_sum<G>(est) * T.scalef;
     prec = est > A.flag_S;
   }
   const bool warp_prec = PMODE == 1 || (PMODE == 2 && __any_sync(0xffffffffu, prec));

@@ -264,6 +264,41 @@ def test_escalation_counts_and_strong_faraday_parity():
     parity.assert_maps_close(maps2, ref, what="cfg4@nside32 forward, float64 chain everywhere")
 
 
+@pytest.mark.parametrize("escalate_rad", [250.0, 300.0, 600.0])
+def test_forward_split_mode_sampled_pixels(escalate_rad):
+    """Calls of >= 262,144 sightlines with 2-75 % of them above the escalation threshold are split by
+    classify_kernel into one list per chain (fp32 kernel / float64-chain kernel).  cfg-4 model at 408 MHz + 1.4 GHz,
+    nside 256 x 256 samples; thresholds chosen so that the flagged share is between 1/5 and 2/3."""
+    import dataclasses
+    w = dataclasses.replace(wl.config(4), n_los=256, freqs=np.array([0.408e9, 1.4e9]))
+    maps, stats = parity.gpu_forward(w, escalate_rad=escalate_rad)
+    assert 0.02 * w.npix < stats["escalated"] < 0.9 * w.npix, stats
+    pix = _cfg4_sample_pixels(w)
+    ref = parity.oracle_forward(w, pix=pix)
+    parity.assert_maps_close(tuple(m[..., pix] for m in maps), ref, what=f"split forward, escalate_rad={escalate_rad}")
+    assert all(np.all(np.isfinite(m)) for m in maps)
+    # every sightline is written by the right kernel whichever list it went to: over the WHOLE map the result stays
+    # within the bound of the float64 chain everywhere (the fp32 sightlines' error grows with the threshold:
+    # measured 2.4e-5 at 300 rad, 2.3e-4 at 1000 rad; the default is 100 rad)
+    maps2, _ = parity.gpu_forward(w, precision=2)
+    for a, b in zip(maps, maps2):
+        rms = np.sqrt(np.mean(b ** 2, axis=-1, keepdims=True))
+        assert np.max(np.abs(a - b) / rms) < parity.MAP_TOL * max(1.0, escalate_rad / 300.0)
+
+
+def test_forward_split_mode_batched():
+    """Split mode across batch elements (sightline id = b * npix + pix): FULL16 draws at 408 MHz, nside 64 x 6."""
+    import dataclasses
+    w2 = wl.config(2)
+    w = dataclasses.replace(w2, nside=64, n_los=256, freqs=np.array([0.408e9]), params=w2.params[:6].copy())
+    maps, stats = parity.gpu_forward(w, escalate_rad=300.0)
+    n_sl = w.npix * 6
+    assert n_sl >= 262144 and 0.02 * n_sl < stats["escalated"] < 0.9 * n_sl, stats
+    pix = np.arange(3, w.npix, 16)
+    ref = parity.oracle_forward(w, pix=pix)
+    parity.assert_maps_close(tuple(m[..., pix] for m in maps), ref, what="split forward, batch 6")
+
+
 def test_pixel_shards_match_full_plan():
     """synax_plan_create_shard: three contiguous RING ranges reproduce the full-sky maps bit for bit (same lanes per
     sightline) and their partial gradients sum to the full gradient."""
