@@ -308,11 +308,11 @@ template <int CODE, int G>
 static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
-    case 1: forward_f64_kernel<CODE, G, 1><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 2: forward_f64_kernel<CODE, G, 2><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 3: forward_f64_kernel<CODE, G, 3><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 4: forward_f64_kernel<CODE, G, 4><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    default: forward_f64_kernel<CODE, G, 8><<<blocks, kBlock, 0, st>>>(a, ft); break;
+    case 1: forward_f64_kernel<CODE, G, 1><<<blocks, kBlockD, 0, st>>>(a, ft); break;
+    case 2: forward_f64_kernel<CODE, G, 2><<<blocks, kBlockD, 0, st>>>(a, ft); break;
+    case 3: forward_f64_kernel<CODE, G, 3><<<blocks, kBlockD, 0, st>>>(a, ft); break;
+    case 4: forward_f64_kernel<CODE, G, 4><<<blocks, kBlockD, 0, st>>>(a, ft); break;
+    default: forward_f64_kernel<CODE, G, 8><<<blocks, kBlockD, 0, st>>>(a, ft); break;
   }
 }
 template <int CODE>
@@ -417,7 +417,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
         else classify_kernel<kUniform><<<cb, kBlock, 0, st>>>(a, ctrl);
         plan->launches += 3;
       } else {
-        decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 1, 4);   // more than a quarter flagged: all-float64
+        decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 1, 4, kModeAllF64);   // more than a quarter flagged: all-float64
         plan->launches += 2;
       }
       a.mode = ctrl + kCtrlMode;
@@ -431,8 +431,8 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   // Split mode: the list is long (2-85 % of the sightlines), so it takes the lane count of the full pass and a grid
   // sized for all sightlines (CTAs past the list's end exit at once).
   auto blocks_for = [&](int lanes, bool use_list, int run_when) {
-    const int64_t full = (n_sl * lanes + kBlock - 1) / kBlock;
-    return (unsigned)(use_list && run_when != 3 ? std::min<int64_t>(full, (int64_t)sms * 16) : full);
+    const int64_t full = (n_sl * lanes + kBlockD - 1) / kBlockD;
+    return (unsigned)(use_list && run_when != 3 ? std::min<int64_t>(full, (int64_t)sms * 16 * 128 / kBlockD) : full);
   };
   auto run_f64 = [&](int lanes, int run_when, bool use_list) {
     ForwardArgs pa = a;

@@ -461,12 +461,16 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 #ifndef SYNAX_F64_MINB
 #define SYNAX_F64_MINB 4
 #endif
+#ifndef SYNAX_F64_BLOCK
+#define SYNAX_F64_BLOCK 128
+#endif
+constexpr int kBlockD = SYNAX_F64_BLOCK;   // threads per CTA of the float64-chain forward
 template <int CODE, int G, int NF>
-__global__ void __launch_bounds__(kBlock, SYNAX_F64_MINB) forward_f64_kernel(const __grid_constant__ ForwardArgs A,
+__global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(const __grid_constant__ ForwardArgs A,
                                                              const __grid_constant__ FreqTab ft) {
-  const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const int64_t tid = (int64_t)blockIdx.x * kBlockD + threadIdx.x;
   const int g = (int)(tid % G);
-  const int64_t n_groups = ((int64_t)gridDim.x * kBlock) / G;
+  const int64_t n_groups = ((int64_t)gridDim.x * kBlockD) / G;
   const int64_t n_sl = A.geo.npix * A.batch;
   if (A.run_when == 1 && *A.mode != kModeFastThenList) return;
   if (A.run_when == 2 && *A.mode != kModeAllF64) return;
@@ -696,10 +700,10 @@ __global__ void decide_forward_kernel(int* __restrict__ ctrl, int64_t n_pilot) {
   ctrl[kCtrlMode] = (50 * f <= n_pilot) ? kModeFastThenList : (4 * f > 3 * n_pilot) ? kModeAllF64 : kModeSplit;
 }
 
-__global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot, int num, int den) {
+__global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot, int num, int den, int mode_yes) {
   // short forward calls (1/4): more than a quarter flagged -> one float64-chain pass costs less than fp32 + redo.
   // adjoint (0/1): any sampled sightline above half the threshold, see analytic_vjp.
-  ctrl[kCtrlMode] = ((int64_t)den * ctrl[kCtrlPilotFlagged] > (int64_t)num * n_pilot) ? kModeAllF64 : kModeFastThenList;
+  ctrl[kCtrlMode] = ((int64_t)den * ctrl[kCtrlPilotFlagged] > (int64_t)num * n_pilot) ? mode_yes : kModeFastThenList;
 }
 
 }  // namespace synax

@@ -185,7 +185,10 @@ struct VjpArgs {
   const BatchConstsD* bd;   // float64 constants (float64 Faraday chain variant)
   float flag_S;     // PMODE 2: sightlines whose round-off scale exceeds this take the float64 chain
   const int* mode;  // auto: device word from decide_kernel -- kModeAllF64 = "some sightline is near the threshold: run the
-                    // per-sightline variant (PMODE 2)", else the lean fp32 variant (PMODE 0) runs; the other exits; or null
+                    // per-sightline variant (PMODE 2)", kModeSplit = "... run the per-CTA pair (cta_sel)", else the lean
+                    // fp32 variant (PMODE 0) runs; the variants the word does not name exit; or null
+  const unsigned char* cta_sel;   // kModeSplit: [batch][n_blocks] from vjp_classify_kernel, 1 = some sightline of this CTA
+                    // is above the threshold -> the CTA is done by the PMODE 1 launch, 0 -> by the PMODE 0 launch; or null
   const float* dI; const float* dQ; const float* dU;   // may be null
   ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
   float* partial;   // [batch][n_blocks][16]
@@ -230,8 +233,16 @@ __device__ __forceinline__ double faraday_term_d(const BatchConsts& P, const Bat
 template <int CODE, int G, int NF, int PMODE>
 __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
   constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
-  if (A.mode && ((*A.mode == kModeAllF64) != (PMODE == 2))) return;
+  if (A.mode) {
+    const int m = *A.mode;
+    if (A.cta_sel ? (m != kModeSplit) : (m == kModeSplit || (m == kModeAllF64) != (PMODE == 2))) return;
+  }
   const int b = A.b0 + blockIdx.y;
+  if (A.cta_sel && (A.cta_sel[(size_t)b * A.n_blocks + blockIdx.x] != 0) != (PMODE == 1)) {
+    // the other launch of the pair does this CTA; the first launch of the pair defines every partial
+    if (!A.accumulate && threadIdx.x < 16) A.partial[((size_t)b * A.n_blocks + blockIdx.x) * 16 + threadIdx.x] = 0.f;
+    return;
+  }
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
   int64_t pix = tid / G;
@@ -461,6 +472,27 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   }
 }
 
+// kModeSplit (G = 1, long calls): one thread per sightline estimates its round-off scale exactly as PMODE 2 does; a
+// CTA with any sightline above the threshold is handed to the PMODE 1 launch (float64 Faraday angles for its 128
+// sightlines), the others to the lean PMODE 0 launch.  The thread <-> sightline mapping, and so the order of every
+// sum, is the one of a full launch: the gradient stays deterministic.  (In RING order the strongly rotating
+// sightlines -- low latitudes towards the inner Galaxy -- are contiguous runs, so CTA granularity loses little.)
+template <int CODE>
+__global__ void __launch_bounds__(kBlock) vjp_classify_kernel(const __grid_constant__ VjpArgs A,
+                                                              unsigned char* __restrict__ cta_sel) {
+  if (*A.mode != kModeSplit) return;
+  const int b = A.b0 + blockIdx.y;
+  const int64_t pix = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  bool prec = false;
+  if (pix < A.geo.npix) {
+    const BatchConsts& P = A.bc[b];
+    const Triad T = load_triad(A.geo, pix);
+    prec = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, 0, A.geo.n_los) * T.scalef > A.flag_S;
+  }
+  const int any = __syncthreads_or(prec ? 1 : 0);
+  if (threadIdx.x == 0) cta_sel[(size_t)b * A.n_blocks + blockIdx.x] = any ? 1 : 0;
+}
+
 // partial[b][n_blocks][16] -> grad[b][n_params], float64 accumulation, deterministic order
 __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_blocks, int n_params, float* __restrict__ grad) {
   const int b = blockIdx.x;
@@ -522,7 +554,11 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   float k_max = 0.f;
   for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
   a.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
-  a.mode = nullptr;
+  a.mode = nullptr; a.cta_sel = nullptr;
+  // Long calls with one thread per sightline: the work is split per CTA between the lean fp32 variant and the
+  // float64-angle variant (vjp_classify_kernel) instead of deciding per sightline inside one heavier kernel
+  // (cfg 4, 9 % of the sightlines above the threshold: 14.3 -> see DESIGN.md section 5).
+  const bool split = precision == 0 && G == 1 && geo.npix * batch >= 262144;
   if (precision == 0) {
     ForwardArgs pa;
     pa.geo = geo; pa.bc = bc; pa.bd = bd; pa.batch = batch; pa.sg_ne = sg_ne; pa.sg_n0 = sg_n0;
@@ -536,10 +572,14 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
     else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
     else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
     else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(pa, stride, n_pilot, ctrl);
-    decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 0, 1);   // any sampled sightline above half the threshold
+    // any sampled sightline above half the threshold: per-sightline variant, or (long calls) the per-CTA pair
+    decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 0, 1, split ? kModeSplit : kModeAllF64);
     *launches += 2;
     a.mode = ctrl + kCtrlMode;
   }
+  unsigned char* cta_sel = nullptr;
+  if (split && cudaMallocAsync((void**)&cta_sel, (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
+    return SYNAX_ERR_ALLOC;
   float* partial = nullptr;
   if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
     return SYNAX_ERR_ALLOC;
@@ -547,6 +587,13 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   for (int b0 = 0; b0 < batch; b0 += 65535) {   // gridDim.y limit
     const dim3 grid((unsigned)a.n_blocks, (unsigned)std::min(65535, batch - b0));
     a.b0 = b0;
+    if (split) {
+      if (code == kAnalyticDisc) vjp_classify_kernel<kAnalyticDisc><<<grid, kBlock, 0, st>>>(a, cta_sel);
+      else if (code == kStack16) vjp_classify_kernel<kStack16><<<grid, kBlock, 0, st>>>(a, cta_sel);
+      else if (code == kAnalyticFull) vjp_classify_kernel<kAnalyticFull><<<grid, kBlock, 0, st>>>(a, cta_sel);
+      else vjp_classify_kernel<kUniform><<<grid, kBlock, 0, st>>>(a, cta_sel);
+      ++*launches;
+    }
     for (int f0 = 0; f0 < ft.n_freq;) {
       const int rem = ft.n_freq - f0;
       const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
@@ -555,7 +602,16 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       else if (precision == 2) launch_vjp_code<1>(code, G, nf, grid, st, a, ft);
       else {
         launch_vjp_code<0>(code, G, nf, grid, st, a, ft);
-        launch_vjp_code<2>(code, G, nf, grid, st, a, ft);
+        if (split) {   // the per-CTA pair (runs in kModeSplit): PMODE 0 first -- it defines every partial -- then PMODE 1
+          VjpArgs as = a;
+          as.cta_sel = cta_sel;
+          launch_vjp_code<0>(code, G, nf, grid, st, as, ft);
+          as.accumulate = 1;
+          launch_vjp_code<1>(code, G, nf, grid, st, as, ft);
+          ++*launches;
+        } else {
+          launch_vjp_code<2>(code, G, nf, grid, st, a, ft);
+        }
         ++*launches;
       }
       ++*launches;
@@ -566,6 +622,7 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   ++*launches;
   const cudaError_t e = cudaGetLastError();
   cudaFreeAsync(partial, st);
+  if (cta_sel) cudaFreeAsync(cta_sel, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 

@@ -396,3 +396,31 @@ def test_vjp_strong_rotation_uses_float64_angles(ne_scale):
     ref = parity.oracle_vjp(w, cots)
     _check_grad(parity.gpu_vjp(w, cots), ref, f"vjp n_e x{ne_scale} (auto)")
     _check_grad(parity.gpu_vjp(w, cots, precision=2), ref, f"vjp n_e x{ne_scale} (float64 angles)")
+
+
+@pytest.mark.parametrize("batch", [1, 2])
+def test_vjp_per_cta_split_frequency_blocks_and_batch(batch):
+    """Long calls (>= 262,144 sightlines, one thread each) with strong rotation split the adjoint per CTA between
+    the lean fp32 variant and the float64-angle variant (vjp_classify_kernel).  13 frequencies = blocks of 8 + 4 + 1
+    (the pair accumulates into the partials of the first block); batch 2 = two rows of cta_sel.  Sparse cotangent as
+    in test_cfg4_full_size_vjp_sparse_cotangent, oracle over those pixels."""
+    w4 = wl.config(4)
+    params = np.repeat(w4.params, batch, axis=0).copy()
+    if batch > 1:
+        params[1, 0] *= 1.1    # B0
+        params[1, 13] *= 1.5   # n_e0: more sightlines above the threshold than in row 0
+    nside = 256 if batch == 1 else 128
+    w = wl.Workload("cfg4_split", w4.kind, nside, 128, w4.s_max, np.geomspace(0.408e9, 30e9, 13), params, w4.aux,
+                    cot_seed=2104)
+    pix = np.arange(3, w.npix, 96)
+    full = w.cotangents()
+    cots = tuple(np.zeros_like(c) for c in full)
+    for c, f in zip(cots, full):
+        c[..., pix] = f[..., pix]
+    ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots), pix=pix)
+    g = parity.gpu_vjp(w, cots)
+    _check_grad(g, ref, f"vjp per-CTA split, 13 frequencies, batch {batch}")
+    # same call twice: the split keeps the thread <-> sightline mapping, so the gradient is bit-reproducible
+    assert np.array_equal(g, parity.gpu_vjp(w, cots))
+    # and the float64-angle variant everywhere agrees within the bound as well
+    _check_grad(parity.gpu_vjp(w, cots, precision=2), ref, "vjp float64 angles everywhere")
