@@ -51,6 +51,8 @@ struct synax_plan {
   int* d_vjp_ctrl;    // device control block of the adjoint's pilot (kCtrlWords ints)
   int* d_flag_count;  // device control block, kCtrlWords ints: [flag count, pilot flagged, mode, -]
   int* h_flag_count;  // pinned host mirror (last forward)
+  cudaStream_t aux;   // second stream for the float64-angle member of the adjoint's per-CTA pair (fork / join by events)
+  cudaEvent_t ev_fork, ev_join;
   mutable int64_t launches;
   mutable int64_t last_n_sl;  // sightlines of the last forward (for stats when every one took the float64 chain)
 };
@@ -120,6 +122,9 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, kCtrlWords * sizeof(int));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_vjp_ctrl, kCtrlWords * sizeof(int));
   if (e == cudaSuccess) e = cudaMallocHost((void**)&p->h_flag_count, kCtrlWords * sizeof(int));
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->aux, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
   if (e == cudaSuccess) {
     for (int i = 0; i < kCtrlWords; ++i) p->h_flag_count[i] = 0;
     e = cudaMemset(p->d_flag_count, 0, kCtrlWords * sizeof(int));
@@ -137,6 +142,9 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
     if (p->d_flag_count) cudaFree(p->d_flag_count);
     if (p->d_vjp_ctrl) cudaFree(p->d_vjp_ctrl);
     if (p->h_flag_count) cudaFreeHost(p->h_flag_count);
+    if (p->aux) cudaStreamDestroy(p->aux);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     delete p;
     return st;
   }
@@ -151,6 +159,9 @@ extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
   cudaFree(plan->d_flag_count);
   cudaFree(plan->d_vjp_ctrl);
   cudaFreeHost(plan->h_flag_count);
+  cudaStreamDestroy(plan->aux);
+  cudaEventDestroy(plan->ev_fork);
+  cudaEventDestroy(plan->ev_join);
   delete plan;
   return SYNAX_OK;
 }
@@ -508,7 +519,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
-                      plan->d_vjp_ctrl,
+                      plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
                       dI, dQ, dU, grad, st, &plan->launches);
   cudaFreeAsync(bc, st);
   if (bd) cudaFreeAsync(bd, st);

@@ -238,11 +238,8 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
     if (A.cta_sel ? (m != kModeSplit) : (m == kModeSplit || (m == kModeAllF64) != (PMODE == 2))) return;
   }
   const int b = A.b0 + blockIdx.y;
-  if (A.cta_sel && (A.cta_sel[(size_t)b * A.n_blocks + blockIdx.x] != 0) != (PMODE == 1)) {
-    // the other launch of the pair does this CTA; the first launch of the pair defines every partial
-    if (!A.accumulate && threadIdx.x < 16) A.partial[((size_t)b * A.n_blocks + blockIdx.x) * 16 + threadIdx.x] = 0.f;
-    return;
-  }
+  // the other launch of the pair does this CTA (and owns its partial: the two launches run concurrently)
+  if (A.cta_sel && (A.cta_sel[(size_t)b * A.n_blocks + blockIdx.x] != 0) != (PMODE == 1)) return;
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
   int64_t pix = tid / G;
@@ -545,6 +542,7 @@ constexpr double kVjpEscalateFactor = 10.0;
 static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                                  const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
                                  const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int* ctrl,
+                                 cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
                                  const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
                                  int64_t* launches) {
   VjpArgs a;
@@ -593,6 +591,7 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       else if (code == kAnalyticFull) vjp_classify_kernel<kAnalyticFull><<<grid, kBlock, 0, st>>>(a, cta_sel);
       else vjp_classify_kernel<kUniform><<<grid, kBlock, 0, st>>>(a, cta_sel);
       ++*launches;
+      if (cudaEventRecord(ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(aux, ev_fork, 0) != cudaSuccess) return SYNAX_ERR_CUDA;
     }
     for (int f0 = 0; f0 < ft.n_freq;) {
       const int rem = ft.n_freq - f0;
@@ -602,12 +601,14 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       else if (precision == 2) launch_vjp_code<1>(code, G, nf, grid, st, a, ft);
       else {
         launch_vjp_code<0>(code, G, nf, grid, st, a, ft);
-        if (split) {   // the per-CTA pair (runs in kModeSplit): PMODE 0 first -- it defines every partial -- then PMODE 1
+        if (split) {
+          // the per-CTA pair (runs in kModeSplit).  Every CTA's partial belongs to exactly one member, so the two run
+          // concurrently: the float64-angle member (few, long CTAs: 2.7 waves at cfg 4) on the plan's second stream,
+          // forked after the classify kernel and joined before the reduction, fills its tail with the other's CTAs.
           VjpArgs as = a;
           as.cta_sel = cta_sel;
+          launch_vjp_code<1>(code, G, nf, grid, aux, as, ft);
           launch_vjp_code<0>(code, G, nf, grid, st, as, ft);
-          as.accumulate = 1;
-          launch_vjp_code<1>(code, G, nf, grid, st, as, ft);
           ++*launches;
         } else {
           launch_vjp_code<2>(code, G, nf, grid, st, a, ft);
@@ -617,6 +618,8 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       ++*launches;
       f0 += nf;
     }
+    if (split && (cudaEventRecord(ev_join, aux) != cudaSuccess || cudaStreamWaitEvent(st, ev_join, 0) != cudaSuccess))
+      return SYNAX_ERR_CUDA;
   }
   vjp_reduce_kernel<<<batch, 256, 0, st>>>(partial, a.n_blocks, n_params, grad);
   ++*launches;

@@ -135,3 +135,36 @@ def test_forward_and_vjp_are_cuda_graph_capturable():
     torch.cuda.synchronize()
     assert all(torch.equal(a, b) for a, b in zip(out, eager))
     plan.close()
+
+
+@pytest.mark.gpu
+def test_adjoint_pair_on_two_streams_is_graph_capturable_and_ordered():
+    """Long calls run the adjoint's per-CTA pair on two streams (fork after vjp_classify_kernel, join before the
+    reduction).  The fork / join must be capturable in a CUDA graph and ordered with the caller's stream: the
+    gradient read right after the call on the caller's stream is complete and bit-identical on replay."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w4 = wl.config(4)
+    w = wl.Workload("cfg4_pair", w4.kind, 256, 64, w4.s_max, w4.freqs, w4.params, w4.aux, cot_seed=2104)
+    plan, model, params = parity.gpu_objects(w)
+    cots = [torch.from_numpy(c).cuda() for c in w.cotangents()]
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g = sx.vjp(plan, model, params, *cots)
+        g_host = g.cpu()                                         # stream-ordered read right behind the call
+        sx.vjp(plan, model, params, *cots, out=g)
+    s.synchronize()
+    assert torch.equal(g.cpu(), g_host) and bool(torch.isfinite(g_host).all())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        sx.vjp(plan, model, params, *cots, out=g)
+    g.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(g.cpu(), g_host)
+    plan.set_option("precision", 2)                               # float64 angles everywhere: within the bound of it
+    gp = sx.vjp(plan, model, params, *cots)
+    torch.cuda.synchronize()
+    rel = ((gp.cpu() - g_host).abs() / gp.cpu().abs()).max().item()
+    assert rel <= 1e-3, rel
+    plan.close()
