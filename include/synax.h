@@ -124,7 +124,11 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
 /* VJP.  dI, dQ, dU: DEVICE fp32 [batch][n_freq][npix] cotangents (any may be NULL = zeros).
  * grad: DEVICE fp32 [batch][n_params] (GRID_B: [nx][ny][nz][3]); overwritten:
  * grad[b][j] = sum_{f,p} dI dI/dtheta_j + dQ dQ/dtheta_j + dU dU/dtheta_j.
- * DISC4 / GRID_B: `aux` values are constants (not differentiated). */
+ * DISC4 / GRID_B: `aux` values are constants (not differentiated).
+ * Ordering: all work is ordered with `cuda_stream` (results are complete when the stream reaches the end of the
+ * call).  Long calls (>= 262,144 sightlines) may run part of their kernels on a second stream owned by the plan,
+ * forked from and joined back to `cuda_stream` by events inside the call (CUDA-graph capturable); a plan must
+ * therefore not be used by two calls that run concurrently -- use one plan per stream. */
 synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,
                        int32_t batch, const float* dI, const float* dQ, const float* dU, float* grad,
                        void* cuda_stream);
