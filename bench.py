@@ -400,7 +400,10 @@ def run_ours(args):
             "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,
             "sample_freq_per_s": total * w.n_freq / t_step,
             "e2e": {"value": total / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
-                    "ms_per_step": 1e3 * t_e2e},
+                    "ms_per_step": 1e3 * t_e2e,
+                    "note": "synax_forward_host + synax_vjp_host on page-locked host buffers: parameters and cotangents "
+                            "copied host -> device inside the call, gradient copied back, the I/Q/U maps stored by the "
+                            "forward kernel straight into the host buffers (d2h bytes = the bytes that land there)"},
             "e2e_loglike": None if "t_fused" not in e else {
                 "value": total / e["t_fused"], "unit": UNIT, "ms_per_step": 1e3 * e["t_fused"],
                 "h2d_bytes_per_step": e["fused_h2d"], "d2h_bytes_per_step": e["fused_d2h"],

@@ -134,7 +134,10 @@ synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const f
                        void* cuda_stream);
 
 /* Same operations with HOST buffers of the same shapes: the call copies the inputs to the device,
- * runs, copies the results back and synchronises the stream before returning. */
+ * runs, copies the results back and synchronises the stream before returning.  When I, Q and U are all page-locked
+ * (cudaHostAlloc / cudaHostRegister) the forward kernels store the maps straight into them and no copy is made.
+ * Scratch comes from the device's default stream-ordered memory pool, whose release threshold the first plan raises
+ * to 4 GB (unless the application has set a larger one) so that it is not re-mapped at every call. */
 synax_status synax_forward_host(const synax_plan* plan, const synax_model* model, const float* params,
                                 int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
 synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, const float* params,

@@ -344,6 +344,26 @@ def test_host_entry_points_match_device_entry_points():
     plan.close()
 
 
+@pytest.mark.parametrize("cfg", [1, 3, 4])
+def test_forward_host_into_page_locked_buffers(cfg):
+    """synax_forward_host stores straight into page-locked map buffers (no staging copy): same bits as the device
+    entry point, for the fp32 pass + float64 redo of flagged sightlines (cfg 1: a sightline is written twice), the
+    gridded kernel (cfg 3) and the float64-chain kernel with 8 frequencies (cfg 4 scaled)."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = {1: lambda: wl.config(1), 3: lambda: wl.config(3).scaled(nside=16, n_los=256),
+         4: lambda: wl.config(4).scaled(nside=32, n_los=256)}[cfg]()
+    plan, model, params = parity.gpu_objects(w)
+    dev = sx.forward(plan, model, params)
+    torch.cuda.synchronize()
+    pinned = tuple(torch.full((w.batch, w.n_freq, w.npix), float("nan"), dtype=torch.float32).pin_memory() for _ in range(3))
+    out = tuple(t.numpy() for t in pinned)
+    sx.forward_host(plan, model, w.params, out=out)
+    for a, b in zip(dev, pinned):
+        assert torch.equal(a.cpu(), b)
+    plan.close()
+
+
 def test_gpu_invariants():
     """SURVEY C-3 #4 on the GPU path: P <= Pi I; I ~ N0 (linear); joint sign flip (B, n_e) -> (-B, -n_e)."""
     w = wl.config(4).scaled(nside=8, n_los=256)
