@@ -30,3 +30,32 @@ def test_random_full16_forward_and_vjp(seed):
     th = w.params[0].astype(np.float64)
     lg, lref = g * th, ref * th
     assert np.all(np.abs(lg - lref) <= 1e-3 * np.abs(lref) + 1e-5 * np.abs(lref).max()), (seed, np.abs(lg - lref) / np.abs(lref))
+
+
+def _draw_large(seed):
+    """As _draw, at nside 256 (786,432 sightlines: the long-call strategies -- forward split lists, adjoint per-CTA pair
+    on two streams) with few samples per sightline, low frequencies drawn more often."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    p = wl.FULL16_NOMINAL * np.exp(rng.uniform(-np.log(1.5), np.log(1.5), 16))
+    p[12] = rng.uniform(2.4, 3.4)
+    p[[0, 5]] *= rng.choice([-1.0, 1.0], 2)
+    freqs = np.sort(np.exp(rng.uniform(np.log(0.3e9), np.log(5e9), int(rng.integers(1, 11)))))
+    return wl.Workload(f"fuzzL{seed}", "full16", 256, int(rng.integers(48, 160)), float(rng.uniform(15.0, 35.0)), freqs,
+                       p[None, :].astype(np.float32), None, cot_seed=seed)
+
+
+@pytest.mark.parametrize("seed", range(4100, 4106))
+def test_random_full16_long_calls_sampled_pixels(seed):
+    w = _draw_large(seed)
+    pix = np.arange(seed % 89, w.npix, 89)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(tuple(m[..., pix] for m in maps), parity.oracle_forward(w, pix=pix), what=w.name)
+    full = w.cotangents()
+    cots = tuple(np.zeros_like(c) for c in full)
+    for c, f in zip(cots, full):
+        c[..., pix] = f[..., pix]
+    g = parity.gpu_vjp(w, cots)[0]
+    ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots), pix=pix)[0]
+    th = w.params[0].astype(np.float64)
+    lg, lref = g * th, ref * th
+    assert np.all(np.abs(lg - lref) <= 1e-3 * np.abs(lref) + 1e-5 * np.abs(lref).max()), (seed, np.abs(lg - lref) / np.abs(lref))
