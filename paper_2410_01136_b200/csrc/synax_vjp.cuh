@@ -469,25 +469,35 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   }
 }
 
-// kModeSplit (G = 1, long calls): one thread per sightline estimates its round-off scale exactly as PMODE 2 does; a
-// CTA with any sightline above the threshold is handed to the PMODE 1 launch (float64 Faraday angles for its 128
+// kModeSplit (long calls): the G lanes of a sightline estimate its round-off scale exactly as PMODE 2 does; a
+// CTA with any sightline above the threshold is handed to the PMODE 1 launch (float64 Faraday angles for its 128 / G
 // sightlines), the others to the lean PMODE 0 launch.  The thread <-> sightline mapping, and so the order of every
 // sum, is the one of a full launch: the gradient stays deterministic.  (In RING order the strongly rotating
 // sightlines -- low latitudes towards the inner Galaxy -- are contiguous runs, so CTA granularity loses little.)
-template <int CODE>
+template <int CODE, int G>
 __global__ void __launch_bounds__(kBlock) vjp_classify_kernel(const __grid_constant__ VjpArgs A,
                                                               unsigned char* __restrict__ cta_sel) {
   if (*A.mode != kModeSplit) return;
   const int b = A.b0 + blockIdx.y;
-  const int64_t pix = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-  bool prec = false;
-  if (pix < A.geo.npix) {
-    const BatchConsts& P = A.bc[b];
-    const Triad T = load_triad(A.geo, pix);
-    prec = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, 0, A.geo.n_los) * T.scalef > A.flag_S;
-  }
-  const int any = __syncthreads_or(prec ? 1 : 0);
+  const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const int g = (int)(tid % G);
+  int64_t pix = tid / G;
+  const bool valid = pix < A.geo.npix;
+  if (!valid) pix = A.geo.npix - 1;   // keep the lane alive for the shuffles
+  const BatchConsts& P = A.bc[b];
+  const Triad T = load_triad(A.geo, pix);
+  const int C = (A.geo.n_los + G - 1) / G;
+  const int n0 = g * C, n1 = min(n0 + C, A.geo.n_los);
+  float est = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, n0, n1);   // as PMODE 2 does, lane by lane
+  est = group_sum<G>(est) * T.scalef;
+  const int any = __syncthreads_or((valid && est > A.flag_S) ? 1 : 0);
   if (threadIdx.x == 0) cta_sel[(size_t)b * A.n_blocks + blockIdx.x] = any ? 1 : 0;
+}
+template <int CODE>
+static void launch_vjp_classify(int G, dim3 grid, cudaStream_t st, const VjpArgs& a, unsigned char* cta_sel) {
+  if (G == 1) vjp_classify_kernel<CODE, 1><<<grid, kBlock, 0, st>>>(a, cta_sel);
+  else if (G == 8) vjp_classify_kernel<CODE, 8><<<grid, kBlock, 0, st>>>(a, cta_sel);
+  else vjp_classify_kernel<CODE, 32><<<grid, kBlock, 0, st>>>(a, cta_sel);
 }
 
 // partial[b][n_blocks][16] -> grad[b][n_params], float64 accumulation, deterministic order
@@ -556,7 +566,8 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   // Long calls with one thread per sightline: the work is split per CTA between the lean fp32 variant and the
   // float64-angle variant (vjp_classify_kernel) instead of deciding per sightline inside one heavier kernel
   // (cfg 4, 9 % of the sightlines above the threshold: 14.3 -> see DESIGN.md section 5).
-  const bool split = precision == 0 && G == 1 && geo.npix * batch >= 262144;
+  // (G lanes per sightline, G > 1: a CTA holds 128 / G sightlines; worth its three extra launches from ~1M threads)
+  const bool split = precision == 0 && (G == 1 ? geo.npix * batch >= 262144 : geo.npix * batch * G >= 1000000);
   if (precision == 0) {
     ForwardArgs pa;
     pa.geo = geo; pa.bc = bc; pa.bd = bd; pa.batch = batch; pa.sg_ne = sg_ne; pa.sg_n0 = sg_n0;
@@ -586,10 +597,10 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
     const dim3 grid((unsigned)a.n_blocks, (unsigned)std::min(65535, batch - b0));
     a.b0 = b0;
     if (split) {
-      if (code == kAnalyticDisc) vjp_classify_kernel<kAnalyticDisc><<<grid, kBlock, 0, st>>>(a, cta_sel);
-      else if (code == kStack16) vjp_classify_kernel<kStack16><<<grid, kBlock, 0, st>>>(a, cta_sel);
-      else if (code == kAnalyticFull) vjp_classify_kernel<kAnalyticFull><<<grid, kBlock, 0, st>>>(a, cta_sel);
-      else vjp_classify_kernel<kUniform><<<grid, kBlock, 0, st>>>(a, cta_sel);
+      if (code == kAnalyticDisc) launch_vjp_classify<kAnalyticDisc>(G, grid, st, a, cta_sel);
+      else if (code == kStack16) launch_vjp_classify<kStack16>(G, grid, st, a, cta_sel);
+      else if (code == kAnalyticFull) launch_vjp_classify<kAnalyticFull>(G, grid, st, a, cta_sel);
+      else launch_vjp_classify<kUniform>(G, grid, st, a, cta_sel);
       ++*launches;
       if (cudaEventRecord(ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(aux, ev_fork, 0) != cudaSuccess) return SYNAX_ERR_CUDA;
     }

@@ -418,8 +418,8 @@ def test_vjp_strong_rotation_uses_float64_angles(ne_scale):
     _check_grad(parity.gpu_vjp(w, cots, precision=2), ref, f"vjp n_e x{ne_scale} (float64 angles)")
 
 
-@pytest.mark.parametrize("batch", [1, 2])
-def test_vjp_per_cta_split_frequency_blocks_and_batch(batch):
+@pytest.mark.parametrize("batch,nside", [(1, 256), (2, 128), (1, 128)])
+def test_vjp_per_cta_split_frequency_blocks_and_batch(batch, nside):
     """Long calls (>= 262,144 sightlines, one thread each) with strong rotation split the adjoint per CTA between
     the lean fp32 variant and the float64-angle variant (vjp_classify_kernel).  13 frequencies = blocks of 8 + 4 + 1
     (the pair accumulates into the partials of the first block); batch 2 = two rows of cta_sel.  Sparse cotangent as
@@ -429,7 +429,7 @@ def test_vjp_per_cta_split_frequency_blocks_and_batch(batch):
     if batch > 1:
         params[1, 0] *= 1.1    # B0
         params[1, 13] *= 1.5   # n_e0: more sightlines above the threshold than in row 0
-    nside = 256 if batch == 1 else 128
+    # (1, 128): 196,608 sightlines with 8 lanes each (1.57 M threads): the split with 16 sightlines per CTA
     w = wl.Workload("cfg4_split", w4.kind, nside, 128, w4.s_max, np.geomspace(0.408e9, 30e9, 13), params, w4.aux,
                     cot_seed=2104)
     pix = np.arange(3, w.npix, 96)
@@ -439,7 +439,7 @@ def test_vjp_per_cta_split_frequency_blocks_and_batch(batch):
         c[..., pix] = f[..., pix]
     ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots), pix=pix)
     g = parity.gpu_vjp(w, cots)
-    _check_grad(g, ref, f"vjp per-CTA split, 13 frequencies, batch {batch}")
+    _check_grad(g, ref, f"vjp per-CTA split, 13 frequencies, batch {batch}, nside {nside}")
     # same call twice: the split keeps the thread <-> sightline mapping, so the gradient is bit-reproducible
     assert np.array_equal(g, parity.gpu_vjp(w, cots))
     # and the float64-angle variant everywhere agrees within the bound as well
