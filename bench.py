@@ -411,7 +411,9 @@ def run_ours(args):
                         "parameters in and (logL, grad) out per step; observed Q/U maps resident on the device"},
             "gpu_launches": r["launches"], "escalated_sightlines": r["escalated"],
             "clocks": clocks,
-            "roofline": {"bound": "alu", "kernel": "vjp_kernel (analytic adjoint)" if w.kind != "grid_b" else "grid_vjp_kernel",
+            "roofline": {"bound": "alu", "kernel": ("vjp_kernel (analytic adjoint; long calls: vjp_classify_kernel + the fp32-angle / float64-angle "
+                                    "pair of vjp_kernel launches on two streams, timed as one call)")
+                         if w.kind != "grid_b" else "grid_vjp_kernel",
                          "achieved": achieved, "peak": peak, "unit": "T fp32 lane-instr/s", "frac": achieved / peak,
                          "traffic": traffic, "peak_source": f"148 SM x 128 FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
                          "alg_fp32_per_sample": fp_vjp, "forward": {"alg_fp32_per_sample": fp_fwd,
