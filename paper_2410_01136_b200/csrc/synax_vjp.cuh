@@ -590,9 +590,12 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
   if (split && cudaMallocAsync((void**)&cta_sel, (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
     return SYNAX_ERR_ALLOC;
   float* partial = nullptr;
-  if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
+  if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess) {
+    if (cta_sel) cudaFreeAsync(cta_sel, st);
     return SYNAX_ERR_ALLOC;
+  }
   a.partial = partial;
+  cudaError_t stream_err = cudaSuccess;   // fork / join of the second stream
   for (int b0 = 0; b0 < batch; b0 += 65535) {   // gridDim.y limit
     const dim3 grid((unsigned)a.n_blocks, (unsigned)std::min(65535, batch - b0));
     a.b0 = b0;
@@ -602,7 +605,9 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       else if (code == kAnalyticFull) launch_vjp_classify<kAnalyticFull>(G, grid, st, a, cta_sel);
       else launch_vjp_classify<kUniform>(G, grid, st, a, cta_sel);
       ++*launches;
-      if (cudaEventRecord(ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(aux, ev_fork, 0) != cudaSuccess) return SYNAX_ERR_CUDA;
+      cudaError_t r = cudaEventRecord(ev_fork, st);
+      if (r == cudaSuccess) r = cudaStreamWaitEvent(aux, ev_fork, 0);
+      if (r != cudaSuccess) { stream_err = r; break; }   // nothing launched on the second stream yet: clean up below
     }
     for (int f0 = 0; f0 < ft.n_freq;) {
       const int rem = ft.n_freq - f0;
@@ -629,12 +634,18 @@ static synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& ge
       ++*launches;
       f0 += nf;
     }
-    if (split && (cudaEventRecord(ev_join, aux) != cudaSuccess || cudaStreamWaitEvent(st, ev_join, 0) != cudaSuccess))
-      return SYNAX_ERR_CUDA;
+    if (split) {
+      cudaError_t r = cudaEventRecord(ev_join, aux);
+      if (r == cudaSuccess) r = cudaStreamWaitEvent(st, ev_join, 0);
+      if (r != cudaSuccess) { stream_err = r; cudaStreamSynchronize(aux); break; }   // join by hand, then clean up
+    }
   }
-  vjp_reduce_kernel<<<batch, 256, 0, st>>>(partial, a.n_blocks, n_params, grad);
-  ++*launches;
-  const cudaError_t e = cudaGetLastError();
+  if (stream_err == cudaSuccess) {
+    vjp_reduce_kernel<<<batch, 256, 0, st>>>(partial, a.n_blocks, n_params, grad);
+    ++*launches;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (stream_err != cudaSuccess) e = stream_err;
   cudaFreeAsync(partial, st);
   if (cta_sel) cudaFreeAsync(cta_sel, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
