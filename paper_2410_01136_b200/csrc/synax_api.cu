@@ -10,9 +10,8 @@
 #include <cstring>
 #include <new>
 
-#include "synax_forward.cuh"
-#include "synax_vjp.cuh"
-#include "synax_grid.cuh"
+#include "synax_launch.h"
+#include "synax_plan_kernels.cuh"
 
 using namespace synax;
 
@@ -312,41 +311,11 @@ static int next_freq_block(int remaining) {
   return remaining;  // 1, 2, 3
 }
 
-template <int CODE, int G, bool LIST>
-static void launch_forward_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
-  const FreqTab ft = shift_freqs(ft0, a.f0);
-  switch (nf) {
-    case 1: forward_kernel<CODE, G, 1, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 2: forward_kernel<CODE, G, 2, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 3: forward_kernel<CODE, G, 3, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    case 4: forward_kernel<CODE, G, 4, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
-    default: forward_kernel<CODE, G, 8, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
-  }
+namespace synax {
+void launch_decide(int* ctrl, int64_t n_pilot, int num, int den, int mode_yes, cudaStream_t st) {
+  decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, num, den, mode_yes);
 }
-template <int CODE, bool LIST>
-static void launch_forward(int G, int nf, int64_t n_sl, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
-  const unsigned blocks = (unsigned)((n_sl * G + kBlock - 1) / kBlock);
-  if (G == 1) launch_forward_nf<CODE, 1, LIST>(nf, blocks, st, a, ft);
-  else if (G == 8) launch_forward_nf<CODE, 8, LIST>(nf, blocks, st, a, ft);
-  else launch_forward_nf<CODE, 32, LIST>(nf, blocks, st, a, ft);
-}
-template <int CODE, int G>
-static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
-  const FreqTab ft = shift_freqs(ft0, a.f0);
-  switch (nf) {
-    case 1: forward_f64_kernel<CODE, G, 1><<<blocks, kBlockD, 0, st>>>(a, ft); break;
-    case 2: forward_f64_kernel<CODE, G, 2><<<blocks, kBlockD, 0, st>>>(a, ft); break;
-    case 3: forward_f64_kernel<CODE, G, 3><<<blocks, kBlockD, 0, st>>>(a, ft); break;
-    case 4: forward_f64_kernel<CODE, G, 4><<<blocks, kBlockD, 0, st>>>(a, ft); break;
-    default: forward_f64_kernel<CODE, G, 8><<<blocks, kBlockD, 0, st>>>(a, ft); break;
-  }
-}
-template <int CODE>
-static void launch_f64(int G, int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft) {
-  if (G == 1) launch_f64_nf<CODE, 1>(nf, blocks, st, a, ft);
-  else if (G == 8) launch_f64_nf<CODE, 8>(nf, blocks, st, a, ft);
-  else launch_f64_nf<CODE, 32>(nf, blocks, st, a, ft);
-}
+}  // namespace synax
 
 static AuxHost make_aux(const synax_model* m) {
   AuxHost a;
@@ -426,10 +395,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       const int64_t stride = (n_sl / 8192) | 1;
       const int64_t n_pilot = (n_sl + stride - 1) / stride;
       const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
-      if (code == kAnalyticDisc) pilot_kernel<kAnalyticDisc><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
-      else if (code == kStack16) pilot_kernel<kStack16><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
-      else if (code == kAnalyticFull) pilot_kernel<kAnalyticFull><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
-      else pilot_kernel<kUniform><<<pb, kBlock, 0, st>>>(a, stride, n_pilot, ctrl);
+      SYNAX_DISPATCH_CODE(code, fwd_launch_pilot, pb, st, a, stride, n_pilot, ctrl);
       // the split mode costs four more launches: only for calls long enough not to notice (cfg 1: 0.19 ms in all)
       split_ok = n_sl >= 262144;
       if (split_ok) {
@@ -437,13 +403,10 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
         CUDA_TRY(cudaMallocAsync((void**)&a.list_u, sizeof(int) * (size_t)n_sl, st));
         a.count_u = ctrl + kCtrlCountU;
         const unsigned cb = (unsigned)std::min<int64_t>((n_sl + kBlock - 1) / kBlock, (int64_t)sm_count(plan->device) * 16);
-        if (code == kAnalyticDisc) classify_kernel<kAnalyticDisc><<<cb, kBlock, 0, st>>>(a, ctrl);
-        else if (code == kStack16) classify_kernel<kStack16><<<cb, kBlock, 0, st>>>(a, ctrl);
-        else if (code == kAnalyticFull) classify_kernel<kAnalyticFull><<<cb, kBlock, 0, st>>>(a, ctrl);
-        else classify_kernel<kUniform><<<cb, kBlock, 0, st>>>(a, ctrl);
+        SYNAX_DISPATCH_CODE(code, fwd_launch_classify, cb, st, a, ctrl);
         plan->launches += 3;
       } else {
-        decide_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot, 1, 4, kModeAllF64);   // more than a quarter flagged: all-float64
+        launch_decide(ctrl, n_pilot, 1, 4, kModeAllF64, st);   // more than a quarter flagged: all-float64
         plan->launches += 2;
       }
       a.mode = ctrl + kCtrlMode;
@@ -467,10 +430,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       pa.f0 = f0;
-      if (code == kAnalyticDisc) launch_f64<kAnalyticDisc>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
-      else if (code == kStack16) launch_f64<kStack16>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
-      else if (code == kAnalyticFull) launch_f64<kAnalyticFull>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
-      else launch_f64<kUniform>(lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
+      SYNAX_DISPATCH_CODE(code, fwd_launch_f64, lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
       plan->launches++;
       f0 += nf;
     }
@@ -479,16 +439,10 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       a.f0 = f0;
-      if (code == kAnalyticDisc) launch_forward<kAnalyticDisc, false>(G, nf, n_sl, st, a, plan->ft);
-      else if (code == kStack16) launch_forward<kStack16, false>(G, nf, n_sl, st, a, plan->ft);
-      else if (code == kAnalyticFull) launch_forward<kAnalyticFull, false>(G, nf, n_sl, st, a, plan->ft);
-      else launch_forward<kUniform, false>(G, nf, n_sl, st, a, plan->ft);
+      SYNAX_DISPATCH_CODE(code, fwd_launch_fast, false, G, nf, n_sl, st, a, plan->ft);
       plan->launches++;
       if (split_ok) {   // the same pass over list_u (exits at once unless the pilot chose the split mode)
-        if (code == kAnalyticDisc) launch_forward<kAnalyticDisc, true>(G, nf, n_sl, st, a, plan->ft);
-        else if (code == kStack16) launch_forward<kStack16, true>(G, nf, n_sl, st, a, plan->ft);
-        else if (code == kAnalyticFull) launch_forward<kAnalyticFull, true>(G, nf, n_sl, st, a, plan->ft);
-        else launch_forward<kUniform, true>(G, nf, n_sl, st, a, plan->ft);
+        SYNAX_DISPATCH_CODE(code, fwd_launch_fast, true, G, nf, n_sl, st, a, plan->ft);
         plan->launches++;
       }
       f0 += nf;

@@ -16,15 +16,15 @@ namespace synax {
 
 // Polynomial coefficients live in constant memory so that DFMA takes them as c[bank][offset] operands
 // (a 64-bit literal costs two UMOV issue slots each time it is used).
-__constant__ double kExp2C[9] = {   // ln2^k / k!, k = 9 .. 1
+static __constant__ double kExp2C[9] = {   // ln2^k / k!, k = 9 .. 1
     1.0178086009239699e-7, 1.3215486790144307e-6, 1.5252733804059841e-5, 1.5403530393381609e-4,
     1.3333558146428443e-3, 9.6181291076284772e-3, 5.5504108664821580e-2, 2.4022650695910071e-1,
     6.9314718055994531e-1};
-__constant__ double kSinC[5] = {-2.5052108385441718775e-8, 2.7557319223985890653e-6, -1.9841269841269841270e-4,
+static __constant__ double kSinC[5] = {-2.5052108385441718775e-8, 2.7557319223985890653e-6, -1.9841269841269841270e-4,
                                 8.3333333333333333333e-3, -1.6666666666666666667e-1};
-__constant__ double kCosC[6] = {2.0876756987868098979e-9, -2.7557319223985890653e-7, 2.4801587301587301587e-5,
+static __constant__ double kCosC[6] = {2.0876756987868098979e-9, -2.7557319223985890653e-7, 2.4801587301587301587e-5,
                                 -1.3888888888888888889e-3, 4.1666666666666666667e-2, -0.5};
-__constant__ double kMiscC[4] = {6755399441055744.0,          // 1.5 * 2^52
+static __constant__ double kMiscC[4] = {6755399441055744.0,          // 1.5 * 2^52
                                  0.63661977236758134308,      // 2/pi
                                  -1.5707963267948966192,      // -pi/2 hi
                                  -6.1232339957367658860e-17}; // -pi/2 lo

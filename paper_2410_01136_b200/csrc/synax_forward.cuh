@@ -23,182 +23,6 @@ constexpr float kTilePhase = 96.0f;  // ... and at most about this much Faraday 
 enum ModelCode { kAnalyticDisc = 0, kAnalyticFull = 1, kGridB = 2, kUniform = 3, kStack16 = 4 };
 
 // ------------------------------------------------------------------------------------------------
-// A1: HEALPix RING pixel -> (cos l, sin l, cos b, sin b) in float64 (Gorski et al. 2005).
-// Integer ring arithmetic as in DESIGN.md section 4; once per plan.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int64_t isqrt_i64(int64_t v) {
-  int64_t r = (int64_t)sqrt((double)v);
-  while (r * r > v) --r;
-  while ((r + 1) * (r + 1) <= v) ++r;
-  return r;
-}
-
-// Writes dirs[i] for the `count` pixels p = pix0 + i of the nside map (a plan may hold a shard of the sky).
-__global__ void pix2ang_kernel(int64_t nside, int64_t pix0, int64_t count, double* __restrict__ dirs) {
-  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= count) return;
-  const int64_t p = pix0 + idx;
-  const int64_t npix = 12 * nside * nside;
-  const int64_t ncap = 2 * nside * (nside - 1);
-  double z, phi, omz;  // omz = 1 - |z| kept separately for accurate cos b near the poles
-  if (p < ncap) {
-    const int64_t i = (1 + isqrt_i64(1 + 2 * p)) / 2;
-    const int64_t j = p + 1 - 2 * i * (i - 1);
-    omz = (double)(i * i) / (3.0 * (double)(nside * nside));
-    z = 1.0 - omz;
-    phi = ((double)j - 0.5) * SYNAX_PI / (2.0 * (double)i);
-  } else if (p < npix - ncap) {
-    const int64_t pp = p - ncap;
-    const int64_t i = pp / (4 * nside) + nside;
-    const int64_t j = pp % (4 * nside) + 1;
-    const double s = ((i + nside) & 1) ? 1.0 : 0.5;
-    z = (double)(2 * nside - i) * 2.0 / (3.0 * (double)nside);
-    omz = 1.0 - fabs(z);
-    phi = ((double)j - s) * SYNAX_PI / (2.0 * (double)nside);
-  } else {
-    const int64_t pp = npix - p;
-    const int64_t i = (1 + isqrt_i64(2 * pp - 1)) / 2;
-    const int64_t j = 4 * i + 1 - (pp - 2 * i * (i - 1));
-    omz = (double)(i * i) / (3.0 * (double)(nside * nside));
-    z = -1.0 + omz;
-    phi = ((double)j - 0.5) * SYNAX_PI / (2.0 * (double)i);
-  }
-  double sl, cl;
-  sincos(phi, &sl, &cl);
-  const double cb = sqrt(omz * (1.0 + fabs(z)));  // sin(theta) = sqrt((1-|z|)(1+|z|))
-  dirs[4 * idx + 0] = cl; dirs[4 * idx + 1] = sl; dirs[4 * idx + 2] = cb; dirs[4 * idx + 3] = z;
-}
-
-// Path length of every sightline of the plan from the observer (strictly inside the box) to the face of a box of
-// side lengths `box` centred on the Galactic centre, in units of s_ref (Fig. 1): path[i] = L_i / s_ref.
-__global__ void box_path_kernel(const double* __restrict__ dirs, int64_t count, double ox, double oy, double oz,
-                                double hx, double hy, double hz, double inv_s_ref, double* __restrict__ path) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= count) return;
-  const double4 d = *reinterpret_cast<const double4*>(dirs + 4 * i);   // cos l, sin l, cos b, sin b
-  const double n[3] = {d.z * d.x, d.z * d.y, d.w};
-  const double o[3] = {ox, oy, oz}, h[3] = {hx, hy, hz};
-  double L = 1.0e300;
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    if (n[k] > 0.0) L = fmin(L, (h[k] - o[k]) / n[k]);
-    else if (n[k] < 0.0) L = fmin(L, (-h[k] - o[k]) / n[k]);
-  }
-  path[i] = L * inv_s_ref;
-}
-
-// ------------------------------------------------------------------------------------------------
-// Prologue: raw parameters -> BatchConsts (float64 math, once per batch element per call).
-// Folds Eq.(2)'s constants, the Rayleigh-Jeans conversion (S:C-2#1) and the units into
-// c_f(alpha) so that I_f = c_f Delta sum_n N_0 (B_perp^2)^((alpha+1)/4)  with B in uG.
-// ------------------------------------------------------------------------------------------------
-struct AuxHost { float v[7]; };  // C0, h_r, h_z, alpha, ne0, h_er, h_ez
-
-__global__ void prologue_kernel(int code, const float* __restrict__ params, int n_params, int batch,
-                                AuxHost aux, FreqTab ft, double delta, BatchConsts* __restrict__ out,
-                                BatchConstsD* __restrict__ outd) {
-  const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= batch) return;
-  BatchConsts c;
-  for (int j = 0; j < 16; ++j) c.sp[j] = 0.0f;
-  double p[16];
-  for (int j = 0; j < 16; ++j) p[j] = 0.0;
-  double alpha;
-  if (code == kAnalyticFull) {
-    for (int j = 0; j < 16; ++j) p[j] = (double)params[(size_t)b * n_params + j];
-  } else if (code == kUniform) {
-    const float* q = params + (size_t)b * n_params;
-    c.uB[0] = q[0]; c.uB[1] = q[1]; c.uB[2] = q[2]; c.uN0 = q[3]; c.une = q[4];
-    p[12] = (double)q[5];
-    p[4] = p[7] = p[8] = p[10] = p[11] = p[14] = p[15] = 1.0;
-  } else {  // DISC4, STACK16 or GRID_B: densities and alpha from aux
-    if (code == kStack16)
-      for (int j = 0; j < 16; ++j) c.sp[j] = params[(size_t)b * n_params + j];
-    if (code == kAnalyticDisc)
-      for (int j = 0; j < 4; ++j) p[j] = (double)params[(size_t)b * n_params + j];
-    p[4] = 1.0;  // unused: k_hb = 0
-    p[6] = 0.0; p[7] = 1.0; p[8] = 1.0;
-    p[9] = aux.v[0]; p[10] = aux.v[1]; p[11] = aux.v[2]; p[12] = aux.v[3];
-    p[13] = aux.v[4]; p[14] = aux.v[5]; p[15] = aux.v[6];
-  }
-  alpha = p[12];
-  for (int j = 0; j < 16; ++j) c.p[j] = (float)p[j];
-  const double log2e = 1.4426950408889634;
-  c.k_hb = (code == kAnalyticFull) ? (float)(-log2e / p[4]) : 0.0f;
-  c.k_hb_lo = (code == kAnalyticFull) ? (float)(-log2e / p[4] - (double)c.k_hb) : 0.0f;
-  c.inv_wh = (float)(1.0 / p[8]);
-  c.inv_rh = (float)(1.0 / p[7]);
-  c.k_hr = (float)(-log2e / p[10]);
-  c.k_hz = (float)(-2.0 * log2e / fabs(p[11]));
-  c.k_her = (float)(-log2e / p[14]);
-  c.k_her_lo = (float)(-log2e / p[14] - (double)c.k_her);
-  c.k_hez = (float)(-2.0 * log2e / fabs(p[15]));
-  c.q_exp = (float)((alpha - 3.0) * 0.25);
-  c.pi_frac = (float)((alpha + 1.0) / (alpha + 7.0 / 3.0));
-  c.alpha_is_3 = (c.p[12] == 3.0f) ? 1 : 0;
-  c.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4; |ln(rho/8)| < 1 in the annulus
-  c.dpi_dalpha_over_pi = (float)(1.0 / (alpha + 1.0) - 1.0 / (alpha + 7.0 / 3.0));
-  // Eq.(2) prefactor with B^((1+alpha)/2) nu^((1-alpha)/2) factored out
-  const double g1 = tgamma(alpha * 0.25 - 1.0 / 12.0), g2 = tgamma(alpha * 0.25 + 19.0 / 12.0);
-  const double w = 4.0 * SYNAX_PI * SYNAX_ME * SYNAX_C / (3.0 * SYNAX_QE);
-  const double A_I = sqrt(3.0) * SYNAX_QE * SYNAX_QE * SYNAX_QE / (8.0 * SYNAX_PI * SYNAX_ME * SYNAX_C * SYNAX_C) *
-                     pow(w, (1.0 - alpha) * 0.5) * pow(2.0, (alpha + 1.0) * 0.5) / (alpha + 1.0) * g1 * g2;
-  const double dlnA = -0.5 * log(w) + 0.5 * log(2.0) - 1.0 / (alpha + 1.0) +
-                      0.25 * digamma_d(alpha * 0.25 - 1.0 / 12.0) + 0.25 * digamma_d(alpha * 0.25 + 19.0 / 12.0) +
-                      0.5 * log(1.0e-6);
-  for (int f = 0; f < kMaxFreq; ++f) {
-    if (f < ft.n_freq) {
-      const double nu = ft.freq[f];
-      const double TRJ = SYNAX_C * SYNAX_C / (2.0 * SYNAX_KB * nu * nu);
-      const double cf = TRJ * A_I * pow(nu, (1.0 - alpha) * 0.5) * pow(1.0e-6, (alpha + 1.0) * 0.5) * SYNAX_KPC * delta;
-      c.coefI[f] = (float)cf;
-      c.coefP[f] = (float)(cf * (alpha + 1.0) / (alpha + 7.0 / 3.0));
-      c.dlnc_dalpha[f] = (float)(dlnA - 0.5 * log(nu));
-    } else {
-      c.coefI[f] = c.coefP[f] = c.dlnc_dalpha[f] = 0.0f;
-    }
-  }
-  // Tile length of the float64-chain kernel: the fp32 angle k_f * (tile-local Faraday sum) must stay small
-  // enough for its 6e-8 relative round-off not to matter.  Bound on |n_e B_LOS| per sample:
-  {
-    double gmax;
-    if (code == kUniform) {
-      gmax = fabs((double)c.une) * (fabs((double)c.uB[0]) + fabs((double)c.uB[1]) + fabs((double)c.uB[2]));
-    } else {
-      double bmax = fabs(p[0]);
-      if (code == kStack16) bmax = 0.6 * fabs((double)c.sp[0]) + 0.3 * fabs((double)c.sp[4]) + 0.1 * fabs((double)c.sp[8]) + 0.3 * fabs((double)c.sp[12]);
-      if (code == kAnalyticFull) bmax = bmax * fmax(exp(5.0 / p[4]), exp(-12.0 / p[4])) + fabs(p[5]);
-      gmax = fabs(p[13]) * bmax;
-    }
-    double kmax = 0.0;
-    for (int f = 0; f < ft.n_freq; ++f) kmax = fmax(kmax, (double)ft.k_rad[f]);
-    const double per_step = kmax * gmax;
-    int t = kTileDMax;
-    if (per_step * t > (double)kTilePhase) t = (int)((double)kTilePhase / per_step);
-    if (t > kUnrollD) t -= t % kUnrollD;
-    c.tile_d = t < 1 ? 1 : t;
-  }
-  out[b] = c;
-  if (outd) {
-    BatchConstsD d;
-    d.b0 = p[0]; d.psi0 = p[1]; d.psi1 = p[2]; d.chi0 = p[3];
-    d.k_hb = (code == kAnalyticFull) ? -log2e / p[4] : 0.0;
-    d.Bh = p[5]; d.zh0 = p[6]; d.inv_rh = 1.0 / p[7]; d.inv_wh = 1.0 / p[8];
-    d.ne0x4 = 4.0 * p[13]; d.k_her = -log2e / p[14]; d.k_hez = -2.0 * log2e / fabs(p[15]);
-    d.psi1_small = fabs(p[2]) <= 0.05 ? 1 : 0;
-    d.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4
-    d.hez_is_one = (p[15] == 1.0 || p[15] == -1.0) ? 1 : 0;
-    for (int k = 0; k < 4; ++k) {
-      const bool st = code == kStack16;
-      const double w = k == 0 ? 0.6 : (k == 2 ? 0.1 : 0.3);
-      d.sb0[k] = st ? w * (double)c.sp[4 * k] : 0.0; d.spsi0[k] = st ? (double)c.sp[4 * k + 1] : 0.0;
-      d.spsi1[k] = st ? (double)c.sp[4 * k + 2] : 0.0; d.schi0[k] = st ? (double)c.sp[4 * k + 3] : 0.0;
-    }
-    outd[b] = d;
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
 // small warp helpers over groups of G lanes (G = 1, 2, 4, ..., 32; groups are aligned)
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double shfl_up_d(double v, int d, int width) {
@@ -690,20 +514,6 @@ __global__ void __launch_bounds__(kBlock) classify_kernel(const __grid_constant_
   }
   __syncthreads();
   }
-}
-
-// Forward: the pilot's flagged share picks the mode -- below 1/50: fp32 pass + float64 redo of its flag list; above
-// 3/4: float64 chain for every sightline; in between: split by classify_kernel.  (cfg 4 @ 408 MHz, fp32 pass 7.2 ms,
-// float64 pass 11.1 ms: measured split 11.9 / 10.4 / 9.1 ms at 78 / 50 / 28 % flagged.)
-__global__ void decide_forward_kernel(int* __restrict__ ctrl, int64_t n_pilot) {
-  const int64_t f = ctrl[kCtrlPilotFlagged];
-  ctrl[kCtrlMode] = (50 * f <= n_pilot) ? kModeFastThenList : (4 * f > 3 * n_pilot) ? kModeAllF64 : kModeSplit;
-}
-
-__global__ void decide_kernel(int* __restrict__ ctrl, int64_t n_pilot, int num, int den, int mode_yes) {
-  // short forward calls (1/4): more than a quarter flagged -> one float64-chain pass costs less than fp32 + redo.
-  // adjoint (0/1): any sampled sightline above half the threshold, see analytic_vjp.
-  ctrl[kCtrlMode] = ((int64_t)den * ctrl[kCtrlPilotFlagged] > (int64_t)num * n_pilot) ? mode_yes : kModeFastThenList;
 }
 
 }  // namespace synax

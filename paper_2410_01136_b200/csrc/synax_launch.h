@@ -1,0 +1,47 @@
+// synax_launch.h -- host-side launchers of the template kernels.  Each model code is instantiated in its own
+// translation unit (synax_fwd_<code>.cu, synax_vjp_<code>.cu) so that the library builds in parallel; synax_api.cu and
+// synax_vjp_driver.cu see only these declarations.
+#pragma once
+#include "../../include/synax.h"
+#include "synax_forward.cuh"
+#include "synax_vjp.cuh"
+
+namespace synax {
+
+// ---- forward (synax_fwd_impl.cuh, explicitly instantiated per CODE)
+template <int CODE> void fwd_launch_pilot(unsigned blocks, cudaStream_t st, const ForwardArgs& a, int64_t stride, int64_t n_pilot, int* ctrl);
+template <int CODE> void fwd_launch_classify(unsigned blocks, cudaStream_t st, const ForwardArgs& a, int* ctrl);
+template <int CODE> void fwd_launch_fast(bool list, int G, int nf, int64_t n_sl, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft);
+template <int CODE> void fwd_launch_f64(int G, int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft);
+
+// ---- adjoint (synax_vjp_impl.cuh, explicitly instantiated per CODE)
+template <int CODE> void vjp_launch(int pmode, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft);
+template <int CODE> void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, const VjpArgs& a, unsigned char* cta_sel);
+
+// dispatch on the run-time model code (kAnalyticDisc, kAnalyticFull, kStack16, kUniform)
+#define SYNAX_DISPATCH_CODE(code, FN, ...)                                   \
+  do {                                                                       \
+    if ((code) == kAnalyticDisc) FN<kAnalyticDisc>(__VA_ARGS__);             \
+    else if ((code) == kStack16) FN<kStack16>(__VA_ARGS__);                  \
+    else if ((code) == kAnalyticFull) FN<kAnalyticFull>(__VA_ARGS__);        \
+    else FN<kUniform>(__VA_ARGS__);                                          \
+  } while (0)
+
+// ---- synax_vjp_driver.cu
+synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
+                          const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
+                          const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int* ctrl,
+                          cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
+                          const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
+                          int64_t* launches);
+
+// ---- synax_grid.cu
+synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_model* m, const float* grid,
+                          int precision, double escalate_rad, int sms, int* d_flag_count, int* h_flag_count,
+                          cudaStream_t st, int64_t* launches);
+synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const BatchConstsD* bd,
+                      const synax_model* m, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0,
+                      const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
+                      int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches);
+
+}  // namespace synax

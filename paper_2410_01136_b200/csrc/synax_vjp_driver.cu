@@ -1,0 +1,136 @@
+// synax_vjp_driver.cu -- host-side orchestration of the analytic adjoint: pilot, per-CTA pair on two streams,
+// frequency passes, deterministic reduction ("VJP").
+#include <algorithm>
+
+#include "synax_launch.h"
+
+namespace synax {
+
+// decide_kernel lives in synax_api.cu's translation unit (synax_plan_kernels.cuh)
+void launch_decide(int* ctrl, int64_t n_pilot, int num, int den, int mode_yes, cudaStream_t st);
+
+static void launch_pmode(int code, int pmode, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
+  SYNAX_DISPATCH_CODE(code, vjp_launch, pmode, G, nf, grid, st, a, ft);
+}
+
+// partial[b][n_blocks][16] -> grad[b][n_params], float64 accumulation, deterministic order
+__global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_blocks, int n_params, float* __restrict__ grad) {
+  const int b = blockIdx.x;
+  const int j = threadIdx.x & 15;
+  const int part = threadIdx.x >> 4;        // 16 partial sums per parameter
+  __shared__ double sh[16][17];
+  double s = 0.0;
+  if (j < n_params)
+    for (int k = part; k < n_blocks; k += 16) s += (double)partial[((size_t)b * n_blocks + k) * 16 + j];
+  sh[part][j] = s;
+  __syncthreads();
+  if (threadIdx.x < n_params) {
+    double t = 0.0;
+    for (int k = 0; k < 16; ++k) t += sh[k][threadIdx.x];
+    grad[(size_t)b * n_params + threadIdx.x] = (float)t;
+  }
+}
+
+// The adjoint tolerates ~10x the Faraday round-off scale the forward does (gradients are sums over all pixels,
+// bound 1e-3 instead of 1e-4).  precision 0: per sightline (PMODE 2), threshold 10 x escalate_rad -- unless a pilot
+// over ~8k sightlines finds none above HALF that threshold, in which case the lean fp32 variant (PMODE 0: fewer
+// registers, no estimate) runs (cfg 2 at 23 GHz: 8.2 instead of 9.5 ms).  Decided on the device, no host sync.
+constexpr double kVjpEscalateFactor = 10.0;
+
+synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
+                                 const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
+                                 const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int* ctrl,
+                                 cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
+                                 const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
+                                 int64_t* launches) {
+  VjpArgs a;
+  a.geo = geo; a.bc = bc; a.bd = bd; a.batch = batch; a.n_freq_total = ft.n_freq;
+  a.dI = dI; a.dQ = dQ; a.dU = dU; a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
+  a.n_blocks = (int)((geo.npix * G + kBlock - 1) / kBlock);
+  float k_max = 0.f;
+  for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
+  a.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
+  a.mode = nullptr; a.cta_sel = nullptr;
+  // Long calls with one thread per sightline: the work is split per CTA between the lean fp32 variant and the
+  // float64-angle variant (vjp_classify_kernel) instead of deciding per sightline inside one heavier kernel
+  // (cfg 4, 9 % of the sightlines above the threshold: 14.3 -> see DESIGN.md section 5).
+  // (G lanes per sightline, G > 1: a CTA holds 128 / G sightlines; worth its three extra launches from ~1M threads)
+  const bool split = precision == 0 && (G == 1 ? geo.npix * batch >= 262144 : geo.npix * batch * G >= 1000000);
+  if (precision == 0) {
+    ForwardArgs pa;
+    pa.geo = geo; pa.bc = bc; pa.bd = bd; pa.batch = batch; pa.sg_ne = sg_ne; pa.sg_n0 = sg_n0;
+    pa.flag_S = 0.5f * a.flag_S;
+    const int64_t n_sl = geo.npix * batch;
+    const int64_t stride = (n_sl / 8192) | 1;
+    const int64_t n_pilot = (n_sl + stride - 1) / stride;
+    const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
+    if (cudaMemsetAsync(ctrl, 0, kCtrlWords * sizeof(int), st) != cudaSuccess) return SYNAX_ERR_CUDA;
+    SYNAX_DISPATCH_CODE(code, fwd_launch_pilot, pb, st, pa, stride, n_pilot, ctrl);
+    // any sampled sightline above half the threshold: per-sightline variant, or (long calls) the per-CTA pair
+    launch_decide(ctrl, n_pilot, 0, 1, split ? kModeSplit : kModeAllF64, st);
+    *launches += 2;
+    a.mode = ctrl + kCtrlMode;
+  }
+  unsigned char* cta_sel = nullptr;
+  if (split && cudaMallocAsync((void**)&cta_sel, (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
+    return SYNAX_ERR_ALLOC;
+  float* partial = nullptr;
+  if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess) {
+    if (cta_sel) cudaFreeAsync(cta_sel, st);
+    return SYNAX_ERR_ALLOC;
+  }
+  a.partial = partial;
+  cudaError_t stream_err = cudaSuccess;   // fork / join of the second stream
+  for (int b0 = 0; b0 < batch; b0 += 65535) {   // gridDim.y limit
+    const dim3 grid((unsigned)a.n_blocks, (unsigned)std::min(65535, batch - b0));
+    a.b0 = b0;
+    if (split) {
+      SYNAX_DISPATCH_CODE(code, vjp_launch_classify, G, grid, st, a, cta_sel);
+      ++*launches;
+      cudaError_t r = cudaEventRecord(ev_fork, st);
+      if (r == cudaSuccess) r = cudaStreamWaitEvent(aux, ev_fork, 0);
+      if (r != cudaSuccess) { stream_err = r; break; }   // nothing launched on the second stream yet: clean up below
+    }
+    for (int f0 = 0; f0 < ft.n_freq;) {
+      const int rem = ft.n_freq - f0;
+      const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
+      a.f0 = f0; a.accumulate = f0 > 0;
+      if (precision == 1) launch_pmode(code, 0, G, nf, grid, st, a, ft);
+      else if (precision == 2) launch_pmode(code, 1, G, nf, grid, st, a, ft);
+      else {
+        launch_pmode(code, 0, G, nf, grid, st, a, ft);
+        if (split) {
+          // the per-CTA pair (runs in kModeSplit).  Every CTA's partial belongs to exactly one member, so the two run
+          // concurrently: the float64-angle member (few, long CTAs: 2.7 waves at cfg 4) on the plan's second stream,
+          // forked after the classify kernel and joined before the reduction, fills its tail with the other's CTAs.
+          VjpArgs as = a;
+          as.cta_sel = cta_sel;
+          launch_pmode(code, 1, G, nf, grid, aux, as, ft);
+          launch_pmode(code, 0, G, nf, grid, st, as, ft);
+          ++*launches;
+        } else {
+          launch_pmode(code, 2, G, nf, grid, st, a, ft);
+        }
+        ++*launches;
+      }
+      ++*launches;
+      f0 += nf;
+    }
+    if (split) {
+      cudaError_t r = cudaEventRecord(ev_join, aux);
+      if (r == cudaSuccess) r = cudaStreamWaitEvent(st, ev_join, 0);
+      if (r != cudaSuccess) { stream_err = r; cudaStreamSynchronize(aux); break; }   // join by hand, then clean up
+    }
+  }
+  if (stream_err == cudaSuccess) {
+    vjp_reduce_kernel<<<batch, 256, 0, st>>>(partial, a.n_blocks, n_params, grad);
+    ++*launches;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (stream_err != cudaSuccess) e = stream_err;
+  cudaFreeAsync(partial, st);
+  if (cta_sel) cudaFreeAsync(cta_sel, st);
+  return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
+}
+
+}  // namespace synax
