@@ -103,13 +103,19 @@ int64_t synax_plan_npix(const synax_plan* plan);  /* pixels of this plan (12 nsi
  * HOST pointer; synchronises the device. */
 synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
 
-/* Options.  key "precision": 0 = auto (default), 1 = fp32 only, 2 = float64 Faraday chain for every sightline.
+/* Options.  key "precision": 0 = auto (default), 1 = fp32 only, 2 = float64 Faraday chain for every sightline,
+ * 3 = everything in float64 (the paper's default precision; analytic models).
  * Auto, forward: sightlines whose Faraday round-off scale k_max sum_n |n_e| (|B_LOS|+|B_N|+|B_E|) exceeds
- * "escalate_rad" (default 100 rad) take the float64 Faraday chain -- as a redo of a flagged list after the fp32
- * pass, or for every sightline when a device-side pilot finds more than a quarter flagged.  Auto, VJP: decided per
- * sightline inside the kernel -- those above 10 x escalate_rad take their Faraday angles from the float64 chain.
+ * "escalate_rad" (default 300 rad, calibrated against the oracle: DESIGN.md section 5) take the float64 Faraday
+ * chain -- as a redo of a flagged list after the fp32 pass, for every sightline when a device-side pilot finds most of
+ * them flagged, or split between the two chains in between.  Auto, VJP: decided per sightline (per CTA in long calls)
+ * -- those above 10/3 x escalate_rad take their Faraday angles from the float64 chain.
  * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0).
- * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32). */
+ * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).
+ * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool
+ * (from which every call takes its scratch) to this many MB, so that the pool is not unmapped at every stream
+ * synchronisation -- matters for the *_host calls (hundreds of MB of staging per call).  Process-wide for that
+ * device, hence opt-in; never lowers a larger threshold set by the application. */
 synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value);
 
 /* Pixel directions as cached by the plan: out[4*p..] = (cos l, sin l, cos b, sin b), DEVICE float64
@@ -128,7 +134,10 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
  * Ordering: all work is ordered with `cuda_stream` (results are complete when the stream reaches the end of the
  * call).  Long calls (>= 262,144 sightlines) may run part of their kernels on a second stream owned by the plan,
  * forked from and joined back to `cuda_stream` by events inside the call (CUDA-graph capturable); a plan must
- * therefore not be used by two calls that run concurrently -- use one plan per stream. */
+ * therefore not be used by two calls that run concurrently -- use one plan per stream.  (synax_forward does the same
+ * in its split mode.)
+ * GRID_B: n_los <= 4096 (the per-sample hand-over between the two sweeps lives in shared memory); larger n_los
+ * returns SYNAX_ERR_UNSUPPORTED. */
 synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,
                        int32_t batch, const float* dI, const float* dQ, const float* dU, float* grad,
                        void* cuda_stream);
@@ -136,8 +145,7 @@ synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const f
 /* Same operations with HOST buffers of the same shapes: the call copies the inputs to the device,
  * runs, copies the results back and synchronises the stream before returning.  When I, Q and U are all page-locked
  * (cudaHostAlloc / cudaHostRegister) the forward kernels store the maps straight into them and no copy is made.
- * Scratch comes from the device's default stream-ordered memory pool, whose release threshold the first plan raises
- * to 4 GB (unless the application has set a larger one) so that it is not re-mapped at every call. */
+ * Scratch comes from the device's default stream-ordered memory pool (see option "pool_release_threshold_mb"). */
 synax_status synax_forward_host(const synax_plan* plan, const synax_model* model, const float* params,
                                 int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
 synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, const float* params,

@@ -284,7 +284,8 @@ void disc_field_vjp(double b0, double psi0, double psi1, double chi0, double hb,
   const double Bb_phi = (-Bb[0] * y + Bb[1] * x) / rho;
   const double Bb_z = Bb[2];
   const double B_dot_Bb = A * (cp * cc * Bb_rho + sp * cc * Bb_phi + sc * Bb_z);
-  *g_b0 += B_dot_Bb / b0;
+  // dB/db0 = B_disc / b0 (App. D.3), written as the unit-amplitude field so that b0 = 0 is not 0/0
+  *g_b0 += s * (cp * cc * Bb_rho + sp * cc * Bb_phi + sc * Bb_z);
   const double dpsi = A * cc * (-sp * Bb_rho + cp * Bb_phi);
   *g_psi0 += dpsi;
   *g_psi1 += lr * dpsi;
@@ -311,7 +312,7 @@ void halo_field_vjp(double Bh, double zh0, double rh, double wh, double x, doubl
 void exp_disc_vjp(double amp, double hr, double hz, double rho, double z, double bar,
                   double* g_amp, double* g_hr, double* g_hz) {
   const double v = exp_disc(amp, hr, hz, rho, z);
-  *g_amp += bar * v / amp;
+  *g_amp += bar * exp_disc(1.0, hr, hz, rho, z);   // d/d amp = profile at unit amplitude (App. D.3), finite at amp = 0
   *g_hr += bar * v * rho / (hr * hr);
   *g_hz += bar * v * 2.0 * std::tanh(z / hz) * z / (hz * hz);
 }
@@ -559,7 +560,8 @@ void sightline_vjp(const Model& m, const Sightline& S, const Triad& T,
       chi0bar[n] += chibar;
       // j ~ N0 * Bt^((alpha+1)/2) * (alpha-dependent factor)
       const double w = jIbar * jI + jPbar * jP;
-      N0bar[n] += w / F[n].N0;
+      // j is linear in N_0 (Eq. 2, 5): N0bar = jbar * j(N_0 = 1), finite where N_0 = 0
+      N0bar[n] += jIbar * emissivity_I(nu, Bt * 1.0e-6, 1.0, F[n].alpha) + jPbar * emissivity_P(nu, Bt * 1.0e-6, 1.0, F[n].alpha);
       Btbar[n] += w * 0.5 * (F[n].alpha + 1.0) / Bt;
       alphabar[n] += jIbar * jI * dln_emissivity_I_dalpha(nu, Bt * 1.0e-6, F[n].alpha) +
                      jPbar * jP * dln_emissivity_P_dalpha(nu, Bt * 1.0e-6, F[n].alpha);

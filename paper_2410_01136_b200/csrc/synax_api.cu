@@ -18,6 +18,13 @@ using namespace synax;
 // ------------------------------------------------------------------------------------------------
 static thread_local char g_err[512] = "";
 
+// Forward, precision 0: sightlines whose Faraday round-off scale exceeds this many radians take the float64 chain.
+// Calibrated on B200 against the oracle (profiles/r02_escalate_calibration.md): over seven workloads (cfg-4 model at
+// nside 64 / 128, 256 and 1024 samples, n_e x 0.5 .. 4, B x 0.7 .. 1.5, the cfg-1 disc at 408 MHz) the largest map error
+// among the sightlines left to the fp32 chain is 2.7e-5 x RMS at 300 rad (bound 1e-4: safety factor 3.7) and
+// 0.85-1.8e-4 at 1000 rad (fails); the error grows about linearly with the threshold.
+static constexpr double kDefaultEscalateRad = 300.0;
+
 static synax_status fail(synax_status st, const char* fmt, ...) {
   va_list ap;
   va_start(ap, fmt);
@@ -70,8 +77,9 @@ static void fill_freq_table(synax_plan* p) {
       const double lam = SYNAX_C / p->freqs[f] * 1.0e-2;  // m
       const double k = 2.0 * lam * lam * KF * p->delta;   // rad per unit sum(n_e B_LOS)
       p->ft.k_rad[f] = (float)k; p->ft.k_turn[f] = k / (2.0 * SYNAX_PI); p->ft.freq[f] = p->freqs[f];
+      p->ft.ln_nu[f] = (float)std::log(p->freqs[f]);
     } else {
-      p->ft.k_rad[f] = 0.f; p->ft.k_turn[f] = 0.0; p->ft.freq[f] = 1.0;
+      p->ft.k_rad[f] = 0.f; p->ft.k_turn[f] = 0.0; p->ft.freq[f] = 1.0; p->ft.ln_nu[f] = 0.f;
     }
   }
 }
@@ -114,24 +122,9 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los; p->s_max_fixed = s_max_kpc; p->path = nullptr;
   for (int f = 0; f < n_freq; ++f) p->freqs[f] = freqs_hz[f];
   for (int i = 0; i < 3; ++i) p->obs[i] = observer_kpc[i];
-  p->precision = 0; p->escalate_rad = 100.0; p->lanes = 0;
+  p->precision = 0; p->escalate_rad = kDefaultEscalateRad; p->lanes = 0;
   fill_freq_table(p);
   cudaError_t e = cudaGetDevice(&p->device);
-  if (e == cudaSuccess) {
-    // Per-call scratch (constants, flag lists, block partials, the host entry points' staging buffers) comes from the
-    // device's stream-ordered pool.  Its default release threshold is 0: every stream synchronisation hands the memory
-    // back to the driver and the next call pays for mapping it again (hundreds of MB in the *_host calls: measured
-    // outliers of +10 ms per step).  Keep up to 4 GB cached; a larger setting made by the application is left alone.
-    cudaMemPool_t pool;
-    if (cudaDeviceGetDefaultMemPool(&pool, p->device) == cudaSuccess) {
-      uint64_t thr = 0;
-      if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr) == cudaSuccess && thr < (4ull << 30)) {
-        thr = 4ull << 30;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-      }
-    }
-    cudaGetLastError();
-  }
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->dirs, (size_t)p->npix * 4 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flag_count, kCtrlWords * sizeof(int));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_vjp_ctrl, kCtrlWords * sizeof(int));
@@ -184,6 +177,8 @@ extern "C" int64_t synax_plan_npix(const synax_plan* plan) { return plan ? plan-
 
 extern "C" synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]) {
   if (!plan) return fail(SYNAX_ERR_INVALID_ARG, "plan is NULL");
+  // in-flight calls on the caller's (non-blocking) streams may still read plan->path and the frequency table
+  CUDA_TRY(cudaDeviceSynchronize());
   if (!box_kpc) {   // back to the fixed [0, s_max]
     if (plan->path) { cudaFree(plan->path); plan->path = nullptr; }
     plan->s_max = plan->s_max_fixed; plan->delta = plan->s_max / (double)plan->n_los;
@@ -221,6 +216,18 @@ extern "C" synax_status synax_plan_set_option(synax_plan* plan, const char* key,
   } else if (!std::strcmp(key, "lanes")) {
     if (value != 0 && value != 1 && value != 8 && value != 32) return fail(SYNAX_ERR_INVALID_ARG, "lanes must be 0, 1, 8 or 32");
     plan->lanes = (int)value;
+  } else if (!std::strcmp(key, "pool_release_threshold_mb")) {
+    // Per-call scratch (constants, flag lists, block partials, the host entry points' staging buffers) comes from the
+    // device's stream-ordered pool.  Its default release threshold is 0: every stream synchronisation hands the memory
+    // back to the driver and the next call pays for mapping it again (hundreds of MB in the *_host calls: measured
+    // outliers of +10 ms per step at cfg 4).  This option raises the threshold of the DEVICE's default pool -- a
+    // process-wide setting, hence opt-in; a larger value already set by the application is left alone.
+    if (!(value >= 0) || value > 1.0e6) return fail(SYNAX_ERR_INVALID_ARG, "pool_release_threshold_mb must be in 0 .. 1e6");
+    cudaMemPool_t pool;
+    CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, plan->device));
+    uint64_t thr = 0, want = (uint64_t)value << 20;
+    CUDA_TRY(cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr));
+    if (thr < want) CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &want));
   } else {
     return fail(SYNAX_ERR_INVALID_ARG, "unknown option '%s'", key);
   }
@@ -237,7 +244,8 @@ extern "C" synax_status synax_plan_directions(const synax_plan* plan, double* ou
 extern "C" synax_status synax_plan_stats(const synax_plan* plan, int64_t out[2]) {
   if (!plan || !out) return fail(SYNAX_ERR_INVALID_ARG, "plan or out is NULL");
   out[0] = plan->launches;
-  out[1] = plan->h_flag_count[kCtrlMode] == kModeAllF64 ? plan->last_n_sl : plan->h_flag_count[kCtrlFlagCount];
+  out[1] = plan->h_flag_count[kCtrlMode] == kModeAllF64 ? plan->last_n_sl
+                                                             : plan->h_flag_count[kCtrlFlagCount] + plan->h_flag_count[kCtrlCountM];
   return SYNAX_OK;
 }
 
@@ -342,6 +350,51 @@ static int sm_count(int device) {
   return cached[device];
 }
 
+// Per-call scratch from the device's stream-ordered pool; everything handed out is given back (cudaFreeAsync on the
+// same stream) when the guard leaves scope, whatever path the call returns on.
+struct StreamScratch {
+  cudaStream_t st;
+  void* blocks[12];
+  int n = 0;
+  explicit StreamScratch(cudaStream_t s) : st(s) {}
+  StreamScratch(const StreamScratch&) = delete;
+  StreamScratch& operator=(const StreamScratch&) = delete;
+  ~StreamScratch() {
+    for (int i = n - 1; i >= 0; --i) cudaFreeAsync(blocks[i], st);
+  }
+  template <typename T>
+  cudaError_t get(T** out, size_t bytes) {
+    void* q = nullptr;
+    if (n >= 12) { *out = nullptr; return cudaErrorMemoryAllocation; }
+    const cudaError_t e = cudaMallocAsync(&q, bytes ? bytes : 1, st);
+    if (e == cudaSuccess) blocks[n++] = q;
+    *out = (T*)q;
+    return e;
+  }
+};
+
+// Per-batch constants of a call (prologue_kernel).  When a gridded n_e replaces the analytic disc, the bound on
+// |n_e B_LOS| that sizes the float64 chain's tiles (BatchConsts::tile_d) comes from max |ne_grid|, reduced on the device
+// first -- the aux n_e entries are ignored then and say nothing about the grid (synax.h).
+static synax_status run_prologue(const synax_plan* plan, const synax_model* model, int code, const float* params, int batch,
+                                 StreamScratch& scratch, BatchConsts** bc, BatchConstsD** bd, cudaStream_t st) {
+  CUDA_TRY(scratch.get(bc, sizeof(BatchConsts) * (size_t)batch));
+  CUDA_TRY(scratch.get(bd, sizeof(BatchConstsD) * (size_t)batch));
+  float* ne_max = nullptr;
+  if (model->ne_grid) {
+    const int64_t n = (int64_t)model->ne_n[0] * model->ne_n[1] * model->ne_n[2];
+    CUDA_TRY(scratch.get(&ne_max, sizeof(float)));
+    CUDA_TRY(cudaMemsetAsync(ne_max, 0, sizeof(float), st));
+    absmax_kernel<<<(unsigned)std::min<int64_t>((n + 1023) / 1024, 1184), 256, 0, st>>>(model->ne_grid, n, ne_max);
+    plan->launches++;
+  }
+  prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
+                                                      make_aux(model), plan->ft, plan->delta, ne_max, *bc, *bd);
+  plan->launches++;
+  CUDA_TRY(cudaGetLastError());
+  return SYNAX_OK;
+}
+
 extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
                                       int32_t batch, float* I, float* Q, float* U, void* cuda_stream) {
   int code = 0;
@@ -350,14 +403,12 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int64_t n_sl = plan->npix * batch;
+  StreamScratch scratch(st);
 
   BatchConsts* bc = nullptr;
   BatchConstsD* bd = nullptr;
-  CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
-  CUDA_TRY(cudaMallocAsync((void**)&bd, sizeof(BatchConstsD) * (size_t)batch, st));
-  prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
-                                                      make_aux(model), plan->ft, plan->delta, bc, bd);
-  plan->launches++;
+  stt = run_prologue(plan, model, code, params, batch, scratch, &bc, &bd, st);
+  if (stt != SYNAX_OK) return stt;
 
   ForwardArgs a;
   a.geo = make_geo(plan); a.bc = bc; a.bd = bd; a.batch = batch; a.I = I; a.Q = Q; a.U = U;
@@ -365,12 +416,11 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   a.sg_ne = make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l);
   a.sg_n0 = make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l);
   a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
+  a.append_count = plan->d_flag_count + kCtrlFlagCount; a.append_list = nullptr;
 
   if (code == kGridB) {
     synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, sm_count(plan->device),
                                    plan->d_flag_count, plan->h_flag_count, st, &plan->launches);
-    cudaFreeAsync(bc, st);
-    cudaFreeAsync(bd, st);
     if (gs != SYNAX_OK) return fail(gs, "grid forward failed: %s", cudaGetErrorString(cudaGetLastError()));
     return SYNAX_OK;
   }
@@ -388,21 +438,24 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   // sightlines" (hardly any flagged), "float64 Faraday chain for every sightline" (nearly all flagged) and "split":
   // classify_kernel sorts the sightlines into one list per chain (decide_forward_kernel).
   bool piloted = false, split_ok = false;
+  int* miss_list = nullptr;
   if (escalate) {
-    CUDA_TRY(cudaMallocAsync((void**)&a.flag_list, sizeof(int) * (size_t)n_sl, st));
+    CUDA_TRY(scratch.get(&a.flag_list, sizeof(int) * (size_t)n_sl));
+    a.append_list = a.flag_list;
     a.flag_S = (float)(plan->escalate_rad / (double)k_max);
     if (n_sl > 16384) {
       const int64_t stride = (n_sl / 8192) | 1;
       const int64_t n_pilot = (n_sl + stride - 1) / stride;
       const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
       SYNAX_DISPATCH_CODE(code, fwd_launch_pilot, pb, st, a, stride, n_pilot, ctrl);
-      // the split mode costs four more launches: only for calls long enough not to notice (cfg 1: 0.19 ms in all)
+      // the split mode costs a handful of extra launches: only for calls long enough not to notice (cfg 1: 0.19 ms in all)
       split_ok = n_sl >= 262144;
       if (split_ok) {
         decide_forward_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot);
-        CUDA_TRY(cudaMallocAsync((void**)&a.list_u, sizeof(int) * (size_t)n_sl, st));
+        CUDA_TRY(scratch.get(&a.list_u, sizeof(int) * (size_t)n_sl));
+        CUDA_TRY(scratch.get(&miss_list, sizeof(int) * (size_t)n_sl));
         a.count_u = ctrl + kCtrlCountU;
-        const unsigned cb = (unsigned)std::min<int64_t>((n_sl + kBlock - 1) / kBlock, (int64_t)sm_count(plan->device) * 16);
+        const unsigned cb = (unsigned)std::min<int64_t>((n_sl + kBlock - 1) / kBlock, (int64_t)sms * 16);
         SYNAX_DISPATCH_CODE(code, fwd_launch_classify, cb, st, a, ctrl);
         plan->launches += 3;
       } else {
@@ -423,43 +476,59 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     const int64_t full = (n_sl * lanes + kBlockD - 1) / kBlockD;
     return (unsigned)(use_list && run_when != 3 ? std::min<int64_t>(full, (int64_t)sms * 16 * 128 / kBlockD) : full);
   };
-  auto run_f64 = [&](int lanes, int run_when, bool use_list) {
+  auto run_f64 = [&](cudaStream_t on, int lanes, int run_when, int* list, int* count) {
     ForwardArgs pa = a;
     pa.run_when = run_when;
-    if (!use_list) pa.flag_list = nullptr;
+    pa.flag_list = list; pa.flag_count = count;
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       pa.f0 = f0;
-      SYNAX_DISPATCH_CODE(code, fwd_launch_f64, lanes, nf, blocks_for(lanes, use_list, run_when), st, pa, plan->ft);
+      SYNAX_DISPATCH_CODE(code, fwd_launch_f64, lanes, nf, blocks_for(lanes, list != nullptr, run_when), on, pa, plan->ft);
       plan->launches++;
       f0 += nf;
     }
   };
+  cudaError_t stream_err = cudaSuccess;
   if (fast) {
+    if (split_ok) {
+      // all-float64 / split: the float64-chain kernel (every sightline, or classify_kernel's flag list) runs on the plan's
+      // second stream beside the fp32 kernel over list_u; what the fp32 kernel's exact criterion still flags goes to a
+      // separate list (the flag list is being read) and is redone after the join.  Fork after classify_kernel.
+      stream_err = cudaEventRecord(plan->ev_fork, st);
+      if (stream_err == cudaSuccess) stream_err = cudaStreamWaitEvent(plan->aux, plan->ev_fork, 0);
+      if (stream_err != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward: stream fork failed: %s", cudaGetErrorString(stream_err));
+      run_f64(plan->aux, G, 3, a.flag_list, ctrl + kCtrlFlagCount);
+    }
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       a.f0 = f0;
       SYNAX_DISPATCH_CODE(code, fwd_launch_fast, false, G, nf, n_sl, st, a, plan->ft);
       plan->launches++;
       if (split_ok) {   // the same pass over list_u (exits at once unless the pilot chose the split mode)
-        SYNAX_DISPATCH_CODE(code, fwd_launch_fast, true, G, nf, n_sl, st, a, plan->ft);
+        ForwardArgs al = a;
+        al.append_count = ctrl + kCtrlCountM; al.append_list = miss_list;
+        SYNAX_DISPATCH_CODE(code, fwd_launch_fast, true, G, nf, n_sl, st, al, plan->ft);
         plan->launches++;
       }
       f0 += nf;
     }
-    if (escalate) {
-      run_f64(8, piloted ? 1 : 0, true);          // the flagged list, 8 lanes per sightline
-      if (piloted) run_f64(G, 3, true);           // or the long list of the split mode / every sightline (all-float64)
+    if (escalate) run_f64(st, 8, piloted ? 1 : 0, a.flag_list, ctrl + kCtrlFlagCount);   // fast-then-list: the flagged list, 8 lanes per sightline
+    if (split_ok) {
+      stream_err = cudaEventRecord(plan->ev_join, plan->aux);
+      if (stream_err == cudaSuccess) stream_err = cudaStreamWaitEvent(st, plan->ev_join, 0);
+      if (stream_err != cudaSuccess) {
+        cudaStreamSynchronize(plan->aux);   // join by hand so that the scratch is not freed under the second stream
+        return fail(SYNAX_ERR_CUDA, "forward: stream join failed: %s", cudaGetErrorString(stream_err));
+      }
+      run_f64(st, 8, 4, miss_list, ctrl + kCtrlCountM);
+    } else if (piloted) {
+      run_f64(st, G, 2, nullptr, ctrl + kCtrlFlagCount);   // short calls: every sightline when the pilot says all-float64
     }
   } else {
-    run_f64(G, 0, false);
+    run_f64(st, G, 0, nullptr, ctrl + kCtrlFlagCount);
   }
   cudaError_t e = cudaGetLastError();
   cudaMemcpyAsync(plan->h_flag_count, ctrl, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
-  if (escalate) cudaFreeAsync(a.flag_list, st);
-  if (a.list_u) cudaFreeAsync(a.list_u, st);
-  cudaFreeAsync(bc, st);
-  cudaFreeAsync(bd, st);
   if (e != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward launch failed: %s", cudaGetErrorString(e));
   return SYNAX_OK;
 }
@@ -472,13 +541,11 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   if (stt != SYNAX_OK) return stt;
   if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  StreamScratch scratch(st);
   BatchConsts* bc = nullptr;
   BatchConstsD* bd = nullptr;
-  CUDA_TRY(cudaMallocAsync((void**)&bc, sizeof(BatchConsts) * (size_t)batch, st));
-  CUDA_TRY(cudaMallocAsync((void**)&bd, sizeof(BatchConstsD) * (size_t)batch, st));
-  prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
-                                                      make_aux(model), plan->ft, plan->delta, bc, bd);
-  plan->launches++;
+  stt = run_prologue(plan, model, code, params, batch, scratch, &bc, &bd, st);
+  if (stt != SYNAX_OK) return stt;
   synax_status rs;
   if (code == kGridB)
     rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
@@ -490,8 +557,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
                       plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
                       dI, dQ, dU, grad, st, &plan->launches);
-  cudaFreeAsync(bc, st);
-  if (bd) cudaFreeAsync(bd, st);
+  if (rs == SYNAX_ERR_UNSUPPORTED) return fail(rs, "GRID_B vjp: n_los too large for the shared-memory hand-over (see synax.h)");
   if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));
   return SYNAX_OK;
 }
@@ -538,8 +604,9 @@ extern "C" synax_status synax_loglike_vjp(const synax_plan* plan, const synax_mo
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int64_t per_batch = (int64_t)plan->n_freq * plan->npix;
   const size_t count = (size_t)batch * (size_t)per_batch;
+  StreamScratch scratch(st);
   float* maps = nullptr;
-  CUDA_TRY(cudaMallocAsync((void**)&maps, 3 * count * sizeof(float), st));
+  CUDA_TRY(scratch.get(&maps, 3 * count * sizeof(float)));
   float* m[3] = {maps, maps + count, maps + 2 * count};
   synax_status rs = synax_forward(plan, model, params, batch, m[0], m[1], m[2], cuda_stream);
   if (rs == SYNAX_OK) {
@@ -560,7 +627,6 @@ extern "C" synax_status synax_loglike_vjp(const synax_plan* plan, const synax_mo
     if (e != cudaSuccess) rs = fail(SYNAX_ERR_CUDA, "loglike residual launch failed: %s", cudaGetErrorString(e));
     else rs = synax_vjp(plan, model, params, batch, cot[0], cot[1], cot[2], grad, cuda_stream);
   }
-  cudaFreeAsync(maps, st);
   return rs;
 }
 
@@ -613,7 +679,8 @@ extern "C" synax_status synax_forward_host(const synax_plan* plan, const synax_m
   const size_t pbytes = sizeof(float) * (size_t)model->n_params * (size_t)batch;
   const size_t mbytes = sizeof(float) * (size_t)batch * plan->n_freq * (size_t)plan->npix;
   float *dp = nullptr, *dm = nullptr;
-  CUDA_TRY(cudaMallocAsync((void**)&dp, pbytes, st));
+  StreamScratch scratch(st);
+  CUDA_TRY(scratch.get(&dp, pbytes));
   CUDA_TRY(cudaMemcpyAsync(dp, params, pbytes, cudaMemcpyHostToDevice, st));
   // Page-locked map buffers: the kernels store straight into them.  A map value is written exactly once, by the
   // thread that finishes its sightline, in 128-byte runs of adjacent pixels, and never read back -- posted writes
@@ -622,11 +689,10 @@ extern "C" synax_status synax_forward_host(const synax_plan* plan, const synax_m
   float *zI = pinned_alias(I), *zQ = pinned_alias(Q), *zU = pinned_alias(U);
   if (zI && zQ && zU) {
     synax_status rz = synax_forward(plan, model, dp, batch, zI, zQ, zU, cuda_stream);
-    cudaFreeAsync(dp, st);
     CUDA_TRY(cudaStreamSynchronize(st));
     return rz;
   }
-  CUDA_TRY(cudaMallocAsync((void**)&dm, 3 * mbytes, st));
+  CUDA_TRY(scratch.get(&dm, 3 * mbytes));
   float* dI = dm; float* dQ = dm + mbytes / sizeof(float); float* dU = dm + 2 * (mbytes / sizeof(float));
   synax_status rs = synax_forward(plan, model, dp, batch, dI, dQ, dU, cuda_stream);
   if (rs == SYNAX_OK) {
@@ -634,8 +700,6 @@ extern "C" synax_status synax_forward_host(const synax_plan* plan, const synax_m
     CUDA_TRY(cudaMemcpyAsync(Q, dQ, mbytes, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(U, dU, mbytes, cudaMemcpyDeviceToHost, st));
   }
-  cudaFreeAsync(dp, st);
-  cudaFreeAsync(dm, st);
   CUDA_TRY(cudaStreamSynchronize(st));
   return rs;
 }
@@ -651,9 +715,10 @@ extern "C" synax_status synax_vjp_host(const synax_plan* plan, const synax_model
   const size_t pbytes = sizeof(float) * (size_t)model->n_params * (size_t)batch;
   const size_t mcount = (size_t)batch * plan->n_freq * (size_t)plan->npix;
   float *dp = nullptr, *dg = nullptr, *dc = nullptr;
-  CUDA_TRY(cudaMallocAsync((void**)&dp, pbytes, st));
-  CUDA_TRY(cudaMallocAsync((void**)&dg, pbytes, st));
-  CUDA_TRY(cudaMallocAsync((void**)&dc, 3 * mcount * sizeof(float), st));
+  StreamScratch scratch(st);
+  CUDA_TRY(scratch.get(&dp, pbytes));
+  CUDA_TRY(scratch.get(&dg, pbytes));
+  CUDA_TRY(scratch.get(&dc, 3 * mcount * sizeof(float)));
   CUDA_TRY(cudaMemcpyAsync(dp, params, pbytes, cudaMemcpyHostToDevice, st));
   const float* src[3] = {dI, dQ, dU};
   const float* dev[3] = {nullptr, nullptr, nullptr};
@@ -664,7 +729,6 @@ extern "C" synax_status synax_vjp_host(const synax_plan* plan, const synax_model
     }
   synax_status rs = synax_vjp(plan, model, dp, batch, dev[0], dev[1], dev[2], dg, cuda_stream);
   if (rs == SYNAX_OK) CUDA_TRY(cudaMemcpyAsync(grad, dg, pbytes, cudaMemcpyDeviceToHost, st));
-  cudaFreeAsync(dp, st); cudaFreeAsync(dg, st); cudaFreeAsync(dc, st);
   CUDA_TRY(cudaStreamSynchronize(st));
   return rs;
 }

@@ -117,6 +117,7 @@ struct BatchConsts {
   // VJP only
   float dlnc_dalpha[kMaxFreq];  // d ln c_f / d alpha
   float dpi_dalpha_over_pi;     // d ln Pi / d alpha
+  float dlnA_dalpha;            // d ln c_f / d alpha + ln(nu_f) / 2 (the frequency-independent part)
   // uniform model
   float uB[3], uN0, une;
 };
@@ -126,6 +127,7 @@ struct FreqTab {
   float k_rad[kMaxFreq];    // 2 lambda_f^2 K_F Delta : Faraday angle (rad) per unit sum(n_e B_LOS)
   double k_turn[kMaxFreq];  // the same / (2 pi), float64, for exact turn reduction of large offsets
   double freq[kMaxFreq];
+  float ln_nu[kMaxFreq];    // ln(nu_f / Hz)
 };
 
 // the table of one frequency pass: entries f0 .. f0 + n - 1 moved to the front, so that the kernels index it with
@@ -134,7 +136,7 @@ static inline FreqTab shift_freqs(const FreqTab& ft, int f0) {
   FreqTab o = ft;
   for (int f = 0; f < kMaxFreq; ++f) {
     const int g = f0 + f < kMaxFreq ? f0 + f : kMaxFreq - 1;
-    o.k_rad[f] = ft.k_rad[g]; o.k_turn[f] = ft.k_turn[g]; o.freq[f] = ft.freq[g];
+    o.k_rad[f] = ft.k_rad[g]; o.k_turn[f] = ft.k_turn[g]; o.freq[f] = ft.freq[g]; o.ln_nu[f] = ft.ln_nu[g];
   }
   return o;
 }
@@ -225,7 +227,8 @@ struct AnalyticAux {
   float lr;                // ln(rho/8)
   float sp, cp, sc, cc;    // sin/cos psi, sin/cos chi
   float t;                 // tanh(z / 1 kpc)
-  float A;                 // b0 exp(-(rho-8)/h_b) inside the annulus, else 0
+  float A;                 // exp(-(rho-8)/h_b) inside the annulus, else 0 (unit amplitude: B_disc = b0 A [...])
+  float N0u, neu;          // N_0 / n0 and n_e / ne0 (unit amplitudes)
   float u, L, R;           // halo: u, 1/(1+u^2), (rho/r_h) exp(1-rho/r_h)
   float thz, thez;         // tanh(z/h_z), tanh(z/h_ez)
 };
@@ -270,10 +273,11 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
     const float dr = a.rho - 8.0f;
     rad = kAcc ? exp2_fma(fmaf(P.k_hb, dr, P.k_hb_lo * dr)) : mufu_ex2(P.k_hb * dr);
   }
-  a.A = inside ? P.p[0] * rad : 0.0f;
-  const float Brho = a.A * a.cp * a.cc;
-  float Bphi = a.A * a.sp * a.cc;
-  const float Bz = a.A * a.sc;
+  a.A = inside ? rad : 0.0f;
+  const float Ab = P.p[0] * a.A;
+  const float Brho = Ab * a.cp * a.cc;
+  float Bphi = Ab * a.sp * a.cc;
+  const float Bz = Ab * a.sc;
   if (kHalo) {  // toroidal halo, S:App.C
     a.u = (az - P.p[6]) * P.inv_wh;
     const float q = a.rho * P.inv_rh;
@@ -296,19 +300,22 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
   const float ez = mufu_ex2(P.k_hz * az);
   const float dz = 1.0f + ez;
   const float iz = mufu_rcp(dz * dz);
-  S.N0 = 4.0f * P.p[9] * mufu_ex2(P.k_hr * a.rho) * ez * iz;
+  a.N0u = 4.0f * mufu_ex2(P.k_hr * a.rho) * ez * iz;
+  S.N0 = P.p[9] * a.N0u;
   a.thz = copysignf((1.0f - ez) * dz * iz, z);                  // tanh = (1-e)/(1+e)
   if (kAcc) {
     const float ee = exp2_fma(P.k_hez * az);
     const float de = 1.0f + ee;
     const float ie = rcp_nr(de * de);
-    S.ne = 4.0f * P.p[13] * exp2_fma(fmaf(P.k_her, a.rho, P.k_her_lo * a.rho)) * ee * ie;
+    a.neu = 4.0f * exp2_fma(fmaf(P.k_her, a.rho, P.k_her_lo * a.rho)) * ee * ie;
+    S.ne = P.p[13] * a.neu;
     a.thez = copysignf((1.0f - ee) * de * ie, z);
   } else {
     const float ee = mufu_ex2(P.k_hez * az);
     const float de = 1.0f + ee;
     const float ie = mufu_rcp(de * de);
-    S.ne = 4.0f * P.p[13] * mufu_ex2(P.k_her * a.rho) * ee * ie;
+    a.neu = 4.0f * mufu_ex2(P.k_her * a.rho) * ee * ie;
+    S.ne = P.p[13] * a.neu;
     a.thez = copysignf((1.0f - ee) * de * ie, z);
   }
 }

@@ -101,7 +101,11 @@ struct ForwardArgs {
   ScalarGridDesc sg_ne, sg_n0;  // gridded n_e / N_0 replacing the analytic discs (DISC4, GRID_B), g == nullptr: unused
   const int* mode;        // device: kModeFastThenList / kModeAllF64 / kModeSplit (written by decide_kernel), or null
   int run_when;           // forward_f64_kernel: 0 always, 1 only in mode fast-then-list (flag list), 2 only in mode
-                          // all-float64 (every sightline), 3 in both all-float64 (every sightline) and split (flag list)
+                          // all-float64 (every sightline), 3 in both all-float64 (every sightline) and split (flag list),
+                          // 4 only in mode split (flag list)
+  int* append_count;      // where forward_kernel appends the sightlines its exact criterion flags: the flag list itself
+  int* append_list;       // (fast-then-list), or a separate "missed" list in split mode, where the float64 kernel reads
+                          // the flag list concurrently on the plan's second stream
   int* list_u;            // kModeSplit: sightlines classify_kernel left to the fp32 kernel (count in ctrl[kCtrlCountU])
   const int* count_u;
 };
@@ -109,7 +113,7 @@ struct ForwardArgs {
 // kModeSplit: classify_kernel sorts the sightlines by an estimate of the round-off scale into the flag list (float64
 // chain) and list_u (fp32 kernel, whose exact criterion still appends what the estimate missed to the flag list).
 enum { kModeFastThenList = 0, kModeAllF64 = 1, kModeSplit = 2 };
-enum { kCtrlFlagCount = 0, kCtrlPilotFlagged = 1, kCtrlMode = 2, kCtrlCountU = 3, kCtrlWords = 4 };
+enum { kCtrlFlagCount = 0, kCtrlPilotFlagged = 1, kCtrlMode = 2, kCtrlCountU = 3, kCtrlCountM = 4, kCtrlWords = 8 };
 
 // Estimate of one lane's share of the round-off scale  sum_n |n_e| (|B_LOS| + |B_N| + |B_E|)  over samples [n0, n1):
 // every 16th sample (all of them for short chunks), MUFU-grade fp32 chain; the caller sums the lanes of the
@@ -269,8 +273,8 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
     }
     if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
-      const int k = atomicAdd(A.flag_count, 1);
-      A.flag_list[k] = (int)sl;
+      const int k = atomicAdd(A.append_count, 1);
+      A.append_list[k] = (int)sl;
     }
   }
 }
@@ -299,6 +303,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
   if (A.run_when == 1 && *A.mode != kModeFastThenList) return;
   if (A.run_when == 2 && *A.mode != kModeAllF64) return;
   if (A.run_when == 3 && *A.mode == kModeFastThenList) return;
+  if (A.run_when == 4 && *A.mode != kModeSplit) return;
   const bool use_list = A.flag_list && (A.run_when == 3 ? *A.mode == kModeSplit : A.run_when != 2);
   const int64_t count = use_list ? (int64_t)(*A.flag_count) : n_sl;
   const int C = (A.geo.n_los + G - 1) / G;

@@ -65,8 +65,6 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   a.geo = geo; a.bc = bc; a.bd = bd; a.grid = make_grid_desc(m, grid); a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_freq_total = ft.n_freq; a.dI = dI; a.dQ = dQ; a.dU = dU;
   const int64_t n_nodes = (int64_t)m->nx * m->ny * m->nz;
-  if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
-  if (cudaMemsetAsync(a.grad4, 0, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_CUDA;
   int cl = 0;
   while ((32 << cl) < geo.n_los) ++cl;
   a.chunk_log2 = cl;
@@ -75,6 +73,11 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   a.mode = precision; a.flag_S = (float)(escalate_rad / (double)k_max);
   const size_t smem = (size_t)(kBlock / 32) * 3 * 32 * ((1u << cl) + 1) * sizeof(float);
   if (smem > 200 * 1024) return SYNAX_ERR_UNSUPPORTED;  // n_los too large for the shared-memory hand-over
+  if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
+  if (cudaMemsetAsync(a.grad4, 0, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) {
+    cudaFreeAsync(a.grad4, st);
+    return SYNAX_ERR_CUDA;
+  }
   const unsigned blocks = (unsigned)min((int64_t)sms * 8, (geo.npix * 32 + kBlock - 1) / kBlock);
   for (int f0 = 0; f0 < ft.n_freq;) {
     const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);

@@ -77,9 +77,19 @@ __global__ void box_path_kernel(const double* __restrict__ dirs, int64_t count, 
 // ------------------------------------------------------------------------------------------------
 struct AuxHost { float v[7]; };  // C0, h_r, h_z, alpha, ne0, h_er, h_ez
 
+// max |g[i]| of a non-negative-comparable float array into *out (zero on entry): non-negative floats order like ints
+__global__ void absmax_kernel(const float* __restrict__ g, int64_t n, float* __restrict__ out) {
+  float m = 0.f;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) m = fmaxf(m, fabsf(__ldg(g + i)));
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+  if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMax(reinterpret_cast<int*>(out), __float_as_int(m));
+}
+
+// ne_max: device scalar max |ne_grid| when a gridded n_e replaces the analytic disc, else null
 __global__ void prologue_kernel(int code, const float* __restrict__ params, int n_params, int batch,
-                                AuxHost aux, FreqTab ft, double delta, BatchConsts* __restrict__ out,
-                                BatchConstsD* __restrict__ outd) {
+                                AuxHost aux, FreqTab ft, double delta, const float* __restrict__ ne_max,
+                                BatchConsts* __restrict__ out, BatchConstsD* __restrict__ outd) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= batch) return;
   BatchConsts c;
@@ -129,6 +139,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
   const double dlnA = -0.5 * log(w) + 0.5 * log(2.0) - 1.0 / (alpha + 1.0) +
                       0.25 * digamma_d(alpha * 0.25 - 1.0 / 12.0) + 0.25 * digamma_d(alpha * 0.25 + 19.0 / 12.0) +
                       0.5 * log(1.0e-6);
+  c.dlnA_dalpha = (float)dlnA;
   for (int f = 0; f < kMaxFreq; ++f) {
     if (f < ft.n_freq) {
       const double nu = ft.freq[f];
@@ -151,7 +162,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
       double bmax = fabs(p[0]);
       if (code == kStack16) bmax = 0.6 * fabs((double)c.sp[0]) + 0.3 * fabs((double)c.sp[4]) + 0.1 * fabs((double)c.sp[8]) + 0.3 * fabs((double)c.sp[12]);
       if (code == kAnalyticFull) bmax = bmax * fmax(exp(5.0 / p[4]), exp(-12.0 / p[4])) + fabs(p[5]);
-      gmax = fabs(p[13]) * bmax;
+      gmax = (ne_max ? (double)*ne_max : fabs(p[13])) * bmax;
     }
     double kmax = 0.0;
     for (int f = 0; f < ft.n_freq; ++f) kmax = fmax(kmax, (double)ft.k_rad[f]);

@@ -11,171 +11,217 @@
 namespace synax {
 
 // ------------------------------------------------------------------------------------------------
-// Per-lane gradient accumulators.  Every parameter gradient is  acc1_j + Tw * acc2_j  where acc2
-// collects the unweighted Faraday terms h_mj = d(n_e B_LOS)_m / d theta_j  and acc1 the direct terms
-// minus (P_m - 1/2 Sbar_m) h_mj; Tw = T - P_off is known only after the sweep.
+// Per-lane gradient accumulators.  The Faraday-coupled part of a parameter gradient is
+//   sum_m gbar_m h_mj,   gbar_m = sum_{n>m} Sbar_n + Sbar_m / 2  (transposed half-cell scan, S:App.D.2),
+// h_mj = d(n_e B_LOS)_m / d theta_j.  Swapping the order of summation,
+//   sum_m gbar_m h_mj = sum_n Sbar_n (H_{j,n-1} + h_nj / 2),   H_{j,n} = sum_{m<=n} h_mj,
+// which one forward-order sweep evaluates with a running prefix H_j per parameter and no subtraction of large
+// terms (the earlier T - P_m form, S:App.D.4, lost the w_h component to cancellation on under-resolved
+// sightlines: 1.1e-2 at nside 16 x 256 samples with the box clip).
+// Amplitude parameters (b0, B_h, n0, ne0, ...) are accumulated with the UNIT-amplitude field, so their derivative
+// needs no division by the parameter and stays finite when the amplitude is exactly zero.
 // ------------------------------------------------------------------------------------------------
-template <int CODE>
-struct GradAcc;
-
 // rho/phi/z components of a Cartesian vector at a point with unit vectors rho_hat = (xr, yr, 0)
-__device__ __forceinline__ void to_cyl(float vx, float vy, float xr, float yr, float& vr, float& vp) {
-  vr = fmaf(vx, xr, vy * yr);
-  vp = fmaf(vy, xr, -vx * yr);
+__device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
+
+template <typename R>
+__device__ __forceinline__ void to_cyl(R vx, R vy, R xr, R yr, R& vr, R& vp) {
+  vr = fma_r(vx, xr, vy * yr);
+  vp = fma_r(vy, xr, -vx * yr);
 }
 
-template <bool kFull>
+// g += d1 + Sbar * H (H = prefix over the earlier samples), then H += d2
+template <typename R>
+__device__ __forceinline__ void prefix_update(R& g, R& H, R Sbar, R d1, R d2) {
+  g = fma_r(Sbar, H, g + d1);
+  H += d2;
+}
+
+// lanes of a group own consecutive chunks: add Sbar-total-of-this-lane x (prefix H of the preceding lanes)
+template <int G, typename R>
+__device__ __forceinline__ void prefix_combine(R& g, R H, R Pl, int lane_in_group) {
+  if (G > 1) g = fma_r((R)group_exclusive_scan<G>((double)H, lane_in_group), Pl, g);
+}
+
+// R = float (the fp32 kernels) or double (the all-float64 kernels of synax_dd.cuh); P, T, a, S are the matching structs
+template <bool kFull, typename R = float>
 struct AnalyticGrad {
   static constexpr int NB = kFull ? 9 : 4;
-  float b1[NB], b2[NB];      // B parameters: functional applied to V1 / V2
-  float n1[3];               // CR density parameters (direct only)
-  float e1[3], e2[3];        // n_e parameters
+  R g[NB], H[NB];        // B parameters (unit amplitudes)
+  R n1[3];               // CR density parameters (direct only)
+  R ge[3], He[3];        // n_e parameters
   __device__ __forceinline__ void zero() {
 #pragma unroll
-    for (int j = 0; j < NB; ++j) { b1[j] = 0.f; b2[j] = 0.f; }
+    for (int j = 0; j < NB; ++j) { g[j] = (R)0.0; H[j] = (R)0.0; }
 #pragma unroll
-    for (int j = 0; j < 3; ++j) { n1[j] = 0.f; e1[j] = 0.f; e2[j] = 0.f; }
+    for (int j = 0; j < 3; ++j) { n1[j] = (R)0.0; ge[j] = (R)0.0; He[j] = (R)0.0; }
   }
-  // V1 = BbarN e_N + BbarE e_E - wgt ne n ; V2 = ne n ; MK = N0bar * N0 ; h-terms for n_e
-  __device__ __forceinline__ void add(const BatchConsts& P, const Triad& T, const AnalyticAux& a, const SampleF& S,
-                                      float z, float BNb, float BEb, float wgt, float MK) {
-    const float wn = wgt * S.ne;
-    const float v1x = fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, -wn * T.nx));
-    const float v1y = fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, -wn * T.ny));
-    const float v1z = fmaf(BNb, T.eNz, -wn * T.nz);
-    float v1r, v1p, nr, np;
+  // V1 = BbarN e_N + BbarE e_E + Sbar/2 ne n ; V2 = ne n ; MKu = N0bar * N0 / n0 ; a.A, a.N0u, a.neu: unit amplitudes
+  template <typename PT, typename TT, typename AT, typename ST>
+  __device__ __forceinline__ void add(const PT& P, const TT& T, const AT& a, const ST& S,
+                                      R z, R BNb, R BEb, R Sbar, R MKu) {
+    const R hs = (R)0.5 * Sbar * S.ne;
+    const R v1x = fma_r(BNb, T.eNx, fma_r(BEb, T.eEx, hs * T.nx));
+    const R v1y = fma_r(BNb, T.eNy, fma_r(BEb, T.eEy, hs * T.ny));
+    const R v1z = fma_r(BNb, T.eNz, hs * T.nz);
+    R v1r, v1p, nr, np;
     to_cyl(v1x, v1y, a.xr, a.yr, v1r, v1p);
     to_cyl(T.nx, T.ny, a.xr, a.yr, nr, np);
-    const float v2r = S.ne * nr, v2p = S.ne * np, v2z = S.ne * T.nz;
-    // disc: B = A [cp cc rho_hat + sp cc phi_hat + sc z_hat]
-    const float Acc = a.A * a.cc;
+    const R v2r = S.ne * nr, v2p = S.ne * np, v2z = S.ne * T.nz;
+    // disc: B = b0 A [cp cc rho_hat + sp cc phi_hat + sc z_hat], A = exp(-(rho-8)/h_b) inside the annulus
+    const R Acc = a.A * a.cc, Asc = a.A * a.sc;
     {
-      const float d1 = fmaf(Acc, fmaf(a.cp, v1r, a.sp * v1p), a.A * a.sc * v1z);  // B_disc . V1
-      const float d2 = fmaf(Acc, fmaf(a.cp, v2r, a.sp * v2p), a.A * a.sc * v2z);
-      b1[0] += d1; b2[0] += d2;                                                    // * 1/b0 at the end
-      const float p1 = Acc * fmaf(a.cp, v1p, -a.sp * v1r);                        // dB/dpsi0 . V
-      const float p2 = Acc * fmaf(a.cp, v2p, -a.sp * v2r);
-      b1[1] += p1; b2[1] += p2;
-      b1[2] = fmaf(a.lr, p1, b1[2]); b2[2] = fmaf(a.lr, p2, b2[2]);
-      const float tA = a.t * a.A;
-      b1[3] = fmaf(tA, fmaf(a.cc, v1z, -a.sc * fmaf(a.cp, v1r, a.sp * v1p)), b1[3]);
-      b2[3] = fmaf(tA, fmaf(a.cc, v2z, -a.sc * fmaf(a.cp, v2r, a.sp * v2p)), b2[3]);
+      const R al1 = fma_r(a.cp, v1r, a.sp * v1p), al2 = fma_r(a.cp, v2r, a.sp * v2p);
+      const R d1 = fma_r(Acc, al1, Asc * v1z), d2 = fma_r(Acc, al2, Asc * v2z);   // (B_disc / b0) . V
+      prefix_update(g[0], H[0], Sbar, d1, d2);
+      const R p1 = Acc * fma_r(a.cp, v1p, -a.sp * v1r);                          // (dB/dpsi0) / b0 . V
+      const R p2 = Acc * fma_r(a.cp, v2p, -a.sp * v2r);
+      prefix_update(g[1], H[1], Sbar, p1, p2);
+      prefix_update(g[2], H[2], Sbar, a.lr * p1, a.lr * p2);
+      const R c1 = a.t * fma_r(Acc, v1z, -Asc * al1), c2 = a.t * fma_r(Acc, v2z, -Asc * al2);
+      prefix_update(g[3], H[3], Sbar, c1, c2);
       if (kFull) {
-        const float dr = a.rho - 8.0f;
-        b1[4] = fmaf(dr, d1, b1[4]); b2[4] = fmaf(dr, d2, b2[4]);                 // * 1/h_b^2
+        const R dr = a.rho - (R)8.0;
+        prefix_update(g[4], H[4], Sbar, dr * d1, dr * d2);                          // * b0 / h_b^2
       }
     }
     if (kFull) {  // halo: B_h L R phi_hat
-      const float LR = a.L * a.R;
-      b1[5] = fmaf(LR, v1p, b1[5]); b2[5] = fmaf(LR, v2p, b2[5]);
-      const float RuL2 = a.R * a.u * a.L * a.L;
-      b1[6] = fmaf(RuL2, v1p, b1[6]); b2[6] = fmaf(RuL2, v2p, b2[6]);             // * 2 B_h / w_h
-      const float q = LR * fmaf(a.rho, P.inv_rh, -1.0f);
-      b1[7] = fmaf(q, v1p, b1[7]); b2[7] = fmaf(q, v2p, b2[7]);                   // * B_h / r_h
-      const float Ru2L2 = RuL2 * a.u;
-      b1[8] = fmaf(Ru2L2, v1p, b1[8]); b2[8] = fmaf(Ru2L2, v2p, b2[8]);           // * 2 B_h / w_h
+      const R LR = a.L * a.R;
+      prefix_update(g[5], H[5], Sbar, LR * v1p, LR * v2p);
+      const R RuL2 = a.R * a.u * a.L * a.L;
+      prefix_update(g[6], H[6], Sbar, RuL2 * v1p, RuL2 * v2p);                      // * 2 B_h / w_h
+      const R q = LR * fma_r(a.rho, P.inv_rh, (R)-1.0);
+      prefix_update(g[7], H[7], Sbar, q * v1p, q * v2p);                            // * B_h / r_h
+      const R Ru2L2 = RuL2 * a.u;
+      prefix_update(g[8], H[8], Sbar, Ru2L2 * v1p, Ru2L2 * v2p);                    // * 2 B_h / w_h
     }
     if (kFull) {
       // N_0 = n0 exp(-rho/h_r) sech^2(z/h_z):  dN0/dn0 = N0/n0, /dh_r = N0 rho/h_r^2, /dh_z = N0 2 tanh(z/h_z) z/h_z^2
-      n1[0] += MK; n1[1] = fmaf(MK, a.rho, n1[1]); n1[2] = fmaf(MK * a.thz, z, n1[2]);
-      const float h = S.ne * S.Bpar;  // d(ne Bpar)/d ln ne
-      const float hw = -wgt * h;
-      e1[0] += hw; e1[1] = fmaf(hw, a.rho, e1[1]); e1[2] = fmaf(hw * a.thez, z, e1[2]);
-      e2[0] += h; e2[1] = fmaf(h, a.rho, e2[1]); e2[2] = fmaf(h * a.thez, z, e2[2]);
+      n1[0] += MKu; n1[1] = fma_r(MKu, a.rho, n1[1]); n1[2] = fma_r(MKu * a.thz, z, n1[2]);
+      const R h = T.scalef * a.neu * S.Bpar;   // d(ne Bpar Delta_i/Delta) / d ne0
+      const R hh = (R)0.5 * Sbar * h;
+      prefix_update(ge[0], He[0], Sbar, hh, h);
+      prefix_update(ge[1], He[1], Sbar, hh * a.rho, h * a.rho);
+      const R tz = a.thez * z;
+      prefix_update(ge[2], He[2], Sbar, hh * tz, h * tz);
+    }
+  }
+  template <int G>
+  __device__ __forceinline__ void combine(R Pl, int lane_in_group) {
+#pragma unroll
+    for (int j = 0; j < NB; ++j) prefix_combine<G, R>(g[j], H[j], Pl, lane_in_group);
+    if (kFull) {
+#pragma unroll
+      for (int j = 0; j < 3; ++j) prefix_combine<G, R>(ge[j], He[j], Pl, lane_in_group);
     }
   }
   // out[0..15] in canonical order (alpha handled by the caller)
-  __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
-    float g[NB];
-#pragma unroll
-    for (int j = 0; j < NB; ++j) g[j] = fmaf(Tw, b2[j], b1[j]);
-    out[0] = g[0] / P.p[0];
-    out[1] = g[1]; out[2] = g[2]; out[3] = g[3];
+  template <typename PT>
+  __device__ __forceinline__ void finish(const PT& P, R* out) {
+    const R b0 = P.p[0];
+    out[0] = g[0];
+    out[1] = b0 * g[1]; out[2] = b0 * g[2]; out[3] = b0 * g[3];
     if (kFull) {
-      out[4] = g[4] / (P.p[4] * P.p[4]);
+      out[4] = b0 * g[4] / (P.p[4] * P.p[4]);
       out[5] = g[5];
-      out[6] = g[6] * 2.0f * P.p[5] * P.inv_wh;
+      out[6] = g[6] * (R)2.0 * P.p[5] * P.inv_wh;
       out[7] = g[7] * P.p[5] * P.inv_rh;
-      out[8] = g[8] * 2.0f * P.p[5] * P.inv_wh;
-      out[9] = n1[0] / P.p[9];
-      out[10] = n1[1] / (P.p[10] * P.p[10]);
-      out[11] = n1[2] * 2.0f / (P.p[11] * P.p[11]);
-      const float e0 = fmaf(Tw, e2[0], e1[0]), e1v = fmaf(Tw, e2[1], e1[1]), e2v = fmaf(Tw, e2[2], e1[2]);
-      out[13] = e0 / P.p[13];
-      out[14] = e1v / (P.p[14] * P.p[14]);
-      out[15] = e2v * 2.0f / (P.p[15] * P.p[15]);
+      out[8] = g[8] * (R)2.0 * P.p[5] * P.inv_wh;
+      out[9] = n1[0];
+      out[10] = P.p[9] * n1[1] / (P.p[10] * P.p[10]);
+      out[11] = P.p[9] * n1[2] * (R)2.0 / (P.p[11] * P.p[11]);
+      out[13] = ge[0];
+      out[14] = P.p[13] * ge[1] / (P.p[14] * P.p[14]);
+      out[15] = P.p[13] * ge[2] * (R)2.0 / (P.p[15] * P.p[15]);
     }
   }
 };
 
+template <typename R = float>
 struct UniformGrad {
-  float b1[3], b2[3], n1, e1, e2;
+  R g[3], H[3], n1, ge, He;
   __device__ __forceinline__ void zero() {
-    for (int j = 0; j < 3; ++j) { b1[j] = 0.f; b2[j] = 0.f; }
-    n1 = e1 = e2 = 0.f;
+    for (int j = 0; j < 3; ++j) { g[j] = (R)0.0; H[j] = (R)0.0; }
+    n1 = ge = He = (R)0.0;
   }
-  __device__ __forceinline__ void add(const Triad& T, const SampleF& S, float BNb, float BEb, float wgt, float MK) {
-    const float wn = wgt * S.ne;
-    b1[0] += fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, -wn * T.nx));
-    b1[1] += fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, -wn * T.ny));
-    b1[2] += fmaf(BNb, T.eNz, -wn * T.nz);
-    b2[0] += S.ne * T.nx; b2[1] += S.ne * T.ny; b2[2] += S.ne * T.nz;
-    n1 += MK;                         // * 1/N0
-    e1 -= wgt * T.scalef * S.Bpar; e2 += T.scalef * S.Bpar;  // d(scale ne Bpar)/d ne = scale Bpar (S.ne carries scale)
+  // wK = N0bar (the cotangent of N0 itself: M K / N0)
+  template <typename TT, typename ST>
+  __device__ __forceinline__ void add(const TT& T, const ST& S, R BNb, R BEb, R Sbar, R wK) {
+    const R hs = (R)0.5 * Sbar * S.ne;
+    prefix_update(g[0], H[0], Sbar, fma_r(BNb, T.eNx, fma_r(BEb, T.eEx, hs * T.nx)), S.ne * T.nx);
+    prefix_update(g[1], H[1], Sbar, fma_r(BNb, T.eNy, fma_r(BEb, T.eEy, hs * T.ny)), S.ne * T.ny);
+    prefix_update(g[2], H[2], Sbar, fma_r(BNb, T.eNz, hs * T.nz), S.ne * T.nz);
+    n1 += wK;
+    const R h = T.scalef * S.Bpar;   // d(scale ne Bpar)/d ne = scale Bpar (S.ne carries scale)
+    prefix_update(ge, He, Sbar, (R)0.5 * Sbar * h, h);
   }
-  __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
-    for (int j = 0; j < 3; ++j) out[j] = fmaf(Tw, b2[j], b1[j]);
-    out[3] = n1 / P.uN0;
-    out[4] = fmaf(Tw, e2, e1);
+  template <int G>
+  __device__ __forceinline__ void combine(R Pl, int lane_in_group) {
+    for (int j = 0; j < 3; ++j) prefix_combine<G, R>(g[j], H[j], Pl, lane_in_group);
+    prefix_combine<G, R>(ge, He, Pl, lane_in_group);
+  }
+  template <typename PT>
+  __device__ __forceinline__ void finish(const PT& P, R* out) {
+    for (int j = 0; j < 3; ++j) out[j] = g[j];
+    out[3] = n1;
+    out[4] = ge;
   }
 };
 
 // STACK16 (Eq.(16)): (b0, psi0, psi1, chi0) of the four stacked spirals.  The cotangent of B_k is the
-// un-permuted total cotangent (the weight w_k is folded into the amplitude A, as in eval_stack16_f32).
+// un-permuted total cotangent; amplitudes are accumulated per unit b0_k (weight w_k and annulus mask only).
+template <typename R = float>
 struct StackGrad {
-  float b1[16], b2[16];
+  R g[16], H[16];
   __device__ __forceinline__ void zero() {
 #pragma unroll
-    for (int j = 0; j < 16; ++j) { b1[j] = 0.f; b2[j] = 0.f; }
+    for (int j = 0; j < 16; ++j) { g[j] = (R)0.0; H[j] = (R)0.0; }
   }
-  __device__ __forceinline__ void add(const BatchConsts& P, const Triad& T, const StackAux& a, const SampleF& S,
-                                      float BNb, float BEb, float wgt) {
-    const float wn = wgt * S.ne;
-    const float v1[3] = {fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, -wn * T.nx)), fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, -wn * T.ny)),
-                         fmaf(BNb, T.eNz, -wn * T.nz)};
-    const float v2[3] = {S.ne * T.nx, S.ne * T.ny, S.ne * T.nz};
+  template <typename PT, typename TT, typename AT, typename ST>
+  __device__ __forceinline__ void add(const PT& P, const TT& T, const AT& a, const ST& S,
+                                      R BNb, R BEb, R Sbar) {
+    const R hs = (R)0.5 * Sbar * S.ne;
+    const R v1[3] = {fma_r(BNb, T.eNx, fma_r(BEb, T.eEx, hs * T.nx)), fma_r(BNb, T.eNy, fma_r(BEb, T.eEy, hs * T.ny)),
+                         fma_r(BNb, T.eNz, hs * T.nz)};
+    const R v2[3] = {S.ne * T.nx, S.ne * T.ny, S.ne * T.nz};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      float u1[3], u2[3];
+      R u1[3], u2[3];
 #pragma unroll
       for (int c = 0; c < 3; ++c) { u1[stack_src(k, c)] = v1[c]; u2[stack_src(k, c)] = v2[c]; }
-      float u1r, u1p, u2r, u2p;
+      R u1r, u1p, u2r, u2p;
       to_cyl(u1[0], u1[1], a.xr, a.yr, u1r, u1p);
       to_cyl(u2[0], u2[1], a.xr, a.yr, u2r, u2p);
-      const float A = a.mask * stack_w(k) * P.sp[4 * k];
-      const float Acc = A * a.cc[k], Asc = A * a.sc[k];
-      const float h1 = fmaf(a.cp[k], u1r, a.sp[k] * u1p), h2 = fmaf(a.cp[k], u2r, a.sp[k] * u2p);
-      b1[4 * k] += fmaf(Acc, h1, Asc * u1[2]);                       // B_k . V  (* 1/b0 at the end)
-      b2[4 * k] += fmaf(Acc, h2, Asc * u2[2]);
-      const float p1 = Acc * fmaf(a.cp[k], u1p, -a.sp[k] * u1r), p2 = Acc * fmaf(a.cp[k], u2p, -a.sp[k] * u2r);
-      b1[4 * k + 1] += p1; b2[4 * k + 1] += p2;
-      b1[4 * k + 2] = fmaf(a.lr, p1, b1[4 * k + 2]); b2[4 * k + 2] = fmaf(a.lr, p2, b2[4 * k + 2]);
-      const float tA = a.t * A;
-      b1[4 * k + 3] = fmaf(tA, fmaf(a.cc[k], u1[2], -a.sc[k] * h1), b1[4 * k + 3]);
-      b2[4 * k + 3] = fmaf(tA, fmaf(a.cc[k], u2[2], -a.sc[k] * h2), b2[4 * k + 3]);
+      const R A = a.mask * (R)stack_w(k);
+      const R Acc = A * a.cc[k], Asc = A * a.sc[k];
+      const R h1 = fma_r(a.cp[k], u1r, a.sp[k] * u1p), h2 = fma_r(a.cp[k], u2r, a.sp[k] * u2p);
+      prefix_update(g[4 * k], H[4 * k], Sbar, fma_r(Acc, h1, Asc * u1[2]), fma_r(Acc, h2, Asc * u2[2]));   // (B_k / b0_k) . V
+      const R p1 = Acc * fma_r(a.cp[k], u1p, -a.sp[k] * u1r), p2 = Acc * fma_r(a.cp[k], u2p, -a.sp[k] * u2r);
+      prefix_update(g[4 * k + 1], H[4 * k + 1], Sbar, p1, p2);
+      prefix_update(g[4 * k + 2], H[4 * k + 2], Sbar, a.lr * p1, a.lr * p2);
+      prefix_update(g[4 * k + 3], H[4 * k + 3], Sbar, a.t * fma_r(Acc, u1[2], -Asc * h1), a.t * fma_r(Acc, u2[2], -Asc * h2));
     }
   }
-  __device__ __forceinline__ void finish(const BatchConsts& P, float Tw, float* out) {
+  template <int G>
+  __device__ __forceinline__ void combine(R Pl, int lane_in_group) {
 #pragma unroll
-    for (int j = 0; j < 16; ++j) out[j] = fmaf(Tw, b2[j], b1[j]);
+    for (int j = 0; j < 16; ++j) prefix_combine<G, R>(g[j], H[j], Pl, lane_in_group);
+  }
+  template <typename PT>
+  __device__ __forceinline__ void finish(const PT& P, R* out) {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) out[4 * k] /= P.sp[4 * k];
+    for (int k = 0; k < 4; ++k) {
+      out[4 * k] = g[4 * k];
+#pragma unroll
+      for (int j = 1; j < 4; ++j) out[4 * k + j] = P.sp[4 * k] * g[4 * k + j];
+    }
   }
 };
 
-template <int CODE> struct GradOf { using type = AnalyticGrad<CODE == kAnalyticFull>; };
-template <> struct GradOf<kUniform> { using type = UniformGrad; };
-template <> struct GradOf<kStack16> { using type = StackGrad; };
+template <int CODE, typename R = float> struct GradOf { using type = AnalyticGrad<CODE == kAnalyticFull, R>; };
+template <typename R> struct GradOf<kUniform, R> { using type = UniformGrad<R>; };
+template <typename R> struct GradOf<kStack16, R> { using type = StackGrad<R>; };
 
 struct VjpArgs {
   Geometry geo;
@@ -264,13 +310,16 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   // cotangents of this sightline, coefficients folded in (zero for padded lanes)
   // (dQ, dU are re-read at every tile start -- L1 hits -- instead of being held in 2 NF registers)
   float cI = 0.f;
+  float cIa = 0.f;   // sum_f Ibar_f c_f d ln c_f / d alpha (alpha gradient)
   const int64_t o0 = ((int64_t)b * A.n_freq_total + A.f0) * A.geo.npix + pix;
 #pragma unroll
   for (int f = 0; f < NF; ++f) {
     const float vI = (valid && A.dI) ? A.dI[o0 + f * A.geo.npix] : 0.f;
     cI = fmaf(vI, P.coefI[A.f0 + f], cI);
+    if (kAlpha) cIa = fmaf(vI * P.coefI[A.f0 + f], P.dlnc_dalpha[A.f0 + f], cIa);
   }
   cI *= T.scalef;   // the maps are scale * coef * sums (per-sightline segment length, synax_plan_set_box)
+  cIa *= T.scalef;
 
   // ---- pre-pass (G > 1): Faraday sum of each lane's chunk -> float64 offset of the preceding lanes
   double off = 0.0;
@@ -314,10 +363,10 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   acc.zero();
   float gAlpha = 0.f;          // sum_n 1/4 ln(B_perp^2) M K
   float sumE = 0.f;            // sum_n e~_n
-  float pq[NF];                // sum_n (a u_f + b v_f) = Qbar_f Q_f + Ubar_f U_f (coefficients folded)
-#pragma unroll
-  for (int f = 0; f < NF; ++f) pq[f] = 0.f;
-  float Pl = 0.f;              // lane-local inclusive prefix of Sbar
+  float gPol = 0.f;            // sum_f (d ln c_f / d alpha + d ln Pi / d alpha) (Qbar_f Q_f + Ubar_f U_f)
+  // d ln c_f / d alpha = dlnA - ln(nu_f) / 2: the frequency-dependent part comes from the constant bank (ft.ln_nu)
+  const float cPol = kAlpha ? P.dlnA_dalpha + P.dpi_dalpha_over_pi : 0.f;
+  float Pl = 0.f;              // sum of Sbar over this lane's samples
   double carry = 0.0;
   double s_d = ((double)n0 + 0.5) * delta;
   const int tile = warp_prec ? P.tile_d : kTile;
@@ -389,7 +438,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         hi = sum;
       }
       // A9: fan-out over frequencies
-      float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f;
+      float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f, Zc = 0.f, Zs = 0.f;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         const float th = ft.k_rad[f] * ph;
@@ -398,8 +447,9 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         const float v = fmaf(ru[f], c, -rq[f] * s);
         Xc += u; Xs += v;
         Yc = fmaf(ft.k_rad[f], u, Yc); Ys = fmaf(ft.k_rad[f], v, Ys);
-        if (kAlpha) pq[f] = fmaf(a, u, fmaf(bq, v, pq[f]));
+        if (kAlpha) { Zc = fmaf(ft.ln_nu[f], u, Zc); Zs = fmaf(ft.ln_nu[f], v, Zs); }
       }
+      if (kAlpha) gPol = fmaf(a, fmaf(cPol, Xc, -0.5f * Zc), fmaf(bq, fmaf(cPol, Xs, -0.5f * Zs), gPol));
       // L_n = M K,  K = cI Bt2 + Xc d2 + Xs p2
       const float K = fmaf(cI, Bt2, fmaf(Xc, d2, Xs * p2));
       const float MK = M * K;
@@ -408,44 +458,27 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       // cotangent of the phase variable S at this sample, and the D.4 weight
       const float Sbar = fmaf(a, Ys, -bq * Yc);
       Pl += Sbar;
-      const float wgt = fmaf(-0.5f, Sbar, Pl);
       // B_N, B_E cotangents (direct): from M, d2, p2, Bt2 and the (B_perp^2)^q factor
       float tq_ = 0.f;                                             // d/dBt2 through w (alpha != 3 only)
       if (!P.alpha_is_3 && Bt2 > 0.f) tq_ = P.q_exp * MK * mufu_rcp(Bt2);
       const float BEb = 2.0f * fmaf(M, fmaf(S.BE, cI + Xc, S.BN * Xs), S.BE * tq_);
       const float BNb = 2.0f * fmaf(M, fmaf(S.BN, cI - Xc, S.BE * Xs), S.BN * tq_);
-      if constexpr (CODE == kUniform) acc.add(T, S, BNb, BEb, wgt, MK);
-      else if constexpr (CODE == kStack16) acc.add(P, T, sa, S, BNb, BEb, wgt);
-      else acc.add(P, T, aux, S, zf, BNb, BEb, wgt, MK);
+      if constexpr (CODE == kUniform) acc.add(T, S, BNb, BEb, Sbar, w * K);
+      else if constexpr (CODE == kStack16) acc.add(P, T, sa, S, BNb, BEb, Sbar);
+      else acc.add(P, T, aux, S, zf, BNb, BEb, Sbar, w * aux.N0u * K);
     }
     carry += (PMODE != 0 && prec) ? dl : (double)hi + (double)lo;
   }
 
-  // ---- combine: Tw = T - P_off for this lane
-  float Tw;
-  if (G > 1) {
-    const double Poff = group_exclusive_scan<G>((double)Pl, g);
-    float Tt = Pl;
-    Tt = group_sum<G>(Tt);
-    Tw = Tt - (float)Poff;
-  } else {
-    Tw = Pl;
-  }
+  // ---- combine the lanes of the sightline (prefix of the preceding lanes' h-sums times this lane's Sbar total)
+  acc.template combine<G>(Pl, g);
   float out[16];
 #pragma unroll
   for (int j = 0; j < 16; ++j) out[j] = 0.f;
-  acc.finish(P, Tw, out);
+  acc.finish(P, out);
   if (kAlpha) {
     // alpha: 1/4 ln(B_perp^2) term + d ln c_f / d alpha * (Ibar I + Qbar Q + Ubar U) + dPi/Pi * (Qbar Q + Ubar U)
-    float ga = 0.25f * 0.6931471805599453f * gAlpha;
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-      const int64_t o = ((int64_t)b * A.n_freq_total + A.f0 + f) * A.geo.npix + pix;
-      const float vI = (valid && A.dI) ? A.dI[o] * P.coefI[A.f0 + f] * T.scalef : 0.f;
-      ga = fmaf(P.dlnc_dalpha[A.f0 + f], fmaf(vI, sumE, pq[f]), ga);
-      ga = fmaf(P.dpi_dalpha_over_pi, pq[f], ga);
-    }
-    out[CODE == kUniform ? 5 : 12] = ga;
+    out[CODE == kUniform ? 5 : 12] = fmaf(0.25f * 0.6931471805599453f, gAlpha, fmaf(cIa, sumE, gPol));
   }
 
   // ---- block reduction -> partial[b][block][16]

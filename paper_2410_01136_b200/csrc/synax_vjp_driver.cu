@@ -32,10 +32,10 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_block
 }
 
 // The adjoint tolerates ~10x the Faraday round-off scale the forward does (gradients are sums over all pixels,
-// bound 1e-3 instead of 1e-4).  precision 0: per sightline (PMODE 2), threshold 10 x escalate_rad -- unless a pilot
+// bound 1e-3 instead of 1e-4).  precision 0: per sightline (PMODE 2), threshold 10/3 x escalate_rad = 1000 rad -- unless a pilot
 // over ~8k sightlines finds none above HALF that threshold, in which case the lean fp32 variant (PMODE 0: fewer
 // registers, no estimate) runs (cfg 2 at 23 GHz: 8.2 instead of 9.5 ms).  Decided on the device, no host sync.
-constexpr double kVjpEscalateFactor = 10.0;
+constexpr double kVjpEscalateFactor = 10.0 / 3.0;   // x escalate_rad (300 rad by default): 1000 rad
 
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                                  const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,

@@ -127,3 +127,29 @@ def test_b0_homogeneity_without_faraday():
     L2 = (cots[0] * I).sum() + (cots[1] * Q).sum() + (cots[2] * U).sum()
     g2 = oracle.vjp(m2, 8, 64, 20.0, [0.408e9], *cots)
     assert abs(g2[0, 0] - 2.0 / p[0] * L2) > 1e-3 * abs(g2[0, 0])
+
+
+@pytest.mark.parametrize("zero", [(0,), (5,), (9,), (13,), (0, 13)])
+def test_fd_full16_zero_amplitudes(zero):
+    """Amplitude parameters exactly at zero (b0 at the edge of the paper's U[0,10] prior, n_e0 = 0 to switch Faraday
+    rotation off, ...): the derivative with respect to an amplitude is the unit-amplitude field (App. D.3:
+    dB/db0 = B_disc / b0), finite there; checked by central differences straddling zero."""
+    p = wl.FULL16_NOMINAL.copy()
+    scale = {0: 6.0, 5: 2.0, 9: 2.1e-4, 13: 0.03}
+    for j in zero:
+        p[j] = 0.0
+    geom = (4, 64, 25.0, np.array([0.408e9, 1.4e9]))
+    pix = np.array([3, 77, 90, 101, 188])
+    rng = np.random.default_rng(40)
+    cots = [rng.standard_normal((1, 2, len(pix))) for _ in range(3)]
+    model = lambda q: oracle.Model("full16", q)   # noqa: E731
+    g = oracle.vjp(model(p), *geom, *cots, pix=pix).ravel()
+    assert np.all(np.isfinite(g))
+    for j in zero:
+        h = (1e-7 if j == 13 else 1e-5) * scale[j]   # n_e0 enters through cos / sin of up to ~1500 rad x n_e0 / 0.03
+        pp, pm = p.copy(), p.copy()
+        pp[j] += h; pm[j] -= h
+        fd = (loss(model, pp, geom, cots, pix) - loss(model, pm, geom, cots, pix)) / (2 * h)
+        assert g[j] == pytest.approx(fd, rel=2e-6, abs=1e-9 * np.abs(g).max()), (j, g[j], fd)
+    if 9 in zero:      # N_0 = 0: no emission, every other derivative vanishes exactly
+        assert np.all(g[np.arange(16) != 9] == 0.0) and g[9] != 0.0

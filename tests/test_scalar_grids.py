@@ -100,6 +100,27 @@ def test_gpu_gridded_scalars_parity(case):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("ne_amp", [0.12, 0.5])
+def test_gpu_strong_ne_grid_with_zero_aux_ne(ne_amp):
+    """The aux n_e entries are ignored when a gridded n_e is given (synax.h), so the caller may leave them at zero: the
+    float64 chain's tile length (fp32 in-tile Faraday angle) must then be sized from the grid itself.  n_e grid 4-17 x
+    the nominal disc at 408 MHz, few samples (several rad per step)."""
+    w = wl.config(1).scaled(nside=16, n_los=128)
+    w.freqs = np.array([0.408e9])
+    w.aux = w.aux.copy(); w.aux[4] = 0.0
+    w.ne_grid, w.ne_box = wl.clumpy_disc_grid((64, 64, 16), BOX, ne_amp, 20.0, 1.0, seed=83), BOX
+    ref = parity.oracle_forward(w)
+    for precision in (0, 2):
+        maps, _ = parity.gpu_forward(w, precision=precision)
+        parity.assert_maps_close(maps, ref, what=f"strong n_e grid, aux ne0 = 0, precision {precision}")
+    cots = w.cotangents()
+    gr = parity.oracle_vjp(w, cots)
+    for precision in (0, 2):
+        g = parity.gpu_vjp(w, cots, precision=precision)
+        assert np.all(np.abs(g - gr) <= parity.GRAD_TOL * np.abs(gr)), (precision, np.abs(g - gr) / np.abs(gr))
+
+
+@pytest.mark.gpu
 def test_gpu_gridded_scalars_rejected_for_full16():
     import torch
     import paper_2410_01136_b200 as sx
