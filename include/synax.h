@@ -104,7 +104,7 @@ int64_t synax_plan_npix(const synax_plan* plan);  /* pixels of this plan (12 nsi
 synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
 
 /* Options.  key "precision": 0 = auto (default), 1 = fp32 only, 2 = float64 Faraday chain for every sightline,
- * 3 = everything in float64 (the paper's default precision; analytic models).
+ * (everything in float64, the paper's default precision: synax_forward_f64 / synax_vjp_f64 below).
  * Auto, forward: sightlines whose Faraday round-off scale k_max sum_n |n_e| (|B_LOS|+|B_N|+|B_E|) exceeds
  * "escalate_rad" (default 300 rad, calibrated against the oracle: DESIGN.md section 5) take the float64 Faraday
  * chain -- as a redo of a flagged list after the fp32 pass, for every sightline when a device-side pilot finds most of
@@ -141,6 +141,18 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
 synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,
                        int32_t batch, const float* dI, const float* dQ, const float* dU, float* grad,
                        void* cuda_stream);
+
+/* The paper's own arithmetic (section 2.4: "the default precision is double ... for all examples"): the same two
+ * operations with EVERY step in float64 -- positions, fields, emissivity (Eq. 2, 5), Faraday depth (Eq. 7), rotation
+ * (Eq. 6), sums (Eq. 9) and the whole adjoint -- on float64 buffers: params DEVICE float64 [batch][n_params]; I, Q, U
+ * and the cotangents DEVICE float64 [batch][n_freq][npix]; grad DEVICE float64 [batch][n_params].  Analytic models only
+ * (DISC4, FULL16, STACK16, UNIFORM; GRID_B returns SYNAX_ERR_UNSUPPORTED); optional n_e / N_0 grids stay fp32 arrays,
+ * interpolated in float64.  The plan's precision / escalate_rad options do not apply.  Asynchronous on `cuda_stream`. */
+synax_status synax_forward_f64(const synax_plan* plan, const synax_model* model, const double* params,
+                               int32_t batch, double* I, double* Q, double* U, void* cuda_stream);
+synax_status synax_vjp_f64(const synax_plan* plan, const synax_model* model, const double* params,
+                           int32_t batch, const double* dI, const double* dQ, const double* dU, double* grad,
+                           void* cuda_stream);
 
 /* Same operations with HOST buffers of the same shapes: the call copies the inputs to the device,
  * runs, copies the results back and synchronises the stream before returning.  When I, Q and U are all page-locked

@@ -19,7 +19,7 @@ KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3, "stack16": 4}
 
 # every symbol include/synax.h declares
 exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_box", "synax_plan_set_option",
-                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
+                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_f64", "synax_vjp_f64", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
 
@@ -69,7 +69,8 @@ def load_library() -> ctypes.CDLL:
     L.synax_plan_stats.restype = ctypes.c_int
     fwd = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, vp]
     bwd = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, vp, vp]
-    for name, at in (("synax_forward", fwd), ("synax_forward_host", fwd), ("synax_vjp", bwd), ("synax_vjp_host", bwd)):
+    for name, at in (("synax_forward", fwd), ("synax_forward_host", fwd), ("synax_vjp", bwd), ("synax_vjp_host", bwd),
+                     ("synax_forward_f64", fwd), ("synax_vjp_f64", bwd)):
         getattr(L, name).argtypes = at
         getattr(L, name).restype = ctypes.c_int
     L.synax_loglike_vjp.argtypes = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, ctypes.POINTER(dbl), vp, vp, vp]
@@ -142,6 +143,7 @@ class Plan:
             _check(L.synax_plan_create_shard(int(nside), int(n_los), float(s_max), fp, int(f.size), op,
                                              int(pix_range[0]), int(pix_range[1]), ctypes.byref(h)))
         self.pix_range = None if pix_range is None else (int(pix_range[0]), int(pix_range[1]))
+        self.device = int(torch.cuda.current_device())
         self.h = h
         self.nside, self.n_los, self.s_max, self.freqs = int(nside), int(n_los), float(s_max), f
         self.n_freq = int(f.size)
@@ -186,11 +188,24 @@ def _stream():
     return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
-def _dev_f32(t, what):
+def _dev_f32(t, what, numel=None):
+    """Pointer of a contiguous float32 CUDA tensor; the C ABI cannot check sizes, so the element count is checked here."""
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
         raise TypeError(f"{what} must be a contiguous float32 CUDA tensor")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{what} has {t.numel()} elements, expected {numel}")
     return ctypes.c_void_p(t.data_ptr())
+
+
+def _check_device(plan, *tensors):
+    """The plan lives on the device that was current when it was created: every tensor and the current device must match."""
+    import torch
+    if torch.cuda.current_device() != plan.device:
+        raise RuntimeError(f"the plan was created on cuda:{plan.device}, the current device is cuda:{torch.cuda.current_device()}")
+    for t in tensors:
+        if t is not None and t.device.index != plan.device:
+            raise ValueError(f"tensor on {t.device}, the plan is on cuda:{plan.device}")
 
 
 def _batch_of(model: Model, params) -> int:
@@ -210,8 +225,10 @@ def forward(plan: Plan, model: Model, params, out=None):
     if out is None:
         out = tuple(torch.empty((batch, plan.n_freq, plan.npix), dtype=torch.float32, device=params.device) for _ in range(3))
     I, Q, U = out
+    n = batch * plan.n_freq * plan.npix
+    _check_device(plan, params, I, Q, U)
     _check(load_library().synax_forward(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
-                                        _dev_f32(I, "I"), _dev_f32(Q, "Q"), _dev_f32(U, "U"), _stream()))
+                                        _dev_f32(I, "I", n), _dev_f32(Q, "Q", n), _dev_f32(U, "U", n), _stream()))
     return I, Q, U
 
 
@@ -221,9 +238,46 @@ def vjp(plan: Plan, model: Model, params, dI, dQ, dU, out=None):
     batch = _batch_of(model, params)
     if out is None:
         out = torch.empty_like(params)
-    ptr = lambda t, n: ctypes.c_void_p(None) if t is None else _dev_f32(t, n)  # noqa: E731
+    n = batch * plan.n_freq * plan.npix
+    ptr = lambda t, w: ctypes.c_void_p(None) if t is None else _dev_f32(t, w, n)  # noqa: E731
+    _check_device(plan, params, dI, dQ, dU, out)
     _check(load_library().synax_vjp(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
-                                    ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _dev_f32(out, "grad"), _stream()))
+                                    ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _dev_f32(out, "grad", params.numel()), _stream()))
+    return out
+
+
+def _dev_f64(t, what, numel=None):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{what} must be a contiguous float64 CUDA tensor")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{what} has {t.numel()} elements, expected {numel}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def forward_f64(plan: Plan, model: Model, params, out=None):
+    """synax_forward_f64 (the paper's all-float64 arithmetic): params CUDA float64 [batch][P] -> (I, Q, U) CUDA float64."""
+    import torch
+    batch = _batch_of(model, params)
+    n = batch * plan.n_freq * plan.npix
+    if out is None:
+        out = tuple(torch.empty((batch, plan.n_freq, plan.npix), dtype=torch.float64, device=params.device) for _ in range(3))
+    I, Q, U = out
+    _check(load_library().synax_forward_f64(plan.h, ctypes.byref(model.c), _dev_f64(params, "params"), batch,
+                                            _dev_f64(I, "I", n), _dev_f64(Q, "Q", n), _dev_f64(U, "U", n), _stream()))
+    return I, Q, U
+
+
+def vjp_f64(plan: Plan, model: Model, params, dI, dQ, dU, out=None):
+    """synax_vjp_f64: cotangent maps CUDA float64 [batch][n_freq][npix] (None = zeros) -> grad CUDA float64 like params."""
+    import torch
+    batch = _batch_of(model, params)
+    n = batch * plan.n_freq * plan.npix
+    if out is None:
+        out = torch.empty_like(params)
+    ptr = lambda t, w: ctypes.c_void_p(None) if t is None else _dev_f64(t, w, n)  # noqa: E731
+    _check(load_library().synax_vjp_f64(plan.h, ctypes.byref(model.c), _dev_f64(params, "params"), batch,
+                                        ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _dev_f64(out, "grad", params.numel()), _stream()))
     return out
 
 
@@ -260,9 +314,11 @@ def adam_step(theta, grad, m, v, t: int, lr=1e-3, beta1=0.9, beta2=0.999, eps=1e
     return theta
 
 
-def _host_f32(a, what):
+def _host_f32(a, what, size=None):
     if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous):
         raise TypeError(f"{what} must be a C-contiguous float32 numpy array")
+    if size is not None and a.size != size:
+        raise ValueError(f"{what} has {a.size} elements, expected {size}")
     return ctypes.c_void_p(a.ctypes.data)
 
 
@@ -272,8 +328,9 @@ def forward_host(plan: Plan, model: Model, params: np.ndarray, out=None):
     if out is None:
         out = tuple(np.empty((batch, plan.n_freq, plan.npix), dtype=np.float32) for _ in range(3))
     I, Q, U = out
-    _check(load_library().synax_forward_host(plan.h, ctypes.byref(model.c), _host_f32(params, "params"), batch,
-                                             _host_f32(I, "I"), _host_f32(Q, "Q"), _host_f32(U, "U"), _stream()))
+    n = batch * plan.n_freq * plan.npix
+    _check(load_library().synax_forward_host(plan.h, ctypes.byref(model.c), _host_f32(params, "params", batch * model.n_params), batch,
+                                             _host_f32(I, "I", n), _host_f32(Q, "Q", n), _host_f32(U, "U", n), _stream()))
     return I, Q, U
 
 
@@ -282,7 +339,8 @@ def vjp_host(plan: Plan, model: Model, params: np.ndarray, dI, dQ, dU, out=None)
     batch = 1 if model.kind == "grid_b" else int(params.size // model.n_params)
     if out is None:
         out = np.empty_like(params)
-    ptr = lambda a, n: ctypes.c_void_p(None) if a is None else _host_f32(a, n)  # noqa: E731
-    _check(load_library().synax_vjp_host(plan.h, ctypes.byref(model.c), _host_f32(params, "params"), batch,
-                                         ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _host_f32(out, "grad"), _stream()))
+    n = batch * plan.n_freq * plan.npix
+    ptr = lambda a, w: ctypes.c_void_p(None) if a is None else _host_f32(a, w, n)  # noqa: E731
+    _check(load_library().synax_vjp_host(plan.h, ctypes.byref(model.c), _host_f32(params, "params", batch * model.n_params), batch,
+                                         ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _host_f32(out, "grad", params.size), _stream()))
     return out

@@ -563,6 +563,54 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
 }
 
 // ------------------------------------------------------------------------------------------------
+// The paper's arithmetic: everything in float64, float64 buffers at the boundary (synax_dd.cuh).
+// ------------------------------------------------------------------------------------------------
+static synax_status check_f64_model(const synax_plan* plan, const synax_model* model, const void* params, int32_t batch, int* code) {
+  synax_status stt = check_model(plan, model, params, batch, code);
+  if (stt != SYNAX_OK) return stt;
+  if (*code == kGridB) return fail(SYNAX_ERR_UNSUPPORTED, "the float64 entry points take the analytic models (DISC4, FULL16, STACK16, UNIFORM)");
+  return SYNAX_OK;
+}
+
+extern "C" synax_status synax_forward_f64(const synax_plan* plan, const synax_model* model, const double* params,
+                                          int32_t batch, double* I, double* Q, double* U, void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_f64_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  StreamScratch scratch(st);
+  void* bc64 = nullptr;
+  CUDA_TRY(scratch.get(&bc64, dd_consts_bytes(batch)));
+  stt = dd_forward(code, plan->ft, make_geo(plan), params, model->n_params, batch, make_aux(model),
+                   make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l), make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l),
+                   pick_lanes(plan, plan->npix * batch), bc64, I, Q, U, st, &plan->launches);
+  if (stt != SYNAX_OK) return fail(stt, "float64 forward launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+  return SYNAX_OK;
+}
+
+extern "C" synax_status synax_vjp_f64(const synax_plan* plan, const synax_model* model, const double* params,
+                                      int32_t batch, const double* dI, const double* dQ, const double* dU, double* grad,
+                                      void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_f64_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  StreamScratch scratch(st);
+  void* bc64 = nullptr;
+  double* partial = nullptr;
+  const int G = pick_lanes(plan, plan->npix * batch);
+  CUDA_TRY(scratch.get(&bc64, dd_consts_bytes(batch)));
+  CUDA_TRY(scratch.get(&partial, sizeof(double) * 16 * (size_t)dd_vjp_blocks(plan->npix, G) * (size_t)batch));
+  stt = dd_vjp(code, plan->ft, make_geo(plan), params, model->n_params, batch, make_aux(model),
+               make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l), make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l),
+               G, bc64, partial, dI, dQ, dU, grad, st, &plan->launches);
+  if (stt != SYNAX_OK) return fail(stt, "float64 vjp launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+  return SYNAX_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Fused Gaussian likelihood (Eq.(15)): forward -> residual cotangents + logL -> VJP.
 // ------------------------------------------------------------------------------------------------
 // In place: map <- -w (map - obs) (the cotangent of logL), and logL[b] -= w/2 sum (map - obs)^2.

@@ -104,7 +104,7 @@ __device__ __forceinline__ void eval_stack16_dd(const BatchConsts64& P, const Tr
   for (int k = 0; k < 4; ++k) {
     sincos(fma(P.sp[4 * k + 2], a.lr, P.sp[4 * k + 1]), &a.sp[k], &a.cp[k]);
     sincos(P.sp[4 * k + 3] * a.t, &a.sc[k], &a.cc[k]);
-    const double A = a.mask * (double)stack_w(k) * P.sp[4 * k];
+    const double A = a.mask * stack_w_d(k) * P.sp[4 * k];
     const double Brho = A * a.cp[k] * a.cc[k], Bphi = A * a.sp[k] * a.cc[k];
     const double comp[3] = {Brho * a.xr - Bphi * a.yr, fma(Brho, a.yr, Bphi * a.xr), A * a.sc[k]};
 #pragma unroll

@@ -122,6 +122,8 @@ struct BatchConsts {
   float uB[3], uN0, une;
 };
 
+struct AuxHost { float v[7]; };  // synax_model::aux by value: C0, h_r, h_z, alpha, ne0, h_er, h_ez
+
 struct FreqTab {
   int n_freq;
   float k_rad[kMaxFreq];    // 2 lambda_f^2 K_F Delta : Faraday angle (rad) per unit sum(n_e B_LOS)
@@ -327,6 +329,10 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
 // (DESIGN.md section 3 on the "rotation before stacking").  CR / n_e / alpha from aux as for DISC4.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float stack_w(int k) { return k == 0 ? 0.6f : (k == 2 ? 0.1f : 0.3f); }
+__device__ __forceinline__ double stack_w_d(int k) { return k == 0 ? 0.6 : (k == 2 ? 0.1 : 0.3); }
+template <typename R> __device__ __forceinline__ R stack_weight(int k);
+template <> __device__ __forceinline__ float stack_weight<float>(int k) { return stack_w(k); }
+template <> __device__ __forceinline__ double stack_weight<double>(int k) { return stack_w_d(k); }
 // component of B_k that feeds component c of the total
 __device__ __forceinline__ constexpr int stack_src(int k, int c) {
   return k == 0 ? c : (k == 1 ? (c == 0 ? 0 : (c == 1 ? 2 : 1)) : (k == 2 ? (c == 0 ? 2 : (c == 1 ? 1 : 0)) : (c == 0 ? 1 : (c == 1 ? 0 : 2))));

@@ -44,4 +44,15 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
                       const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
                       int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches);
 
+// ---- synax_dd.cu: the all-float64 path (synax_forward_f64 / synax_vjp_f64)
+size_t dd_consts_bytes(int batch);
+int dd_vjp_blocks(int64_t npix, int G);
+synax_status dd_forward(int code, const FreqTab& ft, const Geometry& geo, const double* params, int n_params, int batch,
+                        const AuxHost& aux, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0, int G, void* bc64,
+                        double* I, double* Q, double* U, cudaStream_t st, int64_t* launches);
+synax_status dd_vjp(int code, const FreqTab& ft, const Geometry& geo, const double* params, int n_params, int batch,
+                    const AuxHost& aux, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0, int G, void* bc64,
+                    double* partial, const double* dI, const double* dQ, const double* dU, double* grad, cudaStream_t st,
+                    int64_t* launches);
+
 }  // namespace synax

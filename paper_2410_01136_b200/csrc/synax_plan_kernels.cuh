@@ -75,7 +75,6 @@ __global__ void box_path_kernel(const double* __restrict__ dirs, int64_t count, 
 // Folds Eq.(2)'s constants, the Rayleigh-Jeans conversion (S:C-2#1) and the units into
 // c_f(alpha) so that I_f = c_f Delta sum_n N_0 (B_perp^2)^((alpha+1)/4)  with B in uG.
 // ------------------------------------------------------------------------------------------------
-struct AuxHost { float v[7]; };  // C0, h_r, h_z, alpha, ne0, h_er, h_ez
 
 // max |g[i]| of a non-negative-comparable float array into *out (zero on entry): non-negative floats order like ints
 __global__ void absmax_kernel(const float* __restrict__ g, int64_t n, float* __restrict__ out) {

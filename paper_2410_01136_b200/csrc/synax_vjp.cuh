@@ -69,42 +69,49 @@ struct AnalyticGrad {
     to_cyl(v1x, v1y, a.xr, a.yr, v1r, v1p);
     to_cyl(T.nx, T.ny, a.xr, a.yr, nr, np);
     const R v2r = S.ne * nr, v2p = S.ne * np, v2z = S.ne * T.nz;
-    // disc: B = b0 A [cp cc rho_hat + sp cc phi_hat + sc z_hat], A = exp(-(rho-8)/h_b) inside the annulus
+    // disc: B = b0 A [cp cc rho_hat + sp cc phi_hat + sc z_hat], A = exp(-(rho-8)/h_b) inside the annulus.
+    // Every accumulator first takes Sbar x (its prefix H), then the direct term is fused into its last FMAs.
+#pragma unroll
+    for (int j = 0; j < NB; ++j) g[j] = fma_r(Sbar, H[j], g[j]);
     const R Acc = a.A * a.cc, Asc = a.A * a.sc;
     {
       const R al1 = fma_r(a.cp, v1r, a.sp * v1p), al2 = fma_r(a.cp, v2r, a.sp * v2p);
-      const R d1 = fma_r(Acc, al1, Asc * v1z), d2 = fma_r(Acc, al2, Asc * v2z);   // (B_disc / b0) . V
-      prefix_update(g[0], H[0], Sbar, d1, d2);
-      const R p1 = Acc * fma_r(a.cp, v1p, -a.sp * v1r);                          // (dB/dpsi0) / b0 . V
-      const R p2 = Acc * fma_r(a.cp, v2p, -a.sp * v2r);
-      prefix_update(g[1], H[1], Sbar, p1, p2);
-      prefix_update(g[2], H[2], Sbar, a.lr * p1, a.lr * p2);
-      const R c1 = a.t * fma_r(Acc, v1z, -Asc * al1), c2 = a.t * fma_r(Acc, v2z, -Asc * al2);
-      prefix_update(g[3], H[3], Sbar, c1, c2);
       if (kFull) {
+        const R d1 = fma_r(Acc, al1, Asc * v1z), d2 = fma_r(Acc, al2, Asc * v2z);   // (B_disc / b0) . V
         const R dr = a.rho - (R)8.0;
-        prefix_update(g[4], H[4], Sbar, dr * d1, dr * d2);                          // * b0 / h_b^2
+        g[0] += d1; H[0] += d2;
+        g[4] = fma_r(dr, d1, g[4]); H[4] = fma_r(dr, d2, H[4]);                    // * b0 / h_b^2
+      } else {
+        g[0] = fma_r(Acc, al1, fma_r(Asc, v1z, g[0])); H[0] = fma_r(Acc, al2, fma_r(Asc, v2z, H[0]));
       }
+      const R p1 = Acc * fma_r(a.cp, v1p, -a.sp * v1r);                            // (dB/dpsi0) / b0 . V
+      const R p2 = Acc * fma_r(a.cp, v2p, -a.sp * v2r);
+      g[1] += p1; H[1] += p2;
+      g[2] = fma_r(a.lr, p1, g[2]); H[2] = fma_r(a.lr, p2, H[2]);
+      const R tAcc = a.t * Acc, tAsc = a.t * Asc;                                  // (dB/dchi0) / b0 = t A (cc z_hat - sc (...))
+      g[3] = fma_r(tAcc, v1z, fma_r(-tAsc, al1, g[3])); H[3] = fma_r(tAcc, v2z, fma_r(-tAsc, al2, H[3]));
     }
     if (kFull) {  // halo: B_h L R phi_hat
       const R LR = a.L * a.R;
-      prefix_update(g[5], H[5], Sbar, LR * v1p, LR * v2p);
+      g[5] = fma_r(LR, v1p, g[5]); H[5] = fma_r(LR, v2p, H[5]);
       const R RuL2 = a.R * a.u * a.L * a.L;
-      prefix_update(g[6], H[6], Sbar, RuL2 * v1p, RuL2 * v2p);                      // * 2 B_h / w_h
+      g[6] = fma_r(RuL2, v1p, g[6]); H[6] = fma_r(RuL2, v2p, H[6]);                // * 2 B_h / w_h
       const R q = LR * fma_r(a.rho, P.inv_rh, (R)-1.0);
-      prefix_update(g[7], H[7], Sbar, q * v1p, q * v2p);                            // * B_h / r_h
+      g[7] = fma_r(q, v1p, g[7]); H[7] = fma_r(q, v2p, H[7]);                      // * B_h / r_h
       const R Ru2L2 = RuL2 * a.u;
-      prefix_update(g[8], H[8], Sbar, Ru2L2 * v1p, Ru2L2 * v2p);                    // * 2 B_h / w_h
+      g[8] = fma_r(Ru2L2, v1p, g[8]); H[8] = fma_r(Ru2L2, v2p, H[8]);              // * 2 B_h / w_h
     }
     if (kFull) {
       // N_0 = n0 exp(-rho/h_r) sech^2(z/h_z):  dN0/dn0 = N0/n0, /dh_r = N0 rho/h_r^2, /dh_z = N0 2 tanh(z/h_z) z/h_z^2
       n1[0] += MKu; n1[1] = fma_r(MKu, a.rho, n1[1]); n1[2] = fma_r(MKu * a.thz, z, n1[2]);
       const R h = T.scalef * a.neu * S.Bpar;   // d(ne Bpar Delta_i/Delta) / d ne0
       const R hh = (R)0.5 * Sbar * h;
-      prefix_update(ge[0], He[0], Sbar, hh, h);
-      prefix_update(ge[1], He[1], Sbar, hh * a.rho, h * a.rho);
+#pragma unroll
+      for (int j = 0; j < 3; ++j) ge[j] = fma_r(Sbar, He[j], ge[j]);
+      ge[0] += hh; He[0] += h;
+      ge[1] = fma_r(hh, a.rho, ge[1]); He[1] = fma_r(h, a.rho, He[1]);
       const R tz = a.thez * z;
-      prefix_update(ge[2], He[2], Sbar, hh * tz, h * tz);
+      ge[2] = fma_r(hh, tz, ge[2]); He[2] = fma_r(h, tz, He[2]);
     }
   }
   template <int G>
@@ -193,7 +200,7 @@ struct StackGrad {
       R u1r, u1p, u2r, u2p;
       to_cyl(u1[0], u1[1], a.xr, a.yr, u1r, u1p);
       to_cyl(u2[0], u2[1], a.xr, a.yr, u2r, u2p);
-      const R A = a.mask * (R)stack_w(k);
+      const R A = a.mask * stack_weight<R>(k);
       const R Acc = A * a.cc[k], Asc = A * a.sc[k];
       const R h1 = fma_r(a.cp[k], u1r, a.sp[k] * u1p), h2 = fma_r(a.cp[k], u2r, a.sp[k] * u2p);
       prefix_update(g[4 * k], H[4 * k], Sbar, fma_r(Acc, h1, Asc * u1[2]), fma_r(Acc, h2, Asc * u2[2]));   // (B_k / b0_k) . V
