@@ -11,10 +11,30 @@ namespace synax {
 // ------------------------------------------------------------------------------------------------
 static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
   GridDesc g;
-  g.g = grid; g.nx = m->nx; g.ny = m->ny; g.nz = m->nz;
+  g.g = grid; g.g4 = nullptr; g.gd4 = nullptr; g.nx = m->nx; g.ny = m->ny; g.nz = m->nz;
   g.sx = (double)(m->nx - 1) / (double)m->lx; g.sy = (double)(m->ny - 1) / (double)m->ly; g.sz = (double)(m->nz - 1) / (double)m->lz;
   g.bx = 0.5 * (double)(m->nx - 1); g.by = 0.5 * (double)(m->ny - 1); g.bz = 0.5 * (double)(m->nz - 1);
   return g;
+}
+
+// Repacked per-call copies of the grid (GridDesc::g4 / gd4) from the stream-ordered pool; 0 on success.
+static synax_status pack_grid(GridDesc& g, bool want_f64, cudaStream_t st, int64_t* launches) {
+  const int64_t n_nodes = (int64_t)g.nx * g.ny * g.nz;
+  float4* g4 = nullptr;
+  double4* gd4 = nullptr;
+  if (cudaMallocAsync((void**)&g4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
+  if (want_f64 && cudaMallocAsync((void**)&gd4, sizeof(double4) * (size_t)n_nodes, st) != cudaSuccess) {
+    cudaFreeAsync(g4, st);
+    return SYNAX_ERR_ALLOC;
+  }
+  grid_pack_kernel<<<(unsigned)((n_nodes + 255) / 256), 256, 0, st>>>(g.g, n_nodes, g4, gd4);
+  ++*launches;
+  g.g4 = g4; g.gd4 = gd4;
+  return SYNAX_OK;
+}
+static void unpack_grid(const GridDesc& g, cudaStream_t st) {
+  if (g.g4) cudaFreeAsync((void*)g.g4, st);
+  if (g.gd4) cudaFreeAsync((void*)g.gd4, st);
 }
 
 static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft0) {
@@ -45,7 +65,11 @@ synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_
   ga.f.flag_list = nullptr; ga.f.flag_count = d_flag_count;
   ga.f.flag_S = (float)(escalate_rad / (double)k_max);
   cudaMemsetAsync(d_flag_count, 0, kCtrlWords * sizeof(int), st);
-  const unsigned blocks = (unsigned)min((int64_t)sms * 16, (a0.geo.npix * 32 + kBlock - 1) / kBlock);
+  const synax_status ps = pack_grid(ga.grid, precision != 1, st, launches);
+  if (ps != SYNAX_OK) return ps;
+  // one warp per sightline; the hardware block scheduler balances the CTAs (a persistent grid of 16 CTAs/SM ran 2.3
+  // waves of the 7 CTAs/SM that fit, with a thin last wave)
+  const unsigned blocks = (unsigned)((a0.geo.npix * 32 + kBlock - 1) / kBlock);
   for (int f0 = 0; f0 < ft.n_freq;) {
     const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
     ga.f.f0 = f0;
@@ -53,6 +77,7 @@ synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_
     f0 += nf;
   }
   const cudaError_t e = cudaGetLastError();
+  unpack_grid(ga.grid, st);
   cudaMemcpyAsync(h_flag_count, d_flag_count, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
@@ -78,18 +103,30 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
     cudaFreeAsync(a.grad4, st);
     return SYNAX_ERR_CUDA;
   }
-  const unsigned blocks = (unsigned)min((int64_t)sms * 8, (geo.npix * 32 + kBlock - 1) / kBlock);
+  const synax_status ps = pack_grid(a.grid, precision != 1, st, launches);
+  if (ps != SYNAX_OK) {
+    cudaFreeAsync(a.grad4, st);
+    return ps;
+  }
+  const int64_t max_blocks = (geo.npix * 32 + kBlock - 1) / kBlock;
   for (int f0 = 0; f0 < ft.n_freq;) {
     const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
     a.f0 = f0;
     const bool sg = a.sg_ne.g || a.sg_n0.g;
 #define SYNAX_GV(NFV)                                                                                              \
   do {                                                                                                             \
+    /* persistent warps (per-warp shared-memory state): exactly the CTAs that are resident at once, so no thin last wave */ \
     if (sg) {                                                                                                      \
       cudaFuncSetAttribute(grid_vjp_kernel<NFV, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
+      int occ = 1;                                                                                                 \
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, grid_vjp_kernel<NFV, true>, kBlock, smem);               \
+      const unsigned blocks = (unsigned)std::min<int64_t>((int64_t)sms * std::max(occ, 1), max_blocks);            \
       grid_vjp_kernel<NFV, true><<<blocks, kBlock, smem, st>>>(a, shift_freqs(ft, a.f0));                          \
     } else {                                                                                                       \
       cudaFuncSetAttribute(grid_vjp_kernel<NFV, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   \
+      int occ = 1;                                                                                                 \
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, grid_vjp_kernel<NFV, false>, kBlock, smem);              \
+      const unsigned blocks = (unsigned)std::min<int64_t>((int64_t)sms * std::max(occ, 1), max_blocks);            \
       grid_vjp_kernel<NFV, false><<<blocks, kBlock, smem, st>>>(a, shift_freqs(ft, a.f0));                         \
     }                                                                                                              \
   } while (0)
@@ -108,6 +145,7 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   ++*launches;
   const cudaError_t e = cudaGetLastError();
   cudaFreeAsync(a.grad4, st);
+  unpack_grid(a.grid, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 

@@ -13,14 +13,19 @@
 namespace synax {
 
 struct GridDesc {
-  const float* g;       // [nx][ny][nz][3]
+  const float* g;       // caller's grid [nx][ny][nz][3]
+  // Per-call repacked copies (grid_pack_kernel; L2-resident like the grid itself).  The kernels are bound by L1 gather
+  // throughput (ncu: l1tex 73 %, long-scoreboard stalls), so a node is padded to one 16-byte vector: a corner costs one
+  // LDG.128 instead of three LDG.32, and the float64 chain gathers float64 nodes (two LDG.128) with no conversion.
+  const float4* g4;     // [node] = (Bx, By, Bz, 0)
+  const double4* gd4;   // the same in float64, or null (precision 1)
   int nx, ny, nz;
   double sx, sy, sz;    // (n-1)/l
   double bx, by, bz;    // (n-1)/2
 };
 
 struct Cell {
-  int base;             // float index of corner (i,j,k), component 0
+  int base;             // node index of corner (i,j,k)
   float tx, ty, tz;
   bool inbox;
 };
@@ -33,7 +38,7 @@ __device__ __forceinline__ Cell locate(const GridDesc& G, double x, double y, do
   int i = __double2int_rd(ux), j = __double2int_rd(uy), k = __double2int_rd(uz);
   i = max(0, min(i, G.nx - 2)); j = max(0, min(j, G.ny - 2)); k = max(0, min(k, G.nz - 2));
   c.tx = (float)(ux - (double)i); c.ty = (float)(uy - (double)j); c.tz = (float)(uz - (double)k);
-  c.base = ((i * G.ny + j) * G.nz + k) * 3;
+  c.base = (i * G.ny + j) * G.nz + k;
   return c;
 }
 
@@ -46,7 +51,7 @@ __device__ __forceinline__ void weights(const Cell& c, float w[8]) {
 }
 
 __device__ __forceinline__ int corner_offset(const GridDesc& G, int q) {  // q = a*4 + b*2 + d
-  return (((q >> 2) * G.ny + ((q >> 1) & 1)) * G.nz + (q & 1)) * 3;
+  return ((q >> 2) * G.ny + ((q >> 1) & 1)) * G.nz + (q & 1);   // in nodes
 }
 
 __device__ __forceinline__ void gather_B(const GridDesc& G, const Cell& c, float B[3]) {
@@ -56,10 +61,10 @@ __device__ __forceinline__ void gather_B(const GridDesc& G, const Cell& c, float
   if (!c.inbox) return;
 #pragma unroll
   for (int q = 0; q < 8; ++q) {
-    const float* p = G.g + c.base + corner_offset(G, q);
-    B[0] = fmaf(w[q], __ldg(p), B[0]);
-    B[1] = fmaf(w[q], __ldg(p + 1), B[1]);
-    B[2] = fmaf(w[q], __ldg(p + 2), B[2]);
+    const float4 v = __ldg(G.g4 + c.base + corner_offset(G, q));
+    B[0] = fmaf(w[q], v.x, B[0]);
+    B[1] = fmaf(w[q], v.y, B[1]);
+    B[2] = fmaf(w[q], v.z, B[2]);
   }
 }
 
@@ -119,14 +124,15 @@ __device__ __forceinline__ void fields_f64(const GridDesc& G, const BatchConsts&
   const double tx = ux - (double)i, ty = uy - (double)j, tz = uz - (double)k;
   double B[3] = {0.0, 0.0, 0.0};
   if (inbox) {
-    const int base = ((i * G.ny + j) * G.nz + k) * 3;
+    const int base = (i * G.ny + j) * G.nz + k;
     const double x0 = 1.0 - tx, y0 = 1.0 - ty, z0 = 1.0 - tz;
     const double wxy[4] = {x0 * y0, x0 * ty, tx * y0, tx * ty};
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       const double w = wxy[q >> 1] * ((q & 1) ? tz : z0);
-      const float* p = G.g + base + corner_offset(G, q);
-      B[0] = fma(w, (double)__ldg(p), B[0]); B[1] = fma(w, (double)__ldg(p + 1), B[1]); B[2] = fma(w, (double)__ldg(p + 2), B[2]);
+      const double2* p = reinterpret_cast<const double2*>(G.gd4 + base + corner_offset(G, q));
+      const double2 xy = __ldg(p), zw = __ldg(p + 1);
+      B[0] = fma(w, xy.x, B[0]); B[1] = fma(w, xy.y, B[1]); B[2] = fma(w, zw.x, B[2]);
     }
   }
   const double rho2 = fma(xd, xd, yd * yd);
@@ -162,13 +168,43 @@ struct GridFwdArgs {
   int mode;            // 0 auto, 1 fp32 chain only, 2 float64 Faraday chain for every sightline
 };
 
+// Samples n_lo <= n < n_hi of a sightline that can lie inside the grid box -- a conservative superset (slab
+// intersection of the ray with the box in float64, one sample of margin at either end); the exact per-sample box test
+// stays in the sweeps.  Outside the box B = 0: such a sample adds nothing to I, Q, U, the Faraday depth or any
+// cotangent, so the sweeps skip the tiles before n_lo and after n_hi (cfg 3: the 40 x 40 x 8 kpc box holds less than
+// half of the samples of the 20-kpc sightlines).  Warp-uniform.
+__device__ __forceinline__ void box_sample_range(const GridDesc& G, const Geometry& geo, const Triad& T, int& n_lo, int& n_hi) {
+  const double delta = geo.delta * T.scale;
+  double s_in = 0.0, s_out = (double)geo.n_los * delta;
+  const double dir[3] = {T.nxd, T.nyd, T.nzd};
+  const double half[3] = {G.bx / G.sx, G.by / G.sy, G.bz / G.sz};   // l / 2
+  bool empty = false;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double o = geo.obs[a];
+    if (dir[a] != 0.0) {
+      const double t1 = (-half[a] - o) / dir[a], t2 = (half[a] - o) / dir[a];
+      s_in = fmax(s_in, fmin(t1, t2));
+      s_out = fmin(s_out, fmax(t1, t2));
+    } else if (fabs(o) > half[a]) {
+      empty = true;
+    }
+  }
+  if (empty || !(s_out >= s_in)) { n_lo = 0; n_hi = 0; return; }
+  n_lo = max(0, (int)floor(s_in / delta - 0.5) - 1);
+  n_hi = min(geo.n_los, (int)ceil(s_out / delta - 0.5) + 2);
+  if (n_hi < n_lo) n_hi = n_lo;
+}
+
 // Round-off scale of a sightline's Faraday sum, k-independent part: sum_n |n_e| (|B_LOS| + |B_N| + |B_E|),
 // estimated from every 8th sample with the fp32 chain (whole warp; returns the same value in every lane).
 template <bool SG>
 __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const BatchConsts& P, const Triad& T,
                                                         const Geometry& geo, const ScalarGridDesc& sg_ne, int lane) {
   float acc = 0.f;
-  for (int n = 4 + 8 * lane; n < geo.n_los; n += 256) {
+  int n_lo, n_hi;
+  box_sample_range(G, geo, T, n_lo, n_hi);
+  for (int n = (n_lo & ~7) + 4 + 8 * lane; n < n_hi; n += 256) {
     const double s_d = ((double)n + 0.5) * geo.delta * T.scale;
     const double xd = fma(s_d, T.nxd, geo.obs[0]), yd = fma(s_d, T.nyd, geo.obs[1]), zd = fma(s_d, T.nzd, geo.obs[2]);
     const Cell c = locate(G, xd, yd, zd);
@@ -197,7 +233,9 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
   double carry = 0.0;
   float absS = 0.f;
   const double delta = A.geo.delta * T.scale;
-  for (int nt = 0; nt < A.geo.n_los; nt += 32) {
+  int n_lo, n_hi;
+  box_sample_range(G, A.geo, T, n_lo, n_hi);
+  for (int nt = n_lo & ~31; nt < n_hi; nt += 32) {
     const int n = nt + lane;
     const bool active = n < A.geo.n_los;
     const double s_d = ((double)n + 0.5) * delta;
@@ -296,6 +334,15 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c) 
   asm volatile("red.global.v4.f32.add [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(0.0f) : "memory");
 }
 
+// caller's [node][3] grid -> padded fp32 nodes and (optionally) float64 nodes
+__global__ void grid_pack_kernel(const float* __restrict__ g, int64_t n_nodes, float4* __restrict__ g4, double4* __restrict__ gd4) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_nodes) return;
+  const float x = g[3 * i], y = g[3 * i + 1], z = g[3 * i + 2];
+  g4[i] = make_float4(x, y, z, 0.f);
+  if (gd4) gd4[i] = make_double4((double)x, (double)y, (double)z, 0.0);
+}
+
 // [n][4] accumulation buffer -> caller's [n][3] gradient
 __global__ void grid_grad_compact_kernel(const float4* __restrict__ g4, int64_t n_nodes, float* __restrict__ grad) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -329,14 +376,15 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
                                                  const BatchConsts& P, const BatchConstsD& D, const Triad& T,
                                                  const double4 dir, int lane,
                                                  float cI, const float (&cQ)[NF], const float (&cU)[NF],
-                                                 const float (&kr)[NF], float* st_w, float* st_n, float* st_e) {
-  const int C = 1 << A.chunk_log2, Cp = C + 1;
+                                                 const float (&kr)[NF], int n_lo, int n_hi, int cl2,
+                                                 float* st_w, float* st_n, float* st_e) {
+  const int C = 1 << cl2, Cp = C + 1;   // this sightline's chunk length: 32 C >= n_hi - n_lo
   const double delta = A.geo.delta * T.scale;
   double carry = 0.0;
   float absS = 0.f;
-  for (int nt = 0; nt < A.geo.n_los; nt += 32) {
+  for (int nt = n_lo; nt < n_hi; nt += 32) {
     const int n = nt + lane;
-    const bool active = n < A.geo.n_los;
+    const bool active = n < n_hi;
     const double s_d = ((double)n + 0.5) * delta;
     const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
     const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
@@ -393,7 +441,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
     const float BEb = 2.0f * fmaf(M, fmaf(BE, cI + Xc, BN * Xs), BE * tq_);
     const float BNb = 2.0f * fmaf(M, fmaf(BN, cI - Xc, BE * Xs), BN * tq_);
     if (active) {
-      const int idx = (n >> A.chunk_log2) * Cp + (n & (C - 1));
+      const int idx = ((n - n_lo) >> cl2) * Cp + ((n - n_lo) & (C - 1));
       st_w[idx] = Sbar; st_n[idx] = BNb; st_e[idx] = BEb;
     }
   }
@@ -429,22 +477,29 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     }
     // ---- sweep 1: consecutive samples per lane; fp32 chain first, redone with the float64 Faraday chain
     // when the rotation angle of this sightline is large (warp-uniform decision)
+    // the samples that can lie inside the box (the others add nothing to the gradient), cut into 32 chunks of
+    // C2 = 2^cl2 samples: the layout of the hand-over and of sweep 2's lanes
+    int n_lo, n_hi;
+    box_sample_range(G, A.geo, T, n_lo, n_hi);
+    int cl2 = 0;
+    while ((32 << cl2) < n_hi - n_lo) ++cl2;
     float absS = 0.f;
     bool precise = A.mode == 2;
     if (A.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
-    if (!precise) absS = grid_vjp_sweep1<NF, false, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
+    if (!precise) absS = grid_vjp_sweep1<NF, false, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, n_lo, n_hi, cl2, st_w, st_n, st_e);
     if (precise || (A.mode == 0 && absS > A.flag_S)) {
       __syncwarp();
-      grid_vjp_sweep1<NF, true, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, st_w, st_n, st_e);
+      grid_vjp_sweep1<NF, true, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, n_lo, n_hi, cl2, st_w, st_n, st_e);
     }
     __syncwarp();
     // ---- sweep 2: contiguous chunk per lane walked BACKWARDS, so that the suffix sum of Sbar that the
     // transposed half-cell scan needs (gbar_m = sum_{n>m} Sbar_n + Sbar_m / 2) is a running sum with no
     // cancellation; register accumulation per cell, red.global.add only when the cell changes.
-    const int m0 = lane << A.chunk_log2;
-    const int m1 = min(m0 + C, A.geo.n_los);
+    const int C2 = 1 << cl2, Cq = C2 + 1;
+    const int mb = n_lo + (lane << cl2);                // this lane's chunk [mb, mb + C2) of the in-box range
+    const int m0 = min(mb, n_hi), m1 = min(mb + C2, n_hi);
     float tot = 0.f;
-    for (int m = m0; m < m1; ++m) tot += st_w[lane * Cp + (m - m0)];
+    for (int m = m0; m < m1; ++m) tot += st_w[lane * Cq + (m - mb)];
     float incl = tot;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -474,14 +529,14 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
             // one 16-byte vector reduction per corner node (measured 2.6x the throughput of three scalar reds)
-            red_add_v4(A.grad4 + (size_t)(cur / 3 + corner_offset(G, q) / 3) * 4, acc[3 * q], acc[3 * q + 1], acc[3 * q + 2]);
+            red_add_v4(A.grad4 + (size_t)(cur + corner_offset(G, q)) * 4, acc[3 * q], acc[3 * q + 1], acc[3 * q + 2]);
             acc[3 * q] = 0.f; acc[3 * q + 1] = 0.f; acc[3 * q + 2] = 0.f;
           }
         }
         cur = cell;
       }
       if (m >= m0) {
-        const int idx = lane * Cp + (m - m0);
+        const int idx = lane * Cq + (m - mb);
         const float Sb = st_w[idx];
         const float gbar = fmaf(0.5f, Sb, suf);
         suf += Sb;
