@@ -112,6 +112,8 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * -- those above 10/3 x escalate_rad take their Faraday angles from the float64 chain.
  * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0).
  * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).
+ * key "batch_share": parameter vectors integrated per thread when a batch of analytic models is evaluated at one
+ * frequency with one thread per sightline -- they share the sightline geometry (0 = heuristic, else 1, 2 or 4).
  * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool
  * (from which every call takes its scratch) to this many MB, so that the pool is not unmapped at every stream
  * synchronisation -- matters for the *_host calls (hundreds of MB of staging per call).  Process-wide for that

@@ -54,6 +54,7 @@ struct synax_plan {
   int precision;      // 0 auto, 1 fp32 only, 2 float64 chain everywhere
   double escalate_rad;
   int lanes;          // 0 heuristic
+  int batch_share;    // parameter vectors per thread in the batched kernels: 0 heuristic, else 1, 2 or 4
   int* d_vjp_ctrl;    // device control block of the adjoint's pilot (kCtrlWords ints)
   int* d_flag_count;  // device control block, kCtrlWords ints: [flag count, pilot flagged, mode, -]
   int* h_flag_count;  // pinned host mirror (last forward)
@@ -216,6 +217,9 @@ extern "C" synax_status synax_plan_set_option(synax_plan* plan, const char* key,
   } else if (!std::strcmp(key, "lanes")) {
     if (value != 0 && value != 1 && value != 8 && value != 32) return fail(SYNAX_ERR_INVALID_ARG, "lanes must be 0, 1, 8 or 32");
     plan->lanes = (int)value;
+  } else if (!std::strcmp(key, "batch_share")) {
+    if (value != 0 && value != 1 && value != 2 && value != 4) return fail(SYNAX_ERR_INVALID_ARG, "batch_share must be 0, 1, 2 or 4");
+    plan->batch_share = (int)value;
   } else if (!std::strcmp(key, "pool_release_threshold_mb")) {
     // Per-call scratch (constants, flag lists, block partials, the host entry points' staging buffers) comes from the
     // device's stream-ordered pool.  Its default release threshold is 0: every stream synchronisation hands the memory
@@ -502,7 +506,13 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     for (int f0 = 0; f0 < plan->n_freq;) {
       const int nf = next_freq_block(plan->n_freq - f0);
       a.f0 = f0;
-      SYNAX_DISPATCH_CODE(code, fwd_launch_fast, false, G, nf, n_sl, st, a, plan->ft);
+      // batches of parameter vectors on modest maps: NB vectors per thread share the sightline geometry (A12)
+      const int nb = plan->batch_share ? plan->batch_share : (batch >= 4 ? 4 : (batch >= 2 ? 2 : 1));
+      if (nb > 1 && G == 1 && nf == 1 && plan->n_freq == 1 && (code == kAnalyticDisc || code == kAnalyticFull) &&
+          !model->ne_grid && !model->n0_grid)
+        SYNAX_DISPATCH_CODE(code, fwd_launch_batched, nb, st, a, plan->ft);
+      else
+        SYNAX_DISPATCH_CODE(code, fwd_launch_fast, false, G, nf, n_sl, st, a, plan->ft);
       plan->launches++;
       if (split_ok) {   // the same pass over list_u (exits at once unless the pilot chose the split mode)
         ForwardArgs al = a;
@@ -555,7 +565,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
-                      plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
+                      plan->batch_share, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
                       dI, dQ, dU, grad, st, &plan->launches);
   if (rs == SYNAX_ERR_UNSUPPORTED) return fail(rs, "GRID_B vjp: n_los too large for the shared-memory hand-over (see synax.h)");
   if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));

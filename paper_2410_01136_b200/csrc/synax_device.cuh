@@ -51,37 +51,6 @@ __device__ __forceinline__ void sincos_fma(float x, float& s, float& c) {
   c = ((q + 1) & 2) ? -cs : cs;
 }
 
-// 2^x on the FMA pipe: round-to-nearest split x = k + f, |f| <= 1/2, degree-6 near-minimax polynomial
-// (approximation error 2.6e-9, so what is left is fp32 rounding: ~3e-8 rms, mean 1e-9, i.e. it
-// averages out along a sightline, unlike the table-based MUFU.EX2 whose ~1e-7 error is systematic
-// over many consecutive samples).  Used for every exponential the Faraday integrand n_e B_LOS sees
-// (DESIGN.md section 5).  x is clamped at -125 (result stays a normal number).
-__device__ __forceinline__ float exp2_fma(float x) {
-  x = fmaxf(x, -125.0f);
-  const float t = x + 12582912.0f;                 // 1.5 * 2^23: the integer part lands in the low mantissa bits
-  const float f = x - (t - 12582912.0f);           // exact
-  float p = fmaf(1.5469732170458883e-4f, f, 1.3400432653725147e-3f);
-  p = fmaf(p, f, 9.61802527308464e-3f);
-  p = fmaf(p, f, 5.550327152013779e-2f);
-  p = fmaf(p, f, 2.4022650718688965e-1f);
-  p = fmaf(p, f, 6.931471824645996e-1f);
-  p = fmaf(p, f, 1.0f);
-  return __int_as_float(__float_as_int(p) + (__float_as_int(t) << 23));
-}
-// 1/x: MUFU seed + one Newton step (removes the seed's systematic ~1 ulp error)
-__device__ __forceinline__ float rcp_nr(float x) {
-  const float y = mufu_rcp(x);
-  return fmaf(y, fmaf(-x, y, 1.0f), y);
-}
-// 1/sqrt(x) and sqrt(x): MUFU seed + one Newton step each
-__device__ __forceinline__ void rsqrt_sqrt_nr(float x, float& ir, float& r) {
-  float y = mufu_rsqrt(x);
-  y = fmaf(0.5f * y, fmaf(-x * y, y, 1.0f), y);
-  float s = x * y;
-  s = fmaf(0.5f * y, fmaf(-s, s, x), s);
-  ir = y; r = s;
-}
-
 // the same polynomials without the reduction, for |x| <= pi/4 (BatchConsts::angles_small)
 __device__ __forceinline__ void sincos_fma_small(float r, float& s, float& c) {
   const float r2 = r * r;
@@ -103,7 +72,6 @@ struct BatchConsts {
   float sp[16];      // STACK16 only: (b0, psi0, psi1, chi0) of the four stacked spirals (p[] then holds the aux densities)
   // derived fp32
   float k_hb;        // -log2(e)/h_b      (0 for DISC4)
-  float k_hb_lo, k_her_lo;  // float64 value minus its fp32 rounding (the constants multiply rho ~ 10 kpc)
   float inv_wh, inv_rh;
   float k_hr, k_hz;  // -log2(e)/h_r, -2 log2(e)/h_z
   float k_her, k_hez;
@@ -235,46 +203,44 @@ struct AnalyticAux {
   float thz, thez;         // tanh(z/h_z), tanh(z/h_ez)
 };
 
-// kFastTrig: sin/cos of the pitch and tilt angles on the MUFU (abs err 5e-7: enough for the 1e-3 gradient bound)
-template <bool kHalo, bool kAcc = false, bool kFastTrig = false>
-__device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Triad& T, float x, float y,
-                                                  float z, float rho2, bool inside, SampleF& S,
-                                                  AnalyticAux& a) {
-  // kAcc: everything the Faraday integrand n_e B_LOS depends on is evaluated so that no error is
-  // systematic along the sightline above ~1e-8 (Newton-corrected reciprocals/roots, FMA-pipe
-  // exponentials, hi+lo constants); N_0 (emission only) stays on the MUFU.
+// The part of the analytic evaluation that does not depend on the model parameters (S:8(a) A12: shared by the
+// parameter vectors of a batch): cylindrical geometry, ln(rho/8), tanh(z / 1 kpc).  4 MUFU.
+struct SharedGeomF {
+  float ir, rho, xr, yr;   // 1/rho, rho, x/rho, y/rho
+  float lr;                // ln(rho/8)
+  float az, t;             // |z|, tanh(z / 1 kpc)
+};
+__device__ __forceinline__ void analytic_shared_f32(float x, float y, float z, float rho2, SharedGeomF& g) {
   const float kLog2e = 1.4426950408889634f;
   rho2 = fmaxf(rho2, 1.0e-30f);
-  if (kAcc) {
-    rsqrt_sqrt_nr(rho2, a.ir, a.rho);
-  } else {
-    a.ir = mufu_rsqrt(rho2);
-    a.rho = rho2 * a.ir;
-  }
-  a.xr = x * a.ir; a.yr = y * a.ir;
-  const float az = fabsf(z);
+  g.ir = mufu_rsqrt(rho2);
+  g.rho = rho2 * g.ir;
+  g.xr = x * g.ir; g.yr = y * g.ir;
+  g.az = fabsf(z);
+  g.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;        // ln(rho/8) = ln2/2 (lg2 rho^2 - 6)
+  const float e1 = mufu_ex2(-2.0f * kLog2e * g.az);             // tanh(|z|) = (1-e)/(1+e)
+  g.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
+}
+
+// The parameter-dependent part.  kFastTrig: sin/cos of the pitch and tilt angles on the MUFU (abs err 5e-7: enough for
+// the 1e-3 gradient bound)
+template <bool kHalo, bool kFastTrig>
+__device__ __forceinline__ void analytic_fields_f32(const BatchConsts& P, const Triad& T, const SharedGeomF& g, float z,
+                                                    bool inside, SampleF& S, AnalyticAux& a) {
+  const float kLog2e = 1.4426950408889634f;
+  a.ir = g.ir; a.rho = g.rho; a.xr = g.xr; a.yr = g.yr; a.lr = g.lr; a.t = g.t;
+  const float az = g.az;
   // --- disc: B = A [cos psi cos chi rho_hat + sin psi cos chi phi_hat + sin chi z_hat]   Eq.(13)
-  a.lr = (mufu_lg2(rho2) - 6.0f) * 0.34657359027997264f;        // ln(rho/8) = ln2/2 (lg2 rho^2 - 6)
   const float psi = fmaf(P.p[2], a.lr, P.p[1]);
   if (kFastTrig) { a.sp = mufu_sin(psi); a.cp = mufu_cos(psi); }
   else if (P.angles_small) sincos_fma_small(psi, a.sp, a.cp);
   else sincos_fma(psi, a.sp, a.cp);
-  if (kAcc) {
-    const float e1 = exp2_fma(-2.0f * kLog2e * az);             // tanh(|z|) = (1-e)/(1+e)
-    a.t = copysignf((1.0f - e1) * rcp_nr(1.0f + e1), z);
-  } else {
-    const float e1 = mufu_ex2(-2.0f * kLog2e * az);
-    a.t = copysignf((1.0f - e1) * mufu_rcp(1.0f + e1), z);
-  }
   const float chi = P.p[3] * a.t;
   if (kFastTrig) { a.sc = mufu_sin(chi); a.cc = mufu_cos(chi); }
   else if (P.angles_small) sincos_fma_small(chi, a.sc, a.cc);
   else sincos_fma(chi, a.sc, a.cc);
   float rad = 1.0f;
-  if (P.k_hb != 0.0f) {
-    const float dr = a.rho - 8.0f;
-    rad = kAcc ? exp2_fma(fmaf(P.k_hb, dr, P.k_hb_lo * dr)) : mufu_ex2(P.k_hb * dr);
-  }
+  if (P.k_hb != 0.0f) rad = mufu_ex2(P.k_hb * (a.rho - 8.0f));
   a.A = inside ? rad : 0.0f;
   const float Ab = P.p[0] * a.A;
   const float Brho = Ab * a.cp * a.cc;
@@ -283,19 +249,13 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
   if (kHalo) {  // toroidal halo, S:App.C
     a.u = (az - P.p[6]) * P.inv_wh;
     const float q = a.rho * P.inv_rh;
-    if (kAcc) {
-      a.L = rcp_nr(fmaf(a.u, a.u, 1.0f));
-      a.R = q * exp2_fma(kLog2e * (1.0f - q));
-    } else {
-      a.L = mufu_rcp(fmaf(a.u, a.u, 1.0f));
-      a.R = q * mufu_ex2(kLog2e * (1.0f - q));
-    }
+    a.L = mufu_rcp(fmaf(a.u, a.u, 1.0f));
+    a.R = q * mufu_ex2(kLog2e * (1.0f - q));
     Bphi = fmaf(P.p[5] * a.L, a.R, Bphi);
   }
   const float Bx = Brho * a.xr - Bphi * a.yr;
   const float By = fmaf(Brho, a.yr, Bphi * a.xr);
   S.Bpar = fmaf(Bx, T.nx, fmaf(By, T.ny, Bz * T.nz));           // B.n, signed (S:C-2#3)
-  if (kAcc) S.Bpar += fmaf(Bx, T.nxl, fmaf(By, T.nyl, Bz * T.nzl));
   S.BN = fmaf(Bx, T.eNx, fmaf(By, T.eNy, Bz * T.eNz));          // Eq.(8) numerator
   S.BE = fmaf(Bx, T.eEx, By * T.eEy);                           // Eq.(8) denominator (S:C-2#4)
   // --- N_0 = n0 exp(-rho/h_r) sech^2(z/h_z)  Eq.(12);  sech^2 w = 4e/(1+e)^2, e = exp(-2|w|)
@@ -305,21 +265,21 @@ __device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Tr
   a.N0u = 4.0f * mufu_ex2(P.k_hr * a.rho) * ez * iz;
   S.N0 = P.p[9] * a.N0u;
   a.thz = copysignf((1.0f - ez) * dz * iz, z);                  // tanh = (1-e)/(1+e)
-  if (kAcc) {
-    const float ee = exp2_fma(P.k_hez * az);
-    const float de = 1.0f + ee;
-    const float ie = rcp_nr(de * de);
-    a.neu = 4.0f * exp2_fma(fmaf(P.k_her, a.rho, P.k_her_lo * a.rho)) * ee * ie;
-    S.ne = P.p[13] * a.neu;
-    a.thez = copysignf((1.0f - ee) * de * ie, z);
-  } else {
-    const float ee = mufu_ex2(P.k_hez * az);
-    const float de = 1.0f + ee;
-    const float ie = mufu_rcp(de * de);
-    a.neu = 4.0f * mufu_ex2(P.k_her * a.rho) * ee * ie;
-    S.ne = P.p[13] * a.neu;
-    a.thez = copysignf((1.0f - ee) * de * ie, z);
-  }
+  const float ee = mufu_ex2(P.k_hez * az);
+  const float de = 1.0f + ee;
+  const float ie = mufu_rcp(de * de);
+  a.neu = 4.0f * mufu_ex2(P.k_her * a.rho) * ee * ie;
+  S.ne = P.p[13] * a.neu;
+  a.thez = copysignf((1.0f - ee) * de * ie, z);
+}
+
+template <bool kHalo, bool kFastTrig = false>
+__device__ __forceinline__ void eval_analytic_f32(const BatchConsts& P, const Triad& T, float x, float y,
+                                                  float z, float rho2, bool inside, SampleF& S,
+                                                  AnalyticAux& a) {
+  SharedGeomF g;
+  analytic_shared_f32(x, y, z, rho2, g);
+  analytic_fields_f32<kHalo, kFastTrig>(P, T, g, z, inside, S, a);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -384,44 +344,6 @@ __device__ __forceinline__ void eval_stack16_f32(const BatchConsts& P, const Tri
 // Used only for sightlines whose Faraday rotation is so large that fp32 round-off in n_e B_LOS
 // would exceed the parity tolerance.
 // ------------------------------------------------------------------------------------------------
-struct SampleD { double Bpar, BN, BE, N0, ne; };
-
-template <bool kHalo>
-__device__ __forceinline__ void eval_analytic_f64(const BatchConsts& P, const double4 dir, double x, double y,
-                                                  double z, SampleD& S) {
-  const double rho2 = x * x + y * y;
-  const double rho = sqrt(rho2);
-  const bool inside = (rho2 > 9.0) && (rho2 < 400.0);
-  double Brho = 0.0, Bphi = 0.0, Bz = 0.0;
-  const double az = fabs(z);
-  if (inside) {
-    const double psi = (double)P.p[1] + (double)P.p[2] * log(rho * 0.125);
-    const double chi = (double)P.p[3] * tanh(z);
-    double sp, cp, sc, cc;
-    sincos(psi, &sp, &cp);
-    sincos(chi, &sc, &cc);
-    double A = (double)P.p[0];
-    if (P.k_hb != 0.0f) A *= exp(-(rho - 8.0) / (double)P.p[4]);
-    Brho = A * cp * cc; Bphi = A * sp * cc; Bz = A * sc;
-  }
-  if (kHalo) {
-    const double u = (az - (double)P.p[6]) / (double)P.p[8];
-    const double q = rho / (double)P.p[7];
-    Bphi += (double)P.p[5] / (1.0 + u * u) * q * exp(1.0 - q);
-  }
-  const double ir = (rho > 0.0) ? 1.0 / rho : 0.0;
-  const double xr = x * ir, yr = y * ir;
-  const double Bx = Brho * xr - Bphi * yr, By = Brho * yr + Bphi * xr;
-  const double cl = dir.x, sl = dir.y, cb = dir.z, sb = dir.w;
-  S.Bpar = Bx * (cb * cl) + By * (cb * sl) + Bz * sb;
-  S.BN = Bz * cb - sb * (Bx * cl + By * sl);
-  S.BE = By * cl - Bx * sl;
-  const double chz = cosh(z / (double)P.p[11]);
-  S.N0 = (double)P.p[9] * exp(-rho / (double)P.p[10]) / (chz * chz);
-  const double che = cosh(z / (double)P.p[15]);
-  S.ne = (double)P.p[13] * exp(-rho / (double)P.p[14]) / (che * che);
-}
-
 // digamma for x > 0 (prologue only)
 __device__ inline double digamma_d(double x) {
   double r = 0.0;

@@ -5,12 +5,6 @@
 
 namespace synax {
 
-#ifndef SYNAX_FWD_FASTTRIG
-#define SYNAX_FWD_FASTTRIG false
-#endif
-#ifndef SYNAX_FAST_ACC
-#define SYNAX_FAST_ACC false
-#endif
 constexpr int kBlock = 128;   // threads per CTA for the sightline kernels
 constexpr int kTile = 32;     // samples between re-basing of the local Faraday sum
 constexpr int kTileDMax = 16;  // float64-chain kernel: at most this many samples per tile (BatchConsts::tile_d)
@@ -138,7 +132,7 @@ __device__ __forceinline__ float roundoff_scale_estimate(const Geometry& geo, co
         eval_stack16_f32<true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, sa);
       } else {
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
       if ((CODE == kAnalyticDisc || CODE == kStack16) && sg_ne.g) S.ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
     }
@@ -209,7 +203,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
         const double rho2d = fma(xd, xd, yd * yd);
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull, SYNAX_FAST_ACC, SYNAX_FWD_FASTTRIG>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
       }
       if (CODE == kAnalyticDisc || CODE == kStack16) {
         if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
@@ -275,6 +269,100 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
     if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)sl;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Forward, fp32 chain, batched (S:8(a) A12, "batch acceleration"): one thread integrates the SAME sightline for
+// NB consecutive parameter vectors of the batch, so everything that does not depend on the parameters -- the float64
+// sample position and annulus test, their four conversions to fp32, 1/rho, ln(rho/8), tanh z (8 of the ~29 XU
+// operations per sample and vector at cfg 2, where this kernel is XU-bound) -- is evaluated once per sample instead
+// of once per vector.  One frequency, one thread per sightline (the shape of HMC-style batches: many vectors, modest
+// maps).  Per vector the arithmetic, and so every map value, is that of forward_kernel<CODE, 1, 1, false>.
+// ------------------------------------------------------------------------------------------------
+template <int CODE, int NB>
+__global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_constant__ ForwardArgs A,
+                                                                 const __grid_constant__ FreqTab ft) {
+  static_assert(CODE == kAnalyticDisc || CODE == kAnalyticFull, "analytic models only");
+  if (A.mode && *A.mode != kModeFastThenList) return;
+  const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const int n_groups = (A.batch + NB - 1) / NB;
+  if (tid >= A.geo.npix * n_groups) return;
+  const int bg = (int)(tid / A.geo.npix);
+  const int64_t pix = tid - (int64_t)bg * A.geo.npix;
+  int bj[NB];
+  bool live[NB];
+#pragma unroll
+  for (int j = 0; j < NB; ++j) { live[j] = bg * NB + j < A.batch; bj[j] = live[j] ? bg * NB + j : A.batch - 1; }
+  const Triad T = load_triad(A.geo, pix);
+  const double delta = A.geo.delta * T.scale;
+  double s_d = 0.5 * delta;
+  const float k_rad = ft.k_rad[0];
+
+  float accI[NB], accQ[NB], accU[NB], gabs[NB];
+  double carry[NB];
+#pragma unroll
+  for (int j = 0; j < NB; ++j) { accI[j] = 0.f; accQ[j] = 0.f; accU[j] = 0.f; gabs[j] = 0.f; carry[j] = 0.0; }
+  for (int ts = 0; ts < A.geo.n_los; ts += kTile) {
+    const int te = min(ts + kTile, A.geo.n_los);
+    float hi[NB], lo[NB], tq[NB], tu[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) { hi[j] = 0.f; lo[j] = 0.f; tq[j] = 0.f; tu[j] = 0.f; }
+    for (int n = ts; n < te; ++n) {
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      s_d += delta;
+      const double rho2d = fma(xd, xd, yd * yd);
+      const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+      const float zf = (float)zd;
+      SharedGeomF geom;
+      analytic_shared_f32((float)xd, (float)yd, zf, (float)rho2d, geom);
+#pragma unroll
+      for (int j = 0; j < NB; ++j) {
+        const BatchConsts& P = A.bc[bj[j]];
+        SampleF S;
+        AnalyticAux aux;
+        analytic_fields_f32<CODE == kAnalyticFull, false>(P, T, geom, zf, inside, S, aux);
+        S.ne *= T.scalef;
+        float eI, a, bq;
+        emission(P, S.BN, S.BE, S.N0, eI, a, bq);
+        accI[j] += eI;
+        const float gn = S.ne * S.Bpar;
+        gabs[j] = fmaf(fabsf(S.ne), fabsf(S.Bpar) + fabsf(S.BN) + fabsf(S.BE), gabs[j]);
+        const float ph = fmaf(0.5f, gn, hi[j]);
+        const float sum = hi[j] + gn;
+        lo[j] += gn - (sum - hi[j]);
+        hi[j] = sum;
+        const float th = k_rad * ph;
+        const float c = mufu_cos(th), sn = mufu_sin(th);
+        tq[j] = fmaf(a, c, fmaf(-bq, sn, tq[j]));
+        tu[j] = fmaf(a, sn, fmaf(bq, c, tu[j]));
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      if (ts == 0) {
+        accQ[j] = tq[j]; accU[j] = tu[j];
+      } else {
+        rotate_by_offset(ft.k_turn[0], carry[j], tq[j], tu[j]);
+        accQ[j] += tq[j]; accU[j] += tu[j];
+      }
+      carry[j] += (double)hi[j] + (double)lo[j];
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    if (!live[j]) continue;
+    const BatchConsts& P = A.bc[bj[j]];
+    const int64_t o = ((int64_t)bj[j] * A.n_freq_total + A.f0) * A.geo.npix + pix;
+    A.I[o] = P.coefI[A.f0] * T.scalef * accI[j];
+    A.Q[o] = P.coefP[A.f0] * T.scalef * accQ[j];
+    A.U[o] = P.coefP[A.f0] * T.scalef * accU[j];
+    if (A.f0 == 0 && A.flag_S > 0.0f && gabs[j] > A.flag_S) {
+      const int k = atomicAdd(A.append_count, 1);
+      A.append_list[k] = (int)((int64_t)bj[j] * A.geo.npix + pix);
     }
   }
 }

@@ -38,6 +38,17 @@ void fwd_launch_fast(bool list, int G, int nf, int64_t n_sl, cudaStream_t st, co
   else launch_forward_g<CODE, false>(G, nf, n_sl, st, a, ft);
 }
 
+template <int CODE>
+void fwd_launch_batched(int nb, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
+  if constexpr (CODE == kAnalyticDisc || CODE == kAnalyticFull) {
+    const FreqTab ft = shift_freqs(ft0, a.f0);
+    const int64_t threads = a.geo.npix * ((a.batch + nb - 1) / nb);
+    const unsigned blocks = (unsigned)((threads + kBlock - 1) / kBlock);
+    if (nb == 4) forward_batched_kernel<CODE, 4><<<blocks, kBlock, 0, st>>>(a, ft);
+    else forward_batched_kernel<CODE, 2><<<blocks, kBlock, 0, st>>>(a, ft);
+  }
+}
+
 template <int CODE, int G>
 static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
@@ -60,6 +71,7 @@ void fwd_launch_f64(int G, int nf, unsigned blocks, cudaStream_t st, const Forwa
   template void fwd_launch_pilot<CODE>(unsigned, cudaStream_t, const ForwardArgs&, int64_t, int64_t, int*);                \
   template void fwd_launch_classify<CODE>(unsigned, cudaStream_t, const ForwardArgs&, int*);                               \
   template void fwd_launch_fast<CODE>(bool, int, int, int64_t, cudaStream_t, const ForwardArgs&, const FreqTab&);          \
+  template void fwd_launch_batched<CODE>(int, cudaStream_t, const ForwardArgs&, const FreqTab&);                           \
   template void fwd_launch_f64<CODE>(int, int, unsigned, cudaStream_t, const ForwardArgs&, const FreqTab&);
 
 }  // namespace synax

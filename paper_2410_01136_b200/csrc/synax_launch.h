@@ -12,10 +12,14 @@ namespace synax {
 template <int CODE> void fwd_launch_pilot(unsigned blocks, cudaStream_t st, const ForwardArgs& a, int64_t stride, int64_t n_pilot, int* ctrl);
 template <int CODE> void fwd_launch_classify(unsigned blocks, cudaStream_t st, const ForwardArgs& a, int* ctrl);
 template <int CODE> void fwd_launch_fast(bool list, int G, int nf, int64_t n_sl, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft);
+// batched fp32 forward (forward_batched_kernel; DISC4 and FULL16, one frequency, one thread per sightline), nb = 2 or 4
+template <int CODE> void fwd_launch_batched(int nb, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft);
 template <int CODE> void fwd_launch_f64(int G, int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft);
 
 // ---- adjoint (synax_vjp_impl.cuh, explicitly instantiated per CODE)
 template <int CODE> void vjp_launch(int pmode, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft);
+// batched lean adjoint (vjp_batched_kernel; DISC4 and FULL16), nb = 2 or 4, grid = (n_blocks, ceil(batch / nb))
+template <int CODE> void vjp_launch_batched(int nb, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft);
 template <int CODE> void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, const VjpArgs& a, unsigned char* cta_sel);
 
 // dispatch on the run-time model code (kAnalyticDisc, kAnalyticFull, kStack16, kUniform)
@@ -30,7 +34,7 @@ template <int CODE> void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, 
 // ---- synax_vjp_driver.cu
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                           const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
-                          const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int* ctrl,
+                          const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, int* ctrl,
                           cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
                           const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
                           int64_t* launches);

@@ -117,13 +117,11 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
   for (int j = 0; j < 16; ++j) c.p[j] = (float)p[j];
   const double log2e = 1.4426950408889634;
   c.k_hb = (code == kAnalyticFull) ? (float)(-log2e / p[4]) : 0.0f;
-  c.k_hb_lo = (code == kAnalyticFull) ? (float)(-log2e / p[4] - (double)c.k_hb) : 0.0f;
   c.inv_wh = (float)(1.0 / p[8]);
   c.inv_rh = (float)(1.0 / p[7]);
   c.k_hr = (float)(-log2e / p[10]);
   c.k_hz = (float)(-2.0 * log2e / fabs(p[11]));
   c.k_her = (float)(-log2e / p[14]);
-  c.k_her_lo = (float)(-log2e / p[14] - (double)c.k_her);
   c.k_hez = (float)(-2.0 * log2e / fabs(p[15]));
   c.q_exp = (float)((alpha - 3.0) * 0.25);
   c.pi_frac = (float)((alpha + 1.0) / (alpha + 7.0 / 3.0));

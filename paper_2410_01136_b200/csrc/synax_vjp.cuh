@@ -351,7 +351,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
+        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
         if (CODE == kAnalyticDisc && A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
       }
@@ -412,7 +412,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         S.N0 = P.uN0; S.ne = P.une;
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
-        eval_analytic_f32<CODE == kAnalyticFull, false, true>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
+        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
                                                  (rho2d > 9.0) && (rho2d < 400.0), S, aux);
         if (CODE == kAnalyticDisc) {
           if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
@@ -506,6 +506,141 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
     for (int k = 0; k < kBlock / 32; ++k) v += red[k][threadIdx.x];
     float* dst = A.partial + ((size_t)b * A.n_blocks + blockIdx.x) * 16 + threadIdx.x;
     *dst = A.accumulate ? (*dst + v) : v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Adjoint, batched (S:8(a) A12): the lean variant (fp32 Faraday angles, one thread per sightline, one frequency) for NB
+// consecutive parameter vectors per thread, sharing the sample geometry as forward_batched_kernel does.  Per vector the
+// arithmetic is that of vjp_kernel<CODE, 1, 1, 0>.  grid = (n_blocks, ceil(batch / NB)).
+// ------------------------------------------------------------------------------------------------
+template <int CODE, int NB>
+__global__ void __launch_bounds__(kBlock) vjp_batched_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
+  static_assert(CODE == kAnalyticDisc || CODE == kAnalyticFull, "analytic models only");
+  constexpr bool kAlpha = CODE == kAnalyticFull;
+  if (A.mode) {   // runs where the lean fp32 variant would
+    const int m = *A.mode;
+    if (m == kModeSplit || m == kModeAllF64) return;
+  }
+  int64_t pix = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  const bool valid = pix < A.geo.npix;
+  if (!valid) pix = A.geo.npix - 1;
+  int bj[NB];
+  bool live[NB];
+#pragma unroll
+  for (int j = 0; j < NB; ++j) { live[j] = (int)blockIdx.y * NB + j < A.batch; bj[j] = live[j] ? (int)blockIdx.y * NB + j : A.batch - 1; }
+  const Triad T = load_triad(A.geo, pix);
+  const double delta = A.geo.delta * T.scale;
+  const float k_rad = ft.k_rad[0], ln_nu = ft.ln_nu[0];
+
+  typename GradOf<CODE>::type acc[NB];
+  float cI[NB], cIa[NB], cq[NB], cu[NB], gAlpha[NB], sumE[NB], gPol[NB], cPol[NB], Pl[NB];
+  double carry[NB];
+#pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    const BatchConsts& P = A.bc[bj[j]];
+    const int64_t o = ((int64_t)bj[j] * A.n_freq_total + A.f0) * A.geo.npix + pix;
+    const bool on = valid && live[j];
+    const float vI = (on && A.dI) ? A.dI[o] : 0.f;
+    cI[j] = vI * P.coefI[A.f0] * T.scalef;
+    cIa[j] = kAlpha ? vI * P.coefI[A.f0] * P.dlnc_dalpha[A.f0] * T.scalef : 0.f;
+    cq[j] = (on && A.dQ) ? __ldg(A.dQ + o) * P.coefP[A.f0] * T.scalef : 0.f;
+    cu[j] = (on && A.dU) ? __ldg(A.dU + o) * P.coefP[A.f0] * T.scalef : 0.f;
+    cPol[j] = kAlpha ? P.dlnA_dalpha + P.dpi_dalpha_over_pi : 0.f;
+    acc[j].zero();
+    gAlpha[j] = 0.f; sumE[j] = 0.f; gPol[j] = 0.f; Pl[j] = 0.f; carry[j] = 0.0;
+  }
+  double s_d = 0.5 * delta;
+  for (int ts = 0; ts < A.geo.n_los; ts += kTile) {
+    const int te = min(ts + kTile, A.geo.n_los);
+    float rq[NB], ru[NB], hi[NB], lo[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {   // cotangents rotated by the Faraday angle of everything before this tile
+      float q = cq[j], u = cu[j];
+      rotate_by_offset(-ft.k_turn[0], carry[j], q, u);
+      rq[j] = q; ru[j] = u; hi[j] = 0.f; lo[j] = 0.f;
+    }
+    for (int n = ts; n < te; ++n) {
+      const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
+      const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
+      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
+      s_d += delta;
+      const double rho2d = fma(xd, xd, yd * yd);
+      const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
+      const float zf = (float)zd;
+      SharedGeomF geom;
+      analytic_shared_f32((float)xd, (float)yd, zf, (float)rho2d, geom);
+#pragma unroll
+      for (int j = 0; j < NB; ++j) {
+        const BatchConsts& P = A.bc[bj[j]];
+        SampleF S;
+        AnalyticAux aux;
+        analytic_fields_f32<CODE == kAnalyticFull, true>(P, T, geom, zf, inside, S, aux);
+        S.ne *= T.scalef;
+        const float bn2 = S.BN * S.BN, be2 = S.BE * S.BE;
+        const float Bt2 = bn2 + be2;
+        float w = 1.0f, lgB = 0.f;
+        if (kAlpha || !P.alpha_is_3) {
+          lgB = (Bt2 > 0.f) ? mufu_lg2(Bt2) : 0.f;
+          if (!P.alpha_is_3) w = (Bt2 > 0.f) ? mufu_ex2(P.q_exp * lgB) : 0.f;
+        }
+        const float M = w * S.N0;
+        const float d2 = be2 - bn2, p2 = 2.0f * S.BE * S.BN;
+        const float a = M * d2, bq = M * p2;
+        const float gn = S.ne * S.Bpar;
+        const float ph = fmaf(0.5f, gn, hi[j]);
+        const float sum = hi[j] + gn;
+        lo[j] += gn - (sum - hi[j]);
+        hi[j] = sum;
+        const float th = k_rad * ph;
+        const float c = mufu_cos(th), sn = mufu_sin(th);
+        const float Xc = fmaf(rq[j], c, ru[j] * sn);
+        const float Xs = fmaf(ru[j], c, -rq[j] * sn);
+        const float Yc = k_rad * Xc, Ys = k_rad * Xs;
+        if (kAlpha) gPol[j] = fmaf(a, fmaf(cPol[j], Xc, -0.5f * ln_nu * Xc), fmaf(bq, fmaf(cPol[j], Xs, -0.5f * ln_nu * Xs), gPol[j]));
+        const float K = fmaf(cI[j], Bt2, fmaf(Xc, d2, Xs * p2));
+        const float MK = M * K;
+        sumE[j] = fmaf(M, Bt2, sumE[j]);
+        if (kAlpha) gAlpha[j] = fmaf(lgB, MK, gAlpha[j]);
+        const float Sbar = fmaf(a, Ys, -bq * Yc);
+        Pl[j] += Sbar;
+        float tq_ = 0.f;
+        if (!P.alpha_is_3 && Bt2 > 0.f) tq_ = P.q_exp * MK * mufu_rcp(Bt2);
+        const float BEb = 2.0f * fmaf(M, fmaf(S.BE, cI[j] + Xc, S.BN * Xs), S.BE * tq_);
+        const float BNb = 2.0f * fmaf(M, fmaf(S.BN, cI[j] - Xc, S.BE * Xs), S.BN * tq_);
+        acc[j].add(P, T, aux, S, zf, BNb, BEb, Sbar, w * aux.N0u * K);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NB; ++j) carry[j] += (double)hi[j] + (double)lo[j];
+  }
+  constexpr int NP = CODE == kAnalyticFull ? 16 : 4;
+  __shared__ float red[kBlock / 32][16];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+  for (int j = 0; j < NB; ++j) {
+    const BatchConsts& P = A.bc[bj[j]];
+    float out[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) out[k] = 0.f;
+    acc[j].finish(P, out);
+    if (kAlpha) out[12] = fmaf(0.25f * 0.6931471805599453f, gAlpha[j], fmaf(cIa[j], sumE[j], gPol[j]));
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+      float v = out[k];
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+      if (lane == 0) red[wid][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < NP && live[j]) {
+      float v = 0.f;
+#pragma unroll
+      for (int k = 0; k < kBlock / 32; ++k) v += red[k][threadIdx.x];
+      float* dst = A.partial + ((size_t)bj[j] * A.n_blocks + blockIdx.x) * 16 + threadIdx.x;
+      *dst = A.accumulate ? (*dst + v) : v;
+    }
+    __syncthreads();
   }
 }
 

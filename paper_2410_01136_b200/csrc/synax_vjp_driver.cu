@@ -13,6 +13,16 @@ static void launch_pmode(int code, int pmode, int G, int nf, dim3 grid, cudaStre
   SYNAX_DISPATCH_CODE(code, vjp_launch, pmode, G, nf, grid, st, a, ft);
 }
 
+// the lean fp32 variant, or its batched form (nb parameter vectors per thread sharing the sightline geometry, A12)
+static void launch_lean(int code, int nb, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
+  if (nb > 1) {
+    const dim3 gb(grid.x, (unsigned)((a.batch + nb - 1) / nb));
+    SYNAX_DISPATCH_CODE(code, vjp_launch_batched, nb, gb, st, a, ft);
+  } else {
+    launch_pmode(code, 0, G, nf, grid, st, a, ft);
+  }
+}
+
 // partial[b][n_blocks][16] -> grad[b][n_params], float64 accumulation, deterministic order
 __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_blocks, int n_params, float* __restrict__ grad) {
   const int b = blockIdx.x;
@@ -39,7 +49,7 @@ constexpr double kVjpEscalateFactor = 10.0 / 3.0;   // x escalate_rad (300 rad b
 
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                                  const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
-                                 const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int* ctrl,
+                                 const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, int* ctrl,
                                  cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
                                  const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
                                  int64_t* launches) {
@@ -74,6 +84,11 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   unsigned char* cta_sel = nullptr;
   if (split && cudaMallocAsync((void**)&cta_sel, (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
     return SYNAX_ERR_ALLOC;
+  // measured at cfg 2 (256 vectors, B200): sharing pays in the forward (5.09 -> 4.68 ms at 4 vectors per thread) but not here
+  // -- two or four sets of 27 gradient accumulators per thread cost more occupancy than the shared geometry saves (8.46 ->
+  // 8.82 / 9.53 ms) -- so the adjoint shares only on request (option "batch_share")
+  int nb = batch_share ? batch_share : 1;
+  if (!(G == 1 && ft.n_freq == 1 && (code == kAnalyticDisc || code == kAnalyticFull) && !sg_ne.g && !sg_n0.g && batch <= 65535)) nb = 1;
   float* partial = nullptr;
   if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess) {
     if (cta_sel) cudaFreeAsync(cta_sel, st);
@@ -95,10 +110,10 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
       const int rem = ft.n_freq - f0;
       const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
       a.f0 = f0; a.accumulate = f0 > 0;
-      if (precision == 1) launch_pmode(code, 0, G, nf, grid, st, a, ft);
+      if (precision == 1) launch_lean(code, nb, G, nf, grid, st, a, ft);
       else if (precision == 2) launch_pmode(code, 1, G, nf, grid, st, a, ft);
       else {
-        launch_pmode(code, 0, G, nf, grid, st, a, ft);
+        launch_lean(code, nb, G, nf, grid, st, a, ft);
         if (split) {
           // the per-CTA pair (runs in kModeSplit).  Every CTA's partial belongs to exactly one member, so the two run
           // concurrently: the float64-angle member (few, long CTAs: 2.7 waves at cfg 4) on the plan's second stream,

@@ -12,6 +12,15 @@ void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, const VjpArgs& a, un
   else vjp_classify_kernel<CODE, 32><<<grid, kBlock, 0, st>>>(a, cta_sel);
 }
 
+template <int CODE>
+void vjp_launch_batched(int nb, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft0) {
+  if constexpr (CODE == kAnalyticDisc || CODE == kAnalyticFull) {
+    const FreqTab ft = shift_freqs(ft0, a.f0);
+    if (nb == 4) vjp_batched_kernel<CODE, 4><<<grid, kBlock, 0, st>>>(a, ft);
+    else vjp_batched_kernel<CODE, 2><<<grid, kBlock, 0, st>>>(a, ft);
+  }
+}
+
 template <int CODE, int G, int PMODE>
 static void launch_vjp_nf(int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
@@ -38,6 +47,7 @@ void vjp_launch(int pmode, int G, int nf, dim3 grid, cudaStream_t st, const VjpA
 
 #define SYNAX_INSTANTIATE_VJP(CODE)                                                                           \
   template void vjp_launch<CODE>(int, int, int, dim3, cudaStream_t, const VjpArgs&, const FreqTab&);           \
+  template void vjp_launch_batched<CODE>(int, dim3, cudaStream_t, const VjpArgs&, const FreqTab&);             \
   template void vjp_launch_classify<CODE>(int, dim3, cudaStream_t, const VjpArgs&, unsigned char*);
 
 }  // namespace synax

@@ -1,0 +1,71 @@
+"""Batched calls share the sightline geometry between NB parameter vectors per thread (PAPER.md L13
+"batch acceleration"): per vector the arithmetic is unchanged, so the maps are BIT-identical to the unshared path and the
+gradients agree to rounding of the block sums."""
+import numpy as np
+import pytest
+
+import parity
+from paper_2410_01136_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("kind,batch", [("full16", 7), ("full16", 8), ("disc4", 5), ("full16", 2)])
+def test_shared_geometry_is_bit_identical_and_matches_oracle(kind, batch):
+    if kind == "full16":
+        w = wl.config(2).scaled(nside=8, n_los=200, batch=batch)
+    else:
+        w = wl.config(1).scaled(nside=8, n_los=200)
+        w.freqs = np.array([23e9])
+        rng = np.random.Generator(np.random.PCG64(77))
+        w.params = (w.params[0][None, :] * (1.0 + 0.2 * rng.uniform(-1, 1, (batch, 4)))).astype(np.float32)
+    ref_maps, _ = parity.gpu_forward(w, lanes=1, batch_share=1)
+    cots = w.cotangents()
+    g1 = parity.gpu_vjp(w, cots, lanes=1, batch_share=1)
+    oracle_maps = parity.oracle_forward(w)
+    oracle_grad = parity.oracle_vjp(w, cots)
+    for nb in (0, 2, 4):
+        maps, _ = parity.gpu_forward(w, lanes=1, batch_share=nb)
+        for a, b in zip(maps, ref_maps):
+            if kind == "full16":
+                assert np.array_equal(a, b), (kind, batch, nb)
+            else:   # DISC4: the compiler contracts a few multiply-adds differently in the two kernels (last-bit differences)
+                assert np.all(np.abs(a - b) <= 3e-7 * np.abs(b)), (kind, batch, nb)
+        parity.assert_maps_close(maps, oracle_maps, what=f"batch_share={nb}")
+        g = parity.gpu_vjp(w, cots, lanes=1, batch_share=nb)
+        assert np.all(np.abs(g - g1) <= 2e-6 * np.abs(g1).max(axis=1, keepdims=True)), (nb, np.abs(g - g1).max())
+        nz = oracle_grad != 0
+        assert np.all(np.abs(g - oracle_grad)[nz] <= parity.GRAD_TOL * np.abs(oracle_grad)[nz]), nb
+
+
+def test_cfg2_full_launch_shared_vs_unshared():
+    """BASELINE.json configs[2] at full size (256 vectors x 12,288 sightlines): every map value equal to the unshared path."""
+    w = wl.config(2)
+    a, _ = parity.gpu_forward(w, batch_share=1)
+    b, _ = parity.gpu_forward(w)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    cots = w.cotangents()
+    g1, g = parity.gpu_vjp(w, cots, batch_share=1), parity.gpu_vjp(w, cots, batch_share=2)
+    assert np.all(np.abs(g - g1) <= 2e-6 * np.abs(g1).max(axis=1, keepdims=True))
+
+
+def test_batch_share_with_alpha_not_three_and_low_frequency():
+    """alpha != 3 (lg2/ex2 branch) and a call whose pilot sends it to the float64-angle variants: the batched kernels
+    must stand aside (mode word) and the result must not depend on the option."""
+    w = wl.config(2).scaled(nside=8, n_los=256, batch=6)
+    p = w.params.copy(); p[:, 12] = [2.6, 2.8, 3.0, 3.1, 3.3, 3.4]
+    w.params = p
+    cots = w.cotangents()
+    ref = parity.oracle_vjp(w, cots)
+    for nb in (1, 4):
+        g = parity.gpu_vjp(w, cots, lanes=1, batch_share=nb)
+        assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), nb
+    w.freqs = np.array([0.3e9])
+    ref = parity.oracle_vjp(w, cots)
+    refm = parity.oracle_forward(w)
+    for nb in (1, 4):
+        maps, _ = parity.gpu_forward(w, lanes=1, batch_share=nb)
+        parity.assert_maps_close(maps, refm, what=f"300 MHz batch_share={nb}")
+        g = parity.gpu_vjp(w, cots, lanes=1, batch_share=nb)
+        assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), nb
