@@ -10,8 +10,10 @@ fwd+VJP) at nside=256 x 1024 pts").  Default workload = BASELINE.json configs[4]
 multiplied in).  `value` = samples / (forward + VJP time), inputs resident in HBM.  `e2e` = the same
 through synax_forward_host / synax_vjp_host with pinned HOST buffers (copies inside the timed region).
 
-N > 1 (torchrun, one rank per GPU): weak scaling -- every rank integrates the full sky for its own
-parameter vector (independent HMC chains); no data-path collective.
+N > 1 (torchrun, one rank per GPU): the partition of SURVEY.md 8(e) -- contiguous RING pixel shards of ONE map, no
+exchange in the forward, one sum all-reduce of the gradient per VJP ("scaling": "strong": the map is fixed).
+--scaling weak runs independent parameter vectors (HMC chains) per rank instead, with no data-path collective
+(DESIGN.md section 9).
 
 --impl reference: the float64 CPU oracle (oracle/), as it stands, on the host cores, on a bounded pixel
 subset of the same workload; rank 0 only.
@@ -43,8 +45,21 @@ ALG_FP = {
     "grid_b": dict(fwd=(120, 12), vjp=(120 + 60, 12 + 14)),
     "uniform": dict(fwd=(30, 12), vjp=(60, 26)),
 }
-ALG_MUFU = {"disc4": (14, 2), "full16": (19, 2), "grid_b": (10, 2), "uniform": (0, 2)}
+ALG_MUFU = {"disc4": (14, 2), "full16": (19, 2), "grid_b": (10, 2), "uniform": (0, 2), "stack16": (24, 2)}
+ALG_FP["stack16"] = dict(fwd=(110, 12), vjp=(110 + 150, 12 + 14))
 SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16
+
+
+def alg_mufu(kind, n_freq, which):
+    s, f = ALG_MUFU[kind]
+    return s + f * n_freq + (2 if which == "vjp" else 0)     # the adjoint re-evaluates the forward's MUFU work + 2
+
+
+def bound_seconds(kind, n_freq, samples, sm_mhz, legs=("fwd", "vjp")):
+    """cycles per sample = max(FP32 / 128, MUFU / 16) per SM, summed over the legs as ONE instruction mix."""
+    fp = sum(alg_fp(kind, n_freq, leg) for leg in legs)
+    mu = sum(alg_mufu(kind, n_freq, leg) for leg in legs)
+    return max(fp / FP32_LANES, mu / MUFU_LANES) * samples / (SM_COUNT * sm_mhz * 1e6)
 
 
 def alg_fp(kind, n_freq, which):
@@ -120,7 +135,7 @@ def rank_workload(cfg, rank):
     """Weak scaling: rank r > 0 takes the config's model with its own parameter vector(s) (an independent
     chain): each analytic parameter scaled by (1 + 0.05 u), u ~ U[-1,1] from seed 7000 + r.  Rank 0 is the
     config as BASELINE.json states it."""
-    from paper_2410_01136_b200 import workloads as wl
+    from harness import workloads as wl
     w = wl.config(cfg)
     if rank > 0 and w.kind != "grid_b":
         rng = np.random.Generator(np.random.PCG64(7000 + rank))
@@ -156,8 +171,7 @@ def oracle_sample_pixels(w, target_samples):
 
 def oracle_step(w, pix, cots_sub):
     """One forward + VJP of the oracle over the pixel subset; returns seconds."""
-    sys.path.insert(0, str(ROOT / "tests"))
-    import parity
+    from harness import parity
     t = time.perf_counter()
     parity.oracle_forward(w, pix=pix)
     t1 = time.perf_counter()
@@ -166,10 +180,19 @@ def oracle_step(w, pix, cots_sub):
     return t1 - t, t2 - t1
 
 
-def oracle_baseline(w, seconds_budget=15.0, steps=1, warmup=0):
+def oracle_baseline(w, seconds_budget=15.0, steps=1, warmup=0, threads=None):
     import oracle
     oracle.build()
-    cores = oracle.num_threads()
+    all_cores = oracle.num_threads()
+    if threads is not None:
+        oracle.set_num_threads(threads)
+    try:
+        return _oracle_baseline(w, seconds_budget, steps, warmup, oracle.num_threads())
+    finally:
+        oracle.set_num_threads(all_cores)
+
+
+def _oracle_baseline(w, seconds_budget, steps, warmup, cores):
     # ~7 us per sample per core for FULL16 at 8 frequencies forward+VJP (measured on the build box): size the
     # sample so one step is about `seconds_budget` of wall time on this host
     per_sample_core = 1.2e-6 * (1.0 + 0.6 * w.n_freq)
@@ -185,7 +208,7 @@ def oracle_baseline(w, seconds_budget=15.0, steps=1, warmup=0):
         a, b = oracle_step(w, pix, cots_sub)
         tf += a; tv += b
     tf /= steps; tv /= steps
-    return dict(value=n_samples / (tf + tv), unit=UNIT, cores=cores, kind="oracle",
+    return dict(value=n_samples / (tf + tv), unit=UNIT, cores=int(cores), kind="oracle",
                 sample=f"pixels p = 0 (mod {stride}) of {w.name}: {pix.size} sightlines x {w.n_los} samples x batch {w.batch} "
                        f"= {n_samples} LoS samples per step, forward + VJP, float64, OpenMP over sightlines",
                 forward_samples_per_s=n_samples / tf, ms_per_step=1e3 * (tf + tv), samples_per_step=int(n_samples))
@@ -195,7 +218,7 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return 0
-    from paper_2410_01136_b200 import workloads as wl
+    from harness import workloads as wl
     w = apply_overrides(wl.config(args.config), args)
     steps, warmup = max(1, args.steps), max(0, args.warmup)
     # keep the whole run within a few minutes: total oracle time ~ 120 s split over steps + warm-ups
@@ -222,6 +245,8 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     scaling), with the one gradient all-reduce of the method inside the timed VJP when reduce_grad is set."""
     from paper_2410_01136_b200 import sharding
     plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
+    if want_e2e:   # the *_host calls stage hundreds of MB per call in the stream-ordered pool: keep it mapped (opt-in)
+        plan.set_option("pool_release_threshold_mb", 4096)
     npix = plan.npix
     p0 = 0 if pix_range is None else pix_range[0]
     if w.kind == "grid_b":
@@ -256,8 +281,10 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     l1 = plan.stats()["launches"]
     tf = np.array([e[0].elapsed_time(e[1]) for e in evs]) * 1e-3
     tv = np.array([e[1].elapsed_time(e[2]) for e in evs]) * 1e-3
+    stat = lambda a: {"mean": float(1e3 * a.mean()), "median": float(1e3 * np.median(a)), "best": float(1e3 * a.min())}  # noqa: E731
     res = dict(t_fwd=float(tf.mean()), t_vjp=float(tv.mean()), t_fwd_min=float(tf.min()), t_vjp_min=float(tv.min()),
-               launches=int(l1 - l0), escalated=plan.stats()["escalated"])
+               launches=int(l1 - l0), escalated=plan.stats()["escalated"],
+               timing={"forward_ms": stat(tf), "vjp_ms": stat(tv), "step_ms": stat(tf + tv)})
     if graph and not reduce_grad:
         # the whole step captured once in a CUDA graph and replayed (pays off when a step is launch-bound: cfg 0, 1)
         side = torch.cuda.Stream()
@@ -328,6 +355,76 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     return res
 
 
+def wl_config(i):
+    from harness import workloads as wl
+    return wl.config(i)
+
+
+def committed_csv(name):
+    """profiles/<name>: rows of a committed ncu summary as dicts (first line = header), or []."""
+    f = ROOT / "profiles" / name
+    if not f.exists():
+        return []
+    rows = [ln.split(",") for ln in f.read_text().splitlines() if ln.strip() and not ln.startswith("#")]
+    return [dict(zip(rows[0], r)) for r in rows[1:]]
+
+
+def alu_roofline(w, r, local_samples, peak, sm_max, peak_src, strong, clocks):
+    """Analytic path: bound by plain ALU issue.  Dominant kernel = the adjoint."""
+    fp_vjp, fp_fwd = alg_fp(w.kind, w.n_freq, "vjp"), alg_fp(w.kind, w.n_freq, "fwd")
+    achieved = fp_vjp * local_samples / r["t_vjp"] / 1e12
+    t_bound = bound_seconds(w.kind, w.n_freq, local_samples, sm_max)
+    traffic, ncu = None, None
+    if w.name.startswith("cfg4") and not strong:
+        for row in committed_csv("r02_cfg4_dram_traffic.csv"):
+            if row.get("kernel") == "vjp_kernel":
+                traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+        rows = committed_csv("r02_cfg4_pipes.csv")
+        if rows:   # ncu --set full capture of the committed build (profiles/r02_cfg4_ncu_full.md): % of peak, sustained active
+            ncu = {row["kernel"]: {k: float(v) for k, v in row.items() if k != "kernel"} for row in rows}
+    out = {"bound": "alu",
+           "kernel": ("vjp_kernel (analytic adjoint; long calls: vjp_classify_kernel + the fp32-angle / float64-angle pair of vjp_kernel "
+                      "launches on two streams, timed as one call)"),
+           "achieved": achieved, "peak": peak, "unit": "T fp32 lane-instr/s", "frac": achieved / peak, "traffic": traffic,
+           "peak_source": f"148 SM x 128 FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
+           "alg_fp32_per_sample": fp_vjp, "alg_mufu_per_sample": alg_mufu(w.kind, w.n_freq, "vjp"),
+           "forward": {"alg_fp32_per_sample": fp_fwd, "alg_mufu_per_sample": alg_mufu(w.kind, w.n_freq, "fwd"),
+                       "achieved": fp_fwd * local_samples / r["t_fwd"] / 1e12,
+                       "frac": fp_fwd * local_samples / r["t_fwd"] / 1e12 / peak,
+                       "xu_bound_frac": bound_seconds(w.kind, w.n_freq, local_samples, sm_max, legs=("fwd",)) / r["t_fwd"]},
+           # the whole step against SURVEY.md 8(d)'s FP32/SFU bound for forward + VJP (north_star's >= 0.50 bar)
+           "step_bound_ms": 1e3 * t_bound, "step_frac": t_bound / (r["t_fwd"] + r["t_vjp"]),
+           "ncu": ncu}
+    if clocks and clocks.get("sm_mhz"):
+        out["frac_at_sustained_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
+    return out
+
+
+def grid_roofline(w, r, local_samples):
+    """Gridded path: bound by L1/L2 gathers (forward) and L2 vector reductions (adjoint); the ceilings are measured live
+    by the two microbenchmarks of SURVEY.md 8(d) on cfg 3's actual index stream (paper_2410_01136_b200/ubench)."""
+    try:
+        from paper_2410_01136_b200.ubench.__main__ import run as ubench_run
+        txt = ubench_run("grid_streams")
+        m = json.loads([ln for ln in txt.splitlines() if ln.startswith("JSON ")][-1][5:])
+    except Exception as ex:   # no nvcc on the box: say so rather than guess
+        return {"bound": "red", "kernel": "grid_vjp_kernel", "achieved": None, "peak": None, "frac": None, "traffic": None,
+                "note": f"microbenchmarks unavailable: {ex}"}
+    scale = local_samples / m["samples"]      # the microbenchmarks run cfg 3's geometry (49,152 x 512 samples)
+    reds = m["red_v4_count"] * scale
+    return {"bound": "red", "kernel": "grid_vjp_kernel (two sweeps; per-cell register aggregation, red.global.v4.f32.add)",
+            "achieved": reds / r["t_vjp"], "peak": m["red_v4_count"] / (m["red_v4_ms"] * 1e-3), "unit": "red.v4/s",
+            "frac": (m["red_v4_ms"] * 1e-3 * scale) / r["t_vjp"], "traffic": None,
+            "peak_source": "ubench grid_streams (R): red.global.v4.f32.add on the kernel's index stream, per-cell aggregated, measured in this run",
+            "alg_red_v4_per_call": reds,
+            "forward": {"bound": "l2-gather", "kernel": "grid_forward_kernel",
+                        "achieved": m["gather_bytes"] * scale / r["t_fwd"] / 1e9, "peak": m["gather_bytes"] / (m["gather_ms"] * 1e-3) / 1e9,
+                        "unit": "GB/s requested (96 B per in-box sample)", "frac": (m["gather_ms"] * 1e-3 * scale) / r["t_fwd"],
+                        "peak_source": "ubench grid_streams (G): 8-corner x 3 gather on the kernel's index stream, measured in this run",
+                        "frac_vs_padded_gather": (m["gather_v4_ms"] * 1e-3 * scale) / r["t_fwd"]},
+            "ceilings_ms": {k: m[k] for k in ("gather_ms", "gather_v4_ms", "red_v4_ms")}}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -342,7 +439,8 @@ def run_ours(args):
     strong = args.scaling == "strong" and world > 1
     pix_range = None
     if strong:      # one map, pixel shards, one gradient all-reduce per step
-        from paper_2410_01136_b200 import sharding, workloads as wl
+        from paper_2410_01136_b200 import sharding
+        from harness import workloads as wl
         w = apply_overrides(wl.config(args.config), args)
         pix_range = sharding.shard_of(w.npix, rank, world)
     else:           # independent chains: every rank integrates the whole sky for its own parameter vector
@@ -378,26 +476,17 @@ def run_ours(args):
     if rank == 0:
         sm_max, peak_src = peaks()
         peak = SM_COUNT * FP32_LANES * sm_max * 1e6 / 1e12       # T lane-instr/s
-        fp_vjp = alg_fp(w.kind, w.n_freq, "vjp")
-        fp_fwd = alg_fp(w.kind, w.n_freq, "fwd")
-        achieved = fp_vjp * local_samples / r["t_vjp"] / 1e12
-        traffic = None
-        tcsv = ROOT / "profiles" / "r01_dram_traffic.csv"
-        if tcsv.exists() and w.name.startswith("cfg4") and not strong:
-            for row in tcsv.read_text().splitlines()[1:]:
-                c = row.split(",")
-                if c[0] == "vjp_kernel":
-                    traffic = int(c[1]) + int(c[2])
         line = {
             "metric": METRIC, "value": total / t_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "strong" if strong else "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, workloads.py)",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, harness/workloads.py)",
             "config": {"workload": w.name, "nside": w.nside, "n_los": w.n_los, "n_freq": w.n_freq, "batch": w.batch,
                        "model": w.kind, "samples_per_step": samples, "l2": "flushed between timed steps (256 MB write)",
                        "parallelism": ("single GPU" if world == 1 else f"pixel shards x{world} + gradient all-reduce" if strong
                                        else f"independent parameter vectors x{world}")},
             "forward_samples_per_s": total / t_fwd, "vjp_samples_per_s": total / t_vjp,
             "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,
+            "timing": r["timing"],          # per timed step on this rank: mean / median / best, ms
             "sample_freq_per_s": total * w.n_freq / t_step,
             "e2e": {"value": total / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
                     "ms_per_step": 1e3 * t_e2e,
@@ -411,25 +500,19 @@ def run_ours(args):
                         "parameters in and (logL, grad) out per step; observed Q/U maps resident on the device"},
             "gpu_launches": r["launches"], "escalated_sightlines": r["escalated"],
             "clocks": clocks,
-            "roofline": {"bound": "alu", "kernel": ("vjp_kernel (analytic adjoint; long calls: vjp_classify_kernel + the fp32-angle / float64-angle "
-                                    "pair of vjp_kernel launches on two streams, timed as one call)")
-                         if w.kind != "grid_b" else "grid_vjp_kernel",
-                         "achieved": achieved, "peak": peak, "unit": "T fp32 lane-instr/s", "frac": achieved / peak,
-                         "traffic": traffic, "peak_source": f"148 SM x 128 FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
-                         "alg_fp32_per_sample": fp_vjp, "forward": {"alg_fp32_per_sample": fp_fwd,
-                                                                    "achieved": fp_fwd * local_samples / r["t_fwd"] / 1e12,
-                                                                    "frac": fp_fwd * local_samples / r["t_fwd"] / 1e12 / peak}},
         }
+        line["roofline"] = (grid_roofline(w, r, local_samples) if w.kind == "grid_b"
+                            else alu_roofline(w, r, local_samples, peak, sm_max, peak_src, strong, clocks))
         if "t_graph" in r:
             line["cuda_graph"] = {"ms_per_step": 1e3 * r["t_graph"], "value": samples / r["t_graph"], "unit": UNIT,
                                   "note": "forward + VJP captured once, replayed back to back (no L2 flush between replays)"}
-        if clocks and clocks.get("sm_mhz"):
-            line["roofline"]["frac_at_sustained_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
         if world == 1 and not args.no_cpu_baseline:
-            from paper_2410_01136_b200 import workloads as wl
-            line["cpu_baseline"] = {k: v for k, v in oracle_baseline(apply_overrides(wl.config(args.config), args),
-                                                                     seconds_budget=args.cpu_seconds).items()
-                                    if k in ("value", "unit", "cores", "kind", "sample", "forward_samples_per_s")}
+            wo = apply_overrides(wl_config(args.config), args)
+            cb = oracle_baseline(wo, seconds_budget=args.cpu_seconds)
+            line["cpu_baseline"] = {k: v for k, v in cb.items() if k in ("value", "unit", "cores", "kind", "sample", "forward_samples_per_s")}
+            if cb["cores"] > 1:   # the oracle on one core as well, on a 1/cores share of the same sample
+                c1 = oracle_baseline(wo, seconds_budget=args.cpu_seconds / 3.0, threads=1)
+                line["cpu_baseline"]["one_core"] = {k: c1[k] for k in ("value", "unit", "cores", "sample", "forward_samples_per_s")}
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -445,9 +528,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: the metric's workload)")
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
-    ap.add_argument("--scaling", choices=("weak", "strong"), default="weak",
-                    help="N > 1: weak = one parameter vector (chain) per rank, no collective; strong = pixel shards of one map "
-                         "+ one gradient all-reduce per step")
+    ap.add_argument("--scaling", choices=("weak", "strong"), default="strong",
+                    help="N > 1: strong (default) = pixel shards of one map + one gradient all-reduce per step (SURVEY.md 8(e)); "
+                         "weak = one parameter vector (chain) per rank, no collective")
     ap.add_argument("--nside", type=int, default=0, help="override the config's nside (runtime sweeps)")
     ap.add_argument("--n-los", type=int, default=0, help="override the config's samples per sightline")
     ap.add_argument("--freq-hz", type=float, default=0.0, help="run at this single frequency instead of the config's")

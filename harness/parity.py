@@ -1,11 +1,11 @@
 """Shared helpers for the GPU parity tests: run the CUDA library and the oracle on the same seeded
-inputs (paper_2410_01136_b200.workloads) and compare per map.  Imported only by tests/ and bench.py."""
+inputs (harness.workloads) and compare per map.  Imported only by tests/, bench.py and __graft_entry__.smoke()."""
 from __future__ import annotations
 
 import numpy as np
 
 import oracle
-from paper_2410_01136_b200 import workloads as wl
+from harness import workloads as wl
 
 MAP_TOL = 1.0e-4    # max |delta| <= MAP_TOL * RMS(oracle map), per (batch, frequency, Stokes) -- BASELINE.json north_star
 GRAD_TOL = 1.0e-3   # relative error per gradient component -- BASELINE.json north_star
@@ -113,3 +113,13 @@ def assert_sampled_maps_close(gpu_sub, ref_sub, rms_mask, tol=MAP_TOL, what=""):
         assert e.max() <= tol, f"{what}: max|d|/RMS = {e.max():.3e} > {tol:g} (per map: {e.max(axis=-1)})"
         worst = max(worst, float(e.max()))
     return worst
+
+
+def assert_log_gradient_close(g, ref, theta, what="", rel=GRAD_TOL, floor=1.0e-5):
+    """Gradient check away from the configs' own parameters (random draws, reading C-2#14b): in log-parameter
+    space, |d(g_j theta_j)| <= rel |g_j theta_j| + floor max_k |g_k theta_k|.  The floor is the fp32 round-off of the
+    accumulations (~1e-6 .. 1e-5 of the largest terms): a component more than 100x below the largest one is a cancelling
+    sum whose RELATIVE error the arithmetic does not bound."""
+    lg, lref = np.asarray(g) * theta, np.asarray(ref) * theta
+    bound = rel * np.abs(lref) + floor * np.abs(lref).max(axis=-1, keepdims=True)
+    assert np.all(np.abs(lg - lref) <= bound), f"{what}: {np.abs(lg - lref) / np.abs(lref)}"

@@ -13,15 +13,20 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 
 
+def run(name: str) -> str:
+    """Compile <name>.cu for sm_100a into a temporary binary, run it on the current GPU, return its stdout."""
+    with tempfile.TemporaryDirectory() as d:
+        exe = Path(d) / name
+        subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+                        "-o", str(exe), str(HERE / f"{name}.cu")], check=True)
+        return subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+
+
 def main():
     which = sys.argv[1:] or ["pipes", "grid_streams"]
     for name in which:
-        with tempfile.TemporaryDirectory() as d:
-            exe = Path(d) / name
-            subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-                            "-o", str(exe), str(HERE / f"{name}.cu")], check=True)
-            print(f"== {name}", flush=True)
-            subprocess.run([str(exe)], check=True)
+        print(f"== {name}", flush=True)
+        print(run(name), end="", flush=True)
 
 
 if __name__ == "__main__":

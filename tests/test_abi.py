@@ -125,7 +125,7 @@ def test_invalid_arguments_return_codes():
 def test_calls_are_asynchronous_on_the_given_stream():
     import torch
     import paper_2410_01136_b200 as sx
-    from paper_2410_01136_b200 import workloads as wl
+    from harness import workloads as wl
     w = wl.config(1).scaled(nside=16, n_los=128)
     plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs)
     model = sx.Model("disc4", aux=w.aux)

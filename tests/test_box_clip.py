@@ -4,9 +4,9 @@ import numpy as np
 import pytest
 
 import oracle
-import parity
+from harness import parity
 from conftest import load_golden
-from paper_2410_01136_b200 import workloads as wl
+from harness import workloads as wl
 
 BOX = (40.0, 40.0, 10.0)          # the paper's box
 OBS = (-8.3, 0.0, 0.006)

@@ -9,8 +9,8 @@ import numpy as np
 import pytest
 
 import oracle
-import parity
-from paper_2410_01136_b200 import workloads as wl
+from harness import parity
+from harness import workloads as wl
 
 pytestmark = pytest.mark.gpu
 

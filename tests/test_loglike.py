@@ -3,8 +3,8 @@ import numpy as np
 import pytest
 
 import oracle
-import parity
-from paper_2410_01136_b200 import workloads as wl
+from harness import parity
+from harness import workloads as wl
 
 SIGMA = 1.0e-3     # K: "sigma = 1 mK" per pixel on Q and U
 
@@ -80,7 +80,10 @@ def test_gpu_loglike_vjp_matches_oracle(case):
     torch.cuda.synchronize()
     ll, g = ll.cpu().numpy(), g.cpu().numpy().astype(np.float64)
     plan.close()
-    # logL is a sum of squares of (map - obs) / sigma: the map tolerance 1e-4 RMS moves it by at most ~2 |r| 1e-4 RMS / sigma^2
+    # DESIGN.md reading C-2#23: logL = -1/2 sum w r^2 with r = map - obs; a map error |d| <= 1e-4 RMS moves it by
+    # <= 2 (1e-4 RMS / r_rms) |logL| to first order, and the cotangent -w r (hence the gradient) by the same relative
+    # amount on top of the adjoint's own 1e-3.  At this test's 2 % parameter offset r_rms ~ 0.05 RMS: 2e-3 + 1e-3 allowed,
+    # 2e-3 asserted.
     assert np.all(np.abs(ll - ll_ref) <= 2e-3 * np.abs(ll_ref))
     if w.kind == "grid_b":
         rms = np.sqrt(np.mean(g_ref[g_ref != 0] ** 2))

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_2410_01136_b200 import workloads as wl
+from harness import workloads as wl
 
 
 def loss(model_factory, p, geom, cots, pix):

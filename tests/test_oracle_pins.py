@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_2410_01136_b200 import workloads as wl
+from harness import workloads as wl
 
 C_CM = 2.99792458e10
 KPC_CM = 3.0856775814913673e21

@@ -3,8 +3,8 @@ import numpy as np
 import pytest
 
 import oracle
-import parity
-from paper_2410_01136_b200 import workloads as wl
+from harness import parity
+from harness import workloads as wl
 
 BOX = (40.0, 40.0, 10.0)
 

@@ -16,7 +16,6 @@ import torch.multiprocessing as mp
 
 ROOT = Path(__file__).resolve().parent.parent
 sys.path.insert(0, str(ROOT))
-sys.path.insert(0, str(ROOT / "tests"))
 
 from paper_2410_01136_b200 import sharding  # noqa: E402
 
@@ -50,8 +49,8 @@ def _worker(rank, world, port, out_dir):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         import oracle
-        import parity
-        from paper_2410_01136_b200 import workloads as wl
+        from harness import parity
+        from harness import workloads as wl
         oracle.set_num_threads(2)
         w = wl.config(2).scaled(nside=4, n_los=64, batch=3)           # FULL16, batch 3, 192 pixels
         begin, count = sharding.shard_of(w.npix, rank, world)
@@ -90,7 +89,7 @@ def _bench_worker(rank, world, port, out_dir):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         import bench
-        from paper_2410_01136_b200 import workloads as wl
+        from harness import workloads as wl
         w = bench.rank_workload(0, rank)
         t = torch.from_numpy(w.params.astype(np.float64).ravel().copy())
         ts = [torch.empty_like(t) for _ in range(world)]

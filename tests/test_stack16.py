@@ -3,8 +3,8 @@ import numpy as np
 import pytest
 
 import oracle
-import parity
-from paper_2410_01136_b200 import workloads as wl
+from harness import parity
+from harness import workloads as wl
 
 W = (0.6, 0.3, 0.1, 0.3)                                  # weights printed in Eq. (16)
 SRC = ((0, 1, 2), (0, 2, 1), (2, 1, 0), (1, 0, 2))        # B_x = .6 B1x + .3 B2x + .1 B3z + .3 B4y, etc.

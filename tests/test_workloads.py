@@ -1,7 +1,7 @@
 """Seeded input generators: shapes, determinism, the stated recipe.  CPU only."""
 import numpy as np
 
-from paper_2410_01136_b200 import workloads as wl
+from harness import workloads as wl
 
 
 def test_config_table_sizes():
