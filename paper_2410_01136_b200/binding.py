@@ -225,7 +225,7 @@ def forward(plan: Plan, model: Model, params, out=None):
     if out is None:
         out = tuple(torch.empty((batch, plan.n_freq, plan.npix), dtype=torch.float32, device=params.device) for _ in range(3))
     I, Q, U = out
-    n = batch * plan.n_freq * plan.npix
+    n = batch * plan.n_freq * plan.npix if batch * plan.npix < 2 ** 31 else None   # (the library rejects larger calls itself)
     _check_device(plan, params, I, Q, U)
     _check(load_library().synax_forward(plan.h, ctypes.byref(model.c), _dev_f32(params, "params"), batch,
                                         _dev_f32(I, "I", n), _dev_f32(Q, "Q", n), _dev_f32(U, "U", n), _stream()))

@@ -60,6 +60,13 @@ struct synax_plan {
   int* h_flag_count;  // pinned host mirror (last forward)
   cudaStream_t aux;   // second stream for the float64-angle member of the adjoint's per-CTA pair (fork / join by events)
   cudaEvent_t ev_fork, ev_join;
+  // What the last analytic forward left for the next adjoint (which sweeps backwards and needs every sightline's Faraday
+  // total first): the totals, the parameters they belong to (device copy, compared on the device) and a host-side stamp
+  // of everything else they depend on.
+  mutable double* phi_cache; mutable size_t phi_cap;          // [batch][npix]
+  mutable float* phi_params; mutable size_t phi_params_cap;   // [batch][n_params]
+  mutable int* d_phi_ok;
+  mutable struct PhiStamp { int valid, code, batch, n_params, precision; double escalate_rad, delta; const double* path; float aux[7]; } phi_stamp;
   mutable int64_t launches;
   mutable int64_t last_n_sl;  // sightlines of the last forward (for stats when every one took the float64 chain)
 };
@@ -164,6 +171,9 @@ extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
   if (!plan) return SYNAX_OK;
   cudaFree(plan->dirs);
   if (plan->path) cudaFree(plan->path);
+  if (plan->phi_cache) cudaFree(plan->phi_cache);
+  if (plan->phi_params) cudaFree(plan->phi_params);
+  if (plan->d_phi_ok) cudaFree(plan->d_phi_ok);
   cudaFree(plan->d_flag_count);
   cudaFree(plan->d_vjp_ctrl);
   cudaFreeHost(plan->h_flag_count);
@@ -180,6 +190,7 @@ extern "C" synax_status synax_plan_set_box(synax_plan* plan, const double box_kp
   if (!plan) return fail(SYNAX_ERR_INVALID_ARG, "plan is NULL");
   // in-flight calls on the caller's (non-blocking) streams may still read plan->path and the frequency table
   CUDA_TRY(cudaDeviceSynchronize());
+  plan->phi_stamp.valid = 0;
   if (!box_kpc) {   // back to the fixed [0, s_max]
     if (plan->path) { cudaFree(plan->path); plan->path = nullptr; }
     plan->s_max = plan->s_max_fixed; plan->delta = plan->s_max / (double)plan->n_los;
@@ -399,6 +410,37 @@ static synax_status run_prologue(const synax_plan* plan, const synax_model* mode
   return SYNAX_OK;
 }
 
+static synax_plan::PhiStamp make_phi_stamp(const synax_plan* plan, const synax_model* model, int code, int batch) {
+  synax_plan::PhiStamp st;
+  std::memset(&st, 0, sizeof(st));
+  st.valid = 1; st.code = code; st.batch = batch; st.n_params = model->n_params; st.precision = plan->precision;
+  st.escalate_rad = plan->escalate_rad; st.delta = plan->delta; st.path = plan->path;
+  for (int i = 0; i < 7; ++i) st.aux[i] = model->aux ? model->aux[i] : 0.f;
+  return st;
+}
+
+// Buffers for the Faraday totals of an analytic forward of `batch` parameter vectors (grown on demand: the first call
+// of a given size allocates, and so synchronises, once).  Gridded n_e is left out: the grid's contents can change
+// between the forward and the adjoint without the library seeing it.
+static bool phi_buffers(const synax_plan* plan, const synax_model* model, int batch) {
+  if (model->ne_grid) return false;
+  const size_t need = (size_t)plan->npix * (size_t)batch, needp = (size_t)batch * (size_t)model->n_params;
+  if (plan->phi_cap < need) {
+    if (plan->phi_cache) cudaFree(plan->phi_cache);
+    plan->phi_cache = nullptr; plan->phi_cap = 0;
+    if (cudaMalloc((void**)&plan->phi_cache, need * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return false; }
+    plan->phi_cap = need;
+  }
+  if (plan->phi_params_cap < needp) {
+    if (plan->phi_params) cudaFree(plan->phi_params);
+    plan->phi_params = nullptr; plan->phi_params_cap = 0;
+    if (cudaMalloc((void**)&plan->phi_params, needp * sizeof(float)) != cudaSuccess) { cudaGetLastError(); return false; }
+    plan->phi_params_cap = needp;
+  }
+  if (!plan->d_phi_ok && cudaMalloc((void**)&plan->d_phi_ok, sizeof(int)) != cudaSuccess) { cudaGetLastError(); return false; }
+  return true;
+}
+
 extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
                                       int32_t batch, float* I, float* Q, float* U, void* cuda_stream) {
   int code = 0;
@@ -421,6 +463,8 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   a.sg_n0 = make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l);
   a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
   a.append_count = plan->d_flag_count + kCtrlFlagCount; a.append_list = nullptr;
+  a.phi = nullptr;
+  plan->phi_stamp.valid = 0;
 
   if (code == kGridB) {
     synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, sm_count(plan->device),
@@ -471,6 +515,9 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     }
   }
   const int G = pick_lanes(plan, n_sl);
+  // one thread per sightline: the adjoint will want the Faraday totals (it has a pre-pass of its own otherwise)
+  const bool keep_phi = G == 1 && phi_buffers(plan, model, batch);
+  if (keep_phi) a.phi = plan->phi_cache;
   // Every sightline (count known on the host): one group per sightline and the hardware block scheduler balances the
   // CTAs (a persistent grid of 16 CTAs/SM left a 14 % tail at cfg 4: 2.6 sightlines per thread).  Flag list (length
   // known only on the device): persistent grid, groups stride over the list.
@@ -540,6 +587,12 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   cudaError_t e = cudaGetLastError();
   cudaMemcpyAsync(plan->h_flag_count, ctrl, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
   if (e != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward launch failed: %s", cudaGetErrorString(e));
+  if (keep_phi && cudaMemcpyAsync(plan->phi_params, params, sizeof(float) * (size_t)batch * model->n_params,
+                                  cudaMemcpyDeviceToDevice, st) == cudaSuccess)
+  {
+    const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
+    std::memcpy(&plan->phi_stamp, &now, sizeof(now));   // byte copy: the stamp is compared with memcmp
+  }
   return SYNAX_OK;
 }
 
@@ -556,6 +609,17 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   BatchConstsD* bd = nullptr;
   stt = run_prologue(plan, model, code, params, batch, scratch, &bc, &bd, st);
   if (stt != SYNAX_OK) return stt;
+  // Faraday totals of the last forward: usable when everything but the parameter values matches on the host side; the
+  // values themselves are compared on the device (no synchronisation)
+  const double* phi = nullptr;
+  if (code != kGridB && plan->phi_stamp.valid && !model->ne_grid && pick_lanes(plan, plan->npix * batch) == 1) {
+    const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
+    if (std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0) {
+      phi_validate_kernel<<<1, 256, 0, st>>>(params, plan->phi_params, (int64_t)batch * model->n_params, plan->d_phi_ok);
+      plan->launches++;
+      phi = plan->phi_cache;
+    }
+  }
   synax_status rs;
   if (code == kGridB)
     rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
@@ -565,7 +629,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
-                      plan->batch_share, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
+                      plan->batch_share, phi, plan->d_phi_ok, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
                       dI, dQ, dU, grad, st, &plan->launches);
   if (rs == SYNAX_ERR_UNSUPPORTED) return fail(rs, "GRID_B vjp: n_los too large for the shared-memory hand-over (see synax.h)");
   if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));

@@ -115,17 +115,6 @@ __device__ __forceinline__ void eval_stack16_dd(const BatchConsts64& P, const Tr
   S.ne = P.p[13] * exp(-rho / P.p[14]) * sech2_d(z / P.p[15]);
 }
 
-template <int G>
-__device__ __forceinline__ double group_sum_d(double v) {
-#pragma unroll
-  for (int d = G / 2; d >= 1; d >>= 1) {
-    int lo = __double2loint(v), hi = __double2hiint(v);
-    lo = __shfl_xor_sync(0xffffffffu, lo, d, G); hi = __shfl_xor_sync(0xffffffffu, hi, d, G);
-    v += __hiloint2double(hi, lo);
-  }
-  return v;
-}
-
 // cos, sin of the Faraday angle 2 pi k_turn S, the turn count reduced before the trigonometric call
 __device__ __forceinline__ void faraday_phasor_d(double k_turn, double S, double& c, double& s) {
   double t = k_turn * S;

@@ -45,6 +45,16 @@ __device__ __forceinline__ float group_sum(float v) {
   return v;
 }
 template <int G>
+__device__ __forceinline__ double group_sum_d(double v) {
+#pragma unroll
+  for (int d = G / 2; d >= 1; d >>= 1) {
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_xor_sync(0xffffffffu, lo, d, G); hi = __shfl_xor_sync(0xffffffffu, hi, d, G);
+    v += __hiloint2double(hi, lo);
+  }
+  return v;
+}
+template <int G>
 __device__ __forceinline__ float group_max(float v) {
 #pragma unroll
   for (int d = G / 2; d >= 1; d >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, d, G));
@@ -100,6 +110,8 @@ struct ForwardArgs {
   int* append_count;      // where forward_kernel appends the sightlines its exact criterion flags: the flag list itself
   int* append_list;       // (fast-then-list), or a separate "missed" list in split mode, where the float64 kernel reads
                           // the flag list concurrently on the plan's second stream
+  double* phi;            // [batch][npix]: every sightline's Faraday sum sum_n n_e B_LOS Delta_i / Delta, stored for the plan's
+                          // next adjoint (which sweeps backwards and needs the total first), or null
   int* list_u;            // kModeSplit: sightlines classify_kernel left to the fp32 kernel (count in ctrl[kCtrlCountU])
   const int* count_u;
 };
@@ -244,6 +256,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
 
   // combine the G lanes of the sightline
   float absS;
+  const double phi_total = G > 1 ? group_sum_d<G>(carry) : carry;
   if (G > 1) {
     const double off = group_exclusive_scan<G>(carry, g);
 #pragma unroll
@@ -266,6 +279,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       A.Q[o] = P.coefP[A.f0 + f] * T.scalef * accQ[f];
       A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
     }
+    if (A.f0 == 0 && A.phi) A.phi[sl] = phi_total;
     if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)sl;
@@ -360,6 +374,7 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
     A.I[o] = P.coefI[A.f0] * T.scalef * accI[j];
     A.Q[o] = P.coefP[A.f0] * T.scalef * accQ[j];
     A.U[o] = P.coefP[A.f0] * T.scalef * accU[j];
+    if (A.f0 == 0 && A.phi) A.phi[(int64_t)bj[j] * A.geo.npix + pix] = carry[j];
     if (A.f0 == 0 && A.flag_S > 0.0f && gabs[j] > A.flag_S) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)((int64_t)bj[j] * A.geo.npix + pix);
@@ -497,6 +512,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
         accQ[f] += tq[f]; accU[f] += tu[f];
       }
     }
+    const double phi_total = G > 1 ? group_sum_d<G>(S_loc) : S_loc;
     if (G > 1) {
       const double off = group_exclusive_scan<G>(S_loc, g);
 #pragma unroll
@@ -516,6 +532,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
         A.Q[o] = P.coefP[A.f0 + f] * T.scalef * accQ[f];
         A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
       }
+      if (A.f0 == 0 && A.phi) A.phi[sl] = phi_total;
     }
   }
 }

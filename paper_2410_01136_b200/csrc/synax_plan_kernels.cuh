@@ -85,6 +85,16 @@ __global__ void absmax_kernel(const float* __restrict__ g, int64_t n, float* __r
   if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMax(reinterpret_cast<int*>(out), __float_as_int(m));
 }
 
+// *ok = 1 when the n floats of `now` equal `saved` bit for bit (the parameters the plan's last forward ran with), else 0.
+// One block.
+__global__ void phi_validate_kernel(const float* __restrict__ now, const float* __restrict__ saved, int64_t n, int* __restrict__ ok) {
+  int same = 1;
+  for (int64_t i = threadIdx.x; i < n; i += blockDim.x)
+    if (__float_as_int(now[i]) != __float_as_int(saved[i])) same = 0;
+  same = __syncthreads_and(same);
+  if (threadIdx.x == 0) *ok = same;
+}
+
 // ne_max: device scalar max |ne_grid| when a gridded n_e replaces the analytic disc, else null
 __global__ void prologue_kernel(int code, const float* __restrict__ params, int n_params, int batch,
                                 AuxHost aux, FreqTab ft, double delta, const float* __restrict__ ne_max,

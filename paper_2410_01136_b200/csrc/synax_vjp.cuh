@@ -114,6 +114,66 @@ struct AnalyticGrad {
       ge[2] = fma_r(hh, tz, ge[2]); He[2] = fma_r(h, tz, He[2]);
     }
   }
+  // Backward sweep (vjp_kernel): the reverse Faraday scan's gbar_m = sum_{n>m} Sbar_n + Sbar_m / 2 is a running suffix
+  // sum there, so B's whole cotangent W = BbarN e_N + BbarE e_E + gbar ne n is known at the sample and every parameter
+  // needs ONE functional and one accumulator.  kLanes (G > 1): the suffix over the LATER lanes of the sightline is
+  // known only after the sweep, so the lane also sums the Faraday terms h alone (H, He) for combine_suffix().
+  template <bool kLanes, typename PT, typename TT, typename AT, typename ST>
+  __device__ __forceinline__ void add_w(const PT& P, const TT& T, const AT& a, const ST& S, R z, R BNb, R BEb, R gbar, R MKu) {
+    const R gne = gbar * S.ne;
+    const R wx = fma_r(BNb, T.eNx, fma_r(BEb, T.eEx, gne * T.nx));
+    const R wy = fma_r(BNb, T.eNy, fma_r(BEb, T.eEy, gne * T.ny));
+    const R wz = fma_r(BNb, T.eNz, gne * T.nz);
+    R wr, wp;
+    to_cyl(wx, wy, a.xr, a.yr, wr, wp);
+    const R Acc = a.A * a.cc, Asc = a.A * a.sc;
+    apply(P, a, wr, wp, wz, Acc, Asc, g);
+    if (kLanes) {
+      R nr, np;
+      to_cyl((R)T.nx, (R)T.ny, a.xr, a.yr, nr, np);
+      apply(P, a, S.ne * nr, S.ne * np, S.ne * (R)T.nz, Acc, Asc, H);
+    }
+    if (kFull) {
+      n1[0] += MKu; n1[1] = fma_r(MKu, a.rho, n1[1]); n1[2] = fma_r(MKu * a.thz, z, n1[2]);
+      const R h = T.scalef * a.neu * S.Bpar;   // d(ne Bpar Delta_i/Delta) / d ne0
+      const R tz = a.thez * z;
+      const R gh = gbar * h;
+      ge[0] += gh; ge[1] = fma_r(gh, a.rho, ge[1]); ge[2] = fma_r(gh, tz, ge[2]);
+      if (kLanes) { He[0] += h; He[1] = fma_r(h, a.rho, He[1]); He[2] = fma_r(h, tz, He[2]); }
+    }
+  }
+  // acc[j] += (dB/dtheta_j at unit amplitude) . (vr, vp, vz)
+  template <typename PT, typename AT>
+  __device__ __forceinline__ void apply(const PT& P, const AT& a, R vr, R vp, R vz, R Acc, R Asc, R (&acc)[NB]) {
+    const R al = fma_r(a.cp, vr, a.sp * vp);
+    const R d = fma_r(Acc, al, Asc * vz);                       // (B_disc / b0) . V
+    acc[0] += d;
+    const R pp = Acc * fma_r(a.cp, vp, -a.sp * vr);             // (dB/dpsi0) / b0 . V
+    acc[1] += pp;
+    acc[2] = fma_r(a.lr, pp, acc[2]);
+    acc[3] = fma_r(a.t, fma_r(Acc, vz, -Asc * al), acc[3]);     // (dB/dchi0) / b0 . V
+    if (kFull) {
+      acc[4] = fma_r(a.rho - (R)8.0, d, acc[4]);                // * b0 / h_b^2
+      const R LR = a.L * a.R;                                   // halo: B_h L R phi_hat
+      acc[5] = fma_r(LR, vp, acc[5]);
+      const R RuL2 = a.R * a.u * a.L * a.L;
+      acc[6] = fma_r(RuL2, vp, acc[6]);                         // * 2 B_h / w_h
+      acc[7] = fma_r(LR * fma_r(a.rho, P.inv_rh, (R)-1.0), vp, acc[7]);   // * B_h / r_h
+      acc[8] = fma_r(RuL2 * a.u, vp, acc[8]);                   // * 2 B_h / w_h
+    }
+  }
+  // G > 1: add (sum of Sbar over the later lanes of the sightline) x (this lane's sum of Faraday terms)
+  template <int G>
+  __device__ __forceinline__ void combine_suffix(R later) {
+    if (G > 1) {
+#pragma unroll
+      for (int j = 0; j < NB; ++j) g[j] = fma_r(later, H[j], g[j]);
+      if (kFull) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) ge[j] = fma_r(later, He[j], ge[j]);
+      }
+    }
+  }
   template <int G>
   __device__ __forceinline__ void combine(R Pl, int lane_in_group) {
 #pragma unroll
@@ -163,6 +223,24 @@ struct UniformGrad {
     const R h = T.scalef * S.Bpar;   // d(scale ne Bpar)/d ne = scale Bpar (S.ne carries scale)
     prefix_update(ge, He, Sbar, (R)0.5 * Sbar * h, h);
   }
+  template <bool kLanes, typename TT, typename ST>
+  __device__ __forceinline__ void add_w(const TT& T, const ST& S, R BNb, R BEb, R gbar, R wK) {
+    const R gne = gbar * S.ne;
+    g[0] += fma_r(BNb, T.eNx, fma_r(BEb, T.eEx, gne * T.nx));
+    g[1] += fma_r(BNb, T.eNy, fma_r(BEb, T.eEy, gne * T.ny));
+    g[2] += fma_r(BNb, T.eNz, gne * T.nz);
+    n1 += wK;
+    const R h = T.scalef * S.Bpar;
+    ge = fma_r(gbar, h, ge);
+    if (kLanes) { H[0] += S.ne * T.nx; H[1] += S.ne * T.ny; H[2] += S.ne * T.nz; He += h; }
+  }
+  template <int G>
+  __device__ __forceinline__ void combine_suffix(R later) {
+    if (G > 1) {
+      for (int j = 0; j < 3; ++j) g[j] = fma_r(later, H[j], g[j]);
+      ge = fma_r(later, He, ge);
+    }
+  }
   template <int G>
   __device__ __forceinline__ void combine(R Pl, int lane_in_group) {
     for (int j = 0; j < 3; ++j) prefix_combine<G, R>(g[j], H[j], Pl, lane_in_group);
@@ -210,6 +288,41 @@ struct StackGrad {
       prefix_update(g[4 * k + 3], H[4 * k + 3], Sbar, a.t * fma_r(Acc, u1[2], -Asc * h1), a.t * fma_r(Acc, u2[2], -Asc * h2));
     }
   }
+  template <bool kLanes, typename PT, typename TT, typename AT, typename ST>
+  __device__ __forceinline__ void add_w(const PT& P, const TT& T, const AT& a, const ST& S, R BNb, R BEb, R gbar) {
+    const R gne = gbar * S.ne;
+    const R w1[3] = {fma_r(BNb, T.eNx, fma_r(BEb, T.eEx, gne * T.nx)), fma_r(BNb, T.eNy, fma_r(BEb, T.eEy, gne * T.ny)),
+                     fma_r(BNb, T.eNz, gne * T.nz)};
+    const R v2[3] = {S.ne * T.nx, S.ne * T.ny, S.ne * T.nz};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const R A = a.mask * stack_weight<R>(k);
+      const R Acc = A * a.cc[k], Asc = A * a.sc[k];
+      apply_k(a, k, w1, Acc, Asc, g);
+      if (kLanes) apply_k(a, k, v2, Acc, Asc, H);
+    }
+  }
+  template <typename AT>
+  __device__ __forceinline__ void apply_k(const AT& a, int k, const R (&v)[3], R Acc, R Asc, R (&acc)[16]) {
+    R u[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) u[stack_src(k, c)] = v[c];
+    R ur, up;
+    to_cyl(u[0], u[1], a.xr, a.yr, ur, up);
+    const R h = fma_r(a.cp[k], ur, a.sp[k] * up);
+    acc[4 * k] += fma_r(Acc, h, Asc * u[2]);                                   // (B_k / b0_k) . V
+    const R pp = Acc * fma_r(a.cp[k], up, -a.sp[k] * ur);
+    acc[4 * k + 1] += pp;
+    acc[4 * k + 2] = fma_r(a.lr, pp, acc[4 * k + 2]);
+    acc[4 * k + 3] = fma_r(a.t, fma_r(Acc, u[2], -Asc * h), acc[4 * k + 3]);
+  }
+  template <int G>
+  __device__ __forceinline__ void combine_suffix(R later) {
+    if (G > 1) {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) g[j] = fma_r(later, H[j], g[j]);
+    }
+  }
   template <int G>
   __device__ __forceinline__ void combine(R Pl, int lane_in_group) {
 #pragma unroll
@@ -244,6 +357,8 @@ struct VjpArgs {
                     // is above the threshold -> the CTA is done by the PMODE 1 launch, 0 -> by the PMODE 0 launch; or null
   const float* dI; const float* dQ; const float* dU;   // may be null
   ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
+  const double* phi;      // [batch][npix] Faraday sum of every sightline as the plan's last forward stored it, or null
+  const int* phi_ok;      // device word: 1 = that forward ran with exactly these parameters (phi_validate_kernel)
   float* partial;   // [batch][n_blocks][16]
   int n_blocks;     // blocks per batch element (gridDim.x)
   int accumulate;   // 0: overwrite partials (first frequency block), 1: add
@@ -328,11 +443,18 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   cI *= T.scalef;   // the maps are scale * coef * sums (per-sightline segment length, synax_plan_set_box)
   cIa *= T.scalef;
 
-  // ---- pre-pass (G > 1): Faraday sum of each lane's chunk -> float64 offset of the preceding lanes
-  double off = 0.0;
-  if (G > 1) {
+  // ---- Faraday sum of this lane's chunk.  The sweep below runs BACKWARDS (far end first), where the reverse scan of the
+  // Faraday cotangent (S:App.D.2) is a running sum; the forward Faraday depth of a sample is then
+  //   phi_n = (sum over the whole sightline) - (sum over the samples after n) - g_n / 2,
+  // so the sightline total is needed first: taken from the value the last forward of this plan stored for exactly these
+  // parameters (A.phi, validated on the device: *A.phi_ok) when the thread owns the whole sightline, else from a
+  // forward-order pre-pass over the Faraday integrand alone.
+  double Sl = 0.0;
+  const bool cached = G == 1 && A.phi != nullptr && *A.phi_ok != 0;
+  if (cached) {
+    Sl = A.phi[(int64_t)b * A.geo.npix + pix];
+  } else {
     double s_d = ((double)n0 + 0.5) * delta;
-    double Sl = 0.0;
     float hi = 0.f, lo = 0.f;
     for (int n = n0; n < n1; ++n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
@@ -362,10 +484,15 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       if (((n - n0) & (kTile - 1)) == kTile - 1) { Sl += (double)hi + (double)lo; hi = 0.f; lo = 0.f; }
     }
     Sl += (double)hi + (double)lo;
-    off = group_exclusive_scan<G>(Sl, g);
+  }
+  double total = Sl, after = 0.0;   // Faraday sum of the whole sightline / of the lanes after this one
+  if (G > 1) {
+    const double before = group_exclusive_scan<G>(Sl, g);
+    total = group_sum_d<G>(Sl);
+    after = total - before - Sl;
   }
 
-  // ---- main sweep
+  // ---- main sweep, backwards
   typename GradOf<CODE>::type acc;
   acc.zero();
   float gAlpha = 0.f;          // sum_n 1/4 ln(B_perp^2) M K
@@ -373,29 +500,29 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
   float gPol = 0.f;            // sum_f (d ln c_f / d alpha + d ln Pi / d alpha) (Qbar_f Q_f + Ubar_f U_f)
   // d ln c_f / d alpha = dlnA - ln(nu_f) / 2: the frequency-dependent part comes from the constant bank (ft.ln_nu)
   const float cPol = kAlpha ? P.dlnA_dalpha + P.dpi_dalpha_over_pi : 0.f;
-  float Pl = 0.f;              // sum of Sbar over this lane's samples
-  double carry = 0.0;
-  double s_d = ((double)n0 + 0.5) * delta;
+  float suf = 0.f;             // sum of Sbar over this lane's samples after the current one
+  double carry = after;        // Faraday sum over everything after the current tile
   const int tile = warp_prec ? P.tile_d : kTile;
-  for (int ts = n0; ts < n1; ts += tile) {
-    const int te = min(ts + tile, n1);
-    // cotangents rotated by the Faraday angle of everything before this tile
+  for (int te = n1; te > n0; te -= tile) {
+    const int ts = max(te - tile, n0);
+    // cotangents rotated by the Faraday angle at the far end of this tile
     float rq[NF], ru[NF];
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
       // Qb cos(tb + tl) + Ub sin(tb + tl) = Qb' cos tl + Ub' sin tl,  Qb' = Qb cb + Ub sb, Ub' = -Qb sb + Ub cb
       float q = (valid && A.dQ) ? __ldg(A.dQ + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] * T.scalef : 0.f;
       float u = (valid && A.dU) ? __ldg(A.dU + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] * T.scalef : 0.f;
-      rotate_by_offset(-ft.k_turn[f], off + carry, q, u);
+      rotate_by_offset(-ft.k_turn[f], total - carry, q, u);
       rq[f] = q; ru[f] = u;
     }
-    float hi = 0.f, lo = 0.f;
-    double dl = 0.0;             // float64-chain sightlines: tile-local Faraday sum in float64
-    for (int n = ts; n < te; ++n) {
+    float hi = 0.f, lo = 0.f;    // tile-local Faraday sum over the samples after the current one (two-float)
+    double dl = 0.0;             // the same in float64 (float64-chain sightlines)
+    double s_d = ((double)te - 0.5) * delta;   // midpoint of sample te - 1
+    for (int n = te - 1; n >= ts; --n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
       const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
-      s_d += delta;
+      s_d -= delta;
       SampleF S;
       AnalyticAux aux;
       StackAux sa;
@@ -431,15 +558,15 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const float M = w * S.N0;
       const float d2 = be2 - bn2, p2 = 2.0f * S.BE * S.BN;
       const float a = M * d2, bq = M * p2;
-      // Faraday phase of this sample, tile-local
+      // Faraday phase of this sample relative to the far end of the tile: -(sum after it within the tile + g_n / 2)
       float ph;
       if (PMODE != 0 && prec) {
         const double gd = faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd);
-        ph = (float)fma(0.5, gd, dl);
+        ph = -(float)fma(0.5, gd, dl);
         dl += gd;
       } else {
         const float gn = S.ne * S.Bpar;
-        ph = fmaf(0.5f, gn, hi);
+        ph = -fmaf(0.5f, gn, hi);
         const float sum = hi + gn;
         lo += gn - (sum - hi);
         hi = sum;
@@ -462,23 +589,29 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
       const float MK = M * K;
       sumE = fmaf(M, Bt2, sumE);
       if (kAlpha) gAlpha = fmaf(lgB, MK, gAlpha);
-      // cotangent of the phase variable S at this sample, and the D.4 weight
+      // A10: cotangent Sbar of the Faraday sum at this sample; transposed half-cell scan gbar = sum_{later} Sbar + Sbar / 2
       const float Sbar = fmaf(a, Ys, -bq * Yc);
-      Pl += Sbar;
+      const float gbar = fmaf(0.5f, Sbar, suf);
+      suf += Sbar;
       // B_N, B_E cotangents (direct): from M, d2, p2, Bt2 and the (B_perp^2)^q factor
       float tq_ = 0.f;                                             // d/dBt2 through w (alpha != 3 only)
       if (!P.alpha_is_3 && Bt2 > 0.f) tq_ = P.q_exp * MK * mufu_rcp(Bt2);
       const float BEb = 2.0f * fmaf(M, fmaf(S.BE, cI + Xc, S.BN * Xs), S.BE * tq_);
       const float BNb = 2.0f * fmaf(M, fmaf(S.BN, cI - Xc, S.BE * Xs), S.BN * tq_);
-      if constexpr (CODE == kUniform) acc.add(T, S, BNb, BEb, Sbar, w * K);
-      else if constexpr (CODE == kStack16) acc.add(P, T, sa, S, BNb, BEb, Sbar);
-      else acc.add(P, T, aux, S, zf, BNb, BEb, Sbar, w * aux.N0u * K);
+      // A11: field partials
+      if constexpr (CODE == kUniform) acc.template add_w<(G > 1)>(T, S, BNb, BEb, gbar, w * K);
+      else if constexpr (CODE == kStack16) acc.template add_w<(G > 1)>(P, T, sa, S, BNb, BEb, gbar);
+      else acc.template add_w<(G > 1)>(P, T, aux, S, zf, BNb, BEb, gbar, w * aux.N0u * K);
     }
     carry += (PMODE != 0 && prec) ? dl : (double)hi + (double)lo;
   }
 
-  // ---- combine the lanes of the sightline (prefix of the preceding lanes' h-sums times this lane's Sbar total)
-  acc.template combine<G>(Pl, g);
+  // ---- lanes of a sightline: the Sbar totals of the LATER lanes weight this lane's Faraday terms
+  if (G > 1) {
+    const float before = (float)group_exclusive_scan<G>((double)suf, g);
+    const float all = group_sum<G>(suf);
+    acc.template combine_suffix<G>(all - before - suf);
+  }
   float out[16];
 #pragma unroll
   for (int j = 0; j < 16; ++j) out[j] = 0.f;

@@ -49,7 +49,8 @@ constexpr double kVjpEscalateFactor = 10.0 / 3.0;   // x escalate_rad (300 rad b
 
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                                  const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
-                                 const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, int* ctrl,
+                                 const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, const double* phi, const int* phi_ok,
+                          int* ctrl,
                                  cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
                                  const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
                                  int64_t* launches) {
@@ -61,6 +62,7 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
   a.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
   a.mode = nullptr; a.cta_sel = nullptr;
+  a.phi = phi; a.phi_ok = phi_ok;
   // Long calls with one thread per sightline: the work is split per CTA between the lean fp32 variant and the
   // float64-angle variant (vjp_classify_kernel) instead of deciding per sightline inside one heavier kernel
   // (cfg 4, 9 % of the sightlines above the threshold: 14.3 -> see DESIGN.md section 5).

@@ -33,7 +33,8 @@ def test_shared_geometry_is_bit_identical_and_matches_oracle(kind, batch):
                 assert np.all(np.abs(a - b) <= 3e-7 * np.abs(b).max(axis=-1, keepdims=True)), (kind, batch, nb)
         parity.assert_maps_close(maps, oracle_maps, what=f"batch_share={nb}")
         g = parity.gpu_vjp(w, cots, lanes=1, batch_share=nb)
-        assert np.all(np.abs(g - g1) <= 2e-6 * np.abs(g1).max(axis=1, keepdims=True)), (nb, np.abs(g - g1).max())
+        # (the unshared adjoint sweeps backwards, the batched one forwards with the prefix form: same sums, other order)
+        parity.assert_log_gradient_close(g, g1, w.params.astype(np.float64), what=f"batch_share={nb} vs 1")
         nz = oracle_grad != 0
         assert np.all(np.abs(g - oracle_grad)[nz] <= parity.GRAD_TOL * np.abs(oracle_grad)[nz]), nb
 
@@ -48,7 +49,7 @@ def test_cfg2_full_launch_shared_vs_unshared():
     cots = w.cotangents()
     g1, g = parity.gpu_vjp(w, cots, batch_share=1), parity.gpu_vjp(w, cots, batch_share=2)
     th = w.params.astype(np.float64)
-    parity.assert_log_gradient_close(g, g1, th, what="cfg2 shared vs unshared", rel=1e-4, floor=1e-5)
+    parity.assert_log_gradient_close(g, g1, th, what="cfg2 shared vs unshared")
 
 
 def test_batch_share_with_alpha_not_three_and_low_frequency():
