@@ -1,0 +1,75 @@
+"""The adjoint sweeps each sightline backwards and needs its Faraday total first: it takes it from what the plan's last
+forward stored (one float64 per sightline) when that forward ran with exactly the same parameters and settings, else
+from a pre-pass of its own.  Both routes must give the oracle's gradient; a stale store must never be used."""
+import numpy as np
+import pytest
+
+from harness import parity
+from harness import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def _grad(plan, model, params, cots):
+    import torch
+    import paper_2410_01136_b200 as sx
+    g = sx.vjp(plan, model, params, *cots)
+    torch.cuda.synchronize()
+    return g.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("case", ["cfg1", "cfg4_408MHz", "cfg2_batch", "stack16", "uniform"])
+def test_adjoint_after_forward_and_alone(case):
+    import torch
+    import paper_2410_01136_b200 as sx
+    if case == "cfg1":
+        w = wl.config(1).scaled(nside=16, n_los=200)
+    elif case == "cfg4_408MHz":
+        w = wl.config(4).scaled(nside=16, n_los=512)          # strong rotation: float64-angle variants
+    elif case == "cfg2_batch":
+        w = wl.config(2).scaled(nside=8, n_los=128, batch=3)
+    elif case == "stack16":
+        w = wl.stack16(nside=8, n_los=128, freqs=(1.4e9, 23e9))
+    else:
+        w = wl.uniform_toy(bvec=(2.0, -3.0, 1.5), nside=4, n_los=100, freqs=(0.408e9, 2.4e9))
+    cots_h = w.cotangents()
+    ref = parity.oracle_vjp(w, cots_h)
+    nz = ref != 0
+    plan, model, params = parity.gpu_objects(w, lanes=1, batch_share=1)   # one thread per sightline: the route with the store
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    g_alone = _grad(plan, model, params, cots)                # nothing stored yet: pre-pass
+    sx.forward(plan, model, params)
+    g_after = _grad(plan, model, params, cots)                # totals from the forward
+    for g, what in ((g_alone, "pre-pass"), (g_after, "stored totals")):
+        assert np.all(np.abs(g - ref)[nz] <= parity.GRAD_TOL * np.abs(ref)[nz]), (case, what, np.abs(g - ref)[nz] / np.abs(ref)[nz])
+    # other parameters: the store is stale and must not be used
+    p2 = (params * 1.07).contiguous()
+    w2 = wl.Workload(w.name, w.kind, w.nside, w.n_los, w.s_max, w.freqs, p2.cpu().numpy(), w.aux, cot_seed=w.cot_seed)
+    ref2 = parity.oracle_vjp(w2, cots_h)
+    g2 = _grad(plan, model, p2, cots)
+    assert np.all(np.abs(g2 - ref2)[nz] <= parity.GRAD_TOL * np.abs(ref2)[nz]), (case, "stale store", np.abs(g2 - ref2)[nz] / np.abs(ref2)[nz])
+    # ... and the original parameters again are recognised again
+    g3 = _grad(plan, model, params, cots)
+    assert np.array_equal(g3, g_after)
+    plan.close()
+
+
+def test_store_is_dropped_when_the_geometry_or_the_settings_change():
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(4).scaled(nside=8, n_los=256)
+    cots_h = w.cotangents()
+    plan, model, params = parity.gpu_objects(w, lanes=1)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    sx.forward(plan, model, params)
+    box = (40.0, 40.0, 10.0)
+    plan.set_box(box)                                         # other sample positions: the stored totals are void
+    w.clip_box = box
+    ref = parity.oracle_vjp(w, cots_h)
+    g = _grad(plan, model, params, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
+    sx.forward(plan, model, params)
+    plan.set_option("precision", 2)                           # float64 angles everywhere: totals of an fp32 forward are not enough
+    g = _grad(plan, model, params, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref))
+    plan.close()
