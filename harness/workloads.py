@@ -207,3 +207,27 @@ def uniform_toy(bvec=(6.0, 0.0, 0.0), n0=4.01e-5, ne=0.01, alpha=3.0, nside=8, n
     p = np.array([bvec[0], bvec[1], bvec[2], n0, ne, alpha])
     return Workload("uniform_toy", "uniform", nside, n_los, s_max, np.asarray(freqs, dtype=np.float64),
                     _f32(p)[None, :], None, cot_seed=999)
+
+
+# PAPER.md section 3.1 (L175-180): WMAP B with the paper's true values, WMAP N_0, n_e on a (256, 256, 64) grid (the paper's
+# is the YMW16 model, not in the container: a seeded clumpy exponential disc stands in for it), NSIDE 64, N_int 512,
+# 2.4 GHz (Fig. 3), integration from the observer to the faces of the (40, 40, 10) kpc box of section 2.4.
+SECTION31_B = np.array([1.2, 0.4712, 0.0157, 0.4363])
+SECTION31_BOX = (40.0, 40.0, 10.0)
+
+
+def paper_section31(nside=64, n_los=512, ne_shape=(256, 256, 64), freqs=(2.4e9,), seed=3101) -> Workload:
+    w = Workload("paper_section31", "disc4", nside, n_los, 30.0, np.asarray(freqs, dtype=np.float64),
+                 _f32(SECTION31_B)[None, :], _f32(AUX_NOMINAL), cot_seed=3102, clip_box=SECTION31_BOX)
+    w.ne_grid, w.ne_box = clumpy_disc_grid(ne_shape, SECTION31_BOX, 0.03, 20.0, 1.0, seed=seed), SECTION31_BOX
+    return w
+
+
+def section31_gridded_b(n_x, base: Workload) -> Workload:
+    """The same model with B given on a (n_x, n_x, n_x / 4) grid filled from the analytic spiral at the nodes (Fig. 6
+    lower panel)."""
+    shape = (n_x, n_x, n_x // 4)
+    X, Y, Z = grid_nodes(shape, SECTION31_BOX)
+    g = spiral_pattern(X, Y, Z, *base.params[0].astype(np.float64))
+    w = dataclasses.replace(base, name=f"paper_section31_gridB{n_x}", kind="grid_b", params=_f32(g), box=SECTION31_BOX)
+    return w

@@ -100,6 +100,20 @@ def test_gpu_gridded_scalars_parity(case):
 
 
 @pytest.mark.gpu
+def test_gpu_paper_section31_workload_full_size():
+    """PAPER.md section 3.1 at the paper's sizes (L180): NSIDE 64, N_int 512, n_e on a (256, 256, 64) grid (16.8 MB: another
+    cache regime than the small grids above), WMAP B with the paper's true values, box-clipped integration; forward and
+    gradient against the oracle on every pixel."""
+    w = wl.paper_section31()
+    assert w.ne_grid.shape == (256, 256, 64) and w.npix * w.n_los == 25165824
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what="section 3.1 forward")
+    cots = w.cotangents()
+    g, ref = parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("ne_amp", [0.12, 0.5])
 def test_gpu_strong_ne_grid_with_zero_aux_ne(ne_amp):
     """The aux n_e entries are ignored when a gridded n_e is given (synax.h), so the caller may leave them at zero: the
