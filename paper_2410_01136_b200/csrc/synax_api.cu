@@ -349,7 +349,7 @@ static AuxHost make_aux(const synax_model* m) {
 static Geometry make_geo(const synax_plan* plan) {
   Geometry g;
   g.npix = plan->npix; g.n_los = plan->n_los; g.delta = plan->delta;
-  for (int i = 0; i < 3; ++i) g.obs[i] = plan->obs[i];
+  for (int i = 0; i < 3; ++i) { g.obs[i] = plan->obs[i]; g.obsf[i] = (float)plan->obs[i]; }
   g.dirs = plan->dirs; g.path = plan->path;
   return g;
 }

@@ -116,6 +116,7 @@ struct Geometry {
   int n_los;
   double delta;   // s_max / n_los  (kpc)
   double obs[3];
+  float obsf[3];  // the observer rounded to fp32 (constant-bank operands of the fp32 position FMAs)
   const double* dirs;  // [npix][4] = cos l, sin l, cos b, sin b
   const double* path;  // [npix] path length of the sightline in units of s_max = n_los * delta, or null (= 1):
                        // set by synax_plan_set_box (integration from the observer to the box face)
@@ -246,12 +247,27 @@ __device__ __forceinline__ void analytic_fields_f32(const BatchConsts& P, const 
   const float Brho = Ab * a.cp * a.cc;
   float Bphi = Ab * a.sp * a.cc;
   const float Bz = Ab * a.sc;
+  // The three reciprocals of a sample -- the halo's Lorentzian 1/(1+u^2) and the two sech^2 denominators 1/(1+e)^2 --
+  // share ONE MUFU.RCP of their product (the kernels are XU-bound: a reciprocal costs 8 issue cycles of that pipe, a
+  // multiply one of the FMA pipe); every factor is >= 1, the product stays far below the fp32 range.
+  const float ez = mufu_ex2(P.k_hz * az);
+  const float dz = 1.0f + ez, dz2 = dz * dz;
+  const float ee = mufu_ex2(P.k_hez * az);
+  const float de = 1.0f + ee, de2 = de * de;
+  float iz, ie;
   if (kHalo) {  // toroidal halo, S:App.C
     a.u = (az - P.p[6]) * P.inv_wh;
     const float q = a.rho * P.inv_rh;
-    a.L = mufu_rcp(fmaf(a.u, a.u, 1.0f));
+    const float lu = fmaf(a.u, a.u, 1.0f), dd = dz2 * de2;
+    const float inv = mufu_rcp(lu * dd);
+    a.L = inv * dd;
+    const float il = inv * lu;
+    iz = il * de2; ie = il * dz2;
     a.R = q * mufu_ex2(kLog2e * (1.0f - q));
     Bphi = fmaf(P.p[5] * a.L, a.R, Bphi);
+  } else {
+    const float inv = mufu_rcp(dz2 * de2);
+    iz = inv * de2; ie = inv * dz2;
   }
   const float Bx = Brho * a.xr - Bphi * a.yr;
   const float By = fmaf(Brho, a.yr, Bphi * a.xr);
@@ -259,15 +275,9 @@ __device__ __forceinline__ void analytic_fields_f32(const BatchConsts& P, const 
   S.BN = fmaf(Bx, T.eNx, fmaf(By, T.eNy, Bz * T.eNz));          // Eq.(8) numerator
   S.BE = fmaf(Bx, T.eEx, By * T.eEy);                           // Eq.(8) denominator (S:C-2#4)
   // --- N_0 = n0 exp(-rho/h_r) sech^2(z/h_z)  Eq.(12);  sech^2 w = 4e/(1+e)^2, e = exp(-2|w|)
-  const float ez = mufu_ex2(P.k_hz * az);
-  const float dz = 1.0f + ez;
-  const float iz = mufu_rcp(dz * dz);
   a.N0u = 4.0f * mufu_ex2(P.k_hr * a.rho) * ez * iz;
   S.N0 = P.p[9] * a.N0u;
   a.thz = copysignf((1.0f - ez) * dz * iz, z);                  // tanh = (1-e)/(1+e)
-  const float ee = mufu_ex2(P.k_hez * az);
-  const float de = 1.0f + ee;
-  const float ie = mufu_rcp(de * de);
   a.neu = 4.0f * mufu_ex2(P.k_her * a.rho) * ee * ie;
   S.ne = P.p[13] * a.neu;
   a.thez = copysignf((1.0f - ee) * de * ie, z);

@@ -91,6 +91,25 @@ __device__ __forceinline__ void emission(const BatchConsts& P, float BN, float B
 // (no per-sample scan: each lane integrates with a chunk-local Faraday depth and its partial Q+iU
 // is rotated once by the float64 offset of the preceding lanes).  NF frequencies per pass.
 // ------------------------------------------------------------------------------------------------
+// Sample positions for the fp32 field chain, evaluated in fp32 on their own: s = s0 + n Delta_i from an exactly represented
+// sample counter, then one fused multiply-add per coordinate (error ~2 ulp of the coordinate, the accuracy class of the
+// rest of that chain).  The float64 positions are still formed for the decisions (annulus / box tests) and the float64
+// chain, but are no longer CONVERTED per sample: four F2F.F32.F64 were 10 % of the XU-pipe work of the fp32 kernels,
+// which are bound by that pipe (ncu: XU 86 % in the fp32 forward).
+struct PosF {
+  float s0, dlt, nf;
+  __device__ __forceinline__ void init(double delta, int n_first) {
+    s0 = (float)(((double)n_first + 0.5) * delta); dlt = (float)delta; nf = 0.f;
+  }
+  // position of the current sample, then step by `dir` samples (+1 forward sweeps, -1 backward sweeps)
+  __device__ __forceinline__ void next(const Geometry& geo, const Triad& T, float dir, float& x, float& y, float& z, float& rho2) {
+    const float sf = fmaf(nf, dlt, s0);
+    nf += dir;
+    x = fmaf(sf, T.nx, geo.obsf[0]); y = fmaf(sf, T.ny, geo.obsf[1]); z = fmaf(sf, T.nz, geo.obsf[2]);
+    rho2 = fmaf(x, x, y * y);
+  }
+};
+
 struct ForwardArgs {
   Geometry geo;
   const BatchConsts* bc;
@@ -178,6 +197,8 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
   const int n1 = min(n0 + C, A.geo.n_los);
   const double delta = A.geo.delta * T.scale;
   double s_d = ((double)n0 + 0.5) * delta;
+  PosF pf;
+  pf.init(delta, n0);
 
   float k_rad[NF];
 #pragma unroll
@@ -201,6 +222,8 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
       const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       s_d += delta;
+      float xf, yf, zf, rho2f;
+      pf.next(A.geo, T, 1.0f, xf, yf, zf, rho2f);
       SampleF S;
       if (CODE == kUniform) {
         S.Bpar = fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz));
@@ -210,12 +233,12 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       } else if (CODE == kStack16) {
         const double rho2d = fma(xd, xd, yd * yd);
         StackAux sa;
-        eval_stack16_f32<false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
+        eval_stack16_f32<false>(P, T, xf, yf, zf, rho2f, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
         const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
         AnalyticAux aux;
-        eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, (float)xd, (float)yd, (float)zd, (float)rho2d, inside, S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, false>(P, T, xf, yf, zf, rho2f, inside, S, aux);
       }
       if (CODE == kAnalyticDisc || CODE == kStack16) {
         if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
@@ -312,6 +335,8 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
   const Triad T = load_triad(A.geo, pix);
   const double delta = A.geo.delta * T.scale;
   double s_d = 0.5 * delta;
+  PosF pf;
+  pf.init(delta, 0);
   const float k_rad = ft.k_rad[0];
 
   float accI[NB], accQ[NB], accU[NB], gabs[NB];
@@ -326,13 +351,13 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
     for (int n = ts; n < te; ++n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
-      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       s_d += delta;
       const double rho2d = fma(xd, xd, yd * yd);
       const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
-      const float zf = (float)zd;
+      float xf, yf, zf, rho2f;
+      pf.next(A.geo, T, 1.0f, xf, yf, zf, rho2f);
       SharedGeomF geom;
-      analytic_shared_f32((float)xd, (float)yd, zf, (float)rho2d, geom);
+      analytic_shared_f32(xf, yf, zf, rho2f, geom);
 #pragma unroll
       for (int j = 0; j < NB; ++j) {
         const BatchConsts& P = A.bc[bj[j]];

@@ -399,7 +399,7 @@ __device__ __forceinline__ double faraday_term_d(const BatchConsts& P, const Bat
 #define SYNAX_VJP_MINB 1
 #endif
 template <int CODE, int G, int NF, int PMODE>
-__global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
+__global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MINB < 3) ? 3 : SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
   constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
   if (A.mode) {
     const int m = *A.mode;
@@ -518,18 +518,21 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
     float hi = 0.f, lo = 0.f;    // tile-local Faraday sum over the samples after the current one (two-float)
     double dl = 0.0;             // the same in float64 (float64-chain sightlines)
     double s_d = ((double)te - 0.5) * delta;   // midpoint of sample te - 1
+    PosF pf;
+    pf.init(delta, te - 1);
     for (int n = te - 1; n >= ts; --n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
       const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       s_d -= delta;
+      float xf, yf, zf, rho2f;
+      pf.next(A.geo, T, -1.0f, xf, yf, zf, rho2f);
       SampleF S;
       AnalyticAux aux;
       StackAux sa;
-      const float zf = (float)zd;
       if (CODE == kStack16) {
         const double rho2d = fma(xd, xd, yd * yd);
-        eval_stack16_f32<true>(P, T, (float)xd, (float)yd, zf, (float)rho2d, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
+        eval_stack16_f32<true>(P, T, xf, yf, zf, rho2f, (rho2d > 9.0) && (rho2d < 400.0), S, sa);
         if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
         if (A.sg_n0.g) S.N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
       } else if (CODE == kUniform) {
@@ -539,8 +542,7 @@ __global__ void __launch_bounds__(kBlock, SYNAX_VJP_MINB) vjp_kernel(const __gri
         S.N0 = P.uN0; S.ne = P.une;
       } else {
         const double rho2d = fma(xd, xd, yd * yd);
-        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, (float)xd, (float)yd, zf, (float)rho2d,
-                                                 (rho2d > 9.0) && (rho2d < 400.0), S, aux);
+        eval_analytic_f32<CODE == kAnalyticFull, true>(P, T, xf, yf, zf, rho2f, (rho2d > 9.0) && (rho2d < 400.0), S, aux);
         if (CODE == kAnalyticDisc) {
           if (A.sg_ne.g) S.ne = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
           if (A.sg_n0.g) S.N0 = scalar_grid_at<float>(A.sg_n0, xd, yd, zd);
@@ -684,6 +686,8 @@ __global__ void __launch_bounds__(kBlock) vjp_batched_kernel(const __grid_consta
     gAlpha[j] = 0.f; sumE[j] = 0.f; gPol[j] = 0.f; Pl[j] = 0.f; carry[j] = 0.0;
   }
   double s_d = 0.5 * delta;
+  PosF pf;
+  pf.init(delta, 0);
   for (int ts = 0; ts < A.geo.n_los; ts += kTile) {
     const int te = min(ts + kTile, A.geo.n_los);
     float rq[NB], ru[NB], hi[NB], lo[NB];
@@ -696,13 +700,13 @@ __global__ void __launch_bounds__(kBlock) vjp_batched_kernel(const __grid_consta
     for (int n = ts; n < te; ++n) {
       const double xd = fma(s_d, T.nxd, A.geo.obs[0]);
       const double yd = fma(s_d, T.nyd, A.geo.obs[1]);
-      const double zd = fma(s_d, T.nzd, A.geo.obs[2]);
       s_d += delta;
       const double rho2d = fma(xd, xd, yd * yd);
       const bool inside = (rho2d > 9.0) && (rho2d < 400.0);
-      const float zf = (float)zd;
+      float xf, yf, zf, rho2f;
+      pf.next(A.geo, T, 1.0f, xf, yf, zf, rho2f);
       SharedGeomF geom;
-      analytic_shared_f32((float)xd, (float)yd, zf, (float)rho2d, geom);
+      analytic_shared_f32(xf, yf, zf, rho2f, geom);
 #pragma unroll
       for (int j = 0; j < NB; ++j) {
         const BatchConsts& P = A.bc[bj[j]];

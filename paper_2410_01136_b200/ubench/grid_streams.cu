@@ -143,7 +143,7 @@ int main() {
   CK(cudaMemset(grid, 0, ngrid * 4)); CK(cudaMemset(grad, 0, ngrid * 4));
   pix2ang_kernel<<<(unsigned)((npix + 255) / 256), 256>>>(nside, 0, npix, dirs);
   Geometry geo; geo.npix = npix; geo.n_los = n_los; geo.delta = s_max / n_los;
-  geo.obs[0] = -8.3; geo.obs[1] = 0.0; geo.obs[2] = 0.006; geo.dirs = dirs; geo.path = nullptr;
+  geo.obs[0] = -8.3; geo.obs[1] = 0.0; geo.obs[2] = 0.006; geo.obsf[0] = -8.3f; geo.obsf[1] = 0.f; geo.obsf[2] = 0.006f; geo.dirs = dirs; geo.path = nullptr;
   float4* grid4; CK(cudaMalloc(&grid4, ngrid / 3 * sizeof(float4))); CK(cudaMemset(grid4, 0, ngrid / 3 * sizeof(float4)));
   GridDesc G; G.g = grid; G.g4 = grid4; G.gd4 = nullptr; G.nx = nx; G.ny = ny; G.nz = nz;
   G.sx = (nx - 1) / 40.0; G.sy = (ny - 1) / 40.0; G.sz = (nz - 1) / 8.0;
