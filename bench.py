@@ -365,7 +365,8 @@ def committed_csv(name):
     f = ROOT / "profiles" / name
     if not f.exists():
         return []
-    rows = [ln.split(",") for ln in f.read_text().splitlines() if ln.strip() and not ln.startswith("#")]
+    import csv
+    rows = list(csv.reader(ln for ln in f.read_text().splitlines() if ln.strip() and not ln.startswith("#")))
     return [dict(zip(rows[0], r)) for r in rows[1:]]
 
 
@@ -381,7 +382,8 @@ def alu_roofline(w, r, local_samples, peak, sm_max, peak_src, strong, clocks):
                 traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
         rows = committed_csv("r02_cfg4_pipes.csv")
         if rows:   # ncu --set full capture of the committed build (profiles/r02_cfg4_ncu_full.md): % of peak, sustained active
-            ncu = {row["kernel"]: {k: float(v) for k, v in row.items() if k != "kernel"} for row in rows}
+            ncu = {"source": "profiles/r02_cfg4_ncu_full.md (ncu --set full of the committed build; % of peak, sustained active)",
+                   "kernels": {row["kernel"]: {k: float(v) for k, v in row.items() if k != "kernel"} for row in rows}}
     out = {"bound": "alu",
            "kernel": ("vjp_kernel (analytic adjoint; long calls: vjp_classify_kernel + the fp32-angle / float64-angle pair of vjp_kernel "
                       "launches on two streams, timed as one call)"),
