@@ -10,13 +10,6 @@
 #include "../../include/synax.h"
 #include "synax_forward.cuh"
 
-#ifndef SYNAX_GRID_FWD_MINB
-#define SYNAX_GRID_FWD_MINB 1
-#endif
-#ifndef SYNAX_GRID_VJP_MINB
-#define SYNAX_GRID_VJP_MINB 1
-#endif
-
 namespace synax {
 
 struct GridDesc {
@@ -303,7 +296,7 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
 // strong; otherwise the fp32 sweep runs and is redone in float64 only if its exact criterion fires.
 // ------------------------------------------------------------------------------------------------
 template <int NF, bool SG>
-__global__ void __launch_bounds__(kBlock, SYNAX_GRID_FWD_MINB) grid_forward_kernel(const __grid_constant__ GridFwdArgs GA,
+__global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_constant__ GridFwdArgs GA,
                                                               const __grid_constant__ FreqTab ft) {
   const ForwardArgs& A = GA.f;
   const GridDesc& G = GA.grid;
@@ -456,7 +449,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
 }
 
 template <int NF, bool SG>
-__global__ void __launch_bounds__(kBlock, SYNAX_GRID_VJP_MINB) grid_vjp_kernel(const __grid_constant__ GridVjpArgs A,
+__global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant__ GridVjpArgs A,
                                                           const __grid_constant__ FreqTab ft) {
   extern __shared__ float smem[];
   const GridDesc& G = A.grid;
