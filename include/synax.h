@@ -125,7 +125,13 @@ synax_status synax_plan_set_option(synax_plan* plan, const char* key, double val
 synax_status synax_plan_directions(const synax_plan* plan, double* out_device, void* cuda_stream);
 
 /* Forward.  params: DEVICE fp32 [batch][n_params] (GRID_B: the grid, batch == 1).
- * I, Q, U: DEVICE fp32 [batch][n_freq][npix], overwritten, Kelvin. */
+ * I, Q, U: DEVICE fp32 [batch][n_freq][npix], overwritten, Kelvin.
+ * Side effect kept inside the plan: a call that integrates every sightline with one thread (>= 300,000 sightlines, or
+ * option "lanes" = 1; analytic models without a gridded n_e) also stores each sightline's Faraday sum (one float64, Eq.(7)
+ * P:L79 at the far end) and a device copy of `params` for the next synax_vjp of this plan.  The buffers are plan-owned and
+ * grown with cudaMalloc the first time a call of a given size comes (that call synchronises the device once).
+ * GRID_B: per-call scratch of 48 bytes per grid node (16-byte fp32 nodes + 32-byte float64 nodes) from the stream-ordered
+ * pool. */
 synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
                            int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
 
@@ -133,6 +139,10 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
  * grad: DEVICE fp32 [batch][n_params] (GRID_B: [nx][ny][nz][3]); overwritten:
  * grad[b][j] = sum_{f,p} dI dI/dtheta_j + dQ dQ/dtheta_j + dU dU/dtheta_j.
  * DISC4 / GRID_B: `aux` values are constants (not differentiated).
+ * The adjoint sweeps every sightline from its far end to the observer and needs the sightline's Faraday sum first: it takes
+ * the sums the plan's last synax_forward stored when that call had the same model, batch, options and integration extent and
+ * `params` holds bit-identical values (compared on the device, no synchronisation), and otherwise recomputes them in a
+ * pre-pass (+30 % work).  Results do not depend on the route beyond rounding.
  * Ordering: all work is ordered with `cuda_stream` (results are complete when the stream reaches the end of the
  * call).  Long calls (>= 262,144 sightlines) may run part of their kernels on a second stream owned by the plan,
  * forked from and joined back to `cuda_stream` by events inside the call (CUDA-graph capturable); a plan must
