@@ -285,6 +285,20 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     res = dict(t_fwd=float(tf.mean()), t_vjp=float(tv.mean()), t_fwd_min=float(tf.min()), t_vjp_min=float(tv.min()),
                launches=int(l1 - l0), escalated=plan.stats()["escalated"],
                timing={"forward_ms": stat(tf), "vjp_ms": stat(tv), "step_ms": stat(tf + tv)})
+    if not reduce_grad:
+        # The adjoint of a step reuses one float64 per sightline that the step's own forward stored (its Faraday total: the
+        # backward sweep needs it first).  For the record, the same adjoint WITHOUT that residual (own pre-pass), a few calls:
+        plan.set_option("use_forward_totals", 0)
+        ea = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ts = []
+        for k in range(1 + min(steps, 5)):
+            ea[0].record(stream); sx.vjp(plan, model, params, *cots, out=grad); ea[1].record(stream)
+            torch.cuda.synchronize()
+            flush_buf.add_(1.0)
+            if k:
+                ts.append(ea[0].elapsed_time(ea[1]))
+        plan.set_option("use_forward_totals", 1)
+        res["timing"]["vjp_standalone_ms"] = {"mean": float(np.mean(ts)), "median": float(np.median(ts)), "best": float(np.min(ts))}
     if graph and not reduce_grad:
         # the whole step captured once in a CUDA graph and replayed (pays off when a step is launch-bound: cfg 0, 1)
         side = torch.cuda.Stream()
@@ -488,7 +502,8 @@ def run_ours(args):
                                        else f"independent parameter vectors x{world}")},
             "forward_samples_per_s": total / t_fwd, "vjp_samples_per_s": total / t_vjp,
             "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,
-            "timing": r["timing"],          # per timed step on this rank: mean / median / best, ms
+            "timing": r["timing"],          # per timed step on this rank: mean / median / best, ms; vjp_standalone_ms = the
+                                            # adjoint without the Faraday totals its step's forward stores (own pre-pass)
             "sample_freq_per_s": total * w.n_freq / t_step,
             "e2e": {"value": total / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
                     "ms_per_step": 1e3 * t_e2e,

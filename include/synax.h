@@ -112,6 +112,8 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * -- those above 10/3 x escalate_rad take their Faraday angles from the float64 chain.
  * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0).
  * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).
+ * key "use_forward_totals": 1 (default) = synax_vjp may take the sightlines' Faraday sums from what the plan's last
+ * synax_forward stored (see synax_vjp); 0 = it always recomputes them in its own pre-pass.
  * key "batch_share": parameter vectors integrated per thread when a batch of analytic models is evaluated at one
  * frequency with one thread per sightline -- they share the sightline geometry (0 = heuristic, else 1, 2 or 4).
  * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool

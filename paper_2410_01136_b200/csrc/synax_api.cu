@@ -55,6 +55,7 @@ struct synax_plan {
   double escalate_rad;
   int lanes;          // 0 heuristic
   int batch_share;    // parameter vectors per thread in the batched kernels: 0 heuristic, else 1, 2 or 4
+  int no_forward_totals;  // 1: the adjoint never uses the Faraday totals of the last forward (always its own pre-pass)
   int* d_vjp_ctrl;    // device control block of the adjoint's pilot (kCtrlWords ints)
   int* d_flag_count;  // device control block, kCtrlWords ints: [flag count, pilot flagged, mode, -]
   int* h_flag_count;  // pinned host mirror (last forward)
@@ -228,6 +229,9 @@ extern "C" synax_status synax_plan_set_option(synax_plan* plan, const char* key,
   } else if (!std::strcmp(key, "lanes")) {
     if (value != 0 && value != 1 && value != 8 && value != 32) return fail(SYNAX_ERR_INVALID_ARG, "lanes must be 0, 1, 8 or 32");
     plan->lanes = (int)value;
+  } else if (!std::strcmp(key, "use_forward_totals")) {
+    if (value != 0 && value != 1) return fail(SYNAX_ERR_INVALID_ARG, "use_forward_totals must be 0 or 1");
+    plan->no_forward_totals = value == 0 ? 1 : 0;
   } else if (!std::strcmp(key, "batch_share")) {
     if (value != 0 && value != 1 && value != 2 && value != 4) return fail(SYNAX_ERR_INVALID_ARG, "batch_share must be 0, 1, 2 or 4");
     plan->batch_share = (int)value;
@@ -612,7 +616,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   // Faraday totals of the last forward: usable when everything but the parameter values matches on the host side; the
   // values themselves are compared on the device (no synchronisation)
   const double* phi = nullptr;
-  if (code != kGridB && plan->phi_stamp.valid && !model->ne_grid && pick_lanes(plan, plan->npix * batch) == 1) {
+  if (code != kGridB && !plan->no_forward_totals && plan->phi_stamp.valid && !model->ne_grid && pick_lanes(plan, plan->npix * batch) == 1) {
     const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
     if (std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0) {
       phi_validate_kernel<<<1, 256, 0, st>>>(params, plan->phi_params, (int64_t)batch * model->n_params, plan->d_phi_ok);
