@@ -65,9 +65,12 @@ struct synax_plan {
   // total first): the totals, the parameters they belong to (device copy, compared on the device) and a host-side stamp
   // of everything else they depend on.
   mutable double* phi_cache; mutable size_t phi_cap;          // [batch][npix]
+  mutable double* phi_base; mutable size_t phi_base_cap;      // [ceil(n_los / 32)][batch * npix]: tile bases of the float64-chain sightlines
+  mutable unsigned char* phi_has; mutable size_t phi_has_cap; // [batch * npix]
   mutable float* phi_params; mutable size_t phi_params_cap;   // [batch][n_params]
   mutable int* d_phi_ok;
   mutable struct PhiStamp { int valid, code, batch, n_params, precision; double escalate_rad, delta; const double* path; float aux[7]; } phi_stamp;
+  mutable int phi_has_bases;   // the last forward also stored tile bases
   mutable int64_t launches;
   mutable int64_t last_n_sl;  // sightlines of the last forward (for stats when every one took the float64 chain)
 };
@@ -173,6 +176,8 @@ extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
   cudaFree(plan->dirs);
   if (plan->path) cudaFree(plan->path);
   if (plan->phi_cache) cudaFree(plan->phi_cache);
+  if (plan->phi_base) cudaFree(plan->phi_base);
+  if (plan->phi_has) cudaFree(plan->phi_has);
   if (plan->phi_params) cudaFree(plan->phi_params);
   if (plan->d_phi_ok) cudaFree(plan->d_phi_ok);
   cudaFree(plan->d_flag_count);
@@ -442,6 +447,23 @@ static bool phi_buffers(const synax_plan* plan, const synax_model* model, int ba
     plan->phi_params_cap = needp;
   }
   if (!plan->d_phi_ok && cudaMalloc((void**)&plan->d_phi_ok, sizeof(int)) != cudaSuccess) { cudaGetLastError(); return false; }
+  // Tile bases (the Faraday depth before every 32nd sample of the sightlines the float64 chain integrates): 8 bytes per 32
+  // samples -- 201 MB at cfg 4.  Optional: when the memory is not there the adjoint keeps its own float64-angle variants.
+  const size_t tiles = (size_t)(plan->n_los + 31) / 32;
+  if (plan->precision != 1 && tiles > 1) {
+    if (plan->phi_base_cap < need * tiles) {
+      if (plan->phi_base) cudaFree(plan->phi_base);
+      plan->phi_base = nullptr; plan->phi_base_cap = 0;
+      if (cudaMalloc((void**)&plan->phi_base, need * tiles * sizeof(double)) == cudaSuccess) plan->phi_base_cap = need * tiles;
+      else cudaGetLastError();
+    }
+    if (plan->phi_has_cap < need) {
+      if (plan->phi_has) cudaFree(plan->phi_has);
+      plan->phi_has = nullptr; plan->phi_has_cap = 0;
+      if (cudaMalloc((void**)&plan->phi_has, need) == cudaSuccess) plan->phi_has_cap = need;
+      else cudaGetLastError();
+    }
+  }
   return true;
 }
 
@@ -467,7 +489,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   a.sg_n0 = make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l);
   a.flag_count = plan->d_flag_count; a.flag_list = nullptr; a.flag_S = 0.0f;
   a.append_count = plan->d_flag_count + kCtrlFlagCount; a.append_list = nullptr;
-  a.phi = nullptr;
+  a.phi = nullptr; a.phi_base = nullptr; a.phi_has = nullptr;
   plan->phi_stamp.valid = 0;
 
   if (code == kGridB) {
@@ -522,6 +544,9 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   // one thread per sightline: the adjoint will want the Faraday totals (it has a pre-pass of its own otherwise)
   const bool keep_phi = G == 1 && phi_buffers(plan, model, batch);
   if (keep_phi) a.phi = plan->phi_cache;
+  const bool keep_base = keep_phi && plan->precision != 1 && plan->phi_base && plan->phi_has &&
+                         plan->phi_base_cap >= (size_t)n_sl * ((size_t)(plan->n_los + 31) / 32) && plan->phi_has_cap >= (size_t)n_sl;
+  if (keep_base) { a.phi_base = plan->phi_base; a.phi_has = plan->phi_has; }
   // Every sightline (count known on the host): one group per sightline and the hardware block scheduler balances the
   // CTAs (a persistent grid of 16 CTAs/SM left a 14 % tail at cfg 4: 2.6 sightlines per thread).  Flag list (length
   // known only on the device): persistent grid, groups stride over the list.
@@ -596,6 +621,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   {
     const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
     std::memcpy(&plan->phi_stamp, &now, sizeof(now));   // byte copy: the stamp is compared with memcmp
+    plan->phi_has_bases = keep_base ? 1 : 0;
   }
   return SYNAX_OK;
 }
@@ -616,12 +642,15 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   // Faraday totals of the last forward: usable when everything but the parameter values matches on the host side; the
   // values themselves are compared on the device (no synchronisation)
   const double* phi = nullptr;
+  const double* phi_base = nullptr;
+  const unsigned char* phi_has = nullptr;
   if (code != kGridB && !plan->no_forward_totals && plan->phi_stamp.valid && !model->ne_grid && pick_lanes(plan, plan->npix * batch) == 1) {
     const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
     if (std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0) {
       phi_validate_kernel<<<1, 256, 0, st>>>(params, plan->phi_params, (int64_t)batch * model->n_params, plan->d_phi_ok);
       plan->launches++;
       phi = plan->phi_cache;
+      if (plan->phi_has_bases) { phi_base = plan->phi_base; phi_has = plan->phi_has; }
     }
   }
   synax_status rs;
@@ -633,7 +662,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
-                      plan->batch_share, phi, plan->d_phi_ok, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
+                      plan->batch_share, phi, plan->d_phi_ok, phi_base, phi_has, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
                       dI, dQ, dU, grad, st, &plan->launches);
   if (rs == SYNAX_ERR_UNSUPPORTED) return fail(rs, "GRID_B vjp: n_los too large for the shared-memory hand-over (see synax.h)");
   if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));

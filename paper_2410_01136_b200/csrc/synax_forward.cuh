@@ -131,6 +131,10 @@ struct ForwardArgs {
                           // the flag list concurrently on the plan's second stream
   double* phi;            // [batch][npix]: every sightline's Faraday sum sum_n n_e B_LOS Delta_i / Delta, stored for the plan's
                           // next adjoint (which sweeps backwards and needs the total first), or null
+  double* phi_base;       // [k][batch * npix], k = 1 .. ceil(n_los / 32) - 1: Faraday sum over the samples BEFORE sample 32 k, stored by
+                          // the float64-chain kernel for its sightlines: the adjoint then runs fp32 tile-local angles on exact
+                          // tile bases and needs no float64 chain of its own; phi_has[sl] = 1 marks those sightlines.  Or null.
+  unsigned char* phi_has;
   int* list_u;            // kModeSplit: sightlines classify_kernel left to the fp32 kernel (count in ctrl[kCtrlCountU])
   const int* count_u;
 };
@@ -303,6 +307,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
     }
     if (A.f0 == 0 && A.phi) A.phi[sl] = phi_total;
+    if (A.f0 == 0 && A.phi_has) A.phi_has[sl] = 0;
     if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)sl;
@@ -400,6 +405,7 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
     A.Q[o] = P.coefP[A.f0] * T.scalef * accQ[j];
     A.U[o] = P.coefP[A.f0] * T.scalef * accU[j];
     if (A.f0 == 0 && A.phi) A.phi[(int64_t)bj[j] * A.geo.npix + pix] = carry[j];
+    if (A.f0 == 0 && A.phi_has) A.phi_has[(int64_t)bj[j] * A.geo.npix + pix] = 0;
     if (A.f0 == 0 && A.flag_S > 0.0f && gabs[j] > A.flag_S) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)((int64_t)bj[j] * A.geo.npix + pix);
@@ -514,6 +520,9 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
         for (int j = 0; j < kUnrollD; ++j) {
           double gn = ne[j] * fma(Bx[j], T.nxd, fma(By[j], T.nyd, Bz[j] * T.nzd));   // n_e B.n, signed (S:C-2#3)
           if (!live[j]) gn = 0.0;
+          // tile bases for the adjoint: the lane-local sum before every 32nd sample (lanes add their offset below)
+          if (A.phi_base && A.f0 == 0 && live[j] && valid && ((n + j) & 31) == 0 && n + j > 0)
+            A.phi_base[(size_t)((n + j) >> 5) * (size_t)n_sl + sl] = S_loc;
           const float ph = (float)fma(0.5, gn, S_loc - S_tile);                  // half-cell (S:C-2#5), tile-local
           S_loc += gn;
           const float bx = (float)Bx[j], by = (float)By[j], bz = (float)Bz[j];
@@ -540,6 +549,9 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
     const double phi_total = G > 1 ? group_sum_d<G>(S_loc) : S_loc;
     if (G > 1) {
       const double off = group_exclusive_scan<G>(S_loc, g);
+      if (A.phi_base && A.f0 == 0 && valid && g > 0)   // this lane's tile bases were stored relative to its chunk start
+        for (int k = (n0 + 31) >> 5; (k << 5) < n1; ++k)
+          if (k > 0) A.phi_base[(size_t)k * (size_t)n_sl + sl] += off;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         rotate_by_offset(ft.k_turn[f], off, accQ[f], accU[f]);
@@ -558,6 +570,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
         A.U[o] = P.coefP[A.f0 + f] * T.scalef * accU[f];
       }
       if (A.f0 == 0 && A.phi) A.phi[sl] = phi_total;
+      if (A.f0 == 0 && A.phi_has) A.phi_has[sl] = 1;
     }
   }
 }

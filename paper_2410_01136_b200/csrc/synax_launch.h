@@ -35,7 +35,7 @@ template <int CODE> void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, 
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                           const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
                           const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, const double* phi, const int* phi_ok,
-                          int* ctrl,
+                          const double* phi_base, const unsigned char* phi_has, int* ctrl,
                           cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
                           const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
                           int64_t* launches);

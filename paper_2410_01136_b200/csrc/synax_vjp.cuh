@@ -343,6 +343,8 @@ template <int CODE, typename R = float> struct GradOf { using type = AnalyticGra
 template <typename R> struct GradOf<kUniform, R> { using type = UniformGrad<R>; };
 template <typename R> struct GradOf<kStack16, R> { using type = StackGrad<R>; };
 
+constexpr int kMinTileForBases = 4;   // vjp_kernel: BatchConsts::tile_d from which the forward's tile bases are used
+
 struct VjpArgs {
   Geometry geo;
   const BatchConsts* bc;
@@ -359,6 +361,9 @@ struct VjpArgs {
   ScalarGridDesc sg_ne, sg_n0;   // gridded n_e / N_0 (DISC4), g == nullptr: unused
   const double* phi;      // [batch][npix] Faraday sum of every sightline as the plan's last forward stored it, or null
   const int* phi_ok;      // device word: 1 = that forward ran with exactly these parameters (phi_validate_kernel)
+  const double* phi_base; // [k][batch * npix]: Faraday sum before sample 32 k of the sightlines the forward's float64 chain did
+  const unsigned char* phi_has;   // [batch * npix]: 1 = phi_base holds this sightline (ForwardArgs::phi_base), or null
+  int only_with_bases;    // this launch runs only in the "bases" case (precision 2: the lean variant beside the float64 one)
   float* partial;   // [batch][n_blocks][16]
   int n_blocks;     // blocks per batch element (gridDim.x)
   int accumulate;   // 0: overwrite partials (first frequency block), 1: add
@@ -401,7 +406,17 @@ __device__ __forceinline__ double faraday_term_d(const BatchConsts& P, const Bat
 template <int CODE, int G, int NF, int PMODE>
 __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MINB < 3) ? 3 : SYNAX_VJP_MINB) vjp_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {
   constexpr bool kAlpha = (CODE == kAnalyticFull || CODE == kUniform);  // alpha is a parameter
-  if (A.mode) {
+  // The forward of this plan left, for these very parameters, the Faraday depth at every 32nd sample of each sightline
+  // its float64 chain integrated: fp32 tile-local angles on those exact tile bases are as good as float64 angles, so the
+  // lean variant does EVERY sightline and the float64-angle variants (and their classification) stand aside.
+  // (Not for under-resolved runs: the bases are 32 samples apart, and the fp32 angle inside a tile must stay below ~800 rad
+  // -- tile_d >= 4 means at most 24 rad per step -- for its 6e-8 relative round-off to stay inside the gradient bound.)
+  const bool bases = G == 1 && A.phi_base != nullptr && A.phi != nullptr && *A.phi_ok != 0 && A.bc[A.b0 + blockIdx.y].tile_d >= kMinTileForBases;
+  if (bases) {
+    if (PMODE != 0 || A.cta_sel) return;
+  } else if (A.only_with_bases) {
+    return;
+  } else if (A.mode) {
     const int m = *A.mode;
     if (A.cta_sel ? (m != kModeSplit) : (m == kModeSplit || (m == kModeAllF64) != (PMODE == 2))) return;
   }
@@ -503,8 +518,12 @@ __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MIN
   float suf = 0.f;             // sum of Sbar over this lane's samples after the current one
   double carry = after;        // Faraday sum over everything after the current tile
   const int tile = warp_prec ? P.tile_d : kTile;
-  for (int te = n1; te > n0; te -= tile) {
-    const int ts = max(te - tile, n0);
+  const int64_t slb = (int64_t)b * A.geo.npix + pix;
+  const bool has_base = PMODE == 0 && bases && A.phi_has[slb] != 0;
+  for (int te = n1; te > n0;) {
+    const int ts = max(((te - 1) / tile) * tile, n0);   // tiles are aligned to multiples of the tile length from sample 0
+    // Faraday depth at the far end of this tile: the forward's float64 value where it stored one, else total - (sum after)
+    const double phi_te = (has_base && te < A.geo.n_los) ? A.phi_base[(size_t)(te >> 5) * ((size_t)A.geo.npix * A.batch) + slb] : total - carry;
     // cotangents rotated by the Faraday angle at the far end of this tile
     float rq[NF], ru[NF];
 #pragma unroll
@@ -512,7 +531,7 @@ __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MIN
       // Qb cos(tb + tl) + Ub sin(tb + tl) = Qb' cos tl + Ub' sin tl,  Qb' = Qb cb + Ub sb, Ub' = -Qb sb + Ub cb
       float q = (valid && A.dQ) ? __ldg(A.dQ + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] * T.scalef : 0.f;
       float u = (valid && A.dU) ? __ldg(A.dU + o0 + f * A.geo.npix) * P.coefP[A.f0 + f] * T.scalef : 0.f;
-      rotate_by_offset(-ft.k_turn[f], total - carry, q, u);
+      rotate_by_offset(-ft.k_turn[f], phi_te, q, u);
       rq[f] = q; ru[f] = u;
     }
     float hi = 0.f, lo = 0.f;    // tile-local Faraday sum over the samples after the current one (two-float)
@@ -606,6 +625,7 @@ __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MIN
       else acc.template add_w<(G > 1)>(P, T, aux, S, zf, BNb, BEb, gbar, w * aux.N0u * K);
     }
     carry += (PMODE != 0 && prec) ? dl : (double)hi + (double)lo;
+    te = ts;
   }
 
   // ---- lanes of a sightline: the Sbar totals of the LATER lanes weight this lane's Faraday terms
@@ -790,6 +810,7 @@ template <int CODE, int G>
 __global__ void __launch_bounds__(kBlock) vjp_classify_kernel(const __grid_constant__ VjpArgs A,
                                                               unsigned char* __restrict__ cta_sel) {
   if (*A.mode != kModeSplit) return;
+  if (G == 1 && A.phi_base != nullptr && A.phi != nullptr && *A.phi_ok != 0 && A.bc[A.b0 + blockIdx.y].tile_d >= kMinTileForBases) return;   // vjp_kernel: "bases"
   const int b = A.b0 + blockIdx.y;
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);

@@ -50,7 +50,7 @@ constexpr double kVjpEscalateFactor = 10.0 / 3.0;   // x escalate_rad (300 rad b
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                                  const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
                                  const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, const double* phi, const int* phi_ok,
-                          int* ctrl,
+                          const double* phi_base, const unsigned char* phi_has, int* ctrl,
                                  cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
                                  const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
                                  int64_t* launches) {
@@ -62,7 +62,7 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
   a.flag_S = (float)(kVjpEscalateFactor * escalate_rad / (double)k_max);
   a.mode = nullptr; a.cta_sel = nullptr;
-  a.phi = phi; a.phi_ok = phi_ok;
+  a.phi = phi; a.phi_ok = phi_ok; a.phi_base = phi_base; a.phi_has = phi_has; a.only_with_bases = 0;
   // Long calls with one thread per sightline: the work is split per CTA between the lean fp32 variant and the
   // float64-angle variant (vjp_classify_kernel) instead of deciding per sightline inside one heavier kernel
   // (cfg 4, 9 % of the sightlines above the threshold: 14.3 -> see DESIGN.md section 5).
@@ -113,7 +113,15 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
       const int nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
       a.f0 = f0; a.accumulate = f0 > 0;
       if (precision == 1) launch_lean(code, nb, G, nf, grid, st, a, ft);
-      else if (precision == 2) launch_pmode(code, 1, G, nf, grid, st, a, ft);
+      else if (precision == 2) {
+        launch_pmode(code, 1, G, nf, grid, st, a, ft);
+        if (phi_base) {   // ... or, when the forward left tile bases for every sightline, the lean variant on those (the float64
+          VjpArgs ab = a;  // variant stands aside then)
+          ab.only_with_bases = 1;
+          launch_pmode(code, 0, G, nf, grid, st, ab, ft);
+          ++*launches;
+        }
+      }
       else {
         launch_lean(code, nb, G, nf, grid, st, a, ft);
         if (split) {

@@ -73,3 +73,52 @@ def test_store_is_dropped_when_the_geometry_or_the_settings_change():
     g = _grad(plan, model, params, cots)
     assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref))
     plan.close()
+
+
+@pytest.mark.parametrize("n_los,precision", [(500, 0), (97, 0), (512, 2), (33, 2)])
+def test_tile_bases_from_the_forward(n_los, precision):
+    """Strong rotation (408 MHz), one thread per sightline: the float64-chain forward stores the Faraday depth before every
+    32nd sample and the adjoint runs fp32 tile-local angles on those bases instead of a float64 chain of its own --
+    sample counts that are not multiples of 32, the flagged-list route (8 lanes per sightline add their lane offsets) and
+    float64 everywhere (precision 2)."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(4).scaled(nside=16, n_los=n_los)
+    w.params = w.params.copy()
+    w.params[0, 13] *= 2.0                                     # n_e doubled: fp32 angles alone miss the bound (2.4e-3)
+    cots_h = w.cotangents()
+    ref = parity.oracle_vjp(w, cots_h)
+    plan, model, params = parity.gpu_objects(w, lanes=1, precision=precision)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    sx.forward(plan, model, params)
+    g = _grad(plan, model, params, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
+    plan.set_option("use_forward_totals", 0)                  # the same without them: pre-pass + float64-angle variants
+    g0 = _grad(plan, model, params, cots)
+    assert np.all(np.abs(g0 - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g0 - ref) / np.abs(ref)
+    plan.close()
+
+
+def test_long_call_forward_then_adjoint_sparse_cotangent():
+    """786,432 sightlines (forward in split mode: the two chains side by side, the missed list afterwards), then the adjoint
+    on the stored totals and tile bases; cotangent on every 96th pixel, oracle over those."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w4 = wl.config(4)
+    w = wl.Workload("cfg4_long", w4.kind, 256, 100, w4.s_max, np.array([0.408e9, 1.4e9, 23e9]), w4.params, w4.aux, cot_seed=2204)
+    pix = np.arange(7, w.npix, 96)
+    full = w.cotangents()
+    cots_h = tuple(np.zeros_like(c) for c in full)
+    for c, f in zip(cots_h, full):
+        c[..., pix] = f[..., pix]
+    ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots_h), pix=pix)
+    plan, model, params = parity.gpu_objects(w)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    sx.forward(plan, model, params)
+    torch.cuda.synchronize()
+    stats = plan.stats()
+    assert 0.02 * w.npix < stats["escalated"] < 0.9 * w.npix, stats     # split mode
+    g = _grad(plan, model, params, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
+    assert np.array_equal(g, _grad(plan, model, params, cots))          # bit-reproducible
+    plan.close()
