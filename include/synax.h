@@ -130,8 +130,10 @@ synax_status synax_plan_directions(const synax_plan* plan, double* out_device, v
  * I, Q, U: DEVICE fp32 [batch][n_freq][npix], overwritten, Kelvin.
  * Side effect kept inside the plan: a call that integrates every sightline with one thread (>= 300,000 sightlines, or
  * option "lanes" = 1; analytic models without a gridded n_e) also stores each sightline's Faraday sum (one float64, Eq.(7)
- * P:L79 at the far end) and a device copy of `params` for the next synax_vjp of this plan.  The buffers are plan-owned and
- * grown with cudaMalloc the first time a call of a given size comes (that call synchronises the device once).
+ * P:L79 at the far end), for the sightlines its float64 chain integrates the Faraday depth before every 32nd sample (8 bytes
+ * per 32 samples and sightline: 201 MB at nside 256 x 1024 samples) and a device copy of `params`, for the next synax_vjp of
+ * this plan.  The buffers are plan-owned and grown with cudaMalloc the first time a call of a given size comes (that call
+ * synchronises the device once; never inside a stream capture; if the memory is not there the call goes on without them).
  * GRID_B: per-call scratch of 48 bytes per grid node (16-byte fp32 nodes + 32-byte float64 nodes) from the stream-ordered
  * pool. */
 synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
@@ -144,7 +146,8 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
  * The adjoint sweeps every sightline from its far end to the observer and needs the sightline's Faraday sum first: it takes
  * the sums the plan's last synax_forward stored when that call had the same model, batch, options and integration extent and
  * `params` holds bit-identical values (compared on the device, no synchronisation), and otherwise recomputes them in a
- * pre-pass (+30 % work).  Results do not depend on the route beyond rounding.
+ * pre-pass (+30-50 % work).  With the forward's tile-wise Faraday depths it also needs no float64 Faraday chain of its own.
+ * Results do not depend on the route beyond rounding (both are held to the same bound against the oracle).
  * Ordering: all work is ordered with `cuda_stream` (results are complete when the stream reaches the end of the
  * call).  Long calls (>= 262,144 sightlines) may run part of their kernels on a second stream owned by the plan,
  * forked from and joined back to `cuda_stream` by events inside the call (CUDA-graph capturable); a plan must

@@ -431,9 +431,14 @@ static synax_plan::PhiStamp make_phi_stamp(const synax_plan* plan, const synax_m
 // Buffers for the Faraday totals of an analytic forward of `batch` parameter vectors (grown on demand: the first call
 // of a given size allocates, and so synchronises, once).  Gridded n_e is left out: the grid's contents can change
 // between the forward and the adjoint without the library seeing it.
-static bool phi_buffers(const synax_plan* plan, const synax_model* model, int batch) {
+static bool phi_buffers(const synax_plan* plan, const synax_model* model, int batch, cudaStream_t st) {
   if (model->ne_grid) return false;
   const size_t need = (size_t)plan->npix * (size_t)batch, needp = (size_t)batch * (size_t)model->n_params;
+  // growing a buffer is a cudaMalloc: not inside a stream capture (a captured forward keeps whatever earlier calls allocated)
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); return false; }
+  if (cap != cudaStreamCaptureStatusNone)
+    return plan->phi_cap >= need && plan->phi_params_cap >= needp && plan->d_phi_ok != nullptr;
   if (plan->phi_cap < need) {
     if (plan->phi_cache) cudaFree(plan->phi_cache);
     plan->phi_cache = nullptr; plan->phi_cap = 0;
@@ -542,7 +547,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   }
   const int G = pick_lanes(plan, n_sl);
   // one thread per sightline: the adjoint will want the Faraday totals (it has a pre-pass of its own otherwise)
-  const bool keep_phi = G == 1 && phi_buffers(plan, model, batch);
+  const bool keep_phi = G == 1 && phi_buffers(plan, model, batch, st);
   if (keep_phi) a.phi = plan->phi_cache;
   const bool keep_base = keep_phi && plan->precision != 1 && plan->phi_base && plan->phi_has &&
                          plan->phi_base_cap >= (size_t)n_sl * ((size_t)(plan->n_los + 31) / 32) && plan->phi_has_cap >= (size_t)n_sl;

@@ -122,3 +122,40 @@ def test_long_call_forward_then_adjoint_sparse_cotangent():
     assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
     assert np.array_equal(g, _grad(plan, model, params, cots))          # bit-reproducible
     plan.close()
+
+
+@pytest.mark.parametrize("warm", [True, False])
+def test_stored_totals_inside_a_cuda_graph(warm):
+    """forward + adjoint captured in one CUDA graph with one thread per sightline: the store, the device-side comparison of
+    the parameters and the consumer all replay; new parameter values in the same buffers are picked up.  warm = False: the
+    capture is the plan's first call, the store's buffers cannot be allocated inside it, and the adjoint must fall back."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(4).scaled(nside=8, n_los=256)
+    cots_h = w.cotangents()
+    plan, model, params = parity.gpu_objects(w, lanes=1)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    out = tuple(torch.empty((1, w.n_freq, plan.npix), device="cuda") for _ in range(3))
+    g = torch.empty_like(params)
+    s = torch.cuda.Stream()
+    if warm:
+        with torch.cuda.stream(s):
+            sx.forward(plan, model, params, out=out)
+            sx.vjp(plan, model, params, *cots, out=g)
+        s.synchronize()
+    else:
+        torch.zeros(1, device="cuda").add_(1)
+        torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=s):
+        sx.forward(plan, model, params, out=out)
+        sx.vjp(plan, model, params, *cots, out=g)
+    for scale in (1.0, 1.05):
+        params.mul_(scale)
+        graph.replay()
+        torch.cuda.synchronize()
+        w2 = wl.Workload(w.name, w.kind, w.nside, w.n_los, w.s_max, w.freqs, params.cpu().numpy(), w.aux, cot_seed=w.cot_seed)
+        ref = parity.oracle_vjp(w2, cots_h)
+        got = g.cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(got - ref) <= parity.GRAD_TOL * np.abs(ref)), (warm, scale, np.abs(got - ref) / np.abs(ref))
+    plan.close()
