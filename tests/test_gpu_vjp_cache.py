@@ -159,3 +159,23 @@ def test_stored_totals_inside_a_cuda_graph(warm):
         got = g.cpu().numpy().astype(np.float64)
         assert np.all(np.abs(got - ref) <= parity.GRAD_TOL * np.abs(ref)), (warm, scale, np.abs(got - ref) / np.abs(ref))
     plan.close()
+
+
+def test_tile_bases_with_batch_and_frequency_blocks():
+    """Three parameter vectors (different rotation strengths) x 13 frequencies (passes of 8 + 4 + 1) at one thread per
+    sightline: the stored totals / tile bases are indexed by (vector, pixel) and shared by all frequency passes."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w4 = wl.config(4)
+    params = np.repeat(w4.params, 3, axis=0).copy()
+    params[1, 13] *= 2.0; params[2, 13] *= 0.1; params[2, 0] *= 1.3
+    w = wl.Workload("cfg4_b3_f13", w4.kind, 8, 320, w4.s_max, np.geomspace(0.408e9, 30e9, 13), params, w4.aux, cot_seed=2304)
+    cots_h = w.cotangents()
+    ref = parity.oracle_vjp(w, cots_h)
+    plan, model, dparams = parity.gpu_objects(w, lanes=1)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    maps = tuple(t.cpu().numpy().astype(np.float64) for t in sx.forward(plan, model, dparams))
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what="batch 3 x 13 frequencies forward")
+    g = _grad(plan, model, dparams, cots)
+    assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
+    plan.close()
