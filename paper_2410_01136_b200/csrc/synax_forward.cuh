@@ -468,6 +468,10 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
     for (int ts = n0; ts < n1; ts += tile) {
       const int te = min(ts + tile, n1);
       const double S_tile = S_loc;
+      // tile bases for the adjoint: the Faraday sum before every 32nd sample.  One thread per sightline: tiles (a power of
+      // two long, from sample 0) start on those samples.  Several lanes: see the sample loop.
+      if (G == 1 && A.phi_base && A.f0 == 0 && valid && (ts & 31) == 0 && ts > 0)
+        A.phi_base[(size_t)(ts >> 5) * (size_t)n_sl + sl] = S_loc;
       float tq[NF], tu[NF];
 #pragma unroll
       for (int f = 0; f < NF; ++f) { tq[f] = 0.0f; tu[f] = 0.0f; }
@@ -520,8 +524,9 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
         for (int j = 0; j < kUnrollD; ++j) {
           double gn = ne[j] * fma(Bx[j], T.nxd, fma(By[j], T.nyd, Bz[j] * T.nzd));   // n_e B.n, signed (S:C-2#3)
           if (!live[j]) gn = 0.0;
-          // tile bases for the adjoint: the lane-local sum before every 32nd sample (lanes add their offset below)
-          if (A.phi_base && A.f0 == 0 && live[j] && valid && ((n + j) & 31) == 0 && n + j > 0)
+          // several lanes per sightline (chunks start anywhere): the lane-local sum before every 32nd sample, per sample;
+          // the lanes add their offset below
+          if (G > 1 && A.phi_base && A.f0 == 0 && live[j] && valid && ((n + j) & 31) == 0 && n + j > 0)
             A.phi_base[(size_t)((n + j) >> 5) * (size_t)n_sl + sl] = S_loc;
           const float ph = (float)fma(0.5, gn, S_loc - S_tile);                  // half-cell (S:C-2#5), tile-local
           S_loc += gn;

@@ -177,7 +177,9 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     int t = kTileDMax;
     if (per_step * t > (double)kTilePhase) t = (int)((double)kTilePhase / per_step);
     if (t > kUnrollD) t -= t % kUnrollD;
-    c.tile_d = t < 1 ? 1 : t;
+    t = t < 1 ? 1 : t;
+    while (t & (t - 1)) t &= t - 1;   // a power of two: tiles from sample 0 then start on every multiple of 32, where the
+    c.tile_d = t;                     // float64-chain forward stores its Faraday depth for the adjoint (ForwardArgs::phi_base)
   }
   out[b] = c;
   if (outd) {
