@@ -1,6 +1,8 @@
 // synax_vjp.cuh -- adjoint (VJP) kernels for the analytic models: A9 cotangent fan-out, A10 reverse
-// half-cell scan (single forward-order sweep using sum_{n>m} = T - P_m),
-// A11 field partials and reductions.  Nothing of the forward is stored: everything is recomputed.
+// half-cell scan (vjp_kernel sweeps each sightline BACKWARDS, where that scan is a running sum; the batched and the
+// float64 kernels sweep forwards with a running prefix per parameter), A11 field partials and
+// reductions.  Nothing per SAMPLE is stored: the fields are recomputed; per SIGHTLINE the adjoint uses, when valid, the
+// Faraday total (and tile bases) the plan's last forward left (VjpArgs::phi, phi_base).
 #pragma once
 #include <algorithm>
 #include <type_traits>
