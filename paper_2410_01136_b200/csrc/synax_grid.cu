@@ -11,30 +11,25 @@ namespace synax {
 // ------------------------------------------------------------------------------------------------
 static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
   GridDesc g;
-  g.g = grid; g.g4 = nullptr; g.gd4 = nullptr; g.nx = m->nx; g.ny = m->ny; g.nz = m->nz;
+  g.g = grid; g.g4 = nullptr; g.nx = m->nx; g.ny = m->ny; g.nz = m->nz;
   g.sx = (double)(m->nx - 1) / (double)m->lx; g.sy = (double)(m->ny - 1) / (double)m->ly; g.sz = (double)(m->nz - 1) / (double)m->lz;
   g.bx = 0.5 * (double)(m->nx - 1); g.by = 0.5 * (double)(m->ny - 1); g.bz = 0.5 * (double)(m->nz - 1);
+  g.hx = 0.5 * (double)m->lx; g.hy = 0.5 * (double)m->ly; g.hz = 0.5 * (double)m->lz;
   return g;
 }
 
-// Repacked per-call copies of the grid (GridDesc::g4 / gd4) from the stream-ordered pool; 0 on success.
-static synax_status pack_grid(GridDesc& g, bool want_f64, cudaStream_t st, int64_t* launches) {
+// Repacked per-call copy of the grid (GridDesc::g4) from the stream-ordered pool; 0 on success.
+static synax_status pack_grid(GridDesc& g, cudaStream_t st, int64_t* launches) {
   const int64_t n_nodes = (int64_t)g.nx * g.ny * g.nz;
   float4* g4 = nullptr;
-  double4* gd4 = nullptr;
   if (cudaMallocAsync((void**)&g4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
-  if (want_f64 && cudaMallocAsync((void**)&gd4, sizeof(double4) * (size_t)n_nodes, st) != cudaSuccess) {
-    cudaFreeAsync(g4, st);
-    return SYNAX_ERR_ALLOC;
-  }
-  grid_pack_kernel<<<(unsigned)((n_nodes + 255) / 256), 256, 0, st>>>(g.g, n_nodes, g4, gd4);
+  grid_pack_kernel<<<(unsigned)((n_nodes + 255) / 256), 256, 0, st>>>(g.g, n_nodes, g4);
   ++*launches;
-  g.g4 = g4; g.gd4 = gd4;
+  g.g4 = g4;
   return SYNAX_OK;
 }
 static void unpack_grid(const GridDesc& g, cudaStream_t st) {
   if (g.g4) cudaFreeAsync((void*)g.g4, st);
-  if (g.gd4) cudaFreeAsync((void*)g.gd4, st);
 }
 
 static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft0) {
@@ -65,7 +60,7 @@ synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_
   ga.f.flag_list = nullptr; ga.f.flag_count = d_flag_count;
   ga.f.flag_S = (float)(escalate_rad / (double)k_max);
   cudaMemsetAsync(d_flag_count, 0, kCtrlWords * sizeof(int), st);
-  const synax_status ps = pack_grid(ga.grid, precision != 1, st, launches);
+  const synax_status ps = pack_grid(ga.grid, st, launches);
   if (ps != SYNAX_OK) return ps;
   // one warp per sightline; the hardware block scheduler balances the CTAs (a persistent grid of 16 CTAs/SM ran 2.3
   // waves of the 7 CTAs/SM that fit, with a thin last wave)
@@ -103,7 +98,7 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
     cudaFreeAsync(a.grad4, st);
     return SYNAX_ERR_CUDA;
   }
-  const synax_status ps = pack_grid(a.grid, precision != 1, st, launches);
+  const synax_status ps = pack_grid(a.grid, st, launches);
   if (ps != SYNAX_OK) {
     cudaFreeAsync(a.grad4, st);
     return ps;

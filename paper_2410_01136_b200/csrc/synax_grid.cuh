@@ -14,14 +14,15 @@ namespace synax {
 
 struct GridDesc {
   const float* g;       // caller's grid [nx][ny][nz][3]
-  // Per-call repacked copies (grid_pack_kernel; L2-resident like the grid itself).  The kernels are bound by L1 gather
-  // throughput (ncu: l1tex 73 %, long-scoreboard stalls), so a node is padded to one 16-byte vector: a corner costs one
-  // LDG.128 instead of three LDG.32, and the float64 chain gathers float64 nodes (two LDG.128) with no conversion.
+  // Per-call repacked copy (grid_pack_kernel; L2-resident like the grid itself).  The kernels are bound by L1 gather
+  // wavefronts (ncu: l1tex data pipe 70 %, long-scoreboard stalls), so a node is padded to one 16-byte vector: a corner
+  // costs one LDG.128 instead of three LDG.32.  The float64 chain converts the 24 values of a sample in registers -- a
+  // float64 copy of the nodes (two LDG.128 per corner) was slower: 0.256 vs 0.241 ms for cfg 3's forward.
   const float4* g4;     // [node] = (Bx, By, Bz, 0)
-  const double4* gd4;   // the same in float64, or null (precision 1)
   int nx, ny, nz;
   double sx, sy, sz;    // (n-1)/l
   double bx, by, bz;    // (n-1)/2
+  double hx, hy, hz;    // l/2
 };
 
 struct Cell {
@@ -86,16 +87,6 @@ __device__ __forceinline__ float warp_inclusive_scan(float v, int lane) {
   }
   return v;
 }
-__device__ __forceinline__ double warp_sum_d(double v) {
-#pragma unroll
-  for (int d = 16; d >= 1; d >>= 1) {
-    int lo = __double2loint(v), hi = __double2hiint(v);
-    lo = __shfl_xor_sync(0xffffffffu, lo, d); hi = __shfl_xor_sync(0xffffffffu, hi, d);
-    v += __hiloint2double(hi, lo);
-  }
-  return v;
-}
-
 // sin/cos of the Faraday angle k_turn * S for a float64 S (turn reduction in float64)
 __device__ __forceinline__ void faraday_sincos(double k_turn, double S, float& c, float& s) {
   double t = k_turn * S;
@@ -130,9 +121,8 @@ __device__ __forceinline__ void fields_f64(const GridDesc& G, const BatchConsts&
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       const double w = wxy[q >> 1] * ((q & 1) ? tz : z0);
-      const double2* p = reinterpret_cast<const double2*>(G.gd4 + base + corner_offset(G, q));
-      const double2 xy = __ldg(p), zw = __ldg(p + 1);
-      B[0] = fma(w, xy.x, B[0]); B[1] = fma(w, xy.y, B[1]); B[2] = fma(w, zw.x, B[2]);
+      const float4 v = __ldg(G.g4 + base + corner_offset(G, q));
+      B[0] = fma(w, (double)v.x, B[0]); B[1] = fma(w, (double)v.y, B[1]); B[2] = fma(w, (double)v.z, B[2]);
     }
   }
   const double rho2 = fma(xd, xd, yd * yd);
@@ -174,50 +164,58 @@ struct GridFwdArgs {
 // cotangent, so the sweeps skip the tiles before n_lo and after n_hi (cfg 3: the 40 x 40 x 8 kpc box holds less than
 // half of the samples of the 20-kpc sightlines).  Warp-uniform.
 __device__ __forceinline__ void box_sample_range(const GridDesc& G, const Geometry& geo, const Triad& T, int& n_lo, int& n_hi) {
-  const double delta = geo.delta * T.scale;
-  double s_in = 0.0, s_out = (double)geo.n_los * delta;
+  // in units of samples: s / delta (reciprocals by rcp_d, ~1e-12 relative: far inside the one-sample margin)
+  const double inv_delta = rcp_d(geo.delta * T.scale);
+  double u_in = 0.0, u_out = (double)geo.n_los;
   const double dir[3] = {T.nxd, T.nyd, T.nzd};
-  const double half[3] = {G.bx / G.sx, G.by / G.sy, G.bz / G.sz};   // l / 2
+  const double half[3] = {G.hx, G.hy, G.hz};
   bool empty = false;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     const double o = geo.obs[a];
-    if (dir[a] != 0.0) {
-      const double t1 = (-half[a] - o) / dir[a], t2 = (half[a] - o) / dir[a];
-      s_in = fmax(s_in, fmin(t1, t2));
-      s_out = fmin(s_out, fmax(t1, t2));
+    if (fabs(dir[a]) > 1.0e-200) {
+      const double inv = rcp_d(dir[a]) * inv_delta;
+      const double t1 = (-half[a] - o) * inv, t2 = (half[a] - o) * inv;
+      u_in = fmax(u_in, fmin(t1, t2));
+      u_out = fmin(u_out, fmax(t1, t2));
     } else if (fabs(o) > half[a]) {
       empty = true;
     }
   }
-  if (empty || !(s_out >= s_in)) { n_lo = 0; n_hi = 0; return; }
-  n_lo = max(0, (int)floor(s_in / delta - 0.5) - 1);
-  n_hi = min(geo.n_los, (int)ceil(s_out / delta - 0.5) + 2);
+  if (empty || !(u_out >= u_in)) { n_lo = 0; n_hi = 0; return; }
+  n_lo = max(0, __double2int_rd(u_in - 0.5) - 1);
+  n_hi = min(geo.n_los, __double2int_ru(u_out - 0.5) + 2);
   if (n_hi < n_lo) n_hi = n_lo;
 }
 
 // Round-off scale of a sightline's Faraday sum, k-independent part: sum_n |n_e| (|B_LOS| + |B_N| + |B_E|),
-// estimated from every 8th sample with the fp32 chain (whole warp; returns the same value in every lane).
+// estimated with the fp32 chain from 32 samples spread over the in-box range [n_lo, n_hi), B taken at the NEAREST node
+// (one gather per sample: with the lanes in 32 different cells a trilinear gather costs 8 x 32 L1 wavefronts).  It only
+// routes the sightline -- the fp32 sweep checks the exact sum afterwards.  Whole warp; the same value in every lane.
 template <bool SG>
 __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const BatchConsts& P, const Triad& T,
-                                                        const Geometry& geo, const ScalarGridDesc& sg_ne, int lane) {
+                                                        const Geometry& geo, const ScalarGridDesc& sg_ne, int lane,
+                                                        int n_lo, int n_hi) {
+  const int stride = (n_hi - n_lo + 31) >> 5;
+  const int n = n_lo + lane * stride + (stride >> 1);
   float acc = 0.f;
-  int n_lo, n_hi;
-  box_sample_range(G, geo, T, n_lo, n_hi);
-  for (int n = (n_lo & ~7) + 4 + 8 * lane; n < n_hi; n += 256) {
+  if (n < n_hi) {
     const double s_d = ((double)n + 0.5) * geo.delta * T.scale;
     const double xd = fma(s_d, T.nxd, geo.obs[0]), yd = fma(s_d, T.nyd, geo.obs[1]), zd = fma(s_d, T.nzd, geo.obs[2]);
-    const Cell c = locate(G, xd, yd, zd);
-    float B[3], N0, ne;
-    gather_B(G, c, B);
-    densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
-    if (SG && sg_ne.g) ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
-    const float Bpar = fmaf(B[0], T.nx, fmaf(B[1], T.ny, B[2] * T.nz));
-    const float BN = fmaf(B[0], T.eNx, fmaf(B[1], T.eNy, B[2] * T.eNz));
-    const float BE = fmaf(B[0], T.eEx, B[1] * T.eEy);
-    acc = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), acc);
+    const double ux = fma(xd, G.sx, G.bx), uy = fma(yd, G.sy, G.by), uz = fma(zd, G.sz, G.bz);
+    const int i = __double2int_rn(ux), j = __double2int_rn(uy), k = __double2int_rn(uz);
+    if (i >= 0 && i < G.nx && j >= 0 && j < G.ny && k >= 0 && k < G.nz) {
+      const float4 B = __ldg(G.g4 + (i * G.ny + j) * G.nz + k);
+      float N0, ne;
+      densities_f32(P, (float)fma(xd, xd, yd * yd), (float)zd, N0, ne);
+      if (SG && sg_ne.g) ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
+      const float Bpar = fmaf(B.x, T.nx, fmaf(B.y, T.ny, B.z * T.nz));
+      const float BN = fmaf(B.x, T.eNx, fmaf(B.y, T.eNy, B.z * T.eNz));
+      const float BE = fmaf(B.x, T.eEx, B.y * T.eEy);
+      acc = fabsf(ne) * (fabsf(Bpar) + fabsf(BN) + fabsf(BE));
+    }
   }
-  return 8.0f * T.scalef * group_sum<32>(acc);
+  return (float)stride * T.scalef * group_sum<32>(acc);
 }
 
 // One sightline, whole warp, lanes on CONSECUTIVE samples (neighbouring lanes gather neighbouring cells).
@@ -225,16 +223,14 @@ __device__ __forceinline__ float grid_roundoff_estimate(const GridDesc& G, const
 template <int NF, bool PRECISE, bool SG>
 __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const GridDesc& G, const FreqTab& ft,
                                                     const BatchConsts& P, const BatchConstsD& D, const Triad& T,
-                                                    const double4 dir, int lane, float& accI, float (&accQ)[NF],
-                                                    float (&accU)[NF]) {
+                                                    const double4 dir, int lane, int n_lo, int n_hi, float& accI,
+                                                    float (&accQ)[NF], float (&accU)[NF]) {
   accI = 0.f;
 #pragma unroll
   for (int f = 0; f < NF; ++f) { accQ[f] = 0.f; accU[f] = 0.f; }
   double carry = 0.0;
   float absS = 0.f;
   const double delta = A.geo.delta * T.scale;
-  int n_lo, n_hi;
-  box_sample_range(G, A.geo, T, n_lo, n_hi);
   for (int nt = n_lo & ~31; nt < n_hi; nt += 32) {
     const int n = nt + lane;
     const bool active = n < A.geo.n_los;
@@ -261,7 +257,7 @@ __device__ __forceinline__ float grid_forward_sweep(const ForwardArgs& A, const 
       if (active) absS = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), absS);
       const float incl = warp_inclusive_scan(gn, lane);
       S_here = carry + (double)(incl - 0.5f * gn);
-      carry += warp_sum_d((double)gn);
+      carry += (double)__shfl_sync(0xffffffffu, incl, 31);   // the tile's fp32 sum, as the lanes saw it
     } else {
       double Bpar, BN, BE, ne;
       float N0;
@@ -309,13 +305,15 @@ __global__ void __launch_bounds__(kBlock) grid_forward_kernel(const __grid_const
     const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);
     const Triad T = load_triad(A.geo, pix);
     float accI, accQ[NF], accU[NF];
+    int n_lo, n_hi;   // the samples that can lie inside the box
+    box_sample_range(G, A.geo, T, n_lo, n_hi);
     bool precise = GA.mode == 2;
-    if (GA.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
+    if (GA.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane, n_lo, n_hi) > A.flag_S;
     if (!precise) {
-      const float scale = grid_forward_sweep<NF, false, SG>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
+      const float scale = grid_forward_sweep<NF, false, SG>(A, G, ft, P, D, T, dir, lane, n_lo, n_hi, accI, accQ, accU);
       precise = GA.mode == 0 && scale > A.flag_S;
     }
-    if (precise) grid_forward_sweep<NF, true, SG>(A, G, ft, P, D, T, dir, lane, accI, accQ, accU);
+    if (precise) grid_forward_sweep<NF, true, SG>(A, G, ft, P, D, T, dir, lane, n_lo, n_hi, accI, accQ, accU);
     if (lane == 0) {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
@@ -334,13 +332,12 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c) 
   asm volatile("red.global.v4.f32.add [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(0.0f) : "memory");
 }
 
-// caller's [node][3] grid -> padded fp32 nodes and (optionally) float64 nodes
-__global__ void grid_pack_kernel(const float* __restrict__ g, int64_t n_nodes, float4* __restrict__ g4, double4* __restrict__ gd4) {
+// caller's [node][3] grid -> padded fp32 nodes
+__global__ void grid_pack_kernel(const float* __restrict__ g, int64_t n_nodes, float4* __restrict__ g4) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_nodes) return;
   const float x = g[3 * i], y = g[3 * i + 1], z = g[3 * i + 2];
   g4[i] = make_float4(x, y, z, 0.f);
-  if (gd4) gd4[i] = make_double4((double)x, (double)y, (double)z, 0.0);
 }
 
 // [n][4] accumulation buffer -> caller's [n][3] gradient
@@ -406,7 +403,7 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
       if (active) absS = fmaf(fabsf(ne), fabsf(Bpar) + fabsf(BN) + fabsf(BE), absS);
       const float incl = warp_inclusive_scan(gn, lane);
       S_here = carry + (double)(incl - 0.5f * gn);
-      carry += warp_sum_d((double)gn);
+      carry += (double)__shfl_sync(0xffffffffu, incl, 31);
     } else {
       double Bpar, BNd, BEd, ned;
       fields_f64(G, P, D, dir, xd, yd, zd, Bpar, BNd, BEd, N0, ned);
@@ -485,7 +482,7 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
     while ((32 << cl2) < n_hi - n_lo) ++cl2;
     float absS = 0.f;
     bool precise = A.mode == 2;
-    if (A.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane) > A.flag_S;
+    if (A.mode == 0) precise = grid_roundoff_estimate<SG>(G, P, T, A.geo, A.sg_ne, lane, n_lo, n_hi) > A.flag_S;
     if (!precise) absS = grid_vjp_sweep1<NF, false, SG>(A, ft, G, P, D, T, dir, lane, cI, cQ, cU, kr, n_lo, n_hi, cl2, st_w, st_n, st_e);
     if (precise || (A.mode == 0 && absS > A.flag_S)) {
       __syncwarp();

@@ -145,9 +145,10 @@ int main() {
   Geometry geo; geo.npix = npix; geo.n_los = n_los; geo.delta = s_max / n_los;
   geo.obs[0] = -8.3; geo.obs[1] = 0.0; geo.obs[2] = 0.006; geo.obsf[0] = -8.3f; geo.obsf[1] = 0.f; geo.obsf[2] = 0.006f; geo.dirs = dirs; geo.path = nullptr;
   float4* grid4; CK(cudaMalloc(&grid4, ngrid / 3 * sizeof(float4))); CK(cudaMemset(grid4, 0, ngrid / 3 * sizeof(float4)));
-  GridDesc G; G.g = grid; G.g4 = grid4; G.gd4 = nullptr; G.nx = nx; G.ny = ny; G.nz = nz;
+  GridDesc G; G.g = grid; G.g4 = grid4; G.nx = nx; G.ny = ny; G.nz = nz;
   G.sx = (nx - 1) / 40.0; G.sy = (ny - 1) / 40.0; G.sz = (nz - 1) / 8.0;
   G.bx = 0.5 * (nx - 1); G.by = 0.5 * (ny - 1); G.bz = 0.5 * (nz - 1);
+  G.hx = 20.0; G.hy = 20.0; G.hz = 4.0;
   int sms = 148; cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
   cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
   const double samples = (double)npix * n_los;
