@@ -289,14 +289,12 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
         # The adjoint of a step reuses one float64 per sightline that the step's own forward stored (its Faraday total: the
         # backward sweep needs it first).  For the record, the same adjoint WITHOUT that residual (own pre-pass), a few calls:
         plan.set_option("use_forward_totals", 0)
-        ea = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-        ts = []
-        for k in range(1 + min(steps, 5)):
-            ea[0].record(stream); sx.vjp(plan, model, params, *cots, out=grad); ea[1].record(stream)
-            torch.cuda.synchronize()
+        ea = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(1 + min(steps, 5))]
+        for e in ea:   # no synchronisation between the calls: as in the timed steps, the stream-ordered pool keeps its blocks
+            e[0].record(stream); sx.vjp(plan, model, params, *cots, out=grad); e[1].record(stream)
             flush_buf.add_(1.0)
-            if k:
-                ts.append(ea[0].elapsed_time(ea[1]))
+        torch.cuda.synchronize()
+        ts = [e[0].elapsed_time(e[1]) for e in ea[1:]]
         plan.set_option("use_forward_totals", 1)
         res["timing"]["vjp_standalone_ms"] = {"mean": float(np.mean(ts)), "median": float(np.median(ts)), "best": float(np.min(ts))}
     if graph and not reduce_grad:

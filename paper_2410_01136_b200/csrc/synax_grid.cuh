@@ -27,6 +27,7 @@ struct GridDesc {
 
 struct Cell {
   int base;             // node index of corner (i,j,k)
+  int i, j, k;
   float tx, ty, tz;
   bool inbox;
 };
@@ -40,6 +41,7 @@ __device__ __forceinline__ Cell locate(const GridDesc& G, double x, double y, do
   i = max(0, min(i, G.nx - 2)); j = max(0, min(j, G.ny - 2)); k = max(0, min(k, G.nz - 2));
   c.tx = (float)(ux - (double)i); c.ty = (float)(uy - (double)j); c.tz = (float)(uz - (double)k);
   c.base = (i * G.ny + j) * G.nz + k;
+  c.i = i; c.j = j; c.k = k;
   return c;
 }
 
@@ -366,6 +368,63 @@ struct GridVjpArgs {
   float flag_S;         // auto: redo a sightline in float64 when max |sum n_e B_LOS| exceeds this
 };
 
+// Sweep 2's per-lane accumulators: the 8 x 3 corner contributions of the cell the lane is in.  A ray leaves a cell
+// through a face, and the 4 nodes of that face belong to the next cell too: only the 4 nodes left behind are
+// flushed (red.global.add), the shared ones stay in their registers.  So that nothing has to move, the registers
+// are addressed in "slot" coordinates: slot bit s of an axis means corner bit s ^ flip of that axis, and crossing a
+// face toggles the axis' flip (the kept registers were the far face of the old cell and are the near face of the new
+// one).  The trilinear weights follow by using 1 - t for a flipped axis.
+struct CornerAcc {
+  float acc[24];        // [slot q = (sa << 2) | (sb << 1) | sd][component]
+  int ci, cj, ck;       // the cell
+  int flip;             // bit 2: x, bit 1: y, bit 0: z
+  bool valid;           // in a cell (acc may be non-zero)
+};
+
+// node index of slot q of the current cell
+__device__ __forceinline__ int slot_node(const GridDesc& G, const CornerAcc& S, int q) {
+  const int a = ((q >> 2) ^ (S.flip >> 2)) & 1, b = ((q >> 1) ^ (S.flip >> 1)) & 1, d = (q ^ S.flip) & 1;
+  return ((S.ci + a) * G.ny + (S.cj + b)) * G.nz + (S.ck + d);
+}
+
+// flush (and clear) the slots whose bit of axis AX (2: x, 1: y, 0: z) equals h
+template <int AX>
+__device__ __forceinline__ void flush_half(const GridDesc& G, float* grad4, CornerAcc& S, int h) {
+  if (h == 0) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+      if (((q >> AX) & 1) == 0) {
+        red_add_v4(grad4 + (size_t)slot_node(G, S, q) * 4, S.acc[3 * q], S.acc[3 * q + 1], S.acc[3 * q + 2]);
+        S.acc[3 * q] = 0.f; S.acc[3 * q + 1] = 0.f; S.acc[3 * q + 2] = 0.f;
+      }
+  } else {
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+      if (((q >> AX) & 1) == 1) {
+        red_add_v4(grad4 + (size_t)slot_node(G, S, q) * 4, S.acc[3 * q], S.acc[3 * q + 1], S.acc[3 * q + 2]);
+        S.acc[3 * q] = 0.f; S.acc[3 * q + 1] = 0.f; S.acc[3 * q + 2] = 0.f;
+      }
+  }
+}
+
+// step to the neighbouring cell across the face of axis AX, `wd` = +1 or -1 cells
+template <int AX>
+__device__ __forceinline__ void cross_face(const GridDesc& G, float* grad4, CornerAcc& S, int wd) {
+  const int leave = wd > 0 ? 0 : 1;                       // corner bit of the face left behind
+  flush_half<AX>(G, grad4, S, leave ^ ((S.flip >> AX) & 1));
+  S.flip ^= 1 << AX;
+  if (AX == 2) S.ci += wd; else if (AX == 1) S.cj += wd; else S.ck += wd;
+}
+
+__device__ __forceinline__ void flush_all(const GridDesc& G, float* grad4, CornerAcc& S) {
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    // one 16-byte vector reduction per corner node (measured 2.6x the throughput of three scalar reds)
+    red_add_v4(grad4 + (size_t)slot_node(G, S, q) * 4, S.acc[3 * q], S.acc[3 * q + 1], S.acc[3 * q + 2]);
+    S.acc[3 * q] = 0.f; S.acc[3 * q + 1] = 0.f; S.acc[3 * q + 2] = 0.f;
+  }
+}
+
 // Sweep 1 of the gridded adjoint for one sightline (whole warp): per-sample forward quantities, cotangent
 // fan-out (A9) and the per-sample hand-over to sweep 2 through shared memory.  Returns sum n_e (|B_LOS| + |B_N| + |B_E|).
 template <int NF, bool PRECISE, bool SG>
@@ -504,12 +563,14 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
       if (lane + d < 32) incl += o;
     }
     float suf = incl - tot;      // sum of Sbar over all later lanes
-    float acc[24];
+    CornerAcc S;
 #pragma unroll
-    for (int q = 0; q < 24; ++q) acc[q] = 0.f;
-    int cur = -1;
+    for (int q = 0; q < 24; ++q) S.acc[q] = 0.f;
+    S.ci = S.cj = S.ck = 0; S.flip = 0; S.valid = false;
+    // walking backwards along the sightline the cell indices move against the direction (warp-uniform)
+    const int wdx = T.nxd > 0.0 ? -1 : 1, wdy = T.nyd > 0.0 ? -1 : 1, wdz = T.nzd > 0.0 ? -1 : 1;
     for (int m = m1 - 1; m >= m0 - 1; --m) {
-      Cell c; c.base = -1; c.inbox = false; c.tx = c.ty = c.tz = 0.f;
+      Cell c; c.base = -1; c.i = c.j = c.k = 0; c.inbox = false; c.tx = c.ty = c.tz = 0.f;
       float ne_m = 0.f;   // recomputed (fp32, 4 MUFU) rather than handed over: 25 % less shared memory per warp
       if (m >= m0) {
         const double s_d = ((double)m + 0.5) * delta;
@@ -520,35 +581,40 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
         if (SG && A.sg_ne.g) ne_m = scalar_grid_at<float>(A.sg_ne, xd, yd, zd);
         ne_m *= T.scalef;
       }
-      const int cell = (m >= m0 && c.inbox) ? c.base : -1;
-      if (cell != cur) {
-        if (cur >= 0) {
-#pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            // one 16-byte vector reduction per corner node (measured 2.6x the throughput of three scalar reds)
-            red_add_v4(A.grad4 + (size_t)(cur + corner_offset(G, q)) * 4, acc[3 * q], acc[3 * q + 1], acc[3 * q + 2]);
-            acc[3 * q] = 0.f; acc[3 * q + 1] = 0.f; acc[3 * q + 2] = 0.f;
-          }
+      const bool have = m >= m0 && c.inbox;
+      if (S.valid) {
+        const int di = c.i - S.ci, dj = c.j - S.cj, dk = c.k - S.ck;
+        if (!have || (di != 0 && di != wdx) || (dj != 0 && dj != wdy) || (dk != 0 && dk != wdz)) {
+          flush_all(G, A.grad4, S);      // end of the chunk, out of the box, or not a face neighbour
+          S.valid = false;
+        } else {
+          if (di != 0) cross_face<2>(G, A.grad4, S, wdx);
+          if (dj != 0) cross_face<1>(G, A.grad4, S, wdy);
+          if (dk != 0) cross_face<0>(G, A.grad4, S, wdz);
         }
-        cur = cell;
       }
+      if (have && !S.valid) { S.ci = c.i; S.cj = c.j; S.ck = c.k; S.valid = true; }
       if (m >= m0) {
         const int idx = lane * Cq + (m - mb);
         const float Sb = st_w[idx];
         const float gbar = fmaf(0.5f, Sb, suf);
         suf += Sb;
-        if (cell >= 0) {
+        if (have) {
           const float BNb = st_n[idx], BEb = st_e[idx], gn = gbar * ne_m;
           const float bx = fmaf(BNb, T.eNx, fmaf(BEb, T.eEx, gn * T.nx));
           const float by = fmaf(BNb, T.eNy, fmaf(BEb, T.eEy, gn * T.ny));
           const float bz = fmaf(BNb, T.eNz, gn * T.nz);
+          Cell cs = c;   // weights in slot coordinates
+          if (S.flip & 4) cs.tx = 1.0f - c.tx;
+          if (S.flip & 2) cs.ty = 1.0f - c.ty;
+          if (S.flip & 1) cs.tz = 1.0f - c.tz;
           float w[8];
-          weights(c, w);
+          weights(cs, w);
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
-            acc[3 * q] = fmaf(w[q], bx, acc[3 * q]);
-            acc[3 * q + 1] = fmaf(w[q], by, acc[3 * q + 1]);
-            acc[3 * q + 2] = fmaf(w[q], bz, acc[3 * q + 2]);
+            S.acc[3 * q] = fmaf(w[q], bx, S.acc[3 * q]);
+            S.acc[3 * q + 1] = fmaf(w[q], by, S.acc[3 * q + 1]);
+            S.acc[3 * q + 2] = fmaf(w[q], bz, S.acc[3 * q + 2]);
           }
         }
       }
