@@ -426,11 +426,15 @@ def grid_roofline(w, r, local_samples):
                 "note": f"microbenchmarks unavailable: {ex}"}
     scale = local_samples / m["samples"]      # the microbenchmarks run cfg 3's geometry (49,152 x 512 samples)
     reds = m["red_v4_count"] * scale
-    return {"bound": "red", "kernel": "grid_vjp_kernel (two sweeps; per-cell register aggregation, red.global.v4.f32.add)",
+    return {"bound": "red", "kernel": "grid_vjp_kernel (two sweeps; per-cell register aggregation with the crossed face's 4 corners "
+                                      "carried into the next cell, red.global.v4.f32.add)",
             "achieved": reds / r["t_vjp"], "peak": m["red_v4_count"] / (m["red_v4_ms"] * 1e-3), "unit": "red.v4/s",
             "frac": (m["red_v4_ms"] * 1e-3 * scale) / r["t_vjp"], "traffic": None,
             "peak_source": "ubench grid_streams (R): red.global.v4.f32.add on the kernel's index stream, per-cell aggregated, measured in this run",
             "alg_red_v4_per_call": reds,
+            "note": "achieved / peak count the reference stream of SURVEY.md 8(d): 8 vector reds per cell a lane leaves. The kernel "
+                    "itself issues fewer (4 per face crossing + 8 per chunk end; 1.70e7 against 2.35e7 at cfg 3, ncu "
+                    "lts__t_requests_srcunit_tex_op_red in profiles/r02_cfg3_grid.md); frac = time of the reference stream / time of the call",
             "forward": {"bound": "l2-gather", "kernel": "grid_forward_kernel",
                         "achieved": m["gather_bytes"] * scale / r["t_fwd"] / 1e9, "peak": m["gather_bytes"] / (m["gather_ms"] * 1e-3) / 1e9,
                         "unit": "GB/s requested (96 B per in-box sample)", "frac": (m["gather_ms"] * 1e-3 * scale) / r["t_fwd"],
