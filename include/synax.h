@@ -134,8 +134,8 @@ synax_status synax_plan_directions(const synax_plan* plan, double* out_device, v
  * per 32 samples and sightline: 201 MB at nside 256 x 1024 samples) and a device copy of `params`, for the next synax_vjp of
  * this plan.  The buffers are plan-owned and grown with cudaMalloc the first time a call of a given size comes (that call
  * synchronises the device once; never inside a stream capture; if the memory is not there the call goes on without them).
- * GRID_B: per-call scratch of 48 bytes per grid node (16-byte fp32 nodes + 32-byte float64 nodes) from the stream-ordered
- * pool. */
+ * GRID_B: per-call scratch of 16 bytes per grid node (the grid repacked into 16-byte nodes) from the stream-ordered pool;
+ * synax_vjp takes another 16 bytes per node there for the gradient accumulation. */
 synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
                            int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
 
