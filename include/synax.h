@@ -171,6 +171,19 @@ synax_status synax_vjp_f64(const synax_plan* plan, const synax_model* model, con
                            int32_t batch, const double* dI, const double* dQ, const double* dU, double* grad,
                            void* cuda_stream);
 
+/* synax_vjp_f64 for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, same result, but the call's scratch -- the per-batch float64 constants and the per-CTA
+ * partial gradients -- lives in a fixed 4 MiB array inside the library image (every GPU that loads the library holds it
+ * until the process exits) and the call makes no cudaMalloc, cudaFree or other allocating call.  Limit: a call needs
+ * 872 * batch bytes (rounded up to 256) + 128 * batch * ceil(npix * lanes / 128) bytes (lanes = the "lanes" option, else
+ * 1, 8 or 32 by size); e.g. nside 64 x batch 10 at 8 lanes, or nside 256 x batch 5 at 1 lane.  More returns SYNAX_ERR_UNSUPPORTED and
+ * the message states both numbers; nothing is launched.  The plan's device must be the current device (as for every call).
+ * ALL calls on a device share the array: it keeps the last call's contents (a call clears what it reads before use), and
+ * two calls that overlap on the GPU -- different streams, or different host threads -- race: keep them on one stream. */
+synax_status synax_vjp_f64_noalloc(const synax_plan* plan, const synax_model* model, const double* params,
+                                   int32_t batch, const double* dI, const double* dQ, const double* dU, double* grad,
+                                   void* cuda_stream);
+
 /* Same operations with HOST buffers of the same shapes: the call copies the inputs to the device,
  * runs, copies the results back and synchronises the stream before returning.  When I, Q and U are all page-locked
  * (cudaHostAlloc / cudaHostRegister) the forward kernels store the maps straight into them and no copy is made.

@@ -19,7 +19,7 @@ KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3, "stack16": 4}
 
 # every symbol include/synax.h declares
 exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_box", "synax_plan_set_option",
-                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_f64", "synax_vjp_f64", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
+                    "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_f64", "synax_vjp_f64", "synax_vjp_f64_noalloc", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
 
@@ -70,7 +70,7 @@ def load_library() -> ctypes.CDLL:
     fwd = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, vp]
     bwd = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, vp, vp]
     for name, at in (("synax_forward", fwd), ("synax_forward_host", fwd), ("synax_vjp", bwd), ("synax_vjp_host", bwd),
-                     ("synax_forward_f64", fwd), ("synax_vjp_f64", bwd)):
+                     ("synax_forward_f64", fwd), ("synax_vjp_f64", bwd), ("synax_vjp_f64_noalloc", bwd)):
         getattr(L, name).argtypes = at
         getattr(L, name).restype = ctypes.c_int
     L.synax_loglike_vjp.argtypes = [vp, ctypes.POINTER(_CModel), vp, i32, vp, vp, vp, ctypes.POINTER(dbl), vp, vp, vp]
@@ -278,6 +278,18 @@ def vjp_f64(plan: Plan, model: Model, params, dI, dQ, dU, out=None):
     ptr = lambda t, w: ctypes.c_void_p(None) if t is None else _dev_f64(t, w, n)  # noqa: E731
     _check(load_library().synax_vjp_f64(plan.h, ctypes.byref(model.c), _dev_f64(params, "params"), batch,
                                         ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"), _dev_f64(out, "grad", params.numel()), _stream()))
+    return out
+
+
+def vjp_f64_noalloc(plan: Plan, model: Model, params, dI, dQ, dU, out):
+    """synax_vjp_f64_noalloc: synax_vjp_f64 on the library's fixed scratch array -- no allocation anywhere, so `out` (CUDA
+    float64 like params) is required.  SynaxError (SYNAX_ERR_UNSUPPORTED) when the call needs more than the 4 MiB array."""
+    batch = _batch_of(model, params)
+    n = batch * plan.n_freq * plan.npix
+    ptr = lambda t, w: ctypes.c_void_p(None) if t is None else _dev_f64(t, w, n)  # noqa: E731
+    _check(load_library().synax_vjp_f64_noalloc(plan.h, ctypes.byref(model.c), _dev_f64(params, "params"), batch,
+                                                ptr(dI, "dI"), ptr(dQ, "dQ"), ptr(dU, "dU"),
+                                                _dev_f64(out, "grad", params.numel()), _stream()))
     return out
 
 

@@ -722,6 +722,32 @@ extern "C" synax_status synax_vjp_f64(const synax_plan* plan, const synax_model*
   return SYNAX_OK;
 }
 
+// synax_vjp_f64 without any allocation: the scratch is a fixed array inside the library (synax_dd.cu).
+extern "C" synax_status synax_vjp_f64_noalloc(const synax_plan* plan, const synax_model* model, const double* params,
+                                              int32_t batch, const double* dI, const double* dQ, const double* dU,
+                                              double* grad, void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_f64_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
+  const int G = pick_lanes(plan, plan->npix * batch);
+  const size_t need = dd_noalloc_bytes(plan->npix, G, batch), cap = dd_noalloc_capacity();
+  if (need > cap)
+    return fail(SYNAX_ERR_UNSUPPORTED,
+                "synax_vjp_f64_noalloc: this call needs %zu bytes of scratch (npix %lld x %d lanes, batch %d) but the static "
+                "array holds %zu; use synax_vjp_f64, a smaller batch or fewer lanes",
+                need, (long long)plan->npix, G, (int)batch, cap);
+  cudaError_t ce = cudaSuccess;
+  stt = dd_vjp_noalloc(plan->device, code, plan->ft, make_geo(plan), params, model->n_params, batch, make_aux(model),
+                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
+                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), G, dI, dQ, dU, grad,
+                       (cudaStream_t)cuda_stream, &plan->launches, &ce);
+  if (stt != SYNAX_OK)
+    return fail(stt, "synax_vjp_f64_noalloc failed: %s%s", cudaGetErrorString(ce),
+                ce == cudaErrorInvalidDevice ? " (the plan's device must be the current device)" : "");
+  return SYNAX_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Fused Gaussian likelihood (Eq.(15)): forward -> residual cotangents + logL -> VJP.
 // ------------------------------------------------------------------------------------------------

@@ -59,5 +59,12 @@ synax_status dd_vjp(int code, const FreqTab& ft, const Geometry& geo, const doub
                     const AuxHost& aux, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0, int G, void* bc64,
                     double* partial, const double* dI, const double* dQ, const double* dU, double* grad, cudaStream_t st,
                     int64_t* launches);
+// the adjoint on the library's static scratch array (synax_vjp_f64_noalloc): capacity, bytes a call needs, the call
+size_t dd_noalloc_capacity();
+size_t dd_noalloc_bytes(int64_t npix, int G, int batch);
+synax_status dd_vjp_noalloc(int device, int code, const FreqTab& ft, const Geometry& geo, const double* params, int n_params,
+                            int batch, const AuxHost& aux, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0, int G,
+                            const double* dI, const double* dQ, const double* dU, double* grad, cudaStream_t st,
+                            int64_t* launches, cudaError_t* cuda_error);
 
 }  // namespace synax
