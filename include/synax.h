@@ -115,7 +115,8 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * key "use_forward_totals": 1 (default) = synax_vjp may take the sightlines' Faraday sums from what the plan's last
  * synax_forward stored (see synax_vjp); 0 = it always recomputes them in its own pre-pass.
  * key "batch_share": parameter vectors integrated per thread when a batch of analytic models is evaluated at one
- * frequency with one thread per sightline -- they share the sightline geometry (0 = heuristic, else 1, 2 or 4).
+ * frequency with one thread per sightline -- they share the sightline geometry (0 = heuristic, else 1, 2 or 4).  In
+ * synax_vjp values 2 and 4 apply unless the plan's last forward left tile bases (then the kernel that uses those runs).
  * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool
  * (from which every call takes its scratch) to this many MB, so that the pool is not unmapped at every stream
  * synchronisation -- matters for the *_host calls (hundreds of MB of staging per call).  Process-wide for that

@@ -18,7 +18,8 @@ template <int CODE> void fwd_launch_f64(int G, int nf, unsigned blocks, cudaStre
 
 // ---- adjoint (synax_vjp_impl.cuh, explicitly instantiated per CODE)
 template <int CODE> void vjp_launch(int pmode, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft);
-// batched lean adjoint (vjp_batched_kernel; DISC4 and FULL16), nb = 2 or 4, grid = (n_blocks, ceil(batch / nb))
+// forward-order lean adjoint (vjp_batched_kernel; DISC4 and FULL16, one frequency), nb = 1, 2 or 4 parameter vectors per
+// thread, grid = (n_blocks, ceil(batch / nb))
 template <int CODE> void vjp_launch_batched(int nb, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft);
 template <int CODE> void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, const VjpArgs& a, unsigned char* cta_sel);
 

@@ -669,7 +669,8 @@ __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MIN
 // ------------------------------------------------------------------------------------------------
 // Adjoint, batched (S:8(a) A12): the lean variant (fp32 Faraday angles, one thread per sightline, one frequency) for NB
 // consecutive parameter vectors per thread, sharing the sample geometry as forward_batched_kernel does.  Per vector the
-// arithmetic is that of vjp_kernel<CODE, 1, 1, 0>.  grid = (n_blocks, ceil(batch / NB)).
+// arithmetic is that of vjp_kernel<CODE, 1, 1, 0>, but in FORWARD order (prefix form of the reverse scan): no Faraday total
+// is needed first, so NB = 1 is also the stand-alone adjoint at one frequency.  grid = (n_blocks, ceil(batch / NB)).
 // ------------------------------------------------------------------------------------------------
 template <int CODE, int NB>
 __global__ void __launch_bounds__(kBlock) vjp_batched_kernel(const __grid_constant__ VjpArgs A, const __grid_constant__ FreqTab ft) {

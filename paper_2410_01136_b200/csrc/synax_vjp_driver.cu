@@ -15,7 +15,7 @@ static void launch_pmode(int code, int pmode, int G, int nf, dim3 grid, cudaStre
 
 // the lean fp32 variant, or its batched form (nb parameter vectors per thread sharing the sightline geometry, A12)
 static void launch_lean(int code, int nb, int G, int nf, dim3 grid, cudaStream_t st, const VjpArgs& a, const FreqTab& ft) {
-  if (nb > 1) {
+  if (nb > 0) {
     const dim3 gb(grid.x, (unsigned)((a.batch + nb - 1) / nb));
     SYNAX_DISPATCH_CODE(code, vjp_launch_batched, nb, gb, st, a, ft);
   } else {
@@ -46,6 +46,7 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_block
 // over ~8k sightlines finds none above HALF that threshold, in which case the lean fp32 variant (PMODE 0: fewer
 // registers, no estimate) runs (cfg 2 at 23 GHz: 8.2 instead of 9.5 ms).  Decided on the device, no host sync.
 constexpr double kVjpEscalateFactor = 10.0 / 3.0;   // x escalate_rad (300 rad by default): 1000 rad
+constexpr int kStandAloneVectors = 1;   // vectors per thread of the stand-alone forward-order adjoint (2: 8.25 ms at cfg 2)
 
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                                  const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
@@ -89,8 +90,15 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   // measured at cfg 2 (256 vectors, B200): sharing pays in the forward (5.09 -> 4.68 ms at 4 vectors per thread) but not here
   // -- two or four sets of 27 gradient accumulators per thread cost more occupancy than the shared geometry saves (8.46 ->
   // 8.82 / 9.53 ms) -- so the adjoint shares only on request (option "batch_share")
-  int nb = batch_share ? batch_share : 1;
-  if (!(G == 1 && ft.n_freq == 1 && (code == kAnalyticDisc || code == kAnalyticFull) && !sg_ne.g && !sg_n0.g && batch <= 65535)) nb = 1;
+  // nb: 0 = vjp_kernel (backward sweep), 1 / 2 / 4 = vjp_batched_kernel (forward order, that many vectors per thread).
+  // The backward sweep needs the sightline's Faraday total first.  After a forward of this plan it is there (phi); a call
+  // the host knows to be stand-alone would pay a pre-pass for it -- a second evaluation of the fields, 70 % on top at one
+  // frequency (cfg 2: 11.6 against 6.7 ms) -- so it takes the forward-order kernel instead, whose prefix-form scan needs no
+  // total (cfg 2 stand-alone: 7.7 ms).  With tile bases on offer the lean vjp_kernel is the one that uses them.
+  const bool fo_ok = G == 1 && ft.n_freq == 1 && (code == kAnalyticDisc || code == kAnalyticFull) && !sg_ne.g && !sg_n0.g && batch <= 65535;
+  int nb = 0;
+  if (fo_ok && batch_share > 1 && !phi_base) nb = batch_share;
+  else if (fo_ok && !phi) nb = kStandAloneVectors;
   float* partial = nullptr;
   if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess) {
     if (cta_sel) cudaFreeAsync(cta_sel, st);

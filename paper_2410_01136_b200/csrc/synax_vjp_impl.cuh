@@ -17,7 +17,8 @@ void vjp_launch_batched(int nb, dim3 grid, cudaStream_t st, const VjpArgs& a, co
   if constexpr (CODE == kAnalyticDisc || CODE == kAnalyticFull) {
     const FreqTab ft = shift_freqs(ft0, a.f0);
     if (nb == 4) vjp_batched_kernel<CODE, 4><<<grid, kBlock, 0, st>>>(a, ft);
-    else vjp_batched_kernel<CODE, 2><<<grid, kBlock, 0, st>>>(a, ft);
+    else if (nb == 2) vjp_batched_kernel<CODE, 2><<<grid, kBlock, 0, st>>>(a, ft);
+    else vjp_batched_kernel<CODE, 1><<<grid, kBlock, 0, st>>>(a, ft);
   }
 }
 

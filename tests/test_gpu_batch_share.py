@@ -72,3 +72,36 @@ def test_batch_share_with_alpha_not_three_and_low_frequency():
         parity.assert_maps_close(maps, refm, what=f"300 MHz batch_share={nb}")
         g = parity.gpu_vjp(w, cots, lanes=1, batch_share=nb)
         parity.assert_log_gradient_close(g, ref, th, what=f"300 MHz, batch_share={nb}")
+
+
+def test_batch_share_after_a_forward_that_left_tile_bases():
+    """Long single-frequency call at 408 MHz (strong rotation: device mode "split") with batch_share = 2, the adjoint right
+    after the forward of the same plan: the forward left tile bases, which only the lean vjp_kernel uses -- the shared
+    kernel stands aside for it (before, every launch of that combination stood aside and the gradient was never written)."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w2 = wl.config(2)
+    p = np.repeat(wl.FULL16_NOMINAL[None, :], 6, axis=0).astype(np.float32)
+    p *= (1.0 + 0.02 * np.arange(6, dtype=np.float32))[:, None]
+    w = wl.Workload("full16_408_b6", "full16", 64, 1024, w2.s_max, np.array([0.408e9]), p, w2.aux, cot_seed=515)
+    pix = np.arange(5, w.npix, 48)
+    full = w.cotangents()
+    cots_h = tuple(np.zeros_like(c) for c in full)
+    for c, f in zip(cots_h, full):
+        c[..., pix] = f[..., pix]
+    ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots_h), pix=pix)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    th = w.params.astype(np.float64)
+    for nb in (1, 2):
+        plan, model, params = parity.gpu_objects(w, lanes=1, batch_share=nb)
+        out = torch.full_like(params, float("nan"))
+        sx.vjp(plan, model, params, *cots, out=out)                       # stand-alone
+        torch.cuda.synchronize()
+        parity.assert_log_gradient_close(out.cpu().numpy().astype(np.float64), ref, th, what=f"alone, batch_share={nb}")
+        sx.forward(plan, model, params)
+        out.fill_(float("nan"))
+        sx.vjp(plan, model, params, *cots, out=out)                       # on the forward's totals and tile bases
+        torch.cuda.synchronize()
+        assert plan.stats()["escalated"] > 0.02 * w.npix * 6
+        parity.assert_log_gradient_close(out.cpu().numpy().astype(np.float64), ref, th, what=f"after forward, batch_share={nb}")
+        plan.close()
