@@ -239,7 +239,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False, graph=False):
+def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False, graph=False, lanes=0):
     """Device-resident timing of forward and VJP with CUDA events on the launching stream, L2 flushed between
     timed calls; then (optionally) the host-buffer entry points.  pix_range: this rank's pixel shard (strong
     scaling), with the one gradient all-reduce of the method inside the timed VJP when reduce_grad is set."""
@@ -247,6 +247,8 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
     if want_e2e:   # the *_host calls stage hundreds of MB per call in the stream-ordered pool: keep it mapped (opt-in)
         plan.set_option("pool_release_threshold_mb", 4096)
+    if lanes:
+        plan.set_option("lanes", lanes)
     npix = plan.npix
     p0 = 0 if pix_range is None else pix_range[0]
     if w.kind == "grid_b":
@@ -463,7 +465,7 @@ def run_ours(args):
         pix_range = sharding.shard_of(w.npix, rank, world)
     else:           # independent chains: every rank integrates the whole sky for its own parameter vector
         w = apply_overrides(rank_workload(args.config, rank), args)
-    kw = dict(pix_range=pix_range, reduce_grad=strong)
+    kw = dict(pix_range=pix_range, reduce_grad=strong, lanes=args.lanes)
     flush_buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
 
     def barrier():
@@ -553,6 +555,7 @@ def main():
     ap.add_argument("--nside", type=int, default=0, help="override the config's nside (runtime sweeps)")
     ap.add_argument("--n-los", type=int, default=0, help="override the config's samples per sightline")
     ap.add_argument("--freq-hz", type=float, default=0.0, help="run at this single frequency instead of the config's")
+    ap.add_argument("--lanes", type=int, default=0, help="plan option 'lanes' (threads per sightline: 1, 8 or 32; 0 = the library's choice)")
     ap.add_argument("--graph", action="store_true", help="also time the step captured in a CUDA graph (launch-bound configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline oracle sample")

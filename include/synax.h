@@ -111,7 +111,9 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * them flagged, or split between the two chains in between.  Auto, VJP: decided per sightline (per CTA in long calls)
  * -- those above 10/3 x escalate_rad take their Faraday angles from the float64 chain.
  * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0).
- * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).
+ * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).  Heuristic: one thread per sightline from 150,000
+ * sightlines (npix x batch) in synax_forward, from 300,000 in a stand-alone synax_vjp and the float64 entry points, and from
+ * 24,576 in a synax_vjp that finds the Faraday sums of the plan's last forward; 8 lanes down to an eighth of that, else 32.
  * key "use_forward_totals": 1 (default) = synax_vjp may take the sightlines' Faraday sums from what the plan's last
  * synax_forward stored (see synax_vjp); 0 = it always recomputes them in its own pre-pass.
  * key "batch_share": parameter vectors integrated per thread when a batch of analytic models is evaluated at one
@@ -129,8 +131,8 @@ synax_status synax_plan_directions(const synax_plan* plan, double* out_device, v
 
 /* Forward.  params: DEVICE fp32 [batch][n_params] (GRID_B: the grid, batch == 1).
  * I, Q, U: DEVICE fp32 [batch][n_freq][npix], overwritten, Kelvin.
- * Side effect kept inside the plan: a call that integrates every sightline with one thread (>= 300,000 sightlines, or
- * option "lanes" = 1; analytic models without a gridded n_e) also stores each sightline's Faraday sum (one float64, Eq.(7)
+ * Side effect kept inside the plan: a call over >= 24,576 sightlines (or with option "lanes" = 1; analytic models without
+ * a gridded n_e; any lane count) also stores each sightline's Faraday sum (one float64, Eq.(7)
  * P:L79 at the far end), for the sightlines its float64 chain integrates the Faraday depth before every 32nd sample (8 bytes
  * per 32 samples and sightline: 201 MB at nside 256 x 1024 samples) and a device copy of `params`, for the next synax_vjp of
  * this plan.  The buffers are plan-owned and grown with cudaMalloc the first time a call of a given size comes (that call

@@ -329,9 +329,13 @@ static ScalarGridDesc make_scalar_desc(const float* g, const int32_t n[3], const
   return d;
 }
 
-static int pick_lanes(const synax_plan* plan, int64_t n_sl) {
+// Lanes per sightline.  `want`: sightlines from which one thread each is the better choice -- measured on B200 with the cfg-4
+// model at 8 frequencies (nside 32 ... 192, 256 ... 4096 samples) and cfg 1: 300,000 for a stand-alone adjoint and the
+// float64 entry points (a few waves of 3-CTA-per-SM kernels), 150,000 for the forward, 24,576 for an adjoint that finds the
+// Faraday totals of the plan's last forward (no pre-pass, no lane scans: 0.86 against 1.34 ms at nside 64 x 1024 samples).
+constexpr int64_t kOneLaneFrom = 300000, kOneLaneFromForward = 150000, kOneLaneFromStored = 24576;
+static int pick_lanes(const synax_plan* plan, int64_t n_sl, int64_t want = kOneLaneFrom) {
   if (plan->lanes) return plan->lanes;
-  const int64_t want = 300000;  // threads needed to fill 148 SMs a few times over
   if (n_sl >= want) return 1;
   if (n_sl * 8 >= want) return 8;
   return 32;
@@ -545,9 +549,10 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       piloted = true;
     }
   }
-  const int G = pick_lanes(plan, n_sl);
-  // one thread per sightline: the adjoint will want the Faraday totals (it has a pre-pass of its own otherwise)
-  const bool keep_phi = G == 1 && phi_buffers(plan, model, batch, st);
+  const int G = pick_lanes(plan, n_sl, kOneLaneFromForward);
+  // the adjoint will want the Faraday totals (it has a pre-pass of its own otherwise); whatever the lane count here, it can
+  // then run with one thread per sightline
+  const bool keep_phi = pick_lanes(plan, n_sl, kOneLaneFromStored) == 1 && phi_buffers(plan, model, batch, st);
   if (keep_phi) a.phi = plan->phi_cache;
   const bool keep_base = keep_phi && plan->precision != 1 && plan->phi_base && plan->phi_has &&
                          plan->phi_base_cap >= (size_t)n_sl * ((size_t)(plan->n_los + 31) / 32) && plan->phi_has_cap >= (size_t)n_sl;
@@ -649,9 +654,12 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   const double* phi = nullptr;
   const double* phi_base = nullptr;
   const unsigned char* phi_has = nullptr;
-  if (code != kGridB && !plan->no_forward_totals && plan->phi_stamp.valid && !model->ne_grid && pick_lanes(plan, plan->npix * batch) == 1) {
+  int G = pick_lanes(plan, plan->npix * batch);
+  if (code != kGridB && !plan->no_forward_totals && plan->phi_stamp.valid && !model->ne_grid &&
+      pick_lanes(plan, plan->npix * batch, kOneLaneFromStored) == 1) {
     const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
     if (std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0) {
+      G = 1;
       phi_validate_kernel<<<1, 256, 0, st>>>(params, plan->phi_params, (int64_t)batch * model->n_params, plan->d_phi_ok);
       plan->launches++;
       phi = plan->phi_cache;
@@ -664,7 +672,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
                   make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
                   sm_count(plan->device), st, &plan->launches);
   else
-    rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, pick_lanes(plan, plan->npix * batch),
+    rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, G,
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
                       plan->batch_share, phi, plan->d_phi_ok, phi_base, phi_has, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,

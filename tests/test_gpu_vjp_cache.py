@@ -179,3 +179,33 @@ def test_tile_bases_with_batch_and_frequency_blocks():
     g = _grad(plan, model, dparams, cots)
     assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), np.abs(g - ref) / np.abs(ref)
     plan.close()
+
+
+@pytest.mark.parametrize("freqs,n_los", [((0.408e9, 1.4e9), 500), ((23e9,), 500), ((0.408e9, 2.4e9, 23e9), 1024)])
+def test_mid_size_forward_with_lanes_then_one_thread_adjoint(freqs, n_los):
+    """27,648 sightlines, the library's own lane choice: the forward runs with 8 lanes per sightline and still stores the
+    Faraday totals (and, from its float64 chain, the tile bases -- written per lane and shifted by the lane offsets); the
+    adjoint that follows then takes one thread per sightline on them.  Cotangent on every 24th pixel, oracle over those;
+    the stand-alone adjoint (8 lanes, own pre-pass) must agree too."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w4 = wl.config(4)
+    w = wl.Workload("cfg4_mid", w4.kind, 48, n_los, w4.s_max, np.array(freqs), w4.params, w4.aux, cot_seed=3305)
+    pix = np.arange(3, w.npix, 24)
+    full = w.cotangents()
+    cots_h = tuple(np.zeros_like(c) for c in full)
+    for c, f in zip(cots_h, full):
+        c[..., pix] = f[..., pix]
+    ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots_h), pix=pix)
+    ref_maps = parity.oracle_forward(w, pix=pix)
+    plan, model, params = parity.gpu_objects(w)
+    cots = [torch.from_numpy(c).cuda() for c in cots_h]
+    g_alone = _grad(plan, model, params, cots)
+    maps = sx.forward(plan, model, params)
+    torch.cuda.synchronize()
+    parity.assert_maps_close(tuple(m.cpu().numpy()[..., pix] for m in maps), ref_maps, what="mid-size forward")
+    g_after = _grad(plan, model, params, cots)
+    for g, what in ((g_alone, "stand-alone"), (g_after, "after the forward")):
+        assert np.all(np.abs(g - ref) <= parity.GRAD_TOL * np.abs(ref)), (what, np.abs(g - ref) / np.abs(ref))
+    assert np.array_equal(g_after, _grad(plan, model, params, cots))
+    plan.close()
