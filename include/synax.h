@@ -155,7 +155,7 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
  * call).  Long calls (>= 262,144 sightlines) may run part of their kernels on a second stream owned by the plan,
  * forked from and joined back to `cuda_stream` by events inside the call (CUDA-graph capturable); a plan must
  * therefore not be used by two calls that run concurrently -- use one plan per stream.  (synax_forward does the same
- * in its split mode.)
+ * in its split mode: from 262,144 sightlines, or from 32,768 sightlines with 5e7 or more LoS samples.)
  * GRID_B: n_los <= 4096 (the per-sample hand-over between the two sweeps lives in shared memory); larger n_los
  * returns SYNAX_ERR_UNSUPPORTED. */
 synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,

@@ -333,6 +333,10 @@ static ScalarGridDesc make_scalar_desc(const float* g, const int32_t n[3], const
 // model at 8 frequencies (nside 32 ... 192, 256 ... 4096 samples) and cfg 1: 300,000 for a stand-alone adjoint and the
 // float64 entry points (a few waves of 3-CTA-per-SM kernels), 150,000 for the forward, 24,576 for an adjoint that finds the
 // Faraday totals of the plan's last forward (no pre-pass, no lane scans: 0.86 against 1.34 ms at nside 64 x 1024 samples).
+#ifndef SYNAX_SPLIT_FROM
+#define SYNAX_SPLIT_FROM 50000000
+#endif
+constexpr int64_t kSplitFromSamples = SYNAX_SPLIT_FROM;   // forward: LoS samples from which the split mode is worth its extra launches
 constexpr int64_t kOneLaneFrom = 300000, kOneLaneFromForward = 150000, kOneLaneFromStored = 24576;
 static int pick_lanes(const synax_plan* plan, int64_t n_sl, int64_t want = kOneLaneFrom) {
   if (plan->lanes) return plan->lanes;
@@ -532,7 +536,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       const unsigned pb = (unsigned)((n_pilot * 32 + kBlock - 1) / kBlock);
       SYNAX_DISPATCH_CODE(code, fwd_launch_pilot, pb, st, a, stride, n_pilot, ctrl);
       // the split mode costs a handful of extra launches: only for calls long enough not to notice (cfg 1: 0.19 ms in all)
-      split_ok = n_sl >= 262144;
+      split_ok = n_sl >= 262144 || (n_sl >= 32768 && n_sl * (int64_t)plan->n_los >= kSplitFromSamples);
       if (split_ok) {
         decide_forward_kernel<<<1, 1, 0, st>>>(ctrl, n_pilot);
         CUDA_TRY(scratch.get(&a.list_u, sizeof(int) * (size_t)n_sl));

@@ -181,16 +181,18 @@ def test_tile_bases_with_batch_and_frequency_blocks():
     plan.close()
 
 
-@pytest.mark.parametrize("freqs,n_los", [((0.408e9, 1.4e9), 500), ((23e9,), 500), ((0.408e9, 2.4e9, 23e9), 1024)])
-def test_mid_size_forward_with_lanes_then_one_thread_adjoint(freqs, n_los):
-    """27,648 sightlines, the library's own lane choice: the forward runs with 8 lanes per sightline and still stores the
+@pytest.mark.parametrize("nside,freqs,n_los", [(48, (0.408e9, 1.4e9), 500), (48, (23e9,), 500), (48, (0.408e9, 2.4e9, 23e9), 1024),
+                                               (64, (0.408e9, 2.4e9, 23e9), 1024)])
+def test_mid_size_forward_with_lanes_then_one_thread_adjoint(nside, freqs, n_los):
+    """27,648 sightlines (49,152 in the last case, which is long enough for the forward's split mode: one list per chain,
+    8 lanes each), the library's own lane choice: the forward runs with 8 lanes per sightline and still stores the
     Faraday totals (and, from its float64 chain, the tile bases -- written per lane and shifted by the lane offsets); the
     adjoint that follows then takes one thread per sightline on them.  Cotangent on every 24th pixel, oracle over those;
     the stand-alone adjoint (8 lanes, own pre-pass) must agree too."""
     import torch
     import paper_2410_01136_b200 as sx
     w4 = wl.config(4)
-    w = wl.Workload("cfg4_mid", w4.kind, 48, n_los, w4.s_max, np.array(freqs), w4.params, w4.aux, cot_seed=3305)
+    w = wl.Workload("cfg4_mid", w4.kind, nside, n_los, w4.s_max, np.array(freqs), w4.params, w4.aux, cot_seed=3305)
     pix = np.arange(3, w.npix, 24)
     full = w.cotangents()
     cots_h = tuple(np.zeros_like(c) for c in full)
@@ -203,6 +205,8 @@ def test_mid_size_forward_with_lanes_then_one_thread_adjoint(freqs, n_los):
     g_alone = _grad(plan, model, params, cots)
     maps = sx.forward(plan, model, params)
     torch.cuda.synchronize()
+    if nside == 64:
+        assert 0.02 * w.npix < plan.stats()["escalated"] < 0.9 * w.npix, plan.stats()     # split mode
     parity.assert_maps_close(tuple(m.cpu().numpy()[..., pix] for m in maps), ref_maps, what="mid-size forward")
     g_after = _grad(plan, model, params, cots)
     for g, what in ((g_alone, "stand-alone"), (g_after, "after the forward")):
