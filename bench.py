@@ -239,7 +239,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False, graph=False, lanes=0):
+def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False, graph=False, lanes=0, f64=False):
     """Device-resident timing of forward and VJP with CUDA events on the launching stream, L2 flushed between
     timed calls; then (optionally) the host-buffer entry points.  pix_range: this rank's pixel shard (strong
     scaling), with the one gradient all-reduce of the method inside the timed VJP when reduce_grad is set."""
@@ -299,6 +299,25 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
         ts = [e[0].elapsed_time(e[1]) for e in ea[1:]]
         plan.set_option("use_forward_totals", 1)
         res["timing"]["vjp_standalone_ms"] = {"mean": float(np.mean(ts)), "median": float(np.median(ts)), "best": float(np.min(ts))}
+    if f64 and w.kind != "grid_b" and not reduce_grad:
+        # the paper's own arithmetic (float64 throughout): synax_forward_f64 / synax_vjp_f64 on float64 buffers
+        p64 = params.double()
+        c64 = [c.double() for c in cots]
+        o64 = tuple(torch.empty((w.batch, w.n_freq, npix), dtype=torch.float64, device="cuda") for _ in range(3))
+        g64 = torch.empty_like(p64)
+        n64 = 1 + min(steps, 5)
+        e64 = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(n64)]
+        for e in e64:
+            e[0].record(stream); sx.forward_f64(plan, model, p64, out=o64)
+            e[1].record(stream); sx.vjp_f64(plan, model, p64, *c64, out=g64)
+            e[2].record(stream)
+            flush_buf.add_(1.0)
+        torch.cuda.synchronize()
+        tf64 = np.array([e[0].elapsed_time(e[1]) for e in e64[1:]]); tv64 = np.array([e[1].elapsed_time(e[2]) for e in e64[1:]])
+        res["float64_mode"] = {"forward_ms": float(np.median(tf64)), "vjp_ms": float(np.median(tv64)),
+                               "note": "synax_forward_f64 / synax_vjp_f64: every step in float64 (the paper's default precision), "
+                                       "float64 buffers; medians of %d calls, L2 flushed between" % (n64 - 1)}
+        del p64, c64, o64, g64
     if graph and not reduce_grad:
         # the whole step captured once in a CUDA graph and replayed (pays off when a step is launch-bound: cfg 0, 1)
         side = torch.cuda.Stream()
@@ -480,7 +499,7 @@ def run_ours(args):
     if rank == 0:
         sampler.start()
     barrier()
-    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False, graph=args.graph, **kw)
+    r = time_config(sx, torch, w, args.steps, args.warmup, flush_buf, want_e2e=False, graph=args.graph, f64=args.f64, **kw)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     e = time_config(sx, torch, w, min(args.steps, 5), 1, flush_buf, want_e2e=True, **kw)
@@ -524,6 +543,8 @@ def run_ours(args):
         }
         line["roofline"] = (grid_roofline(w, r, local_samples) if w.kind == "grid_b"
                             else alu_roofline(w, r, local_samples, peak, sm_max, peak_src, strong, clocks))
+        if "float64_mode" in r:
+            line["float64_mode"] = dict(r["float64_mode"], value=samples / (1e-3 * (r["float64_mode"]["forward_ms"] + r["float64_mode"]["vjp_ms"])), unit=UNIT)
         if "t_graph" in r:
             line["cuda_graph"] = {"ms_per_step": 1e3 * r["t_graph"], "value": samples / r["t_graph"], "unit": UNIT,
                                   "note": "forward + VJP captured once, replayed back to back (no L2 flush between replays)"}
@@ -556,6 +577,7 @@ def main():
     ap.add_argument("--n-los", type=int, default=0, help="override the config's samples per sightline")
     ap.add_argument("--freq-hz", type=float, default=0.0, help="run at this single frequency instead of the config's")
     ap.add_argument("--lanes", type=int, default=0, help="plan option 'lanes' (threads per sightline: 1, 8 or 32; 0 = the library's choice)")
+    ap.add_argument("--f64", action="store_true", help="also time the all-float64 entry points (synax_forward_f64 / synax_vjp_f64)")
     ap.add_argument("--graph", action="store_true", help="also time the step captured in a CUDA graph (launch-bound configs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time budget of the cpu_baseline oracle sample")
