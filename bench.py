@@ -10,8 +10,8 @@ fwd+VJP) at nside=256 x 1024 pts").  Default workload = BASELINE.json configs[4]
 multiplied in).  `value` = samples / (forward + VJP time), inputs resident in HBM.  `e2e` = the same
 through synax_forward_host / synax_vjp_host with pinned HOST buffers (copies inside the timed region).
 
-N > 1 (torchrun, one rank per GPU): the partition of SURVEY.md 8(e) -- contiguous RING pixel shards of ONE map, no
-exchange in the forward, one sum all-reduce of the gradient per VJP ("scaling": "strong": the map is fixed).
+N > 1 (torchrun, one rank per GPU): the partition of SURVEY.md 8(e) -- RING pixel shards of ONE map (interleaved: rank r takes
+pixels r, r + N, ..., so that every rank sees every latitude and the ranks take equally long), no exchange in the forward, one sum all-reduce of the gradient per VJP ("scaling": "strong": the map is fixed).
 --scaling weak runs independent parameter vectors (HMC chains) per rank instead, with no data-path collective
 (DESIGN.md section 9).
 
@@ -239,12 +239,12 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
-def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, reduce_grad=False, graph=False, lanes=0, f64=False):
+def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range=None, pix_stride=1, reduce_grad=False, graph=False, lanes=0, f64=False):
     """Device-resident timing of forward and VJP with CUDA events on the launching stream, L2 flushed between
     timed calls; then (optionally) the host-buffer entry points.  pix_range: this rank's pixel shard (strong
     scaling), with the one gradient all-reduce of the method inside the timed VJP when reduce_grad is set."""
     from paper_2410_01136_b200 import sharding
-    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range, pix_stride=pix_stride)
     if want_e2e:   # the *_host calls stage hundreds of MB per call in the stream-ordered pool: keep it mapped (opt-in)
         plan.set_option("pool_release_threshold_mb", 4096)
     if lanes:
@@ -256,7 +256,7 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
     else:
         model = sx.Model(w.kind, aux=w.aux)
     params = torch.from_numpy(w.params).cuda().contiguous()
-    cots_h = tuple(np.ascontiguousarray(c[..., p0:p0 + npix]) for c in w.cotangents())
+    cots_h = tuple(np.ascontiguousarray(c[..., p0:p0 + npix * pix_stride:pix_stride]) for c in w.cotangents())
     cots = [torch.from_numpy(c).cuda() for c in cots_h]
     out = tuple(torch.empty((w.batch, w.n_freq, npix), dtype=torch.float32, device="cuda") for _ in range(3))
     grad = torch.empty_like(params)
@@ -476,15 +476,17 @@ def run_ours(args):
     import paper_2410_01136_b200 as sx
     sx.load_library()                       # fails loudly when libsynax.so is missing
     strong = args.scaling == "strong" and world > 1
-    pix_range = None
+    pix_range, pix_stride = None, 1
     if strong:      # one map, pixel shards, one gradient all-reduce per step
         from paper_2410_01136_b200 import sharding
         from harness import workloads as wl
         w = apply_overrides(wl.config(args.config), args)
-        pix_range = sharding.shard_of(w.npix, rank, world)
+        # interleaved shards (rank r: pixels r, r + N, ...): every rank sees every latitude, so the ranks take equally long
+        begin, pix_stride, count = sharding.strided_shard_of(w.npix, rank, world)
+        pix_range = (begin, count)
     else:           # independent chains: every rank integrates the whole sky for its own parameter vector
         w = apply_overrides(rank_workload(args.config, rank), args)
-    kw = dict(pix_range=pix_range, reduce_grad=strong, lanes=args.lanes)
+    kw = dict(pix_range=pix_range, pix_stride=pix_stride, reduce_grad=strong, lanes=args.lanes)
     flush_buf = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
 
     def barrier():
@@ -521,7 +523,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded, harness/workloads.py)",
             "config": {"workload": w.name, "nside": w.nside, "n_los": w.n_los, "n_freq": w.n_freq, "batch": w.batch,
                        "model": w.kind, "samples_per_step": samples, "l2": "flushed between timed steps (256 MB write)",
-                       "parallelism": ("single GPU" if world == 1 else f"pixel shards x{world} + gradient all-reduce" if strong
+                       "parallelism": ("single GPU" if world == 1 else f"interleaved pixel shards x{world} + gradient all-reduce" if strong
                                        else f"independent parameter vectors x{world}")},
             "forward_samples_per_s": total / t_fwd, "vjp_samples_per_s": total / t_vjp,
             "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,

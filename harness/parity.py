@@ -41,10 +41,10 @@ def _oracle_vjp(w: wl.Workload, cots, pix=None):
                       clip_box=w.clip_box)
 
 
-def gpu_objects(w: wl.Workload, pix_range=None, **options):
+def gpu_objects(w: wl.Workload, pix_range=None, pix_stride=1, **options):
     import torch
     import paper_2410_01136_b200 as sx
-    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range)
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, observer=w.observer, pix_range=pix_range, pix_stride=pix_stride)
     if w.clip_box is not None:
         plan.set_box(w.clip_box)
     for k, v in options.items():

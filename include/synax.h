@@ -93,6 +93,13 @@ synax_status synax_plan_create(int32_t nside, int32_t n_los, double s_max_kpc, c
 synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
                                      int32_t n_freq, const double observer_kpc[3], int64_t pix_begin,
                                      int64_t pix_count, synax_plan** out);
+/* The same for every pix_stride-th pixel: RING pixels pix_begin + i * pix_stride, i < pix_count (all inside the map,
+ * pix_stride >= 1).  Rank r of N taking (r, N, ceil((npix - r) / N)) gives N disjoint shards that each see every latitude,
+ * so their run times are equal -- contiguous RING ranges are latitude bands, and the bands along the Galactic plane take
+ * 1.4x as long as the polar ones at 408 MHz.  Buffers and the partial gradient as for a shard. */
+synax_status synax_plan_create_strided(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
+                                       int32_t n_freq, const double observer_kpc[3], int64_t pix_begin,
+                                       int64_t pix_stride, int64_t pix_count, synax_plan** out);
 synax_status synax_plan_destroy(synax_plan* plan); /* NULL is allowed */
 int64_t synax_plan_npix(const synax_plan* plan);  /* pixels of this plan (12 nside^2 unless a shard), -1 for NULL */
 

@@ -18,7 +18,7 @@ STATUS = {0: "SYNAX_OK", 1: "SYNAX_ERR_INVALID_ARG", 2: "SYNAX_ERR_UNSUPPORTED",
 KINDS = {"disc4": 0, "full16": 1, "grid_b": 2, "uniform": 3, "stack16": 4}
 
 # every symbol include/synax.h declares
-exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_box", "synax_plan_set_option",
+exported_symbols = ("synax_plan_create", "synax_plan_create_shard", "synax_plan_create_strided", "synax_plan_destroy", "synax_plan_npix", "synax_plan_set_box", "synax_plan_set_option",
                     "synax_plan_directions", "synax_forward", "synax_vjp", "synax_forward_f64", "synax_vjp_f64", "synax_vjp_f64_noalloc", "synax_forward_host", "synax_vjp_host", "synax_loglike_vjp", "synax_adam_step",
                     "synax_plan_stats", "synax_last_error", "synax_version")
 
@@ -55,6 +55,9 @@ def load_library() -> ctypes.CDLL:
     L.synax_plan_create_shard.argtypes = [i32, i32, dbl, ctypes.POINTER(dbl), i32, ctypes.POINTER(dbl), i64, i64,
                                           ctypes.POINTER(vp)]
     L.synax_plan_create_shard.restype = ctypes.c_int
+    L.synax_plan_create_strided.argtypes = [i32, i32, dbl, ctypes.POINTER(dbl), i32, ctypes.POINTER(dbl), i64, i64, i64,
+                                            ctypes.POINTER(vp)]
+    L.synax_plan_create_strided.restype = ctypes.c_int
     L.synax_plan_destroy.argtypes = [vp]
     L.synax_plan_destroy.restype = ctypes.c_int
     L.synax_plan_npix.argtypes = [vp]
@@ -124,9 +127,10 @@ class Model:
 
 
 class Plan:
-    """synax_plan_create / synax_plan_create_shard (pix_range=(begin, count)) / synax_plan_destroy."""
+    """synax_plan_create / synax_plan_create_shard (pix_range=(begin, count)) / synax_plan_create_strided
+    (pix_range=(begin, count), pix_stride=n: pixels begin + i * n) / synax_plan_destroy."""
 
-    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006), pix_range=None):
+    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006), pix_range=None, pix_stride=1):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("synax needs a CUDA device (B200); there is no CPU fallback")
@@ -139,10 +143,14 @@ class Plan:
         fp, op = f.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), o.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
         if pix_range is None:
             _check(L.synax_plan_create(int(nside), int(n_los), float(s_max), fp, int(f.size), op, ctypes.byref(h)))
-        else:
+        elif int(pix_stride) == 1:
             _check(L.synax_plan_create_shard(int(nside), int(n_los), float(s_max), fp, int(f.size), op,
                                              int(pix_range[0]), int(pix_range[1]), ctypes.byref(h)))
+        else:
+            _check(L.synax_plan_create_strided(int(nside), int(n_los), float(s_max), fp, int(f.size), op,
+                                               int(pix_range[0]), int(pix_stride), int(pix_range[1]), ctypes.byref(h)))
         self.pix_range = None if pix_range is None else (int(pix_range[0]), int(pix_range[1]))
+        self.pix_stride = int(pix_stride)
         self.device = int(torch.cuda.current_device())
         self.h = h
         self.nside, self.n_los, self.s_max, self.freqs = int(nside), int(n_los), float(s_max), f

@@ -42,8 +42,8 @@ static synax_status fail(synax_status st, const char* fmt, ...) {
 
 struct synax_plan {
   int nside, n_los, n_freq, device;
-  int64_t npix;       // pixels of this plan (a shard holds pix0 .. pix0 + npix - 1 of the map)
-  int64_t pix0;
+  int64_t npix;       // pixels of this plan (a shard holds pixels pix0 + i * pix_stride, i < npix, of the map)
+  int64_t pix0, pix_stride;
   double s_max, delta;
   double obs[3];
   double* dirs;       // device [npix][4]
@@ -111,12 +111,18 @@ extern "C" synax_status synax_plan_create(int32_t nside, int32_t n_los, double s
 extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
                                                 int32_t n_freq, const double observer_kpc[3], int64_t pix_begin,
                                                 int64_t pix_count, synax_plan** out) {
+  return synax_plan_create_strided(nside, n_los, s_max_kpc, freqs_hz, n_freq, observer_kpc, pix_begin, 1, pix_count, out);
+}
+
+extern "C" synax_status synax_plan_create_strided(int32_t nside, int32_t n_los, double s_max_kpc, const double* freqs_hz,
+                                                  int32_t n_freq, const double observer_kpc[3], int64_t pix_begin,
+                                                  int64_t pix_stride, int64_t pix_count, synax_plan** out) {
   if (!out) return fail(SYNAX_ERR_INVALID_ARG, "out is NULL");
   *out = nullptr;
   if (nside < 1 || nside > 8192) return fail(SYNAX_ERR_INVALID_ARG, "nside %d not in 1..8192", nside);
-  if (pix_begin < 0 || pix_count < 1 || pix_begin + pix_count > 12LL * nside * nside)
-    return fail(SYNAX_ERR_INVALID_ARG, "pixel range [%lld, %lld) not inside the nside=%d map", (long long)pix_begin,
-                (long long)(pix_begin + pix_count), nside);
+  if (pix_begin < 0 || pix_count < 1 || pix_stride < 1 || pix_begin + (pix_count - 1) * pix_stride >= 12LL * nside * nside)
+    return fail(SYNAX_ERR_INVALID_ARG, "pixels %lld + i * %lld, i < %lld, not inside the nside=%d map", (long long)pix_begin,
+                (long long)pix_stride, (long long)pix_count, nside);
   if (n_los < 1 || n_los > 65536) return fail(SYNAX_ERR_INVALID_ARG, "n_los %d not in 1..65536", n_los);
   if (!(s_max_kpc > 0.0) || !std::isfinite(s_max_kpc)) return fail(SYNAX_ERR_INVALID_ARG, "s_max must be > 0");
   if (!freqs_hz || n_freq < 1 || n_freq > kMaxFreq) return fail(SYNAX_ERR_INVALID_ARG, "n_freq %d not in 1..32 or freqs NULL", n_freq);
@@ -130,7 +136,7 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   if (!p) return fail(SYNAX_ERR_ALLOC, "host allocation failed");
   std::memset(p, 0, sizeof(*p));
   p->nside = nside; p->n_los = n_los; p->n_freq = n_freq;
-  p->npix = pix_count; p->pix0 = pix_begin;
+  p->npix = pix_count; p->pix0 = pix_begin; p->pix_stride = pix_stride;
   p->s_max = s_max_kpc; p->delta = s_max_kpc / (double)n_los; p->s_max_fixed = s_max_kpc; p->path = nullptr;
   for (int f = 0; f < n_freq; ++f) p->freqs[f] = freqs_hz[f];
   for (int i = 0; i < 3; ++i) p->obs[i] = observer_kpc[i];
@@ -150,7 +156,7 @@ extern "C" synax_status synax_plan_create_shard(int32_t nside, int32_t n_los, do
   }
   if (e == cudaSuccess) {
     const int64_t blocks = (p->npix + 255) / 256;
-    pix2ang_kernel<<<(unsigned)blocks, 256>>>((int64_t)nside, p->pix0, p->npix, p->dirs);
+    pix2ang_kernel<<<(unsigned)blocks, 256>>>((int64_t)nside, p->pix0, p->pix_stride, p->npix, p->dirs);
     p->launches++;
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaDeviceSynchronize();

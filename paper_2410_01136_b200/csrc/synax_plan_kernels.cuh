@@ -16,11 +16,12 @@ __device__ __forceinline__ int64_t isqrt_i64(int64_t v) {
   return r;
 }
 
-// Writes dirs[i] for the `count` pixels p = pix0 + i of the nside map (a plan may hold a shard of the sky).
-__global__ void pix2ang_kernel(int64_t nside, int64_t pix0, int64_t count, double* __restrict__ dirs) {
+// Writes dirs[i] for the `count` pixels p = pix0 + i * stride of the nside map (a plan may hold a shard of the sky: a
+// contiguous range, stride 1, or every stride-th pixel).
+__global__ void pix2ang_kernel(int64_t nside, int64_t pix0, int64_t stride, int64_t count, double* __restrict__ dirs) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= count) return;
-  const int64_t p = pix0 + idx;
+  const int64_t p = pix0 + idx * stride;
   const int64_t npix = 12 * nside * nside;
   const int64_t ncap = 2 * nside * (nside - 1);
   double z, phi, omz;  // omz = 1 - |z| kept separately for accurate cos b near the poles

@@ -141,7 +141,7 @@ int main() {
   CK(cudaMalloc(&grid, ngrid * 4)); CK(cudaMalloc(&grad, ngrid * 4)); CK(cudaMalloc(&out, npix * 4));
   CK(cudaMalloc(&count, 8));
   CK(cudaMemset(grid, 0, ngrid * 4)); CK(cudaMemset(grad, 0, ngrid * 4));
-  pix2ang_kernel<<<(unsigned)((npix + 255) / 256), 256>>>(nside, 0, npix, dirs);
+  pix2ang_kernel<<<(unsigned)((npix + 255) / 256), 256>>>(nside, 0, 1, npix, dirs);
   Geometry geo; geo.npix = npix; geo.n_los = n_los; geo.delta = s_max / n_los;
   geo.obs[0] = -8.3; geo.obs[1] = 0.0; geo.obs[2] = 0.006; geo.obsf[0] = -8.3f; geo.obsf[1] = 0.f; geo.obsf[2] = 0.006f; geo.dirs = dirs; geo.path = nullptr;
   float4* grid4; CK(cudaMalloc(&grid4, ngrid / 3 * sizeof(float4))); CK(cudaMemset(grid4, 0, ngrid / 3 * sizeof(float4)));

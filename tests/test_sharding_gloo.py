@@ -36,6 +36,22 @@ def test_pixel_shards_cover_and_balance():
     assert [c for _, c in sharding.batch_shards(2, 4)] == [1, 1, 0, 0]
 
 
+def test_strided_shards_cover_and_balance():
+    for npix, world in ((768, 1), (768, 2), (768, 5), (12 * 256 * 256, 8), (5, 8)):
+        seen = np.zeros(npix, dtype=np.int64)
+        counts = []
+        for r in range(world):
+            begin, stride, count = sharding.strided_shard_of(npix, r, world)
+            assert begin == r and stride == world
+            if count:
+                assert begin + (count - 1) * stride < npix
+                seen[begin::stride][:count] += 1
+            counts.append(count)
+        assert np.all(seen == 1) and sum(counts) == npix and max(counts) - min(counts) <= 1
+    with pytest.raises(ValueError):
+        sharding.strided_shard_of(10, 3, 3)
+
+
 def _free_port():
     s = socket.socket()
     s.bind(("127.0.0.1", 0))
@@ -44,7 +60,7 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, out_dir):
+def _worker(rank, world, port, out_dir, strided=False):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -53,13 +69,20 @@ def _worker(rank, world, port, out_dir):
         from harness import workloads as wl
         oracle.set_num_threads(2)
         w = wl.config(2).scaled(nside=4, n_los=64, batch=3)           # FULL16, batch 3, 192 pixels
-        begin, count = sharding.shard_of(w.npix, rank, world)
-        pix = np.arange(begin, begin + count)
+        if strided:
+            begin, stride, count = sharding.strided_shard_of(w.npix, rank, world)
+            pix = begin + stride * np.arange(count)
+        else:
+            begin, count = sharding.shard_of(w.npix, rank, world)
+            pix = np.arange(begin, begin + count)
         cots = w.cotangents()
         local = parity.oracle_forward(w, pix=pix)
         g_local = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots), pix=pix)
         g = sharding.reduce_gradient(torch.from_numpy(g_local.copy()))
-        full_Q = sharding.gather_maps(torch.from_numpy(local[1]), w.npix)
+        if strided:   # the gradient is what the shards exchange; the maps stay interleaved on their ranks
+            full_Q = torch.from_numpy(parity.oracle_forward(w)[1]) if rank == 0 else None
+        else:
+            full_Q = sharding.gather_maps(torch.from_numpy(local[1]), w.npix)
         if rank == 0:
             ref = parity.oracle_forward(w)
             g_ref = parity.oracle_vjp(w, cots)
@@ -74,10 +97,10 @@ def _worker(rank, world, port, out_dir):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world", [2, 3])
-def test_gloo_pixel_shards_reduce_to_the_full_gradient(world, tmp_path):
+@pytest.mark.parametrize("world,strided", [(2, False), (3, False), (2, True), (3, True)])
+def test_gloo_pixel_shards_reduce_to_the_full_gradient(world, strided, tmp_path):
     port = _free_port()
-    mp.spawn(_worker, args=(world, port, str(tmp_path)), nprocs=world, join=True)
+    mp.spawn(_worker, args=(world, port, str(tmp_path), strided), nprocs=world, join=True)
     rel_g, dq, shape_ok = np.load(tmp_path / "ok.npy")
     assert rel_g < 1e-13          # float64 partial sums in a different order
     assert dq == 0.0 and shape_ok == 1.0
