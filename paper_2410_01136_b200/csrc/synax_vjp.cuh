@@ -400,7 +400,7 @@ __device__ __forceinline__ double faraday_term_d(const BatchConsts& P, const Bat
 // grid = (n_blocks, batch); block = kBlock threads; G lanes per sightline.
 // PMODE 0: fp32 Faraday angles; 1: Faraday sums and angles from the float64 chain for every sightline; 2: decided per
 // sightline -- its round-off scale k_max sum |n_e|(|B_LOS|+|B_N|+|B_E|), estimated from every 16th sample, against
-// A.flag_S (= 10 x escalate_rad / k_max): sightlines below it carry an angle error <= ~3e-7 x 1000 rad = 3e-4 rad,
+// A.flag_S (= escalate_rad / k_max): sightlines below it carry an angle error <= ~3e-7 x 300 rad = 1e-4 rad,
 // inside the 1e-3 gradient bound; the others take the float64 chain.  The tile length is warp-uniform.
 #ifndef SYNAX_VJP_MINB
 #define SYNAX_VJP_MINB 1

@@ -41,11 +41,14 @@ __global__ void vjp_reduce_kernel(const float* __restrict__ partial, int n_block
   }
 }
 
-// The adjoint tolerates ~10x the Faraday round-off scale the forward does (gradients are sums over all pixels,
-// bound 1e-3 instead of 1e-4).  precision 0: per sightline (PMODE 2), threshold 10/3 x escalate_rad = 1000 rad -- unless a pilot
-// over ~8k sightlines finds none above HALF that threshold, in which case the lean fp32 variant (PMODE 0: fewer
-// registers, no estimate) runs (cfg 2 at 23 GHz: 8.2 instead of 9.5 ms).  Decided on the device, no host sync.
-constexpr double kVjpEscalateFactor = 10.0 / 3.0;   // x escalate_rad (300 rad by default): 1000 rad
+// precision 0: per sightline (PMODE 2), threshold = the forward's, escalate_rad (300 rad) -- unless a pilot over ~8k sightlines
+// finds none above HALF that threshold, in which case the lean fp32 variant (PMODE 0: fewer registers, no estimate) runs
+// (cfg 2 at 23 GHz: 8.2 instead of 9.5 ms).  Decided on the device, no host sync.
+// (Until late in round 2 the adjoint used 10/3 x escalate_rad = 1000 rad, on the argument that a gradient is a sum over all
+// pixels with a 1e-3 bound.  A cotangent that is non-zero on a few hundred pixels only -- a masked likelihood -- takes that
+// averaging away: of 400 seeded random mid-size workloads with such cotangents, 6 missed the bound by up to 5e-2 at 1000 rad,
+// one still at 500 rad, none at 300 rad.  The adjoint after a forward was never affected: it works on the forward's own selection.)
+constexpr double kVjpEscalateFactor = 1.0;   // x escalate_rad
 constexpr int kStandAloneVectors = 1;   // vectors per thread of the stand-alone forward-order adjoint (2: 8.25 ms at cfg 2)
 
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
