@@ -119,6 +119,7 @@ struct ForwardArgs {
   float* I; float* Q; float* U;
   int n_freq_total;
   float flag_S;           // flag a sightline when max |sum n_e B_LOS| exceeds this (<=0: never)
+  float flag_T;           // ... or when the Faraday sum inside one 32-sample tile of the fp32 chain exceeds this (<=0: never)
   int* flag_count;        // device counter
   int* flag_list;         // device list of flagged sightline ids (b * npix + p)
   ScalarGridDesc sg_ne, sg_n0;  // gridded n_e / N_0 replacing the analytic discs (DISC4, GRID_B), g == nullptr: unused
@@ -213,6 +214,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
   for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
   double carry = 0.0;            // chunk-local sum of n_e B_LOS over finished tiles
   float gabs = 0.0f;             // sum n_e (|B_LOS| + |B_N| + |B_E|): scale of the fp32 round-off in the Faraday sum
+  float tmax = 0.0f;             // largest |tile-local Faraday sum|: the fp32 rotation angle inside a tile is k_f times this
 
   for (int ts = n0; ts < n1; ts += kTile) {
     const int te = min(ts + kTile, n1);
@@ -279,6 +281,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
       }
     }
     carry += (double)hi + (double)lo;
+    tmax = fmaxf(tmax, fabsf(hi));
   }
 
   // combine the G lanes of the sightline
@@ -294,6 +297,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
     }
     accI = group_sum<G>(accI);
     absS = group_sum<G>(gabs);
+    tmax = group_max<G>(tmax);
   } else {
     absS = gabs;
   }
@@ -308,7 +312,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
     }
     if (A.f0 == 0 && A.phi) A.phi[sl] = phi_total;
     if (A.f0 == 0 && A.phi_has) A.phi_has[sl] = 0;
-    if (A.f0 == 0 && A.flag_S > 0.0f && absS > A.flag_S) {
+    if (A.f0 == 0 && A.flag_S > 0.0f && (absS > A.flag_S || tmax > A.flag_T)) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)sl;
     }
@@ -344,10 +348,10 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
   pf.init(delta, 0);
   const float k_rad = ft.k_rad[0];
 
-  float accI[NB], accQ[NB], accU[NB], gabs[NB];
+  float accI[NB], accQ[NB], accU[NB], gabs[NB], tmax[NB];
   double carry[NB];
 #pragma unroll
-  for (int j = 0; j < NB; ++j) { accI[j] = 0.f; accQ[j] = 0.f; accU[j] = 0.f; gabs[j] = 0.f; carry[j] = 0.0; }
+  for (int j = 0; j < NB; ++j) { accI[j] = 0.f; accQ[j] = 0.f; accU[j] = 0.f; gabs[j] = 0.f; tmax[j] = 0.f; carry[j] = 0.0; }
   for (int ts = 0; ts < A.geo.n_los; ts += kTile) {
     const int te = min(ts + kTile, A.geo.n_los);
     float hi[NB], lo[NB], tq[NB], tu[NB];
@@ -394,6 +398,7 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
         accQ[j] += tq[j]; accU[j] += tu[j];
       }
       carry[j] += (double)hi[j] + (double)lo[j];
+      tmax[j] = fmaxf(tmax[j], fabsf(hi[j]));
     }
   }
 #pragma unroll
@@ -406,7 +411,7 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
     A.U[o] = P.coefP[A.f0] * T.scalef * accU[j];
     if (A.f0 == 0 && A.phi) A.phi[(int64_t)bj[j] * A.geo.npix + pix] = carry[j];
     if (A.f0 == 0 && A.phi_has) A.phi_has[(int64_t)bj[j] * A.geo.npix + pix] = 0;
-    if (A.f0 == 0 && A.flag_S > 0.0f && gabs[j] > A.flag_S) {
+    if (A.f0 == 0 && A.flag_S > 0.0f && (gabs[j] > A.flag_S || tmax[j] > A.flag_T)) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)((int64_t)bj[j] * A.geo.npix + pix);
     }

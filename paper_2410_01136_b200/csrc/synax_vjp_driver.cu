@@ -75,7 +75,7 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   if (precision == 0) {
     ForwardArgs pa;
     pa.geo = geo; pa.bc = bc; pa.bd = bd; pa.batch = batch; pa.sg_ne = sg_ne; pa.sg_n0 = sg_n0;
-    pa.flag_S = 0.5f * a.flag_S;
+    pa.flag_S = 0.5f * a.flag_S; pa.flag_T = 0.0f;
     const int64_t n_sl = geo.npix * batch;
     const int64_t stride = (n_sl / 8192) | 1;
     const int64_t n_pilot = (n_sl + stride - 1) / stride;
