@@ -288,16 +288,17 @@ def time_config(sx, torch, w, steps, warmup, flush_buf, want_e2e=True, pix_range
                launches=int(l1 - l0), escalated=plan.stats()["escalated"],
                timing={"forward_ms": stat(tf), "vjp_ms": stat(tv), "step_ms": stat(tf + tv)})
     if not reduce_grad:
-        # The adjoint of a step reuses one float64 per sightline that the step's own forward stored (its Faraday total: the
-        # backward sweep needs it first).  For the record, the same adjoint WITHOUT that residual (own pre-pass), a few calls:
-        plan.set_option("use_forward_totals", 0)
+        # The adjoint of a step reuses what the step's own forward stored (Faraday totals, tile bases).  For the record, the same
+        # adjoint on its own: the stored values are dropped before every call (setting the option does that), so each call
+        # runs its Faraday-only pass first (long multi-frequency calls), the forward-order kernel (one frequency), or its
+        # in-kernel pre-pass (small calls).  A few calls, no synchronisation between them.
         ea = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(1 + min(steps, 5))]
-        for e in ea:   # no synchronisation between the calls: as in the timed steps, the stream-ordered pool keeps its blocks
+        for e in ea:
+            plan.set_option("use_forward_totals", 1)
             e[0].record(stream); sx.vjp(plan, model, params, *cots, out=grad); e[1].record(stream)
             flush_buf.add_(1.0)
         torch.cuda.synchronize()
         ts = [e[0].elapsed_time(e[1]) for e in ea[1:]]
-        plan.set_option("use_forward_totals", 1)
         res["timing"]["vjp_standalone_ms"] = {"mean": float(np.mean(ts)), "median": float(np.median(ts)), "best": float(np.min(ts))}
     if f64 and w.kind != "grid_b" and not reduce_grad:
         # the paper's own arithmetic (float64 throughout): synax_forward_f64 / synax_vjp_f64 on float64 buffers
@@ -528,7 +529,7 @@ def run_ours(args):
             "forward_samples_per_s": total / t_fwd, "vjp_samples_per_s": total / t_vjp,
             "ms_forward": 1e3 * t_fwd, "ms_vjp": 1e3 * t_vjp,
             "timing": r["timing"],          # per timed step on this rank: mean / median / best, ms; vjp_standalone_ms = the
-                                            # adjoint without the Faraday totals its step's forward stores (own pre-pass)
+                                            # adjoint on its own (nothing stored by a forward: Faraday-only pass or pre-pass first)
             "sample_freq_per_s": total * w.n_freq / t_step,
             "e2e": {"value": total / t_e2e, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"],
                     "ms_per_step": 1e3 * t_e2e,

@@ -121,7 +121,8 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).  Heuristic: one thread per sightline from 150,000
  * sightlines (npix x batch) in synax_forward, from 300,000 in a stand-alone synax_vjp and the float64 entry points, and from
  * 24,576 in a synax_vjp that finds the Faraday sums of the plan's last forward; 8 lanes down to an eighth of that, else 32.
- * key "use_forward_totals": 1 (default) = synax_vjp may take the sightlines' Faraday sums from what the plan's last
+ * key "use_forward_totals" (setting it, to either value, also drops what the plan has stored): 1 (default) = synax_vjp may
+ * take the sightlines' Faraday sums from what the plan's last
  * synax_forward stored (see synax_vjp); 0 = it always recomputes them in its own pre-pass.
  * key "batch_share": parameter vectors integrated per thread when a batch of analytic models is evaluated at one
  * frequency with one thread per sightline -- they share the sightline geometry (0 = heuristic, else 1, 2 or 4).  In
@@ -155,8 +156,14 @@ synax_status synax_forward(const synax_plan* plan, const synax_model* model, con
  * DISC4 / GRID_B: `aux` values are constants (not differentiated).
  * The adjoint sweeps every sightline from its far end to the observer and needs the sightline's Faraday sum first: it takes
  * the sums the plan's last synax_forward stored when that call had the same model, batch, options and integration extent and
- * `params` holds bit-identical values (compared on the device, no synchronisation), and otherwise recomputes them in a
- * pre-pass (+30-50 % work).  With the forward's tile-wise Faraday depths it also needs no float64 Faraday chain of its own.
+ * `params` holds bit-identical values (compared on the device, no synchronisation).  With the forward's tile-wise Faraday
+ * depths it also needs no float64 Faraday chain of its own.  Otherwise: when the plan holds nothing for this model, batch,
+ * options and extent (no forward yet, or settings changed) and the call is long (>= 24,576 sightlines, >= 5e7 LoS samples,
+ * several frequencies or STACK16 / UNIFORM), the call first runs a Faraday-only pass of the forward (its strategy and
+ * kernels without emission, rotation and maps: about half a forward) and stores the same sums itself -- the plan then holds
+ * them for later calls with these parameters; at one frequency (DISC4 / FULL16, one thread per sightline) a forward-order
+ * kernel runs that needs no sums; in all other cases (short calls; stored sums that turn out on the device to belong to
+ * other parameter values) the sums come from a pre-pass inside the adjoint kernel (+30-70 % work).
  * Results do not depend on the route beyond rounding (both are held to the same bound against the oracle).
  * Ordering: all work is ordered with `cuda_stream` (results are complete when the stream reaches the end of the
  * call).  Long calls (>= 262,144 sightlines) may run part of their kernels on a second stream owned by the plan,

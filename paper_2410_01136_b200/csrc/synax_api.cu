@@ -243,6 +243,7 @@ extern "C" synax_status synax_plan_set_option(synax_plan* plan, const char* key,
   } else if (!std::strcmp(key, "use_forward_totals")) {
     if (value != 0 && value != 1) return fail(SYNAX_ERR_INVALID_ARG, "use_forward_totals must be 0 or 1");
     plan->no_forward_totals = value == 0 ? 1 : 0;
+    plan->phi_stamp.valid = 0;   // setting the option (to either value) also drops what the plan has stored
   } else if (!std::strcmp(key, "batch_share")) {
     if (value != 0 && value != 1 && value != 2 && value != 4) return fail(SYNAX_ERR_INVALID_ARG, "batch_share must be 0, 1, 2 or 4");
     plan->batch_share = (int)value;
@@ -487,14 +488,17 @@ static bool phi_buffers(const synax_plan* plan, const synax_model* model, int ba
   return true;
 }
 
-extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
-                                      int32_t batch, float* I, float* Q, float* U, void* cuda_stream) {
-  int code = 0;
-  synax_status stt = check_model(plan, model, params, batch, &code);
-  if (stt != SYNAX_OK) return stt;
-  if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+// The forward.  faraday_only: the pass the adjoint runs when the plan holds no Faraday totals for these parameters -- the
+// same strategy (pilot, the two chains, lists) with kernels that integrate the Faraday depth alone (NF = 0 instantiations: no
+// emission, no rotation, no maps) and leave every sightline's total, the tile bases of the float64-chain sightlines and the
+// stamp behind, exactly as a forward would; *stored says whether they are there afterwards.
+static synax_status forward_core(const synax_plan* plan, const synax_model* model, int code, const float* params,
+                                 int32_t batch, float* I, float* Q, float* U, cudaStream_t st, bool faraday_only, bool* stored) {
+  synax_status stt = SYNAX_OK;
+  if (stored) *stored = false;
   const int64_t n_sl = plan->npix * batch;
+  if (faraday_only && !(code != kGridB && pick_lanes(plan, n_sl, kOneLaneFromStored) == 1 && phi_buffers(plan, model, batch, st)))
+    return SYNAX_OK;   // nowhere to put them (small call, lanes forced, gridded n_e, capture without buffers)
   StreamScratch scratch(st);
 
   BatchConsts* bc = nullptr;
@@ -577,6 +581,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
   // known only on the device): persistent grid, groups stride over the list.
   // Split mode: the list is long (2-85 % of the sightlines), so it takes the lane count of the full pass and a grid
   // sized for all sightlines (CTAs past the list's end exit at once).
+  const int n_freq_run = faraday_only ? 1 : plan->n_freq;   // Faraday-only: one pass over "zero frequencies"
   auto blocks_for = [&](int lanes, bool use_list, int run_when) {
     const int64_t full = (n_sl * lanes + kBlockD - 1) / kBlockD;
     return (unsigned)(use_list && run_when != 3 ? std::min<int64_t>(full, (int64_t)sms * 16 * 128 / kBlockD) : full);
@@ -585,12 +590,12 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     ForwardArgs pa = a;
     pa.run_when = run_when;
     pa.flag_list = list; pa.flag_count = count;
-    for (int f0 = 0; f0 < plan->n_freq;) {
-      const int nf = next_freq_block(plan->n_freq - f0);
+    for (int f0 = 0; f0 < n_freq_run;) {
+      const int nf = faraday_only ? 0 : next_freq_block(plan->n_freq - f0);
       pa.f0 = f0;
       SYNAX_DISPATCH_CODE(code, fwd_launch_f64, lanes, nf, blocks_for(lanes, list != nullptr, run_when), on, pa, plan->ft);
       plan->launches++;
-      f0 += nf;
+      f0 += faraday_only ? 1 : nf;
     }
   };
   cudaError_t stream_err = cudaSuccess;
@@ -604,8 +609,8 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
       if (stream_err != cudaSuccess) return fail(SYNAX_ERR_CUDA, "forward: stream fork failed: %s", cudaGetErrorString(stream_err));
       run_f64(plan->aux, G, 3, a.flag_list, ctrl + kCtrlFlagCount);
     }
-    for (int f0 = 0; f0 < plan->n_freq;) {
-      const int nf = next_freq_block(plan->n_freq - f0);
+    for (int f0 = 0; f0 < n_freq_run;) {
+      const int nf = faraday_only ? 0 : next_freq_block(plan->n_freq - f0);
       a.f0 = f0;
       // batches of parameter vectors on modest maps: NB vectors per thread share the sightline geometry (A12)
       const int nb = plan->batch_share ? plan->batch_share : (batch >= 4 ? 4 : (batch >= 2 ? 2 : 1));
@@ -621,7 +626,7 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
         SYNAX_DISPATCH_CODE(code, fwd_launch_fast, true, G, nf, n_sl, st, al, plan->ft);
         plan->launches++;
       }
-      f0 += nf;
+      f0 += faraday_only ? 1 : nf;
     }
     if (escalate) run_f64(st, 8, piloted ? 1 : 0, a.flag_list, ctrl + kCtrlFlagCount);   // fast-then-list: the flagged list, 8 lanes per sightline
     if (split_ok) {
@@ -647,8 +652,18 @@ extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model*
     const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
     std::memcpy(&plan->phi_stamp, &now, sizeof(now));   // byte copy: the stamp is compared with memcmp
     plan->phi_has_bases = keep_base ? 1 : 0;
+    if (stored) *stored = true;
   }
   return SYNAX_OK;
+}
+
+extern "C" synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
+                                      int32_t batch, float* I, float* Q, float* U, void* cuda_stream) {
+  int code = 0;
+  synax_status stt = check_model(plan, model, params, batch, &code);
+  if (stt != SYNAX_OK) return stt;
+  if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
+  return forward_core(plan, model, code, params, batch, I, Q, U, (cudaStream_t)cuda_stream, false, nullptr);
 }
 
 extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* model, const float* params,
@@ -670,10 +685,28 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   const double* phi_base = nullptr;
   const unsigned char* phi_has = nullptr;
   int G = pick_lanes(plan, plan->npix * batch);
-  if (code != kGridB && !plan->no_forward_totals && plan->phi_stamp.valid && !model->ne_grid &&
+  if (code != kGridB && !plan->no_forward_totals && !model->ne_grid &&
       pick_lanes(plan, plan->npix * batch, kOneLaneFromStored) == 1) {
-    const synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
-    if (std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0) {
+    synax_plan::PhiStamp now = make_phi_stamp(plan, model, code, batch);
+    bool have = plan->phi_stamp.valid && std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0;
+    // Nothing stored for this plan and these settings (a stand-alone adjoint): a Faraday-only pass with the forward's own
+    // strategy leaves the totals and tile bases behind first, and the lean one-thread kernel then does every sightline --
+    // instead of a pre-pass inside the adjoint kernel plus its float64-angle variants (cfg 4: 20.9 -> see DESIGN.md section 5).
+    // Not where the forward-order kernel runs anyway (one frequency, DISC4 / FULL16, one thread per sightline: no totals needed).
+    const bool forward_order = G == 1 && plan->n_freq == 1 && (code == kAnalyticDisc || code == kAnalyticFull) &&
+                               !model->n0_grid && batch <= 65535;
+    // ... nor for calls so short that the pass's dozen launches show (cfg 1: 0.28 against 0.24 ms)
+    const bool long_call = plan->npix * batch * (int64_t)plan->n_los >= kSplitFromSamples;
+    if (!have && !forward_order && long_call) {
+      bool stored = false;
+      stt = forward_core(plan, model, code, params, batch, nullptr, nullptr, nullptr, st, true, &stored);
+      if (stt != SYNAX_OK) return stt;
+      if (stored) {
+        now = make_phi_stamp(plan, model, code, batch);
+        have = plan->phi_stamp.valid && std::memcmp(&now, &plan->phi_stamp, sizeof(now)) == 0;
+      }
+    }
+    if (have) {
       G = 1;
       phi_validate_kernel<<<1, 256, 0, st>>>(params, plan->phi_params, (int64_t)batch * model->n_params, plan->d_phi_ok);
       plan->launches++;

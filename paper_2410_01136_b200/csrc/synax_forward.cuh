@@ -184,6 +184,7 @@ template <int CODE, int G, int NF, bool LIST>
 __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__ ForwardArgs A,
                                                          const __grid_constant__ FreqTab ft) {
   if (LIST ? (*A.mode != kModeSplit) : (A.mode && *A.mode != kModeFastThenList)) return;
+  constexpr int NFA = NF > 0 ? NF : 1;   // NF = 0: the adjoint's Faraday-only pass (totals and flags, no maps)
   const int64_t tid = (int64_t)blockIdx.x * kBlock + threadIdx.x;
   const int g = (int)(tid % G);
   int64_t sl = tid / G;
@@ -205,11 +206,11 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
   PosF pf;
   pf.init(delta, n0);
 
-  float k_rad[NF];
+  float k_rad[NFA];
 #pragma unroll
   for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[f];
 
-  float accI = 0.0f, accQ[NF], accU[NF];
+  float accI = 0.0f, accQ[NFA], accU[NFA];
 #pragma unroll
   for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
   double carry = 0.0;            // chunk-local sum of n_e B_LOS over finished tiles
@@ -219,7 +220,7 @@ __global__ void __launch_bounds__(kBlock) forward_kernel(const __grid_constant__
   for (int ts = n0; ts < n1; ts += kTile) {
     const int te = min(ts + kTile, n1);
     float hi = 0.0f, lo = 0.0f;  // tile-local two-float sum of n_e B_LOS
-    float tq[NF], tu[NF];
+    float tq[NFA], tu[NFA];
 #pragma unroll
     for (int f = 0; f < NF; ++f) { tq[f] = 0.0f; tu[f] = 0.0f; }
     for (int n = ts; n < te; ++n) {
@@ -439,6 +440,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
   const int g = (int)(tid % G);
   const int64_t n_groups = ((int64_t)gridDim.x * kBlockD) / G;
   const int64_t n_sl = A.geo.npix * A.batch;
+  constexpr int NFA = NF > 0 ? NF : 1;   // NF = 0: the adjoint's Faraday-only pass
   if (A.run_when == 1 && *A.mode != kModeFastThenList) return;
   if (A.run_when == 2 && *A.mode != kModeAllF64) return;
   if (A.run_when == 3 && *A.mode == kModeFastThenList) return;
@@ -449,7 +451,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
   const int n0 = g * C;
   const int n1 = min(n0 + C, A.geo.n_los);
   const double delta0 = A.geo.delta;
-  float k_rad[NF];
+  float k_rad[NFA];
 #pragma unroll
   for (int f = 0; f < NF; ++f) k_rad[f] = ft.k_rad[f];
 
@@ -465,7 +467,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
     const Triad T = load_triad(A.geo, pix);
     const double delta = delta0 * T.scale;
     double s_d = ((double)n0 + 0.5) * delta;
-    float accI = 0.0f, accQ[NF], accU[NF];
+    float accI = 0.0f, accQ[NFA], accU[NFA];
 #pragma unroll
     for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
     double S_loc = 0.0;      // sum of n_e B_LOS over this lane's finished samples
@@ -477,7 +479,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
       // two long, from sample 0) start on those samples.  Several lanes: see the sample loop.
       if (G == 1 && A.phi_base && A.f0 == 0 && valid && (ts & 31) == 0 && ts > 0)
         A.phi_base[(size_t)(ts >> 5) * (size_t)n_sl + sl] = S_loc;
-      float tq[NF], tu[NF];
+      float tq[NFA], tu[NFA];
 #pragma unroll
       for (int f = 0; f < NF; ++f) { tq[f] = 0.0f; tu[f] = 0.0f; }
       for (int n = ts; n < te; n += kUnrollD) {

@@ -18,6 +18,7 @@ template <int CODE, int G, bool LIST>
 static void launch_forward_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
+    case 0: forward_kernel<CODE, G, 0, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;   // Faraday-only pass (synax_vjp)
     case 1: forward_kernel<CODE, G, 1, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
     case 2: forward_kernel<CODE, G, 2, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
     case 3: forward_kernel<CODE, G, 3, LIST><<<blocks, kBlock, 0, st>>>(a, ft); break;
@@ -53,6 +54,7 @@ template <int CODE, int G>
 static void launch_f64_nf(int nf, unsigned blocks, cudaStream_t st, const ForwardArgs& a, const FreqTab& ft0) {
   const FreqTab ft = shift_freqs(ft0, a.f0);
   switch (nf) {
+    case 0: forward_f64_kernel<CODE, G, 0><<<blocks, kBlockD, 0, st>>>(a, ft); break;
     case 1: forward_f64_kernel<CODE, G, 1><<<blocks, kBlockD, 0, st>>>(a, ft); break;
     case 2: forward_f64_kernel<CODE, G, 2><<<blocks, kBlockD, 0, st>>>(a, ft); break;
     case 3: forward_f64_kernel<CODE, G, 3><<<blocks, kBlockD, 0, st>>>(a, ft); break;
