@@ -49,8 +49,6 @@ def test_random_full16_long_calls_sampled_pixels(seed):
     w = _draw_large(seed)
     pix = np.arange(seed % 89, w.npix, 89)
     plan, model, params = parity.gpu_objects(w)
-    maps = tuple(t.cpu().numpy().astype(np.float64) for t in sx.forward(plan, model, params))
-    parity.assert_maps_close(tuple(m[..., pix] for m in maps), parity.oracle_forward(w, pix=pix), what=w.name)
     full = w.cotangents()
     cots = tuple(np.zeros_like(c) for c in full)
     for c, f in zip(cots, full):
@@ -58,10 +56,15 @@ def test_random_full16_long_calls_sampled_pixels(seed):
     ref = parity.oracle_vjp(w, tuple(np.ascontiguousarray(c[..., pix]) for c in cots), pix=pix)[0]
     d = [torch.from_numpy(c).cuda() for c in cots]
     th = w.params[0].astype(np.float64)
+    # before any forward of this plan: the adjoint's own Faraday-only pass (draws with >= 5e7 samples), else its pre-pass
+    ga = sx.vjp(plan, model, params, *d).cpu().numpy().astype(np.float64)[0]
+    parity.assert_log_gradient_close(ga, ref, th, what=w.name + " (nothing stored)")
+    maps = tuple(t.cpu().numpy().astype(np.float64) for t in sx.forward(plan, model, params))
+    parity.assert_maps_close(tuple(m[..., pix] for m in maps), parity.oracle_forward(w, pix=pix), what=w.name)
     # after the forward of the same plan: the adjoint on the stored Faraday totals / tile bases ...
     g = sx.vjp(plan, model, params, *d).cpu().numpy().astype(np.float64)[0]
     parity.assert_log_gradient_close(g, ref, th, what=w.name + " (after forward)")
-    # ... and on its own (pre-pass, float64-angle variants)
+    # ... and with the stored values switched off (in-kernel pre-pass, float64-angle variants)
     plan.set_option("use_forward_totals", 0)
     g0 = sx.vjp(plan, model, params, *d).cpu().numpy().astype(np.float64)[0]
     parity.assert_log_gradient_close(g0, ref, th, what=w.name + " (stand-alone)")
