@@ -70,13 +70,14 @@ typedef struct {
   int32_t n_params; /* 4, 16, nx*ny*nz*3 (<2^31), 6, 16 -- must match kind */
   const float* aux; /* HOST. DISC4 / GRID_B / STACK16: {C0, h_r, h_z, alpha, ne0, h_er, h_ez}; else NULL */
   int32_t nx, ny, nz; /* GRID_B only, each >= 2 */
-  float lx, ly, lz;   /* GRID_B only, kpc, > 0 */
+  double lx, ly, lz;  /* GRID_B only, kpc, > 0 (float64: a length rounded to fp32 rescales the grid by up to 6e-8, which
+                       * is 1e-3 rad of Faraday rotation at 350 MHz through a strong field) */
   /* Optional gridded scalar fields (the paper's n_e is the YMW16 model on a (256,256,64) grid):
    * DEVICE fp32 [n][n][n] (z fastest), nodes on the faces of a box of lengths *_l centred on the Galactic centre,
    * trilinear, zero outside.  DISC4 and GRID_B only; a non-NULL grid REPLACES the analytic disc built from `aux`
    * (its aux entries are then ignored).  Not differentiated.  NULL (and zeroed sizes) = unused. */
-  const float* ne_grid; int32_t ne_n[3]; float ne_l[3];
-  const float* n0_grid; int32_t n0_n[3]; float n0_l[3];
+  const float* ne_grid; int32_t ne_n[3]; double ne_l[3];
+  const float* n0_grid; int32_t n0_n[3]; double n0_l[3];
 } synax_model;
 
 /* Plan = geometry shared by all calls: HEALPix nside (1..8192), samples per sightline n_los

@@ -32,9 +32,9 @@ class SynaxError(RuntimeError):
 class _CModel(ctypes.Structure):
     _fields_ = [("kind", ctypes.c_int32), ("n_params", ctypes.c_int32), ("aux", ctypes.POINTER(ctypes.c_float)),
                 ("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("nz", ctypes.c_int32),
-                ("lx", ctypes.c_float), ("ly", ctypes.c_float), ("lz", ctypes.c_float),
-                ("ne_grid", ctypes.c_void_p), ("ne_n", ctypes.c_int32 * 3), ("ne_l", ctypes.c_float * 3),
-                ("n0_grid", ctypes.c_void_p), ("n0_n", ctypes.c_int32 * 3), ("n0_l", ctypes.c_float * 3)]
+                ("lx", ctypes.c_double), ("ly", ctypes.c_double), ("lz", ctypes.c_double),
+                ("ne_grid", ctypes.c_void_p), ("ne_n", ctypes.c_int32 * 3), ("ne_l", ctypes.c_double * 3),
+                ("n0_grid", ctypes.c_void_p), ("n0_n", ctypes.c_int32 * 3), ("n0_l", ctypes.c_double * 3)]
 
 
 _lib = None

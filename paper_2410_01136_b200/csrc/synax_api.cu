@@ -316,22 +316,22 @@ static synax_status check_model(const synax_plan* plan, const synax_model* m, co
   if ((int64_t)batch * plan->npix >= (1LL << 31)) return fail(SYNAX_ERR_INVALID_ARG, "batch * npix must be < 2^31");
   const float* sg[2] = {m->ne_grid, m->n0_grid};
   const int32_t* sn[2] = {m->ne_n, m->n0_n};
-  const float* sl[2] = {m->ne_l, m->n0_l};
+  const double* sl[2] = {m->ne_l, m->n0_l};
   for (int k = 0; k < 2; ++k) {
     if (!sg[k]) continue;
     if (m->kind != SYNAX_MODEL_DISC4 && m->kind != SYNAX_MODEL_GRID_B && m->kind != SYNAX_MODEL_STACK16)
       return fail(SYNAX_ERR_INVALID_ARG, "gridded n_e / N_0 need a DISC4, STACK16 or GRID_B model");
     for (int a = 0; a < 3; ++a)
-      if (sn[k][a] < 2 || !(sl[k][a] > 0.0f)) return fail(SYNAX_ERR_INVALID_ARG, "scalar grid dims must be >= 2 and box lengths > 0");
+      if (sn[k][a] < 2 || !(sl[k][a] > 0.0)) return fail(SYNAX_ERR_INVALID_ARG, "scalar grid dims must be >= 2 and box lengths > 0");
   }
   return SYNAX_OK;
 }
 
-static ScalarGridDesc make_scalar_desc(const float* g, const int32_t n[3], const float l[3]) {
+static ScalarGridDesc make_scalar_desc(const float* g, const int32_t n[3], const double l[3]) {
   ScalarGridDesc d;
   d.g = g; d.nx = g ? n[0] : 2; d.ny = g ? n[1] : 2; d.nz = g ? n[2] : 2;
-  d.sx = g ? (double)(n[0] - 1) / (double)l[0] : 0.0; d.sy = g ? (double)(n[1] - 1) / (double)l[1] : 0.0;
-  d.sz = g ? (double)(n[2] - 1) / (double)l[2] : 0.0;
+  d.sx = g ? (double)(n[0] - 1) / l[0] : 0.0; d.sy = g ? (double)(n[1] - 1) / l[1] : 0.0;
+  d.sz = g ? (double)(n[2] - 1) / l[2] : 0.0;
   d.bx = 0.5 * (double)(d.nx - 1); d.by = 0.5 * (double)(d.ny - 1); d.bz = 0.5 * (double)(d.nz - 1);
   return d;
 }

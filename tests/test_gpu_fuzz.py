@@ -130,3 +130,41 @@ def test_random_mid_size_sparse_cotangents(seed):
     parity.assert_maps_close(tuple(m[..., pix] for m in maps), parity.oracle_forward(w, pix=pix), what=w.name)
     parity.assert_log_gradient_close(g_alone, ref, th, what=w.name + " (stand-alone)")
     parity.assert_log_gradient_close(g_after, ref, th, what=w.name + " (after forward)")
+
+
+def _draw_grid(seed):
+    """GRID_B: non-cubic grids over boxes of arbitrary float64 lengths, a random field of 0.3-3 x cfg 3's amplitude on a spiral,
+    n_e x 0.5-3, alpha 3 or random, 1-9 frequencies from 0.3 (or 1) GHz, nside 8-48, 40-900 samples."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    shape = (int(rng.choice([24, 32, 48, 64, 96])), int(rng.choice([24, 32, 48, 64, 96])), int(rng.choice([8, 12, 16, 32])))
+    box = (float(rng.uniform(24, 44)), float(rng.uniform(24, 44)), float(rng.uniform(4, 12)))
+    X, Y, Z = wl.grid_nodes(shape, box)
+    amp = float(rng.uniform(0.3, 3.0))
+    g = amp * wl.gaussian_random_field(shape, box, seed) + wl.spiral_pattern(X, Y, Z, *wl.DISC4_NOMINAL) * float(rng.uniform(0.5, 2.0))
+    nside = int(rng.choice([8, 16, 24, 32, 48]))
+    n_los = int(rng.integers(40, 900))
+    nf = int(rng.integers(1, 10))
+    freqs = np.sort(np.exp(rng.uniform(np.log(rng.choice([0.3e9, 1e9])), np.log(30e9), nf)))
+    aux = wl.AUX_NOMINAL.astype(np.float32).copy()
+    aux[4] *= float(rng.uniform(0.5, 3.0))
+    aux[3] = float(rng.choice([3.0, rng.uniform(2.5, 3.3)]))
+    w = wl.Workload(f"grid{seed}", "grid_b", nside, n_los, float(rng.uniform(15, 30)), freqs, g.astype(np.float32), aux, box=box,
+                    cot_seed=seed)
+    if rng.random() < 0.25:
+        w.clip_box = box
+    return w
+
+
+# 8020, 8040: 32 x 64 x 16 and 96 x 24 x 16 nodes over 29.77 x 41.70 x 4.51 and 33.95 x 27.05 x 6.38 kpc at 0.35 / 0.43 GHz -- while
+# synax_model carried the box lengths as fp32 the grid was rescaled by ~3e-8 and Q, U were off by 1e-3 x RMS there
+@pytest.mark.parametrize("seed", [8003, 8016, 8020, 8022, 8040, 8048])
+def test_random_gridded_b(seed):
+    w = _draw_grid(seed)
+    maps, _ = parity.gpu_forward(w)
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=w.name)
+    cots = w.cotangents()
+    g, ref = parity.gpu_vjp(w, cots), parity.oracle_vjp(w, cots)
+    rms = np.sqrt(np.mean(ref * ref))
+    bad = np.abs(g - ref) > parity.GRAD_TOL * np.abs(ref) + 1.0e-4 * rms          # C-2#14, as tests/test_gpu_parity.py
+    assert not bad.any(), (w.name, int(bad.sum()), float(np.abs(g - ref).max() / rms))
+    assert np.array_equal(ref == 0.0, g == 0.0)
