@@ -535,7 +535,8 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
           // the lanes add their offset below
           if (G > 1 && A.phi_base && A.f0 == 0 && live[j] && valid && ((n + j) & 31) == 0 && n + j > 0)
             A.phi_base[(size_t)((n + j) >> 5) * (size_t)n_sl + sl] = S_loc;
-          const float ph = (float)fma(0.5, gn, S_loc - S_tile);                  // half-cell (S:C-2#5), tile-local
+          const double phd = fma(0.5, gn, S_loc - S_tile);                       // half-cell (S:C-2#5), tile-local
+          const float ph = (float)phd;
           S_loc += gn;
           const float bx = (float)Bx[j], by = (float)By[j], bz = (float)Bz[j];
           const float BN = fmaf(bx, T.eNx, fmaf(by, T.eNy, bz * T.eNz));
@@ -543,12 +544,26 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
           float eI, a, bq;
           emission(P, BN, BE, live[j] ? N0[j] : 0.0f, eI, a, bq);
           accI += eI;
+          if (tile == 1) {
+            // under-resolved (one sample already turns by more than 24 rad at the lowest frequency): the half-cell angle is
+            // reduced to turns in float64 for every frequency instead of being formed in fp32
 #pragma unroll
-          for (int f = 0; f < NF; ++f) {
-            const float th = k_rad[f] * ph;
-            const float c = mufu_cos(th), s = mufu_sin(th);
-            tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
-            tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+            for (int f = 0; f < NF; ++f) {
+              double t = ft.k_turn[f] * phd;
+              t -= rint(t);
+              const float th = (float)t * 6.283185307179586f;
+              const float c = mufu_cos(th), s = mufu_sin(th);
+              tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
+              tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+            }
+          } else {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) {
+              const float th = k_rad[f] * ph;
+              const float c = mufu_cos(th), s = mufu_sin(th);
+              tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
+              tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
+            }
           }
         }
       }

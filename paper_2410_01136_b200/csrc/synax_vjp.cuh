@@ -583,9 +583,11 @@ __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MIN
       const float a = M * d2, bq = M * p2;
       // Faraday phase of this sample relative to the far end of the tile: -(sum after it within the tile + g_n / 2)
       float ph;
+      double phd = 0.0;   // the same in float64 (float64-chain sightlines)
       if (PMODE != 0 && prec) {
         const double gd = faraday_term_d<CODE>(P, D, T, A.sg_ne, xd, yd, zd);
-        ph = -(float)fma(0.5, gd, dl);
+        phd = -fma(0.5, gd, dl);
+        ph = (float)phd;
         dl += gd;
       } else {
         const float gn = S.ne * S.Bpar;
@@ -598,7 +600,12 @@ __global__ void __launch_bounds__(kBlock, (PMODE == 0 && G == 1 && SYNAX_VJP_MIN
       float Xc = 0.f, Xs = 0.f, Yc = 0.f, Ys = 0.f, Zc = 0.f, Zs = 0.f;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        const float th = ft.k_rad[f] * ph;
+        float th = ft.k_rad[f] * ph;
+        if (PMODE != 0 && prec && tile == 1) {   // under-resolved: one sample turns by more than 24 rad at the lowest frequency --
+          double t = ft.k_turn[f] * phd;          // its half-cell angle is reduced to turns in float64, not formed in fp32
+          t -= rint(t);
+          th = (float)t * 6.283185307179586f;
+        }
         const float c = mufu_cos(th), s = mufu_sin(th);
         const float u = fmaf(rq[f], c, ru[f] * s);
         const float v = fmaf(ru[f], c, -rq[f] * s);

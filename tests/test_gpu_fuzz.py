@@ -168,3 +168,75 @@ def test_random_gridded_b(seed):
     bad = np.abs(g - ref) > parity.GRAD_TOL * np.abs(ref) + 1.0e-4 * rms          # C-2#14, as tests/test_gpu_parity.py
     assert not bad.any(), (w.name, int(bad.sum()), float(np.abs(g - ref).max() / rms))
     assert np.array_equal(ref == 0.0, g == 0.0)
+
+
+def _draw_options(seed):
+    """Small maps with everything else random: model kind (UNIFORM included), batch 1-8, 1 / 2 / 3 / 31 ... 65 or up to 600 samples,
+    1-32 frequencies (every frequency-block split), box clip, gridded n_e / N_0, and the options lanes, precision, batch_share."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    kind = rng.choice(["full16", "disc4", "stack16", "uniform", "disc4"])
+    nside = int(rng.choice([1, 2, 3, 4, 8, 12, 16, 24, 32]))
+    batch = int(rng.choice([1, 1, 2, 3, 5, 8]))
+    n_los = int(rng.choice([1, 2, 3, 31, 32, 33, 63, 64, 65, int(rng.integers(66, 600))]))
+    nf = int(rng.choice([1, 2, 3, 4, 5, 7, 8, 9, 12, 13, 16, 17, 31, 32]))
+    freqs = np.sort(np.exp(rng.uniform(np.log(rng.choice([0.3e9, 1e9, 5e9])), np.log(40e9), nf)))
+    s_max = float(rng.uniform(10.0, 40.0))
+    aux = None
+    if kind == "full16":
+        p = wl.FULL16_NOMINAL * np.exp(rng.uniform(-np.log(1.4), np.log(1.4), (batch, 16)))
+        p[:, 12] = rng.uniform(2.5, 3.3, batch)
+        if rng.random() < 0.3:
+            p[:, 12] = 3.0
+    elif kind == "disc4":
+        p = wl.DISC4_NOMINAL * np.exp(rng.uniform(-np.log(1.4), np.log(1.4), (batch, 4)))
+        aux = wl.AUX_NOMINAL.astype(np.float32).copy()
+        if rng.random() < 0.5:
+            aux[3] = float(rng.uniform(2.5, 3.3))
+    elif kind == "stack16":
+        w0 = wl.stack16()
+        p = np.repeat(w0.params.astype(np.float64), batch, axis=0) * np.exp(rng.uniform(-0.2, 0.2, (batch, 16)))
+        aux = w0.aux
+    else:
+        w0 = wl.uniform_toy(bvec=(2.0, -3.0, 1.5))
+        p = np.repeat(w0.params.astype(np.float64), batch, axis=0) * np.exp(rng.uniform(-0.3, 0.3, (batch, w0.params.shape[1])))
+        if rng.random() < 0.5:
+            p[:, 5] = rng.uniform(2.5, 3.3, batch)
+        aux = w0.aux
+    w = wl.Workload(f"opt{seed}_{kind}", kind, nside, n_los, s_max, freqs, p.astype(np.float32), aux, cot_seed=seed)
+    if rng.random() < 0.3:
+        w.clip_box = (float(rng.uniform(30, 50)), float(rng.uniform(30, 50)), float(rng.uniform(6, 14)))
+    if kind in ("disc4", "stack16") and rng.random() < 0.4:
+        shp = (int(rng.choice([8, 16, 24])), int(rng.choice([8, 16, 24])), int(rng.choice([4, 8, 12])))
+        bx = (float(rng.uniform(30, 50)), float(rng.uniform(30, 50)), float(rng.uniform(6, 14)))
+        w.ne_grid, w.ne_box = wl.clumpy_disc_grid(shp, bx, 0.03 * float(rng.uniform(0.5, 2)), 20.0, 1.0, seed=seed), bx
+        if rng.random() < 0.5:
+            w.n0_grid, w.n0_box = wl.clumpy_disc_grid(shp, bx, 2.1e-4, 5.0, 1.0, seed=seed + 1), bx
+    opts = {}
+    if rng.random() < 0.5:
+        opts["lanes"] = int(rng.choice([1, 8, 32]))
+    if rng.random() < 0.25:
+        opts["precision"] = 2
+    if rng.random() < 0.3:
+        opts["batch_share"] = int(rng.choice([1, 2, 4]))
+    return w, opts
+
+
+# 9176 ... 9284: one to three samples per sightline at 0.3-1 GHz -- a single sample turns Q, U by thousands of radians; before the
+# float64 chains reduced that half-cell angle to turns in float64 (tile length 1) these were off by up to 8e-3 x RMS
+@pytest.mark.parametrize("seed", [9001, 9002, 9003, 9010, 9176, 9180, 9205, 9237, 9240, 9265, 9266, 9272, 9282, 9284])
+def test_random_options_and_degenerate_sampling(seed):
+    import torch
+    import paper_2410_01136_b200 as sx
+    w, opts = _draw_options(seed)
+    plan, model, params = parity.gpu_objects(w, **opts)
+    cots_h = w.cotangents()
+    d = [torch.from_numpy(c).cuda() for c in cots_h]
+    th = w.params.astype(np.float64)
+    g_alone = sx.vjp(plan, model, params, *d).cpu().numpy().astype(np.float64)
+    maps = tuple(t.cpu().numpy().astype(np.float64) for t in sx.forward(plan, model, params))
+    g_after = sx.vjp(plan, model, params, *d).cpu().numpy().astype(np.float64)
+    plan.close()
+    parity.assert_maps_close(maps, parity.oracle_forward(w), what=f"{w.name} {opts}")
+    ref = parity.oracle_vjp(w, cots_h)
+    parity.assert_log_gradient_close(g_alone, ref, th, what=f"{w.name} {opts} (stand-alone)")
+    parity.assert_log_gradient_close(g_after, ref, th, what=f"{w.name} {opts} (after forward)")
