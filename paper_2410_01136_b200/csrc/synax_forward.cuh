@@ -349,10 +349,11 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
   pf.init(delta, 0);
   const float k_rad = ft.k_rad[0];
 
-  float accI[NB], accQ[NB], accU[NB], gabs[NB], tmax[NB];
+  float accI[NB], accQ[NB], accU[NB], gabs[NB];
+  float tmax = 0.f;   // largest |tile-local Faraday sum| of the NB vectors together (one register; flags all NB when it fires)
   double carry[NB];
 #pragma unroll
-  for (int j = 0; j < NB; ++j) { accI[j] = 0.f; accQ[j] = 0.f; accU[j] = 0.f; gabs[j] = 0.f; tmax[j] = 0.f; carry[j] = 0.0; }
+  for (int j = 0; j < NB; ++j) { accI[j] = 0.f; accQ[j] = 0.f; accU[j] = 0.f; gabs[j] = 0.f; carry[j] = 0.0; }
   for (int ts = 0; ts < A.geo.n_los; ts += kTile) {
     const int te = min(ts + kTile, A.geo.n_los);
     float hi[NB], lo[NB], tq[NB], tu[NB];
@@ -399,7 +400,7 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
         accQ[j] += tq[j]; accU[j] += tu[j];
       }
       carry[j] += (double)hi[j] + (double)lo[j];
-      tmax[j] = fmaxf(tmax[j], fabsf(hi[j]));
+      tmax = fmaxf(tmax, fabsf(hi[j]));
     }
   }
 #pragma unroll
@@ -412,7 +413,7 @@ __global__ void __launch_bounds__(kBlock) forward_batched_kernel(const __grid_co
     A.U[o] = P.coefP[A.f0] * T.scalef * accU[j];
     if (A.f0 == 0 && A.phi) A.phi[(int64_t)bj[j] * A.geo.npix + pix] = carry[j];
     if (A.f0 == 0 && A.phi_has) A.phi_has[(int64_t)bj[j] * A.geo.npix + pix] = 0;
-    if (A.f0 == 0 && A.flag_S > 0.0f && (gabs[j] > A.flag_S || tmax[j] > A.flag_T)) {
+    if (A.f0 == 0 && A.flag_S > 0.0f && (gabs[j] > A.flag_S || tmax > A.flag_T)) {
       const int k = atomicAdd(A.append_count, 1);
       A.append_list[k] = (int)((int64_t)bj[j] * A.geo.npix + pix);
     }
@@ -472,6 +473,7 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
     for (int f = 0; f < NF; ++f) { accQ[f] = 0.0f; accU[f] = 0.0f; }
     double S_loc = 0.0;      // sum of n_e B_LOS over this lane's finished samples
     const int tile = P.tile_d;
+    const bool one_sample_tiles = tile == 1;
     for (int ts = n0; ts < n1; ts += tile) {
       const int te = min(ts + tile, n1);
       const double S_tile = S_loc;
@@ -535,8 +537,10 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
           // the lanes add their offset below
           if (G > 1 && A.phi_base && A.f0 == 0 && live[j] && valid && ((n + j) & 31) == 0 && n + j > 0)
             A.phi_base[(size_t)((n + j) >> 5) * (size_t)n_sl + sl] = S_loc;
-          const double phd = fma(0.5, gn, S_loc - S_tile);                       // half-cell (S:C-2#5), tile-local
-          const float ph = (float)phd;
+          // half-cell (S:C-2#5), tile-local.  Tile length 1 (under-resolved: one sample already turns by more than 24 rad at the
+          // lowest frequency): the half-cell angle joins the tile offset, which is reduced to turns in float64 below, instead
+          // of being formed in fp32 here -- two selects, the frequency loop stays as it is
+          const float ph = one_sample_tiles ? 0.0f : (float)fma(0.5, gn, S_loc - S_tile);
           S_loc += gn;
           const float bx = (float)Bx[j], by = (float)By[j], bz = (float)Bz[j];
           const float BN = fmaf(bx, T.eNx, fmaf(by, T.eNy, bz * T.eNz));
@@ -544,32 +548,20 @@ __global__ void __launch_bounds__(kBlockD, SYNAX_F64_MINB) forward_f64_kernel(co
           float eI, a, bq;
           emission(P, BN, BE, live[j] ? N0[j] : 0.0f, eI, a, bq);
           accI += eI;
-          if (tile == 1) {
-            // under-resolved (one sample already turns by more than 24 rad at the lowest frequency): the half-cell angle is
-            // reduced to turns in float64 for every frequency instead of being formed in fp32
 #pragma unroll
-            for (int f = 0; f < NF; ++f) {
-              double t = ft.k_turn[f] * phd;
-              t -= rint(t);
-              const float th = (float)t * 6.283185307179586f;
-              const float c = mufu_cos(th), s = mufu_sin(th);
-              tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
-              tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
-            }
-          } else {
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-              const float th = k_rad[f] * ph;
-              const float c = mufu_cos(th), s = mufu_sin(th);
-              tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
-              tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
-            }
+          for (int f = 0; f < NF; ++f) {
+            const float th = k_rad[f] * ph;
+            const float c = mufu_cos(th), s = mufu_sin(th);
+            tq[f] = fmaf(a, c, fmaf(-bq, s, tq[f]));
+            tu[f] = fmaf(a, s, fmaf(bq, c, tu[f]));
           }
         }
       }
+      // one-sample tiles: the sample's half-cell term g_n / 2 = (S_loc - S_tile) / 2 is rotated exactly with the tile offset
+      const double tile_off = one_sample_tiles ? 0.5 * (S_tile + S_loc) : S_tile;
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        rotate_by_offset(ft.k_turn[f], S_tile, tq[f], tu[f]);
+        rotate_by_offset(ft.k_turn[f], tile_off, tq[f], tu[f]);
         accQ[f] += tq[f]; accU[f] += tu[f];
       }
     }
