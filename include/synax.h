@@ -118,7 +118,8 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * chain -- as a redo of a flagged list after the fp32 pass, for every sightline when a device-side pilot finds most of
  * them flagged, or split between the two chains in between.  Auto, VJP: decided per sightline (per CTA in long calls)
  * -- those above escalate_rad take their Faraday angles from the float64 chain.
- * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0).
+ * No mode ever synchronises with the host.  key "escalate_rad": threshold in radians (> 0), for plans with n_los >= 128;
+ * below that the threshold in force is escalate_rad x n_los / 128 (a few samples per sightline average no rounding out).
  * key "lanes": lanes per sightline (0 = heuristic, else 1, 8 or 32).  Heuristic: one thread per sightline from 150,000
  * sightlines (npix x batch) in synax_forward, from 300,000 in a stand-alone synax_vjp and the float64 entry points, and from
  * 24,576 in a synax_vjp that finds the Faraday sums of the plan's last forward; 8 lanes down to an eighth of that, else 32.

@@ -343,6 +343,13 @@ static ScalarGridDesc make_scalar_desc(const float* g, const int32_t n[3], const
 #ifndef SYNAX_SPLIT_FROM
 #define SYNAX_SPLIT_FROM 50000000
 #endif
+// escalate_rad is tuned for sightlines of >= kFullThresholdFromSamples samples, where the fp32 rounding of the single angles
+// averages out over the sum; a sightline of a few samples has nothing to average (parity 1.0 .. 4.2e-4 x RMS at 1 .. 65
+// samples with the full threshold), so the threshold shrinks in proportion below that count.
+constexpr int kFullThresholdFromSamples = 128;
+static double escalate_at(const synax_plan* plan) {
+  return plan->escalate_rad * std::min(1.0, (double)plan->n_los / (double)kFullThresholdFromSamples);
+}
 constexpr double kTileAngleRad = 96.0;   // fp32 chain: largest rotation angle inside a tile before the sightline is redone in float64
 constexpr int64_t kSplitFromSamples = SYNAX_SPLIT_FROM;   // forward: LoS samples from which the split mode is worth its extra launches
 constexpr int64_t kOneLaneFrom = 300000, kOneLaneFromForward = 150000, kOneLaneFromStored = 24576;
@@ -517,7 +524,7 @@ static synax_status forward_core(const synax_plan* plan, const synax_model* mode
   plan->phi_stamp.valid = 0;
 
   if (code == kGridB) {
-    synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, plan->escalate_rad, sm_count(plan->device),
+    synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, escalate_at(plan), sm_count(plan->device),
                                    plan->d_flag_count, plan->h_flag_count, st, &plan->launches);
     if (gs != SYNAX_OK) return fail(gs, "grid forward failed: %s", cudaGetErrorString(cudaGetLastError()));
     return SYNAX_OK;
@@ -540,7 +547,7 @@ static synax_status forward_core(const synax_plan* plan, const synax_model* mode
   if (escalate) {
     CUDA_TRY(scratch.get(&a.flag_list, sizeof(int) * (size_t)n_sl));
     a.append_list = a.flag_list;
-    a.flag_S = (float)(plan->escalate_rad / (double)k_max);
+    a.flag_S = (float)(escalate_at(plan) / (double)k_max);
     // ... and when the rotation angle inside one 32-sample tile of the fp32 chain passes kTileAngleRad: that angle is formed
     // and range-reduced in fp32 (error ~2e-7 x angle).  Well-resolved sightlines below the first criterion stay far below
     // it (<~ 20 rad); a run with a few dozen samples per sightline at low frequency does not (parity 1.1e-4 x RMS at 43 samples).
@@ -717,12 +724,12 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   synax_status rs;
   if (code == kGridB)
     rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
-                  make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), params, dI, dQ, dU, grad, plan->precision, plan->escalate_rad,
+                  make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), params, dI, dQ, dU, grad, plan->precision, escalate_at(plan),
                   sm_count(plan->device), st, &plan->launches);
   else
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, G,
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
-                      make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, plan->escalate_rad,
+                      make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, escalate_at(plan),
                       plan->batch_share, phi, plan->d_phi_ok, phi_base, phi_has, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
                       dI, dQ, dU, grad, st, &plan->launches);
   if (rs == SYNAX_ERR_UNSUPPORTED) return fail(rs, "GRID_B vjp: n_los too large for the shared-memory hand-over (see synax.h)");

@@ -72,36 +72,7 @@ def test_random_full16_long_calls_sampled_pixels(seed):
 
 
 def _draw_mid(seed):
-    """Mid-size maps (12,288 ... 393,216 sightlines: every lane count and forward strategy the library picks by size), random
-    model kind, batch 1-3, 40-1400 samples, 1-12 frequencies from 0.3 (or 2) to 40 GHz, a box-clipped extent now and then."""
-    rng = np.random.Generator(np.random.PCG64(seed))
-    kind = rng.choice(["full16", "full16", "disc4", "stack16"])
-    nside = int(rng.choice([32, 45, 48, 52, 64, 90, 96, 112, 114, 128, 148, 150, 160]))
-    batch = int(rng.choice([1, 1, 2, 3]))
-    if 12 * nside * nside * batch > 400000:
-        batch = 1
-    n_los = int(rng.integers(40, 1400))
-    nf = int(rng.integers(1, 13))
-    lo = rng.choice([0.3e9, 0.3e9, 2e9])
-    freqs = np.sort(np.exp(rng.uniform(np.log(lo), np.log(40e9), nf)))
-    s_max = float(rng.uniform(15.0, 35.0))
-    if kind == "full16":
-        p = wl.FULL16_NOMINAL * np.exp(rng.uniform(-np.log(1.4), np.log(1.4), (batch, 16)))
-        p[:, 12] = rng.uniform(2.5, 3.3, batch)
-        if rng.random() < 0.3:
-            p[:, 12] = 3.0
-        aux = None
-    elif kind == "disc4":
-        p = wl.DISC4_NOMINAL * np.exp(rng.uniform(-np.log(1.4), np.log(1.4), (batch, 4)))
-        aux = wl.AUX_NOMINAL.astype(np.float32)
-    else:
-        w0 = wl.stack16()
-        p = np.repeat(w0.params.astype(np.float64), batch, axis=0) * np.exp(rng.uniform(-0.2, 0.2, (batch, 16)))
-        aux = w0.aux
-    w = wl.Workload(f"mid{seed}_{kind}", kind, nside, n_los, s_max, freqs, p.astype(np.float32), aux, cot_seed=seed)
-    if rng.random() < 0.25:
-        w.clip_box = (40.0, 40.0, 10.0)
-    return w
+    return wl.random_mid(seed)
 
 
 # 7049 ... 7415: the draws (of 400) on which the stand-alone adjoint missed the gradient bound while it escalated at
@@ -133,26 +104,7 @@ def test_random_mid_size_sparse_cotangents(seed):
 
 
 def _draw_grid(seed):
-    """GRID_B: non-cubic grids over boxes of arbitrary float64 lengths, a random field of 0.3-3 x cfg 3's amplitude on a spiral,
-    n_e x 0.5-3, alpha 3 or random, 1-9 frequencies from 0.3 (or 1) GHz, nside 8-48, 40-900 samples."""
-    rng = np.random.Generator(np.random.PCG64(seed))
-    shape = (int(rng.choice([24, 32, 48, 64, 96])), int(rng.choice([24, 32, 48, 64, 96])), int(rng.choice([8, 12, 16, 32])))
-    box = (float(rng.uniform(24, 44)), float(rng.uniform(24, 44)), float(rng.uniform(4, 12)))
-    X, Y, Z = wl.grid_nodes(shape, box)
-    amp = float(rng.uniform(0.3, 3.0))
-    g = amp * wl.gaussian_random_field(shape, box, seed) + wl.spiral_pattern(X, Y, Z, *wl.DISC4_NOMINAL) * float(rng.uniform(0.5, 2.0))
-    nside = int(rng.choice([8, 16, 24, 32, 48]))
-    n_los = int(rng.integers(40, 900))
-    nf = int(rng.integers(1, 10))
-    freqs = np.sort(np.exp(rng.uniform(np.log(rng.choice([0.3e9, 1e9])), np.log(30e9), nf)))
-    aux = wl.AUX_NOMINAL.astype(np.float32).copy()
-    aux[4] *= float(rng.uniform(0.5, 3.0))
-    aux[3] = float(rng.choice([3.0, rng.uniform(2.5, 3.3)]))
-    w = wl.Workload(f"grid{seed}", "grid_b", nside, n_los, float(rng.uniform(15, 30)), freqs, g.astype(np.float32), aux, box=box,
-                    cot_seed=seed)
-    if rng.random() < 0.25:
-        w.clip_box = box
-    return w
+    return wl.random_grid(seed)
 
 
 # 8020, 8040: 32 x 64 x 16 and 96 x 24 x 16 nodes over 29.77 x 41.70 x 4.51 and 33.95 x 27.05 x 6.38 kpc at 0.35 / 0.43 GHz -- while
@@ -171,59 +123,15 @@ def test_random_gridded_b(seed):
 
 
 def _draw_options(seed):
-    """Small maps with everything else random: model kind (UNIFORM included), batch 1-8, 1 / 2 / 3 / 31 ... 65 or up to 600 samples,
-    1-32 frequencies (every frequency-block split), box clip, gridded n_e / N_0, and the options lanes, precision, batch_share."""
-    rng = np.random.Generator(np.random.PCG64(seed))
-    kind = rng.choice(["full16", "disc4", "stack16", "uniform", "disc4"])
-    nside = int(rng.choice([1, 2, 3, 4, 8, 12, 16, 24, 32]))
-    batch = int(rng.choice([1, 1, 2, 3, 5, 8]))
-    n_los = int(rng.choice([1, 2, 3, 31, 32, 33, 63, 64, 65, int(rng.integers(66, 600))]))
-    nf = int(rng.choice([1, 2, 3, 4, 5, 7, 8, 9, 12, 13, 16, 17, 31, 32]))
-    freqs = np.sort(np.exp(rng.uniform(np.log(rng.choice([0.3e9, 1e9, 5e9])), np.log(40e9), nf)))
-    s_max = float(rng.uniform(10.0, 40.0))
-    aux = None
-    if kind == "full16":
-        p = wl.FULL16_NOMINAL * np.exp(rng.uniform(-np.log(1.4), np.log(1.4), (batch, 16)))
-        p[:, 12] = rng.uniform(2.5, 3.3, batch)
-        if rng.random() < 0.3:
-            p[:, 12] = 3.0
-    elif kind == "disc4":
-        p = wl.DISC4_NOMINAL * np.exp(rng.uniform(-np.log(1.4), np.log(1.4), (batch, 4)))
-        aux = wl.AUX_NOMINAL.astype(np.float32).copy()
-        if rng.random() < 0.5:
-            aux[3] = float(rng.uniform(2.5, 3.3))
-    elif kind == "stack16":
-        w0 = wl.stack16()
-        p = np.repeat(w0.params.astype(np.float64), batch, axis=0) * np.exp(rng.uniform(-0.2, 0.2, (batch, 16)))
-        aux = w0.aux
-    else:
-        w0 = wl.uniform_toy(bvec=(2.0, -3.0, 1.5))
-        p = np.repeat(w0.params.astype(np.float64), batch, axis=0) * np.exp(rng.uniform(-0.3, 0.3, (batch, w0.params.shape[1])))
-        if rng.random() < 0.5:
-            p[:, 5] = rng.uniform(2.5, 3.3, batch)
-        aux = w0.aux
-    w = wl.Workload(f"opt{seed}_{kind}", kind, nside, n_los, s_max, freqs, p.astype(np.float32), aux, cot_seed=seed)
-    if rng.random() < 0.3:
-        w.clip_box = (float(rng.uniform(30, 50)), float(rng.uniform(30, 50)), float(rng.uniform(6, 14)))
-    if kind in ("disc4", "stack16") and rng.random() < 0.4:
-        shp = (int(rng.choice([8, 16, 24])), int(rng.choice([8, 16, 24])), int(rng.choice([4, 8, 12])))
-        bx = (float(rng.uniform(30, 50)), float(rng.uniform(30, 50)), float(rng.uniform(6, 14)))
-        w.ne_grid, w.ne_box = wl.clumpy_disc_grid(shp, bx, 0.03 * float(rng.uniform(0.5, 2)), 20.0, 1.0, seed=seed), bx
-        if rng.random() < 0.5:
-            w.n0_grid, w.n0_box = wl.clumpy_disc_grid(shp, bx, 2.1e-4, 5.0, 1.0, seed=seed + 1), bx
-    opts = {}
-    if rng.random() < 0.5:
-        opts["lanes"] = int(rng.choice([1, 8, 32]))
-    if rng.random() < 0.25:
-        opts["precision"] = 2
-    if rng.random() < 0.3:
-        opts["batch_share"] = int(rng.choice([1, 2, 4]))
-    return w, opts
+    return wl.random_options(seed)
 
 
 # 9176 ... 9284: one to three samples per sightline at 0.3-1 GHz -- a single sample turns Q, U by thousands of radians; before the
 # float64 chains reduced that half-cell angle to turns in float64 (tile length 1) these were off by up to 8e-3 x RMS
-@pytest.mark.parametrize("seed", [9001, 9002, 9003, 9010, 9176, 9180, 9205, 9237, 9240, 9265, 9266, 9272, 9282, 9284])
+# 9007 ... 9523: 1 ... 65 samples per sightline, 1.0 ... 4.2e-4 x RMS on single pixels while such sightlines escalated at the same
+# 300 rad as long ones (now escalate_rad x n_los / 128: DESIGN.md section 5 (iii))
+@pytest.mark.parametrize("seed", [9001, 9002, 9003, 9010, 9176, 9180, 9205, 9237, 9240, 9265, 9266, 9272, 9282, 9284,
+                                  9007, 9165, 9345, 9523])
 def test_random_options_and_degenerate_sampling(seed):
     import torch
     import paper_2410_01136_b200 as sx
