@@ -223,7 +223,10 @@ def run_reference(args):
     steps, warmup = max(1, args.steps), max(0, args.warmup)
     # keep the whole run within a few minutes: total oracle time ~ 120 s split over steps + warm-ups
     budget = min(15.0, 120.0 / (steps + warmup))
-    cb = oracle_baseline(w, seconds_budget=budget, steps=steps, warmup=warmup)
+    # torchrun exports OMP_NUM_THREADS=1 to its workers when the variable is unset; rank 0 is the only one that works here,
+    # so it takes the cores the process may run on, as a stand-alone `python bench.py --impl reference` does
+    threads = len(os.sched_getaffinity(0)) if world > 1 else None
+    cb = oracle_baseline(w, seconds_budget=budget, steps=steps, warmup=warmup, threads=threads)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": world, "steps": steps,
             "warmup": warmup, "ms_per_step": cb["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, workloads.py)",
