@@ -162,6 +162,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
   }
   // Tile length of the float64-chain kernel: the fp32 angle k_f * (tile-local Faraday sum) must stay small
   // enough for its 6e-8 relative round-off not to matter.  Bound on |n_e B_LOS| per sample:
+  double per_step_rad;   // ... times the largest k_f: bound on the rotation of one sample
   {
     double gmax;
     if (code == kUniform) {
@@ -175,6 +176,7 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     double kmax = 0.0;
     for (int f = 0; f < ft.n_freq; ++f) kmax = fmax(kmax, (double)ft.k_rad[f]);
     const double per_step = kmax * gmax;
+    per_step_rad = per_step;
     int t = kTileDMax;
     if (per_step * t > (double)kTilePhase) t = (int)((double)kTilePhase / per_step);
     if (t > kUnrollD) t -= t % kUnrollD;
@@ -189,7 +191,10 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     d.k_hb = (code == kAnalyticFull) ? -log2e / p[4] : 0.0;
     d.Bh = p[5]; d.zh0 = p[6]; d.inv_rh = 1.0 / p[7]; d.inv_wh = 1.0 / p[8];
     d.ne0x4 = 4.0 * p[13]; d.k_her = -log2e / p[14]; d.k_hez = -2.0 * log2e / fabs(p[15]);
-    d.psi1_small = fabs(p[2]) <= 0.05 ? 1 : 0;
+    // ln(rho/8) from the MUFU lg2 (abs err ~5e-7) turns the disc field by psi1 x that: a relative error of ~|psi1| x 7e-7 in
+    // a sample's Faraday term.  Harmless when the samples turn by a few radians each (tile_d = 16: <= 3 rad) and there are
+    // hundreds of them; a run with ONE sample of 1,800 rad (psi1 0.014) was off by 2e-5 rad, 1.1e-4 x RMS -- so not then.
+    d.psi1_small = (fabs(p[2]) <= 0.05 && fabs(p[2]) * per_step_rad <= 0.15) ? 1 : 0;
     d.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4
     d.hez_is_one = (p[15] == 1.0 || p[15] == -1.0) ? 1 : 0;
     for (int k = 0; k < 4; ++k) {

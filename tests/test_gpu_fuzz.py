@@ -129,9 +129,10 @@ def _draw_options(seed):
 # 9176 ... 9284: one to three samples per sightline at 0.3-1 GHz -- a single sample turns Q, U by thousands of radians; before the
 # float64 chains reduced that half-cell angle to turns in float64 (tile length 1) these were off by up to 8e-3 x RMS
 # 9007 ... 9523: 1 ... 65 samples per sightline, 1.0 ... 4.2e-4 x RMS on single pixels while such sightlines escalated at the same
-# 300 rad as long ones (now escalate_rad x n_los / 128: DESIGN.md section 5 (iii))
+# 300 rad as long ones (now escalate_rad x n_los / 128: DESIGN.md section 5 (iii)); 9790, 9963: one sample of ~1,800 rad, the
+# float64 chain's ln(rho/8) from the MUFU lg2 (section 5 (iv))
 @pytest.mark.parametrize("seed", [9001, 9002, 9003, 9010, 9176, 9180, 9205, 9237, 9240, 9265, 9266, 9272, 9282, 9284,
-                                  9007, 9165, 9345, 9523])
+                                  9007, 9165, 9345, 9523, 9790, 9963])
 def test_random_options_and_degenerate_sampling(seed):
     import torch
     import paper_2410_01136_b200 as sx
