@@ -1,5 +1,6 @@
 // synax_grid.cu -- host-side dispatch of the gridded-B kernels (synax_grid.cuh).
 #include <algorithm>
+#include <numeric>
 
 #include "synax_launch.h"
 #include "synax_grid.cuh"
@@ -91,6 +92,11 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   float k_max = 0.f;
   for (int f = 0; f < ft.n_freq; ++f) k_max = fmaxf(k_max, ft.k_rad[f]);
   a.mode = precision; a.flag_S = (float)(escalate_rad / (double)k_max);
+  // order of the pixel groups (grid_vjp_kernel): a stride of about the golden section of their count, coprime to it
+  a.n_groups = (geo.npix + kGridGroup - 1) / kGridGroup;
+  a.group_stride = std::max<int64_t>(1, (int64_t)(0.6180339887 * (double)a.n_groups));
+  while (std::gcd(a.group_stride, a.n_groups) != 1) ++a.group_stride;
+  a.group_stride %= a.n_groups;   // (n_groups = 1: stride 0, the one group)
   const size_t smem = (size_t)(kBlock / 32) * 3 * 32 * ((1u << cl) + 1) * sizeof(float);
   if (smem > 200 * 1024) return SYNAX_ERR_UNSUPPORTED;  // n_los too large for the shared-memory hand-over
   if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;

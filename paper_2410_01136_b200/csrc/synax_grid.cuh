@@ -354,6 +354,7 @@ __global__ void grid_grad_compact_kernel(const float4* __restrict__ g4, int64_t 
 // Adjoint.  grad_grid must be zero on entry (the host wrapper clears it).
 // Dynamic shared memory: 3 float arrays of 32*(C+1) per warp, C = chunk length (power of two).
 // ------------------------------------------------------------------------------------------------
+constexpr int kGridGroup = kBlock / 32;   // grid_vjp_kernel: neighbouring pixels taken together (the warps of a CTA)
 struct GridVjpArgs {
   Geometry geo;
   ScalarGridDesc sg_ne, sg_n0;
@@ -366,6 +367,8 @@ struct GridVjpArgs {
   int chunk_log2;       // C = 1 << chunk_log2, 32*C >= n_los
   int mode;             // 0 auto, 1 fp32 chain, 2 float64 Faraday chain
   float flag_S;         // auto: redo a sightline in float64 when max |sum n_e B_LOS| exceeds this
+  int64_t n_groups;     // ceil(npix / kGridGroup): groups of neighbouring pixels, one per CTA pass
+  int64_t group_stride; // coprime to n_groups, ~0.618 n_groups: the order in which the groups are taken (grid_vjp_kernel)
 };
 
 // Sweep 2's per-lane accumulators: the 8 x 3 corner contributions of the cell the lane is in.  A ray leaves a cell
@@ -518,7 +521,14 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
   const int64_t n_warps = ((int64_t)gridDim.x * kBlock) >> 5;
   const BatchConsts& P = A.bc[0];
   const BatchConstsD D = A.bd[0];
-  for (int64_t pix = warp; pix < A.geo.npix; pix += n_warps) {
+  // Sightline order: the warps of a CTA take neighbouring pixels (their gathers share L1 lines), but the CTAs that run at the
+  // same time are spread over the sky -- group q of kBlock / 32 pixels is the (q * group_stride mod n_groups)-th of the map
+  // (group_stride coprime to n_groups: a permutation).  In pixel order the ~3,000 sightlines in flight cross the same cells
+  // at the same time and their red.global.add to the same nodes queue up in L2 (cfg 3: 0.66 -> 0.55 ms).
+  constexpr int64_t kW = kGridGroup;
+  for (int64_t pidx = warp; pidx < A.n_groups * kW; pidx += n_warps) {
+    const int64_t pix = (((pidx / kW) * A.group_stride) % A.n_groups) * kW + pidx % kW;
+    if (pix >= A.geo.npix) continue;   // the last group of a map whose size is no multiple of kW (warp-uniform)
     const Triad T = load_triad(A.geo, pix);
     const double delta = A.geo.delta * T.scale;
     const double4 dir = *reinterpret_cast<const double4*>(A.geo.dirs + 4 * pix);

@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
+#include <numeric>
 #include <vector>
 
 #include "../csrc/synax_grid.cuh"
@@ -101,13 +102,17 @@ __device__ __forceinline__ void red_add_v4(float* p, float a, float b, float c, 
   asm volatile("red.global.v4.f32.add [%0], {%1, %2, %3, %4};" :: "l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 // the same stream into a gradient padded to 4 floats per node: one 16-byte vector red per corner
-__global__ void red_stream_v4(Geometry geo, GridDesc G, float* __restrict__ grad4, unsigned long long* __restrict__ count) {
+// group_stride > 0: the sightlines in grid_vjp_kernel's order (groups of kGridGroup neighbouring pixels, group q -> q * stride mod n)
+__global__ void red_stream_v4(Geometry geo, GridDesc G, float* __restrict__ grad4, unsigned long long* __restrict__ count,
+                              int64_t n_groups, int64_t group_stride) {
   const int lane = threadIdx.x & 31;
   const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
   const int C = (geo.n_los + 31) / 32;
   unsigned long long mine = 0;
-  for (int64_t pix = warp; pix < geo.npix; pix += n_warps) {
+  for (int64_t pidx = warp; pidx < n_groups * kGridGroup; pidx += n_warps) {
+    const int64_t pix = group_stride > 0 ? (((pidx / kGridGroup) * group_stride) % n_groups) * kGridGroup + pidx % kGridGroup : pidx;
+    if (pix >= geo.npix) continue;
     const Triad T = load_triad(geo.dirs, pix);
     const int m0 = min(lane * C, geo.n_los), m1 = min(m0 + C, geo.n_los);
     int cur = -1;
@@ -186,13 +191,21 @@ int main() {
   }
   time_it([&] { red_stream<false><<<sms * 16, 128>>>(geo, G, grad, count); }, "R red.add un-aggregated, 16 CTAs/SM", n_raw, "red");
   float* grad4; CK(cudaMalloc(&grad4, ngrid / 3 * 4 * 4)); CK(cudaMemset(grad4, 0, ngrid / 3 * 4 * 4));
+  const int64_t n_groups = (npix + kGridGroup - 1) / kGridGroup;
+  int64_t group_stride = std::max<int64_t>(1, (int64_t)(0.6180339887 * (double)n_groups));   // as grid_vjp() chooses it
+  while (std::gcd(group_stride, n_groups) != 1) ++group_stride;
+  double best_r4p = 1e30;
   for (int bps : {8, 16}) {
-    char name[64]; snprintf(name, sizeof(name), "R red.add.v4 per-cell aggregated, %d CTAs/SM", bps);
-    best_r4 = std::min(best_r4, time_it([&] { red_stream_v4<<<sms * bps, 128>>>(geo, G, grad4, count); }, name, n_agg / 3, "red.v4"));
+    char name[80]; snprintf(name, sizeof(name), "R red.add.v4 per-cell aggregated, pixel order, %d CTAs/SM", bps);
+    best_r4 = std::min(best_r4, time_it([&] { red_stream_v4<<<sms * bps, 128>>>(geo, G, grad4, count, n_groups, 0); }, name, n_agg / 3, "red.v4"));
+  }
+  for (int bps : {5, 8, 16}) {
+    char name[80]; snprintf(name, sizeof(name), "R red.add.v4, the adjoint's group order, %d CTAs/SM", bps);
+    best_r4p = std::min(best_r4p, time_it([&] { red_stream_v4<<<sms * bps, 128>>>(geo, G, grad4, count, n_groups, group_stride); }, name, n_agg / 3, "red.v4"));
   }
   // one machine-readable line for bench.py --config 3 (the ceilings of the gridded path, best over the CTA counts)
-  printf("JSON {\"gather_ms\": %.5f, \"gather_v4_ms\": %.5f, \"red_v4_ms\": %.5f, \"gather_bytes\": %.6e, \"red_v4_count\": %.6e, \"samples\": %.6e}\n",
-         best_g, best_g4, best_r4, samples * 96.0, n_agg / 3, samples);
+  printf("JSON {\"gather_ms\": %.5f, \"gather_v4_ms\": %.5f, \"red_v4_ms\": %.5f, \"red_v4_group_order_ms\": %.5f, \"gather_bytes\": %.6e, \"red_v4_count\": %.6e, \"samples\": %.6e}\n",
+         best_g, best_g4, best_r4, best_r4p, samples * 96.0, n_agg / 3, samples);
   CK(cudaDeviceSynchronize());
   return 0;
 }
