@@ -99,8 +99,10 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   a.group_stride %= a.n_groups;   // (n_groups = 1: stride 0, the one group)
   const size_t smem = (size_t)(kBlock / 32) * 3 * 32 * ((1u << cl) + 1) * sizeof(float);
   if (smem > 200 * 1024) return SYNAX_ERR_UNSUPPORTED;  // n_los too large for the shared-memory hand-over
-  if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
-  if (cudaMemsetAsync(a.grad4, 0, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) {
+  // (+ one 8-byte ticket counter per frequency block behind the accumulation buffer, cleared with it)
+  if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes + 8 * kMaxFreq, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
+  unsigned long long* tickets = reinterpret_cast<unsigned long long*>(a.grad4 + (size_t)n_nodes * 4);
+  if (cudaMemsetAsync(a.grad4, 0, sizeof(float4) * (size_t)n_nodes + 8 * kMaxFreq, st) != cudaSuccess) {
     cudaFreeAsync(a.grad4, st);
     return SYNAX_ERR_CUDA;
   }
@@ -113,6 +115,7 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   for (int f0 = 0; f0 < ft.n_freq;) {
     const int rem = ft.n_freq - f0, nf = rem >= 8 ? 8 : (rem >= 4 ? 4 : rem);
     a.f0 = f0;
+    a.ticket = tickets + f0;
     const bool sg = a.sg_ne.g || a.sg_n0.g;
 #define SYNAX_GV(NFV)                                                                                              \
   do {                                                                                                             \

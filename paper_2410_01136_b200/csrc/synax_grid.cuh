@@ -368,6 +368,7 @@ struct GridVjpArgs {
   int mode;             // 0 auto, 1 fp32 chain, 2 float64 Faraday chain
   float flag_S;         // auto: redo a sightline in float64 when max |sum n_e B_LOS| exceeds this
   int64_t n_groups;     // ceil(npix / kGridGroup): groups of neighbouring pixels, one per CTA pass
+  unsigned long long* ticket;   // zero on entry: next index of the permuted sequence
   int64_t group_stride; // coprime to n_groups, ~0.618 n_groups: the order in which the groups are taken (grid_vjp_kernel)
 };
 
@@ -524,9 +525,15 @@ __global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant_
   // Sightline order: the warps of a CTA take neighbouring pixels (their gathers share L1 lines), but the CTAs that run at the
   // same time are spread over the sky -- group q of kBlock / 32 pixels is the (q * group_stride mod n_groups)-th of the map
   // (group_stride coprime to n_groups: a permutation).  In pixel order the ~3,000 sightlines in flight cross the same cells
-  // at the same time and their red.global.add to the same nodes queue up in L2 (cfg 3: 0.66 -> 0.55 ms).
+  // at the same time and their red.global.add to the same nodes queue up in L2 (cfg 3: 0.67 -> 0.545 ms).
   constexpr int64_t kW = kGridGroup;
-  for (int64_t pidx = warp; pidx < A.n_groups * kW; pidx += n_warps) {
+  for (;;) {
+    // the next sightline of that sequence goes to whichever warp is free (costs differ: in-box length, fp32 or float64
+    // chain): 0.545 -> 0.536 ms
+    unsigned long long tk = 0;
+    if (lane == 0) tk = atomicAdd(A.ticket, 1ULL);
+    const int64_t pidx = (int64_t)__shfl_sync(0xffffffffu, tk, 0);
+    if (pidx >= A.n_groups * kW) break;
     const int64_t pix = (((pidx / kW) * A.group_stride) % A.n_groups) * kW + pidx % kW;
     if (pix >= A.geo.npix) continue;   // the last group of a map whose size is no multiple of kW (warp-uniform)
     const Triad T = load_triad(A.geo, pix);
