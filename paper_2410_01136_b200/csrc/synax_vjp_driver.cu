@@ -69,7 +69,7 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   a.phi = phi; a.phi_ok = phi_ok; a.phi_base = phi_base; a.phi_has = phi_has; a.only_with_bases = 0;
   // Long calls with one thread per sightline: the work is split per CTA between the lean fp32 variant and the
   // float64-angle variant (vjp_classify_kernel) instead of deciding per sightline inside one heavier kernel
-  // (cfg 4, 9 % of the sightlines above the threshold: 14.3 -> see DESIGN.md section 5).
+  // (cfg 4 stand-alone with nothing stored by a forward: DESIGN.md section 5).
   // (G lanes per sightline, G > 1: a CTA holds 128 / G sightlines; worth its three extra launches from ~1M threads)
   const bool split = precision == 0 && (G == 1 ? geo.npix * batch >= 262144 : geo.npix * batch * G >= 1000000);
   if (precision == 0) {
