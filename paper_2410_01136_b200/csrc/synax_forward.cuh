@@ -611,10 +611,12 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
   const int64_t pix = sl - (int64_t)b * A.geo.npix;
   const BatchConsts& P = A.bc[b];
   const Triad T = load_triad(A.geo, pix);
-  const int C = (A.geo.n_los + 31) / 32;
-  const int n0 = lane * C, n1 = min(n0 + C, A.geo.n_los);
+  // every 16th sample of the sightline (all of them below 32), spread over the lanes: the estimate classify_kernel and the
+  // adjoint use.  It only picks the strategy -- the fp32 kernels check the exact sum -- and costs 1/16 of a full pass
+  // (cfg 1: 12.7 -> see profiles/r02_launches.md; before, the pilot was 8 % of that forward).
+  const int step = A.geo.n_los >= 32 ? 16 : 1;
   float gabs = 0.0f;
-  for (int n = n0; n < n1; ++n) {
+  for (int n = step / 2 + lane * step; n < A.geo.n_los; n += 32 * step) {
     const double s_d = ((double)n + 0.5) * A.geo.delta * T.scale;
     float gn;
     if (CODE == kUniform) {
@@ -638,7 +640,7 @@ __global__ void __launch_bounds__(kBlock) pilot_kernel(const __grid_constant__ F
     }
     gabs += gn;
   }
-  const float absS = T.scalef * group_sum<32>(gabs);
+  const float absS = T.scalef * (float)step * group_sum<32>(gabs);
   if (lane == 0 && absS > A.flag_S) atomicAdd(ctrl + kCtrlPilotFlagged, 1);
 }
 
