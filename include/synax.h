@@ -131,8 +131,12 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * synax_vjp values 2 and 4 apply unless the plan's last forward left tile bases (then the kernel that uses those runs).
  * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool
  * (from which every call takes its scratch) to this many MB, so that the pool is not unmapped at every stream
- * synchronisation -- matters for the *_host calls (hundreds of MB of staging per call).  Process-wide for that
- * device, hence opt-in; never lowers a larger threshold set by the application. */
+ * synchronisation.  With the CUDA default (0) the first call after every stream or device synchronisation waits for
+ * the pool to map memory again: ~0.23 ms of host time during which the GPU idles, whatever the size of the call
+ * (measured on B200: a cfg-1 forward 0.15 -> 0.38 ms, a cfg-3 forward 0.24 -> 0.46 ms when the caller synchronises
+ * after each call).  A loop that reads a result every step should set this once (64 covers the device-buffer calls of
+ * every BASELINE config; the *_host calls stage hundreds of MB per call).  Process-wide for that device, hence opt-in;
+ * never lowers a larger threshold set by the application. */
 synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value);
 
 /* Pixel directions as cached by the plan: out[4*p..] = (cos l, sin l, cos b, sin b), DEVICE float64

@@ -128,9 +128,14 @@ class Model:
 
 class Plan:
     """synax_plan_create / synax_plan_create_shard (pix_range=(begin, count)) / synax_plan_create_strided
-    (pix_range=(begin, count), pix_stride=n: pixels begin + i * n) / synax_plan_destroy."""
+    (pix_range=(begin, count), pix_stride=n: pixels begin + i * n) / synax_plan_destroy.
+    pool_release_threshold_mb: option of the same name (include/synax.h) -- set it (64 is plenty for device-buffer calls) when the
+    loop around the calls synchronises every step: each call takes its scratch from the device's stream-ordered memory pool,
+    whose default is to give everything back at a synchronisation, and the first call after one then waits ~0.23 ms for the
+    pool to map memory again (measured on B200: a cfg-1 forward 0.15 -> 0.38 ms).  Process-wide for the device, hence opt-in."""
 
-    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006), pix_range=None, pix_stride=1):
+    def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006), pix_range=None, pix_stride=1,
+                 pool_release_threshold_mb=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("synax needs a CUDA device (B200); there is no CPU fallback")
@@ -156,6 +161,8 @@ class Plan:
         self.nside, self.n_los, self.s_max, self.freqs = int(nside), int(n_los), float(s_max), f
         self.n_freq = int(f.size)
         self.npix = int(L.synax_plan_npix(h))
+        if pool_release_threshold_mb is not None:
+            self.set_option("pool_release_threshold_mb", float(pool_release_threshold_mb))
 
     def set_box(self, box):
         """synax_plan_set_box: integrate from the observer to the faces of a box (lx, ly, lz kpc); None = fixed s_max."""

@@ -509,7 +509,8 @@ __device__ __forceinline__ float grid_vjp_sweep1(const GridVjpArgs& A, const Fre
 }
 
 template <int NF, bool SG>
-__global__ void __launch_bounds__(kBlock) grid_vjp_kernel(const __grid_constant__ GridVjpArgs A,
+// (one frequency: a sixth CTA per SM for 8 bytes of spill, 0.535 -> 0.525 ms at cfg 3; no gain with 4 or 8 frequencies)
+__global__ void __launch_bounds__(kBlock, NF == 1 ? 6 : 5) grid_vjp_kernel(const __grid_constant__ GridVjpArgs A,
                                                           const __grid_constant__ FreqTab ft) {
   extern __shared__ float smem[];
   const GridDesc& G = A.grid;

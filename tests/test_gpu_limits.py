@@ -168,3 +168,22 @@ def test_adjoint_pair_on_two_streams_is_graph_capturable_and_ordered():
     rel = ((gp.cpu() - g_host).abs() / gp.cpu().abs()).max().item()
     assert rel <= 1e-3, rel
     plan.close()
+
+
+def test_pool_release_threshold_keyword():
+    """Plan(pool_release_threshold_mb=...) sets the option of that name (process-wide, opt-in: include/synax.h); results are
+    those of a plan without it, whether or not the caller synchronises between the calls."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    w = wl.config(1).scaled(nside=16, n_los=96)
+    plan0, model, params = parity.gpu_objects(w)
+    ref = [t.clone() for t in sx.forward(plan0, model, params)]
+    plan0.close()
+    plan = sx.Plan(w.nside, w.n_los, w.s_max, w.freqs, pool_release_threshold_mb=64)
+    for _ in range(3):
+        out = sx.forward(plan, model, params)
+        torch.cuda.synchronize()
+        assert all(torch.equal(a, b) for a, b in zip(out, ref))
+    with pytest.raises(sx.SynaxError):
+        plan.set_option("pool_release_threshold_mb", -1.0)
+    plan.close()
