@@ -129,14 +129,14 @@ synax_status synax_plan_set_box(synax_plan* plan, const double box_kpc[3]);
  * key "batch_share": parameter vectors integrated per thread when a batch of analytic models is evaluated at one
  * frequency with one thread per sightline -- they share the sightline geometry (0 = heuristic, else 1, 2 or 4).  In
  * synax_vjp values 2 and 4 apply unless the plan's last forward left tile bases (then the kernel that uses those runs).
- * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool
- * (from which every call takes its scratch) to this many MB, so that the pool is not unmapped at every stream
- * synchronisation.  With the CUDA default (0) the first call after every stream or device synchronisation waits for
- * the pool to map memory again: ~0.23 ms of host time during which the GPU idles, whatever the size of the call
- * (measured on B200: a cfg-1 forward 0.15 -> 0.38 ms, a cfg-3 forward 0.24 -> 0.46 ms when the caller synchronises
- * after each call).  A loop that reads a result every step should set this once (64 covers the device-buffer calls of
- * every BASELINE config; the *_host calls stage hundreds of MB per call).  Process-wide for that device, hence opt-in;
- * never lowers a larger threshold set by the application. */
+ * key "pool_release_threshold_mb": raise the release threshold of the device's default stream-ordered memory pool to this
+ * many MB.  Per-call scratch comes from a workspace the plan keeps (see "Scratch" below); the pool serves what does not
+ * fit into it -- a call that needs more than 256 MB, e.g. the host entry points' staging of large maps -- and every call
+ * made inside a stream capture.  With CUDA's default threshold (0) the pool hands everything back at each stream or
+ * device synchronisation, and the first pool allocation after one waits ~0.23 ms of host time for memory to be mapped
+ * again (measured on B200; while all scratch came from the pool, a cfg-1 forward took 0.38 instead of 0.15 ms in a loop
+ * that synchronised every step).  Process-wide for that device, hence opt-in; never lowers a larger threshold set by
+ * the application. */
 synax_status synax_plan_set_option(synax_plan* plan, const char* key, double value);
 
 /* Pixel directions as cached by the plan: out[4*p..] = (cos l, sin l, cos b, sin b), DEVICE float64
@@ -151,8 +151,13 @@ synax_status synax_plan_directions(const synax_plan* plan, double* out_device, v
  * per 32 samples and sightline: 201 MB at nside 256 x 1024 samples) and a device copy of `params`, for the next synax_vjp of
  * this plan.  The buffers are plan-owned and grown with cudaMalloc the first time a call of a given size comes (that call
  * synchronises the device once; never inside a stream capture; if the memory is not there the call goes on without them).
- * GRID_B: per-call scratch of 16 bytes per grid node (the grid repacked into 16-byte nodes) from the stream-ordered pool;
- * synax_vjp takes another 16 bytes per node there for the gradient accumulation. */
+ * GRID_B: per-call scratch of 16 bytes per grid node (the grid repacked into 16-byte nodes); synax_vjp takes another 16 bytes
+ * per node for the gradient accumulation.
+ * Scratch (every entry point but synax_vjp_f64_noalloc): constants, lists, block partials and the buffers above are cut, in
+ * stack order, from ONE workspace that stays with the plan (at most 256 MB; grown with cudaFree + cudaMalloc at the start of a
+ * call when an earlier call needed more -- that call synchronises the device once; never inside a stream capture).  What
+ * does not fit, and all scratch of a call made inside a stream capture (a captured graph must not point into a buffer that
+ * may be reallocated), comes from the device's default stream-ordered memory pool (option "pool_release_threshold_mb"). */
 synax_status synax_forward(const synax_plan* plan, const synax_model* model, const float* params,
                            int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
 
@@ -210,7 +215,8 @@ synax_status synax_vjp_f64_noalloc(const synax_plan* plan, const synax_model* mo
 /* Same operations with HOST buffers of the same shapes: the call copies the inputs to the device,
  * runs, copies the results back and synchronises the stream before returning.  When I, Q and U are all page-locked
  * (cudaHostAlloc / cudaHostRegister) the forward kernels store the maps straight into them and no copy is made.
- * Scratch comes from the device's default stream-ordered memory pool (see option "pool_release_threshold_mb"). */
+ * Scratch: the plan's workspace up to 256 MB, beyond that the device's default stream-ordered memory pool (see option
+ * "pool_release_threshold_mb": staging cfg 4's maps takes 226 MB). */
 synax_status synax_forward_host(const synax_plan* plan, const synax_model* model, const float* params,
                                 int32_t batch, float* I, float* Q, float* U, void* cuda_stream);
 synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, const float* params,
@@ -224,7 +230,7 @@ synax_status synax_vjp_host(const synax_plan* plan, const synax_model* model, co
  * I_obs, Q_obs, U_obs: DEVICE fp32 [n_freq][npix], ONE observation shared by all batch elements; a NULL map takes
  * that Stokes parameter out of the likelihood (the paper uses Q and U only, sigma = 1 mK: w = 1/sigma^2 in K^-2).
  * inv_var: HOST, 3 weights >= 0.  logL: DEVICE float64 [batch], overwritten.  grad: DEVICE fp32 as in synax_vjp.
- * Scratch for the three maps ([batch][n_freq][npix] fp32 each) is taken from the stream-ordered pool. */
+ * Scratch for the three maps ([batch][n_freq][npix] fp32 each): the plan's workspace (synax_forward), else the pool. */
 synax_status synax_loglike_vjp(const synax_plan* plan, const synax_model* model, const float* params,
                                int32_t batch, const float* I_obs, const float* Q_obs, const float* U_obs,
                                const double inv_var[3], double* logL, float* grad, void* cuda_stream);

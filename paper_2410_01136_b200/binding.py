@@ -129,10 +129,10 @@ class Model:
 class Plan:
     """synax_plan_create / synax_plan_create_shard (pix_range=(begin, count)) / synax_plan_create_strided
     (pix_range=(begin, count), pix_stride=n: pixels begin + i * n) / synax_plan_destroy.
-    pool_release_threshold_mb: option of the same name (include/synax.h) -- set it (64 is plenty for device-buffer calls) when the
-    loop around the calls synchronises every step: each call takes its scratch from the device's stream-ordered memory pool,
-    whose default is to give everything back at a synchronisation, and the first call after one then waits ~0.23 ms for the
-    pool to map memory again (measured on B200: a cfg-1 forward 0.15 -> 0.38 ms).  Process-wide for the device, hence opt-in."""
+    pool_release_threshold_mb: option of the same name (include/synax.h).  Calls cut their scratch from a workspace the plan
+    keeps; only what exceeds 256 MB (the host entry points' staging of large maps) and calls inside a stream capture go to the
+    device's stream-ordered memory pool, whose default is to give everything back at a synchronisation (the next pool
+    allocation then waits ~0.23 ms).  Process-wide for the device, hence opt-in."""
 
     def __init__(self, nside: int, n_los: int, s_max: float, freqs, observer=(-8.3, 0.0, 0.006), pix_range=None, pix_stride=1,
                  pool_release_threshold_mb=None):

@@ -71,6 +71,7 @@ struct synax_plan {
   mutable int* d_phi_ok;
   mutable struct PhiStamp { int valid, code, batch, n_params, precision; double escalate_rad, delta; const double* path; float aux[7]; } phi_stamp;
   mutable int phi_has_bases;   // the last forward also stored tile bases
+  mutable Workspace ws;        // per-call scratch, kept between calls (synax_launch.h)
   mutable int64_t launches;
   mutable int64_t last_n_sl;  // sightlines of the last forward (for stats when every one took the float64 chain)
 };
@@ -186,6 +187,7 @@ extern "C" synax_status synax_plan_destroy(synax_plan* plan) {
   if (plan->phi_has) cudaFree(plan->phi_has);
   if (plan->phi_params) cudaFree(plan->phi_params);
   if (plan->d_phi_ok) cudaFree(plan->d_phi_ok);
+  if (plan->ws.base) cudaFree(plan->ws.base);
   cudaFree(plan->d_flag_count);
   cudaFree(plan->d_vjp_ctrl);
   cudaFreeHost(plan->h_flag_count);
@@ -397,28 +399,75 @@ static int sm_count(int device) {
   return cached[device];
 }
 
-// Per-call scratch from the device's stream-ordered pool; everything handed out is given back (cudaFreeAsync on the
-// same stream) when the guard leaves scope, whatever path the call returns on.
+// Plan-owned workspace (synax_launch.h).
+namespace synax {
+void* ws_alloc(Workspace* ws, size_t bytes, cudaStream_t st, bool* pooled) {
+  *pooled = false;
+  bytes = (bytes + 255) & ~(size_t)255;
+  if (bytes == 0) bytes = 256;
+  if (ws) {
+    const size_t at = ws->used;
+    ws->used += bytes;
+    if (ws->used > ws->want) ws->want = ws->used;
+    if (ws->base && at + bytes <= ws->cap) {
+      cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+      if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) cudaGetLastError();
+      else if (cap == cudaStreamCaptureStatusNone) return ws->base + at;
+    }
+  }
+  void* q = nullptr;
+  if (cudaMallocAsync(&q, bytes, st) != cudaSuccess) return nullptr;
+  *pooled = true;
+  return q;
+}
+void ws_enter(Workspace* ws, cudaStream_t st, size_t* mark) {
+  *mark = 0;
+  if (!ws) return;
+  if (ws->depth++ == 0) {
+    ws->used = 0;
+    const size_t want = std::min(ws->want, kWorkspaceMax);
+    if (want > ws->cap) {
+      cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+      if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) cudaGetLastError();
+      else if (cap == cudaStreamCaptureStatusNone) {
+        if (ws->base) cudaFree(ws->base);   // (synchronises the device: earlier calls may still be using it)
+        ws->base = nullptr; ws->cap = 0;
+        const size_t grow = std::min(kWorkspaceMax, want + want / 4);
+        if (cudaMalloc((void**)&ws->base, grow) == cudaSuccess) ws->cap = grow;
+        else cudaGetLastError();
+      }
+    }
+  }
+  *mark = ws->used;
+}
+}  // namespace synax
+
+// Per-call scratch in stack order from the plan's workspace (else from the device's stream-ordered pool); everything handed
+// out is given back when the guard leaves scope, whatever path the call returns on.
 struct StreamScratch {
   cudaStream_t st;
+  Workspace* ws;
+  size_t mark = 0;
   void* blocks[12];
   int n = 0;
-  explicit StreamScratch(cudaStream_t s) : st(s) {}
+  StreamScratch(const synax_plan* plan, cudaStream_t s);
   StreamScratch(const StreamScratch&) = delete;
   StreamScratch& operator=(const StreamScratch&) = delete;
   ~StreamScratch() {
     for (int i = n - 1; i >= 0; --i) cudaFreeAsync(blocks[i], st);
+    ws_leave(ws, mark);
   }
   template <typename T>
   cudaError_t get(T** out, size_t bytes) {
-    void* q = nullptr;
+    bool pooled = false;
     if (n >= 12) { *out = nullptr; return cudaErrorMemoryAllocation; }
-    const cudaError_t e = cudaMallocAsync(&q, bytes ? bytes : 1, st);
-    if (e == cudaSuccess) blocks[n++] = q;
+    void* q = ws_alloc(ws, bytes, st, &pooled);
+    if (q && pooled) blocks[n++] = q;
     *out = (T*)q;
-    return e;
+    return q ? cudaSuccess : cudaErrorMemoryAllocation;
   }
 };
+StreamScratch::StreamScratch(const synax_plan* plan, cudaStream_t s) : st(s), ws(&plan->ws) { ws_enter(ws, st, &mark); }
 
 // Per-batch constants of a call (prologue_kernel).  When a gridded n_e replaces the analytic disc, the bound on
 // |n_e B_LOS| that sizes the float64 chain's tiles (BatchConsts::tile_d) comes from max |ne_grid|, reduced on the device
@@ -506,7 +555,7 @@ static synax_status forward_core(const synax_plan* plan, const synax_model* mode
   const int64_t n_sl = plan->npix * batch;
   if (faraday_only && !(code != kGridB && pick_lanes(plan, n_sl, kOneLaneFromStored) == 1 && phi_buffers(plan, model, batch, st)))
     return SYNAX_OK;   // nowhere to put them (small call, lanes forced, gridded n_e, capture without buffers)
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
 
   BatchConsts* bc = nullptr;
   BatchConstsD* bd = nullptr;
@@ -525,7 +574,7 @@ static synax_status forward_core(const synax_plan* plan, const synax_model* mode
 
   if (code == kGridB) {
     synax_status gs = grid_forward(plan->ft, a, model, params, plan->precision, escalate_at(plan), sm_count(plan->device),
-                                   plan->d_flag_count, plan->h_flag_count, st, &plan->launches);
+                                   plan->d_flag_count, plan->h_flag_count, &plan->ws, st, &plan->launches);
     if (gs != SYNAX_OK) return fail(gs, "grid forward failed: %s", cudaGetErrorString(cudaGetLastError()));
     return SYNAX_OK;
   }
@@ -681,7 +730,7 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   if (stt != SYNAX_OK) return stt;
   if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
   BatchConsts* bc = nullptr;
   BatchConstsD* bd = nullptr;
   stt = run_prologue(plan, model, code, params, batch, scratch, &bc, &bd, st);
@@ -725,13 +774,13 @@ extern "C" synax_status synax_vjp(const synax_plan* plan, const synax_model* mod
   if (code == kGridB)
     rs = grid_vjp(plan->ft, make_geo(plan), bc, bd, model, make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                   make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), params, dI, dQ, dU, grad, plan->precision, escalate_at(plan),
-                  sm_count(plan->device), st, &plan->launches);
+                  sm_count(plan->device), &plan->ws, st, &plan->launches);
   else
     rs = analytic_vjp(code, plan->ft, make_geo(plan), bc, bd, batch, model->n_params, G,
                       make_scalar_desc(model->ne_grid, model->ne_n, model->ne_l),
                       make_scalar_desc(model->n0_grid, model->n0_n, model->n0_l), plan->precision, escalate_at(plan),
                       plan->batch_share, phi, plan->d_phi_ok, phi_base, phi_has, plan->d_vjp_ctrl, plan->aux, plan->ev_fork, plan->ev_join,
-                      dI, dQ, dU, grad, st, &plan->launches);
+                      dI, dQ, dU, grad, &plan->ws, st, &plan->launches);
   if (rs == SYNAX_ERR_UNSUPPORTED) return fail(rs, "GRID_B vjp: n_los too large for the shared-memory hand-over (see synax.h)");
   if (rs != SYNAX_OK) return fail(rs, "vjp failed: %s", cudaGetErrorString(cudaGetLastError()));
   return SYNAX_OK;
@@ -754,7 +803,7 @@ extern "C" synax_status synax_forward_f64(const synax_plan* plan, const synax_mo
   if (stt != SYNAX_OK) return stt;
   if (!I || !Q || !U) return fail(SYNAX_ERR_INVALID_ARG, "I, Q or U is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
   void* bc64 = nullptr;
   CUDA_TRY(scratch.get(&bc64, dd_consts_bytes(batch)));
   stt = dd_forward(code, plan->ft, make_geo(plan), params, model->n_params, batch, make_aux(model),
@@ -772,7 +821,7 @@ extern "C" synax_status synax_vjp_f64(const synax_plan* plan, const synax_model*
   if (stt != SYNAX_OK) return stt;
   if (!grad) return fail(SYNAX_ERR_INVALID_ARG, "grad is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
   void* bc64 = nullptr;
   double* partial = nullptr;
   const int G = pick_lanes(plan, plan->npix * batch);
@@ -853,7 +902,7 @@ extern "C" synax_status synax_loglike_vjp(const synax_plan* plan, const synax_mo
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int64_t per_batch = (int64_t)plan->n_freq * plan->npix;
   const size_t count = (size_t)batch * (size_t)per_batch;
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
   float* maps = nullptr;
   CUDA_TRY(scratch.get(&maps, 3 * count * sizeof(float)));
   float* m[3] = {maps, maps + count, maps + 2 * count};
@@ -928,7 +977,7 @@ extern "C" synax_status synax_forward_host(const synax_plan* plan, const synax_m
   const size_t pbytes = sizeof(float) * (size_t)model->n_params * (size_t)batch;
   const size_t mbytes = sizeof(float) * (size_t)batch * plan->n_freq * (size_t)plan->npix;
   float *dp = nullptr, *dm = nullptr;
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
   CUDA_TRY(scratch.get(&dp, pbytes));
   CUDA_TRY(cudaMemcpyAsync(dp, params, pbytes, cudaMemcpyHostToDevice, st));
   // Page-locked map buffers: the kernels store straight into them.  A map value is written exactly once, by the
@@ -964,7 +1013,7 @@ extern "C" synax_status synax_vjp_host(const synax_plan* plan, const synax_model
   const size_t pbytes = sizeof(float) * (size_t)model->n_params * (size_t)batch;
   const size_t mcount = (size_t)batch * plan->n_freq * (size_t)plan->npix;
   float *dp = nullptr, *dg = nullptr, *dc = nullptr;
-  StreamScratch scratch(st);
+  StreamScratch scratch(plan, st);
   CUDA_TRY(scratch.get(&dp, pbytes));
   CUDA_TRY(scratch.get(&dg, pbytes));
   CUDA_TRY(scratch.get(&dc, 3 * mcount * sizeof(float)));

@@ -19,18 +19,18 @@ static GridDesc make_grid_desc(const synax_model* m, const float* grid) {
   return g;
 }
 
-// Repacked per-call copy of the grid (GridDesc::g4) from the stream-ordered pool; 0 on success.
-static synax_status pack_grid(GridDesc& g, cudaStream_t st, int64_t* launches) {
+// Repacked per-call copy of the grid (GridDesc::g4) from the plan's workspace (or the stream-ordered pool); 0 on success.
+static synax_status pack_grid(GridDesc& g, Workspace* ws, bool* pooled, cudaStream_t st, int64_t* launches) {
   const int64_t n_nodes = (int64_t)g.nx * g.ny * g.nz;
-  float4* g4 = nullptr;
-  if (cudaMallocAsync((void**)&g4, sizeof(float4) * (size_t)n_nodes, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
+  float4* g4 = static_cast<float4*>(ws_alloc(ws, sizeof(float4) * (size_t)n_nodes, st, pooled));
+  if (!g4) return SYNAX_ERR_ALLOC;
   grid_pack_kernel<<<(unsigned)((n_nodes + 255) / 256), 256, 0, st>>>(g.g, n_nodes, g4);
   ++*launches;
   g.g4 = g4;
   return SYNAX_OK;
 }
-static void unpack_grid(const GridDesc& g, cudaStream_t st) {
-  if (g.g4) cudaFreeAsync((void*)g.g4, st);
+static void unpack_grid(const GridDesc& g, bool pooled, cudaStream_t st) {
+  ws_release((void*)g.g4, pooled, st);
 }
 
 static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const GridFwdArgs& a, const FreqTab& ft0) {
@@ -53,7 +53,7 @@ static void launch_grid_forward(int nf, unsigned blocks, cudaStream_t st, const 
 
 synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_model* m, const float* grid,
                                  int precision, double escalate_rad, int sms, int* d_flag_count, int* h_flag_count,
-                                 cudaStream_t st, int64_t* launches) {
+                                 Workspace* ws, cudaStream_t st, int64_t* launches) {
   GridFwdArgs ga;
   ga.f = a0; ga.grid = make_grid_desc(m, grid); ga.mode = precision;
   float k_max = 0.f;
@@ -61,7 +61,8 @@ synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_
   ga.f.flag_list = nullptr; ga.f.flag_count = d_flag_count;
   ga.f.flag_S = (float)(escalate_rad / (double)k_max);
   cudaMemsetAsync(d_flag_count, 0, kCtrlWords * sizeof(int), st);
-  const synax_status ps = pack_grid(ga.grid, st, launches);
+  bool g4_pooled = false;
+  const synax_status ps = pack_grid(ga.grid, ws, &g4_pooled, st, launches);
   if (ps != SYNAX_OK) return ps;
   // one warp per sightline; the hardware block scheduler balances the CTAs (a persistent grid of 16 CTAs/SM ran 2.3
   // waves of the 7 CTAs/SM that fit, with a thin last wave)
@@ -73,7 +74,7 @@ synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_
     f0 += nf;
   }
   const cudaError_t e = cudaGetLastError();
-  unpack_grid(ga.grid, st);
+  unpack_grid(ga.grid, g4_pooled, st);
   cudaMemcpyAsync(h_flag_count, d_flag_count, kCtrlWords * sizeof(int), cudaMemcpyDeviceToHost, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
@@ -81,7 +82,7 @@ synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_
 synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const BatchConstsD* bd,
                              const synax_model* m, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0,
                              const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
-                             int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches) {
+                             int precision, double escalate_rad, int sms, Workspace* ws, cudaStream_t st, int64_t* launches) {
   GridVjpArgs a;
   a.geo = geo; a.bc = bc; a.bd = bd; a.grid = make_grid_desc(m, grid); a.sg_ne = sg_ne; a.sg_n0 = sg_n0;
   a.n_freq_total = ft.n_freq; a.dI = dI; a.dQ = dQ; a.dU = dU;
@@ -100,15 +101,18 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   const size_t smem = (size_t)(kBlock / 32) * 3 * 32 * ((1u << cl) + 1) * sizeof(float);
   if (smem > 200 * 1024) return SYNAX_ERR_UNSUPPORTED;  // n_los too large for the shared-memory hand-over
   // (+ one 8-byte ticket counter per frequency block behind the accumulation buffer, cleared with it)
-  if (cudaMallocAsync((void**)&a.grad4, sizeof(float4) * (size_t)n_nodes + 8 * kMaxFreq, st) != cudaSuccess) return SYNAX_ERR_ALLOC;
+  const size_t acc_bytes = sizeof(float4) * (size_t)n_nodes + 8 * kMaxFreq;
+  bool acc_pooled = false, g4_pooled = false;
+  a.grad4 = static_cast<float*>(ws_alloc(ws, acc_bytes, st, &acc_pooled));
+  if (!a.grad4) return SYNAX_ERR_ALLOC;
   unsigned long long* tickets = reinterpret_cast<unsigned long long*>(a.grad4 + (size_t)n_nodes * 4);
-  if (cudaMemsetAsync(a.grad4, 0, sizeof(float4) * (size_t)n_nodes + 8 * kMaxFreq, st) != cudaSuccess) {
-    cudaFreeAsync(a.grad4, st);
+  if (cudaMemsetAsync(a.grad4, 0, acc_bytes, st) != cudaSuccess) {
+    ws_release(a.grad4, acc_pooled, st);
     return SYNAX_ERR_CUDA;
   }
-  const synax_status ps = pack_grid(a.grid, st, launches);
+  const synax_status ps = pack_grid(a.grid, ws, &g4_pooled, st, launches);
   if (ps != SYNAX_OK) {
-    cudaFreeAsync(a.grad4, st);
+    ws_release(a.grad4, acc_pooled, st);
     return ps;
   }
   const int64_t max_blocks = (geo.npix * 32 + kBlock - 1) / kBlock;
@@ -148,8 +152,8 @@ synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts*
   grid_grad_compact_kernel<<<(unsigned)((n_nodes + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(a.grad4), n_nodes, grad);
   ++*launches;
   const cudaError_t e = cudaGetLastError();
-  cudaFreeAsync(a.grad4, st);
-  unpack_grid(a.grid, st);
+  ws_release(a.grad4, acc_pooled, st);
+  unpack_grid(a.grid, g4_pooled, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 

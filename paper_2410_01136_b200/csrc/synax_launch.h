@@ -32,23 +32,45 @@ template <int CODE> void vjp_launch_classify(int G, dim3 grid, cudaStream_t st, 
     else FN<kUniform>(__VA_ARGS__);                                          \
   } while (0)
 
+// ---- plan-owned workspace (synax_api.cu)
+// Per-call scratch (constants, lists, block partials, the gridded path's repacked grid and accumulation buffer ...) is cut
+// from one buffer that stays with the plan, in stack order, instead of coming from the device's stream-ordered memory pool:
+// with CUDA's default release threshold (0) the pool gives everything back at every stream synchronisation, and the first
+// allocation after one waits ~0.23 ms for memory to be mapped again -- more than a whole cfg-1 forward.  The buffer grows
+// (cudaFree + cudaMalloc: synchronises the device, like the plan's other buffers) at the start of a call when an earlier
+// call needed more, up to kWorkspaceMax; what does not fit, and everything inside a stream capture (a captured graph must
+// not hold pointers into a buffer that may be reallocated later), comes from the pool as before.  A plan is not used by two
+// calls at a time (synax.h), and calls that follow each other are ordered by their streams, so a later call may reuse the
+// bytes of an earlier one.
+struct Workspace {
+  char* base; size_t cap;     // zero-initialised with the plan
+  size_t used;                // stack pointer of the call in progress (virtual: counts what went to the pool too)
+  size_t want;                // high-water mark
+  int depth;                  // nesting of WorkspaceScope
+};
+constexpr size_t kWorkspaceMax = (size_t)256 << 20;
+void* ws_alloc(Workspace* ws, size_t bytes, cudaStream_t st, bool* pooled);   // nullptr when nothing is to be had
+inline void ws_release(void* p, bool pooled, cudaStream_t st) { if (p && pooled) cudaFreeAsync(p, st); }
+void ws_enter(Workspace* ws, cudaStream_t st, size_t* mark);                  // grows the buffer at the outermost level
+inline void ws_leave(Workspace* ws, size_t mark) { if (ws) { ws->used = mark; --ws->depth; } }
+
 // ---- synax_vjp_driver.cu
 synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, const BatchConsts* bc,
                           const BatchConstsD* bd, int batch, int n_params, int G, const ScalarGridDesc& sg_ne,
                           const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, const double* phi, const int* phi_ok,
                           const double* phi_base, const unsigned char* phi_has, int* ctrl,
                           cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
-                          const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
+                          const float* dI, const float* dQ, const float* dU, float* grad, Workspace* ws, cudaStream_t st,
                           int64_t* launches);
 
 // ---- synax_grid.cu
 synax_status grid_forward(const FreqTab& ft, const ForwardArgs& a0, const synax_model* m, const float* grid,
                           int precision, double escalate_rad, int sms, int* d_flag_count, int* h_flag_count,
-                          cudaStream_t st, int64_t* launches);
+                          Workspace* ws, cudaStream_t st, int64_t* launches);
 synax_status grid_vjp(const FreqTab& ft, const Geometry& geo, const BatchConsts* bc, const BatchConstsD* bd,
                       const synax_model* m, const ScalarGridDesc& sg_ne, const ScalarGridDesc& sg_n0,
                       const float* grid, const float* dI, const float* dQ, const float* dU, float* grad,
-                      int precision, double escalate_rad, int sms, cudaStream_t st, int64_t* launches);
+                      int precision, double escalate_rad, int sms, Workspace* ws, cudaStream_t st, int64_t* launches);
 
 // ---- synax_dd.cu: the all-float64 path (synax_forward_f64 / synax_vjp_f64)
 size_t dd_consts_bytes(int batch);

@@ -56,7 +56,7 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
                                  const ScalarGridDesc& sg_n0, int precision, double escalate_rad, int batch_share, const double* phi, const int* phi_ok,
                           const double* phi_base, const unsigned char* phi_has, int* ctrl,
                                  cudaStream_t aux, cudaEvent_t ev_fork, cudaEvent_t ev_join,
-                                 const float* dI, const float* dQ, const float* dU, float* grad, cudaStream_t st,
+                                 const float* dI, const float* dQ, const float* dU, float* grad, Workspace* ws, cudaStream_t st,
                                  int64_t* launches) {
   VjpArgs a;
   a.geo = geo; a.bc = bc; a.bd = bd; a.batch = batch; a.n_freq_total = ft.n_freq;
@@ -88,7 +88,8 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
     a.mode = ctrl + kCtrlMode;
   }
   unsigned char* cta_sel = nullptr;
-  if (split && cudaMallocAsync((void**)&cta_sel, (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess)
+  bool sel_pooled = false, partial_pooled = false;
+  if (split && !(cta_sel = static_cast<unsigned char*>(ws_alloc(ws, (size_t)a.n_blocks * (size_t)batch, st, &sel_pooled))))
     return SYNAX_ERR_ALLOC;
   // measured at cfg 2 (256 vectors, B200): sharing pays in the forward (5.09 -> 4.68 ms at 4 vectors per thread) but not here
   // -- two or four sets of 27 gradient accumulators per thread cost more occupancy than the shared geometry saves (8.46 ->
@@ -102,9 +103,9 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   int nb = 0;
   if (fo_ok && batch_share > 1 && !phi_base) nb = batch_share;
   else if (fo_ok && !phi) nb = kStandAloneVectors;
-  float* partial = nullptr;
-  if (cudaMallocAsync((void**)&partial, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st) != cudaSuccess) {
-    if (cta_sel) cudaFreeAsync(cta_sel, st);
+  float* partial = static_cast<float*>(ws_alloc(ws, sizeof(float) * 16 * (size_t)a.n_blocks * (size_t)batch, st, &partial_pooled));
+  if (!partial) {
+    ws_release(cta_sel, sel_pooled, st);
     return SYNAX_ERR_ALLOC;
   }
   a.partial = partial;
@@ -164,8 +165,8 @@ synax_status analytic_vjp(int code, const FreqTab& ft, const Geometry& geo, cons
   }
   cudaError_t e = cudaGetLastError();
   if (stream_err != cudaSuccess) e = stream_err;
-  cudaFreeAsync(partial, st);
-  if (cta_sel) cudaFreeAsync(cta_sel, st);
+  ws_release(partial, partial_pooled, st);
+  ws_release(cta_sel, sel_pooled, st);
   return e == cudaSuccess ? SYNAX_OK : SYNAX_ERR_CUDA;
 }
 

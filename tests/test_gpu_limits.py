@@ -187,3 +187,41 @@ def test_pool_release_threshold_keyword():
     with pytest.raises(sx.SynaxError):
         plan.set_option("pool_release_threshold_mb", -1.0)
     plan.close()
+
+
+def test_workspace_growth_and_reuse_across_call_sizes():
+    """The plan's scratch workspace (include/synax.h "Scratch"): calls of growing and shrinking batch on ONE plan -- the call
+    that outgrows the buffer takes the excess from the pool, the next one reallocates -- give what fresh plans give, with and
+    without a synchronisation between the calls; gridded model too (repacked grid + accumulation buffer in the workspace)."""
+    import torch
+    import paper_2410_01136_b200 as sx
+    base = wl.config(2).scaled(nside=8, n_los=128, batch=8)
+    plan = sx.Plan(base.nside, base.n_los, base.s_max, base.freqs)
+    model = sx.Model("full16")
+    for sync in (True, False):
+        for nb in (1, 8, 3, 8, 1):
+            p = torch.from_numpy(base.params[:nb].copy()).cuda()
+            cots = [torch.from_numpy(np.ascontiguousarray(c[:nb])).cuda() for c in base.cotangents()]
+            fresh = sx.Plan(base.nside, base.n_los, base.s_max, base.freqs)
+            ref = [t.clone() for t in sx.forward(fresh, model, p)]
+            gref = sx.vjp(fresh, model, p, *cots).clone()
+            fresh.close()
+            out = sx.forward(plan, model, p)
+            g = sx.vjp(plan, model, p, *cots)
+            if sync:
+                torch.cuda.synchronize()
+            assert all(torch.equal(a, b) for a, b in zip(out, ref)), (sync, nb)
+            assert bool(((g - gref).abs() <= 1e-5 * gref.abs().max()).all()), (sync, nb)
+    plan.close()
+    w = wl.config(3).scaled(nside=4, n_los=64)
+    plan, model, params = parity.gpu_objects(w)
+    cots = [torch.from_numpy(c).cuda() for c in w.cotangents()]
+    ref = [t.clone() for t in sx.forward(plan, model, params)]
+    gref = sx.vjp(plan, model, params, *cots).clone()
+    for _ in range(3):
+        out = sx.forward(plan, model, params)
+        g = sx.vjp(plan, model, params, *cots)
+        torch.cuda.synchronize()
+        assert all(torch.equal(a, b) for a, b in zip(out, ref))
+        assert bool(((g - gref).abs() <= 1e-5 * gref.abs().max()).all())
+    plan.close()
