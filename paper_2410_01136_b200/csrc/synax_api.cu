@@ -485,7 +485,7 @@ static synax_status run_prologue(const synax_plan* plan, const synax_model* mode
     plan->launches++;
   }
   prologue_kernel<<<(batch + 127) / 128, 128, 0, st>>>(code, code == kGridB ? nullptr : params, model->n_params, batch,
-                                                      make_aux(model), plan->ft, plan->delta, ne_max, *bc, *bd);
+                                                      make_aux(model), plan->ft, plan->delta, plan->n_los, ne_max, *bc, *bd);
   plan->launches++;
   CUDA_TRY(cudaGetLastError());
   return SYNAX_OK;

@@ -136,7 +136,7 @@ struct BatchConstsD {
   double k_hb;            // -log2(e)/h_b, 0 for DISC4
   double Bh, zh0, inv_rh, inv_wh;
   double ne0x4, k_her, k_hez;   // 4 ne0, -log2(e)/h_er, -2 log2(e)/|h_ez|
-  int psi1_small;         // |psi1| <= 0.05 and |psi1| x (bound on one sample's rotation) <= 0.15 rad: the MUFU lg2 is accurate enough for ln(rho/8)
+  int psi1_small;         // |psi1| <= 0.05 and |psi1| x (bound on one sample's rotation) x sqrt(n_los) <= 10 rad: the MUFU lg2 is accurate enough for ln(rho/8)
   int angles_small;       // |psi0| + |psi1| <= pi/4 and |chi0| <= pi/4: psi (|ln(rho/8)| < 1 inside the annulus) and
                           // chi = chi0 tanh z never leave [-pi/4, pi/4], so sincos needs no range reduction
   int hez_is_one;         // h_ez == 1 kpc exactly: exp(-2|z|/h_ez) is the tanh(z / 1 kpc) exponential, evaluated once

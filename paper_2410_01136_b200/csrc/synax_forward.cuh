@@ -148,12 +148,16 @@ enum { kCtrlFlagCount = 0, kCtrlPilotFlagged = 1, kCtrlMode = 2, kCtrlCountU = 3
 // Estimate of one lane's share of the round-off scale  sum_n |n_e| (|B_LOS| + |B_N| + |B_E|)  over samples [n0, n1):
 // every 16th sample (all of them for short chunks), MUFU-grade fp32 chain; the caller sums the lanes of the
 // sightline and multiplies by Triad::scalef.
-template <int CODE>
+// kTileMax: also *tile_max = estimate of the largest |signed Faraday sum inside one 32-sample tile| (forward_kernel's second
+// criterion, ForwardArgs::flag_T), from the same samples (its own instantiation: the bookkeeping costs the plain one 10 %).
+template <int CODE, bool kTileMax = false>
 __device__ __forceinline__ float roundoff_scale_estimate(const Geometry& geo, const BatchConsts& P, const Triad& T,
-                                                         const ScalarGridDesc& sg_ne, int n0, int n1) {
+                                                         const ScalarGridDesc& sg_ne, int n0, int n1, float* tile_max = nullptr) {
   const int step = (n1 - n0 >= 32) ? 16 : 1;
   const double delta = geo.delta * T.scale;
   float est = 0.f;
+  float tsum = 0.f, tmax = 0.f;
+  int tcur = -1;
   for (int n = n0 + step / 2; n < n1; n += step) {
     const double s_e = ((double)n + 0.5) * delta;
     const double xd = fma(s_e, T.nxd, geo.obs[0]), yd = fma(s_e, T.nyd, geo.obs[1]), zd = fma(s_e, T.nzd, geo.obs[2]);
@@ -173,7 +177,13 @@ __device__ __forceinline__ float roundoff_scale_estimate(const Geometry& geo, co
       if ((CODE == kAnalyticDisc || CODE == kStack16) && sg_ne.g) S.ne = scalar_grid_at<float>(sg_ne, xd, yd, zd);
     }
     est = fmaf(fabsf(S.ne), fabsf(S.Bpar) + fabsf(S.BN) + fabsf(S.BE), est);
+    if (kTileMax) {
+      const int t = (n - n0) >> 5;
+      if (t != tcur) { tmax = fmaxf(tmax, fabsf(tsum)); tsum = 0.f; tcur = t; }
+      tsum = fmaf(S.ne, CODE == kUniform ? fmaf(P.uB[0], T.nx, fmaf(P.uB[1], T.ny, P.uB[2] * T.nz)) : S.Bpar, tsum);
+    }
   }
+  if (kTileMax) *tile_max = fmaxf(tmax, fabsf(tsum)) * (float)step;
   return est * (float)step;
 }
 
@@ -664,8 +674,15 @@ __global__ void __launch_bounds__(kBlock) classify_kernel(const __grid_constant_
     const BatchConsts& P = A.bc[b];
     const Triad T = load_triad(A.geo, pix);
     // (3 % under the threshold: a sightline the estimate misses by a little is redone after the join, alone on the GPU --
-    // cfg 4: that redo 0.18 -> 0.11 ms for 10,003 more sightlines on the float64 chain's list, forward 9.17 -> 9.09 ms)
-    flagged = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, 0, A.geo.n_los) * T.scalef > 0.97f * A.flag_S;
+    // cfg 4: that redo 0.18 -> 0.11 ms for 10,003 more sightlines on the float64 chain's list, forward 9.17 -> 9.09 ms.
+    // The kernel's second criterion, the Faraday sum inside one 32-sample tile, is estimated from the same samples: at
+    // nside 128 x 256 samples the redo of what it flagged took 0.15 of 0.89 ms.)
+    // (only where a tile is a sizeable part of the sightline, <= 512 samples: longer ones stay far below it per tile unless
+    // the first criterion flags them anyway, and the bookkeeping costs cfg 4 0.01 ms; a miss is only redone later)
+    float tile_est = 0.f, est;
+    if (A.flag_T > 0.f && A.geo.n_los <= 512) est = roundoff_scale_estimate<CODE, true>(A.geo, P, T, A.sg_ne, 0, A.geo.n_los, &tile_est) * T.scalef;
+    else est = roundoff_scale_estimate<CODE>(A.geo, P, T, A.sg_ne, 0, A.geo.n_los) * T.scalef;
+    flagged = est > 0.97f * A.flag_S || (A.flag_T > 0.f && tile_est * T.scalef > 0.97f * A.flag_T);
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned mf = __ballot_sync(0xffffffffu, valid && flagged), mu = __ballot_sync(0xffffffffu, valid && !flagged);

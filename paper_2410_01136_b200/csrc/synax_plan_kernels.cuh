@@ -98,7 +98,7 @@ __global__ void phi_validate_kernel(const float* __restrict__ now, const float* 
 
 // ne_max: device scalar max |ne_grid| when a gridded n_e replaces the analytic disc, else null
 __global__ void prologue_kernel(int code, const float* __restrict__ params, int n_params, int batch,
-                                AuxHost aux, FreqTab ft, double delta, const float* __restrict__ ne_max,
+                                AuxHost aux, FreqTab ft, double delta, int n_los, const float* __restrict__ ne_max,
                                 BatchConsts* __restrict__ out, BatchConstsD* __restrict__ outd) {
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= batch) return;
@@ -194,10 +194,11 @@ __global__ void prologue_kernel(int code, const float* __restrict__ params, int 
     d.k_hb = (code == kAnalyticFull) ? -log2e / p[4] : 0.0;
     d.Bh = p[5]; d.zh0 = p[6]; d.inv_rh = 1.0 / p[7]; d.inv_wh = 1.0 / p[8];
     d.ne0x4 = 4.0 * p[13]; d.k_her = -log2e / p[14]; d.k_hez = -2.0 * log2e / fabs(p[15]);
-    // ln(rho/8) from the MUFU lg2 (abs err ~5e-7) turns the disc field by psi1 x that: a relative error of ~|psi1| x 7e-7 in
-    // a sample's Faraday term.  Harmless when the samples turn by a few radians each (tile_d = 16: <= 3 rad) and there are
-    // hundreds of them; a run with ONE sample of 1,800 rad (psi1 0.014) was off by 2e-5 rad, 1.1e-4 x RMS -- so not then.
-    d.psi1_small = (fabs(p[2]) <= 0.05 && fabs(p[2]) * per_step_rad <= 0.15) ? 1 : 0;
+    // ln(rho/8) from the MUFU lg2 (abs err ~5e-7, pseudo-random from sample to sample) turns the disc field by psi1 x that:
+    // a relative error of ~|psi1| x 7e-7 in a sample's Faraday term, ~|psi1| x 7e-7 x (rotation per sample) x sqrt(n_los) in
+    // the sightline's angle.  Kept below ~1e-5 rad: a run with ONE sample of 1,800 rad (psi1 0.014) was off by 2e-5 rad,
+    // 1.1e-4 x RMS; 256 samples of <= 25 rad each (the same model at nside 128 x 256) stay at 4e-6 and keep the fast path.
+    d.psi1_small = (fabs(p[2]) <= 0.05 && fabs(p[2]) * per_step_rad * sqrt((double)n_los) <= 10.0) ? 1 : 0;
     d.angles_small = (fabs(p[1]) + fabs(p[2]) <= 0.78 && fabs(p[3]) <= 0.78) ? 1 : 0;   // 0.78 < pi/4
     d.hez_is_one = (p[15] == 1.0 || p[15] == -1.0) ? 1 : 0;
     for (int k = 0; k < 4; ++k) {
